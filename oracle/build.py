@@ -1,0 +1,23 @@
+"""Build the CPU oracle (plain C, gcc) into oracle/libea3d_oracle.so.  TEST INFRASTRUCTURE ONLY."""
+from __future__ import annotations
+
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "ea3d_oracle.c")
+LIB = os.path.join(HERE, "libea3d_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+        return LIB
+    # -ffp-contract=off: the threshold table must be plain double arithmetic (R5).
+    cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", "-Wall", "-Wextra",
+           "-o", LIB, SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True))

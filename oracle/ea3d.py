@@ -1,0 +1,223 @@
+"""ctypes front end of the CPU oracle (oracle/ea3d_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It imports nothing from the CUDA path; the conversions between the canonical
+bit-packed format (include/ising.h) and the oracle's int8 arrays below are the oracle's own.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+PHILOX, MINSTD = 0, 1
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        u32p, u64p, i8p, i64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_int8),
+                                 C.POINTER(C.c_int64))
+        L.oracle_philox4x32_10.argtypes = [u32p, u32p, u32p]
+        L.oracle_philox4x32_10.restype = None
+        L.oracle_splitmix64_output.argtypes = [C.c_uint64, C.c_uint64]
+        L.oracle_splitmix64_output.restype = C.c_uint64
+        L.oracle_minstd_step.argtypes = [C.c_uint32]
+        L.oracle_minstd_step.restype = C.c_uint32
+        L.oracle_minstd_seed_state.argtypes = [C.c_uint64, C.c_uint64]
+        L.oracle_minstd_seed_state.restype = C.c_uint32
+        L.oracle_minstd_draw.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64]
+        L.oracle_minstd_draw.restype = C.c_uint32
+        L.oracle_philox_draw.argtypes = [C.c_int, C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint64]
+        L.oracle_philox_draw.restype = C.c_uint32
+        L.oracle_thresholds.argtypes = [C.c_double, C.c_int, u64p]
+        L.oracle_thresholds.restype = C.c_int
+        L.oracle_energy.argtypes = [C.c_int, C.c_int, i8p, i8p, i8p, i8p, i64p, i64p]
+        L.oracle_energy.restype = None
+        L.oracle_minstd_init.argtypes = [C.c_int, C.c_int, C.c_uint64, u32p]
+        L.oracle_minstd_init.restype = None
+        L.oracle_half_sweep.argtypes = [C.c_int, C.c_int, i8p, i8p, i8p, i8p, C.c_uint64, C.c_int, C.c_uint64,
+                                        u64p, u32p, i64p, i64p]
+        L.oracle_half_sweep.restype = C.c_int
+        L.oracle_site_flips.argtypes = [C.c_int, i8p, i8p, i8p, i8p, C.c_int, C.c_uint64, C.c_int, C.c_uint64,
+                                        u64p, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), u64p]
+        L.oracle_site_flips.restype = C.c_int
+        L.oracle_fnv1a64.argtypes = [C.c_void_p, C.c_uint64]
+        L.oracle_fnv1a64.restype = C.c_uint64
+        L.oracle_set_threads.argtypes = [C.c_int]
+        L.oracle_get_max_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+# ---- thin scalar wrappers ------------------------------------------------------------------
+
+def philox4x32_10(ctr, key):
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    o = np.zeros(4, dtype=np.uint32)
+    lib().oracle_philox4x32_10(_p(c, C.c_uint32), _p(k, C.c_uint32), _p(o, C.c_uint32))
+    return tuple(int(v) for v in o)
+
+
+def splitmix64_output(seed, n):
+    return int(lib().oracle_splitmix64_output(seed & (2**64 - 1), n))
+
+
+def minstd_step(r):
+    return int(lib().oracle_minstd_step(r))
+
+
+def minstd_seed_state(seed, q):
+    return int(lib().oracle_minstd_seed_state(seed, q))
+
+
+def minstd_draw(seed, q, n):
+    return int(lib().oracle_minstd_draw(seed, q, n))
+
+
+def philox_draw(L, seed, sample, x, y, z, t):
+    return int(lib().oracle_philox_draw(L, seed, sample, x, y, z, t))
+
+
+def thresholds(beta, rng_mode):
+    T = np.zeros(3, dtype=np.uint64)
+    rc = lib().oracle_thresholds(float(beta), int(rng_mode), _p(T, C.c_uint64))
+    if rc != 0:
+        raise ValueError("bad beta or rng_mode")
+    return tuple(int(v) for v in T)
+
+
+def fnv1a64(buf) -> int:
+    a = np.ascontiguousarray(buf)
+    return int(lib().oracle_fnv1a64(a.ctypes.data, a.nbytes))
+
+
+def set_threads(n: int):
+    lib().oracle_set_threads(int(n))
+
+
+def max_threads() -> int:
+    return int(lib().oracle_get_max_threads())
+
+
+# ---- canonical packed format <-> int8 arrays (the oracle's own conversions) ------------------
+
+def unpack_bits(words: np.ndarray, n: int) -> np.ndarray:
+    """uint32 words (little-endian bit order: bit i&31 of word i>>5) -> uint8 array of n bits."""
+    w = np.ascontiguousarray(words, dtype="<u4")
+    return np.unpackbits(w.view(np.uint8), bitorder="little")[:n]
+
+
+def pack_bits(bits: np.ndarray) -> np.ndarray:
+    n = bits.size
+    nw = (n + 31) // 32
+    b = np.zeros(nw * 32, dtype=np.uint8)
+    b[:n] = bits
+    return np.packbits(b, bitorder="little").view("<u4").astype(np.uint32)
+
+
+def spins_from_packed(words: np.ndarray, n: int) -> np.ndarray:
+    """PAPER.md:246-249 Eq. 10: bit 1 <=> sigma = +1, bit 0 <=> sigma = -1."""
+    bits = unpack_bits(words, n)
+    out = bits.astype(np.int8)
+    out *= 2
+    out -= 1
+    return out
+
+
+def couplings_from_packed(words: np.ndarray, n: int) -> np.ndarray:
+    """PAPER.md:246-249 Eq. 10: bit 1 <=> J = -1, bit 0 <=> J = +1."""
+    bits = unpack_bits(words, n)
+    out = bits.astype(np.int8)
+    out *= -2
+    out += 1
+    return out
+
+
+def spins_to_packed(sigma: np.ndarray) -> np.ndarray:
+    return pack_bits((sigma > 0).astype(np.uint8))
+
+
+class Oracle:
+    """The reference chain: state in int8 arrays, half-sweep counter t, red (even t) then blue."""
+
+    def __init__(self, L: int, nsamples: int, seed: int, rng_mode: int):
+        if L < 2 or L % 2:
+            raise ValueError("L must be even and >= 2")
+        self.L, self.nsamples, self.seed, self.rng_mode = L, nsamples, int(seed), int(rng_mode)
+        self.N = L ** 3
+        self.t = 0
+        self.sigma = np.ones((nsamples, self.N), dtype=np.int8)
+        self.Jx = np.ones((nsamples, self.N), dtype=np.int8)
+        self.Jy = np.ones((nsamples, self.N), dtype=np.int8)
+        self.Jz = np.ones((nsamples, self.N), dtype=np.int8)
+        self.dE_sum = np.zeros(nsamples, dtype=np.int64)
+        self.stats = np.zeros(11, dtype=np.int64)
+        self.minstd_state = None
+        if rng_mode == MINSTD:
+            self.minstd_state = np.zeros(nsamples * self.N, dtype=np.uint32)
+            lib().oracle_minstd_init(L, nsamples, self.seed, _p(self.minstd_state, C.c_uint32))
+
+    # -- state I/O in the canonical packed format
+    def load_packed(self, spins_words: np.ndarray, J_words: np.ndarray):
+        sw = np.asarray(spins_words).reshape(self.nsamples, -1)
+        jw = np.asarray(J_words).reshape(self.nsamples, 3, -1)
+        for s in range(self.nsamples):
+            self.sigma[s] = spins_from_packed(sw[s], self.N)
+            self.Jx[s] = couplings_from_packed(jw[s, 0], self.N)
+            self.Jy[s] = couplings_from_packed(jw[s, 1], self.N)
+            self.Jz[s] = couplings_from_packed(jw[s, 2], self.N)
+
+    def load_arrays(self, sigma, Jx, Jy, Jz):
+        self.sigma[...] = np.asarray(sigma, dtype=np.int8).reshape(self.nsamples, self.N)
+        self.Jx[...] = np.asarray(Jx, dtype=np.int8).reshape(self.nsamples, self.N)
+        self.Jy[...] = np.asarray(Jy, dtype=np.int8).reshape(self.nsamples, self.N)
+        self.Jz[...] = np.asarray(Jz, dtype=np.int8).reshape(self.nsamples, self.N)
+
+    def spins_packed(self) -> np.ndarray:
+        return np.stack([spins_to_packed(self.sigma[s]) for s in range(self.nsamples)])
+
+    # -- dynamics
+    def half_sweep(self, beta: float):
+        T = np.array(thresholds(beta, self.rng_mode), dtype=np.uint64)
+        ms = _p(self.minstd_state, C.c_uint32) if self.minstd_state is not None else None
+        rc = lib().oracle_half_sweep(self.L, self.nsamples, _p(self.sigma, C.c_int8), _p(self.Jx, C.c_int8),
+                                     _p(self.Jy, C.c_int8), _p(self.Jz, C.c_int8), self.seed, self.rng_mode,
+                                     self.t, _p(T, C.c_uint64), ms, _p(self.dE_sum, C.c_int64),
+                                     _p(self.stats, C.c_int64))
+        if rc != 0:
+            raise RuntimeError("oracle_half_sweep failed")
+        self.t += 1
+
+    def sweep(self, beta: float, nsweeps: int = 1):
+        for _ in range(2 * nsweeps):
+            self.half_sweep(beta)
+
+    def energy(self):
+        E = np.zeros(self.nsamples, dtype=np.int64)
+        M = np.zeros(self.nsamples, dtype=np.int64)
+        lib().oracle_energy(self.L, self.nsamples, _p(self.sigma, C.c_int8), _p(self.Jx, C.c_int8),
+                            _p(self.Jy, C.c_int8), _p(self.Jz, C.c_int8), _p(E, C.c_int64), _p(M, C.c_int64))
+        return E, M
+
+    def site_flips(self, beta: float, sample: int, x: int, y: int, z: int, t: int | None = None):
+        """(flips, dE, R) for one site of the active colour of half-sweep t, from the CURRENT state."""
+        T = np.array(thresholds(beta, self.rng_mode), dtype=np.uint64)
+        dE = C.c_int(0)
+        R = C.c_uint64(0)
+        tt = self.t if t is None else t
+        rc = lib().oracle_site_flips(self.L, _p(self.sigma[sample], C.c_int8), _p(self.Jx[sample], C.c_int8),
+                                     _p(self.Jy[sample], C.c_int8), _p(self.Jz[sample], C.c_int8), sample,
+                                     self.seed, self.rng_mode, tt, _p(T, C.c_uint64), x, y, z, C.byref(dE),
+                                     C.byref(R))
+        return rc, dE.value, R.value
