@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark: ps per spin-flip attempt of the bit-packed checkerboard Metropolis sweep at L=1024.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--L 1024] [--sweeps 20]
+
+One "step" is one pass of the whole hot path over one synthetic lattice of BASELINE.json
+config 5: load the canonical packed state into the internal layout (a10), 20 full sweeps = 40 colour half-sweep launches
+(a1-a8), energy + magnetisation (a9), canonical spins out (a10).  `value` is measured with the inputs resident in HBM;
+`e2e` goes through ising_run_host with pinned HOST buffers (H2D of spins + couplings and D2H of spins, E, M inside the
+timed region).  Philox mode is the headline line; the MINSTD mode of the same config is timed too ("minstd").
+N > 1 runs N independent replicas (the path does not shard: DESIGN.md section 8), one process per GPU, no collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ps_per_spin_flip_attempt"
+UNIT = "ps/flip"
+BETA = 1.0 / 1.1
+
+# Algorithmic work of one flip attempt: integer instructions the definition needs at minimum.
+#   Philox4x32-10 with the launch-constant part folded: 18 wide multiplies + 19 three-input XORs per 4 sites = 9.25
+#   acceptance: one compare + one mask insert per site                                                    = 2
+#   field: 6 bond XORs + 8 adder ops + 4 mask ops + 2 x-alignment ops per 32-site word                    = 0.625
+ALG_INSTR_PER_FLIP = {0: 37 / 4 + 2 + 20 / 32}
+#   MINSTD stateless: SplitMix64 finaliser on a 64-bit Weyl state (2 add, 2x4 xor-shift, 2x3 multiply) + s0 (2) +
+#   mulmod (6) + compare/insert (2) per site                                                              = 26
+ALG_INSTR_PER_FLIP[1] = 26 + 20 / 32
+ALG_BYTES_PER_FLIP = 9 / 8 / 2 * 2  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return float(p.get("hbm_gbs", 6650.0)), float(p.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        sm = sorted(int(r[1]) for r in self.rows if len(r) >= 9 and r[1].isdigit())
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) >= 9:
+                for n, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        smax = max((int(r[2]) for r in self.rows if len(r) >= 9 and r[2].isdigit()), default=None)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def time_oracle(L, sweeps, rng_mode, repeats=1):
+    """The oracle as it stands (OpenMP over the planes of one colour) on this host: seconds per call of `sweeps` sweeps."""
+    from oracle import ea3d
+    from paper_1411_0127_b200 import synth
+
+    o = ea3d.Oracle(L, 1, synth.DYN_SEED, rng_mode)
+    o.load_packed(synth.make_spins(L), synth.make_couplings(L))
+    o.sweep(BETA, 1)  # touch the pages
+    times = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        o.sweep(BETA, sweeps)
+        times.append(time.perf_counter() - t0)
+    return times, ea3d.max_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle is the reference arm of this tier (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    Ls, sweeps = 512, 2
+    times, cores = time_oracle(Ls, sweeps, 0, repeats=args.warmup + args.steps)
+    times = times[args.warmup:]
+    total = sum(times)
+    flips = len(times) * sweeps * Ls**3
+    ps = 1e12 * total / flips
+    sample = f"L={Ls} cube (1/8 of the L=1024 lattice's sites, same J/spin recipe, beta=1/1.1, Philox), {sweeps} sweeps per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": ps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+        "config": {"workload": "BASELINE.json config 5: L=1024 +-J EA cube, 1 sample, beta=1/1.1, Philox", "sample": sample},
+        "flips_per_s": flips / total,
+        "cpu_baseline": {"value": ps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": ps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--L", type=int, default=1024)
+    ap.add_argument("--sweeps", type=int, default=20)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-minstd", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+
+    from paper_1411_0127_b200 import MINSTD, PHILOX, Ising, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t[0])
+
+    L, nsw = args.L, args.sweeps
+    N = L**3
+    # every rank simulates its own disorder sample (replicas): seeds offset by rank
+    spins = synth.make_spins(L, 1, 2 + 1000 * rank)
+    J = synth.make_couplings(L, 1, 1 + 1000 * rank)
+    h_spins = torch.from_numpy(spins.view(np.int32)).pin_memory()
+    h_J = torch.from_numpy(J.view(np.int32)).pin_memory()
+    h_out = torch.empty_like(h_spins).pin_memory()
+    d_spins, d_J = h_spins.cuda(), h_J.cuda()
+    d_out = torch.empty_like(d_spins)
+    stream = torch.cuda.current_stream()
+
+    def bench_mode(rng_mode):
+        g = Ising(L, 1, synth.DYN_SEED, rng_mode)
+
+        def step(ev=None):
+            g.ising_load_state(d_spins, d_J)
+            if ev:
+                ev[0].record(stream)
+            g.ising_sweep(BETA, nsw)
+            if ev:
+                ev[1].record(stream)
+            E, M = g.ising_energy()
+            g.ising_get_spins(d_out)
+            return E, M
+
+        for _ in range(args.warmup):
+            step()
+        barrier()
+        l0 = g.ising_kernel_launches()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for k in range(args.steps):
+            E, M = step(evs[k])
+        e1.record(stream)
+        barrier()
+        total_ms = max_over_ranks(e0.elapsed_time(e1))
+        sweep_ms = max_over_ranks(sum(a.elapsed_time(b) for a, b in evs))
+        launches = g.ising_kernel_launches() - l0
+        res = {"total_ms": total_ms, "sweep_ms": sweep_ms, "launches": launches, "E": int(E[0]), "M": int(M[0])}
+        # end to end through host buffers
+        if not args.no_e2e:
+            for _ in range(2):
+                g.ising_run_host(h_spins, h_J, BETA, nsw, h_out)
+            barrier()
+            t0 = time.perf_counter()
+            e0.record(stream)
+            for _ in range(args.steps):
+                Eh, Mh = g.ising_run_host(h_spins, h_J, BETA, nsw, h_out)
+            e1.record(stream)
+            barrier()
+            res["e2e_ms"] = max_over_ranks(e0.elapsed_time(e1))
+            res["e2e_wall_ms"] = 1e3 * (time.perf_counter() - t0)
+            assert int(Eh[0]) == res["E"], "e2e path and device path disagree"
+        g.ising_destroy()
+        return res
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    philox = bench_mode(PHILOX)
+    clocks = sampler.stop() if rank == 0 else None
+    minstd = None if args.no_minstd else bench_mode(MINSTD)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    hbm_gbs, sm_max_mhz, peaks_src = measured_peaks()
+    flips_per_step = world * nsw * N
+    K = args.steps
+
+    def summarize(res, rng_mode):
+        ps = 1e9 * res["total_ms"] / (K * flips_per_step)
+        half_sweep_ms = res["sweep_ms"] / (K * 2 * nsw)            # average launch duration of the dominant kernel
+        flips_per_launch = N / 2
+        inst_rate = ALG_INSTR_PER_FLIP[rng_mode] * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12  # T thread-instr/s
+        peak = 148 * 4 * 32 * sm_max_mhz * 1e6 / 1e12               # 148 SMs x 4 schedulers x 32 lanes x max clock
+        hbm = ALG_BYTES_PER_FLIP * flips_per_launch / (half_sweep_ms * 1e-3) / 1e9
+        return ps, {
+            "bound": "alu", "achieved": inst_rate, "peak": peak, "unit": "Tinst/s", "frac": inst_rate / peak, "traffic": None,
+            "kernel": "half_sweep_site_packed", "kernel_ms": half_sweep_ms, "kernel_ps_per_flip": 1e9 * half_sweep_ms / flips_per_launch,
+            "alg_instr_per_flip": ALG_INSTR_PER_FLIP[rng_mode], "peak_source": f"148 SM x 4 x 32 lanes x {sm_max_mhz:.0f} MHz ({peaks_src} max clock)",
+            "hbm": {"achieved": hbm, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm / hbm_gbs, "alg_bytes_per_flip": ALG_BYTES_PER_FLIP,
+                    "peak_source": peaks_src},
+        }
+
+    ps, roof = summarize(philox, 0)
+    line = {
+        "metric": METRIC, "value": ps, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": philox["total_ms"] / K, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json config 5: L={L} periodic +-J EA cube, 1 sample, random spins, beta=1/1.1, {nsw} sweeps, Philox4x32-10",
+                   "L": L, "sweeps_per_step": nsw, "rng": "philox4x32-10", "step": "load_state + sweeps + energy + get_spins",
+                   "l2": "inputs larger than L2 (512 MiB packed state > 126 MB), no flush needed",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "flips_per_s": 1e12 / ps, "roofline": roof, "gpu_launches": philox["launches"], "clocks": clocks,
+        "final_energy": philox["E"],
+    }
+    spin_bytes, j_bytes = spins.nbytes, J.nbytes
+    if "e2e_ms" in philox:
+        line["e2e"] = {"value": 1e9 * philox["e2e_ms"] / (K * flips_per_step), "unit": UNIT,
+                       "h2d_bytes_per_step": spin_bytes + j_bytes, "d2h_bytes_per_step": spin_bytes + 16,
+                       "ms_per_step": philox["e2e_ms"] / K, "api": "ising_run_host"}
+    if minstd is not None:
+        ps_m, roof_m = summarize(minstd, 1)
+        line["minstd"] = {"value": ps_m, "unit": UNIT, "ms_per_step": minstd["total_ms"] / K, "roofline": roof_m,
+                          "flips_per_s": 1e12 / ps_m}
+        if "e2e_ms" in minstd:
+            line["minstd"]["e2e"] = 1e9 * minstd["e2e_ms"] / (K * flips_per_step)
+    if world == 1 and not args.no_cpu_baseline:
+        Ls, sw = 512, 8
+        times, cores = time_oracle(Ls, sw, 0)
+        line["cpu_baseline"] = {"value": 1e12 * times[0] / (sw * Ls**3), "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"L={Ls} cube (1/8 of the sites of the L=1024 workload, same recipe, Philox), {sw} sweeps, {times[0]:.1f} s"}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,138 @@
+/*
+ * ising.h -- C ABI of libising_b200: the bit-packed checkerboard (red/blue) Metropolis sweep of the
+ * 3D +-J Edwards-Anderson spin glass on one NVIDIA B200 (sm_100a).
+ *
+ * Method: arXiv 1411.0127 (Lulli, Bernaschi, Parisi).  Citations are PAPER.md:<line> of the paper text
+ * plus the section / equation; "R<n>" are the readings listed in DESIGN.md section 2.
+ *
+ *   H = - sum_<ik> J_ik sigma_i sigma_k   on an L^3 periodic cubic lattice, J = +-1        (Eq. 1-2)
+ *   one sweep = Metropolis update (Eq. 9) of all red sites ((x+y+z) even), then of all blue
+ *   sites; spins and couplings are one bit each (Eq. 10); the energy
+ *   change of a flip is computed word-wise from bond bits (Eq. 11) with a bit-sliced adder (Eq. 12-13)
+ *   and turned into a flip mask (Eq. 14-17).  Every (sample, site, half-sweep) has its
+ *   own 32-bit draw (R9-R12), unlike the paper's one draw per 32-sample word.
+ *
+ * Conventions
+ *   N = L^3, site i = x + L*(y + L*z), colour (x+y+z)&1, red = 0 is updated at even half-sweep index t (R8).
+ *   The half-sweep counter t starts at 0 in ising_create and keeps counting over all sweep calls, so a
+ *   trajectory does not depend on how sweeps are batched into calls.
+ *   Canonical packed format (the only format that crosses this boundary):
+ *     spins      nsamples x W uint32, W = ceil(N/32); bit (i&31) of word (i>>5) is site i; 1 <=> sigma=+1
+ *     couplings  nsamples x 3 x W uint32, [sample][dir x,y,z][word]; the bit of site i in direction d is the
+ *                bond (i, i+d-hat); 1 <=> J=-1                                              (Eq. 10)
+ *     bits above N in the last word are ignored on input and zero on output.
+ *   nsamples = 1 uses a site-packed internal layout (bits of a word = 32 sites of one lattice, "SMSC",
+ *   PAPER.md:227); nsamples = 32*k uses a sample-packed layout (bits of a word = 32 disorder samples at
+ *   one site, "AMSC" storage, with k coded batches).
+ *
+ * Pointers: every pointer named d_* is DEVICE memory owned by the caller (e.g. a torch CUDA tensor), every
+ *   h_* pointer is HOST memory owned by the caller.  The handle owns host metadata only; the workspace
+ *   passed to ising_create must stay alive, and must not be written by the caller, until ising_destroy.
+ *   `stream` is a cudaStream_t passed as void* (0 = the legacy default stream).  Calls taking a stream are
+ *   asynchronous on it unless stated otherwise.
+ *
+ * Errors: every int-returning call returns ISING_OK (0) or a negative code; nothing throws or aborts.
+ *   There is no CPU fallback: without a CUDA device the device calls return ISING_ECUDA.
+ */
+#ifndef ISING_B200_H
+#define ISING_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ISING_OK 0
+#define ISING_EINVAL (-1) /* bad argument: L odd or < 4 or > 2048, nsamples not 1 or a multiple of 32, unknown
+                             rng_mode, null pointer, workspace too small / misaligned, beta < 0 or NaN, nsweeps < 0 */
+#define ISING_ECUDA (-2)  /* a CUDA runtime call or kernel launch failed (sticky errors surface here too) */
+
+#define ISING_RNG_PHILOX 0 /* Philox4x32-10, key (lo32 seed, hi32 seed ^ sample), counter (t, colour-rank>>2)  (R9, R10) */
+#define ISING_RNG_MINSTD 1 /* MINSTD 16807 mod 2^31-1 (Eq. 7), one stream per site seeded by
+                              SplitMix64 (R11), draw of sweep n = 16807^(n+1) * s0 mod (2^31-1) (R12) */
+
+typedef struct ising ising_t; /* opaque */
+
+/* Size in bytes of the device workspace ising_create needs for (L, nsamples): the internal spin and
+ * coupling arrays (8 bit arrays per lattice), a canonical staging area used by
+ * ising_run_host, and the int64 accumulators of the measurement kernel.  rng_mode does not change the size
+ * (no PRNG state is stored: both generators are evaluated statelessly, R9/R12). */
+int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out);
+
+/* Create a handle.  d_workspace: device memory, >= ising_workspace_bytes, 256-byte aligned.  The lattice
+ * content is undefined until ising_load_state.  seed keys the dynamics' random numbers (R9, R11). */
+int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_workspace, size_t workspace_bytes,
+                 ising_t **out);
+
+/* Load spins and couplings given in the canonical packed format (device pointers) into the internal
+ * layout.  Does not change the half-sweep counter. */
+int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, void *stream);
+
+/* nsweeps full sweeps at inverse temperature beta = 2*nsweeps colour half-sweeps, red first (rows a1-a8):
+ * threshold table T[dE] = floor(2^32 exp(-beta dE)) (Philox, R5) or floor((2^31-1) exp(-beta dE)) (MINSTD,
+ * R6) for dE = 4, 8, 12, then per half-sweep the bond bits / adder / flip mask of Eq. 11-17
+ * with acceptance R < T[dE] (strict, R4) applied per bit.  Advances t by 2*nsweeps. */
+int ising_sweep(ising_t *h, double beta, int nsweeps, void *stream);
+
+/* As ising_sweep, and after every `every_half_sweeps`-th half-sweep of this call (counted from 1) writes the
+ * energy (and magnetisation if d_M != NULL) of every sample to record r = 0,1,...:
+ * d_E[r*nsamples + s].  d_E / d_M must hold (2*nsweeps / every_half_sweeps) * nsamples int64. */
+int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_t *d_M, int every_half_sweeps,
+                      void *stream);
+
+/* E[s] = - sum over the 3N bonds of J sigma sigma (Eq. 1, each bond once; R16) and M[s] = sum_i sigma_i for
+ * every sample (row a9).  d_E: nsamples int64; d_M: nsamples int64 or NULL. */
+int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream);
+
+/* Write the spins in the canonical packed format: nsamples x W uint32 (row a10). */
+int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream);
+
+/* The whole path on HOST buffers, for end-to-end timing: copies h_spins / h_J (canonical packed, ideally
+ * pinned) to the staging area of the workspace, loads them, runs nsweeps sweeps, computes E and M, copies
+ * the canonical spins back to h_spins_out (may be NULL) and E / M to h_E / h_M (nsamples int64 each; h_M
+ * may be NULL), and synchronises the stream before returning. */
+int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps,
+                   uint32_t *h_spins_out, int64_t *h_E, int64_t *h_M, void *stream);
+
+/* Host only.  The acceptance thresholds for dE = 4, 8, 12 exactly as the kernels receive them (R5, R6):
+ * out[k] in [0, 2^32] (Philox) or [0, 2^31-1] (MINSTD). */
+int ising_thresholds(double beta, int rng_mode, uint64_t out[3]);
+
+/* Host only.  64-bit FNV-1a (offset basis 0xcbf29ce484222325, prime 0x100000001b3) of nbytes bytes: the
+ * checksum of BASELINE.json config 4 over the canonical packed spin words (little-endian bytes). */
+uint64_t ising_fnv1a64_host(const void *h_data, size_t nbytes);
+
+/* Half-sweep counter t of the handle (get / set): with ising_get_spins + ising_load_state this makes a run
+ * resumable bit-exactly, because no PRNG state exists outside (seed, t). */
+int ising_get_t(const ising_t *h, uint64_t *t);
+int ising_set_t(ising_t *h, uint64_t t);
+
+/* Select the half-sweep kernel: 0 = automatic (the word-parallel kernel where the layout allows it),
+ * 1 = force the generic one-site-at-a-time kernel (any even L; used by the tests to show that results do
+ * not depend on layout or thread mapping). */
+int ising_set_kernel(ising_t *h, int which);
+
+/* Number of kernels this handle has launched so far. */
+uint64_t ising_kernel_launches(const ising_t *h);
+
+/* Host only, test hook: run the word update of the word-parallel kernels (the same __host__ __device__
+ * code: Philox / MINSTD draws, Eq. 11-13 adder, per-bit acceptance, Eq. 17 mask) on ONE 32-site word given
+ * its 13 operand words.  It exists so that the bit logic can be checked without a GPU; it is not a sweep.
+ *   ops[0] = active spins s; ops[1..6] = neighbour spin words already aligned under s in the order
+ *   +x,-x,+y,-y,+z,-z; ops[7..12] = the matching coupling words (same order).
+ *   word_index: index of the word in its colour array (site-packed: colour rank j = 32*word_index + bit);
+ *   site0 / site_stride: canonical site index of bit 0 and its increment per bit (MINSTD stream ids).
+ * Returns the updated word in *out. */
+int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double beta, const uint32_t ops[13],
+                                uint64_t word_index, uint64_t site0, uint64_t site_stride, uint32_t *out);
+
+int ising_destroy(ising_t *h);
+
+const char *ising_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISING_B200_H */

@@ -1,0 +1,200 @@
+"""ctypes binding of libising_b200.so (include/ising.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch supplies device memory
+(`torch.Tensor.data_ptr()`) and streams (`torch.cuda.current_stream().cuda_stream`), nothing else.
+There is no CPU fallback: loading fails if the library cannot be built or found, and the device calls
+raise `IsingError` on a machine without a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+from . import build as _build
+
+PHILOX, MINSTD = 0, 1
+OK, EINVAL, ECUDA = 0, -1, -2
+
+EXPORTS = (
+    "ising_workspace_bytes", "ising_create", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
+    "ising_get_spins", "ising_run_host", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
+    "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
+)
+
+_lib = None
+
+
+class IsingError(RuntimeError):
+    pass
+
+
+def lib() -> C.CDLL:
+    """Load (building first if stale) the C-ABI library and declare its prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    L = C.CDLL(_build.build())
+    vp, u64, i32, sz, dbl = C.c_void_p, C.c_uint64, C.c_int, C.c_size_t, C.c_double
+    L.ising_workspace_bytes.argtypes = [i32, i32, i32, C.POINTER(sz)]
+    L.ising_create.argtypes = [i32, i32, u64, i32, vp, sz, C.POINTER(vp)]
+    L.ising_load_state.argtypes = [vp, vp, vp, vp]
+    L.ising_sweep.argtypes = [vp, dbl, i32, vp]
+    L.ising_sweep_trace.argtypes = [vp, dbl, i32, vp, vp, i32, vp]
+    L.ising_energy.argtypes = [vp, vp, vp, vp]
+    L.ising_get_spins.argtypes = [vp, vp, vp]
+    L.ising_run_host.argtypes = [vp, vp, vp, dbl, i32, vp, vp, vp, vp]
+    L.ising_thresholds.argtypes = [dbl, i32, C.POINTER(u64)]
+    L.ising_fnv1a64_host.argtypes = [vp, sz]
+    L.ising_fnv1a64_host.restype = u64
+    L.ising_get_t.argtypes = [vp, C.POINTER(u64)]
+    L.ising_set_t.argtypes = [vp, u64]
+    L.ising_set_kernel.argtypes = [vp, i32]
+    L.ising_kernel_launches.argtypes = [vp]
+    L.ising_kernel_launches.restype = u64
+    L.ising_hostcheck_update_word.argtypes = [i32, u64, u64, dbl, C.POINTER(C.c_uint32), u64, u64, u64,
+                                              C.POINTER(C.c_uint32)]
+    L.ising_destroy.argtypes = [vp]
+    L.ising_strerror.argtypes = [i32]
+    L.ising_strerror.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != OK:
+        raise IsingError(f"{what}: {lib().ising_strerror(rc).decode()} ({rc})")
+
+
+def ising_workspace_bytes(L: int, nsamples: int, rng_mode: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().ising_workspace_bytes(L, nsamples, rng_mode, C.byref(out)), "ising_workspace_bytes")
+    return out.value
+
+
+def ising_thresholds(beta: float, rng_mode: int) -> tuple[int, int, int]:
+    out = (C.c_uint64 * 3)()
+    _check(lib().ising_thresholds(float(beta), rng_mode, out), "ising_thresholds")
+    return tuple(int(v) for v in out)
+
+
+def ising_fnv1a64_host(buf) -> int:
+    """FNV-1a 64 of a contiguous numpy array / bytes object (host)."""
+    import numpy as np
+
+    a = np.ascontiguousarray(np.frombuffer(buf, dtype=np.uint8) if isinstance(buf, (bytes, bytearray)) else buf)
+    return int(lib().ising_fnv1a64_host(a.ctypes.data, a.nbytes))
+
+
+def ising_hostcheck_update_word(rng_mode, seed, t, beta, ops, word_index, site0=0, site_stride=2) -> int:
+    arr = (C.c_uint32 * 13)(*[int(v) & 0xFFFFFFFF for v in ops])
+    out = C.c_uint32(0)
+    _check(lib().ising_hostcheck_update_word(rng_mode, seed, t, float(beta), arr, word_index, site0, site_stride,
+                                             C.byref(out)), "ising_hostcheck_update_word")
+    return out.value
+
+
+def _stream_ptr(stream=None) -> int:
+    import torch
+
+    return (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+
+
+def _u32(t):
+    """View a 4-byte-element CUDA/CPU tensor's storage as a raw pointer (uint32 words)."""
+    return t.data_ptr()
+
+
+class Ising:
+    """Handle of one simulation: `ising_create` .. `ising_destroy` with torch tensors as buffers.
+
+    spins / couplings are torch int32 (or uint32) CUDA tensors in the canonical packed format:
+    spins (nsamples, W), couplings (nsamples, 3, W), W = ceil(L^3/32).
+    """
+
+    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device="cuda:0"):
+        import torch
+
+        self.L, self.nsamples, self.seed, self.rng_mode = L, nsamples, seed, rng_mode
+        self.N = L ** 3
+        self.W = (self.N + 31) // 32
+        self.device = torch.device(device)
+        nbytes = ising_workspace_bytes(L, nsamples, rng_mode)
+        # torch's caching allocator returns 512-byte aligned blocks
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        h = C.c_void_p()
+        _check(lib().ising_create(L, nsamples, seed, rng_mode, self.workspace.data_ptr(), nbytes, C.byref(h)),
+               "ising_create")
+        self._h = h
+
+    # -- the C-ABI calls, same names
+    def ising_load_state(self, spins, J, stream=None):
+        assert spins.is_cuda and J.is_cuda and spins.is_contiguous() and J.is_contiguous()
+        assert spins.numel() == self.nsamples * self.W and J.numel() == 3 * self.nsamples * self.W
+        _check(lib().ising_load_state(self._h, _u32(spins), _u32(J), _stream_ptr(stream)), "ising_load_state")
+
+    def ising_sweep(self, beta: float, nsweeps: int, stream=None):
+        _check(lib().ising_sweep(self._h, float(beta), int(nsweeps), _stream_ptr(stream)), "ising_sweep")
+
+    def ising_sweep_trace(self, beta: float, nsweeps: int, every_half_sweeps: int = 1, want_M: bool = True, stream=None):
+        """Returns (E, M) int64 CUDA tensors of shape (records, nsamples)."""
+        import torch
+
+        nrec = (2 * nsweeps) // every_half_sweeps
+        E = torch.empty((nrec, self.nsamples), dtype=torch.int64, device=self.device)
+        M = torch.empty((nrec, self.nsamples), dtype=torch.int64, device=self.device) if want_M else None
+        _check(lib().ising_sweep_trace(self._h, float(beta), int(nsweeps), E.data_ptr(), M.data_ptr() if want_M else None,
+                                       int(every_half_sweeps), _stream_ptr(stream)), "ising_sweep_trace")
+        return E, M
+
+    def ising_energy(self, stream=None):
+        """Returns (E, M) int64 CUDA tensors of shape (nsamples,)."""
+        import torch
+
+        E = torch.empty(self.nsamples, dtype=torch.int64, device=self.device)
+        M = torch.empty(self.nsamples, dtype=torch.int64, device=self.device)
+        _check(lib().ising_energy(self._h, E.data_ptr(), M.data_ptr(), _stream_ptr(stream)), "ising_energy")
+        return E, M
+
+    def ising_get_spins(self, out=None, stream=None):
+        import torch
+
+        if out is None:
+            out = torch.empty((self.nsamples, self.W), dtype=torch.int32, device=self.device)
+        _check(lib().ising_get_spins(self._h, _u32(out), _stream_ptr(stream)), "ising_get_spins")
+        return out
+
+    def ising_run_host(self, h_spins, h_J, beta: float, nsweeps: int, h_spins_out=None, stream=None):
+        """Host tensors in (ideally pinned), host results out; returns (E, M) int64 CPU tensors."""
+        import torch
+
+        assert not h_spins.is_cuda and not h_J.is_cuda
+        E = torch.empty(self.nsamples, dtype=torch.int64).pin_memory()
+        M = torch.empty(self.nsamples, dtype=torch.int64).pin_memory()
+        _check(lib().ising_run_host(self._h, _u32(h_spins), _u32(h_J), float(beta), int(nsweeps),
+                                    _u32(h_spins_out) if h_spins_out is not None else None, E.data_ptr(), M.data_ptr(),
+                                    _stream_ptr(stream)), "ising_run_host")
+        return E, M
+
+    def ising_get_t(self) -> int:
+        t = C.c_uint64(0)
+        _check(lib().ising_get_t(self._h, C.byref(t)), "ising_get_t")
+        return t.value
+
+    def ising_set_t(self, t: int):
+        _check(lib().ising_set_t(self._h, int(t)), "ising_set_t")
+
+    def ising_set_kernel(self, which: int):
+        _check(lib().ising_set_kernel(self._h, int(which)), "ising_set_kernel")
+
+    def ising_kernel_launches(self) -> int:
+        return int(lib().ising_kernel_launches(self._h))
+
+    def ising_destroy(self):
+        if self._h:
+            lib().ising_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.ising_destroy()
+        except Exception:
+            pass

@@ -1,0 +1,462 @@
+// ising_api.cu -- the C ABI of include/ising.h: handle, workspace carving, threshold table (row a1) and launches.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/ising.h"
+#include "layout_kernels.cuh"
+#include "measure_kernels.cuh"
+#include "sweep_kernels.cuh"
+
+using namespace isingk;
+
+namespace {
+
+constexpr size_t ALIGN_WORDS = 64;  // 256-byte alignment of every internal array
+constexpr int MAX_L = 2048;         // keeps the Philox group index g = j>>2 below 2^32 (rng.cuh)
+
+inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Geometry {
+    int L, nsamples, nbatches;  // nbatches = 0: site-packed
+    uint64_t N, Hc;             // sites, sites per colour
+    size_t canon_words;         // W = ceil(N/32)
+    size_t array_words;         // words of one internal bit array (padded)
+    size_t arrays_total_words;  // 8 arrays per lattice / batch
+    size_t staging_words;       // canonical spins + couplings of all samples
+    size_t acc_bytes;
+    bool fast;                  // half-rows are whole words and L = 64*2^k
+};
+
+bool make_geometry(int L, int nsamples, Geometry *g)
+{
+    if (L < 4 || (L & 1) || L > MAX_L) return false;
+    if (!(nsamples == 1 || (nsamples > 0 && nsamples % 32 == 0))) return false;
+    g->L = L;
+    g->nsamples = nsamples;
+    g->nbatches = nsamples == 1 ? 0 : nsamples / 32;
+    g->N = (uint64_t)L * L * L;
+    g->Hc = g->N / 2;
+    g->canon_words = (size_t)((g->N + 31) / 32);
+    const size_t raw = nsamples == 1 ? (size_t)((g->Hc + 31) / 32) : (size_t)g->Hc;
+    g->array_words = round_up(raw, ALIGN_WORDS);
+    g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
+    g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
+    g->acc_bytes = round_up((size_t)nsamples * 4 * sizeof(unsigned long long), 256);  // popcounts + E, M of ising_run_host
+    g->fast = nsamples == 1 && L >= 64 && (L & (L - 1)) == 0;
+    return true;
+}
+
+}  // namespace
+
+struct ising {
+    Geometry g;
+    uint64_t seed;
+    int rng_mode;
+    uint64_t t;
+    int kernel_choice;
+    uint64_t launches;
+    uint32_t *ws;
+    uint32_t *staging;
+    unsigned long long *acc;
+
+    LatticeArrays arrays(int batch) const
+    {
+        LatticeArrays A;
+        uint32_t *base = ws + (size_t)batch * 8 * g.array_words;
+        A.S[0] = base;
+        A.S[1] = base + g.array_words;
+        for (int d = 0; d < 3; ++d)
+            for (int c = 0; c < 2; ++c) A.J[d][c] = base + (size_t)(2 + 2 * d + c) * g.array_words;
+        return A;
+    }
+};
+
+namespace {
+
+int check_launch(ising_t *h, int n = 1)
+{
+    h->launches += (uint64_t)n;
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
+}
+
+// Row a1 (R5, R6).  Plain double arithmetic with the C library's exp; compiled without FMA contraction.
+int compute_thresholds(double beta, int rng_mode, uint64_t out[3])
+{
+    if (!(beta >= 0.0)) return ISING_EINVAL;
+    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD) return ISING_EINVAL;
+    for (int k = 0; k < 3; ++k) {
+        const double dE = 4.0 * (double)(k + 1);
+        const double x = beta * dE;
+        const double p = exp(-x);
+        const double scaled = rng_mode == ISING_RNG_PHILOX ? ldexp(p, 32) : 2147483647.0 * p;
+        out[k] = (uint64_t)floor(scaled);
+    }
+    return ISING_OK;
+}
+
+Thresholds kernel_thresholds(const uint64_t T[3])
+{
+    Thresholds k;
+    uint32_t *t = &k.t4, *al = &k.always4;
+    for (int i = 0; i < 3; ++i) {
+        const bool always = T[i] > 0xFFFFFFFFull;
+        t[i] = always ? 0xFFFFFFFFu : (uint32_t)T[i];
+        al[i] = always ? 0xFFFFFFFFu : 0u;
+    }
+    return k;
+}
+
+void fill_rng_launch(const ising_t *h, int batch, RngLaunch *r)
+{
+    memset(r, 0, sizeof(*r));
+    const uint32_t sample_base = (uint32_t)(batch * 32);
+    r->seed = h->seed;
+    r->tlo = (uint32_t)h->t;
+    r->thi = (uint32_t)(h->t >> 32);
+    r->k0 = (uint32_t)h->seed;
+    r->k1base = (uint32_t)(h->seed >> 32);
+    r->sample_base = sample_base;
+    if (h->rng_mode == ISING_RNG_PHILOX) {
+        const int ns = h->g.nsamples == 1 ? 1 : 32;
+        for (int s = 0; s < ns; ++s) fold_philox(h->seed, sample_base + (uint32_t)s, h->t, &r->pc, &r->ps[s]);
+    } else {
+        r->A = minstd_power((h->t >> 1) + 1);
+    }
+}
+
+template <int RNG>
+int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    const int c = (int)(h->t & 1);
+    const int nb = g.nsamples == 1 ? 1 : g.nbatches;
+    for (int b = 0; b < nb; ++b) {
+        const LatticeArrays A = h->arrays(b);
+        SweepArgs a;
+        a.S_act = A.S[c];
+        a.S_oth = A.S[1 - c];
+        for (int d = 0; d < 3; ++d) { a.J_act[d] = A.J[d][c]; a.J_oth[d] = A.J[d][1 - c]; }
+        a.L = g.L;
+        a.colour = c;
+        a.T = T;
+        RngLaunch r;
+        fill_rng_launch(h, b, &r);
+        if (g.nsamples != 1) {
+            const uint64_t ngroups = g.Hc / 4;
+            half_sweep_sample_packed<RNG><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, ngroups, g.N);
+        } else if (g.fast && h->kernel_choice == 0) {
+            const int wpr = g.L >> 6;
+            const int W = wpr >= 4 ? 4 : wpr;
+            const int tpr = wpr / W;
+            const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
+            if (W == 4) half_sweep_site_packed<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, r);
+            else if (W == 2) half_sweep_site_packed<RNG, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, r);
+            else half_sweep_site_packed<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, r);
+        } else {
+            const uint64_t nw = (g.Hc + 31) / 32;
+            half_sweep_site_packed_generic<RNG><<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(a, r, nw, g.Hc);
+        }
+        const int rc = check_launch(h);
+        if (rc != ISING_OK) return rc;
+    }
+    h->t += 1;
+    return ISING_OK;
+}
+
+int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
+{
+    return h->rng_mode == ISING_RNG_PHILOX ? launch_half_sweep<0>(h, T, st) : launch_half_sweep<1>(h, T, st);
+}
+
+int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess)
+        return ISING_ECUDA;
+    const int nb = g.nsamples == 1 ? 1 : g.nbatches;
+    for (int b = 0; b < nb; ++b) {
+        const LatticeArrays A = h->arrays(b);
+        MeasureArgs m;
+        for (int c = 0; c < 2; ++c) {
+            m.S[c] = A.S[c];
+            for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
+        }
+        m.L = g.L;
+        if (g.nsamples != 1) {
+            energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
+        } else if (g.fast && h->kernel_choice == 0) {
+            const uint64_t nthreads = 2ull * (uint64_t)(g.L >> 6) * g.L * g.L;
+            energy_site_packed<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(m, h->acc);
+        } else {
+            const uint64_t nw = (g.Hc + 31) / 32;
+            energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc, nw, g.Hc);
+        }
+        const int rc = check_launch(h);
+        if (rc != ISING_OK) return rc;
+    }
+    finalize_energy<<<(g.nsamples + 127) / 128, 128, 0, st>>>(h->acc, g.nsamples, (long long)g.N, d_E, d_M);
+    return check_launch(h);
+}
+
+}  // namespace
+
+extern "C" {
+
+int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
+{
+    Geometry g;
+    if (!out || !make_geometry(L, nsamples, &g)) return ISING_EINVAL;
+    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD) return ISING_EINVAL;
+    *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
+    return ISING_OK;
+}
+
+int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_workspace, size_t workspace_bytes,
+                 ising_t **out)
+{
+    size_t need = 0;
+    if (!out || !d_workspace) return ISING_EINVAL;
+    if (ising_workspace_bytes(L, nsamples, rng_mode, &need) != ISING_OK) return ISING_EINVAL;
+    if (workspace_bytes < need || ((uintptr_t)d_workspace & 255u)) return ISING_EINVAL;
+    ising_t *h = new (std::nothrow) ising_t;
+    if (!h) return ISING_EINVAL;
+    make_geometry(L, nsamples, &h->g);
+    h->seed = seed;
+    h->rng_mode = rng_mode;
+    h->t = 0;
+    h->kernel_choice = 0;
+    h->launches = 0;
+    h->ws = (uint32_t *)d_workspace;
+    h->staging = h->ws + h->g.arrays_total_words;
+    h->acc = (unsigned long long *)(h->staging + h->g.staging_words);
+    *out = h;
+    return ISING_OK;
+}
+
+int ising_destroy(ising_t *h)
+{
+    delete h;
+    return ISING_OK;
+}
+
+int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, void *stream)
+{
+    if (!h || !d_spins || !d_J) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geometry &g = h->g;
+    const size_t W = g.canon_words;
+    if (g.nsamples == 1) {
+        const LatticeArrays A = h->arrays(0);
+        // the padding words of the arrays must not hold garbage (generic kernels read whole words)
+        if (cudaMemsetAsync(h->ws, 0, g.arrays_total_words * sizeof(uint32_t), st) != cudaSuccess) return ISING_ECUDA;
+        if (g.fast) {
+            SplitArgs s;
+            s.narrays = 4;
+            s.L = g.L;
+            s.canon[0] = d_spins;
+            s.out[0][0] = A.S[0];
+            s.out[0][1] = A.S[1];
+            for (int d = 0; d < 3; ++d) {
+                s.canon[1 + d] = d_J + (size_t)d * W;
+                s.out[1 + d][0] = A.J[d][0];
+                s.out[1 + d][1] = A.J[d][1];
+            }
+            const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
+            split_colours_site_packed<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s);
+            return check_launch(h);
+        }
+        const uint64_t nw = (g.Hc + 31) / 32;
+        const unsigned grid = (unsigned)((nw + 255) / 256);
+        for (int c = 0; c < 2; ++c) {
+            gather_site_packed_generic<<<grid, 256, 0, st>>>(d_spins, A.S[c], c, g.L, nw, g.Hc);
+            for (int d = 0; d < 3; ++d)
+                gather_site_packed_generic<<<grid, 256, 0, st>>>(d_J + (size_t)d * W, A.J[d][c], c, g.L, nw, g.Hc);
+        }
+        return check_launch(h, 8);
+    }
+    const unsigned grid = (unsigned)((g.Hc + 255) / 256);
+    for (int b = 0; b < g.nbatches; ++b) {
+        const LatticeArrays A = h->arrays(b);
+        const uint32_t *sp = d_spins + (size_t)b * 32 * W;
+        const uint32_t *jp = d_J + (size_t)b * 32 * 3 * W;
+        for (int c = 0; c < 2; ++c) {
+            gather_sample_packed<<<grid, 256, 0, st>>>(sp, W, A.S[c], c, g.L, g.Hc);
+            for (int d = 0; d < 3; ++d)
+                gather_sample_packed<<<grid, 256, 0, st>>>(jp + (size_t)d * W, 3 * W, A.J[d][c], c, g.L, g.Hc);
+        }
+        const int rc = check_launch(h, 8);
+        if (rc != ISING_OK) return rc;
+    }
+    return ISING_OK;
+}
+
+int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
+{
+    if (!h || !d_out) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geometry &g = h->g;
+    const size_t W = g.canon_words;
+    if (g.nsamples == 1) {
+        const LatticeArrays A = h->arrays(0);
+        if (g.fast) {
+            const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
+            merge_colours_site_packed<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
+        } else {
+            scatter_site_packed_generic<<<(unsigned)((W + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L, W, g.N);
+        }
+        return check_launch(h);
+    }
+    for (int b = 0; b < g.nbatches; ++b) {
+        const LatticeArrays A = h->arrays(b);
+        const dim3 grid((unsigned)((W + 255) / 256), 32);
+        scatter_sample_packed<<<grid, 256, 0, st>>>(A.S[0], A.S[1], d_out + (size_t)b * 32 * W, W, g.L, W, g.N);
+        const int rc = check_launch(h);
+        if (rc != ISING_OK) return rc;
+    }
+    return ISING_OK;
+}
+
+int ising_sweep(ising_t *h, double beta, int nsweeps, void *stream)
+{
+    return ising_sweep_trace(h, beta, nsweeps, nullptr, nullptr, 0, stream);
+}
+
+int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_t *d_M, int every_half_sweeps, void *stream)
+{
+    if (!h || nsweeps < 0) return ISING_EINVAL;
+    const bool trace = d_E != nullptr || d_M != nullptr;
+    if (trace && every_half_sweeps < 1) return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    const Thresholds kt = kernel_thresholds(T);
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t rec = 0;
+    for (int k = 1; k <= 2 * nsweeps; ++k) {
+        int rc = half_sweep(h, kt, st);
+        if (rc != ISING_OK) return rc;
+        if (trace && k % every_half_sweeps == 0) {
+            rc = measure(h, d_E ? (long long *)d_E + rec * h->g.nsamples : nullptr,
+                         d_M ? (long long *)d_M + rec * h->g.nsamples : nullptr, st);
+            if (rc != ISING_OK) return rc;
+            ++rec;
+        }
+    }
+    return ISING_OK;
+}
+
+int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream)
+{
+    if (!h || !d_E) return ISING_EINVAL;
+    return measure(h, (long long *)d_E, (long long *)d_M, (cudaStream_t)stream);
+}
+
+int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps, uint32_t *h_spins_out,
+                   int64_t *h_E, int64_t *h_M, void *stream)
+{
+    if (!h || !h_spins || !h_J || !h_E || nsweeps < 0 || !(beta >= 0.0)) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geometry &g = h->g;
+    const size_t spin_words = (size_t)g.nsamples * g.canon_words, j_words = 3 * spin_words;
+    uint32_t *d_spins = h->staging, *d_J = h->staging + spin_words;
+    if (cudaMemcpyAsync(d_spins, h_spins, spin_words * sizeof(uint32_t), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(d_J, h_J, j_words * sizeof(uint32_t), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return ISING_ECUDA;
+    int rc = ising_load_state(h, d_spins, d_J, stream);
+    if (rc != ISING_OK) return rc;
+    rc = ising_sweep(h, beta, nsweeps, stream);
+    if (rc != ISING_OK) return rc;
+    long long *d_E = (long long *)(h->acc + 2 * (size_t)g.nsamples), *d_M = d_E + g.nsamples;
+    rc = measure(h, d_E, d_M, st);
+    if (rc != ISING_OK) return rc;
+    if (h_spins_out) {
+        rc = ising_get_spins(h, d_spins, stream);
+        if (rc != ISING_OK) return rc;
+        if (cudaMemcpyAsync(h_spins_out, d_spins, spin_words * sizeof(uint32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            return ISING_ECUDA;
+    }
+    if (cudaMemcpyAsync(h_E, d_E, (size_t)g.nsamples * sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return ISING_ECUDA;
+    if (h_M && cudaMemcpyAsync(h_M, d_M, (size_t)g.nsamples * sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return ISING_ECUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? ISING_OK : ISING_ECUDA;
+}
+
+int ising_thresholds(double beta, int rng_mode, uint64_t out[3])
+{
+    if (!out) return ISING_EINVAL;
+    return compute_thresholds(beta, rng_mode, out);
+}
+
+uint64_t ising_fnv1a64_host(const void *h_data, size_t nbytes)
+{
+    const unsigned char *p = (const unsigned char *)h_data;
+    uint64_t hsh = 0xcbf29ce484222325ull;
+    for (size_t k = 0; k < nbytes; ++k) {
+        hsh ^= (uint64_t)p[k];
+        hsh *= 0x100000001b3ull;
+    }
+    return hsh;
+}
+
+int ising_get_t(const ising_t *h, uint64_t *t)
+{
+    if (!h || !t) return ISING_EINVAL;
+    *t = h->t;
+    return ISING_OK;
+}
+
+int ising_set_t(ising_t *h, uint64_t t)
+{
+    if (!h) return ISING_EINVAL;
+    h->t = t;
+    return ISING_OK;
+}
+
+int ising_set_kernel(ising_t *h, int which)
+{
+    if (!h || which < 0 || which > 1) return ISING_EINVAL;
+    h->kernel_choice = which;
+    return ISING_OK;
+}
+
+uint64_t ising_kernel_launches(const ising_t *h) { return h ? h->launches : 0; }
+
+int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double beta, const uint32_t ops[13],
+                                uint64_t word_index, uint64_t site0, uint64_t site_stride, uint32_t *out)
+{
+    if (!ops || !out) return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    const Thresholds kt = kernel_thresholds(T);
+    uint32_t u[6];
+    for (int d = 0; d < 6; ++d) u[d] = ops[7 + d] ^ ops[1 + d];
+    uint32_t sum2, sum1, sum0, c4, c8, c12;
+    satisfied_bond_count(ops[0], u, sum2, sum1, sum0);
+    if (rng_mode == ISING_RNG_PHILOX) {
+        PhiloxCommonConst pc;
+        PhiloxSampleConst ps;
+        fold_philox(seed, 0, t, &pc, &ps);
+        cond_masks_site_packed_philox(pc, ps, (uint32_t)word_index, kt, c4, c8, c12);
+    } else {
+        cond_masks_site_packed_minstd(seed + (site0 + 1) * SPLITMIX_GAMMA, site_stride * SPLITMIX_GAMMA,
+                                      minstd_power((t >> 1) + 1), kt, c4, c8, c12);
+    }
+    *out = ops[0] ^ flip_mask(sum2, sum1, sum0, c4, c8, c12);
+    return ISING_OK;
+}
+
+const char *ising_strerror(int code)
+{
+    switch (code) {
+        case ISING_OK: return "ok";
+        case ISING_EINVAL: return "invalid argument";
+        case ISING_ECUDA: return "CUDA error";
+        default: return "unknown error";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,297 @@
+// sweep_kernels.cuh -- the colour half-sweep kernels.
+//
+// Internal layout.  Sites are split by colour c = (x+y+z)&1 and numbered within their colour by
+// the colour rank j = (x>>1) + (L/2)*(y + L*z)  (the same j that keys the Philox counter, R9).  Per lattice there are
+// 8 bit arrays indexed by j: spins S[c] and couplings Jd[c], d = x,y,z, where Jd[c] holds the bond (i, i+d-hat) of
+// the colour-c site i.
+//   site-packed   (nsamples = 1):  bit (j&31) of word (j>>5); for L = 64*2^k a half-row (fixed y,z) is L/64 words.
+//   sample-packed (nsamples = 32k): word j of batch b holds samples 32b..32b+31 of site j.
+// An active site of colour c in a row of parity p = (y+z)&1 has x = 2m + xodd, xodd = c^p.  Its +-y and +-z neighbours
+// have the same m in the other colour's arrays; its two x-neighbours are bits m and m-1 (xodd = 0) or m and m+1
+// (xodd = 1) of the other colour's half-row.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "update.cuh"
+
+namespace isingk {
+
+struct LatticeArrays {  // one lattice (site-packed) or one batch of 32 samples (sample-packed)
+    uint32_t *S[2];
+    uint32_t *J[3][2];
+};
+
+struct RngLaunch {  // per-launch PRNG constants, passed by value (constant bank)
+    PhiloxCommonConst pc;
+    PhiloxSampleConst ps[32];  // site-packed kernels use ps[0] only
+    uint64_t seed;             // MINSTD
+    uint32_t A;                // MINSTD: 16807^(n+1) mod M for the sweep n = t>>1 of this launch
+    uint32_t tlo, thi;         // half-sweep counter (generic kernel: unfolded Philox)
+    uint32_t k0, k1base;       // Philox key: k1 = k1base ^ sample
+    uint32_t sample_base;      // first sample of this batch (sample-packed)
+};
+
+struct SweepArgs {
+    uint32_t *S_act;           // active colour spins (read + written)
+    const uint32_t *S_oth;     // other colour spins
+    const uint32_t *J_act[3];  // couplings owned by the active colour: bonds (i, i+d)
+    const uint32_t *J_oth[3];  // couplings owned by the other colour: bonds (i-d, i) seen from the active site i
+    int L;
+    int colour;
+    Thresholds T;
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Word-parallel kernel, site-packed, L = 64 * 2^k.  One thread owns W consecutive words of one half-row
+// (W = 4: one 128-bit load per operand array); TPR = (L/64)/W consecutive lanes own a row, and the bit that crosses
+// a word boundary in x comes from the neighbouring lane by a warp shuffle (or from the thread's own words when it
+// owns the whole row).  A warp covers 32/TPR consecutive y, the 8 warps of a CTA cover 8 consecutive z, so most
+// +-y / +-z operand words are L1 hits.
+// ---------------------------------------------------------------------------------------------------
+template <int W> struct WordVec;
+template <> struct WordVec<1> { typedef uint32_t type; };
+template <> struct WordVec<2> { typedef uint2 type; };
+template <> struct WordVec<4> { typedef uint4 type; };
+
+template <int W>
+__device__ __forceinline__ void load_words(const uint32_t *__restrict__ p, size_t word_off, uint32_t out[W])
+{
+    typedef typename WordVec<W>::type V;
+    const V v = __ldg(reinterpret_cast<const V *>(p + word_off));
+    const uint32_t *pv = reinterpret_cast<const uint32_t *>(&v);
+#pragma unroll
+    for (int k = 0; k < W; ++k) out[k] = pv[k];
+}
+
+constexpr int SWEEP_THREADS = 256;
+
+template <int RNG, int W>
+__global__ void __launch_bounds__(SWEEP_THREADS)
+half_sweep_site_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng)
+{
+    const int L = a.L;
+    const int wpr = L >> 6;                 // words per half-row
+    const int tpr = wpr / W;                // threads (lanes) per row: power of two <= 32
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int rows_per_warp = 32 / tpr;
+    const int lane_in_row = lane & (tpr - 1);
+    const int y = blockIdx.x * rows_per_warp + lane / tpr;
+    const int z = blockIdx.y * (SWEEP_THREADS / 32) + warp;
+    const int k0 = lane_in_row * W;
+
+    const int yp = (y + 1) & (L - 1), ym = (y - 1) & (L - 1);
+    const int zp = (z + 1) & (L - 1), zm = (z - 1) & (L - 1);
+    const size_t row = (size_t)wpr * ((size_t)y + (size_t)L * z) + k0;
+    const size_t row_yp = (size_t)wpr * ((size_t)yp + (size_t)L * z) + k0;
+    const size_t row_ym = (size_t)wpr * ((size_t)ym + (size_t)L * z) + k0;
+    const size_t row_zp = (size_t)wpr * ((size_t)y + (size_t)L * zp) + k0;
+    const size_t row_zm = (size_t)wpr * ((size_t)y + (size_t)L * zm) + k0;
+
+    uint32_t s[W], o[W], oyp[W], oym[W], ozp[W], ozm[W];
+    uint32_t jxa[W], jya[W], jza[W], jxo[W], jyo[W], jzo[W];
+    load_words<W>(a.S_act, row, s);
+    load_words<W>(a.S_oth, row, o);
+    load_words<W>(a.S_oth, row_yp, oyp);
+    load_words<W>(a.S_oth, row_ym, oym);
+    load_words<W>(a.S_oth, row_zp, ozp);
+    load_words<W>(a.S_oth, row_zm, ozm);
+    load_words<W>(a.J_act[0], row, jxa);
+    load_words<W>(a.J_act[1], row, jya);
+    load_words<W>(a.J_act[2], row, jza);
+    load_words<W>(a.J_oth[0], row, jxo);
+    load_words<W>(a.J_oth[1], row_ym, jyo);
+    load_words<W>(a.J_oth[2], row_zm, jzo);
+
+    // x-neighbours (row a3).  xodd = 0: +x is bit m of the other colour, -x is bit m-1, and the bond (i-x, i) is owned
+    // by that neighbour, so the word shifted up by one bit is Y = jxo ^ o.  xodd = 1: -x is bit m (with jxo), +x is
+    // bit m+1, so the word shifted down by one bit is Y = o.  The bit entering at the word boundary comes from the
+    // previous / next word of the half-row (periodic).
+    const int xodd = (y + z + a.colour) & 1;
+    uint32_t Y[W];
+#pragma unroll
+    for (int k = 0; k < W; ++k) Y[k] = xodd ? o[k] : (jxo[k] ^ o[k]);
+    uint32_t edge = xodd ? Y[0] : Y[W - 1];
+    if (tpr > 1) {
+        const int src = (lane & ~(tpr - 1)) | ((lane_in_row + (xodd ? 1 : tpr - 1)) & (tpr - 1));
+        edge = __shfl_sync(0xFFFFFFFFu, edge, src);
+    }
+
+    const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
+
+#pragma unroll
+    for (int k = 0; k < W; ++k) {
+        uint32_t ysh;
+        if (xodd) {
+            const uint32_t nxt = (k + 1 < W) ? Y[(k + 1) % W] : edge;
+            ysh = __funnelshift_r(Y[k], nxt, 1);
+        } else {
+            const uint32_t prv = (k > 0) ? Y[(k + W - 1) % W] : edge;
+            ysh = __funnelshift_l(prv, Y[k], 1);
+        }
+        uint32_t u[6];
+        u[0] = jxa[k] ^ (xodd ? ysh : o[k]);         // +x
+        u[1] = xodd ? (jxo[k] ^ o[k]) : ysh;         // -x
+        u[2] = jya[k] ^ oyp[k];                      // +y
+        u[3] = jyo[k] ^ oym[k];                      // -y
+        u[4] = jza[k] ^ ozp[k];                      // +z
+        u[5] = jzo[k] ^ ozm[k];                      // -z
+        uint32_t sum2, sum1, sum0;
+        satisfied_bond_count(s[k], u, sum2, sum1, sum0);
+
+        const uint32_t word_index = (uint32_t)(row + k);
+        uint32_t c4, c8, c12;
+        if (RNG == 0) {
+            cond_masks_site_packed_philox(rng.pc, rng.ps[0], word_index, a.T, c4, c8, c12);
+        } else {
+            const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
+            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A, a.T, c4, c8,
+                                          c12);
+        }
+        s[k] ^= flip_mask(sum2, sum1, sum0, c4, c8, c12);
+    }
+
+    typedef typename WordVec<W>::type V;
+    V out;
+    uint32_t *po = reinterpret_cast<uint32_t *>(&out);
+#pragma unroll
+    for (int k = 0; k < W; ++k) po[k] = s[k];
+    *reinterpret_cast<V *>(a.S_act + row) = out;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Generic kernel, site-packed, any even L >= 4: one thread per word of the active colour, one site at a time with
+// the scalar rule (dE = 2 sigma_i h_i, Eq. 8) and the unfolded Philox.  Slow; it serves lattices whose half-rows
+// are not whole words (L = 16) and, in the tests, as a second GPU implementation with a different layout access
+// and thread mapping (all schemes must give the same bits).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int get_bit(const uint32_t *__restrict__ p, uint64_t j)
+{
+    return (int)((p[j >> 5] >> (j & 31)) & 1u);
+}
+
+__device__ __forceinline__ uint64_t colour_rank(int L, int x, int y, int z)
+{
+    return (uint64_t)(x >> 1) + (uint64_t)(L >> 1) * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
+}
+
+template <int RNG>
+__global__ void __launch_bounds__(256)
+half_sweep_site_packed_generic(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint64_t n_words, uint64_t Hc)
+{
+    const uint64_t widx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (widx >= n_words) return;
+    const int L = a.L, H = L >> 1;
+    uint32_t word = a.S_act[widx];
+    uint32_t flips = 0;
+    uint32_t R4[4] = {0, 0, 0, 0};
+    for (int b = 0; b < 32; ++b) {
+        const uint64_t j = 32 * widx + b;
+        if (j >= Hc) break;
+        const int m = (int)(j % H);
+        const uint64_t r = j / H;
+        const int y = (int)(r % L), z = (int)(r / L);
+        const int x = 2 * m + ((y + z + a.colour) & 1);
+        const int xp = (x + 1 == L) ? 0 : x + 1, xm = (x == 0) ? L - 1 : x - 1;
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const uint64_t jn[6] = {colour_rank(L, xp, y, z), colour_rank(L, xm, y, z), colour_rank(L, x, yp, z),
+                                colour_rank(L, x, ym, z), colour_rank(L, x, y, zp), colour_rank(L, x, y, zm)};
+        int h = 0;  // local field sum_k J_ik sigma_k, sigma = 2 bit - 1, J = 1 - 2 bit (Eq. 10)
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            const int sk = 2 * get_bit(a.S_oth, jn[d]) - 1;
+            const int Jb = (d & 1) ? get_bit(a.J_oth[d >> 1], jn[d]) : get_bit(a.J_act[d >> 1], j);
+            h += (1 - 2 * Jb) * sk;
+        }
+        const int si = 2 * (int)((word >> b) & 1u) - 1;
+        const int dE = 2 * si * h;
+        uint32_t R;
+        if (RNG == 0) {
+            if ((b & 3) == 0)
+                philox4x32_10(rng.tlo, rng.thi, (uint32_t)(j >> 2), (uint32_t)(j >> 34), rng.k0, rng.k1base, R4);
+            R = R4[b & 3];
+        } else {
+            const uint64_t q = (uint64_t)x + (uint64_t)L * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
+            R = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(rng.seed + (q + 1) * SPLITMIX_GAMMA));
+        }
+        bool acc;
+        if (dE <= 0) acc = true;
+        else if (dE == 4) acc = (R < a.T.t4) || a.T.always4;
+        else if (dE == 8) acc = (R < a.T.t8) || a.T.always8;
+        else acc = (R < a.T.t12) || a.T.always12;
+        if (acc) flips |= 1u << b;
+    }
+    a.S_act[widx] = word ^ flips;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Sample-packed kernel (nsamples = 32 per batch), any even L >= 4.  One thread per Philox group g = 4 consecutive
+// same-colour sites j = 4g..4g+3; for each of the 32 samples (bits) one Philox call keyed by the sample gives the four
+// sites' draws (R9).  Neighbours are whole words, so no x-alignment is needed.
+// ---------------------------------------------------------------------------------------------------
+template <int RNG>
+__global__ void __launch_bounds__(128)
+half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint64_t n_groups, uint64_t N)
+{
+    const uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n_groups) return;
+    const int L = a.L, H = L >> 1;
+    uint32_t s[4], sum2[4], sum1[4], sum0[4];
+    uint64_t site[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint64_t j = 4 * g + w;
+        const int m = (int)(j % H);
+        const uint64_t r = j / H;
+        const int y = (int)(r % L), z = (int)(r / L);
+        const int x = 2 * m + ((y + z + a.colour) & 1);
+        const int xp = (x + 1 == L) ? 0 : x + 1, xm = (x == 0) ? L - 1 : x - 1;
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const uint64_t jn[6] = {colour_rank(L, xp, y, z), colour_rank(L, xm, y, z), colour_rank(L, x, yp, z),
+                                colour_rank(L, x, ym, z), colour_rank(L, x, y, zp), colour_rank(L, x, y, zm)};
+        uint32_t u[6];
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            const uint32_t Jw = (d & 1) ? __ldg(a.J_oth[d >> 1] + jn[d]) : __ldg(a.J_act[d >> 1] + j);
+            u[d] = Jw ^ __ldg(a.S_oth + jn[d]);
+        }
+        s[w] = a.S_act[j];
+        satisfied_bond_count(s[w], u, sum2[w], sum1[w], sum0[w]);
+        site[w] = (uint64_t)x + (uint64_t)L * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
+    }
+    uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};
+#pragma unroll
+    for (int b = 0; b < 32; ++b) {
+        uint32_t R[4];
+        if (RNG == 0) {
+            philox_folded(rng.pc, rng.ps[b], (uint32_t)g, R);
+        } else {
+            const uint64_t qs = (uint64_t)(rng.sample_base + b) * N;
+#pragma unroll
+            for (int w = 0; w < 4; ++w)
+                R[w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(rng.seed + (qs + site[w] + 1) * SPLITMIX_GAMMA));
+        }
+#pragma unroll
+        for (int w = 0; w < 4; ++w) c4[w] |= (R[w] < a.T.t4 ? 1u : 0u) << b;
+        uint32_t mn = R[0] < R[1] ? R[0] : R[1];
+        const uint32_t mn2 = R[2] < R[3] ? R[2] : R[3];
+        mn = mn < mn2 ? mn : mn2;
+        if (mn < a.T.t8) {
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                c8[w] |= (R[w] < a.T.t8 ? 1u : 0u) << b;
+                c12[w] |= (R[w] < a.T.t12 ? 1u : 0u) << b;
+            }
+        }
+    }
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t f = flip_mask(sum2[w], sum1[w], sum0[w], c4[w] | a.T.always4, c8[w] | a.T.always8,
+                                     c12[w] | a.T.always12);
+        a.S_act[4 * g + w] = s[w] ^ f;
+    }
+}
+
+}  // namespace isingk

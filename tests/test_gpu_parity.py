@@ -1,0 +1,328 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle -- tolerance 0.
+
+All outputs are integers (spins, energies, magnetisations, checksums), so every comparison is exact (R15).
+Small and medium cases compare whole trajectories element by element; the L=1024 case (the configuration bench.py
+times) compares one full sweep element by element, then sampled sites of a later half-sweep against the oracle's
+single-site rule, and the word-parallel kernel against the generic one-site-at-a-time kernel (all
+schemes must give the same bits).
+"""
+import os
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import ea3d  # noqa: E402
+from paper_1411_0127_b200 import MINSTD, PHILOX, Ising, binding, synth  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+SEED = synth.DYN_SEED
+FULL = os.environ.get("ISING_FULL_CONFIGS", "0") == "1"  # run configs 2-4 at their full sweep counts (minutes of oracle time)
+
+
+def dev(a: np.ndarray):
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.int32)).cuda()
+
+
+def host_u32(t) -> np.ndarray:
+    return t.cpu().numpy().view(np.uint32)
+
+
+def make_pair(L, nsamples, rng_mode, spins, J, seed=SEED):
+    o = ea3d.Oracle(L, nsamples, seed, rng_mode)
+    o.load_packed(spins, J)
+    g = Ising(L, nsamples, seed, rng_mode)
+    g.ising_load_state(dev(spins), dev(J))
+    return o, g
+
+
+def assert_same_state(o, g, what=""):
+    got = host_u32(g.ising_get_spins())
+    want = o.spins_packed()
+    assert np.array_equal(got, want), f"{what}: {np.count_nonzero(got != want)} of {want.size} spin words differ"
+    E, M = g.ising_energy()
+    Eo, Mo = o.energy()
+    assert np.array_equal(E.cpu().numpy(), Eo) and np.array_equal(M.cpu().numpy(), Mo), what
+
+
+# ------------------------------------------------------------------------------------------------ load / get / energy
+
+@pytest.mark.parametrize("L,nsamples", [(4, 1), (6, 1), (16, 1), (24, 1), (64, 1), (128, 1), (256, 1), (4, 32), (6, 32),
+                                        (16, 64)])
+def test_layout_round_trip_and_energy(L, nsamples):
+    spins, J = synth.make_spins(L, nsamples, 7), synth.make_couplings(L, nsamples, 3)
+    o, g = make_pair(L, nsamples, PHILOX, spins, J)
+    assert_same_state(o, g, "after load")
+    assert np.array_equal(host_u32(g.ising_get_spins()), spins)
+    if nsamples == 1 and L >= 64:  # the generic measurement kernel on the same internal layout
+        g.ising_set_kernel(1)
+        assert_same_state(o, g, "generic measure")
+
+
+def test_energy_closed_forms_on_gpu():
+    L = 64
+    W = synth.words_per_sample(L)
+    up = synth.make_spins(L, 1, init="up")
+    ferro = np.zeros((1, 3, W), dtype=np.uint32)
+    g = Ising(L, 1, 1, PHILOX)
+    g.ising_load_state(dev(up), dev(ferro))
+    E, M = g.ising_energy()
+    assert int(E[0]) == -3 * L**3 and int(M[0]) == L**3
+    J = synth.make_couplings(L, 1, 5)
+    g.ising_load_state(dev(up), dev(J))
+    E, _ = g.ising_energy()
+    nneg = int(np.unpackbits(J.view(np.uint8)).sum())  # all-up: E = -sum J = -(3N - 2 #(J=-1))
+    assert int(E[0]) == -(3 * L**3 - 2 * nneg)
+
+
+# ------------------------------------------------------------------------------------------------ BASELINE.json configs
+
+def test_config1_L16_philox_energy_every_half_sweep():
+    cfg, spins, J = synth.make_config(1)
+    o, g = make_pair(cfg["L"], 1, cfg["rng_mode"], spins, J)
+    E, M = g.ising_sweep_trace(cfg["beta"], cfg["sweeps"], every_half_sweeps=1)
+    E, M = E.cpu().numpy()[:, 0], M.cpu().numpy()[:, 0]
+    for k in range(2 * cfg["sweeps"]):
+        o.half_sweep(cfg["beta"])
+        Eo, Mo = o.energy()
+        assert (int(E[k]), int(M[k])) == (int(Eo[0]), int(Mo[0])), k
+    assert_same_state(o, g, "config 1 final")
+    assert g.ising_get_t() == 20
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L", [4, 6, 16, 24, 32, 64, 128, 256])
+def test_site_packed_trajectories(L, rng_mode):
+    """Ragged and whole-word half-rows, both kernels (word-parallel for L = 64*2^k, generic otherwise)."""
+    spins, J = synth.make_spins(L, 1, 11), synth.make_couplings(L, 1, 5)
+    o, g = make_pair(L, 1, rng_mode, spins, J)
+    nsw = 12 if L <= 64 else 4
+    beta = 0.6
+    for _ in range(nsw):
+        o.sweep(beta, 1)
+    E, M = g.ising_sweep_trace(beta, nsw, every_half_sweeps=2 * nsw)
+    assert_same_state(o, g, f"L={L}")
+    Eo, Mo = o.energy()
+    assert int(E[0, 0]) == int(Eo[0]) and int(M[0, 0]) == int(Mo[0])
+    assert int(Eo[0]) == int(o.dE_sum[0]) + int(ea3d.Oracle.energy(_loaded(L, 1, rng_mode, spins, J))[0][0])
+
+
+def _loaded(L, ns, rng_mode, spins, J):
+    o = ea3d.Oracle(L, ns, SEED, rng_mode)
+    o.load_packed(spins, J)
+    return o
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("beta", [0.0, float("inf"), 1 / 1.1])
+def test_special_temperatures(rng_mode, beta):
+    L = 64
+    spins, J = synth.make_spins(L, 1, 4), synth.make_couplings(L, 1, 9)
+    o, g = make_pair(L, 1, rng_mode, spins, J)
+    E0 = int(g.ising_energy()[0][0])
+    for k in range(3):
+        o.sweep(beta, 1)
+        g.ising_sweep(beta, 1)
+        assert_same_state(o, g, f"beta={beta} sweep {k}")
+    if beta == 0.0:  # every proposal accepted: three sweeps invert every spin three times
+        assert np.array_equal(host_u32(g.ising_get_spins()), ~spins)
+        assert int(g.ising_energy()[0][0]) == E0
+    if beta == float("inf"):
+        assert int(g.ising_energy()[0][0]) <= E0
+
+
+def test_config2_L64_32_samples_philox():
+    cfg, spins, J = synth.make_config(2)
+    nsw = cfg["sweeps"] if FULL else 50
+    o, g = make_pair(cfg["L"], 32, cfg["rng_mode"], spins, J)
+    E, _ = g.ising_sweep_trace(cfg["beta"], nsw, every_half_sweeps=20, want_M=False)  # every 10 sweeps
+    E = E.cpu().numpy()
+    for r in range(nsw // 10):
+        o.sweep(cfg["beta"], 10)
+        assert np.array_equal(E[r], o.energy()[0]), f"record {r}"
+    assert_same_state(o, g, "config 2 final")
+    assert len(set(E[-1].tolist())) > 16  # the 32 samples really are different systems
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (10, 32), (16, 64)])
+def test_sample_packed_small(L, nsamples, rng_mode):
+    spins, J = synth.make_spins(L, nsamples, 21), synth.make_couplings(L, nsamples, 8)
+    o, g = make_pair(L, nsamples, rng_mode, spins, J)
+    o.sweep(0.7, 6)
+    g.ising_sweep(0.7, 6)
+    assert_same_state(o, g, f"L={L} x {nsamples}")
+
+
+def test_config3_L256_minstd_energy_and_magnetisation_per_sweep():
+    cfg, spins, J = synth.make_config(3)
+    nsw = cfg["sweeps"] if FULL else 20
+    o, g = make_pair(cfg["L"], 1, cfg["rng_mode"], spins, J)
+    E, M = g.ising_sweep_trace(cfg["beta"], nsw, every_half_sweeps=2)
+    E, M = E.cpu().numpy()[:, 0], M.cpu().numpy()[:, 0]
+    for k in range(nsw):
+        o.sweep(cfg["beta"], 1)
+        Eo, Mo = o.energy()
+        assert (int(E[k]), int(M[k])) == (int(Eo[0]), int(Mo[0])), k
+    assert_same_state(o, g, "config 3 final")
+
+
+def test_config4_L512_philox_fnv_checksums():
+    cfg, spins, J = synth.make_config(4)
+    nsw = cfg["sweeps"] if FULL else 10
+    o, g = make_pair(cfg["L"], 1, cfg["rng_mode"], spins, J)
+    for r in range(max(1, nsw // 10)):
+        o.sweep(cfg["beta"], 10)
+        g.ising_sweep(cfg["beta"], 10)
+        got = binding.ising_fnv1a64_host(host_u32(g.ising_get_spins()))
+        assert got == ea3d.fnv1a64(o.spins_packed()), f"checksum after {10 * (r + 1)} sweeps"
+    assert_same_state(o, g, "config 4 final")
+    # and the remaining sweeps of the config against the generic kernel (second GPU implementation)
+    g2 = Ising(cfg["L"], 1, SEED, cfg["rng_mode"])
+    g2.ising_load_state(g.ising_get_spins(), dev(J))
+    g2.ising_set_t(g.ising_get_t())
+    g2.ising_set_kernel(1)
+    g.ising_sweep(cfg["beta"], 5)
+    g2.ising_sweep(cfg["beta"], 5)
+    assert torch.equal(g.ising_get_spins(), g2.ising_get_spins())
+
+
+# ------------------------------------------------------------------------------------------------ invariances
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+def test_batching_of_sweeps_into_calls_and_resume(rng_mode):
+    L = 64
+    spins, J = synth.make_spins(L, 1, 2), synth.make_couplings(L, 1, 1)
+    a = Ising(L, 1, SEED, rng_mode)
+    a.ising_load_state(dev(spins), dev(J))
+    a.ising_sweep(0.9, 10)
+    b = Ising(L, 1, SEED, rng_mode)
+    b.ising_load_state(dev(spins), dev(J))
+    for _ in range(10):
+        b.ising_sweep(0.9, 1)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    # checkpoint / resume: (spins, t) is the whole dynamic state
+    c = Ising(L, 1, SEED, rng_mode)
+    c.ising_load_state(dev(spins), dev(J))
+    c.ising_sweep(0.9, 4)
+    d = Ising(L, 1, SEED, rng_mode)
+    d.ising_load_state(c.ising_get_spins(), dev(J))
+    d.ising_set_t(c.ising_get_t())
+    d.ising_sweep(0.9, 6)
+    assert torch.equal(a.ising_get_spins(), d.ising_get_spins())
+    # a different seed gives a different trajectory
+    e = Ising(L, 1, SEED + 1, rng_mode)
+    e.ising_load_state(dev(spins), dev(J))
+    e.ising_sweep(0.9, 10)
+    assert not torch.equal(a.ising_get_spins(), e.ising_get_spins())
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L", [64, 128, 256, 512])
+def test_word_parallel_kernel_equals_generic_kernel(L, rng_mode):
+    spins, J = synth.make_spins(L, 1, 31), synth.make_couplings(L, 1, 32)
+    a = Ising(L, 1, SEED, rng_mode)
+    b = Ising(L, 1, SEED, rng_mode)
+    b.ising_set_kernel(1)
+    for g in (a, b):
+        g.ising_load_state(dev(spins), dev(J))
+        g.ising_sweep(1 / 1.1, 3)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
+
+
+def test_run_host_equals_device_calls():
+    L = 128
+    spins, J = synth.make_spins(L, 1, 2), synth.make_couplings(L, 1, 1)
+    a = Ising(L, 1, SEED, PHILOX)
+    hs = torch.from_numpy(spins.view(np.int32)).pin_memory()
+    hJ = torch.from_numpy(J.view(np.int32)).pin_memory()
+    out = torch.empty_like(hs).pin_memory()
+    E, M = a.ising_run_host(hs, hJ, 1 / 1.1, 5, out)
+    o = _loaded(L, 1, PHILOX, spins, J)
+    o.sweep(1 / 1.1, 5)
+    assert np.array_equal(out.numpy().view(np.uint32), o.spins_packed())
+    assert int(E[0]) == int(o.energy()[0][0]) and int(M[0]) == int(o.energy()[1][0])
+    assert a.ising_kernel_launches() == 1 + 10 + 2 + 1
+
+
+# ------------------------------------------------------------------------------------------------ config 5, full size
+
+def _avail_gib():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 2**30
+    except Exception:
+        return 0.0
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+def test_config5_L1024_full_size(rng_mode):
+    cfg, spins, J = synth.make_config(5)
+    L, beta, nsw = cfg["L"], cfg["beta"], cfg["sweeps"]
+    dJ = dev(J)
+    g = Ising(L, 1, SEED, rng_mode)
+    g.ising_load_state(dev(spins), dJ)
+    assert np.array_equal(host_u32(g.ising_get_spins()), spins)
+    have_ram = _avail_gib() > 24
+    if have_ram:  # one full sweep, element by element (about 10^9 oracle updates)
+        o = _loaded(L, 1, rng_mode, spins, J)
+        o.sweep(beta, 1)
+        g.ising_sweep(beta, 1)
+        assert_same_state(o, g, "L=1024 after one sweep")
+        del o
+    else:
+        g.ising_sweep(beta, 1)
+    g.ising_sweep(beta, nsw - 2)
+    t0 = g.ising_get_t()
+    assert t0 == 2 * (nsw - 1)
+    d_before = g.ising_get_spins().clone()  # state before the last sweep
+    E_trace, _ = g.ising_sweep_trace(beta, 1, every_half_sweeps=1, want_M=False)
+    d_end = g.ising_get_spins().clone()
+
+    # (1) the generic one-site-at-a-time kernel reproduces the last sweep from the same state
+    g2 = Ising(L, 1, SEED, rng_mode)
+    g2.ising_set_kernel(1)
+    g2.ising_load_state(d_before, dJ)
+    g2.ising_set_t(t0)
+    g2.ising_sweep(beta, 1)
+    assert torch.equal(g2.ising_get_spins(), d_end), "word-parallel vs generic kernel at L=1024"
+    assert int(g2.ising_energy()[0][0]) == int(E_trace[-1, 0])
+    del g2
+
+    # (2) all 20 sweeps in one call (the launch pattern bench.py times) from a fresh handle: same bits
+    g3 = Ising(L, 1, SEED, rng_mode)
+    g3.ising_load_state(dev(spins), dJ)
+    g3.ising_sweep(beta, nsw)
+    assert torch.equal(g3.ising_get_spins(), d_end)
+    del g3
+
+    if not have_ram:
+        pytest.skip("not enough host RAM for the int8 oracle arrays at L=1024: oracle checks skipped")
+
+    # (3) sampled sites against the oracle's single-site rule.  Red sites change only in the red half-sweep t0, so their
+    # final value is before ^ flips(t0).  For blue sites a handle is put at the odd counter t0+1 with the same state, so
+    # that its next sweep starts with the blue half-sweep t0+1 (then red t0+2): blue final = before ^ flips(t0+1).
+    s_before = host_u32(d_before)
+    o = _loaded(L, 1, rng_mode, s_before, J)
+    g4 = Ising(L, 1, SEED, rng_mode)
+    g4.ising_load_state(d_before, dJ)
+    g4.ising_set_t(t0 + 1)
+    g4.ising_sweep(beta, 1)
+    before_bits = np.unpackbits(s_before.view(np.uint8), bitorder="little")
+    finals = {0: np.unpackbits(host_u32(d_end).view(np.uint8), bitorder="little"),
+              1: np.unpackbits(host_u32(g4.ising_get_spins()).view(np.uint8), bitorder="little")}
+    rng = np.random.default_rng(123)
+    for colour in (0, 1):
+        n_flipped = 0
+        for _ in range(2000):
+            x, y, z = (int(v) for v in rng.integers(0, L, 3))
+            if ((x + y + z) & 1) != colour:
+                x ^= 1
+            i = x + L * (y + L * z)
+            flips, dE, R = o.site_flips(beta, 0, x, y, z, t0 + colour)
+            assert flips in (0, 1)
+            assert int(finals[colour][i]) == int(before_bits[i]) ^ flips, (colour, x, y, z, dE, R)
+            n_flipped += flips
+        assert 0 < n_flipped < 2000
