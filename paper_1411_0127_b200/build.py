@@ -8,6 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libising_b200.so")
+STAMP = LIB + ".srchash"  # git-ignored with the .so; travels with it to the GPU box
 SOURCES = ["ising_api.cu"]
 HEADERS = ["rng.cuh", "update.cuh", "sweep_kernels.cuh", "measure_kernels.cuh", "layout_kernels.cuh",
            os.path.join("..", "..", "include", "ising.h")]
@@ -24,12 +25,21 @@ def nvcc_command(out: str = LIB, extra: list[str] | None = None) -> list[str]:
             *[os.path.join(CSRC, s) for s in SOURCES], *(extra or [])]
 
 
+def source_hash() -> str:
+    """Hash of every source the library is built from (mtimes do not survive the copy to the GPU box)."""
+    import hashlib
+
+    h = hashlib.sha256()
+    for d in [os.path.join(CSRC, s) for s in SOURCES] + [os.path.join(CSRC, x) for x in HEADERS]:
+        h.update(open(d, "rb").read())
+    h.update(" ".join(a for a in nvcc_command(out="-")[1:] if not a.startswith(HERE)).encode())  # flags, not paths
+    return h.hexdigest()
+
+
 def is_stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + [os.path.join(CSRC, h) for h in HEADERS]
-    return any(os.path.getmtime(d) > t for d in deps)
+    return open(STAMP).read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -39,6 +49,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError("libising_b200.so is not built and nvcc is not available")
         cmd = nvcc_command(extra=["-Xptxas", "-v"] if verbose else None)
         subprocess.run(cmd, check=True)
+        with open(STAMP, "w") as f:
+            f.write(source_hash())
     return LIB
 
 

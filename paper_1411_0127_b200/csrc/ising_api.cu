@@ -107,6 +107,8 @@ Thresholds kernel_thresholds(const uint64_t T[3])
         t[i] = always ? 0xFFFFFFFFu : (uint32_t)T[i];
         al[i] = always ? 0xFFFFFFFFu : 0u;
     }
+    k.k4 = (uint32_t)(0x100000000ull - T[0]);  // (2^32 - T4) mod 2^32: 0 for T4 = 2^32 (never a carry) and for T4 = 0
+    k.never4 = T[0] == 0 ? 0xFFFFFFFFu : 0u;
     return k;
 }
 
@@ -189,8 +191,9 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         if (g.nsamples != 1) {
             energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
         } else if (g.fast && h->kernel_choice == 0) {
-            const uint64_t nthreads = 2ull * (uint64_t)(g.L >> 6) * g.L * g.L;
-            energy_site_packed<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(m, h->acc);
+            const uint64_t nthreads = (uint64_t)(g.L >> 6) * g.L * g.L;  // words per colour; grid-stride above 148 x 16 CTAs
+            const uint64_t nblocks = (nthreads + 255) / 256;
+            energy_site_packed<<<(unsigned)(nblocks < 2368 ? nblocks : 2368), 256, 0, st>>>(m, h->acc);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc, nw, g.Hc);

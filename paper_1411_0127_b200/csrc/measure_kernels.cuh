@@ -27,38 +27,57 @@ __device__ __forceinline__ void warp_reduce_add2(unsigned long long &a, unsigned
     }
 }
 
-// Site-packed, L = 64*2^k: one thread per word of either colour.  The +x neighbour of the colour-c site with bit m is
-// bit m (xodd = 0) or bit m+1 (xodd = 1) of the other colour's half-row; +y / +z neighbours are the same bit one row up.
+// Block-level sum of two counters, then one atomic pair per block.
+__device__ __forceinline__ void block_accumulate2(unsigned long long a, unsigned long long b, unsigned long long *acc)
+{
+    __shared__ unsigned long long sh[2][32];
+    warp_reduce_add2(a, b);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { sh[0][warp] = a; sh[1][warp] = b; }
+    __syncthreads();
+    if (warp == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        a = lane < nw ? sh[0][lane] : 0;
+        b = lane < nw ? sh[1][lane] : 0;
+        warp_reduce_add2(a, b);
+        if (lane == 0) {
+            atomicAdd(&acc[0], a);
+            atomicAdd(&acc[1], b);
+        }
+    }
+}
+
+// Site-packed, L = 64*2^k: a grid-stride loop over the words of both colours.  The +x neighbour of the colour-c site
+// with bit m is bit m (xodd = 0) or bit m+1 (xodd = 1) of the other colour's half-row; +y / +z neighbours are the same
+// bit one row up.  Every word is read once from HBM (the neighbour reads hit L1/L2): 512 MiB at L = 1024.
 __global__ void __launch_bounds__(256)
 energy_site_packed(const MeasureArgs a, unsigned long long *acc /* [0] = unsatisfied bonds, [1] = up spins */)
 {
     const int L = a.L, wpr = L >> 6;
     const uint64_t words_per_colour = (uint64_t)wpr * L * L;
-    const uint64_t tid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long unsat = 0, up = 0;
-    if (tid < 2 * words_per_colour) {
-        const int c = tid >= words_per_colour;
-        const uint64_t widx = tid - (c ? words_per_colour : 0);
-        const int k = (int)(widx % wpr);
-        const uint64_t r = widx / wpr;
-        const int y = (int)(r % L), z = (int)(r / L);
-        const int yp = (y + 1) & (L - 1), zp = (z + 1) & (L - 1);
-        const int xodd = (y + z + c) & 1;
-        const uint32_t *So = a.S[1 - c];
-        const uint32_t s = a.S[c][widx];
-        const size_t rowbase = (size_t)wpr * ((size_t)y + (size_t)L * z);
-        uint32_t nx = So[rowbase + k];
-        if (xodd) nx = __funnelshift_r(nx, So[rowbase + ((k + 1) % wpr)], 1);
-        const uint32_t ny = So[(size_t)wpr * ((size_t)yp + (size_t)L * z) + k];
-        const uint32_t nz = So[(size_t)wpr * ((size_t)y + (size_t)L * zp) + k];
-        unsat = __popc(a.J[0][c][widx] ^ s ^ nx) + __popc(a.J[1][c][widx] ^ s ^ ny) + __popc(a.J[2][c][widx] ^ s ^ nz);
-        up = __popc(s);
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        const uint32_t *__restrict__ Sc = a.S[c], *__restrict__ So = a.S[1 - c];
+        const uint32_t *__restrict__ Jx = a.J[0][c], *__restrict__ Jy = a.J[1][c], *__restrict__ Jz = a.J[2][c];
+        for (uint64_t widx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; widx < words_per_colour;
+             widx += (uint64_t)gridDim.x * blockDim.x) {
+            const int k = (int)(widx % wpr);
+            const uint64_t r = widx / wpr;
+            const int y = (int)(r % L), z = (int)(r / L);
+            const int yp = (y + 1) & (L - 1), zp = (z + 1) & (L - 1);
+            const int xodd = (y + z + c) & 1;
+            const uint32_t s = Sc[widx];
+            const size_t rowbase = (size_t)wpr * r;
+            uint32_t nx = So[rowbase + k];
+            if (xodd) nx = __funnelshift_r(nx, So[rowbase + ((k + 1) % wpr)], 1);
+            const uint32_t ny = So[(size_t)wpr * ((size_t)yp + (size_t)L * z) + k];
+            const uint32_t nz = So[(size_t)wpr * ((size_t)y + (size_t)L * zp) + k];
+            unsat += __popc(Jx[widx] ^ s ^ nx) + __popc(Jy[widx] ^ s ^ ny) + __popc(Jz[widx] ^ s ^ nz);
+            up += __popc(s);
+        }
     }
-    warp_reduce_add2(unsat, up);
-    if ((threadIdx.x & 31) == 0) {
-        atomicAdd(&acc[0], unsat);
-        atomicAdd(&acc[1], up);
-    }
+    block_accumulate2(unsat, up, acc);
 }
 
 // Site-packed, any even L: one thread per word, one site at a time.
@@ -86,11 +105,7 @@ energy_site_packed_generic(const MeasureArgs a, unsigned long long *acc, uint64_
             up += s;
         }
     }
-    warp_reduce_add2(unsat, up);
-    if ((threadIdx.x & 31) == 0) {
-        atomicAdd(&acc[0], unsat);
-        atomicAdd(&acc[1], up);
-    }
+    block_accumulate2(unsat, up, acc);
 }
 
 // Sample-packed: one thread per site (either colour); bit b of every word belongs to sample b, so the per-sample counts

@@ -1,0 +1,53 @@
+"""Integer issue-rate microbenchmark (csrc/int_peak.cu): measures, on the GPU it runs on, the thread-instructions per
+second of the instruction mixes the half-sweep kernel is made of.  `python -m paper_1411_0127_b200.int_peak` prints one
+JSON line; DESIGN.md section 6 uses it to check the ALU roofline denominator (148 SMs x 4 schedulers x 32 lanes x clock
+for the issue limit, half of that per pipe)."""
+from __future__ import annotations
+
+import ctypes as C
+import json
+import os
+import subprocess
+
+from . import build as _build
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "csrc", "int_peak.cu")
+LIB = os.path.join(HERE, "libint_peak.so")
+MIXES = {0: "LOP3 only", 1: "IMAD.WIDE.U32 only", 2: "IMAD.WIDE + LOP3 dependent 1:1", 3: "Philox round (2 IMAD.WIDE + 2 LOP3)",
+         4: "ISETP + SEL + LOP3"}
+
+
+def build(force: bool = False) -> str:
+    import hashlib
+
+    stamp = LIB + ".srchash"
+    digest = hashlib.sha256(open(SRC, "rb").read()).hexdigest()
+    if force or not os.path.exists(LIB) or not os.path.exists(stamp) or open(stamp).read().strip() != digest:
+        subprocess.run([_build.nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+                        "-Xcompiler", "-fPIC", "-shared", "-o", LIB, SRC], check=True)
+        with open(stamp, "w") as f:
+            f.write(digest)
+    return LIB
+
+
+def run(ctas_per_sm: int = 8, iters: int = 4096, reps: int = 5) -> dict:
+    import torch
+
+    lib = C.CDLL(build())
+    lib.int_peak_run.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    scratch = torch.zeros(16, dtype=torch.int32, device="cuda")
+    out = {"sms": sms, "ctas_per_sm": ctas_per_sm, "threads_per_cta": 256, "mixes": {}}
+    for mix, name in MIXES.items():
+        ms, ops = C.c_float(0), C.c_double(0)
+        rc = lib.int_peak_run(mix, sms * ctas_per_sm, iters, reps, scratch.data_ptr(), C.byref(ms), C.byref(ops))
+        if rc != 0:
+            raise RuntimeError(f"int_peak_run({mix}) failed: {rc}")
+        rate = ops.value / (ms.value * 1e-3)
+        out["mixes"][name] = {"Tinst_per_s": rate / 1e12, "inst_per_clk_per_sm_at_1965MHz": rate / sms / 1.965e9, "ms": ms.value}
+    return out
+
+
+if __name__ == "__main__":
+    print(json.dumps(run()))
