@@ -107,8 +107,6 @@ Thresholds kernel_thresholds(const uint64_t T[3])
         t[i] = always ? 0xFFFFFFFFu : (uint32_t)T[i];
         al[i] = always ? 0xFFFFFFFFu : 0u;
     }
-    k.k4 = (uint32_t)(0x100000000ull - T[0]);  // (2^32 - T4) mod 2^32: 0 for T4 = 2^32 (never a carry) and for T4 = 0
-    k.never4 = T[0] == 0 ? 0xFFFFFFFFu : 0u;
     return k;
 }
 
@@ -155,9 +153,14 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             const int W = wpr >= 4 ? 4 : wpr;
             const int tpr = wpr / W;
             const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
-            if (W == 4) half_sweep_site_packed<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, r);
-            else if (W == 2) half_sweep_site_packed<RNG, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, r);
-            else half_sweep_site_packed<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, r);
+            SiteRng sr;
+            sr.pc = r.pc;
+            sr.ps = r.ps[0];
+            sr.seed = r.seed;
+            sr.A2 = 2u * r.A;
+            if (W == 4) half_sweep_site_packed<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+            else if (W == 2) half_sweep_site_packed<RNG, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+            else half_sweep_site_packed<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             half_sweep_site_packed_generic<RNG><<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(a, r, nw, g.Hc);
@@ -435,10 +438,8 @@ int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double 
     uint64_t T[3];
     if (compute_thresholds(beta, rng_mode, T) != ISING_OK) return ISING_EINVAL;
     const Thresholds kt = kernel_thresholds(T);
-    uint32_t u[6];
-    for (int d = 0; d < 6; ++d) u[d] = ops[7 + d] ^ ops[1 + d];
     uint32_t sum2, sum1, sum0, c4, c8, c12;
-    satisfied_bond_count(ops[0], u, sum2, sum1, sum0);
+    satisfied_bond_count(ops[0], ops + 7, ops + 1, sum2, sum1, sum0);
     if (rng_mode == ISING_RNG_PHILOX) {
         PhiloxCommonConst pc;
         PhiloxSampleConst ps;
@@ -446,7 +447,7 @@ int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double 
         cond_masks_site_packed_philox(pc, ps, (uint32_t)word_index, kt, c4, c8, c12);
     } else {
         cond_masks_site_packed_minstd(seed + (site0 + 1) * SPLITMIX_GAMMA, site_stride * SPLITMIX_GAMMA,
-                                      minstd_power((t >> 1) + 1), kt, c4, c8, c12);
+                                      2u * minstd_power((t >> 1) + 1), kt, c4, c8, c12);
     }
     *out = ops[0] ^ flip_mask(sum2, sum1, sum0, c4, c8, c12);
     return ISING_OK;

@@ -136,6 +136,15 @@ ISING_HD uint32_t minstd_mulmod(uint32_t A, uint32_t s0)
     return (x1 & MINSTD_M) + (x1 >> 31);
 }
 
+// The same with the multiplier doubled (A2 = 2A < 2^32): the 63-bit product 2*A*s0 has (A*s0) >> 31 in its high word
+// and (A*s0) & M in bits 1..31 of its low word, so the first fold needs no funnel shift and no mask.
+ISING_HD uint32_t minstd_mulmod2(uint32_t A2, uint32_t s0)
+{
+    const uint64_t p = (uint64_t)A2 * s0;
+    const uint32_t x1 = ((uint32_t)p >> 1) + (uint32_t)(p >> 32);
+    return (x1 & MINSTD_M) + (x1 >> 31);
+}
+
 inline uint32_t minstd_power(uint64_t n_plus_1)
 {  // 16807^(n+1) mod M by square-and-multiply (host, once per sweep)
     uint64_t base = 16807u, acc = 1u, e = n_plus_1;

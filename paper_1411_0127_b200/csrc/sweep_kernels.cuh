@@ -47,7 +47,10 @@ struct SweepArgs {
 // (W = 4: one 128-bit load per operand array); TPR = (L/64)/W consecutive lanes own a row, and the bit that crosses
 // a word boundary in x comes from the neighbouring lane by a warp shuffle (or from the thread's own words when it
 // owns the whole row).  A warp covers 32/TPR consecutive y, the 8 warps of a CTA cover 8 consecutive z, so most
-// +-y / +-z operand words are L1 hits.
+// +-y / +-z operand words are L1 hits and every word leaves HBM once per half-sweep (profiles/: DRAM bytes per launch
+// = 9N/16).  The kernel is bound by integer issue (Philox: 18 IMAD.WIDE + 19 LOP3 per 4 sites), so it is laid out to
+// execute as few other instructions as possible: the 12 operand vectors are loaded first, the field sums of all W
+// words are reduced to three bit planes each (22 logic ops per 32 sites), and only then the random numbers are drawn.
 // ---------------------------------------------------------------------------------------------------
 template <int W> struct WordVec;
 template <> struct WordVec<1> { typedef uint32_t type; };
@@ -64,11 +67,18 @@ __device__ __forceinline__ void load_words(const uint32_t *__restrict__ p, size_
     for (int k = 0; k < W; ++k) out[k] = pv[k];
 }
 
+struct SiteRng {  // per-launch PRNG constants of the site-packed kernel (one sample)
+    PhiloxCommonConst pc;
+    PhiloxSampleConst ps;
+    uint64_t seed;  // MINSTD
+    uint32_t A2;    // MINSTD: 2 * (16807^(n+1) mod M) for the sweep n = t>>1 of this launch
+};
+
 constexpr int SWEEP_THREADS = 256;
 
 template <int RNG, int W>
 __global__ void __launch_bounds__(SWEEP_THREADS)
-half_sweep_site_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng)
+half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng)
 {
     const int L = a.L;
     const int wpr = L >> 6;                 // words per half-row
@@ -82,73 +92,66 @@ half_sweep_site_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng)
 
     const int yp = (y + 1) & (L - 1), ym = (y - 1) & (L - 1);
     const int zp = (z + 1) & (L - 1), zm = (z - 1) & (L - 1);
-    const size_t row = (size_t)wpr * ((size_t)y + (size_t)L * z) + k0;
-    const size_t row_yp = (size_t)wpr * ((size_t)yp + (size_t)L * z) + k0;
-    const size_t row_ym = (size_t)wpr * ((size_t)ym + (size_t)L * z) + k0;
-    const size_t row_zp = (size_t)wpr * ((size_t)y + (size_t)L * zp) + k0;
-    const size_t row_zm = (size_t)wpr * ((size_t)y + (size_t)L * zm) + k0;
+    const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;   // < 2^27 words for L <= 2048
+    const uint32_t row_yp = (uint32_t)wpr * ((uint32_t)yp + (uint32_t)L * z) + k0;
+    const uint32_t row_ym = (uint32_t)wpr * ((uint32_t)ym + (uint32_t)L * z) + k0;
+    const uint32_t row_zp = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zp) + k0;
+    const uint32_t row_zm = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zm) + k0;
 
-    uint32_t s[W], o[W], oyp[W], oym[W], ozp[W], ozm[W];
-    uint32_t jxa[W], jya[W], jza[W], jxo[W], jyo[W], jzo[W];
-    load_words<W>(a.S_act, row, s);
-    load_words<W>(a.S_oth, row, o);
-    load_words<W>(a.S_oth, row_yp, oyp);
-    load_words<W>(a.S_oth, row_ym, oym);
-    load_words<W>(a.S_oth, row_zp, ozp);
-    load_words<W>(a.S_oth, row_zm, ozm);
-    load_words<W>(a.J_act[0], row, jxa);
-    load_words<W>(a.J_act[1], row, jya);
-    load_words<W>(a.J_act[2], row, jza);
-    load_words<W>(a.J_oth[0], row, jxo);
-    load_words<W>(a.J_oth[1], row_ym, jyo);
-    load_words<W>(a.J_oth[2], row_zm, jzo);
-
-    // x-neighbours (row a3).  xodd = 0: +x is bit m of the other colour, -x is bit m-1, and the bond (i-x, i) is owned
-    // by that neighbour, so the word shifted up by one bit is Y = jxo ^ o.  xodd = 1: -x is bit m (with jxo), +x is
-    // bit m+1, so the word shifted down by one bit is Y = o.  The bit entering at the word boundary comes from the
-    // previous / next word of the half-row (periodic).
+    uint32_t s[W], sum2[W], sum1[W], sum0[W];
     const int xodd = (y + z + a.colour) & 1;
-    uint32_t Y[W];
+    {
+        uint32_t o[W], oyp[W], oym[W], ozp[W], ozm[W];
+        uint32_t jxa[W], jya[W], jza[W], jxo[W], jyo[W], jzo[W];
+        load_words<W>(a.S_act, row, s);
+        load_words<W>(a.S_oth, row, o);
+        load_words<W>(a.J_oth[0], row, jxo);
+        load_words<W>(a.J_act[0], row, jxa);
+        load_words<W>(a.S_oth, row_yp, oyp);
+        load_words<W>(a.S_oth, row_ym, oym);
+        load_words<W>(a.S_oth, row_zp, ozp);
+        load_words<W>(a.S_oth, row_zm, ozm);
+        load_words<W>(a.J_act[1], row, jya);
+        load_words<W>(a.J_act[2], row, jza);
+        load_words<W>(a.J_oth[1], row_ym, jyo);
+        load_words<W>(a.J_oth[2], row_zm, jzo);
+
+        // x-neighbours (row a3).  An active site with bit m has x = 2m + xodd.  xodd = 0: its +x neighbour is bit m of
+        // the other colour's half-row and its -x neighbour bit m-1, whose coupling is owned by that neighbour, so the
+        // word B = jxo ^ o is shifted up by one bit.  xodd = 1: -x is bit m (word B unshifted) and +x is bit m+1, so
+        // the word o is shifted down by one bit.  Both are funnel shifts by xodd / 1 - xodd; the bit entering at the
+        // end of the thread's words comes from the neighbouring lane of the row (periodic).
+        uint32_t B[W];
 #pragma unroll
-    for (int k = 0; k < W; ++k) Y[k] = xodd ? o[k] : (jxo[k] ^ o[k]);
-    uint32_t edge = xodd ? Y[0] : Y[W - 1];
-    if (tpr > 1) {
-        const int src = (lane & ~(tpr - 1)) | ((lane_in_row + (xodd ? 1 : tpr - 1)) & (tpr - 1));
-        edge = __shfl_sync(0xFFFFFFFFu, edge, src);
+        for (int k = 0; k < W; ++k) B[k] = jxo[k] ^ o[k];
+        uint32_t edge = xodd ? o[0] : B[W - 1];
+        if (tpr > 1) {
+            const int src = (lane & ~(tpr - 1)) | ((lane_in_row + (xodd ? 1 : tpr - 1)) & (tpr - 1));
+            edge = __shfl_sync(0xFFFFFFFFu, edge, src);
+        }
+        const uint32_t sh_r = (uint32_t)xodd, sh_l = 1u - (uint32_t)xodd;
+#pragma unroll
+        for (int k = 0; k < W; ++k) {
+            const uint32_t o_next = (k + 1 < W) ? o[(k + 1) % W] : edge;
+            const uint32_t B_prev = (k > 0) ? B[(k + W - 1) % W] : edge;
+            const uint32_t J[6] = {jxa[k], 0u, jya[k], jyo[k], jza[k], jzo[k]};
+            const uint32_t nb[6] = {__funnelshift_r(o[k], o_next, sh_r), __funnelshift_l(B_prev, B[k], sh_l), oyp[k], oym[k], ozp[k],
+                                    ozm[k]};
+            satisfied_bond_count(s[k], J, nb, sum2[k], sum1[k], sum0[k]);
+        }
     }
 
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
-
 #pragma unroll
     for (int k = 0; k < W; ++k) {
-        uint32_t ysh;
-        if (xodd) {
-            const uint32_t nxt = (k + 1 < W) ? Y[(k + 1) % W] : edge;
-            ysh = __funnelshift_r(Y[k], nxt, 1);
-        } else {
-            const uint32_t prv = (k > 0) ? Y[(k + W - 1) % W] : edge;
-            ysh = __funnelshift_l(prv, Y[k], 1);
-        }
-        uint32_t u[6];
-        u[0] = jxa[k] ^ (xodd ? ysh : o[k]);         // +x
-        u[1] = xodd ? (jxo[k] ^ o[k]) : ysh;         // -x
-        u[2] = jya[k] ^ oyp[k];                      // +y
-        u[3] = jyo[k] ^ oym[k];                      // -y
-        u[4] = jza[k] ^ ozp[k];                      // +z
-        u[5] = jzo[k] ^ ozm[k];                      // -z
-        uint32_t sum2, sum1, sum0;
-        satisfied_bond_count(s[k], u, sum2, sum1, sum0);
-
-        const uint32_t word_index = (uint32_t)(row + k);
         uint32_t c4, c8, c12;
         if (RNG == 0) {
-            cond_masks_site_packed_philox(rng.pc, rng.ps[0], word_index, a.T, c4, c8, c12);
+            cond_masks_site_packed_philox(rng.pc, rng.ps, row + (uint32_t)k, a.T, c4, c8, c12);
         } else {
             const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
-            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A, a.T, c4, c8,
-                                          c12);
+            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
         }
-        s[k] ^= flip_mask(sum2, sum1, sum0, c4, c8, c12);
+        s[k] ^= flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
     }
 
     typedef typename WordVec<W>::type V;
@@ -251,14 +254,14 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
         const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
         const uint64_t jn[6] = {colour_rank(L, xp, y, z), colour_rank(L, xm, y, z), colour_rank(L, x, yp, z),
                                 colour_rank(L, x, ym, z), colour_rank(L, x, y, zp), colour_rank(L, x, y, zm)};
-        uint32_t u[6];
+        uint32_t Jw[6], nb[6];
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
-            const uint32_t Jw = (d & 1) ? __ldg(a.J_oth[d >> 1] + jn[d]) : __ldg(a.J_act[d >> 1] + j);
-            u[d] = Jw ^ __ldg(a.S_oth + jn[d]);
+            Jw[d] = (d & 1) ? __ldg(a.J_oth[d >> 1] + jn[d]) : __ldg(a.J_act[d >> 1] + j);
+            nb[d] = __ldg(a.S_oth + jn[d]);
         }
         s[w] = a.S_act[j];
-        satisfied_bond_count(s[w], u, sum2[w], sum1[w], sum0[w]);
+        satisfied_bond_count(s[w], Jw, nb, sum2[w], sum1[w], sum0[w]);
         site[w] = (uint64_t)x + (uint64_t)L * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
     }
     uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};

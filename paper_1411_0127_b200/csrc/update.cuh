@@ -10,23 +10,20 @@ namespace isingk {
 // Acceptance thresholds as the kernels use them ("EXP4, EXP8, EXP12"; R4-R6).
 // Philox: accept dE iff R < T[dE] with T in [0, 2^32]; T = 2^32 does not fit a 32-bit compare, so the table holds
 // min(T, 2^32-1) plus an all-ones "always" mask for T = 2^32 (beta = 0).  MINSTD: T in [0, 2^31-1], plain compare.
-// For dE = 4, the test every site needs, the table also holds k4 = (2^32 - T4) mod 2^32: the 33-bit sum R + k4 carries
-// into bit 32 exactly when R >= T4 (for T4 = 2^32 it never does; for T4 = 0 the carry is lost, hence `never4`).
 struct Thresholds {
     uint32_t t4, t8, t12;
     uint32_t always4, always8, always12;  // 0 or 0xFFFFFFFF
-    uint32_t k4;
-    uint32_t never4;  // 0xFFFFFFFF iff T4 = 0 (beta = infinity)
 };
 
 // Per-bit number n of SATISFIED bonds among the six of each site (R2), as three bit planes (Eq. 12-13,
-// PAPER.md:258-271).  u_k = J_k ^ s_k is the neighbour part of the bond bit of Eq. 11;
-// J ^ s_i ^ s_k = 1 marks an unsatisfied bond under the encoding of Eq. 10, so a_k = ~(u_k ^ s) counts satisfied ones.
-// Two full adders, a half adder and a full adder: 8 three-input logic ops on top of the 6 bond XORs.
-ISING_HD void satisfied_bond_count(uint32_t s, const uint32_t u[6], uint32_t &sum2, uint32_t &sum1, uint32_t &sum0)
+// PAPER.md:258-271).  b_k = J_k ^ s_k ^ s is the bond bit of Eq. 11; under the encoding of Eq. 10 it
+// marks an UNSATISFIED bond, so a_k = ~b_k is summed.  Two full adders, a half adder and a full adder.  Written with
+// three-input functions throughout so that every line is one LOP3: 6 bond bits + 8 adder ops.
+ISING_HD void satisfied_bond_count(uint32_t s, const uint32_t J[6], const uint32_t nb[6], uint32_t &sum2, uint32_t &sum1,
+                                   uint32_t &sum0)
 {
-    const uint32_t a0 = ~(u[0] ^ s), a1 = ~(u[1] ^ s), a2 = ~(u[2] ^ s);
-    const uint32_t a3 = ~(u[3] ^ s), a4 = ~(u[4] ^ s), a5 = ~(u[5] ^ s);
+    const uint32_t a0 = ~(J[0] ^ nb[0] ^ s), a1 = ~(J[1] ^ nb[1] ^ s), a2 = ~(J[2] ^ nb[2] ^ s);
+    const uint32_t a3 = ~(J[3] ^ nb[3] ^ s), a4 = ~(J[4] ^ nb[4] ^ s), a5 = ~(J[5] ^ nb[5] ^ s);
     const uint32_t sA = a0 ^ a1 ^ a2, cA = (a0 & a1) | (a2 & (a0 | a1));
     const uint32_t sB = a3 ^ a4 ^ a5, cB = (a3 & a4) | (a5 & (a3 | a4));
     sum0 = sA ^ sB;
@@ -43,83 +40,87 @@ ISING_HD uint32_t flip_mask(uint32_t sum2, uint32_t sum1, uint32_t sum0, uint32_
     return cond12 | ~sum2 | (sum2 & (sum2 ^ sum1) & (cond8 | (cond4 & ~sum0)));
 }
 
-// 2*acc + (R >= T4): shifts the next "not accepted at dE = 4" bit into the accumulator.  On the device this is a carry
-// chain of two instructions: IADD3 (R + k4, carry out = R >= T4) and an add-with-carry acc + acc + C, which ptxas is
-// free to issue as IMAD.X on the FMA pipe, off the ALU pipe that the Philox XORs load.
-ISING_HD uint32_t shift_in_ge(uint32_t acc, uint32_t R, const Thresholds &T)
+// acc |= bit where R < T: one compare and one predicated OR, both on the integer ALU.
+ISING_HD void or_if_lt(uint32_t &acc, uint32_t R, uint32_t T, uint32_t bit)
 {
 #ifdef __CUDA_ARCH__
-    uint32_t out;
-    asm("{ .reg .u32 t; add.cc.u32 t, %1, %2; addc.u32 %0, %3, %3; }" : "=r"(out) : "r"(R), "r"(T.k4), "r"(acc));
-    return out;
+    asm("{ .reg .pred p; setp.lt.u32 p, %1, %2; @p or.b32 %0, %0, %3; }" : "+r"(acc) : "r"(R), "r"(T), "r"(bit));
 #else
-    const uint64_t t = (uint64_t)R + T.k4;
-    return 2u * acc + (uint32_t)(t >> 32);
+    if (R < T) acc |= bit;
 #endif
 }
 
-// The acceptance bits of four draws (sites bit0+3 .. bit0, in this order, so that shifting left leaves site b at bit b
-// once all 32 sites of a word have been shifted in from the top bit down).  nc4 collects R >= T4 (the complement of
-// cond4).  R < T8 happens for < 0.1 % of the draws at the temperatures of interest, so cond8 / cond12 are filled in a
-// rarely taken branch guarded by the minimum of the four draws.
-ISING_HD void accumulate_cond(const uint32_t R[4], int bit0, const Thresholds &T, uint32_t &nc4, uint32_t &c8, uint32_t &c12)
+ISING_HD uint32_t min_u32(uint32_t a, uint32_t b) { return a < b ? a : b; }
+
+// Acceptance bits of NR draws for the sites bit0 .. bit0+NR-1 of a word.  cond4 is needed for every draw.  R < T8
+// happens for < 0.1 % of the draws at the temperatures of interest, so cond8 / cond12 are filled in a rarely taken,
+// warp-uniform branch guarded by the minimum of the draws (one VIMNMX3 per two draws).
+template <int NR>
+ISING_HD void accumulate_cond(const uint32_t *R, int bit0, const Thresholds &T, uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
+    uint32_t mn = 0xFFFFFFFFu;
 #pragma unroll
-    for (int w = 3; w >= 0; --w) nc4 = shift_in_ge(nc4, R[w], T);
-    uint32_t mn = R[0] < R[1] ? R[0] : R[1];
-    const uint32_t mn2 = R[2] < R[3] ? R[2] : R[3];
-    mn = mn < mn2 ? mn : mn2;
+    for (int w = 0; w < NR; ++w) {
+        or_if_lt(c4, R[w], T.t4, 1u << (bit0 + w));
+        mn = min_u32(mn, R[w]);
+    }
 #ifdef __CUDA_ARCH__
     if (__any_sync(0xFFFFFFFFu, mn < T.t8)) {
 #else
     if (mn < T.t8) {
 #endif
 #pragma unroll
-        for (int w = 0; w < 4; ++w) {
-            c8 |= (R[w] < T.t8 ? 1u : 0u) << (bit0 + w);
-            c12 |= (R[w] < T.t12 ? 1u : 0u) << (bit0 + w);
+        for (int w = 0; w < NR; ++w) or_if_lt(c8, R[w], T.t8, 1u << (bit0 + w));
+#ifdef __CUDA_ARCH__
+        if (__any_sync(0xFFFFFFFFu, mn < T.t12)) {
+#else
+        if (mn < T.t12) {
+#endif
+#pragma unroll
+            for (int w = 0; w < NR; ++w) or_if_lt(c12, R[w], T.t12, 1u << (bit0 + w));
         }
     }
 }
 
-ISING_HD void finish_cond(const Thresholds &T, uint32_t nc4, uint32_t &c4, uint32_t &c8, uint32_t &c12)
+ISING_HD void finish_cond(const Thresholds &T, uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
-    c4 = ~(nc4 | T.never4);
+    c4 |= T.always4;
     c8 |= T.always8;
     c12 |= T.always12;
 }
 
 // Site-packed word (bits = 32 consecutive sites of one colour of one lattice): colour rank of bit b is
 // j = 32*word_index + b, so Philox call q = 0..7 has counter g = 8*word_index + q and serves bits 4q..4q+3 (R9).
+// Two calls are generated together: four independent multiply chains hide the IMAD.WIDE latency at any occupancy.
 ISING_HD void cond_masks_site_packed_philox(const PhiloxCommonConst &cc, const PhiloxSampleConst &sc, uint32_t word_index,
                                             const Thresholds &T, uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
-    uint32_t nc4 = 0;
-    c8 = 0; c12 = 0;
+    c4 = 0; c8 = 0; c12 = 0;
+    const uint32_t g0 = 8u * word_index;
 #pragma unroll
-    for (int q = 7; q >= 0; --q) {
-        uint32_t R[4];
-        philox_folded(cc, sc, 8u * word_index + (uint32_t)q, R);
-        accumulate_cond(R, 4 * q, T, nc4, c8, c12);
+    for (int q = 0; q < 8; q += 2) {
+        uint32_t R[8];
+        philox_folded(cc, sc, g0 + (uint32_t)q, R);
+        philox_folded(cc, sc, g0 + (uint32_t)q + 1u, R + 4);
+        accumulate_cond<8>(R, 4 * q, T, c4, c8, c12);
     }
-    finish_cond(T, nc4, c4, c8, c12);
+    finish_cond(T, c4, c8, c12);
 }
 
 // MINSTD, site-packed word: the stream id of bit b is q_b = site0 + b*site_stride (canonical site index, sample 0),
 // i.e. the SplitMix64 Weyl state advances by site_stride*GAMMA per bit.  `weyl0` = seed + (site0+1)*GAMMA.
-ISING_HD void cond_masks_site_packed_minstd(uint64_t weyl0, uint64_t weyl_step, uint32_t A, const Thresholds &T,
+ISING_HD void cond_masks_site_packed_minstd(uint64_t weyl0, uint64_t weyl_step, uint32_t A2, const Thresholds &T,
                                             uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
-    uint32_t nc4 = 0;
-    c8 = 0; c12 = 0;
+    c4 = 0; c8 = 0; c12 = 0;
 #pragma unroll
-    for (int q = 7; q >= 0; --q) {
+    for (int q = 0; q < 8; ++q) {
         uint32_t R[4];
 #pragma unroll
-        for (int w = 0; w < 4; ++w) R[w] = minstd_mulmod(A, minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + w) * weyl_step));
-        accumulate_cond(R, 4 * q, T, nc4, c8, c12);
+        for (int w = 0; w < 4; ++w) R[w] = minstd_mulmod2(A2, minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + w) * weyl_step));
+        accumulate_cond<4>(R, 4 * q, T, c4, c8, c12);
     }
-    finish_cond(T, nc4, c4, c8, c12);
+    finish_cond(T, c4, c8, c12);
 }
 
 }  // namespace isingk
