@@ -28,15 +28,15 @@ METRIC = "ps_per_spin_flip_attempt"
 UNIT = "ps/flip"
 BETA = 1.0 / 1.1
 
-# Algorithmic work of one flip attempt: integer instructions the definition needs at minimum.
-#   Philox4x32-10 with the launch-constant part folded: 18 wide multiplies + 19 three-input XORs per 4 sites = 9.25
-#   acceptance: one compare + one mask insert per site                                                    = 2
-#   field: 6 bond XORs + 8 adder ops + 4 mask ops + 2 x-alignment ops per 32-site word                    = 0.625
-ALG_INSTR_PER_FLIP = {0: 37 / 4 + 2 + 20 / 32}
-#   MINSTD stateless: SplitMix64 finaliser on a 64-bit Weyl state (2 add, 2x4 xor-shift, 2x3 multiply) + s0 (2) +
-#   mulmod (6) + compare/insert (2) per site                                                              = 26
-ALG_INSTR_PER_FLIP[1] = 26 + 20 / 32
+# Algorithmic integer work of one flip attempt on the binding pipe.
+#   Philox: fma pipe.  18 wide multiplies per call of 4 sites, IMAD.WIDE = 2 passes of the 32-bit multiplier -> 9.0 slots
+#   MINSTD (stateless SplitMix64 seed + multiply-mod): alu pipe.  16 per site + 22/32 field logic
+ALG_SLOTS_PER_FLIP = {0: 18 * 2 / 4, 1: 16 + 22 / 32}
+BINDING_PIPE = {0: "fma (IMAD.WIDE)", 1: "alu"}
 ALG_BYTES_PER_FLIP = 9 / 8  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
+# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch at L=1024 from the ncu --set full capture in
+# profiles/r1b_restructured_kernel.md (algorithmic: 9N/16 = 603,979,776 B)
+NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 57.73e6, 1: 537.12e6 + 57.60e6}
 
 
 def measured_peaks():
@@ -145,7 +145,7 @@ def main():
     import numpy as np
     import torch
 
-    from paper_1411_0127_b200 import MINSTD, PHILOX, Ising, synth
+    from paper_1411_0127_b200 import MINSTD, PHILOX, Ising, replicas, synth
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -165,17 +165,14 @@ def main():
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t[0])
+        return replicas.max_over_ranks(x, dist, "cuda")
 
     L, nsw = args.L, args.sweeps
     N = L**3
     # every rank simulates its own disorder sample (replicas): seeds offset by rank
-    spins = synth.make_spins(L, 1, 2 + 1000 * rank)
-    J = synth.make_couplings(L, 1, 1 + 1000 * rank)
+    s_seed, j_seed = replicas.replica_seeds(rank)
+    spins = synth.make_spins(L, 1, s_seed)
+    J = synth.make_couplings(L, 1, j_seed)
     h_spins = torch.from_numpy(spins.view(np.int32)).pin_memory()
     h_J = torch.from_numpy(J.view(np.int32)).pin_memory()
     h_out = torch.empty_like(h_spins).pin_memory()
@@ -249,18 +246,21 @@ def main():
     K = args.steps
 
     def summarize(res, rng_mode):
-        ps = 1e9 * res["total_ms"] / (K * flips_per_step)
+        ps = replicas.ps_per_flip(res["total_ms"], K, world, nsw, L)
         half_sweep_ms = res["sweep_ms"] / (K * 2 * nsw)            # average launch duration of the dominant kernel
         flips_per_launch = N / 2
-        inst_rate = ALG_INSTR_PER_FLIP[rng_mode] * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12  # T thread-instr/s
-        peak = 148 * 4 * 32 * sm_max_mhz * 1e6 / 1e12               # 148 SMs x 4 schedulers x 32 lanes x max clock
+        slot_rate = ALG_SLOTS_PER_FLIP[rng_mode] * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12  # T slots/s
+        peak = 148 * 4 * 16 * sm_max_mhz * 1e6 / 1e12               # one pipe: 148 SMs x 4 SMSPs x 16 lanes x max clock
         hbm = ALG_BYTES_PER_FLIP * flips_per_launch / (half_sweep_ms * 1e-3) / 1e9
         return ps, {
-            "bound": "alu", "achieved": inst_rate, "peak": peak, "unit": "Tinst/s", "frac": inst_rate / peak, "traffic": None,
+            "bound": "alu", "achieved": slot_rate, "peak": peak, "unit": "Tinst/s", "frac": slot_rate / peak,
+            "traffic": NCU_TRAFFIC_BYTES_L1024[rng_mode] if L == 1024 else None,
             "kernel": "half_sweep_site_packed", "kernel_ms": half_sweep_ms, "kernel_ps_per_flip": 1e9 * half_sweep_ms / flips_per_launch,
-            "alg_instr_per_flip": ALG_INSTR_PER_FLIP[rng_mode], "peak_source": f"148 SM x 4 x 32 lanes x {sm_max_mhz:.0f} MHz ({peaks_src} max clock)",
+            "binding_pipe": BINDING_PIPE[rng_mode], "alg_slots_per_flip": ALG_SLOTS_PER_FLIP[rng_mode],
+            "roofline_ps_per_flip": 1e12 * ALG_SLOTS_PER_FLIP[rng_mode] / (peak * 1e12),
+            "peak_source": f"guide unit counts: 148 SM x 4 SMSP x 16 lanes (rt_SMSP=2) x {sm_max_mhz:.0f} MHz ({peaks_src} max clock), per pipe",
             "hbm": {"achieved": hbm, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm / hbm_gbs, "alg_bytes_per_flip": ALG_BYTES_PER_FLIP,
-                    "peak_source": peaks_src},
+                    "alg_bytes_per_launch": ALG_BYTES_PER_FLIP * flips_per_launch, "peak_source": peaks_src + " (burst copy)"},
         }
 
     ps, roof = summarize(philox, 0)
