@@ -55,10 +55,12 @@ extern "C" {
 
 typedef struct ising ising_t; /* opaque */
 
-/* Size in bytes of the device workspace ising_create needs for (L, nsamples): the internal spin and
+/* Size in bytes of the device workspace ising_create needs for (L, nsamples, rng_mode): the internal spin and
  * coupling arrays (8 bit arrays per lattice), a canonical staging area used by
- * ising_run_host, and the int64 accumulators of the measurement kernel.  rng_mode does not change the size
- * (no PRNG state is stored: both generators are evaluated statelessly, R9/R12). */
+ * ising_run_host, the int64 accumulators of the measurement kernel and, in MINSTD mode with nsamples = 1 and
+ * L = 64*2^k, a table of the per-site seed states s0 (4 bytes per site, R11).  No PRNG *state* is stored: both
+ * generators are evaluated statelessly from (seed, sample, site, t) (R9, R12); the table only caches the
+ * time-independent SplitMix64 seeding of the MINSTD streams and is filled by the first sweep call. */
 int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out);
 
 /* Create a handle.  d_workspace: device memory, >= ising_workspace_bytes, 256-byte aligned.  The lattice
@@ -109,9 +111,10 @@ uint64_t ising_fnv1a64_host(const void *h_data, size_t nbytes);
 int ising_get_t(const ising_t *h, uint64_t *t);
 int ising_set_t(ising_t *h, uint64_t t);
 
-/* Select the half-sweep kernel: 0 = automatic (the word-parallel kernel where the layout allows it),
- * 1 = force the generic one-site-at-a-time kernel (any even L; used by the tests to show that results do
- * not depend on layout or thread mapping). */
+/* Select the half-sweep kernel: 0 = automatic (the word-parallel kernel where the layout allows it, with the
+ * cached seed table in MINSTD mode), 1 = force the generic one-site-at-a-time kernel (any even L), 2 = the
+ * word-parallel kernel without the seed table (MINSTD seeds recomputed per draw).  All give the same bits;
+ * the tests use this to show that results do not depend on layout, thread mapping or caching. */
 int ising_set_kernel(ising_t *h, int which);
 
 /* Number of kernels this handle has launched so far. */

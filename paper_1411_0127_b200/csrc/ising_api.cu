@@ -28,6 +28,7 @@ struct Geometry {
     size_t arrays_total_words;  // 8 arrays per lattice / batch
     size_t staging_words;       // canonical spins + couplings of all samples
     size_t acc_bytes;
+    size_t s0_words;            // cached MINSTD seed states: 32 words per word of each colour array (fast layout only)
     bool fast;                  // half-rows are whole words and L = 64*2^k
 };
 
@@ -47,6 +48,7 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
     g->acc_bytes = round_up((size_t)nsamples * 4 * sizeof(unsigned long long), 256);  // popcounts + E, M of ising_run_host
     g->fast = nsamples == 1 && L >= 64 && (L & (L - 1)) == 0;
+    g->s0_words = g->fast ? (size_t)g->N : 0;  // 2 colours x N/2 sites x 4 bytes
     return true;
 }
 
@@ -62,6 +64,8 @@ struct ising {
     uint32_t *ws;
     uint32_t *staging;
     unsigned long long *acc;
+    uint32_t *s0tab;   // MINSTD mode, fast layout: seed-state tables of the two colours (nullptr otherwise)
+    bool s0_ready;
 
     LatticeArrays arrays(int batch) const
     {
@@ -148,7 +152,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
             half_sweep_sample_packed<RNG><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, ngroups, g.N);
-        } else if (g.fast && h->kernel_choice == 0) {
+        } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = wpr >= 4 ? 4 : wpr;
             const int tpr = wpr / W;
@@ -158,7 +162,25 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             sr.ps = r.ps[0];
             sr.seed = r.seed;
             sr.A2 = 2u * r.A;
-            if (W == 4) half_sweep_site_packed<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+            sr.s0tab = nullptr;
+            const bool cached = RNG == 1 && h->kernel_choice == 0 && h->s0tab != nullptr;
+            if (cached) {
+                uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
+                if (!h->s0_ready) {  // once per handle: the seed states depend on (seed, site) only (R11)
+                    for (int cc = 0; cc < 2; ++cc) {
+                        if (W == 4) minstd_fill_s0<4><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                        else if (W == 2) minstd_fill_s0<2><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                        else minstd_fill_s0<1><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                    }
+                    const int rc = check_launch(h, 2);
+                    if (rc != ISING_OK) return rc;
+                    h->s0_ready = true;
+                }
+                sr.s0tab = tab[c];
+                if (W == 4) half_sweep_site_packed<2, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+                else if (W == 2) half_sweep_site_packed<2, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+                else half_sweep_site_packed<2, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+            } else if (W == 4) half_sweep_site_packed<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
             else if (W == 2) half_sweep_site_packed<RNG, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
             else half_sweep_site_packed<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
         } else {
@@ -193,7 +215,7 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         m.L = g.L;
         if (g.nsamples != 1) {
             energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
-        } else if (g.fast && h->kernel_choice == 0) {
+        } else if (g.fast && h->kernel_choice != 1) {
             const uint64_t nthreads = (uint64_t)(g.L >> 6) * g.L * g.L;  // words per colour; grid-stride above 148 x 16 CTAs
             const uint64_t nblocks = (nthreads + 255) / 256;
             energy_site_packed<<<(unsigned)(nblocks < 2368 ? nblocks : 2368), 256, 0, st>>>(m, h->acc);
@@ -218,6 +240,7 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
     if (!out || !make_geometry(L, nsamples, &g)) return ISING_EINVAL;
     if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD) return ISING_EINVAL;
     *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
+    if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
     return ISING_OK;
 }
 
@@ -239,6 +262,8 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->ws = (uint32_t *)d_workspace;
     h->staging = h->ws + h->g.arrays_total_words;
     h->acc = (unsigned long long *)(h->staging + h->g.staging_words);
+    h->s0tab = (rng_mode == ISING_RNG_MINSTD && h->g.s0_words) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
+    h->s0_ready = false;
     *out = h;
     return ISING_OK;
 }
@@ -424,7 +449,7 @@ int ising_set_t(ising_t *h, uint64_t t)
 
 int ising_set_kernel(ising_t *h, int which)
 {
-    if (!h || which < 0 || which > 1) return ISING_EINVAL;
+    if (!h || which < 0 || which > 2) return ISING_EINVAL;
     h->kernel_choice = which;
     return ISING_OK;
 }

@@ -72,7 +72,19 @@ struct SiteRng {  // per-launch PRNG constants of the site-packed kernel (one sa
     PhiloxSampleConst ps;
     uint64_t seed;  // MINSTD
     uint32_t A2;    // MINSTD: 2 * (16807^(n+1) mod M) for the sweep n = t>>1 of this launch
+    uint4 *s0tab;   // MINSTD with cached seeds (RNG = 2): seed states s0 of the active colour, see minstd_s0_index
 };
+
+// Cached MINSTD seed states (RNG = 2).  s0 = (SplitMix64(seed, site) >> 34) + 1 (R11) does not depend on time, so it
+// can be computed once per handle and streamed from HBM (4 B per site per sweep) instead of being recomputed (about
+// 17 integer instructions per site per sweep).  The table is laid out for the thread mapping of the kernel: the
+// 16-byte element (warp w of the grid, word k of the thread, bits 4q..4q+3, lane l) is at ((w*W + k)*8 + q)*32 + l,
+// so every load instruction of a warp reads 512 contiguous bytes.
+template <int W>
+__device__ __forceinline__ size_t minstd_s0_index(uint32_t warp_global, int k, int q, int lane)
+{
+    return (((size_t)warp_global * W + k) * 8 + q) * 32 + lane;
+}
 
 constexpr int SWEEP_THREADS = 256;
 
@@ -142,8 +154,40 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     }
 
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
+    if (RNG == 2) {
+        // seeds from the table, two groups of 16 sites in flight: while one half-word's draws are compared, the next
+        // half-word's four 16-byte loads are outstanding (about 2 KB per warp, enough to keep HBM busy)
+        const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
+        const uint4 *tab = rng.s0tab;
+        uint4 cur[4], nxt[4];
 #pragma unroll
-    for (int k = 0; k < W; ++k) {
+        for (int i = 0; i < 4; ++i) cur[i] = __ldcs(tab + minstd_s0_index<W>(warp_global, 0, i, lane));
+        uint32_t c4 = 0, c8 = 0, c12 = 0;
+#pragma unroll
+        for (int h = 0; h < 2 * W; ++h) {
+            const int k = h >> 1, half = h & 1;
+            if (h + 1 < 2 * W) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    nxt[i] = __ldcs(tab + minstd_s0_index<W>(warp_global, (h + 1) >> 1, 4 * ((h + 1) & 1) + i, lane));
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const uint32_t R[4] = {minstd_mulmod2(rng.A2, cur[i].x), minstd_mulmod2(rng.A2, cur[i].y),
+                                       minstd_mulmod2(rng.A2, cur[i].z), minstd_mulmod2(rng.A2, cur[i].w)};
+                accumulate_cond<4>(R, 16 * half + 4 * i, a.T, c4, c8, c12);
+            }
+            if (half) {
+                finish_cond(a.T, c4, c8, c12);
+                s[k] ^= flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
+                c4 = 0; c8 = 0; c12 = 0;
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < W && RNG != 2; ++k) {
         uint32_t c4, c8, c12;
         if (RNG == 0) {
             cond_masks_site_packed_philox(rng.pc, rng.ps, row + (uint32_t)k, a.T, c4, c8, c12);
@@ -160,6 +204,34 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
 #pragma unroll
     for (int k = 0; k < W; ++k) po[k] = s[k];
     *reinterpret_cast<V *>(a.S_act + row) = out;
+}
+
+// Fills the seed table of colour `colour` with the thread mapping of half_sweep_site_packed<2, W> (same grid).
+template <int W>
+__global__ void __launch_bounds__(SWEEP_THREADS) minstd_fill_s0(uint4 *tab, int L, int colour, uint64_t seed)
+{
+    const int wpr = L >> 6, tpr = wpr / W;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane_in_row = lane & (tpr - 1);
+    const int y = blockIdx.x * (32 / tpr) + lane / tpr;
+    const int z = blockIdx.y * (SWEEP_THREADS / 32) + warp;
+    const int k0 = lane_in_row * W;
+    const int xodd = (y + z + colour) & 1;
+    const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;
+    const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
+#pragma unroll 1
+    for (int k = 0; k < W; ++k) {
+        const uint64_t weyl0 = seed + (row_site0 + 64ull * (uint64_t)(k0 + k) + 1) * SPLITMIX_GAMMA;
+#pragma unroll 1
+        for (int q = 0; q < 8; ++q) {
+            uint4 v;
+            v.x = minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + 0) * (2 * SPLITMIX_GAMMA));
+            v.y = minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + 1) * (2 * SPLITMIX_GAMMA));
+            v.z = minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + 2) * (2 * SPLITMIX_GAMMA));
+            v.w = minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + 3) * (2 * SPLITMIX_GAMMA));
+            __stcs(tab + minstd_s0_index<W>(warp_global, k, q, lane), v);
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------

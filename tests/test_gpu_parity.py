@@ -232,6 +232,29 @@ def test_word_parallel_kernel_equals_generic_kernel(L, rng_mode):
     assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
 
 
+@pytest.mark.parametrize("L", [64, 128, 256, 512])
+def test_minstd_cached_seed_table_equals_recomputed_seeds(L):
+    """MINSTD: the default word-parallel kernel streams the seed states s0 from a table filled once per handle; kernel
+    choice 2 recomputes SplitMix64 per draw.  Same bits, also across separate calls (the table is reused) and after a
+    reload of the lattice (the table depends on (seed, site) only)."""
+    spins, J = synth.make_spins(L, 1, 41), synth.make_couplings(L, 1, 42)
+    a = Ising(L, 1, SEED, MINSTD)
+    b = Ising(L, 1, SEED, MINSTD)
+    b.ising_set_kernel(2)
+    for g in (a, b):
+        g.ising_load_state(dev(spins), dev(J))
+        g.ising_sweep(1 / 0.7, 2)
+        g.ising_sweep(1 / 0.7, 1)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert a.ising_kernel_launches() == b.ising_kernel_launches() + 2  # the two table fills
+    spins2 = synth.make_spins(L, 1, 43)
+    for g in (a, b):
+        g.ising_load_state(dev(spins2), dev(J))
+        g.ising_sweep(0.5, 2)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
+
+
 def test_run_host_equals_device_calls():
     L = 128
     spins, J = synth.make_spins(L, 1, 2), synth.make_couplings(L, 1, 1)
