@@ -30,13 +30,13 @@ BETA = 1.0 / 1.1
 
 # Algorithmic integer work of one flip attempt on the binding pipe.
 #   Philox: fma pipe.  18 wide multiplies per call of 4 sites, IMAD.WIDE = 2 passes of the 32-bit multiplier -> 9.0 slots
-#   MINSTD (stateless SplitMix64 seed + multiply-mod): alu pipe.  16 per site + 22/32 field logic
-ALG_SLOTS_PER_FLIP = {0: 18 * 2 / 4, 1: 16 + 22 / 32}
-BINDING_PIPE = {0: "fma (IMAD.WIDE)", 1: "alu"}
-ALG_BYTES_PER_FLIP = 9 / 8  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
+#   MINSTD with the cached seed table (the shipped variant): HBM-bound, 9/8 B of lattice + 4 B of seed state per flip
+ALG_SLOTS_PER_FLIP = {0: 18 * 2 / 4}
+BINDING_PIPE = {0: "fma (IMAD.WIDE)"}
+ALG_BYTES_PER_FLIP = {0: 9 / 8, 1: 9 / 8 + 4}  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch at L=1024 from the ncu --set full capture in
 # profiles/r1b_restructured_kernel.md (algorithmic: 9N/16 = 603,979,776 B)
-NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 57.73e6, 1: 537.12e6 + 57.60e6}
+NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 57.73e6, 1: None}
 
 
 def measured_peaks():
@@ -249,18 +249,21 @@ def main():
         ps = replicas.ps_per_flip(res["total_ms"], K, world, nsw, L)
         half_sweep_ms = res["sweep_ms"] / (K * 2 * nsw)            # average launch duration of the dominant kernel
         flips_per_launch = N / 2
+        hbm = ALG_BYTES_PER_FLIP[rng_mode] * flips_per_launch / (half_sweep_ms * 1e-3) / 1e9
+        hbm_obj = {"achieved": hbm, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm / hbm_gbs, "alg_bytes_per_flip": ALG_BYTES_PER_FLIP[rng_mode],
+                   "alg_bytes_per_launch": ALG_BYTES_PER_FLIP[rng_mode] * flips_per_launch, "peak_source": peaks_src + " (burst copy)"}
+        common = {"traffic": NCU_TRAFFIC_BYTES_L1024[rng_mode] if L == 1024 else None,
+                  "kernel": "half_sweep_site_packed", "kernel_ms": half_sweep_ms, "kernel_ps_per_flip": 1e9 * half_sweep_ms / flips_per_launch}
+        if rng_mode == 1:  # MINSTD with cached seed states: bound by HBM
+            return ps, {"bound": "hbm", **hbm_obj, **common}
         slot_rate = ALG_SLOTS_PER_FLIP[rng_mode] * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12  # T slots/s
         peak = 148 * 4 * 16 * sm_max_mhz * 1e6 / 1e12               # one pipe: 148 SMs x 4 SMSPs x 16 lanes x max clock
-        hbm = ALG_BYTES_PER_FLIP * flips_per_launch / (half_sweep_ms * 1e-3) / 1e9
         return ps, {
-            "bound": "alu", "achieved": slot_rate, "peak": peak, "unit": "Tinst/s", "frac": slot_rate / peak,
-            "traffic": NCU_TRAFFIC_BYTES_L1024[rng_mode] if L == 1024 else None,
-            "kernel": "half_sweep_site_packed", "kernel_ms": half_sweep_ms, "kernel_ps_per_flip": 1e9 * half_sweep_ms / flips_per_launch,
+            "bound": "alu", "achieved": slot_rate, "peak": peak, "unit": "Tinst/s", "frac": slot_rate / peak, **common,
             "binding_pipe": BINDING_PIPE[rng_mode], "alg_slots_per_flip": ALG_SLOTS_PER_FLIP[rng_mode],
             "roofline_ps_per_flip": 1e12 * ALG_SLOTS_PER_FLIP[rng_mode] / (peak * 1e12),
             "peak_source": f"guide unit counts: 148 SM x 4 SMSP x 16 lanes (rt_SMSP=2) x {sm_max_mhz:.0f} MHz ({peaks_src} max clock), per pipe",
-            "hbm": {"achieved": hbm, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm / hbm_gbs, "alg_bytes_per_flip": ALG_BYTES_PER_FLIP,
-                    "alg_bytes_per_launch": ALG_BYTES_PER_FLIP * flips_per_launch, "peak_source": peaks_src + " (burst copy)"},
+            "hbm": hbm_obj,
         }
 
     ps, roof = summarize(philox, 0)
