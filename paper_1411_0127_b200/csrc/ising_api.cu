@@ -30,6 +30,7 @@ struct Geometry {
     size_t acc_bytes;
     size_t s0_words;            // cached MINSTD seed states: 32 words per word of each colour array (fast layout only)
     bool fast;                  // half-rows are whole words and L = 64*2^k
+    int W;                      // words per thread of the word-parallel kernel (fast layout)
 };
 
 bool make_geometry(int L, int nsamples, Geometry *g)
@@ -49,6 +50,9 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->acc_bytes = round_up((size_t)nsamples * 4 * sizeof(unsigned long long), 256);  // popcounts + E, M of ising_run_host
     g->fast = nsamples == 1 && L >= 64 && (L & (L - 1)) == 0;
     g->s0_words = g->fast ? (size_t)g->N : 0;  // 2 colours x N/2 sites x 4 bytes
+    // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
+    // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
+    g->W = (g->fast && (L >> 6) >= 8) ? 4 : 1;
     return true;
 }
 
@@ -154,7 +158,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             half_sweep_sample_packed<RNG><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, ngroups, g.N);
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
-            const int W = wpr >= 4 ? 4 : wpr;
+            const int W = g.W;
             const int tpr = wpr / W;
             const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
             SiteRng sr;
