@@ -155,7 +155,11 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         fill_rng_launch(h, b, &r);
         if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
-            half_sweep_sample_packed<RNG><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, ngroups, g.N);
+            // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs
+            if (ngroups < 148u * 1024u)
+                half_sweep_sample_packed<RNG, 4><<<(unsigned)((ngroups + 31) / 32), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
+            else
+                half_sweep_sample_packed<RNG, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = g.W;

@@ -301,31 +301,40 @@ half_sweep_site_packed_generic(const SweepArgs a, const __grid_constant__ RngLau
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Sample-packed kernel (nsamples = 32 per batch), any even L >= 4.  One thread per Philox group g = 4 consecutive
-// same-colour sites j = 4g..4g+3; for each of the 32 samples (bits) one Philox call keyed by the sample gives the four
-// sites' draws (R9).  Neighbours are whole words, so no x-alignment is needed.
+// Sample-packed kernel (nsamples = 32 per batch), any even L >= 4.  A Philox group g = 4 consecutive same-colour sites
+// j = 4g..4g+3 needs one call per sample (bit), keyed by the sample (R9).  Neighbours are whole words, so no
+// x-alignment is needed.  A CTA has 4 warps.  PARTS = 1: one thread per group, all 32 samples (large lattices: index
+// arithmetic, 52 loads and the field logic are paid once per 32 calls).  PARTS = 4: lane = group, warp p = samples
+// 8p..8p+7 (warp-uniform Philox constants), each warp updates byte p of its groups' words; the loads of the four warps
+// coincide (L1 hits).  This spreads a small lattice (config 2: 32768 groups) over every SM.
 // ---------------------------------------------------------------------------------------------------
-template <int RNG>
+template <int RNG, int PARTS>
 __global__ void __launch_bounds__(128)
-half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint64_t n_groups, uint64_t N)
+half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_groups, uint64_t N)
 {
-    const uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_groups) return;
-    const int L = a.L, H = L >> 1;
+    constexpr int SPT = 32 / PARTS;  // samples per thread
+    const int part = PARTS == 1 ? 0 : (int)(threadIdx.x >> 5);  // warp-uniform
+    const uint32_t g_raw = PARTS == 1 ? blockIdx.x * 128u + threadIdx.x : blockIdx.x * 32u + (threadIdx.x & 31u);
+    const bool valid = g_raw < n_groups;
+    const uint32_t g = valid ? g_raw : n_groups - 1;  // keep the warp converged for the votes below
+    const uint32_t L = (uint32_t)a.L, H = L >> 1, HL = H * L, Hc = HL * L;  // Hc = N/2 < 2^32 for L <= 2048
     uint32_t s[4], sum2[4], sum1[4], sum0[4];
     uint64_t site[4];
+    const uint32_t j0 = 4u * g;
+    uint32_t m = j0 % H;
+    const uint32_t r0 = j0 / H;
+    uint32_t y = r0 % L, z = r0 / L;
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
-        const uint64_t j = 4 * g + w;
-        const int m = (int)(j % H);
-        const uint64_t r = j / H;
-        const int y = (int)(r % L), z = (int)(r / L);
-        const int x = 2 * m + ((y + z + a.colour) & 1);
-        const int xp = (x + 1 == L) ? 0 : x + 1, xm = (x == 0) ? L - 1 : x - 1;
-        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
-        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
-        const uint64_t jn[6] = {colour_rank(L, xp, y, z), colour_rank(L, xm, y, z), colour_rank(L, x, yp, z),
-                                colour_rank(L, x, ym, z), colour_rank(L, x, y, zp), colour_rank(L, x, y, zm)};
+        const uint32_t j = j0 + w;
+        const uint32_t xodd = (y + z + (uint32_t)a.colour) & 1u;
+        // colour ranks of the six neighbours (other colour): same row for +-x, rows y+-1 and planes z+-1 otherwise
+        const uint32_t rowbase = j - m;
+        const uint32_t m_other = xodd ? (m + 1 == H ? 0u : m + 1) : (m == 0 ? H - 1 : m - 1);
+        const uint32_t jxp = rowbase + (xodd ? m_other : m), jxm = rowbase + (xodd ? m : m_other);
+        const uint32_t jyp = (y + 1 == L) ? j - (HL - H) : j + H, jym = (y == 0) ? j + (HL - H) : j - H;
+        const uint32_t jzp = (z + 1 == L) ? j - (Hc - HL) : j + HL, jzm = (z == 0) ? j + (Hc - HL) : j - HL;
+        const uint32_t jn[6] = {jxp, jxm, jyp, jym, jzp, jzm};
         uint32_t Jw[6], nb[6];
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
@@ -334,38 +343,51 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
         }
         s[w] = a.S_act[j];
         satisfied_bond_count(s[w], Jw, nb, sum2[w], sum1[w], sum0[w]);
-        site[w] = (uint64_t)x + (uint64_t)L * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
+        site[w] = (uint64_t)(2u * m + xodd) + (uint64_t)L * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
+        if (++m == H) {  // next site of the colour: next row
+            m = 0;
+            if (++y == L) { y = 0; ++z; }
+        }
     }
     uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};
 #pragma unroll
-    for (int b = 0; b < 32; ++b) {
-        uint32_t R[4];
+    for (int i = 0; i < SPT; i += 2) {
+        const int b = SPT * part + i;
+        uint32_t R[8];
         if (RNG == 0) {
-            philox_folded(rng.pc, rng.ps[b], (uint32_t)g, R);
+            philox_folded(rng.pc, rng.ps[b], g, R);
+            philox_folded(rng.pc, rng.ps[b + 1], g, R + 4);
         } else {
-            const uint64_t qs = (uint64_t)(rng.sample_base + b) * N;
 #pragma unroll
-            for (int w = 0; w < 4; ++w)
-                R[w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(rng.seed + (qs + site[w] + 1) * SPLITMIX_GAMMA));
+            for (int e = 0; e < 2; ++e) {
+                const uint64_t qs = (uint64_t)(rng.sample_base + b + e) * N;
+#pragma unroll
+                for (int w = 0; w < 4; ++w)
+                    R[4 * e + w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(rng.seed + (qs + site[w] + 1) * SPLITMIX_GAMMA));
+            }
         }
+        uint32_t mn = 0xFFFFFFFFu;
 #pragma unroll
-        for (int w = 0; w < 4; ++w) c4[w] |= (R[w] < a.T.t4 ? 1u : 0u) << b;
-        uint32_t mn = R[0] < R[1] ? R[0] : R[1];
-        const uint32_t mn2 = R[2] < R[3] ? R[2] : R[3];
-        mn = mn < mn2 ? mn : mn2;
-        if (mn < a.T.t8) {
+        for (int e = 0; e < 8; ++e) {
+            or_if_lt(c4[e & 3], R[e], a.T.t4, 1u << (i + (e >> 2)));
+            mn = min_u32(mn, R[e]);
+        }
+        if (__any_sync(0xFFFFFFFFu, mn < a.T.t8)) {
 #pragma unroll
-            for (int w = 0; w < 4; ++w) {
-                c8[w] |= (R[w] < a.T.t8 ? 1u : 0u) << b;
-                c12[w] |= (R[w] < a.T.t12 ? 1u : 0u) << b;
+            for (int e = 0; e < 8; ++e) {
+                or_if_lt(c8[e & 3], R[e], a.T.t8, 1u << (i + (e >> 2)));
+                or_if_lt(c12[e & 3], R[e], a.T.t12, 1u << (i + (e >> 2)));
             }
         }
     }
+    if (!valid) return;
+    const int sh = SPT * part;
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
-        const uint32_t f = flip_mask(sum2[w], sum1[w], sum0[w], c4[w] | a.T.always4, c8[w] | a.T.always8,
+        const uint32_t f = flip_mask(sum2[w] >> sh, sum1[w] >> sh, sum0[w] >> sh, c4[w] | a.T.always4, c8[w] | a.T.always8,
                                      c12[w] | a.T.always12);
-        a.S_act[4 * g + w] = s[w] ^ f;
+        if (PARTS == 1) a.S_act[j0 + w] = s[w] ^ f;
+        else reinterpret_cast<unsigned char *>(a.S_act + j0 + w)[part] = (unsigned char)((s[w] >> sh) ^ f);  // little-endian
     }
 }
 
