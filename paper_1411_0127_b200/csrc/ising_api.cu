@@ -47,7 +47,8 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->array_words = round_up(raw, ALIGN_WORDS);
     g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
-    g->acc_bytes = round_up((size_t)nsamples * 4 * sizeof(unsigned long long), 256);  // popcounts + E, M of ising_run_host
+    // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs of the word-parallel energy kernel
+    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS) * sizeof(unsigned long long), 256);
     g->fast = nsamples == 1 && L >= 64 && (L & (L - 1)) == 0;
     g->s0_words = g->fast ? (size_t)g->N : 0;  // 2 colours x N/2 sites x 4 bytes
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
@@ -210,7 +211,9 @@ int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
 int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
 {
     const Geometry &g = h->g;
-    if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess)
+    unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;
+    bool use_slots = false;
+    if (cudaMemsetAsync(h->acc, 0, g.acc_bytes, st) != cudaSuccess)
         return ISING_ECUDA;
     const int nb = g.nsamples == 1 ? 1 : g.nbatches;
     for (int b = 0; b < nb; ++b) {
@@ -224,9 +227,11 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         if (g.nsamples != 1) {
             energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
         } else if (g.fast && h->kernel_choice != 1) {
-            const uint64_t nthreads = (uint64_t)(g.L >> 6) * g.L * g.L;  // words per colour; grid-stride above 148 x 16 CTAs
-            const uint64_t nblocks = (nthreads + 255) / 256;
-            energy_site_packed<<<(unsigned)(nblocks < 2368 ? nblocks : 2368), 256, 0, st>>>(m, h->acc);
+            const int tpr = (g.L >> 6) / g.W;
+            const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
+            if (g.W == 4) energy_site_packed<4><<<grid, SWEEP_THREADS, 0, st>>>(m, slots);
+            else energy_site_packed<1><<<grid, SWEEP_THREADS, 0, st>>>(m, slots);
+            use_slots = true;
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc, nw, g.Hc);
@@ -234,7 +239,7 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         const int rc = check_launch(h);
         if (rc != ISING_OK) return rc;
     }
-    finalize_energy<<<(g.nsamples + 127) / 128, 128, 0, st>>>(h->acc, g.nsamples, (long long)g.N, d_E, d_M);
+    finalize_energy<<<(g.nsamples + 127) / 128, 128, 0, st>>>(h->acc, g.nsamples, (long long)g.N, d_E, d_M, use_slots ? slots : nullptr);
     return check_launch(h);
 }
 
@@ -305,7 +310,8 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
                 s.out[1 + d][1] = A.J[d][1];
             }
             const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
-            split_colours_site_packed<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s);
+            if (g.W == 4) split_colours_site_packed<4><<<(unsigned)((n / 4 + 255) / 256), 256, 0, st>>>(s);
+            else split_colours_site_packed<1><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s);
             return check_launch(h);
         }
         const uint64_t nw = (g.Hc + 31) / 32;
@@ -343,7 +349,8 @@ int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
         const LatticeArrays A = h->arrays(0);
         if (g.fast) {
             const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
-            merge_colours_site_packed<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
+            if (g.W == 4) merge_colours_site_packed<4><<<(unsigned)((n / 4 + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
+            else merge_colours_site_packed<1><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
         } else {
             scatter_site_packed_generic<<<(unsigned)((W + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L, W, g.N);
         }

@@ -42,38 +42,57 @@ struct SplitArgs {
     int L;
 };
 
+template <int V>  // V internal words (2V canonical words) per thread, V <= L/64
 __global__ void __launch_bounds__(256) split_colours_site_packed(const SplitArgs a)
 {
+    typedef typename WordVec<V>::type Vec;
     const int L = a.L, wpr = L >> 6;
     const uint64_t n = (uint64_t)wpr * L * L;
-    const uint64_t widx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t widx = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * V;
     if (widx >= n) return;
-    const uint64_t r = widx / wpr;
-    const int p = (int)((r % L) + (r / L)) & 1;
+    const uint64_t r = widx / (unsigned)wpr;               // L is a power of two here: shifts
+    const int p = (int)((r & (L - 1)) + (r / (unsigned)L)) & 1;
     for (int q = 0; q < a.narrays; ++q) {
-        const uint2 v = *reinterpret_cast<const uint2 *>(a.canon[q] + 2 * widx);
-        const uint32_t even = compress_even_bits(v.x) | (compress_even_bits(v.y) << 16);
-        const uint32_t odd = compress_even_bits(v.x >> 1) | (compress_even_bits(v.y >> 1) << 16);
-        a.out[q][p][widx] = even;
-        a.out[q][1 - p][widx] = odd;
+        uint32_t c[2 * V], even[V], odd[V];
+        const Vec lo = __ldcs(reinterpret_cast<const Vec *>(a.canon[q] + 2 * widx));
+        const Vec hi = __ldcs(reinterpret_cast<const Vec *>(a.canon[q] + 2 * widx + V));
+#pragma unroll
+        for (int k = 0; k < V; ++k) {
+            c[k] = reinterpret_cast<const uint32_t *>(&lo)[k];
+            c[V + k] = reinterpret_cast<const uint32_t *>(&hi)[k];
+        }
+#pragma unroll
+        for (int k = 0; k < V; ++k) {
+            even[k] = compress_even_bits(c[2 * k]) | (compress_even_bits(c[2 * k + 1]) << 16);
+            odd[k] = compress_even_bits(c[2 * k] >> 1) | (compress_even_bits(c[2 * k + 1] >> 1) << 16);
+        }
+        *reinterpret_cast<Vec *>(a.out[q][p] + widx) = *reinterpret_cast<const Vec *>(even);
+        *reinterpret_cast<Vec *>(a.out[q][1 - p] + widx) = *reinterpret_cast<const Vec *>(odd);
     }
 }
 
+template <int V>
 __global__ void __launch_bounds__(256)
 merge_colours_site_packed(const uint32_t *__restrict__ S0, const uint32_t *__restrict__ S1, uint32_t *__restrict__ canon, int L)
 {
+    typedef typename WordVec<V>::type Vec;
     const int wpr = L >> 6;
     const uint64_t n = (uint64_t)wpr * L * L;
-    const uint64_t widx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t widx = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * V;
     if (widx >= n) return;
-    const uint64_t r = widx / wpr;
-    const int p = (int)((r % L) + (r / L)) & 1;
-    const uint32_t even = p ? S1[widx] : S0[widx];
-    const uint32_t odd = p ? S0[widx] : S1[widx];
-    uint2 v;
-    v.x = spread_to_even_bits(even) | (spread_to_even_bits(odd) << 1);
-    v.y = spread_to_even_bits(even >> 16) | (spread_to_even_bits(odd >> 16) << 1);
-    *reinterpret_cast<uint2 *>(canon + 2 * widx) = v;
+    const uint64_t r = widx / (unsigned)wpr;
+    const int p = (int)((r & (L - 1)) + (r / (unsigned)L)) & 1;
+    const Vec ve = *reinterpret_cast<const Vec *>((p ? S1 : S0) + widx);
+    const Vec vo = *reinterpret_cast<const Vec *>((p ? S0 : S1) + widx);
+    uint32_t out[2 * V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        const uint32_t even = reinterpret_cast<const uint32_t *>(&ve)[k], odd = reinterpret_cast<const uint32_t *>(&vo)[k];
+        out[2 * k] = spread_to_even_bits(even) | (spread_to_even_bits(odd) << 1);
+        out[2 * k + 1] = spread_to_even_bits(even >> 16) | (spread_to_even_bits(odd >> 16) << 1);
+    }
+    __stcs(reinterpret_cast<Vec *>(canon + 2 * widx), *reinterpret_cast<const Vec *>(out));
+    __stcs(reinterpret_cast<Vec *>(canon + 2 * widx + V), *reinterpret_cast<const Vec *>(out + V));
 }
 
 // Site-packed, any even L: one thread per internal word of one colour array, one bit at a time.

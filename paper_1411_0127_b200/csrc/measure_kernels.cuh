@@ -12,6 +12,10 @@
 
 namespace isingk {
 
+// The word-parallel site-packed kernel spreads its per-CTA atomics over ACC_SLOTS counter pairs (one address would
+// serialise 16384 atomics in L2 at L = 1024); finalize_energy adds them up.
+constexpr int ACC_SLOTS = 64;
+
 struct MeasureArgs {
     const uint32_t *S[2];
     const uint32_t *J[3][2];
@@ -47,37 +51,48 @@ __device__ __forceinline__ void block_accumulate2(unsigned long long a, unsigned
     }
 }
 
-// Site-packed, L = 64*2^k: a grid-stride loop over the words of both colours.  The +x neighbour of the colour-c site
-// with bit m is bit m (xodd = 0) or bit m+1 (xodd = 1) of the other colour's half-row; +y / +z neighbours are the same
-// bit one row up.  Every word is read once from HBM (the neighbour reads hit L1/L2): 512 MiB at L = 1024.
-__global__ void __launch_bounds__(256)
-energy_site_packed(const MeasureArgs a, unsigned long long *acc /* [0] = unsatisfied bonds, [1] = up spins */)
+// Site-packed, L = 64*2^k: the thread mapping of the half-sweep kernel (a thread owns W consecutive words of a half-row,
+// for both colours).  The +x neighbour of the colour-c site with bit m is bit m (xodd = 0) or bit m+1 (xodd = 1) of the
+// other colour's half-row (a funnel shift by xodd; the bit entering at the end of the thread's words comes from the
+// next lane of the row); +y / +z neighbours are the same bit one row up.  Every word is read once from HBM with 128-bit
+// loads (the neighbour reads hit L1/L2): 512 MiB at L = 1024.
+template <int W>
+__global__ void __launch_bounds__(SWEEP_THREADS)
+energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {unsatisfied bonds, up spins} */)
 {
-    const int L = a.L, wpr = L >> 6;
-    const uint64_t words_per_colour = (uint64_t)wpr * L * L;
-    unsigned long long unsat = 0, up = 0;
+    const int L = a.L, wpr = L >> 6, tpr = wpr / W;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane_in_row = lane & (tpr - 1);
+    const int y = blockIdx.x * (32 / tpr) + lane / tpr;
+    const int z = blockIdx.y * (SWEEP_THREADS / 32) + warp;
+    const int k0 = lane_in_row * W;
+    const int yp = (y + 1) & (L - 1), zp = (z + 1) & (L - 1);
+    const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;
+    const uint32_t row_yp = (uint32_t)wpr * ((uint32_t)yp + (uint32_t)L * z) + k0;
+    const uint32_t row_zp = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zp) + k0;
+    const int next_lane = (lane & ~(tpr - 1)) | ((lane_in_row + 1) & (tpr - 1));
+    unsigned int unsat = 0, up = 0;
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
-        const uint32_t *__restrict__ Sc = a.S[c], *__restrict__ So = a.S[1 - c];
-        const uint32_t *__restrict__ Jx = a.J[0][c], *__restrict__ Jy = a.J[1][c], *__restrict__ Jz = a.J[2][c];
-        for (uint64_t widx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; widx < words_per_colour;
-             widx += (uint64_t)gridDim.x * blockDim.x) {
-            const int k = (int)(widx % wpr);
-            const uint64_t r = widx / wpr;
-            const int y = (int)(r % L), z = (int)(r / L);
-            const int yp = (y + 1) & (L - 1), zp = (z + 1) & (L - 1);
-            const int xodd = (y + z + c) & 1;
-            const uint32_t s = Sc[widx];
-            const size_t rowbase = (size_t)wpr * r;
-            uint32_t nx = So[rowbase + k];
-            if (xodd) nx = __funnelshift_r(nx, So[rowbase + ((k + 1) % wpr)], 1);
-            const uint32_t ny = So[(size_t)wpr * ((size_t)yp + (size_t)L * z) + k];
-            const uint32_t nz = So[(size_t)wpr * ((size_t)y + (size_t)L * zp) + k];
-            unsat += __popc(Jx[widx] ^ s ^ nx) + __popc(Jy[widx] ^ s ^ ny) + __popc(Jz[widx] ^ s ^ nz);
-            up += __popc(s);
+        uint32_t s[W], o[W], oyp[W], ozp[W], jx[W], jy[W], jz[W];
+        load_words<W>(a.S[c], row, s);
+        load_words<W>(a.S[1 - c], row, o);
+        load_words<W>(a.S[1 - c], row_yp, oyp);
+        load_words<W>(a.S[1 - c], row_zp, ozp);
+        load_words<W>(a.J[0][c], row, jx);
+        load_words<W>(a.J[1][c], row, jy);
+        load_words<W>(a.J[2][c], row, jz);
+        const uint32_t xodd = (uint32_t)((y + z + c) & 1);
+        uint32_t edge = o[0];
+        if (tpr > 1) edge = __shfl_sync(0xFFFFFFFFu, edge, next_lane);
+#pragma unroll
+        for (int k = 0; k < W; ++k) {
+            const uint32_t nx = __funnelshift_r(o[k], (k + 1 < W) ? o[(k + 1) % W] : edge, xodd);
+            unsat += __popc(jx[k] ^ s[k] ^ nx) + __popc(jy[k] ^ s[k] ^ oyp[k]) + __popc(jz[k] ^ s[k] ^ ozp[k]);
+            up += __popc(s[k]);
         }
     }
-    block_accumulate2(unsat, up, acc);
+    block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
 }
 
 // Site-packed, any even L: one thread per word, one site at a time.
@@ -152,13 +167,17 @@ energy_sample_packed(const MeasureArgs a, unsigned long long *acc /* [32][2] */,
     }
 }
 
-// E = 2*unsat - 3N, M = 2*up - N  (R16), one thread per sample.
-__global__ void finalize_energy(const unsigned long long *acc, int nsamples, long long N, long long *E, long long *M)
+// E = 2*unsat - 3N, M = 2*up - N  (R16), one thread per sample.  slots: nullptr, or ACC_SLOTS counter pairs of sample 0.
+__global__ void finalize_energy(const unsigned long long *acc, int nsamples, long long N, long long *E, long long *M,
+                                const unsigned long long *slots)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= nsamples) return;
-    if (E) E[s] = 2 * (long long)acc[2 * s] - 3 * N;
-    if (M) M[s] = 2 * (long long)acc[2 * s + 1] - N;
+    unsigned long long unsat = acc[2 * s], up = acc[2 * s + 1];
+    if (slots && s == 0)
+        for (int k = 0; k < ACC_SLOTS; ++k) { unsat += slots[2 * k]; up += slots[2 * k + 1]; }
+    if (E) E[s] = 2 * (long long)unsat - 3 * N;
+    if (M) M[s] = 2 * (long long)up - N;
 }
 
 }  // namespace isingk
