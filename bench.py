@@ -107,7 +107,7 @@ def run_reference(args):
     """--impl reference: the CPU oracle is the reference arm of this tier (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    Ls, sweeps = 512, 2
+    Ls, sweeps = 512, 8
     times, cores = time_oracle(Ls, sweeps, 0, repeats=args.warmup + args.steps)
     times = times[args.warmup:]
     total = sum(times)
@@ -290,7 +290,7 @@ def main():
         if "e2e_ms" in minstd:
             line["minstd"]["e2e"] = 1e9 * minstd["e2e_ms"] / (K * flips_per_step)
     if world == 1 and not args.no_cpu_baseline:
-        Ls, sw = 512, 8
+        Ls, sw = 512, 64  # about 15 s on the 16 host cores of the GPU box
         times, cores = time_oracle(Ls, sw, 0)
         line["cpu_baseline"] = {"value": 1e12 * times[0] / (sw * Ls**3), "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"L={Ls} cube (1/8 of the sites of the L=1024 workload, same recipe, Philox), {sw} sweeps, {times[0]:.1f} s"}
