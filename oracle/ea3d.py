@@ -12,7 +12,7 @@ import numpy as np
 
 from . import build as _build
 
-PHILOX, MINSTD = 0, 1
+PHILOX, MINSTD, PHILOX_SHARED = 0, 1, 2  # PHILOX_SHARED: one draw per 32-sample word (R18)
 
 _lib = None
 

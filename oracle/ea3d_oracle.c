@@ -30,6 +30,10 @@
 
 #define ORACLE_RNG_PHILOX 0
 #define ORACLE_RNG_MINSTD 1
+/* The paper's own asynchronous multispin coding (Eq. 15): the 32 samples coded in
+ * one word share ONE random number per (site, half-sweep).  DESIGN.md R18: the shared draw of the samples 32b..32b+31
+ * (coded batch b) is the Philox draw of "sample" b, i.e. oracle_philox_draw(..., sample >> 5, ...). */
+#define ORACLE_RNG_PHILOX_SHARED 2
 
 /* ------------------------------------------------------------------------------------------ */
 /* Random number generators                                                                    */
@@ -120,12 +124,12 @@ uint32_t oracle_philox_draw(int L, uint64_t seed, int sample, int x, int y, int 
 int oracle_thresholds(double beta, int rng_mode, uint64_t T[3])
 {
     if (!(beta >= 0.0)) return -1;
-    if (rng_mode != ORACLE_RNG_PHILOX && rng_mode != ORACLE_RNG_MINSTD) return -1;
+    if (rng_mode != ORACLE_RNG_PHILOX && rng_mode != ORACLE_RNG_MINSTD && rng_mode != ORACLE_RNG_PHILOX_SHARED) return -1;
     for (int k = 0; k < 3; ++k) {
         double dE = 4.0 * (double)(k + 1);
         double x = beta * dE;
         double p = exp(-x);
-        double scaled = (rng_mode == ORACLE_RNG_PHILOX) ? ldexp(p, 32) : 2147483647.0 * p;
+        double scaled = (rng_mode != ORACLE_RNG_MINSTD) ? ldexp(p, 32) : 2147483647.0 * p;
         T[k] = (uint64_t)floor(scaled);
     }
     return 0;
@@ -237,6 +241,8 @@ int oracle_half_sweep(int L, int nsamples, int8_t *sigma, const int8_t *Jx, cons
                     uint64_t R;
                     if (rng_mode == ORACLE_RNG_PHILOX) {
                         R = oracle_philox_draw(L, seed, s, x, y, z, t);
+                    } else if (rng_mode == ORACLE_RNG_PHILOX_SHARED) {
+                        R = oracle_philox_draw(L, seed, s >> 5, x, y, z, t);
                     } else {
                         uint32_t *st = &minstd_state[(int64_t)s * N + i];
                         *st = oracle_minstd_step(*st);
@@ -287,6 +293,8 @@ int oracle_site_flips(int L, const int8_t *sigma, const int8_t *Jx, const int8_t
     uint64_t R;
     if (rng_mode == ORACLE_RNG_PHILOX)
         R = oracle_philox_draw(L, seed, sample, x, y, z, t);
+    else if (rng_mode == ORACLE_RNG_PHILOX_SHARED)
+        R = oracle_philox_draw(L, seed, sample >> 5, x, y, z, t);
     else
         R = oracle_minstd_draw(seed, (uint64_t)sample * (uint64_t)N + (uint64_t)site_index(L, x, y, z), t >> 1);
     if (dE_out) *dE_out = dE;
