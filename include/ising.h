@@ -53,6 +53,10 @@ extern "C" {
 #define ISING_RNG_MINSTD 1 /* MINSTD 16807 mod 2^31-1 (Eq. 7), one stream per site seeded by
                               SplitMix64 (R11), draw of sweep n = 16807^(n+1) * s0 mod (2^31-1) (R12) */
 
+#define ISING_RNG_PHILOX_SHARED 2 /* the paper's asynchronous multispin coding proper (Eq. 15): the 32
+                              samples of a word share ONE Philox draw per (site, half-sweep); nsamples = 32k only; the draw
+                              of the samples 32b..32b+31 is the ISING_RNG_PHILOX draw with the key's sample field = b (R18) */
+
 typedef struct ising ising_t; /* opaque */
 
 /* Size in bytes of the device workspace ising_create needs for (L, nsamples, rng_mode): the internal spin and

@@ -11,7 +11,7 @@ import ctypes as C
 
 from . import build as _build
 
-PHILOX, MINSTD = 0, 1
+PHILOX, MINSTD, PHILOX_SHARED = 0, 1, 2
 OK, EINVAL, ECUDA = 0, -1, -2
 
 EXPORTS = (

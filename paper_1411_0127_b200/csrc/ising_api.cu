@@ -96,12 +96,12 @@ int check_launch(ising_t *h, int n = 1)
 int compute_thresholds(double beta, int rng_mode, uint64_t out[3])
 {
     if (!(beta >= 0.0)) return ISING_EINVAL;
-    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD) return ISING_EINVAL;
+    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD && rng_mode != ISING_RNG_PHILOX_SHARED) return ISING_EINVAL;
     for (int k = 0; k < 3; ++k) {
         const double dE = 4.0 * (double)(k + 1);
         const double x = beta * dE;
         const double p = exp(-x);
-        const double scaled = rng_mode == ISING_RNG_PHILOX ? ldexp(p, 32) : 2147483647.0 * p;
+        const double scaled = rng_mode != ISING_RNG_MINSTD ? ldexp(p, 32) : 2147483647.0 * p;
         out[k] = (uint64_t)floor(scaled);
     }
     return ISING_OK;
@@ -132,6 +132,8 @@ void fill_rng_launch(const ising_t *h, int batch, RngLaunch *r)
     if (h->rng_mode == ISING_RNG_PHILOX) {
         const int ns = h->g.nsamples == 1 ? 1 : 32;
         for (int s = 0; s < ns; ++s) fold_philox(h->seed, sample_base + (uint32_t)s, h->t, &r->pc, &r->ps[s]);
+    } else if (h->rng_mode == ISING_RNG_PHILOX_SHARED) {
+        fold_philox(h->seed, (uint32_t)batch, h->t, &r->pc, &r->ps[0]);  // R18: the sample field of the key is the batch
     } else {
         r->A = minstd_power((h->t >> 1) + 1);
     }
@@ -154,7 +156,22 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         a.T = T;
         RngLaunch r;
         fill_rng_launch(h, b, &r);
-        if (g.nsamples != 1) {
+        if (RNG == 2) {
+            const uint64_t ngroups = g.Hc / 4;
+            if (g.L % 8 == 0 && h->kernel_choice != 1) {
+                SiteRng sr;
+                sr.pc = r.pc;
+                sr.ps = r.ps[0];
+                sr.seed = 0;
+                sr.A2 = 0;
+                sr.s0tab = nullptr;
+                const uint32_t gpr = (uint32_t)g.L / 8;
+                const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L);
+                half_sweep_shared_vec<<<grid, 128, 0, st>>>(a, sr, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr));
+            } else {
+                half_sweep_sample_packed<2, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
+            }
+        } else if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
             // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs
             if (ngroups < 148u * 1024u)
@@ -205,6 +222,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
 
 int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
 {
+    if (h->rng_mode == ISING_RNG_PHILOX_SHARED) return launch_half_sweep<2>(h, T, st);
     return h->rng_mode == ISING_RNG_PHILOX ? launch_half_sweep<0>(h, T, st) : launch_half_sweep<1>(h, T, st);
 }
 
@@ -251,7 +269,8 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
 {
     Geometry g;
     if (!out || !make_geometry(L, nsamples, &g)) return ISING_EINVAL;
-    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD) return ISING_EINVAL;
+    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD && rng_mode != ISING_RNG_PHILOX_SHARED) return ISING_EINVAL;
+    if (rng_mode == ISING_RNG_PHILOX_SHARED && nsamples % 32 != 0) return ISING_EINVAL;  // one draw per 32-sample word
     *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
     if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
     return ISING_OK;
@@ -474,7 +493,7 @@ uint64_t ising_kernel_launches(const ising_t *h) { return h ? h->launches : 0; }
 int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double beta, const uint32_t ops[13],
                                 uint64_t word_index, uint64_t site0, uint64_t site_stride, uint32_t *out)
 {
-    if (!ops || !out) return ISING_EINVAL;
+    if (!ops || !out || rng_mode == ISING_RNG_PHILOX_SHARED) return ISING_EINVAL;  // a site-packed word has no shared draw
     uint64_t T[3];
     if (compute_thresholds(beta, rng_mode, T) != ISING_OK) return ISING_EINVAL;
     const Thresholds kt = kernel_thresholds(T);

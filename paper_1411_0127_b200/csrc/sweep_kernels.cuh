@@ -88,6 +88,19 @@ __device__ __forceinline__ size_t minstd_s0_index(uint32_t warp_global, int k, i
 
 constexpr int SWEEP_THREADS = 256;
 
+// Eq. 15 for the shared-random-number mode (R18): one draw per site decides for all 32 samples of
+// the word, so cond4 / cond8 / cond12 are all-ones or zero words.
+__device__ __forceinline__ void shared_cond_words(const uint32_t R[4], const Thresholds &T, uint32_t c4[4], uint32_t c8[4],
+                                                  uint32_t c12[4])
+{
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        c4[w] = R[w] < T.t4 ? 0xFFFFFFFFu : 0u;
+        c8[w] = R[w] < T.t8 ? 0xFFFFFFFFu : 0u;
+        c12[w] = R[w] < T.t12 ? 0xFFFFFFFFu : 0u;
+    }
+}
+
 template <int RNG, int W>
 __global__ void __launch_bounds__(SWEEP_THREADS)
 half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng)
@@ -350,8 +363,13 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
         }
     }
     uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};
+    if (RNG == 2) {  // shared draw: Eq. 15 verbatim, the cond words are all ones or zero
+        uint32_t R[4];
+        philox_folded(rng.pc, rng.ps[0], g, R);
+        shared_cond_words(R, a.T, c4, c8, c12);
+    }
 #pragma unroll
-    for (int i = 0; i < SPT; i += 2) {
+    for (int i = 0; i < SPT && RNG != 2; i += 2) {
         const int b = SPT * part + i;
         uint32_t R[8];
         if (RNG == 0) {
@@ -389,6 +407,69 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
         if (PARTS == 1) a.S_act[j0 + w] = s[w] ^ f;
         else reinterpret_cast<unsigned char *>(a.S_act + j0 + w)[part] = (unsigned char)((s[w] >> sh) ^ f);  // little-endian
     }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Shared-random-number mode (rng_mode 2, R18), sample-packed, L % 8 == 0: the paper's own asynchronous multispin
+// coding.  One Philox call per group of 4 consecutive sites serves 4 x 32 flip attempts, so the
+// kernel is bound by HBM (1.125 B per flip attempt), not by the generator.  With L/2 a multiple of 4 a group never
+// leaves its row: own spins and couplings, the y+-1 / z+-1 neighbours and their couplings are 128-bit loads, the two
+// x-neighbours are the same four words of the other colour shifted by one word (one extra 32-bit load).
+// grid = (ceil(L * L/8 / 128), L): blockIdx.y = z, the x index runs over (y, group in row).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+half_sweep_shared_vec(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t gpr /* groups per row = L/8 */,
+                      uint32_t gpr_inv /* ceil(2^32 / gpr) */)
+{
+    const uint32_t L = (uint32_t)a.L, H = L >> 1;
+    const uint32_t p = blockIdx.x * 128u + threadIdx.x;
+    if (p >= L * gpr) return;
+    const uint32_t y = gpr == 1 ? p : __umulhi(p, gpr_inv), z = blockIdx.y;   // exact: p < 2^19, 2 <= gpr <= 2^8
+    const uint32_t m0 = 4u * (p - y * gpr);
+    const uint32_t rowbase = H * (y + L * z);
+    const uint32_t j0 = rowbase + m0;
+    const uint32_t HL = H * L, Hc = HL * L;
+    const uint32_t jyp = (y + 1 == L) ? j0 - (HL - H) : j0 + H, jym = (y == 0) ? j0 + (HL - H) : j0 - H;
+    const uint32_t jzp = (z + 1 == L) ? j0 - (Hc - HL) : j0 + HL, jzm = (z == 0) ? j0 + (Hc - HL) : j0 - HL;
+    const uint32_t xodd = (y + z + (uint32_t)a.colour) & 1u;
+    // the word next to the four: m0+4 (xodd = 1, +x neighbour of the last site) or m0-1 (xodd = 0, -x of the first)
+    const uint32_t m_extra = xodd ? (m0 + 4 == H ? 0u : m0 + 4) : (m0 == 0 ? H - 1 : m0 - 1);
+
+    uint32_t s[4], o[4], oyp[4], oym[4], ozp[4], ozm[4], jxa[4], jya[4], jza[4], jxo[4], jyo[4], jzo[4];
+    load_words<4>(a.S_act, j0, s);
+    load_words<4>(a.S_oth, j0, o);
+    load_words<4>(a.J_oth[0], j0, jxo);
+    const uint32_t o_extra = __ldg(a.S_oth + rowbase + m_extra);
+    const uint32_t jxo_extra = __ldg(a.J_oth[0] + rowbase + m_extra);
+    load_words<4>(a.J_act[0], j0, jxa);
+    load_words<4>(a.S_oth, jyp, oyp);
+    load_words<4>(a.S_oth, jym, oym);
+    load_words<4>(a.S_oth, jzp, ozp);
+    load_words<4>(a.S_oth, jzm, ozm);
+    load_words<4>(a.J_act[1], j0, jya);
+    load_words<4>(a.J_act[2], j0, jza);
+    load_words<4>(a.J_oth[1], jym, jyo);
+    load_words<4>(a.J_oth[2], jzm, jzo);
+
+    uint32_t R[4], c4[4], c8[4], c12[4];
+    philox_folded(rng.pc, rng.ps, j0 >> 2, R);
+    shared_cond_words(R, a.T, c4, c8, c12);
+
+    uint32_t out[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        // xodd = 0: +x is word m (own coupling), -x is word m-1 with that neighbour's coupling;
+        // xodd = 1: -x is word m with its coupling, +x is word m+1 (own coupling)
+        const uint32_t o_up = (w < 3) ? o[(w + 1) & 3] : o_extra;                    // word m+1 (xodd = 1)
+        const uint32_t o_dn = (w > 0) ? o[(w + 3) & 3] : o_extra;                    // word m-1 (xodd = 0)
+        const uint32_t jx_dn = (w > 0) ? jxo[(w + 3) & 3] : jxo_extra;
+        const uint32_t J[6] = {jxa[w], xodd ? jxo[w] : jx_dn, jya[w], jyo[w], jza[w], jzo[w]};
+        const uint32_t nb[6] = {xodd ? o_up : o[w], xodd ? o[w] : o_dn, oyp[w], oym[w], ozp[w], ozm[w]};
+        uint32_t sum2, sum1, sum0;
+        satisfied_bond_count(s[w], J, nb, sum2, sum1, sum0);
+        out[w] = s[w] ^ flip_mask(sum2, sum1, sum0, c4[w] | a.T.always4, c8[w] | a.T.always8, c12[w] | a.T.always12);
+    }
+    *reinterpret_cast<uint4 *>(a.S_act + j0) = *reinterpret_cast<const uint4 *>(out);
 }
 
 }  // namespace isingk

@@ -57,6 +57,8 @@ def test_argument_validation_without_a_gpu():
     for L, ns in ((3, 1), (2, 1), (0, 1), (-4, 1), (4096, 1), (16, 2), (16, 0), (16, 48)):
         assert lib.ising_workspace_bytes(L, ns, 0, C.byref(out)) == binding.EINVAL, (L, ns)
     assert lib.ising_workspace_bytes(16, 1, 7, C.byref(out)) == binding.EINVAL
+    assert lib.ising_workspace_bytes(16, 1, 2, C.byref(out)) == binding.EINVAL   # shared draws need 32-sample words
+    assert lib.ising_workspace_bytes(16, 32, 2, C.byref(out)) == binding.OK
     assert lib.ising_workspace_bytes(16, 1, 0, None) == binding.EINVAL
     # sizes: 8 internal bit arrays + canonical staging + accumulators
     for L, ns in ((16, 1), (64, 32), (256, 1), (1024, 1), (6, 1), (4, 64)):

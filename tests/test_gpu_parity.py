@@ -14,7 +14,7 @@ import pytest
 torch = pytest.importorskip("torch")
 
 from oracle import ea3d  # noqa: E402
-from paper_1411_0127_b200 import MINSTD, PHILOX, Ising, binding, synth  # noqa: E402
+from paper_1411_0127_b200 import MINSTD, PHILOX, PHILOX_SHARED, Ising, binding, synth  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 SEED = synth.DYN_SEED
@@ -253,6 +253,40 @@ def test_minstd_cached_seed_table_equals_recomputed_seeds(L):
         g.ising_sweep(0.5, 2)
     assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
     assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
+
+
+# ------------------------------------------------------------------------------------------------ shared-random-number mode
+
+@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (8, 32), (8, 64), (12, 32), (16, 64), (24, 32), (40, 32), (64, 32)])
+def test_shared_random_number_mode_equals_the_oracle(L, nsamples):
+    """rng_mode 2 (R18): one Philox draw per 32-sample word.  The vectorised kernel (L % 8 == 0) and
+    the generic sample-packed kernel (kernel choice 1, and every other L) against the oracle, trajectory and energies."""
+    spins, J = synth.make_spins(L, nsamples, 51), synth.make_couplings(L, nsamples, 52)
+    o, g = make_pair(L, nsamples, PHILOX_SHARED, spins, J)
+    g2 = Ising(L, nsamples, SEED, PHILOX_SHARED)
+    g2.ising_set_kernel(1)
+    g2.ising_load_state(dev(spins), dev(J))
+    for beta, n in ((1 / 1.1, 2), (0.3, 1), (1 / 0.7, 2)):
+        o.sweep(beta, n)
+        g.ising_sweep(beta, n)
+        g2.ising_sweep(beta, n)
+        assert_same_state(o, g, f"shared mode L={L} beta={beta}")
+        assert torch.equal(g.ising_get_spins(), g2.ising_get_spins())
+
+
+@pytest.mark.parametrize("beta", [0.0, float("inf")])
+def test_shared_mode_special_temperatures(beta):
+    L, ns = 16, 32
+    spins, J = synth.make_spins(L, ns, 53), synth.make_couplings(L, ns, 54)
+    o, g = make_pair(L, ns, PHILOX_SHARED, spins, J)
+    o.sweep(beta, 2)
+    g.ising_sweep(beta, 2)
+    assert_same_state(o, g, f"shared mode beta={beta}")
+
+
+def test_shared_mode_needs_whole_words_of_samples():
+    with pytest.raises(binding.IsingError):
+        Ising(16, 1, SEED, PHILOX_SHARED)
 
 
 def test_run_host_equals_device_calls():
