@@ -138,6 +138,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-minstd", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-shared", action="store_true", help="skip the shared-random-number (paper's AMSC) timing")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -229,12 +230,39 @@ def main():
         g.ising_destroy()
         return res
 
+    def bench_shared(Ls, ns, sweeps):
+        """the paper's own scheme, one draw per 32-sample word (rng_mode 2); sweeps only."""
+        from paper_1411_0127_b200 import PHILOX_SHARED
+
+        sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
+        Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
+        g = Ising(Ls, ns, synth.DYN_SEED, PHILOX_SHARED)
+        g.ising_load_state(sp, Jc)
+        g.ising_sweep(BETA, 2)
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        g.ising_sweep(BETA, sweeps)
+        b.record(stream)
+        barrier()
+        ms = a.elapsed_time(b)
+        g.ising_destroy()
+        flips = sweeps * ns * Ls**3
+        gbs = ALG_BYTES_PER_FLIP[0] * flips / (ms * 1e-3) / 1e9
+        return {"workload": f"L={Ls} cube x {ns} samples ({ns // 32} coded batches), {sweeps} sweeps, one Philox draw per 32-sample word",
+                "value": 1e9 * ms / flips, "unit": UNIT, "half_sweep_us": 1e3 * ms / (2 * sweeps),
+                "roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "alg_bytes_per_flip": ALG_BYTES_PER_FLIP[0]}}
+
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
     philox = bench_mode(PHILOX)
     clocks = sampler.stop() if rank == 0 else None
     minstd = None if args.no_minstd else bench_mode(MINSTD)
+
+    shared = None
+    if world == 1 and not args.no_shared:
+        shared = [bench_shared(128, 256, 20), bench_shared(512, 32, 4)]
 
     if rank != 0:
         if dist is not None:
@@ -289,6 +317,11 @@ def main():
                           "flips_per_s": 1e12 / ps_m}
         if "e2e_ms" in minstd:
             line["minstd"]["e2e"] = 1e9 * minstd["e2e_ms"] / (K * flips_per_step)
+    if shared is not None:
+        hbm_gbs_, _, src_ = measured_peaks()
+        for sh in shared:
+            sh["roofline"].update({"peak": hbm_gbs_, "frac": sh["roofline"]["achieved"] / hbm_gbs_, "peak_source": src_ + " (burst copy)"})
+        line["amsc_shared_random_number"] = shared
     if world == 1 and not args.no_cpu_baseline:
         Ls, sw = 512, 64  # about 15 s on the 16 host cores of the GPU box
         times, cores = time_oracle(Ls, sw, 0)

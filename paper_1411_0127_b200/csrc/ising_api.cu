@@ -159,18 +159,18 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         if (RNG == 2) {
             const uint64_t ngroups = g.Hc / 4;
             if (g.L % 8 == 0 && h->kernel_choice != 1) {
-                SiteRng sr;
-                sr.pc = r.pc;
-                sr.ps = r.ps[0];
-                sr.seed = 0;
-                sr.A2 = 0;
-                sr.s0tab = nullptr;
+                // all coded batches in one launch (blockIdx.z = batch): a is batch 0 here, b == 0
+                SharedRng sr;
+                sr.tlo = r.tlo; sr.thi = r.thi; sr.k0 = r.k0; sr.k1base = r.k1base;
                 const uint32_t gpr = (uint32_t)g.L / 8;
-                const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L);
-                half_sweep_shared_vec<<<grid, 128, 0, st>>>(a, sr, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr));
-            } else {
-                half_sweep_sample_packed<2, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
+                const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L, (unsigned)nb);
+                half_sweep_shared_vec<<<grid, 128, 0, st>>>(a, sr, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
+                                                          8 * g.array_words);
+                const int rc = check_launch(h);
+                if (rc != ISING_OK) return rc;
+                break;
             }
+            half_sweep_sample_packed<2, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
         } else if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
             // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs

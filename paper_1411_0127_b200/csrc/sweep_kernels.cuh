@@ -415,12 +415,26 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
 // kernel is bound by HBM (1.125 B per flip attempt), not by the generator.  With L/2 a multiple of 4 a group never
 // leaves its row: own spins and couplings, the y+-1 / z+-1 neighbours and their couplings are 128-bit loads, the two
 // x-neighbours are the same four words of the other colour shifted by one word (one extra 32-bit load).
-// grid = (ceil(L * L/8 / 128), L): blockIdx.y = z, the x index runs over (y, group in row).
+// grid = (ceil(L * L/8 / 128), L, batches): blockIdx.y = z, the x index runs over (y, group in row), blockIdx.z is the
+// coded batch (k batches of 32 samples in one launch); the arrays of batch b start b * batch_stride
+// words after those of batch 0, and its draws use the key (k0, k1base ^ b) (R18).  With several batches per launch the
+// launch constants cannot be folded per batch, so the plain ten rounds are run (the kernel is HBM-bound either way).
 // ---------------------------------------------------------------------------------------------------
+struct SharedRng {
+    uint32_t tlo, thi, k0, k1base;
+};
+
 __global__ void __launch_bounds__(128)
-half_sweep_shared_vec(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t gpr /* groups per row = L/8 */,
-                      uint32_t gpr_inv /* ceil(2^32 / gpr) */)
+half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups per row = L/8 */,
+                      uint32_t gpr_inv /* ceil(2^32 / gpr) */, size_t batch_stride)
 {
+    {
+        const size_t off = (size_t)blockIdx.z * batch_stride;
+        a.S_act += off;
+        a.S_oth += off;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
+    }
     const uint32_t L = (uint32_t)a.L, H = L >> 1;
     const uint32_t p = blockIdx.x * 128u + threadIdx.x;
     if (p >= L * gpr) return;
@@ -452,7 +466,7 @@ half_sweep_shared_vec(const SweepArgs a, const __grid_constant__ SiteRng rng, ui
     load_words<4>(a.J_oth[2], jzm, jzo);
 
     uint32_t R[4], c4[4], c8[4], c12[4];
-    philox_folded(rng.pc, rng.ps, j0 >> 2, R);
+    philox4x32_10(rng.tlo, rng.thi, j0 >> 2, 0u, rng.k0, rng.k1base ^ blockIdx.z, R);
     shared_cond_words(R, a.T, c4, c8, c12);
 
     uint32_t out[4];
