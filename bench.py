@@ -139,6 +139,7 @@ def main():
     ap.add_argument("--no-minstd", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-shared", action="store_true", help="skip the shared-random-number (paper's AMSC) timing")
+    ap.add_argument("--only-shared", action="store_true", help="time only the shared-random-number mode (for ncu captures)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -252,6 +253,10 @@ def main():
         return {"workload": f"L={Ls} cube x {ns} samples ({ns // 32} coded batches), {sweeps} sweeps, one Philox draw per 32-sample word",
                 "value": 1e9 * ms / flips, "unit": UNIT, "half_sweep_us": 1e3 * ms / (2 * sweeps),
                 "roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "alg_bytes_per_flip": ALG_BYTES_PER_FLIP[0]}}
+
+    if args.only_shared:
+        print(json.dumps({"amsc_shared_random_number": [bench_shared(512, 32, 4)]}))
+        return
 
     sampler = ClockSampler(local)
     if rank == 0:
