@@ -289,6 +289,67 @@ def test_shared_mode_needs_whole_words_of_samples():
         Ising(16, 1, SEED, PHILOX_SHARED)
 
 
+# ------------------------------------------------------------------------------------------------ edge cases
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+def test_zero_sweeps_is_a_no_op(rng_mode):
+    L = 64
+    spins, J = synth.make_spins(L, 1, 61), synth.make_couplings(L, 1, 62)
+    g = Ising(L, 1, SEED, rng_mode)
+    g.ising_load_state(dev(spins), dev(J))
+    n0 = g.ising_kernel_launches()
+    g.ising_sweep(0.7, 0)
+    assert g.ising_get_t() == 0 and g.ising_kernel_launches() == n0
+    assert np.array_equal(host_u32(g.ising_get_spins()), spins)
+    with pytest.raises(binding.IsingError):
+        g.ising_sweep(0.7, -1)
+    with pytest.raises(binding.IsingError):
+        g.ising_sweep(-0.1, 1)
+
+
+@pytest.mark.parametrize("rng_mode,kernel", [(PHILOX, 0), (MINSTD, 2)])
+def test_maximum_size_L2048_word_parallel_equals_generic(rng_mode, kernel):
+    """L = 2048 is the largest lattice the library accepts (Philox group index < 2^32): 2^33 spins, 1 GiB of spin bits.
+    The oracle cannot hold it (34 GB of int8 per array); the word-parallel kernel is compared with the generic
+    one-site-at-a-time kernel over one sweep, and the energy bookkeeping with the spin count."""
+    L = 2048
+    W = L**3 // 32
+    gen = torch.Generator(device="cuda").manual_seed(7)
+    d_spins = torch.randint(-2**31, 2**31 - 1, (W,), dtype=torch.int32, device="cuda", generator=gen)
+    d_J = torch.randint(-2**31, 2**31 - 1, (3 * W,), dtype=torch.int32, device="cuda", generator=gen)
+    a = Ising(L, 1, SEED, rng_mode)
+    a.ising_set_kernel(kernel)
+    a.ising_load_state(d_spins, d_J)
+    assert torch.equal(a.ising_get_spins().flatten(), d_spins)
+    a.ising_sweep(1 / 1.1, 1)
+    out_a = a.ising_get_spins().clone()
+    Ea, Ma = a.ising_energy()
+    a.ising_destroy()
+    del a
+    b = Ising(L, 1, SEED, rng_mode)
+    b.ising_set_kernel(1)
+    b.ising_load_state(d_spins, d_J)
+    b.ising_sweep(1 / 1.1, 1)
+    assert torch.equal(b.ising_get_spins(), out_a)
+    Eb, Mb = b.ising_energy()
+    assert int(Ea[0]) == int(Eb[0]) and int(Ma[0]) == int(Mb[0])
+    up = int(sum(bin(int(w) & 0xFFFFFFFF).count("1") for w in out_a.flatten()[:4096].cpu().tolist()))  # spot check of the bit order
+    assert 0 < up < 32 * 4096
+    assert abs(int(Ea[0])) < 3 * L**3 and abs(int(Ma[0])) <= L**3 and int(Ea[0]) % 2 == (3 * L**3) % 2
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+def test_sample_packed_large_lattice_one_thread_per_group(rng_mode):
+    """L = 128 x 32 samples has more than 148 x 1024 Philox groups, so the one-thread-per-group variant of the
+    sample-packed kernel runs (smaller lattices use four threads per group); two batches exercise the batch loop."""
+    L, ns = 128, 64
+    spins, J = synth.make_spins(L, ns, 71), synth.make_couplings(L, ns, 72)
+    o, g = make_pair(L, ns, rng_mode, spins, J)
+    o.sweep(1 / 1.1, 1)
+    g.ising_sweep(1 / 1.1, 1)
+    assert_same_state(o, g, f"sample-packed L={L} x {ns}")
+
+
 def test_run_host_equals_device_calls():
     L = 128
     spins, J = synth.make_spins(L, 1, 2), synth.make_couplings(L, 1, 1)
