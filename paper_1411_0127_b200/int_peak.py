@@ -15,7 +15,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "int_peak.cu")
 LIB = os.path.join(HERE, "libint_peak.so")
 MIXES = {0: "LOP3 only", 1: "IMAD.WIDE.U32 only", 2: "IMAD.WIDE + LOP3 dependent 1:1", 3: "Philox round (2 IMAD.WIDE + 2 LOP3)",
-         4: "ISETP + SEL + LOP3"}
+         4: "ISETP + SEL + LOP3", 5: "IMAD.HI.U32 only", 6: "IMAD (lo) only", 7: "Philox round + 1 LOP3", 8: "Philox round + 2 LOP3",
+         9: "Philox round + 3 LOP3", 10: "Philox round + 4 LOP3", 11: "Philox round via DFMA.RM (hi) + IMAD (lo)"}
+# source-level instructions per chain-iteration of each mix (csrc/int_peak.cu)
+OPS = {0: 4, 1: 2, 2: 4, 3: 4, 4: 6, 5: 2, 6: 2, 7: 5, 8: 6, 9: 7, 10: 8, 11: 6}
 
 
 def build(force: bool = False) -> str:
@@ -45,7 +48,10 @@ def run(ctas_per_sm: int = 8, iters: int = 4096, reps: int = 5) -> dict:
         if rc != 0:
             raise RuntimeError(f"int_peak_run({mix}) failed: {rc}")
         rate = ops.value / (ms.value * 1e-3)
-        out["mixes"][name] = {"Tinst_per_s": rate / 1e12, "inst_per_clk_per_sm_at_1965MHz": rate / sms / 1.965e9, "ms": ms.value}
+        # cycles one SMSP spends per warp on one chain-iteration: 16 warps per SMSP (8 CTAs x 8 warps / 4), 8 chains
+        cyc = ms.value * 1e-3 * 1.965e9 / (iters * 8 * (ctas_per_sm * 8 / 4))
+        out["mixes"][name] = {"Tinst_per_s": rate / 1e12, "inst_per_clk_per_sm_at_1965MHz": rate / sms / 1.965e9, "ms": ms.value,
+                              "cycles_per_warp_iteration": cyc, "instructions_per_iteration": OPS[mix]}
     return out
 
 
