@@ -10,7 +10,8 @@
  *   sites; spins and couplings are one bit each (Eq. 10); the energy
  *   change of a flip is computed word-wise from bond bits (Eq. 11) with a bit-sliced adder (Eq. 12-13)
  *   and turned into a flip mask (Eq. 14-17).  Every (sample, site, half-sweep) has its
- *   own 32-bit draw (R9-R12), unlike the paper's one draw per 32-sample word.
+ *   own 32-bit draw (R9-R12); the paper's one draw per 32-sample word is the separate
+ *   mode ISING_RNG_PHILOX_SHARED (R18).
  *
  * Conventions
  *   N = L^3, site i = x + L*(y + L*z), colour (x+y+z)&1, red = 0 is updated at even half-sweep index t (R8).

@@ -3,7 +3,7 @@
 //   E = - sum over the 3N bonds of J sigma sigma (Eq. 1, each bond once).  With the encoding of Eq. 10 the
 //   bond bit e = J ^ s_i ^ s_k (Eq. 11) is 1 exactly when -J sigma_i sigma_k = +1, so E = 2*popc(e over all bonds) - 3N,
 //   and M = 2*popc(s) - N.  The kernels accumulate the two popcounts per sample into uint64 counters (warp shuffle
-//   reduction, one atomic per warp); finalize_energy turns them into int64 E and M.
+//   reduction, then a block reduction and one atomic pair per CTA); finalize_energy turns them into int64 E and M.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

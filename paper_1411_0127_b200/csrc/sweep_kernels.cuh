@@ -9,6 +9,10 @@
 // An active site of colour c in a row of parity p = (y+z)&1 has x = 2m + xodd, xodd = c^p.  Its +-y and +-z neighbours
 // have the same m in the other colour's arrays; its two x-neighbours are bits m and m-1 (xodd = 0) or m and m+1
 // (xodd = 1) of the other colour's half-row.
+//
+// Kernels: half_sweep_site_packed<RNG, W> (RNG 0 = Philox, 1 = MINSTD stateless, 2 = MINSTD with cached seed states),
+// minstd_fill_s0<W>, half_sweep_site_packed_generic<RNG>, half_sweep_sample_packed<RNG, PARTS> (RNG 2 = shared draw, R18),
+// half_sweep_shared_vec (shared draw, 128-bit loads, all coded batches in one launch).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -24,7 +28,7 @@ struct LatticeArrays {  // one lattice (site-packed) or one batch of 32 samples 
 
 struct RngLaunch {  // per-launch PRNG constants, passed by value (constant bank)
     PhiloxCommonConst pc;
-    PhiloxSampleConst ps[32];  // site-packed kernels use ps[0] only
+    PhiloxSampleConst ps[32];  // one per sample of the batch; the generic site-packed and the shared-draw kernels use ps[0] only
     uint64_t seed;             // MINSTD
     uint32_t A;                // MINSTD: 16807^(n+1) mod M for the sweep n = t>>1 of this launch
     uint32_t tlo, thi;         // half-sweep counter (generic kernel: unfolded Philox)
