@@ -174,7 +174,14 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         } else if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
             // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs
-            if (ngroups < 148u * 1024u)
+            if (g.L % 8 == 0 && h->kernel_choice != 1) {  // 128-bit loads
+                const uint32_t gpr = (uint32_t)g.L / 8, inv = (uint32_t)((0x100000000ull + gpr - 1) / gpr);
+                const uint64_t per_plane = (uint64_t)g.L * gpr;
+                if (ngroups < 148u * 1024u)
+                    half_sweep_sample_packed_vec<RNG, 4><<<dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L), 128, 0, st>>>(a, r, gpr, inv, g.N);
+                else
+                    half_sweep_sample_packed_vec<RNG, 1><<<dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L), 128, 0, st>>>(a, r, gpr, inv, g.N);
+            } else if (ngroups < 148u * 1024u)
                 half_sweep_sample_packed<RNG, 4><<<(unsigned)((ngroups + 31) / 32), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
             else
                 half_sweep_sample_packed<RNG, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);

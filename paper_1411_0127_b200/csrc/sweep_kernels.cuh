@@ -372,7 +372,10 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
         philox_folded(rng.pc, rng.ps[0], g, R);
         shared_cond_words(R, a.T, c4, c8, c12);
     }
-#pragma unroll
+    // PARTS = 1: a rolled loop over the 16 sample pairs (the unrolled body of 32 calls is 40 KB of code that every warp
+    // walks through once, and the instruction cache misses showed up as the top stall); PARTS = 4: 4 pairs, unrolled.
+    uint32_t bit_lo = 1u;  // 1 << i
+#pragma unroll(PARTS == 1 ? 1 : 4)
     for (int i = 0; i < SPT && RNG != 2; i += 2) {
         const int b = SPT * part + i;
         uint32_t R[8];
@@ -388,19 +391,21 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
                     R[4 * e + w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(rng.seed + (qs + site[w] + 1) * SPLITMIX_GAMMA));
             }
         }
+        const uint32_t bit_hi = bit_lo << 1;
         uint32_t mn = 0xFFFFFFFFu;
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
-            or_if_lt(c4[e & 3], R[e], a.T.t4, 1u << (i + (e >> 2)));
+            or_if_lt(c4[e & 3], R[e], a.T.t4, e < 4 ? bit_lo : bit_hi);
             mn = min_u32(mn, R[e]);
         }
         if (__any_sync(0xFFFFFFFFu, mn < a.T.t8)) {
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
-                or_if_lt(c8[e & 3], R[e], a.T.t8, 1u << (i + (e >> 2)));
-                or_if_lt(c12[e & 3], R[e], a.T.t12, 1u << (i + (e >> 2)));
+                or_if_lt(c8[e & 3], R[e], a.T.t8, e < 4 ? bit_lo : bit_hi);
+                or_if_lt(c12[e & 3], R[e], a.T.t12, e < 4 ? bit_lo : bit_hi);
             }
         }
+        bit_lo <<= 2;
     }
     if (!valid) return;
     const int sh = SPT * part;
@@ -410,6 +415,55 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
                                      c12[w] | a.T.always12);
         if (PARTS == 1) a.S_act[j0 + w] = s[w] ^ f;
         else reinterpret_cast<unsigned char *>(a.S_act + j0 + w)[part] = (unsigned char)((s[w] >> sh) ^ f);  // little-endian
+    }
+}
+
+// Loads and field sums of one group of four consecutive same-colour sites of a row, sample-packed, L % 8 == 0 (so that
+// L/2 is a multiple of 4 and a group never leaves its row): own spins and couplings, the y+-1 / z+-1 neighbours and their
+// couplings are 128-bit loads; the two x-neighbours are the same four words of the other colour shifted by one word
+// (one extra 32-bit load each for spins and couplings).  p = index of the group within the plane z (y = p / gpr).
+__device__ __forceinline__ void vec_group_sums(const SweepArgs &a, uint32_t gpr, uint32_t gpr_inv, uint32_t p, uint32_t z,
+                                               uint32_t &j0, uint64_t &site0, uint32_t s[4], uint32_t sum2[4], uint32_t sum1[4],
+                                               uint32_t sum0[4])
+{
+    const uint32_t L = (uint32_t)a.L, H = L >> 1;
+    const uint32_t y = gpr == 1 ? p : __umulhi(p, gpr_inv);   // exact: p < 2^19, 2 <= gpr <= 2^8
+    const uint32_t m0 = 4u * (p - y * gpr);
+    const uint32_t rowbase = H * (y + L * z);
+    j0 = rowbase + m0;
+    const uint32_t HL = H * L, Hc = HL * L;
+    const uint32_t jyp = (y + 1 == L) ? j0 - (HL - H) : j0 + H, jym = (y == 0) ? j0 + (HL - H) : j0 - H;
+    const uint32_t jzp = (z + 1 == L) ? j0 - (Hc - HL) : j0 + HL, jzm = (z == 0) ? j0 + (Hc - HL) : j0 - HL;
+    const uint32_t xodd = (y + z + (uint32_t)a.colour) & 1u;
+    site0 = (uint64_t)(2u * m0 + xodd) + (uint64_t)L * ((uint64_t)y + (uint64_t)L * (uint64_t)z);
+    // the word next to the four: m0+4 (xodd = 1, +x neighbour of the last site) or m0-1 (xodd = 0, -x of the first)
+    const uint32_t m_extra = xodd ? (m0 + 4 == H ? 0u : m0 + 4) : (m0 == 0 ? H - 1 : m0 - 1);
+
+    uint32_t o[4], oyp[4], oym[4], ozp[4], ozm[4], jxa[4], jya[4], jza[4], jxo[4], jyo[4], jzo[4];
+    load_words<4>(a.S_act, j0, s);
+    load_words<4>(a.S_oth, j0, o);
+    load_words<4>(a.J_oth[0], j0, jxo);
+    const uint32_t o_extra = __ldg(a.S_oth + rowbase + m_extra);
+    const uint32_t jxo_extra = __ldg(a.J_oth[0] + rowbase + m_extra);
+    load_words<4>(a.J_act[0], j0, jxa);
+    load_words<4>(a.S_oth, jyp, oyp);
+    load_words<4>(a.S_oth, jym, oym);
+    load_words<4>(a.S_oth, jzp, ozp);
+    load_words<4>(a.S_oth, jzm, ozm);
+    load_words<4>(a.J_act[1], j0, jya);
+    load_words<4>(a.J_act[2], j0, jza);
+    load_words<4>(a.J_oth[1], jym, jyo);
+    load_words<4>(a.J_oth[2], jzm, jzo);
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        // xodd = 0: +x is word m (own coupling), -x is word m-1 with that neighbour's coupling;
+        // xodd = 1: -x is word m with its coupling, +x is word m+1 (own coupling)
+        const uint32_t o_up = (w < 3) ? o[(w + 1) & 3] : o_extra;                    // word m+1 (xodd = 1)
+        const uint32_t o_dn = (w > 0) ? o[(w + 3) & 3] : o_extra;                    // word m-1 (xodd = 0)
+        const uint32_t jx_dn = (w > 0) ? jxo[(w + 3) & 3] : jxo_extra;
+        const uint32_t J[6] = {jxa[w], xodd ? jxo[w] : jx_dn, jya[w], jyo[w], jza[w], jzo[w]};
+        const uint32_t nb[6] = {xodd ? o_up : o[w], xodd ? o[w] : o_dn, oyp[w], oym[w], ozp[w], ozm[w]};
+        satisfied_bond_count(s[w], J, nb, sum2[w], sum1[w], sum0[w]);
     }
 }
 
@@ -439,35 +493,12 @@ half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups p
 #pragma unroll
         for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
     }
-    const uint32_t L = (uint32_t)a.L, H = L >> 1;
+    const uint32_t L = (uint32_t)a.L;
     const uint32_t p = blockIdx.x * 128u + threadIdx.x;
     if (p >= L * gpr) return;
-    const uint32_t y = gpr == 1 ? p : __umulhi(p, gpr_inv), z = blockIdx.y;   // exact: p < 2^19, 2 <= gpr <= 2^8
-    const uint32_t m0 = 4u * (p - y * gpr);
-    const uint32_t rowbase = H * (y + L * z);
-    const uint32_t j0 = rowbase + m0;
-    const uint32_t HL = H * L, Hc = HL * L;
-    const uint32_t jyp = (y + 1 == L) ? j0 - (HL - H) : j0 + H, jym = (y == 0) ? j0 + (HL - H) : j0 - H;
-    const uint32_t jzp = (z + 1 == L) ? j0 - (Hc - HL) : j0 + HL, jzm = (z == 0) ? j0 + (Hc - HL) : j0 - HL;
-    const uint32_t xodd = (y + z + (uint32_t)a.colour) & 1u;
-    // the word next to the four: m0+4 (xodd = 1, +x neighbour of the last site) or m0-1 (xodd = 0, -x of the first)
-    const uint32_t m_extra = xodd ? (m0 + 4 == H ? 0u : m0 + 4) : (m0 == 0 ? H - 1 : m0 - 1);
-
-    uint32_t s[4], o[4], oyp[4], oym[4], ozp[4], ozm[4], jxa[4], jya[4], jza[4], jxo[4], jyo[4], jzo[4];
-    load_words<4>(a.S_act, j0, s);
-    load_words<4>(a.S_oth, j0, o);
-    load_words<4>(a.J_oth[0], j0, jxo);
-    const uint32_t o_extra = __ldg(a.S_oth + rowbase + m_extra);
-    const uint32_t jxo_extra = __ldg(a.J_oth[0] + rowbase + m_extra);
-    load_words<4>(a.J_act[0], j0, jxa);
-    load_words<4>(a.S_oth, jyp, oyp);
-    load_words<4>(a.S_oth, jym, oym);
-    load_words<4>(a.S_oth, jzp, ozp);
-    load_words<4>(a.S_oth, jzm, ozm);
-    load_words<4>(a.J_act[1], j0, jya);
-    load_words<4>(a.J_act[2], j0, jza);
-    load_words<4>(a.J_oth[1], jym, jyo);
-    load_words<4>(a.J_oth[2], jzm, jzo);
+    uint32_t j0, s[4], sum2[4], sum1[4], sum0[4];
+    uint64_t site0;
+    vec_group_sums(a, gpr, gpr_inv, p, blockIdx.y, j0, site0, s, sum2, sum1, sum0);
 
     uint32_t R[4], c4[4], c8[4], c12[4];
     philox4x32_10(rng.tlo, rng.thi, j0 >> 2, 0u, rng.k0, rng.k1base ^ blockIdx.z, R);
@@ -475,19 +506,81 @@ half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups p
 
     uint32_t out[4];
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
-        // xodd = 0: +x is word m (own coupling), -x is word m-1 with that neighbour's coupling;
-        // xodd = 1: -x is word m with its coupling, +x is word m+1 (own coupling)
-        const uint32_t o_up = (w < 3) ? o[(w + 1) & 3] : o_extra;                    // word m+1 (xodd = 1)
-        const uint32_t o_dn = (w > 0) ? o[(w + 3) & 3] : o_extra;                    // word m-1 (xodd = 0)
-        const uint32_t jx_dn = (w > 0) ? jxo[(w + 3) & 3] : jxo_extra;
-        const uint32_t J[6] = {jxa[w], xodd ? jxo[w] : jx_dn, jya[w], jyo[w], jza[w], jzo[w]};
-        const uint32_t nb[6] = {xodd ? o_up : o[w], xodd ? o[w] : o_dn, oyp[w], oym[w], ozp[w], ozm[w]};
-        uint32_t sum2, sum1, sum0;
-        satisfied_bond_count(s[w], J, nb, sum2, sum1, sum0);
-        out[w] = s[w] ^ flip_mask(sum2, sum1, sum0, c4[w] | a.T.always4, c8[w] | a.T.always8, c12[w] | a.T.always12);
-    }
+    for (int w = 0; w < 4; ++w)
+        out[w] = s[w] ^ flip_mask(sum2[w], sum1[w], sum0[w], c4[w] | a.T.always4, c8[w] | a.T.always8, c12[w] | a.T.always12);
     *reinterpret_cast<uint4 *>(a.S_act + j0) = *reinterpret_cast<const uint4 *>(out);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Independent draws (Philox or MINSTD per sample), sample-packed, L % 8 == 0: the loads and field sums of
+// half_sweep_shared_vec, then one Philox call per sample as in half_sweep_sample_packed (same PARTS scheme: PARTS = 4
+// spreads the 32 samples of a group over the four warps of the CTA, each updating one byte of the four words).
+// grid = (ceil(L * L/8 / (128 / PARTS)), L), one launch per batch of 32 samples.
+// ---------------------------------------------------------------------------------------------------
+template <int RNG, int PARTS>
+__global__ void __launch_bounds__(128)
+half_sweep_sample_packed_vec(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t gpr, uint32_t gpr_inv, uint64_t N)
+{
+    constexpr int SPT = 32 / PARTS;
+    const uint32_t L = (uint32_t)a.L;
+    const int part = PARTS == 1 ? 0 : (int)(threadIdx.x >> 5);  // warp-uniform
+    const uint32_t p_raw = PARTS == 1 ? blockIdx.x * 128u + threadIdx.x : blockIdx.x * 32u + (threadIdx.x & 31u);
+    const bool valid = p_raw < L * gpr;
+    const uint32_t p = valid ? p_raw : L * gpr - 1;  // keep the warp converged for the votes below
+    uint32_t j0, s[4], sum2[4], sum1[4], sum0[4];
+    uint64_t site0;
+    vec_group_sums(a, gpr, gpr_inv, p, blockIdx.y, j0, site0, s, sum2, sum1, sum0);
+    const uint32_t g = j0 >> 2;
+
+    uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};
+    uint32_t bit_lo = 1u;  // 1 << i
+#pragma unroll(PARTS == 1 ? 1 : 4)
+    for (int i = 0; i < SPT; i += 2) {
+        const int b = SPT * part + i;
+        uint32_t R[8];
+        if (RNG == 0) {
+            philox_folded(rng.pc, rng.ps[b], g, R);
+            philox_folded(rng.pc, rng.ps[b + 1], g, R + 4);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const uint64_t w0 = rng.seed + ((uint64_t)(rng.sample_base + b + e) * N + site0 + 1) * SPLITMIX_GAMMA;
+#pragma unroll
+                for (int w = 0; w < 4; ++w)  // consecutive sites of the colour are 2 apart in the canonical index
+                    R[4 * e + w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(w0 + (uint64_t)w * (2 * SPLITMIX_GAMMA)));
+            }
+        }
+        const uint32_t bit_hi = bit_lo << 1;
+        uint32_t mn = 0xFFFFFFFFu;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            or_if_lt(c4[e & 3], R[e], a.T.t4, e < 4 ? bit_lo : bit_hi);
+            mn = min_u32(mn, R[e]);
+        }
+        if (__any_sync(0xFFFFFFFFu, mn < a.T.t8)) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                or_if_lt(c8[e & 3], R[e], a.T.t8, e < 4 ? bit_lo : bit_hi);
+                or_if_lt(c12[e & 3], R[e], a.T.t12, e < 4 ? bit_lo : bit_hi);
+            }
+        }
+        bit_lo <<= 2;
+    }
+    if (!valid) return;
+    const int sh = SPT * part;
+    uint32_t out[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t f = flip_mask(sum2[w] >> sh, sum1[w] >> sh, sum0[w] >> sh, c4[w] | a.T.always4, c8[w] | a.T.always8,
+                                     c12[w] | a.T.always12);
+        out[w] = (s[w] >> sh) ^ f;
+    }
+    if (PARTS == 1) {
+        *reinterpret_cast<uint4 *>(a.S_act + j0) = *reinterpret_cast<const uint4 *>(out);
+    } else {
+#pragma unroll
+        for (int w = 0; w < 4; ++w) reinterpret_cast<unsigned char *>(a.S_act + j0 + w)[part] = (unsigned char)out[w];  // little-endian
+    }
 }
 
 }  // namespace isingk

@@ -339,6 +339,22 @@ def test_maximum_size_L2048_word_parallel_equals_generic(rng_mode, kernel):
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L,nsamples", [(8, 32), (24, 64), (64, 32), (128, 32)])
+def test_sample_packed_vector_kernel_equals_scalar_kernel(L, nsamples, rng_mode):
+    """L % 8 == 0: the sample-packed kernel with 128-bit loads (default) against the scalar-load kernel (kernel choice 1),
+    both thread-per-group variants (L = 128 x 32 has more than 148 x 1024 groups)."""
+    spins, J = synth.make_spins(L, nsamples, 81), synth.make_couplings(L, nsamples, 82)
+    a = Ising(L, nsamples, SEED, rng_mode)
+    b = Ising(L, nsamples, SEED, rng_mode)
+    b.ising_set_kernel(1)
+    for g in (a, b):
+        g.ising_load_state(dev(spins), dev(J))
+        g.ising_sweep(1 / 1.1, 2)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
 def test_sample_packed_large_lattice_one_thread_per_group(rng_mode):
     """L = 128 x 32 samples has more than 148 x 1024 Philox groups, so the one-thread-per-group variant of the
     sample-packed kernel runs (smaller lattices use four threads per group); two batches exercise the batch loop."""
