@@ -139,6 +139,23 @@ void fill_rng_launch(const ising_t *h, int batch, RngLaunch *r)
     }
 }
 
+// Launch with programmatic stream serialization (the kernel calls wait_for_previous_kernel() before its first load).
+template <typename... KArgs, typename... Args>
+void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, args...);  // errors surface through cudaGetLastError in check_launch
+}
+
 template <int RNG>
 int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
 {
@@ -164,13 +181,13 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 sr.tlo = r.tlo; sr.thi = r.thi; sr.k0 = r.k0; sr.k1base = r.k1base;
                 const uint32_t gpr = (uint32_t)g.L / 8;
                 const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L, (unsigned)nb);
-                half_sweep_shared_vec<<<grid, 128, 0, st>>>(a, sr, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
-                                                          8 * g.array_words);
+                launch_pdl(half_sweep_shared_vec, grid, dim3(128), st, a, sr, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
+                           (size_t)(8 * g.array_words));
                 const int rc = check_launch(h);
                 if (rc != ISING_OK) return rc;
                 break;
             }
-            half_sweep_sample_packed<2, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
+            launch_pdl(half_sweep_sample_packed<2, 1>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
         } else if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
             // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs
@@ -178,13 +195,13 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 const uint32_t gpr = (uint32_t)g.L / 8, inv = (uint32_t)((0x100000000ull + gpr - 1) / gpr);
                 const uint64_t per_plane = (uint64_t)g.L * gpr;
                 if (ngroups < 148u * 1024u)
-                    half_sweep_sample_packed_vec<RNG, 4><<<dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L), 128, 0, st>>>(a, r, gpr, inv, g.N);
+                    launch_pdl(half_sweep_sample_packed_vec<RNG, 4>, dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N);
                 else
-                    half_sweep_sample_packed_vec<RNG, 1><<<dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L), 128, 0, st>>>(a, r, gpr, inv, g.N);
+                    launch_pdl(half_sweep_sample_packed_vec<RNG, 1>, dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N);
             } else if (ngroups < 148u * 1024u)
-                half_sweep_sample_packed<RNG, 4><<<(unsigned)((ngroups + 31) / 32), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
+                launch_pdl(half_sweep_sample_packed<RNG, 4>, dim3((unsigned)((ngroups + 31) / 32)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
             else
-                half_sweep_sample_packed<RNG, 1><<<(unsigned)((ngroups + 127) / 128), 128, 0, st>>>(a, r, (uint32_t)ngroups, g.N);
+                launch_pdl(half_sweep_sample_packed<RNG, 1>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = g.W;
@@ -210,15 +227,15 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                     h->s0_ready = true;
                 }
                 sr.s0tab = tab[c];
-                if (W == 4) half_sweep_site_packed<2, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
-                else if (W == 2) half_sweep_site_packed<2, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
-                else half_sweep_site_packed<2, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
-            } else if (W == 4) half_sweep_site_packed<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
-            else if (W == 2) half_sweep_site_packed<RNG, 2><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
-            else half_sweep_site_packed<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+                if (W == 4) launch_pdl(half_sweep_site_packed<2, 4>, grid, dim3(SWEEP_THREADS), st, a, sr);
+                else if (W == 2) launch_pdl(half_sweep_site_packed<2, 2>, grid, dim3(SWEEP_THREADS), st, a, sr);
+                else launch_pdl(half_sweep_site_packed<2, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
+            } else if (W == 4) launch_pdl(half_sweep_site_packed<RNG, 4>, grid, dim3(SWEEP_THREADS), st, a, sr);
+            else if (W == 2) launch_pdl(half_sweep_site_packed<RNG, 2>, grid, dim3(SWEEP_THREADS), st, a, sr);
+            else launch_pdl(half_sweep_site_packed<RNG, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
-            half_sweep_site_packed_generic<RNG><<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(a, r, nw, g.Hc);
+            launch_pdl(half_sweep_site_packed_generic<RNG>, dim3((unsigned)((nw + 255) / 256)), dim3(256), st, a, r, (uint64_t)nw, (uint64_t)g.Hc);
         }
         const int rc = check_launch(h);
         if (rc != ISING_OK) return rc;

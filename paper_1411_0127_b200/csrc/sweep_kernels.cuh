@@ -92,6 +92,11 @@ __device__ __forceinline__ size_t minstd_s0_index(uint32_t warp_global, int k, i
 
 constexpr int SWEEP_THREADS = 256;
 
+// Programmatic dependent launch: a half-sweep launched with the programmatic-stream-serialization attribute may start
+// its CTAs (index arithmetic) while the previous half-sweep drains; it must not touch the lattice before this point.
+// Without the attribute this is a no-op.
+__device__ __forceinline__ void wait_for_previous_kernel() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // Eq. 15 for the shared-random-number mode (R18): one draw per site decides for all 32 samples of
 // the word, so cond4 / cond8 / cond12 are all-ones or zero words.
 __device__ __forceinline__ void shared_cond_words(const uint32_t R[4], const Thresholds &T, uint32_t c4[4], uint32_t c8[4],
@@ -129,6 +134,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
 
     uint32_t s[W], sum2[W], sum1[W], sum0[W];
     const int xodd = (y + z + a.colour) & 1;
+    wait_for_previous_kernel();
     {
         uint32_t o[W], oyp[W], oym[W], ozp[W], ozm[W];
         uint32_t jxa[W], jya[W], jza[W], jxo[W], jyo[W], jzo[W];
@@ -274,6 +280,7 @@ half_sweep_site_packed_generic(const SweepArgs a, const __grid_constant__ RngLau
     const uint64_t widx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (widx >= n_words) return;
     const int L = a.L, H = L >> 1;
+    wait_for_previous_kernel();
     uint32_t word = a.S_act[widx];
     uint32_t flips = 0;
     uint32_t R4[4] = {0, 0, 0, 0};
@@ -341,6 +348,7 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
     uint32_t m = j0 % H;
     const uint32_t r0 = j0 / H;
     uint32_t y = r0 % L, z = r0 / L;
+    wait_for_previous_kernel();
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
         const uint32_t j = j0 + w;
@@ -440,6 +448,7 @@ __device__ __forceinline__ void vec_group_sums(const SweepArgs &a, uint32_t gpr,
     const uint32_t m_extra = xodd ? (m0 + 4 == H ? 0u : m0 + 4) : (m0 == 0 ? H - 1 : m0 - 1);
 
     uint32_t o[4], oyp[4], oym[4], ozp[4], ozm[4], jxa[4], jya[4], jza[4], jxo[4], jyo[4], jzo[4];
+    wait_for_previous_kernel();
     load_words<4>(a.S_act, j0, s);
     load_words<4>(a.S_oth, j0, o);
     load_words<4>(a.J_oth[0], j0, jxo);
