@@ -140,6 +140,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-shared", action="store_true", help="skip the shared-random-number (paper's AMSC) timing")
     ap.add_argument("--only-shared", action="store_true", help="time only the shared-random-number mode (for ncu captures)")
+    ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -253,6 +254,35 @@ def main():
         return {"workload": f"L={Ls} cube x {ns} samples ({ns // 32} coded batches), {sweeps} sweeps, one Philox draw per 32-sample word",
                 "value": 1e9 * ms / flips, "unit": UNIT, "half_sweep_us": 1e3 * ms / (2 * sweeps),
                 "roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "alg_bytes_per_flip": ALG_BYTES_PER_FLIP[0]}}
+
+    if args.scan:
+        from paper_1411_0127_b200 import PHILOX_SHARED
+
+        rows = []
+        cases = [(Ls, 1, m) for Ls in (64, 128, 256, 512, 1024, 2048) for m in (PHILOX, MINSTD)]
+        cases += [(Ls, 32, m) for Ls in (32, 64, 128, 256) for m in (PHILOX, MINSTD)]
+        cases += [(64, 32, PHILOX_SHARED), (128, 32, PHILOX_SHARED), (128, 256, PHILOX_SHARED), (256, 32, PHILOX_SHARED),
+                  (512, 32, PHILOX_SHARED)]
+        for Ls, ns, mode in cases:
+            sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
+            Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
+            g = Ising(Ls, ns, synth.DYN_SEED, mode)
+            g.ising_load_state(sp, Jc)
+            g.ising_sweep(BETA, 2)
+            nsweeps = max(2, min(200, int(2e10 / (ns * Ls**3))))
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            g.ising_sweep(BETA, nsweeps)
+            b.record(stream)
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            g.ising_destroy()
+            del g, sp, Jc
+            rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
+                         "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
+        print(json.dumps({"scan": rows}))
+        return
 
     if args.only_shared:
         print(json.dumps({"amsc_shared_random_number": [bench_shared(512, 32, 4)]}))
