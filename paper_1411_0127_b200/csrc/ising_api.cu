@@ -47,8 +47,8 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->array_words = round_up(raw, ALIGN_WORDS);
     g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
-    // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs of the word-parallel energy kernel
-    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS) * sizeof(unsigned long long), 256);
+    // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs and the ticket of the word-parallel energy kernel
+    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1) * sizeof(unsigned long long), 256);
     g->fast = nsamples == 1 && L >= 64 && (L & (L - 1)) == 0;
     g->s0_words = g->fast ? (size_t)g->N : 0;  // 2 colours x N/2 sites x 4 bytes
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
@@ -71,6 +71,7 @@ struct ising {
     unsigned long long *acc;
     uint32_t *s0tab;   // MINSTD mode, fast layout: seed-state tables of the two colours (nullptr otherwise)
     bool s0_ready;
+    bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
 
     LatticeArrays arrays(int batch) const
     {
@@ -254,8 +255,25 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
 {
     const Geometry &g = h->g;
     unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;
-    bool use_slots = false;
-    if (cudaMemsetAsync(h->acc, 0, g.acc_bytes, st) != cudaSuccess)
+    if (g.nsamples == 1 && g.fast && h->kernel_choice != 1) {  // one fused launch (measure_kernels.cuh)
+        if (!h->slots_clean) {
+            if (cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
+            h->slots_clean = true;
+        }
+        const LatticeArrays A = h->arrays(0);
+        MeasureArgs m;
+        for (int c = 0; c < 2; ++c) {
+            m.S[c] = A.S[c];
+            for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
+        }
+        m.L = g.L;
+        const int tpr = (g.L >> 6) / g.W;
+        const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
+        if (g.W == 4) launch_pdl(energy_site_packed<4>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
+        else launch_pdl(energy_site_packed<1>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
+        return check_launch(h);
+    }
+    if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess)
         return ISING_ECUDA;
     const int nb = g.nsamples == 1 ? 1 : g.nbatches;
     for (int b = 0; b < nb; ++b) {
@@ -268,12 +286,6 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         m.L = g.L;
         if (g.nsamples != 1) {
             energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
-        } else if (g.fast && h->kernel_choice != 1) {
-            const int tpr = (g.L >> 6) / g.W;
-            const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
-            if (g.W == 4) energy_site_packed<4><<<grid, SWEEP_THREADS, 0, st>>>(m, slots);
-            else energy_site_packed<1><<<grid, SWEEP_THREADS, 0, st>>>(m, slots);
-            use_slots = true;
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc, nw, g.Hc);
@@ -281,7 +293,7 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         const int rc = check_launch(h);
         if (rc != ISING_OK) return rc;
     }
-    finalize_energy<<<(g.nsamples + 127) / 128, 128, 0, st>>>(h->acc, g.nsamples, (long long)g.N, d_E, d_M, use_slots ? slots : nullptr);
+    finalize_energy<<<(g.nsamples + 127) / 128, 128, 0, st>>>(h->acc, g.nsamples, (long long)g.N, d_E, d_M);
     return check_launch(h);
 }
 
@@ -320,6 +332,7 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->acc = (unsigned long long *)(h->staging + h->g.staging_words);
     h->s0tab = (rng_mode == ISING_RNG_MINSTD && h->g.s0_words) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->s0_ready = false;
+    h->slots_clean = false;
     *out = h;
     return ISING_OK;
 }

@@ -13,7 +13,7 @@
 namespace isingk {
 
 // The word-parallel site-packed kernel spreads its per-CTA atomics over ACC_SLOTS counter pairs (one address would
-// serialise 16384 atomics in L2 at L = 1024); finalize_energy adds them up.
+// serialise 16384 atomics in L2 at L = 1024); the last CTA adds them up.
 constexpr int ACC_SLOTS = 64;
 
 struct MeasureArgs {
@@ -56,9 +56,13 @@ __device__ __forceinline__ void block_accumulate2(unsigned long long a, unsigned
 // other colour's half-row (a funnel shift by xodd; the bit entering at the end of the thread's words comes from the
 // next lane of the row); +y / +z neighbours are the same bit one row up.  Every word is read once from HBM with 128-bit
 // loads (the neighbour reads hit L1/L2): 512 MiB at L = 1024.
+// One launch does everything: the CTAs add their counts to the slots, and the last CTA to finish (a ticket counter
+// behind the slots) sums the slots, writes E and M (R16), and clears slots and counter for the next call, so a trace of
+// E per half-sweep costs one small launch per record instead of memset + kernel + finalize.
 template <int W>
 __global__ void __launch_bounds__(SWEEP_THREADS)
-energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {unsatisfied bonds, up spins} */)
+energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {unsatisfied bonds, up spins}, then the ticket */,
+                   long long N, long long *E, long long *M)
 {
     const int L = a.L, wpr = L >> 6, tpr = wpr / W;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -72,6 +76,7 @@ energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {
     const uint32_t row_zp = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zp) + k0;
     const int next_lane = (lane & ~(tpr - 1)) | ((lane_in_row + 1) & (tpr - 1));
     unsigned int unsat = 0, up = 0;
+    wait_for_previous_kernel();
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
         uint32_t s[W], o[W], oyp[W], ozp[W], jx[W], jy[W], jz[W];
@@ -93,6 +98,26 @@ energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {
         }
     }
     block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
+    __shared__ bool is_last;
+    unsigned int *ticket = reinterpret_cast<unsigned int *>(acc + 2 * ACC_SLOTS);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        is_last = atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1;  // every other CTA's atomics are visible then
+    }
+    __syncthreads();
+    if (is_last && threadIdx.x < 32) {  // warp 0 of the last CTA: read-and-clear the slots, two per lane
+        unsigned long long tu = 0, tp = 0;
+        for (int k = threadIdx.x; k < ACC_SLOTS; k += 32) {
+            tu += atomicExch(&acc[2 * k], 0ull);
+            tp += atomicExch(&acc[2 * k + 1], 0ull);
+        }
+        warp_reduce_add2(tu, tp);
+        if (threadIdx.x == 0) {
+            if (E) E[0] = 2 * (long long)tu - 3 * N;
+            if (M) M[0] = 2 * (long long)tp - N;
+            *ticket = 0u;
+        }
+    }
 }
 
 // Site-packed, any even L: one thread per word, one site at a time.
@@ -167,17 +192,13 @@ energy_sample_packed(const MeasureArgs a, unsigned long long *acc /* [32][2] */,
     }
 }
 
-// E = 2*unsat - 3N, M = 2*up - N  (R16), one thread per sample.  slots: nullptr, or ACC_SLOTS counter pairs of sample 0.
-__global__ void finalize_energy(const unsigned long long *acc, int nsamples, long long N, long long *E, long long *M,
-                                const unsigned long long *slots)
+// E = 2*unsat - 3N, M = 2*up - N  (R16), one thread per sample (sample-packed and generic paths).
+__global__ void finalize_energy(const unsigned long long *acc, int nsamples, long long N, long long *E, long long *M)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= nsamples) return;
-    unsigned long long unsat = acc[2 * s], up = acc[2 * s + 1];
-    if (slots && s == 0)
-        for (int k = 0; k < ACC_SLOTS; ++k) { unsat += slots[2 * k]; up += slots[2 * k + 1]; }
-    if (E) E[s] = 2 * (long long)unsat - 3 * N;
-    if (M) M[s] = 2 * (long long)up - N;
+    if (E) E[s] = 2 * (long long)acc[2 * s] - 3 * N;
+    if (M) M[s] = 2 * (long long)acc[2 * s + 1] - N;
 }
 
 }  // namespace isingk
