@@ -87,11 +87,21 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def time_oracle(L, sweeps, rng_mode, repeats=1):
+def time_oracle(L, sweeps, rng_mode, repeats=1, threads=None):
     """The oracle as it stands (OpenMP over the planes of one colour) on this host: seconds per call of `sweeps` sweeps."""
     from oracle import ea3d
     from paper_1411_0127_b200 import synth
 
+    all_threads = ea3d.max_threads()
+    if threads is not None:
+        ea3d.set_threads(threads)
+    try:
+        return _time_oracle(ea3d, synth, L, sweeps, rng_mode, repeats), (threads or all_threads)
+    finally:
+        ea3d.set_threads(all_threads)
+
+
+def _time_oracle(ea3d, synth, L, sweeps, rng_mode, repeats):
     o = ea3d.Oracle(L, 1, synth.DYN_SEED, rng_mode)
     o.load_packed(synth.make_spins(L), synth.make_couplings(L))
     o.sweep(BETA, 1)  # touch the pages
@@ -100,7 +110,7 @@ def time_oracle(L, sweeps, rng_mode, repeats=1):
         t0 = time.perf_counter()
         o.sweep(BETA, sweeps)
         times.append(time.perf_counter() - t0)
-    return times, ea3d.max_threads()
+    return times
 
 
 def run_reference(args):
@@ -212,7 +222,9 @@ def main():
         total_ms = max_over_ranks(e0.elapsed_time(e1))
         sweep_ms = max_over_ranks(sum(a.elapsed_time(b) for a, b in evs))
         launches = g.ising_kernel_launches() - l0
-        res = {"total_ms": total_ms, "sweep_ms": sweep_ms, "launches": launches, "E": int(E[0]), "M": int(M[0])}
+        per_step = sorted(a.elapsed_time(b) for a, b in evs)  # this rank's sweep regions (20 sweeps = 40 launches each)
+        res = {"total_ms": total_ms, "sweep_ms": sweep_ms, "launches": launches, "E": int(E[0]), "M": int(M[0]),
+               "sweep_ms_median": per_step[len(per_step) // 2], "sweep_ms_best": per_step[0]}
         # end to end through host buffers
         if not args.no_e2e:
             for _ in range(2):
@@ -316,7 +328,8 @@ def main():
         hbm_obj = {"achieved": hbm, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm / hbm_gbs, "alg_bytes_per_flip": ALG_BYTES_PER_FLIP[rng_mode],
                    "alg_bytes_per_launch": ALG_BYTES_PER_FLIP[rng_mode] * flips_per_launch, "peak_source": peaks_src + " (burst copy)"}
         common = {"traffic": NCU_TRAFFIC_BYTES_L1024[rng_mode] if L == 1024 else None,
-                  "kernel": "half_sweep_site_packed", "kernel_ms": half_sweep_ms, "kernel_ps_per_flip": 1e9 * half_sweep_ms / flips_per_launch}
+                  "kernel": "half_sweep_site_packed", "kernel_ms": half_sweep_ms, "kernel_ps_per_flip": 1e9 * half_sweep_ms / flips_per_launch,
+                  "kernel_ms_median": res["sweep_ms_median"] / (2 * nsw), "kernel_ms_best": res["sweep_ms_best"] / (2 * nsw)}
         if rng_mode == 1:  # MINSTD with cached seed states: bound by HBM
             return ps, {"bound": "hbm", **hbm_obj, **common}
         slot_rate = ALG_SLOTS_PER_FLIP[rng_mode] * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12  # T slots/s
@@ -362,6 +375,9 @@ def main():
         times, cores = time_oracle(Ls, sw, 0)
         line["cpu_baseline"] = {"value": 1e12 * times[0] / (sw * Ls**3), "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"L={Ls} cube (1/8 of the sites of the L=1024 workload, same recipe, Philox), {sw} sweeps, {times[0]:.1f} s"}
+        t1, _ = time_oracle(256, 8, 0, threads=1)  # single-thread figure too (about 4 s)
+        line["cpu_baseline"]["single_thread"] = {"value": 1e12 * t1[0] / (8 * 256**3), "unit": UNIT, "cores": 1,
+                                                 "sample": f"L=256 cube, 8 sweeps, {t1[0]:.1f} s"}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
