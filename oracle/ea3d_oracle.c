@@ -17,8 +17,10 @@
  * beta=inf / beta=0 special cases, incremental-vs-recomputed energy, gauge invariance, closed-form
  * energies, cuRAND's host Philox4_32_10 generator, C++ std::minstd_rand0 and the Park-Miller
  * 10000th-value check, an independent pure-Python big-integer implementation (oracle/ea3d_py.py).
- * SplitMix64 has no external reference in this container: "parity unpinned" for that one function
- * (two independent implementations + an inverse round-trip only) -- see DESIGN.md.
+ * SplitMix64: the generator's published check sequence for seed 1234567 (tests/golden/splitmix64_seed1234567.txt),
+ * two independent implementations and an inverse round trip of the finaliser.  The shared-random-number mode
+ * (rng_mode 2) is pinned sample by sample against the independent mode (tests/test_oracle_shared.py).
+ * No function is left "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
