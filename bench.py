@@ -35,7 +35,7 @@ ALG_SLOTS_PER_FLIP = {0: 18 * 2 / 4}
 BINDING_PIPE = {0: "fma (IMAD.WIDE)"}
 ALG_BYTES_PER_FLIP = {0: 9 / 8, 1: 9 / 8 + 4}  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch at L=1024 from the ncu --set full capture in
-# profiles/r1c_final_kernels.md (algorithmic: 9N/16 = 603,979,776 B)
+# profiles/r1h_end_of_round.md (algorithmic: 9N/16 = 603,979,776 B)
 NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 57.63e6, 1: 2684.5e6 + 60.9e6}
 
 
