@@ -209,11 +209,26 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
             for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
         }
     }
+    // The two thresholds every draw is compared with live in ordinary registers (row < 2^27, so the OR adds nothing; it
+    // only keeps them out of the uniform register file, which the 19 Philox constants fill: ptxas otherwise reloads
+    // them from the constant bank after every rare-path branch).
+    Thresholds Tr = a.T;
+    Tr.t4 |= row >> 31;
+    Tr.t8 |= row >> 31;
+    PhiloxCommonConst pcr = rng.pc;
+    PhiloxSampleConst psr = rng.ps;
+    if (RNG == 0) {  // likewise the round keys of the last two rounds
+        pcr.k0[5] |= row >> 31;
+        pcr.k0[6] |= row >> 31;
+        psr.k1[5] |= row >> 31;
+        psr.k1[6] |= row >> 31;
+        psr.k1[7] |= row >> 31;
+    }
 #pragma unroll
     for (int k = 0; k < W && RNG != 2; ++k) {
         uint32_t c4, c8, c12;
         if (RNG == 0) {
-            cond_masks_site_packed_philox(rng.pc, rng.ps, row + (uint32_t)k, a.T, c4, c8, c12);
+            cond_masks_site_packed_philox(pcr, psr, row + (uint32_t)k, Tr, c4, c8, c12);
         } else {
             const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
             cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
