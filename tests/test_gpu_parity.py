@@ -307,6 +307,23 @@ def test_zero_sweeps_is_a_no_op(rng_mode):
         g.ising_sweep(-0.1, 1)
 
 
+@pytest.mark.parametrize("L,nsamples,rng_mode", [(64, 1, PHILOX), (6, 1, PHILOX), (8, 32, PHILOX), (10, 32, PHILOX),
+                                                  (8, 64, PHILOX_SHARED), (6, 32, PHILOX_SHARED)])
+def test_64_bit_seed_and_half_sweep_counter_across_2_to_32(L, nsamples, rng_mode):
+    """Philox key and counter are 64-bit quantities split into 32-bit words (R9): a seed with a non-zero high word and a
+    half-sweep counter that crosses 2^32 during the run exercise hi32(seed) ^ sample and hi32(t) in every kernel."""
+    seed = 0xDEADBEEF12345678
+    t0 = 2**32 - 2
+    spins, J = synth.make_spins(L, nsamples, 91), synth.make_couplings(L, nsamples, 92)
+    o, g = make_pair(L, nsamples, rng_mode, spins, J, seed=seed)
+    o.t = t0
+    g.ising_set_t(t0)
+    o.sweep(1 / 1.1, 2)
+    g.ising_sweep(1 / 1.1, 2)
+    assert g.ising_get_t() == t0 + 4 == o.t
+    assert_same_state(o, g, f"L={L} x {nsamples}, mode {rng_mode}, t across 2^32")
+
+
 @pytest.mark.parametrize("rng_mode,kernel", [(PHILOX, 0), (MINSTD, 2)])
 def test_maximum_size_L2048_word_parallel_equals_generic(rng_mode, kernel):
     """L = 2048 is the largest lattice the library accepts (Philox group index < 2^32): 2^33 spins, 1 GiB of spin bits.
