@@ -110,16 +110,24 @@ class Ising:
     spins (nsamples, W), couplings (nsamples, 3, W), W = ceil(L^3/32).
     """
 
-    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device="cuda:0"):
+    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device="cuda:0", workspace=None):
+        """`workspace`: optional caller-owned uint8 CUDA tensor of at least ising_workspace_bytes bytes, 256-byte aligned
+        (default: allocated here)."""
         import torch
 
         self.L, self.nsamples, self.seed, self.rng_mode = L, nsamples, seed, rng_mode
         self.N = L ** 3
         self.W = (self.N + 31) // 32
-        self.device = torch.device(device)
         nbytes = ising_workspace_bytes(L, nsamples, rng_mode)
-        # torch's caching allocator returns 512-byte aligned blocks
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        if workspace is None:
+            self.device = torch.device(device)
+            # torch's caching allocator returns 512-byte aligned blocks
+            workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        else:
+            assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()
+            self.device = workspace.device
+            nbytes = workspace.numel()
+        self.workspace = workspace
         h = C.c_void_p()
         _check(lib().ising_create(L, nsamples, seed, rng_mode, self.workspace.data_ptr(), nbytes, C.byref(h)),
                "ising_create")

@@ -324,6 +324,37 @@ def test_64_bit_seed_and_half_sweep_counter_across_2_to_32(L, nsamples, rng_mode
     assert_same_state(o, g, f"L={L} x {nsamples}, mode {rng_mode}, t across 2^32")
 
 
+@pytest.mark.parametrize("L,nsamples,rng_mode,kernel", [(64, 1, PHILOX, 0), (128, 1, MINSTD, 0), (512, 1, MINSTD, 0), (64, 1, MINSTD, 2),
+                                                         (6, 1, PHILOX, 0), (16, 1, MINSTD, 0), (64, 1, PHILOX, 1), (8, 32, PHILOX, 0),
+                                                         (6, 32, MINSTD, 0), (16, 64, PHILOX, 1), (8, 64, PHILOX_SHARED, 0),
+                                                         (6, 32, PHILOX_SHARED, 0)])
+def test_no_kernel_writes_outside_the_workspace(L, nsamples, rng_mode, kernel):
+    """Memory safety without a sanitizer: the workspace sits between two guard regions of 1 MiB filled with a pattern,
+    and so do the output buffers; every entry point runs; the guards must be untouched."""
+    nbytes = binding.ising_workspace_bytes(L, nsamples, rng_mode)
+    G = 1 << 20
+    buf = torch.full((G + nbytes + G,), 0xA5, dtype=torch.uint8, device="cuda")
+    W = (L**3 + 31) // 32
+    out = torch.full((G // 4 + nsamples * W + G // 4,), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    spins, J = synth.make_spins(L, nsamples, 95), synth.make_couplings(L, nsamples, 96)
+    g = Ising(L, nsamples, SEED, rng_mode, workspace=buf[G:G + nbytes])
+    g.ising_set_kernel(kernel)
+    g.ising_load_state(dev(spins), dev(J))
+    g.ising_sweep(1 / 1.1, 2)
+    E, M = g.ising_sweep_trace(1 / 1.1, 1, every_half_sweeps=1)
+    g.ising_energy()
+    g.ising_get_spins(out[G // 4:G // 4 + nsamples * W])
+    torch.cuda.synchronize()
+    assert bool((buf[:G] == 0xA5).all()) and bool((buf[G + nbytes:] == 0xA5).all()), "workspace guard overwritten"
+    assert bool((out[:G // 4] == 0x5A5A5A5A).all()) and bool((out[G // 4 + nsamples * W:] == 0x5A5A5A5A).all()), "output guard"
+    # and the run is the same as with a private workspace
+    ref = Ising(L, nsamples, SEED, rng_mode)
+    ref.ising_set_kernel(kernel)
+    ref.ising_load_state(dev(spins), dev(J))
+    ref.ising_sweep(1 / 1.1, 3)
+    assert torch.equal(ref.ising_get_spins().flatten(), out[G // 4:G // 4 + nsamples * W])
+
+
 @pytest.mark.parametrize("rng_mode,kernel", [(PHILOX, 0), (MINSTD, 2)])
 def test_maximum_size_L2048_word_parallel_equals_generic(rng_mode, kernel):
     """L = 2048 is the largest lattice the library accepts (Philox group index < 2^32): 2^33 spins, 1 GiB of spin bits.
