@@ -402,6 +402,26 @@ def test_sample_packed_vector_kernel_equals_scalar_kernel(L, nsamples, rng_mode)
     assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
 
 
+@pytest.mark.parametrize("rng_mode,nsamples", [(PHILOX, 32), (PHILOX_SHARED, 32), (PHILOX_SHARED, 96)])
+def test_sample_packed_L256_vector_kernels_equal_scalar_kernel(rng_mode, nsamples):
+    """The largest sample-packed sizes bench.py times (L = 256 x 32 samples and more): the 128-bit-load kernels (default)
+    against the scalar-load kernel (kernel choice 1) over one sweep (the scalar kernel is compared with the oracle at
+    small sizes)."""
+    L = 256
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    W = L**3 // 32
+    d_spins = torch.randint(-2**31, 2**31 - 1, (nsamples * W,), dtype=torch.int32, device="cuda", generator=gen)
+    d_J = torch.randint(-2**31, 2**31 - 1, (nsamples * 3 * W,), dtype=torch.int32, device="cuda", generator=gen)
+    a = Ising(L, nsamples, SEED, rng_mode)
+    b = Ising(L, nsamples, SEED, rng_mode)
+    b.ising_set_kernel(1)
+    for g in (a, b):
+        g.ising_load_state(d_spins, d_J)
+        g.ising_sweep(1 / 1.1, 1)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
+
+
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
 def test_sample_packed_large_lattice_one_thread_per_group(rng_mode):
     """L = 128 x 32 samples has more than 148 x 1024 Philox groups, so the one-thread-per-group variant of the
