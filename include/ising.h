@@ -63,7 +63,7 @@ typedef struct ising ising_t; /* opaque */
 /* Size in bytes of the device workspace ising_create needs for (L, nsamples, rng_mode): the internal spin and
  * coupling arrays (8 bit arrays per lattice), a canonical staging area used by
  * ising_run_host, the int64 accumulators of the measurement kernel and, in MINSTD mode with nsamples = 1 and
- * L = 64*2^k, a table of the per-site seed states s0 (4 bytes per site, R11).  No PRNG *state* is stored: both
+ * L a multiple of 64, a table of the per-site seed states s0 (4 bytes per site, R11).  No PRNG *state* is stored: both
  * generators are evaluated statelessly from (seed, sample, site, t) (R9, R12); the table only caches the
  * time-independent SplitMix64 seeding of the MINSTD streams and is filled by the first sweep call. */
 int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out);

@@ -29,7 +29,7 @@ struct Geometry {
     size_t staging_words;       // canonical spins + couplings of all samples
     size_t acc_bytes;
     size_t s0_words;            // cached MINSTD seed states: 32 words per word of each colour array (fast layout only)
-    bool fast;                  // half-rows are whole words and L = 64*2^k
+    bool fast;                  // half-rows are whole words: L is a multiple of 64
     int W;                      // words per thread of the word-parallel kernel (fast layout)
 };
 
@@ -49,11 +49,13 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
     // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs and the ticket of the word-parallel energy kernel
     g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1) * sizeof(unsigned long long), 256);
-    g->fast = nsamples == 1 && L >= 64 && (L & (L - 1)) == 0;
-    g->s0_words = g->fast ? (size_t)g->N : 0;  // 2 colours x N/2 sites x 4 bytes
+    g->fast = nsamples == 1 && L % 64 == 0;
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
     // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
-    g->W = (g->fast && (L >> 6) >= 8) ? 4 : 1;
+    g->W = (g->fast && (L >> 6) >= 8 && (L >> 6) % 4 == 0) ? 4 : 1;
+    // cached MINSTD seed states: 2 colours x one 4-byte word per site of every thread of the word-parallel grid (rows
+    // whose lane count is not a power of two are padded, RowMap in sweep_kernels.cuh); N words when L = 64*2^k
+    g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
     return true;
 }
 
@@ -206,8 +208,8 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = g.W;
-            const int tpr = wpr / W;
-            const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
+            const int tpr_pad = row_map_tpr_pad(wpr / W);
+            const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
             SiteRng sr;
             sr.pc = r.pc;
             sr.ps = r.ps[0];
@@ -267,8 +269,8 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
             for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
         }
         m.L = g.L;
-        const int tpr = (g.L >> 6) / g.W;
-        const dim3 grid((unsigned)(g.L / (32 / tpr)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
+        const int tpr_pad = row_map_tpr_pad((g.L >> 6) / g.W);
+        const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
         if (g.W == 4) launch_pdl(energy_site_packed<4>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
         else launch_pdl(energy_site_packed<1>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
         return check_launch(h);

@@ -32,7 +32,7 @@ __device__ __forceinline__ uint32_t spread_to_even_bits(uint32_t v)
     return v;
 }
 
-// Site-packed, L = 64*2^k.  A canonical row (fixed y,z) is L/32 words; its even-x bits belong to colour p = (y+z)&1
+// Site-packed, L a multiple of 64.  A canonical row (fixed y,z) is L/32 words; its even-x bits belong to colour p = (y+z)&1
 // and its odd-x bits to colour 1-p.  One thread de-interleaves canonical words 2k, 2k+1 of a row into word k of the
 // half-row of both colours, for `narrays` canonical bit arrays at once (spins, Jx, Jy, Jz).
 struct SplitArgs {
@@ -50,8 +50,8 @@ __global__ void __launch_bounds__(256) split_colours_site_packed(const SplitArgs
     const uint64_t n = (uint64_t)wpr * L * L;
     const uint64_t widx = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * V;
     if (widx >= n) return;
-    const uint64_t r = widx / (unsigned)wpr;               // L is a power of two here: shifts
-    const int p = (int)((r & (L - 1)) + (r / (unsigned)L)) & 1;
+    const uint64_t r = widx / (unsigned)wpr;
+    const int p = (int)((r % (unsigned)L) + (r / (unsigned)L)) & 1;
     for (int q = 0; q < a.narrays; ++q) {
         uint32_t c[2 * V], even[V], odd[V];
         const Vec lo = __ldcs(reinterpret_cast<const Vec *>(a.canon[q] + 2 * widx));
@@ -81,7 +81,7 @@ merge_colours_site_packed(const uint32_t *__restrict__ S0, const uint32_t *__res
     const uint64_t widx = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * V;
     if (widx >= n) return;
     const uint64_t r = widx / (unsigned)wpr;
-    const int p = (int)((r & (L - 1)) + (r / (unsigned)L)) & 1;
+    const int p = (int)((r % (unsigned)L) + (r / (unsigned)L)) & 1;
     const Vec ve = *reinterpret_cast<const Vec *>((p ? S1 : S0) + widx);
     const Vec vo = *reinterpret_cast<const Vec *>((p ? S0 : S1) + widx);
     uint32_t out[2 * V];

@@ -51,7 +51,7 @@ __device__ __forceinline__ void block_accumulate2(unsigned long long a, unsigned
     }
 }
 
-// Site-packed, L = 64*2^k: the thread mapping of the half-sweep kernel (a thread owns W consecutive words of a half-row,
+// Site-packed, L a multiple of 64: the thread mapping of the half-sweep kernel (a thread owns W consecutive words of a half-row,
 // for both colours).  The +x neighbour of the colour-c site with bit m is bit m (xodd = 0) or bit m+1 (xodd = 1) of the
 // other colour's half-row (a funnel shift by xodd; the bit entering at the end of the thread's words comes from the
 // next lane of the row); +y / +z neighbours are the same bit one row up.  Every word is read once from HBM with 128-bit
@@ -64,17 +64,14 @@ __global__ void __launch_bounds__(SWEEP_THREADS)
 energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {unsatisfied bonds, up spins}, then the ticket */,
                    long long N, long long *E, long long *M)
 {
-    const int L = a.L, wpr = L >> 6, tpr = wpr / W;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int lane_in_row = lane & (tpr - 1);
-    const int y = blockIdx.x * (32 / tpr) + lane / tpr;
-    const int z = blockIdx.y * (SWEEP_THREADS / 32) + warp;
-    const int k0 = lane_in_row * W;
-    const int yp = (y + 1) & (L - 1), zp = (z + 1) & (L - 1);
+    const int L = a.L, wpr = L >> 6;
+    const RowMap rm = row_map<W>(L);
+    const int tpr = rm.tpr, y = rm.y, z = rm.z, k0 = rm.k0;
+    const int yp = y + 1 == L ? 0 : y + 1, zp = z + 1 == L ? 0 : z + 1;
     const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;
     const uint32_t row_yp = (uint32_t)wpr * ((uint32_t)yp + (uint32_t)L * z) + k0;
     const uint32_t row_zp = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zp) + k0;
-    const int next_lane = (lane & ~(tpr - 1)) | ((lane_in_row + 1) & (tpr - 1));
+    const int next_lane = rm.next_lane;
     unsigned int unsat = 0, up = 0;
     wait_for_previous_kernel();
 #pragma unroll
@@ -93,8 +90,10 @@ energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {
 #pragma unroll
         for (int k = 0; k < W; ++k) {
             const uint32_t nx = __funnelshift_r(o[k], (k + 1 < W) ? o[(k + 1) % W] : edge, xodd);
-            unsat += __popc(jx[k] ^ s[k] ^ nx) + __popc(jy[k] ^ s[k] ^ oyp[k]) + __popc(jz[k] ^ s[k] ^ ozp[k]);
-            up += __popc(s[k]);
+            if (rm.active) {  // idle lanes of a padded row shadow lane 0: count nothing twice
+                unsat += __popc(jx[k] ^ s[k] ^ nx) + __popc(jy[k] ^ s[k] ^ oyp[k]) + __popc(jz[k] ^ s[k] ^ ozp[k]);
+                up += __popc(s[k]);
+            }
         }
     }
     block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));

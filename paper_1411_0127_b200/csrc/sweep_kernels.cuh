@@ -4,7 +4,7 @@
 // the colour rank j = (x>>1) + (L/2)*(y + L*z)  (the same j that keys the Philox counter, R9).  Per lattice there are
 // 8 bit arrays indexed by j: spins S[c] and couplings Jd[c], d = x,y,z, where Jd[c] holds the bond (i, i+d-hat) of
 // the colour-c site i.
-//   site-packed   (nsamples = 1):  bit (j&31) of word (j>>5); for L = 64*2^k a half-row (fixed y,z) is L/64 words.
+//   site-packed   (nsamples = 1):  bit (j&31) of word (j>>5); for L a multiple of 64 a half-row (fixed y,z) is L/64 words.
 //   sample-packed (nsamples = 32k): word j of batch b holds samples 32b..32b+31 of site j.
 // An active site of colour c in a row of parity p = (y+z)&1 has x = 2m + xodd, xodd = c^p.  Its +-y and +-z neighbours
 // have the same m in the other colour's arrays; its two x-neighbours are bits m and m-1 (xodd = 0) or m and m+1
@@ -47,7 +47,7 @@ struct SweepArgs {
 };
 
 // ---------------------------------------------------------------------------------------------------
-// Word-parallel kernel, site-packed, L = 64 * 2^k.  One thread owns W consecutive words of one half-row
+// Word-parallel kernel, site-packed, L a multiple of 64.  One thread owns W consecutive words of one half-row
 // (W = 4: one 128-bit load per operand array); TPR = (L/64)/W consecutive lanes own a row, and the bit that crosses
 // a word boundary in x comes from the neighbouring lane by a warp shuffle (or from the thread's own words when it
 // owns the whole row).  A warp covers 32/TPR consecutive y, the 8 warps of a CTA cover 8 consecutive z, so most
@@ -110,22 +110,55 @@ __device__ __forceinline__ void shared_cond_words(const uint32_t R[4], const Thr
     }
 }
 
+// Thread mapping of the word-parallel kernels (half-sweep, seed table, energy), any L that is a multiple of 64: a row of
+// wpr = L/64 words is owned by tpr = wpr/W consecutive lanes.  When tpr is not a power of two (L = 192, 320, 384, ...)
+// the row is padded to tpr_pad = the next power of two lanes; the idle lanes shadow lane 0 of the row (their loads stay
+// in bounds) and store nothing.  grid = (L / (32 / tpr_pad), L / 8), 256 threads.
+struct RowMap {
+    int lane, warp, tpr, tpr_pad, lane_in_row, y, z, k0;
+    int next_lane, prev_lane;  // lanes owning the next / previous words of the row (periodic)
+    bool active;
+};
+
+inline int row_map_tpr_pad(int tpr)
+{
+    int p = 1;
+    while (p < tpr) p <<= 1;
+    return p;
+}
+
+template <int W>
+__device__ __forceinline__ RowMap row_map(int L)
+{
+    RowMap m;
+    m.tpr = (L >> 6) / W;
+    const int lg = m.tpr <= 1 ? 0 : 32 - __clz(m.tpr - 1);
+    m.tpr_pad = 1 << lg;
+    m.lane = threadIdx.x & 31;
+    m.warp = threadIdx.x >> 5;
+    const int lir = m.lane & (m.tpr_pad - 1);
+    m.active = lir < m.tpr;
+    m.lane_in_row = m.active ? lir : 0;
+    m.y = blockIdx.x * (32 >> lg) + (m.lane >> lg);
+    m.z = blockIdx.y * (SWEEP_THREADS / 32) + m.warp;
+    m.k0 = m.lane_in_row * W;
+    const int base = m.lane & ~(m.tpr_pad - 1);
+    m.next_lane = base | (m.lane_in_row + 1 == m.tpr ? 0 : m.lane_in_row + 1);
+    m.prev_lane = base | (m.lane_in_row == 0 ? m.tpr - 1 : m.lane_in_row - 1);
+    return m;
+}
+
 template <int RNG, int W>
 __global__ void __launch_bounds__(SWEEP_THREADS)
 half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng)
 {
     const int L = a.L;
     const int wpr = L >> 6;                 // words per half-row
-    const int tpr = wpr / W;                // threads (lanes) per row: power of two <= 32
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int rows_per_warp = 32 / tpr;
-    const int lane_in_row = lane & (tpr - 1);
-    const int y = blockIdx.x * rows_per_warp + lane / tpr;
-    const int z = blockIdx.y * (SWEEP_THREADS / 32) + warp;
-    const int k0 = lane_in_row * W;
+    const RowMap rm = row_map<W>(L);
+    const int tpr = rm.tpr, lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z, k0 = rm.k0;
 
-    const int yp = (y + 1) & (L - 1), ym = (y - 1) & (L - 1);
-    const int zp = (z + 1) & (L - 1), zm = (z - 1) & (L - 1);
+    const int yp = y + 1 == L ? 0 : y + 1, ym = y == 0 ? L - 1 : y - 1;
+    const int zp = z + 1 == L ? 0 : z + 1, zm = z == 0 ? L - 1 : z - 1;
     const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;   // < 2^27 words for L <= 2048
     const uint32_t row_yp = (uint32_t)wpr * ((uint32_t)yp + (uint32_t)L * z) + k0;
     const uint32_t row_ym = (uint32_t)wpr * ((uint32_t)ym + (uint32_t)L * z) + k0;
@@ -160,10 +193,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
 #pragma unroll
         for (int k = 0; k < W; ++k) B[k] = jxo[k] ^ o[k];
         uint32_t edge = xodd ? o[0] : B[W - 1];
-        if (tpr > 1) {
-            const int src = (lane & ~(tpr - 1)) | ((lane_in_row + (xodd ? 1 : tpr - 1)) & (tpr - 1));
-            edge = __shfl_sync(0xFFFFFFFFu, edge, src);
-        }
+        if (tpr > 1) edge = __shfl_sync(0xFFFFFFFFu, edge, xodd ? rm.next_lane : rm.prev_lane);
         const uint32_t sh_r = (uint32_t)xodd, sh_l = 1u - (uint32_t)xodd;
 #pragma unroll
         for (int k = 0; k < W; ++k) {
@@ -241,19 +271,15 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     uint32_t *po = reinterpret_cast<uint32_t *>(&out);
 #pragma unroll
     for (int k = 0; k < W; ++k) po[k] = s[k];
-    *reinterpret_cast<V *>(a.S_act + row) = out;
+    if (rm.active) *reinterpret_cast<V *>(a.S_act + row) = out;
 }
 
 // Fills the seed table of colour `colour` with the thread mapping of half_sweep_site_packed<2, W> (same grid).
 template <int W>
 __global__ void __launch_bounds__(SWEEP_THREADS) minstd_fill_s0(uint4 *tab, int L, int colour, uint64_t seed)
 {
-    const int wpr = L >> 6, tpr = wpr / W;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int lane_in_row = lane & (tpr - 1);
-    const int y = blockIdx.x * (32 / tpr) + lane / tpr;
-    const int z = blockIdx.y * (SWEEP_THREADS / 32) + warp;
-    const int k0 = lane_in_row * W;
+    const RowMap rm = row_map<W>(L);
+    const int lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z, k0 = rm.k0;
     const int xodd = (y + z + colour) & 1;
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;
     const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;

@@ -232,6 +232,43 @@ def test_word_parallel_kernel_equals_generic_kernel(L, rng_mode):
     assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
 
 
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L", [192, 320])
+def test_word_parallel_layout_for_L_not_a_power_of_two_equals_the_oracle(L, rng_mode):
+    """L = 192, 320 (multiples of 64 that are not powers of two: rows of 3 and 5 words, padded to 4 and 8 lanes):
+    layout round trip, trajectory, energy and magnetisation against the oracle."""
+    spins, J = synth.make_spins(L, 1, 33), synth.make_couplings(L, 1, 34)
+    o, g = make_pair(L, 1, rng_mode, spins, J)
+    assert np.array_equal(host_u32(g.ising_get_spins())[0], spins.reshape(-1))
+    assert_same_state(o, g, f"L={L} loaded")
+    for beta, n in ((1 / 1.1, 2), (1 / 0.7, 1)):
+        o.sweep(beta, n)
+        g.ising_sweep(beta, n)
+        assert_same_state(o, g, f"L={L} rng {rng_mode} beta {beta}")
+
+
+@pytest.mark.parametrize("rng_mode,kernel", [(PHILOX, 0), (MINSTD, 0), (MINSTD, 2)])
+@pytest.mark.parametrize("L", [192, 384, 576, 768, 1280])
+def test_word_parallel_kernel_equals_generic_kernel_for_any_multiple_of_64(L, rng_mode, kernel):
+    """Rows of 3, 6, 9 words (one word per thread, 4 / 8 / 16 lanes per row) and of 12 and 20 words (four words per
+    thread, 3 and 5 lanes per row padded to 4 and 8)."""
+    W = L**3 // 32
+    gen = torch.Generator(device="cuda").manual_seed(L)
+    d_spins = torch.randint(-2**31, 2**31 - 1, (W,), dtype=torch.int32, device="cuda", generator=gen)
+    d_J = torch.randint(-2**31, 2**31 - 1, (3 * W,), dtype=torch.int32, device="cuda", generator=gen)
+    a = Ising(L, 1, SEED, rng_mode)
+    a.ising_set_kernel(kernel)
+    b = Ising(L, 1, SEED, rng_mode)
+    b.ising_set_kernel(1)
+    for g in (a, b):
+        g.ising_load_state(d_spins, d_J)
+        g.ising_sweep(1 / 1.1, 2)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    Ea, Ma = a.ising_energy()
+    Eb, Mb = b.ising_energy()
+    assert torch.equal(Ea, Eb) and torch.equal(Ma, Mb)
+
+
 @pytest.mark.parametrize("L", [64, 128, 256, 512])
 def test_minstd_cached_seed_table_equals_recomputed_seeds(L):
     """MINSTD: the default word-parallel kernel streams the seed states s0 from a table filled once per handle; kernel
