@@ -32,6 +32,7 @@ BETA = 1.0 / 1.1
 #   Philox: fma pipe.  18 wide multiplies per call of 4 sites, IMAD.WIDE = 2 passes of the 32-bit multiplier -> 9.0 slots
 #   MINSTD with the cached seed table (the shipped variant): HBM-bound, 9/8 B of lattice + 4 B of seed state per flip
 ALG_SLOTS_PER_FLIP = {0: 18 * 2 / 4}
+ALG_INT_OPS_PER_FLIP = 37 / 4 + 2 + 22 / 32
 BINDING_PIPE = {0: "fma (IMAD.WIDE)"}
 ALG_BYTES_PER_FLIP = {0: 9 / 8, 1: 9 / 8 + 4}  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch at L=1024 from the ncu --set full capture in
@@ -338,6 +339,12 @@ def main():
             "bound": "alu", "achieved": slot_rate, "peak": peak, "unit": "Tinst/s", "frac": slot_rate / peak, **common,
             "binding_pipe": BINDING_PIPE[rng_mode], "alg_slots_per_flip": ALG_SLOTS_PER_FLIP[rng_mode],
             "roofline_ps_per_flip": 1e12 * ALG_SLOTS_PER_FLIP[rng_mode] / (peak * 1e12),
+            # BASELINE.json's wording, "integer ops per flip (PRNG + field logic) at the INT32 issue rate": all 11.94 algorithmic
+            # integer instructions per flip attempt (37/4 Philox + 2 acceptance + 22/32 field) against one 16-lane pipe per
+            # SMSP (the measured LOP3 / IMAD rate) and against both pipes issuing together (the warp scheduler's limit)
+            "int32_issue_reading": {"alg_int_ops_per_flip": ALG_INT_OPS_PER_FLIP,
+                                    "frac_at_64_lanes_per_sm": ALG_INT_OPS_PER_FLIP * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12 / peak,
+                                    "frac_at_128_lanes_per_sm": ALG_INT_OPS_PER_FLIP * flips_per_launch / (half_sweep_ms * 1e-3) / 1e12 / (2 * peak)},
             "peak_source": f"guide unit counts: 148 SM x 4 SMSP x 16 lanes (rt_SMSP=2) x {sm_max_mhz:.0f} MHz ({peaks_src} max clock), per pipe",
             "hbm": hbm_obj,
         }
