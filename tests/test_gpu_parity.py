@@ -486,6 +486,27 @@ def test_run_host_equals_device_calls():
     assert a.ising_kernel_launches() == 1 + 10 + 1 + 1  # load, 10 half-sweeps, fused energy, get
 
 
+@pytest.mark.parametrize("L,nsamples,rng_mode", [(64, 1, MINSTD), (16, 1, PHILOX), (8, 32, PHILOX), (6, 64, MINSTD),
+                                                  (8, 64, PHILOX_SHARED)])
+def test_run_host_every_layout(L, nsamples, rng_mode):
+    """ising_run_host (host buffers in, host results out) for the word-parallel, generic, sample-packed and shared-draw
+    paths: spins, E and M of every sample against the oracle; without the optional outputs too."""
+    spins, J = synth.make_spins(L, nsamples, 97), synth.make_couplings(L, nsamples, 98)
+    a = Ising(L, nsamples, SEED, rng_mode)
+    hs = torch.from_numpy(spins.view(np.int32)).pin_memory()
+    hJ = torch.from_numpy(J.view(np.int32)).pin_memory()
+    out = torch.empty_like(hs).pin_memory()
+    E, M = a.ising_run_host(hs, hJ, 1 / 1.1, 3, out)
+    o = _loaded(L, nsamples, rng_mode, spins, J)
+    o.sweep(1 / 1.1, 3)
+    assert np.array_equal(out.numpy().view(np.uint32).reshape(nsamples, -1), o.spins_packed())
+    Eo, Mo = o.energy()
+    assert np.array_equal(E.numpy(), Eo) and np.array_equal(M.numpy(), Mo)
+    a.ising_set_t(0)
+    E2, _ = a.ising_run_host(hs, hJ, 1 / 1.1, 3, None)  # same job again, spins not wanted
+    assert np.array_equal(E2.numpy(), Eo)
+
+
 # ------------------------------------------------------------------------------------------------ config 5, full size
 
 def _avail_gib():
