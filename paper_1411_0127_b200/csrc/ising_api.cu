@@ -52,7 +52,15 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->fast = nsamples == 1 && L % 64 == 0;
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
     // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
-    g->W = (g->fast && (L >> 6) >= 8 && (L >> 6) % 4 == 0) ? 4 : 1;
+    g->W = 1;
+    if (g->fast) {
+        const int wpr = L >> 6;
+        int odd = wpr;
+        while (odd % 2 == 0) odd /= 2;
+        if (odd == 3 || odd == 5) g->W = odd;  // rows of 3 * 2^e or 5 * 2^e words: 3 or 5 words per thread, no idle lanes
+        else if (odd == 1 && wpr >= 8) g->W = 4;
+        // other odd parts (7, 9, 11, ...): one word per thread, the row padded to a power of two of lanes
+    }
     // cached MINSTD seed states: 2 colours x one 4-byte word per site of every thread of the word-parallel grid (rows
     // whose lane count is not a power of two are padded, RowMap in sweep_kernels.cuh); N words when L = 64*2^k
     g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
@@ -222,7 +230,8 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 if (!h->s0_ready) {  // once per handle: the seed states depend on (seed, site) only (R11)
                     for (int cc = 0; cc < 2; ++cc) {
                         if (W == 4) minstd_fill_s0<4><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
-                        else if (W == 2) minstd_fill_s0<2><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                        else if (W == 3) minstd_fill_s0<3><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                        else if (W == 5) minstd_fill_s0<5><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
                         else minstd_fill_s0<1><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
                     }
                     const int rc = check_launch(h, 2);
@@ -231,10 +240,12 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 }
                 sr.s0tab = tab[c];
                 if (W == 4) launch_pdl(half_sweep_site_packed<2, 4>, grid, dim3(SWEEP_THREADS), st, a, sr);
-                else if (W == 2) launch_pdl(half_sweep_site_packed<2, 2>, grid, dim3(SWEEP_THREADS), st, a, sr);
+                else if (W == 3) launch_pdl(half_sweep_site_packed<2, 3>, grid, dim3(SWEEP_THREADS), st, a, sr);
+                else if (W == 5) launch_pdl(half_sweep_site_packed<2, 5>, grid, dim3(SWEEP_THREADS), st, a, sr);
                 else launch_pdl(half_sweep_site_packed<2, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
             } else if (W == 4) launch_pdl(half_sweep_site_packed<RNG, 4>, grid, dim3(SWEEP_THREADS), st, a, sr);
-            else if (W == 2) launch_pdl(half_sweep_site_packed<RNG, 2>, grid, dim3(SWEEP_THREADS), st, a, sr);
+            else if (W == 3) launch_pdl(half_sweep_site_packed<RNG, 3>, grid, dim3(SWEEP_THREADS), st, a, sr);
+            else if (W == 5) launch_pdl(half_sweep_site_packed<RNG, 5>, grid, dim3(SWEEP_THREADS), st, a, sr);
             else launch_pdl(half_sweep_site_packed<RNG, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
@@ -272,6 +283,8 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         const int tpr_pad = row_map_tpr_pad((g.L >> 6) / g.W);
         const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
         if (g.W == 4) launch_pdl(energy_site_packed<4>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
+        else if (g.W == 3) launch_pdl(energy_site_packed<3>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
+        else if (g.W == 5) launch_pdl(energy_site_packed<5>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
         else launch_pdl(energy_site_packed<1>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
         return check_launch(h);
     }

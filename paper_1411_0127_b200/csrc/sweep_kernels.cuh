@@ -60,15 +60,45 @@ template <int W> struct WordVec;
 template <> struct WordVec<1> { typedef uint32_t type; };
 template <> struct WordVec<2> { typedef uint2 type; };
 template <> struct WordVec<4> { typedef uint4 type; };
+template <int W> struct IsVectorWidth { static constexpr bool value = W == 1 || W == 2 || W == 4; };
+
+// W = 3 or 5 words per thread (rows of 3 * 2^e or 5 * 2^e words, L = 192, 320, 384, 640, 768, 1280, ...): the thread's
+// words are not a power-of-two vector, so they move as W 32-bit accesses.
+template <int W>
+__device__ __forceinline__ void load_words_scalar(const uint32_t *__restrict__ p, size_t word_off, uint32_t out[W])
+{
+#pragma unroll
+    for (int k = 0; k < W; ++k) out[k] = __ldg(p + word_off + k);
+}
 
 template <int W>
 __device__ __forceinline__ void load_words(const uint32_t *__restrict__ p, size_t word_off, uint32_t out[W])
 {
-    typedef typename WordVec<W>::type V;
-    const V v = __ldg(reinterpret_cast<const V *>(p + word_off));
-    const uint32_t *pv = reinterpret_cast<const uint32_t *>(&v);
+    if constexpr (!IsVectorWidth<W>::value) {
+        load_words_scalar<W>(p, word_off, out);
+    } else {
+        typedef typename WordVec<W>::type V;
+        const V v = __ldg(reinterpret_cast<const V *>(p + word_off));
+        const uint32_t *pv = reinterpret_cast<const uint32_t *>(&v);
 #pragma unroll
-    for (int k = 0; k < W; ++k) out[k] = pv[k];
+        for (int k = 0; k < W; ++k) out[k] = pv[k];
+    }
+}
+
+template <int W>
+__device__ __forceinline__ void store_words(uint32_t *p, size_t word_off, const uint32_t in[W])
+{
+    if constexpr (!IsVectorWidth<W>::value) {
+#pragma unroll
+        for (int k = 0; k < W; ++k) p[word_off + k] = in[k];
+    } else {
+        typedef typename WordVec<W>::type V;
+        V out;
+        uint32_t *po = reinterpret_cast<uint32_t *>(&out);
+#pragma unroll
+        for (int k = 0; k < W; ++k) po[k] = in[k];
+        *reinterpret_cast<V *>(p + word_off) = out;
+    }
 }
 
 struct SiteRng {  // per-launch PRNG constants of the site-packed kernel (one sample)
@@ -266,12 +296,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
         s[k] ^= flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
     }
 
-    typedef typename WordVec<W>::type V;
-    V out;
-    uint32_t *po = reinterpret_cast<uint32_t *>(&out);
-#pragma unroll
-    for (int k = 0; k < W; ++k) po[k] = s[k];
-    if (rm.active) *reinterpret_cast<V *>(a.S_act + row) = out;
+    if (rm.active) store_words<W>(a.S_act, row, s);
 }
 
 // Fills the seed table of colour `colour` with the thread mapping of half_sweep_site_packed<2, W> (same grid).

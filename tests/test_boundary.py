@@ -61,7 +61,7 @@ def test_argument_validation_without_a_gpu():
     assert lib.ising_workspace_bytes(16, 32, 2, C.byref(out)) == binding.OK
     assert lib.ising_workspace_bytes(16, 1, 0, None) == binding.EINVAL
     # sizes: 8 internal bit arrays + canonical staging + accumulators
-    for L, ns in ((16, 1), (64, 32), (256, 1), (1024, 1), (6, 1), (4, 64), (192, 1), (768, 1)):
+    for L, ns in ((16, 1), (64, 32), (256, 1), (1024, 1), (6, 1), (4, 64), (192, 1), (768, 1), (448, 1), (576, 1)):
         nbytes = binding.ising_workspace_bytes(L, ns, 0)
         N = L**3
         assert nbytes >= ns * (N // 8) * 8 and nbytes % 256 == 0
@@ -69,13 +69,15 @@ def test_argument_validation_without_a_gpu():
         # (word-parallel layout: L a multiple of 64; rows whose lane count is not a power of two are padded)
         table = 0
         if ns == 1 and L % 64 == 0:
-            wpr = L // 64
-            W = 4 if wpr >= 8 and wpr % 4 == 0 else 1
+            wpr = odd = L // 64
+            while odd % 2 == 0:
+                odd //= 2
+            W = odd if odd in (3, 5) else (4 if odd == 1 and wpr >= 8 else 1)  # words per thread
             pad = 1
             while pad < wpr // W:
                 pad *= 2
             table = 4 * 2 * L * L * pad * W * 32
-            assert table >= 4 * N and (table == 4 * N) == (L & (L - 1) == 0)
+            assert table >= 4 * N and (table == 4 * N) == (odd in (1, 3, 5))
         assert binding.ising_workspace_bytes(L, ns, 1) == nbytes + table
     assert binding.ising_workspace_bytes(1024, 1, 0) < 1100 * 2**20
     h = C.c_void_p()

@@ -235,7 +235,7 @@ def test_word_parallel_kernel_equals_generic_kernel(L, rng_mode):
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
 @pytest.mark.parametrize("L", [192, 320])
 def test_word_parallel_layout_for_L_not_a_power_of_two_equals_the_oracle(L, rng_mode):
-    """L = 192, 320 (multiples of 64 that are not powers of two: rows of 3 and 5 words, padded to 4 and 8 lanes):
+    """L = 192, 320 (multiples of 64 that are not powers of two: rows of 3 and 5 words, one thread per row):
     layout round trip, trajectory, energy and magnetisation against the oracle."""
     spins, J = synth.make_spins(L, 1, 33), synth.make_couplings(L, 1, 34)
     o, g = make_pair(L, 1, rng_mode, spins, J)
@@ -248,10 +248,10 @@ def test_word_parallel_layout_for_L_not_a_power_of_two_equals_the_oracle(L, rng_
 
 
 @pytest.mark.parametrize("rng_mode,kernel", [(PHILOX, 0), (MINSTD, 0), (MINSTD, 2)])
-@pytest.mark.parametrize("L", [192, 384, 576, 768, 1280])
+@pytest.mark.parametrize("L", [192, 320, 384, 448, 576, 768, 1280])
 def test_word_parallel_kernel_equals_generic_kernel_for_any_multiple_of_64(L, rng_mode, kernel):
-    """Rows of 3, 6, 9 words (one word per thread, 4 / 8 / 16 lanes per row) and of 12 and 20 words (four words per
-    thread, 3 and 5 lanes per row padded to 4 and 8)."""
+    """Rows of 3, 6, 12 words (three words per thread, 1 / 2 / 4 lanes per row), of 5 and 20 words (five words per thread)
+    and of 7 and 9 words (one word per thread, the row padded to 8 and 16 lanes, idle lanes store nothing)."""
     W = L**3 // 32
     gen = torch.Generator(device="cuda").manual_seed(L)
     d_spins = torch.randint(-2**31, 2**31 - 1, (W,), dtype=torch.int32, device="cuda", generator=gen)
