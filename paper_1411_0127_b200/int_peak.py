@@ -16,9 +16,16 @@ SRC = os.path.join(HERE, "csrc", "int_peak.cu")
 LIB = os.path.join(HERE, "libint_peak.so")
 MIXES = {0: "LOP3 only", 1: "IMAD.WIDE.U32 only", 2: "IMAD.WIDE + LOP3 dependent 1:1", 3: "Philox round (2 IMAD.WIDE + 2 LOP3)",
          4: "ISETP + SEL + LOP3", 5: "IMAD.HI.U32 only", 6: "IMAD (lo) only", 7: "Philox round + 1 LOP3", 8: "Philox round + 2 LOP3",
-         9: "Philox round + 3 LOP3", 10: "Philox round + 4 LOP3", 11: "Philox round via DFMA.RM (hi) + IMAD (lo)"}
+         9: "Philox round + 3 LOP3", 10: "Philox round + 4 LOP3", 11: "Philox round via DFMA.RM (hi) + IMAD (lo)",
+         12: "IMAD (lo) + LOP3 1:1 independent", 13: "FFMA only", 14: "FFMA + LOP3 1:1 independent",
+         15: "IMAD (lo) + IADD3 1:1 independent", 16: "IMAD (lo) + FFMA 1:1 independent",
+         17: "IMAD.HI + LOP3 1:1 independent", 18: "IMAD.HI + 3 LOP3 independent", 19: "IMAD.WIDE, multiplier in a register",
+         20: "DFMA only", 21: "DFMA + LOP3 1:1 independent", 22: "IMAD.WIDE + IMAD (lo) 1:1",
+         23: "Philox round from IMAD.HI + IMAD (lo), + 2 LOP3", 24: "Philox round (register multipliers) + 4 LOP3",
+         25: "IMAD.WIDE + FFMA 1:1", 26: "IMAD.WIDE + 3 LOP3 independent",
+         27: "2 Philox rounds via DFMA.RM + IMAD (lo), state in register pairs", 28: "same + 2 x 2 LOP3", 29: "same + 2 x 4 LOP3"}
 # source-level instructions per chain-iteration of each mix (csrc/int_peak.cu)
-OPS = {0: 4, 1: 2, 2: 4, 3: 4, 4: 6, 5: 2, 6: 2, 7: 5, 8: 6, 9: 7, 10: 8, 11: 6}
+OPS = {0: 4, 1: 2, 2: 4, 3: 4, 4: 6, 5: 2, 6: 2, 7: 5, 8: 6, 9: 7, 10: 8, 11: 6, 12: 4, 13: 4, 14: 4, 15: 4, 16: 4, 17: 4, 18: 8, 19: 2, 20: 2, 21: 4, 22: 6, 23: 8, 24: 8, 25: 6, 26: 4, 27: 12, 28: 16, 29: 20}
 
 
 def build(force: bool = False) -> str:
