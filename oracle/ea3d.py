@@ -13,6 +13,7 @@ import numpy as np
 from . import build as _build
 
 PHILOX, MINSTD, PHILOX_SHARED = 0, 1, 2  # PHILOX_SHARED: one draw per 32-sample word (R18)
+PR_LANES, MT_LANES = 3, 4  # shared draw from stored-state generators, one per lane (R19)
 
 _lib = None
 
@@ -49,6 +50,27 @@ def lib():
         L.oracle_site_flips.restype = C.c_int
         L.oracle_fnv1a64.argtypes = [C.c_void_p, C.c_uint64]
         L.oracle_fnv1a64.restype = C.c_uint64
+        L.oracle_pr_next.argtypes = [u32p, u64p]
+        L.oracle_pr_next.restype = C.c_uint32
+        L.oracle_pr_seed.argtypes = [C.c_uint64, C.c_uint64, u32p]
+        L.oracle_pr_seed.restype = None
+        L.oracle_mt_seed.argtypes = [C.c_uint32, u32p]
+        L.oracle_mt_seed.restype = None
+        L.oracle_mt_next.argtypes = [u32p, u64p]
+        L.oracle_mt_next.restype = C.c_uint32
+        L.oracle_mt_lane_seed.argtypes = [C.c_uint64, C.c_uint64]
+        L.oracle_mt_lane_seed.restype = C.c_uint32
+        L.oracle_lane_state_words.argtypes = [C.c_int]
+        L.oracle_lane_state_words.restype = C.c_int
+        L.oracle_lanes_init.argtypes = [C.c_int, C.c_uint64, C.c_int64, u32p, u64p]
+        L.oracle_lanes_init.restype = C.c_int
+        L.oracle_lanes_draw_table.argtypes = [C.c_int, C.c_int64, u32p, u64p, C.c_int64, C.c_int, u32p]
+        L.oracle_lanes_draw_table.restype = C.c_int
+        L.oracle_half_sweep_lanes.argtypes = [C.c_int, C.c_int, i8p, i8p, i8p, i8p, C.c_int, C.c_int64, u32p, u64p,
+                                              C.c_uint64, u64p, u32p, i64p, i64p]
+        L.oracle_half_sweep_lanes.restype = C.c_int
+        L.oracle_count_odd.argtypes = [C.c_int, C.c_uint64, C.c_int64, C.c_int64, u64p, u64p]
+        L.oracle_count_odd.restype = C.c_int
         L.oracle_set_threads.argtypes = [C.c_int]
         L.oracle_get_max_threads.restype = C.c_int
         _lib = L
@@ -87,6 +109,48 @@ def minstd_draw(seed, q, n):
 
 def philox_draw(L, seed, sample, x, y, z, t):
     return int(lib().oracle_philox_draw(L, seed, sample, x, y, z, t))
+
+
+def pr_sequence(seed_words, n):
+    """n draws of the Parisi-Rapuano generator from the 62 seed words ira[0..61]."""
+    ring = np.asarray(seed_words, dtype=np.uint32).copy()
+    assert ring.size == 62
+    nd = C.c_uint64(0)
+    return [int(lib().oracle_pr_next(_p(ring, C.c_uint32), C.byref(nd))) for _ in range(n)]
+
+
+def pr_seed_words(seed, lane):
+    ring = np.zeros(62, dtype=np.uint32)
+    lib().oracle_pr_seed(seed, lane, _p(ring, C.c_uint32))
+    return ring
+
+
+def mt_sequence(s, n):
+    """n draws of MT19937 seeded by init_genrand(s)."""
+    mt = np.zeros(624, dtype=np.uint32)
+    lib().oracle_mt_seed(s, _p(mt, C.c_uint32))
+    nd = C.c_uint64(0)
+    return [int(lib().oracle_mt_next(_p(mt, C.c_uint32), C.byref(nd))) for _ in range(n)]
+
+
+def mt_state_after_seed(s):
+    mt = np.zeros(624, dtype=np.uint32)
+    lib().oracle_mt_seed(s, _p(mt, C.c_uint32))
+    return mt
+
+
+def mt_lane_seed(seed, lane):
+    return int(lib().oracle_mt_lane_seed(seed, lane))
+
+
+def count_odd(kind, seed, nlanes, ndraws):
+    """(odd[q], sum[q]) of `ndraws` numbers of every lane (Table II)."""
+    odd = np.zeros(nlanes, dtype=np.uint64)
+    sm = np.zeros(nlanes, dtype=np.uint64)
+    rc = lib().oracle_count_odd(kind, seed, nlanes, ndraws, _p(odd, C.c_uint64), _p(sm, C.c_uint64))
+    if rc != 0:
+        raise ValueError("bad arguments")
+    return odd, sm
 
 
 def thresholds(beta, rng_mode):
@@ -151,9 +215,10 @@ def spins_to_packed(sigma: np.ndarray) -> np.ndarray:
 class Oracle:
     """The reference chain: state in int8 arrays, half-sweep counter t, red (even t) then blue."""
 
-    def __init__(self, L: int, nsamples: int, seed: int, rng_mode: int):
+    def __init__(self, L: int, nsamples: int, seed: int, rng_mode: int, nlanes: int | None = None):
         if L < 2 or L % 2:
             raise ValueError("L must be even and >= 2")
+        self.nlanes = None
         self.L, self.nsamples, self.seed, self.rng_mode = L, nsamples, int(seed), int(rng_mode)
         self.N = L ** 3
         self.t = 0
@@ -167,6 +232,16 @@ class Oracle:
         if rng_mode == MINSTD:
             self.minstd_state = np.zeros(nsamples * self.N, dtype=np.uint32)
             lib().oracle_minstd_init(L, nsamples, self.seed, _p(self.minstd_state, C.c_uint32))
+        if rng_mode in (PR_LANES, MT_LANES):
+            if nlanes is None or nlanes < 1 or nsamples % 32 or self.N % 8:
+                raise ValueError("lane modes need nlanes, nsamples = 32k and N a multiple of 8")
+            self.nlanes = int(nlanes)
+            w = lib().oracle_lane_state_words(rng_mode)
+            self.lane_state = np.zeros(self.nlanes * w, dtype=np.uint32)
+            self.lane_ndrawn = np.zeros(self.nlanes, dtype=np.uint64)
+            self.lane_scratch = np.zeros((nsamples // 32) * (self.N // 2), dtype=np.uint32)
+            lib().oracle_lanes_init(rng_mode, self.seed, self.nlanes, _p(self.lane_state, C.c_uint32),
+                                    _p(self.lane_ndrawn, C.c_uint64))
 
     # -- state I/O in the canonical packed format
     def load_packed(self, spins_words: np.ndarray, J_words: np.ndarray):
@@ -190,6 +265,16 @@ class Oracle:
     # -- dynamics
     def half_sweep(self, beta: float):
         T = np.array(thresholds(beta, self.rng_mode), dtype=np.uint64)
+        if self.nlanes is not None:
+            rc = lib().oracle_half_sweep_lanes(self.L, self.nsamples, _p(self.sigma, C.c_int8), _p(self.Jx, C.c_int8),
+                                               _p(self.Jy, C.c_int8), _p(self.Jz, C.c_int8), self.rng_mode, self.nlanes,
+                                               _p(self.lane_state, C.c_uint32), _p(self.lane_ndrawn, C.c_uint64), self.t,
+                                               _p(T, C.c_uint64), _p(self.lane_scratch, C.c_uint32),
+                                               _p(self.dE_sum, C.c_int64), _p(self.stats, C.c_int64))
+            if rc != 0:
+                raise RuntimeError("oracle_half_sweep_lanes failed")
+            self.t += 1
+            return
         ms = _p(self.minstd_state, C.c_uint32) if self.minstd_state is not None else None
         rc = lib().oracle_half_sweep(self.L, self.nsamples, _p(self.sigma, C.c_int8), _p(self.Jx, C.c_int8),
                                      _p(self.Jy, C.c_int8), _p(self.Jz, C.c_int8), self.seed, self.rng_mode,

@@ -20,6 +20,10 @@
  * SplitMix64: the generator's published check sequence for seed 1234567 (tests/golden/splitmix64_seed1234567.txt),
  * two independent implementations and an inverse round trip of the finaliser.  The shared-random-number mode
  * (rng_mode 2) is pinned sample by sample against the independent mode (tests/test_oracle_shared.py).
+ * The stored-state lane generators (rng_mode 3, 4; R19): MT19937 against C++ std::mt19937 (whose 10000th value
+ * the C++ standard fixes) and numpy's legacy RandomState; Parisi-Rapuano against an unbounded-history restatement of the
+ * paper's two lines in the test; the lane-driven sweep against a per-sample run fed with the same
+ * draw table (tests/test_oracle_lanes.py).
  * No function is left "parity unpinned".
  */
 #include <math.h>
@@ -36,6 +40,11 @@
  * one word share ONE random number per (site, half-sweep).  DESIGN.md R18: the shared draw of the samples 32b..32b+31
  * (coded batch b) is the Philox draw of "sample" b, i.e. oracle_philox_draw(..., sample >> 5, ...). */
 #define ORACLE_RNG_PHILOX_SHARED 2
+/* Shared draw per 32-sample word as in mode 2, but the numbers come from generators with STORED state, one per "lane"
+ * (the paper's one generator per thread), R19: Parisi-Rapuano and
+ * MT19937. */
+#define ORACLE_RNG_PR_LANES 3
+#define ORACLE_RNG_MT_LANES 4
 
 /* ------------------------------------------------------------------------------------------ */
 /* Random number generators                                                                    */
@@ -122,11 +131,12 @@ uint32_t oracle_philox_draw(int L, uint64_t seed, int sample, int x, int y, int 
 /* PAPER.md:242 ("R_max exp(-beta dE) = EXP12, EXP8, EXP4") with the scale of DESIGN.md R5/R6:
  *   Philox:  T[dE] = floor(2^32 * exp(-beta*dE))           in [0, 2^32]   (R uniform in [0, 2^32))
  *   MINSTD:  T[dE] = floor((2^31 - 1) * exp(-beta*dE))     in [0, 2^31-1] (R in [1, 2^31-2])
+ *   Parisi-Rapuano and MT19937 give uniform 32-bit words: the Philox scale.
  * T[0],T[1],T[2] are for dE = 4, 8, 12.  Returns 0, or -1 for beta < 0 / NaN / unknown mode. */
 int oracle_thresholds(double beta, int rng_mode, uint64_t T[3])
 {
     if (!(beta >= 0.0)) return -1;
-    if (rng_mode != ORACLE_RNG_PHILOX && rng_mode != ORACLE_RNG_MINSTD && rng_mode != ORACLE_RNG_PHILOX_SHARED) return -1;
+    if (rng_mode < ORACLE_RNG_PHILOX || rng_mode > ORACLE_RNG_MT_LANES) return -1;
     for (int k = 0; k < 3; ++k) {
         double dE = 4.0 * (double)(k + 1);
         double x = beta * dE;
@@ -219,12 +229,13 @@ void oracle_minstd_init(int L, int nsamples, uint64_t seed, uint32_t *state)
  *   stats[0..10] : += {proposals, accepted, accepted with dE > 0, proposals with dE outside Eq. 8,
  *                      histogram of proposals over dE = -12,-8,-4,0,4,8,12 (stats[4..10])}
  * Returns 0, or -1 on bad arguments. */
-int oracle_half_sweep(int L, int nsamples, int8_t *sigma, const int8_t *Jx, const int8_t *Jy, const int8_t *Jz,
-                      uint64_t seed, int rng_mode, uint64_t t, const uint64_t T[3], uint32_t *minstd_state,
-                      int64_t *dE_sum, int64_t *stats)
+static int half_sweep_core(int L, int nsamples, int8_t *sigma, const int8_t *Jx, const int8_t *Jy, const int8_t *Jz,
+                           uint64_t seed, int rng_mode, uint64_t t, const uint64_t T[3], uint32_t *minstd_state,
+                           const uint32_t *draw_table, int64_t *dE_sum, int64_t *stats)
 {
     if (L < 2 || (L & 1) || nsamples < 1) return -1;
     if (rng_mode == ORACLE_RNG_MINSTD && !minstd_state) return -1;
+    if ((rng_mode == ORACLE_RNG_PR_LANES || rng_mode == ORACLE_RNG_MT_LANES) && !draw_table) return -1;
     int64_t N = (int64_t)L * L * L;
     int colour = (int)(t & 1);
     int64_t st_prop = 0, st_acc = 0, st_up = 0, st_bad = 0;
@@ -245,6 +256,10 @@ int oracle_half_sweep(int L, int nsamples, int8_t *sigma, const int8_t *Jx, cons
                         R = oracle_philox_draw(L, seed, s, x, y, z, t);
                     } else if (rng_mode == ORACLE_RNG_PHILOX_SHARED) {
                         R = oracle_philox_draw(L, seed, s >> 5, x, y, z, t);
+                    } else if (rng_mode == ORACLE_RNG_PR_LANES || rng_mode == ORACLE_RNG_MT_LANES) {
+                        /* DESIGN.md R19: the draw of (coded batch s>>5, colour rank j) of this half-sweep */
+                        int64_t j = (int64_t)(x >> 1) + (int64_t)(L / 2) * ((int64_t)y + (int64_t)L * (int64_t)z);
+                        R = draw_table[(int64_t)(s >> 5) * (N / 2) + j];
                     } else {
                         uint32_t *st = &minstd_state[(int64_t)s * N + i];
                         *st = oracle_minstd_step(*st);
@@ -278,6 +293,14 @@ int oracle_half_sweep(int L, int nsamples, int8_t *sigma, const int8_t *Jx, cons
         stats[10] += h6;
     }
     return 0;
+}
+
+int oracle_half_sweep(int L, int nsamples, int8_t *sigma, const int8_t *Jx, const int8_t *Jy, const int8_t *Jz,
+                      uint64_t seed, int rng_mode, uint64_t t, const uint64_t T[3], uint32_t *minstd_state,
+                      int64_t *dE_sum, int64_t *stats)
+{
+    if (rng_mode == ORACLE_RNG_PR_LANES || rng_mode == ORACLE_RNG_MT_LANES) return -1; /* use oracle_half_sweep_lanes */
+    return half_sweep_core(L, nsamples, sigma, Jx, Jy, Jz, seed, rng_mode, t, T, minstd_state, NULL, dE_sum, stats);
 }
 
 /* The single-site rule on its own, for checks of sampled sites at sizes where a whole oracle
@@ -331,4 +354,174 @@ int oracle_get_max_threads(void)
 #else
     return 1;
 #endif
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Generators with stored state, one per lane (R19)           */
+/* ------------------------------------------------------------------------------------------ */
+
+#define ORACLE_PR_RING 62
+#define ORACLE_MT_N 624
+
+/* Parisi-Rapuano: "a lagged-Fibonacci-like PRNG with a minimal state of 62 words",
+ *     ira[i] = ira[i-24] + ira[i-55];   R = ira[i] ^ ira[i-61];
+ * on 32-bit words (the sum is mod 2^32).  The state is the last 62 words; they are kept in a ring indexed by
+ * i mod 62.  The seed words are ira[0..61], so draw number n (from 0) is R of i = 62 + n. */
+uint32_t oracle_pr_next(uint32_t ring[ORACLE_PR_RING], uint64_t *ndrawn)
+{
+    uint64_t i = (uint64_t)ORACLE_PR_RING + *ndrawn;
+    uint32_t v = ring[(i - 24) % ORACLE_PR_RING] + ring[(i - 55) % ORACLE_PR_RING];
+    uint32_t R = v ^ ring[(i - 61) % ORACLE_PR_RING];
+    ring[i % ORACLE_PR_RING] = v;
+    *ndrawn += 1;
+    return R;
+}
+
+/* Seed words of lane q (R19): ira[r] = high 32 bits of SplitMix64 output number q*62 + r + 1 from `seed`. */
+void oracle_pr_seed(uint64_t seed, uint64_t lane, uint32_t ring[ORACLE_PR_RING])
+{
+    for (int r = 0; r < ORACLE_PR_RING; ++r)
+        ring[r] = (uint32_t)(oracle_splitmix64_output(seed, lane * ORACLE_PR_RING + (uint64_t)r + 1) >> 32);
+}
+
+/* MT19937 (Matsumoto & Nishimura 1998; "the widely known Mersenne Twister MT19937"): seeding by
+ * init_genrand(s), mt[0] = s, mt[i] = 1812433253 * (mt[i-1] ^ (mt[i-1] >> 30)) + i. */
+void oracle_mt_seed(uint32_t s, uint32_t mt[ORACLE_MT_N])
+{
+    mt[0] = s;
+    for (uint32_t i = 1; i < ORACLE_MT_N; ++i) mt[i] = 1812433253u * (mt[i - 1] ^ (mt[i - 1] >> 30)) + i;
+}
+
+/* The textbook generator: when the 624 words are used up the whole block is regenerated,
+ *   y = (mt[k] & UPPER) | (mt[k+1] & LOWER);  mt[k] = mt[k+397] ^ (y >> 1) ^ (y odd ? 0x9908b0df : 0)   (indices mod 624),
+ * and output number n is the tempered word n mod 624 of the current block. */
+uint32_t oracle_mt_next(uint32_t mt[ORACLE_MT_N], uint64_t *ndrawn)
+{
+    uint32_t pos = (uint32_t)(*ndrawn % ORACLE_MT_N);
+    if (pos == 0) {
+        for (int k = 0; k < ORACLE_MT_N; ++k) {
+            uint32_t y = (mt[k] & 0x80000000u) | (mt[(k + 1) % ORACLE_MT_N] & 0x7fffffffu);
+            mt[k] = mt[(k + 397) % ORACLE_MT_N] ^ (y >> 1) ^ ((y & 1u) ? 0x9908b0dfu : 0u);
+        }
+    }
+    uint32_t y = mt[pos];
+    y ^= y >> 11;
+    y ^= (y << 7) & 0x9d2c5680u;
+    y ^= (y << 15) & 0xefc60000u;
+    y ^= y >> 18;
+    *ndrawn += 1;
+    return y;
+}
+
+/* init_genrand seed of lane q (R19): high 32 bits of SplitMix64 output number q + 1 from `seed`. */
+uint32_t oracle_mt_lane_seed(uint64_t seed, uint64_t lane)
+{
+    return (uint32_t)(oracle_splitmix64_output(seed, lane + 1) >> 32);
+}
+
+int oracle_lane_state_words(int rng_mode)
+{
+    return rng_mode == ORACLE_RNG_PR_LANES ? ORACLE_PR_RING : rng_mode == ORACLE_RNG_MT_LANES ? ORACLE_MT_N : 0;
+}
+
+/* state: nlanes * oracle_lane_state_words(mode) words, lane-major; ndrawn: nlanes counters. */
+int oracle_lanes_init(int rng_mode, uint64_t seed, int64_t nlanes, uint32_t *state, uint64_t *ndrawn)
+{
+    const int W = oracle_lane_state_words(rng_mode);
+    if (W == 0 || nlanes < 1) return -1;
+    for (int64_t q = 0; q < nlanes; ++q) {
+        if (rng_mode == ORACLE_RNG_PR_LANES) oracle_pr_seed(seed, (uint64_t)q, state + q * W);
+        else oracle_mt_seed(oracle_mt_lane_seed(seed, (uint64_t)q), state + q * W);
+        ndrawn[q] = 0;
+    }
+    return 0;
+}
+
+static inline uint32_t lane_next(int rng_mode, uint32_t *lane_state, uint64_t *ndrawn)
+{
+    return rng_mode == ORACLE_RNG_PR_LANES ? oracle_pr_next(lane_state, ndrawn) : oracle_mt_next(lane_state, ndrawn);
+}
+
+/* The draws of one colour half-sweep (R19).  The N/2 sites of the colour are numbered by their colour rank j and
+ * taken in groups of four, g = j >> 2 (ngroups = N/8 groups).  Lane q serves the groups g = q, q + nlanes, q + 2 nlanes, ...
+ * in that order; for each group it serves the k coded batches b = 0..k-1 in turn, and for each the four sites w = 0..3 of
+ * the group: the next number of the lane is the draw shared by the 32 samples of batch b at site j = 4g + w
+ * (PAPER.md:228-232).  Every lane takes the same number of draws per half-sweep, 4 k ceil(ngroups / nlanes): a lane whose
+ * last group does not exist draws and discards.  table[b * (N/2) + j] receives the draw. */
+int oracle_lanes_draw_table(int rng_mode, int64_t nlanes, uint32_t *state, uint64_t *ndrawn, int64_t ngroups, int k,
+                            uint32_t *table)
+{
+    const int W = oracle_lane_state_words(rng_mode);
+    if (W == 0 || nlanes < 1 || ngroups < 1 || k < 1) return -1;
+    const int64_t rounds = (ngroups + nlanes - 1) / nlanes;
+    for (int64_t q = 0; q < nlanes; ++q)
+        for (int64_t m = 0; m < rounds; ++m) {
+            const int64_t g = q + m * nlanes;
+            for (int b = 0; b < k; ++b)
+                for (int w = 0; w < 4; ++w) {
+                    const uint32_t R = lane_next(rng_mode, state + q * W, &ndrawn[q]);
+                    if (g < ngroups) table[(int64_t)b * 4 * ngroups + 4 * g + w] = R;
+                }
+        }
+    return 0;
+}
+
+/* One colour half-sweep in a lane mode: the draw table of this half-sweep, then the scalar rule of oracle_half_sweep
+ * with R = table[batch][colour rank].  nsamples must be a multiple of 32, L a multiple of 4 (so that N/2 is a multiple of 4).
+ * scratch: (nsamples/32) * N/2 words. */
+int oracle_half_sweep_lanes(int L, int nsamples, int8_t *sigma, const int8_t *Jx, const int8_t *Jy, const int8_t *Jz,
+                            int rng_mode, int64_t nlanes, uint32_t *state, uint64_t *ndrawn, uint64_t t,
+                            const uint64_t T[3], uint32_t *scratch, int64_t *dE_sum, int64_t *stats)
+{
+    if (nsamples < 32 || nsamples % 32 || L < 2 || ((int64_t)L * L * L) % 8) return -1;
+    const int64_t ngroups = (int64_t)L * L * L / 8;
+    if (oracle_lanes_draw_table(rng_mode, nlanes, state, ndrawn, ngroups, nsamples / 32, scratch) != 0) return -1;
+    return half_sweep_core(L, nsamples, sigma, Jx, Jy, Jz, 0, rng_mode, t, T, NULL, scratch, dE_sum, stats);
+}
+
+/* PAPER.md:196-197 and Table II: "its kernel version counting the fraction of odd numbers".  Every lane
+ * draws `ndraws` numbers; odd[q] = how many were odd, sum[q] = their sum mod 2^64 (a checksum of the whole sequence).
+ * Kinds: 3 = Parisi-Rapuano, 4 = MT19937 (lanes seeded as above), 1 = MINSTD with the seed state of stream q (R11) advanced
+ * ndraws times (Eq. 7), 0 = Philox4x32-10 with key (lo32 seed, hi32 seed) and counter (lo32 c, hi32 c, lo32 q, hi32 q) for call
+ * number c = n >> 2, output word n & 3. */
+int oracle_count_odd(int kind, uint64_t seed, int64_t nlanes, int64_t ndraws, uint64_t *odd, uint64_t *sum)
+{
+    if (nlanes < 1 || ndraws < 0) return -1;
+    if (kind != ORACLE_RNG_PHILOX && kind != ORACLE_RNG_MINSTD && kind != ORACLE_RNG_PR_LANES && kind != ORACLE_RNG_MT_LANES)
+        return -1;
+#pragma omp parallel for schedule(static)
+    for (int64_t q = 0; q < nlanes; ++q) {
+        uint64_t o = 0, s = 0;
+        if (kind == ORACLE_RNG_PR_LANES || kind == ORACLE_RNG_MT_LANES) {
+            uint32_t st[ORACLE_MT_N];
+            uint64_t nd = 0;
+            if (kind == ORACLE_RNG_PR_LANES) oracle_pr_seed(seed, (uint64_t)q, st);
+            else oracle_mt_seed(oracle_mt_lane_seed(seed, (uint64_t)q), st);
+            for (int64_t n = 0; n < ndraws; ++n) {
+                const uint32_t R = lane_next(kind, st, &nd);
+                o += R & 1u;
+                s += R;
+            }
+        } else if (kind == ORACLE_RNG_MINSTD) {
+            uint32_t r = oracle_minstd_seed_state(seed, (uint64_t)q);
+            for (int64_t n = 0; n < ndraws; ++n) {
+                r = oracle_minstd_step(r);
+                o += r & 1u;
+                s += r;
+            }
+        } else {
+            const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+            for (int64_t n = 0; n < ndraws; ++n) {
+                const uint64_t c = (uint64_t)n >> 2;
+                const uint32_t ctr[4] = { (uint32_t)c, (uint32_t)(c >> 32), (uint32_t)q, (uint32_t)((uint64_t)q >> 32) };
+                uint32_t out[4];
+                oracle_philox4x32_10(ctr, key, out);
+                o += out[n & 3] & 1u;
+                s += out[n & 3];
+            }
+        }
+        odd[q] = o;
+        sum[q] = s;
+    }
+    return 0;
 }

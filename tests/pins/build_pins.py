@@ -19,6 +19,13 @@ def build_minstd() -> str:
     return lib
 
 
+def build_mt19937() -> str:
+    src, lib = os.path.join(HERE, "mt19937_shim.cpp"), os.path.join(HERE, "libpin_mt19937.so")
+    if _stale(lib, src):
+        subprocess.run(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", lib, src], check=True)
+    return lib
+
+
 def build_curand_philox() -> str | None:
     """None when nvcc is not installed (the test then skips)."""
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
