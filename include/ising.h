@@ -47,7 +47,8 @@ extern "C" {
 
 #define ISING_OK 0
 #define ISING_EINVAL (-1) /* bad argument: L odd or < 4 or > 2048, nsamples not 1 or a multiple of 32, unknown
-                             rng_mode, null pointer, workspace too small / misaligned, beta < 0 or NaN, nsweeps < 0 */
+                             rng_mode, a mode that does not support (L, nsamples), null pointer, workspace too small /
+                             misaligned, beta < 0 or NaN, nsweeps < 0 */
 #define ISING_ECUDA (-2)  /* a CUDA runtime call or kernel launch failed (sticky errors surface here too) */
 
 #define ISING_RNG_PHILOX 0 /* Philox4x32-10, key (lo32 seed, hi32 seed ^ sample), counter (t, colour-rank>>2)  (R9, R10) */
@@ -57,6 +58,17 @@ extern "C" {
 #define ISING_RNG_PHILOX_SHARED 2 /* the paper's asynchronous multispin coding proper (Eq. 15): the 32
                               samples of a word share ONE Philox draw per (site, half-sweep); nsamples = 32k only; the draw
                               of the samples 32b..32b+31 is the ISING_RNG_PHILOX draw with the key's sample field = b (R18) */
+
+/* The same shared draw, taken from generators with STORED state, one per lane -- the paper's own scheme of one generator
+ * per thread with a strided state array (R19).  nsamples = 32k and L % 8 == 0 only.
+ *   The N/2 sites of a colour are numbered by their colour rank j and taken in groups of four, g = j >> 2.  Lane q serves the
+ *   groups q, q + nlanes, q + 2 nlanes, ... in that order, for each group the coded batches b = 0..k-1, for each the four sites
+ *   w = 0..3; the next number of the lane is the draw of (batch b, site 4g + w).  Every lane takes 4 k ceil((N/8) / nlanes)
+ *   draws per half-sweep (a lane whose last group does not exist draws and discards).  Thresholds as for Philox (R5).
+ *   nlanes defaults to min(N/8, 151552) (ising_get_lanes / ising_set_lanes); the state lives in the workspace. */
+#define ISING_RNG_PR_SHARED 3      /* Parisi-Rapuano: ira[i] = ira[i-24] + ira[i-55]; R = ira[i] ^ ira[i-61];
+                              seed words ira[0..61] of lane q = high words of SplitMix64 outputs q*62 + 1 .. q*62 + 62 of `seed` */
+#define ISING_RNG_MT19937_SHARED 4 /* MT19937, lane q seeded by init_genrand(high word of SplitMix64 output q + 1) */
 
 typedef struct ising ising_t; /* opaque */
 
@@ -114,7 +126,27 @@ uint64_t ising_fnv1a64_host(const void *h_data, size_t nbytes);
 /* Half-sweep counter t of the handle (get / set): with ising_get_spins + ising_load_state this makes a run
  * resumable bit-exactly, because no PRNG state exists outside (seed, t). */
 int ising_get_t(const ising_t *h, uint64_t *t);
-int ising_set_t(ising_t *h, uint64_t t);
+int ising_set_t(ising_t *h, uint64_t t); /* ISING_EINVAL in the lane modes 3, 4: their generator state is not a function of t */
+
+/* Lane modes (3, 4) only.  Number of generator lanes; ising_set_lanes is allowed before the first sweep only, with
+ * 1 <= nlanes <= the default (the workspace is sized for the default).  Other modes: ISING_EINVAL. */
+int ising_get_lanes(const ising_t *h, uint32_t *nlanes);
+int ising_set_lanes(ising_t *h, uint32_t nlanes);
+
+/* The paper's device-API generator benchmark (Table II): every lane draws numbers and counts the odd ones.
+ * kind: ISING_RNG_PHILOX (no state; key (lo32 seed, hi32 seed), counter (lo32 c, hi32 c, lane, 0), c = draw number >> 2, output
+ * word = draw number & 3), ISING_RNG_MINSTD (one word per lane, the seed state of stream `lane`, R11, advanced once per draw),
+ * ISING_RNG_PR_SHARED, ISING_RNG_MT19937_SHARED (62 / 624 words per lane, strided: word r of lane q at d_state[r*nlanes + q],
+ * seeded as above).
+ *   ising_prng_state_bytes  bytes of d_state for (kind, nlanes); 0 for Philox.
+ *   ising_prng_init         seeds the state of every lane.
+ *   ising_prng_count_odd    every lane takes draws number ndrawn_before .. ndrawn_before + ndraws - 1 of its sequence (both
+ *                           multiples of 4; the caller keeps count) and writes d_odd[lane] = how many were odd and d_sum[lane] =
+ *                           their sum mod 2^64 (nlanes uint64 each, overwritten). */
+int ising_prng_state_bytes(int kind, uint32_t nlanes, size_t *out);
+int ising_prng_init(int kind, uint64_t seed, uint32_t nlanes, void *d_state, void *stream);
+int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndrawn_before, uint64_t ndraws, void *d_state,
+                         uint64_t *d_odd, uint64_t *d_sum, void *stream);
 
 /* Select the half-sweep kernel: 0 = automatic (the word-parallel kernel where the layout allows it, with the
  * cached seed table in MINSTD mode), 1 = force the generic one-site-at-a-time kernel (any even L), 2 = the

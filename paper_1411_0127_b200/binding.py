@@ -12,12 +12,14 @@ import ctypes as C
 from . import build as _build
 
 PHILOX, MINSTD, PHILOX_SHARED = 0, 1, 2
+PR_SHARED, MT19937_SHARED = 3, 4  # shared draw from stored-state lane generators (include/ising.h, R19)
 OK, EINVAL, ECUDA = 0, -1, -2
 
 EXPORTS = (
     "ising_workspace_bytes", "ising_create", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
     "ising_get_spins", "ising_run_host", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
+    "ising_get_lanes", "ising_set_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
 )
 
 _lib = None
@@ -52,6 +54,11 @@ def lib() -> C.CDLL:
     L.ising_kernel_launches.restype = u64
     L.ising_hostcheck_update_word.argtypes = [i32, u64, u64, dbl, C.POINTER(C.c_uint32), u64, u64, u64,
                                               C.POINTER(C.c_uint32)]
+    L.ising_get_lanes.argtypes = [vp, C.POINTER(C.c_uint32)]
+    L.ising_set_lanes.argtypes = [vp, C.c_uint32]
+    L.ising_prng_state_bytes.argtypes = [i32, C.c_uint32, C.POINTER(sz)]
+    L.ising_prng_init.argtypes = [i32, u64, C.c_uint32, vp, vp]
+    L.ising_prng_count_odd.argtypes = [i32, u64, C.c_uint32, u64, u64, vp, vp, vp, vp]
     L.ising_destroy.argtypes = [vp]
     L.ising_strerror.argtypes = [i32]
     L.ising_strerror.restype = C.c_char_p
@@ -90,6 +97,25 @@ def ising_hostcheck_update_word(rng_mode, seed, t, beta, ops, word_index, site0=
     _check(lib().ising_hostcheck_update_word(rng_mode, seed, t, float(beta), arr, word_index, site0, site_stride,
                                              C.byref(out)), "ising_hostcheck_update_word")
     return out.value
+
+
+def ising_prng_state_bytes(kind: int, nlanes: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().ising_prng_state_bytes(kind, nlanes, C.byref(out)), "ising_prng_state_bytes")
+    return out.value
+
+
+def ising_prng_init(kind: int, seed: int, nlanes: int, state, stream=None):
+    """state: uint8 CUDA tensor of ising_prng_state_bytes bytes (None for Philox)."""
+    _check(lib().ising_prng_init(kind, seed, nlanes, state.data_ptr() if state is not None else None, _stream_ptr(stream)),
+           "ising_prng_init")
+
+
+def ising_prng_count_odd(kind: int, seed: int, nlanes: int, ndrawn_before: int, ndraws: int, state, odd, total, stream=None):
+    """odd, total: int64 CUDA tensors of nlanes elements (uint64 bit patterns)."""
+    assert odd.is_cuda and total.is_cuda and odd.numel() == nlanes and total.numel() == nlanes
+    _check(lib().ising_prng_count_odd(kind, seed, nlanes, ndrawn_before, ndraws, state.data_ptr() if state is not None else None,
+                                      odd.data_ptr(), total.data_ptr(), _stream_ptr(stream)), "ising_prng_count_odd")
 
 
 def _stream_ptr(stream=None) -> int:
@@ -189,6 +215,14 @@ class Ising:
 
     def ising_set_t(self, t: int):
         _check(lib().ising_set_t(self._h, int(t)), "ising_set_t")
+
+    def ising_get_lanes(self) -> int:
+        n = C.c_uint32(0)
+        _check(lib().ising_get_lanes(self._h, C.byref(n)), "ising_get_lanes")
+        return n.value
+
+    def ising_set_lanes(self, nlanes: int):
+        _check(lib().ising_set_lanes(self._h, int(nlanes)), "ising_set_lanes")
 
     def ising_set_kernel(self, which: int):
         _check(lib().ising_set_kernel(self._h, int(which)), "ising_set_kernel")

@@ -7,6 +7,7 @@
 #include <new>
 
 #include "../../include/ising.h"
+#include "lane_rng.cuh"
 #include "layout_kernels.cuh"
 #include "measure_kernels.cuh"
 #include "sweep_kernels.cuh"
@@ -31,7 +32,15 @@ struct Geometry {
     size_t s0_words;            // cached MINSTD seed states: 32 words per word of each colour array (fast layout only)
     bool fast;                  // half-rows are whole words: L is a multiple of 64
     int W;                      // words per thread of the word-parallel kernel (fast layout)
+    uint32_t lanes_default;     // lane modes (R19): min(N/8, 148 * 1024) generator lanes
 };
+
+constexpr uint32_t MAX_LANES = 148u * 1024u;  // one lane per thread, 1024 threads on each of the 148 SMs: one wave
+
+inline bool lane_mode(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED || rng_mode == ISING_RNG_MT19937_SHARED; }
+inline bool shared_mode(int rng_mode) { return rng_mode == ISING_RNG_PHILOX_SHARED || lane_mode(rng_mode); }
+inline bool known_mode(int rng_mode) { return rng_mode >= ISING_RNG_PHILOX && rng_mode <= ISING_RNG_MT19937_SHARED; }
+inline uint32_t lane_ring(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED ? 62u : rng_mode == ISING_RNG_MT19937_SHARED ? 624u : 0u; }
 
 bool make_geometry(int L, int nsamples, Geometry *g)
 {
@@ -64,6 +73,7 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     // cached MINSTD seed states: 2 colours x one 4-byte word per site of every thread of the word-parallel grid (rows
     // whose lane count is not a power of two are padded, RowMap in sweep_kernels.cuh); N words when L = 64*2^k
     g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
+    g->lanes_default = (uint32_t)((g->N / 8 < MAX_LANES) ? g->N / 8 : MAX_LANES);
     return true;
 }
 
@@ -81,6 +91,9 @@ struct ising {
     unsigned long long *acc;
     uint32_t *s0tab;   // MINSTD mode, fast layout: seed-state tables of the two colours (nullptr otherwise)
     bool s0_ready;
+    uint32_t *lane_state;  // lane modes: ring * nlanes words, strided (lane_rng.cuh)
+    uint32_t nlanes;
+    bool lanes_ready;
     bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
 
     LatticeArrays arrays(int batch) const
@@ -107,7 +120,7 @@ int check_launch(ising_t *h, int n = 1)
 int compute_thresholds(double beta, int rng_mode, uint64_t out[3])
 {
     if (!(beta >= 0.0)) return ISING_EINVAL;
-    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD && rng_mode != ISING_RNG_PHILOX_SHARED) return ISING_EINVAL;
+    if (!known_mode(rng_mode)) return ISING_EINVAL;
     for (int k = 0; k < 3; ++k) {
         const double dE = 4.0 * (double)(k + 1);
         const double x = beta * dE;
@@ -258,8 +271,46 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
     return ISING_OK;
 }
 
+// Lane modes (R19): one launch per half-sweep, thread = lane; the lane state is seeded by the first launch of the handle.
+template <int GEN>
+int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    const unsigned blocks = (h->nlanes + 127u) / 128u;
+    if (!h->lanes_ready) {
+        lanes_init<GEN><<<blocks, 128, 0, st>>>(h->lane_state, h->nlanes, h->seed);
+        const int rc = check_launch(h);
+        if (rc != ISING_OK) return rc;
+        h->lanes_ready = true;
+    }
+    const int c = (int)(h->t & 1);
+    const LatticeArrays A = h->arrays(0);
+    SweepArgs a;
+    a.S_act = A.S[c];
+    a.S_oth = A.S[1 - c];
+    for (int d = 0; d < 3; ++d) { a.J_act[d] = A.J[d][c]; a.J_oth[d] = A.J[d][1 - c]; }
+    a.L = g.L;
+    a.colour = c;
+    a.T = T;
+    const uint32_t ngroups = (uint32_t)(g.N / 8), rounds = (ngroups + h->nlanes - 1) / h->nlanes;
+    const uint64_t per_half_sweep = 4ull * (uint64_t)g.nbatches * rounds;
+    LaneArgs ln;
+    ln.state = h->lane_state;
+    ln.nlanes = h->nlanes;
+    ln.pos0 = (uint32_t)((h->t % LaneRing<GEN>::size) * (per_half_sweep % LaneRing<GEN>::size) % LaneRing<GEN>::size);
+    const uint32_t gpr = (uint32_t)g.L / 8;
+    launch_pdl(half_sweep_shared_lanes<GEN>, dim3(blocks), dim3(128), st, a, ln, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
+               (size_t)(8 * g.array_words), (uint32_t)g.nbatches, ngroups, rounds);
+    const int rc = check_launch(h);
+    if (rc != ISING_OK) return rc;
+    h->t += 1;
+    return ISING_OK;
+}
+
 int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
 {
+    if (h->rng_mode == ISING_RNG_PR_SHARED) return launch_half_sweep_lanes<GEN_PR>(h, T, st);
+    if (h->rng_mode == ISING_RNG_MT19937_SHARED) return launch_half_sweep_lanes<GEN_MT>(h, T, st);
     if (h->rng_mode == ISING_RNG_PHILOX_SHARED) return launch_half_sweep<2>(h, T, st);
     return h->rng_mode == ISING_RNG_PHILOX ? launch_half_sweep<0>(h, T, st) : launch_half_sweep<1>(h, T, st);
 }
@@ -320,10 +371,12 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
 {
     Geometry g;
     if (!out || !make_geometry(L, nsamples, &g)) return ISING_EINVAL;
-    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD && rng_mode != ISING_RNG_PHILOX_SHARED) return ISING_EINVAL;
-    if (rng_mode == ISING_RNG_PHILOX_SHARED && nsamples % 32 != 0) return ISING_EINVAL;  // one draw per 32-sample word
+    if (!known_mode(rng_mode)) return ISING_EINVAL;
+    if (shared_mode(rng_mode) && nsamples % 32 != 0) return ISING_EINVAL;  // one draw per 32-sample word
+    if (lane_mode(rng_mode) && L % 8 != 0) return ISING_EINVAL;            // groups of four sites must not leave their row
     *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
     if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
+    if (lane_mode(rng_mode)) *out += round_up((size_t)lane_ring(rng_mode) * g.lanes_default * sizeof(uint32_t), 256);
     return ISING_OK;
 }
 
@@ -348,6 +401,9 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->s0tab = (rng_mode == ISING_RNG_MINSTD && h->g.s0_words) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->s0_ready = false;
     h->slots_clean = false;
+    h->lane_state = lane_mode(rng_mode) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
+    h->nlanes = lane_mode(rng_mode) ? h->g.lanes_default : 0;
+    h->lanes_ready = false;
     *out = h;
     return ISING_OK;
 }
@@ -528,9 +584,69 @@ int ising_get_t(const ising_t *h, uint64_t *t)
 
 int ising_set_t(ising_t *h, uint64_t t)
 {
-    if (!h) return ISING_EINVAL;
+    if (!h || lane_mode(h->rng_mode)) return ISING_EINVAL;
     h->t = t;
     return ISING_OK;
+}
+
+int ising_get_lanes(const ising_t *h, uint32_t *nlanes)
+{
+    if (!h || !nlanes || !lane_mode(h->rng_mode)) return ISING_EINVAL;
+    *nlanes = h->nlanes;
+    return ISING_OK;
+}
+
+int ising_set_lanes(ising_t *h, uint32_t nlanes)
+{
+    if (!h || !lane_mode(h->rng_mode) || h->lanes_ready || nlanes < 1 || nlanes > h->g.lanes_default) return ISING_EINVAL;
+    h->nlanes = nlanes;
+    return ISING_OK;
+}
+
+int ising_prng_state_bytes(int kind, uint32_t nlanes, size_t *out)
+{
+    if (!out || !known_mode(kind) || kind == ISING_RNG_PHILOX_SHARED || nlanes < 1) return ISING_EINVAL;
+    const size_t words = kind == ISING_RNG_PHILOX ? 0 : kind == ISING_RNG_MINSTD ? 1 : lane_ring(kind);
+    *out = words * nlanes * sizeof(uint32_t);
+    return ISING_OK;
+}
+
+int ising_prng_init(int kind, uint64_t seed, uint32_t nlanes, void *d_state, void *stream)
+{
+    size_t bytes;
+    if (ising_prng_state_bytes(kind, nlanes, &bytes) != ISING_OK || (bytes && !d_state)) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned blocks = (nlanes + 127u) / 128u;
+    if (kind == ISING_RNG_MINSTD) minstd_lanes_init<<<blocks, 128, 0, st>>>((uint32_t *)d_state, nlanes, seed);
+    else if (kind == ISING_RNG_PR_SHARED) lanes_init<GEN_PR><<<blocks, 128, 0, st>>>((uint32_t *)d_state, nlanes, seed);
+    else if (kind == ISING_RNG_MT19937_SHARED) lanes_init<GEN_MT><<<blocks, 128, 0, st>>>((uint32_t *)d_state, nlanes, seed);
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
+}
+
+int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndrawn_before, uint64_t ndraws, void *d_state,
+                         uint64_t *d_odd, uint64_t *d_sum, void *stream)
+{
+    size_t bytes;
+    if (ising_prng_state_bytes(kind, nlanes, &bytes) != ISING_OK || (bytes && !d_state) || !d_odd || !d_sum) return ISING_EINVAL;
+    if ((ndrawn_before & 3u) || (ndraws & 3u)) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned blocks = (nlanes + 127u) / 128u;
+    unsigned long long *odd = (unsigned long long *)d_odd, *sum = (unsigned long long *)d_sum;
+    LaneArgs ln;
+    ln.state = (uint32_t *)d_state;
+    ln.nlanes = nlanes;
+    if (kind == ISING_RNG_PHILOX) {
+        count_odd_philox<<<blocks, 128, 0, st>>>(nlanes, seed, ndrawn_before >> 2, ndraws >> 2, odd, sum);
+    } else if (kind == ISING_RNG_MINSTD) {
+        count_odd_minstd<<<blocks, 128, 0, st>>>((uint32_t *)d_state, nlanes, ndraws, odd, sum);
+    } else if (kind == ISING_RNG_PR_SHARED) {
+        ln.pos0 = (uint32_t)(ndrawn_before % 62u);
+        count_odd_lanes<GEN_PR><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
+    } else {
+        ln.pos0 = (uint32_t)(ndrawn_before % 624u);
+        count_odd_lanes<GEN_MT><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
+    }
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
 }
 
 int ising_set_kernel(ising_t *h, int which)
@@ -545,7 +661,7 @@ uint64_t ising_kernel_launches(const ising_t *h) { return h ? h->launches : 0; }
 int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double beta, const uint32_t ops[13],
                                 uint64_t word_index, uint64_t site0, uint64_t site_stride, uint32_t *out)
 {
-    if (!ops || !out || rng_mode == ISING_RNG_PHILOX_SHARED) return ISING_EINVAL;  // a site-packed word has no shared draw
+    if (!ops || !out || shared_mode(rng_mode)) return ISING_EINVAL;  // a site-packed word has no shared draw
     uint64_t T[3];
     if (compute_thresholds(beta, rng_mode, T) != ISING_OK) return ISING_EINVAL;
     const Thresholds kt = kernel_thresholds(T);
