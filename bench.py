@@ -35,6 +35,9 @@ ALG_SLOTS_PER_FLIP = {0: 18 * 2 / 4}
 ALG_INT_OPS_PER_FLIP = 37 / 4 + 2 + 22 / 32
 BINDING_PIPE = {0: "fma (IMAD.WIDE)"}
 ALG_BYTES_PER_FLIP = {0: 9 / 8, 1: 9 / 8 + 4}  # 9N/16 bytes per half-sweep = 1.125 B per flip attempt
+# stored-state lane generators (rng modes 3, 4): state words moved per draw, 4 B each.  Parisi-Rapuano reads
+# ira[i-24], ira[i-55], ira[i-61] and writes ira[i]; MT19937 in blocks of four draws reads mt[i..i+4], mt[i+397..i+400], writes 4
+LANE_STATE_BYTES_PER_DRAW = {3: 16.0, 4: 13.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch at L=1024 from the ncu --set full capture in
 # profiles/r1h_end_of_round.md (algorithmic: 9N/16 = 603,979,776 B)
 NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 57.63e6, 1: 2684.5e6 + 60.9e6}
@@ -151,6 +154,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-shared", action="store_true", help="skip the shared-random-number (paper's AMSC) timing")
     ap.add_argument("--only-shared", action="store_true", help="time only the shared-random-number mode (for ncu captures)")
+    ap.add_argument("--only-lanes", action="store_true", help="time only the stored-state lane generators (sweep and Table II)")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -245,13 +249,12 @@ def main():
         g.ising_destroy()
         return res
 
-    def bench_shared(Ls, ns, sweeps):
-        """the paper's own scheme, one draw per 32-sample word (rng_mode 2); sweeps only."""
-        from paper_1411_0127_b200 import PHILOX_SHARED
-
+    def bench_shared(Ls, ns, sweeps, mode=2):
+        """the paper's own scheme, one draw per 32-sample word (rng_mode 2); rank 2: the same with the
+        draws taken from stored-state lane generators (rng_mode 3 Parisi-Rapuano, 4 MT19937); sweeps only."""
         sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
         Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
-        g = Ising(Ls, ns, synth.DYN_SEED, PHILOX_SHARED)
+        g = Ising(Ls, ns, synth.DYN_SEED, mode)
         g.ising_load_state(sp, Jc)
         g.ising_sweep(BETA, 2)
         barrier()
@@ -263,10 +266,49 @@ def main():
         ms = a.elapsed_time(b)
         g.ising_destroy()
         flips = sweeps * ns * Ls**3
-        gbs = ALG_BYTES_PER_FLIP[0] * flips / (ms * 1e-3) / 1e9
-        return {"workload": f"L={Ls} cube x {ns} samples ({ns // 32} coded batches), {sweeps} sweeps, one Philox draw per 32-sample word",
+        bpf = ALG_BYTES_PER_FLIP[0] + LANE_STATE_BYTES_PER_DRAW.get(mode, 0.0) / 32.0  # one draw serves 32 flip attempts
+        gbs = bpf * flips / (ms * 1e-3) / 1e9
+        gen = {2: "one Philox draw", 3: "one Parisi-Rapuano draw (62-word state per lane, strided)",
+               4: "one MT19937 draw (624-word state per lane, strided)"}[mode]
+        return {"workload": f"L={Ls} cube x {ns} samples ({ns // 32} coded batches), {sweeps} sweeps, {gen} per 32-sample word",
                 "value": 1e9 * ms / flips, "unit": UNIT, "half_sweep_us": 1e3 * ms / (2 * sweeps),
-                "roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "alg_bytes_per_flip": ALG_BYTES_PER_FLIP[0]}}
+                "roofline": {"bound": "hbm", "achieved": gbs, "unit": "GB/s", "alg_bytes_per_flip": bpf}}
+
+    def bench_table2(kind, nlanes=148 * 1024, ndraws=4096, reps=10):
+        """PAPER.md Table II, the device-API generator test: every lane draws numbers and counts the odd ones; instances/s."""
+        from paper_1411_0127_b200 import binding
+
+        nbytes = binding.ising_prng_state_bytes(kind, nlanes)
+        state = torch.empty(nbytes, dtype=torch.uint8, device="cuda") if nbytes else None
+        odd = torch.zeros(nlanes, dtype=torch.int64, device="cuda")
+        tot = torch.zeros(nlanes, dtype=torch.int64, device="cuda")
+        a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        a.record(stream)
+        binding.ising_prng_init(kind, synth.DYN_SEED, nlanes, state)
+        b.record(stream)
+        binding.ising_prng_count_odd(kind, synth.DYN_SEED, nlanes, 0, ndraws, state, odd, tot)  # warm-up
+        torch.cuda.synchronize()
+        b2 = torch.cuda.Event(enable_timing=True)
+        b2.record(stream)
+        for r in range(reps):
+            binding.ising_prng_count_odd(kind, synth.DYN_SEED, nlanes, (r + 1) * ndraws, ndraws, state, odd, tot)
+        c.record(stream)
+        torch.cuda.synchronize()
+        ms = b2.elapsed_time(c)
+        n = nlanes * ndraws * reps
+        frac_odd = float(odd.sum().item()) / (nlanes * ndraws)
+        row = {"generator": {0: "philox4x32-10", 1: "minstd", 3: "parisi-rapuano", 4: "mt19937"}[kind], "lanes": nlanes,
+               "draws_per_lane": ndraws, "reps": reps, "instances_per_s": n / (ms * 1e-3), "t_init_ms": a.elapsed_time(b),
+               "fraction_odd_last_rep": frac_odd}
+        bpd = LANE_STATE_BYTES_PER_DRAW.get(kind)
+        if bpd:
+            row["state_bytes_per_draw"] = bpd
+            row["state_GBps"] = bpd * n / (ms * 1e-3) / 1e9
+        return row
+
+    def bench_lanes():
+        return {"sweep": [bench_shared(512, 32, 4, 3), bench_shared(512, 32, 4, 4), bench_shared(128, 256, 20, 3)],
+                "table2_device_api": [bench_table2(k) for k in (0, 1, 3, 4)]}
 
     if args.scan:
         from paper_1411_0127_b200 import PHILOX_SHARED
@@ -300,6 +342,9 @@ def main():
     if args.only_shared:
         print(json.dumps({"amsc_shared_random_number": [bench_shared(512, 32, 4)]}))
         return
+    if args.only_lanes:
+        print(json.dumps({"amsc_lane_generators": bench_lanes()}))
+        return
 
     sampler = ClockSampler(local)
     if rank == 0:
@@ -308,9 +353,10 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     minstd = None if args.no_minstd else bench_mode(MINSTD)
 
-    shared = None
+    shared = lanes = None
     if world == 1 and not args.no_shared:
         shared = [bench_shared(128, 256, 20), bench_shared(512, 32, 4)]
+        lanes = bench_lanes()
 
     if rank != 0:
         if dist is not None:
@@ -377,6 +423,9 @@ def main():
         for sh in shared:
             sh["roofline"].update({"peak": hbm_gbs_, "frac": sh["roofline"]["achieved"] / hbm_gbs_, "peak_source": src_ + " (burst copy)"})
         line["amsc_shared_random_number"] = shared
+        for sh in lanes["sweep"]:
+            sh["roofline"].update({"peak": hbm_gbs_, "frac": sh["roofline"]["achieved"] / hbm_gbs_, "peak_source": src_ + " (burst copy)"})
+        line["amsc_lane_generators"] = lanes
     if world == 1 and not args.no_cpu_baseline:
         Ls, sw = 512, 64  # about 15 s on the 16 host cores of the GPU box
         times, cores = time_oracle(Ls, sw, 0)

@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(128) lanes_init(uint32_t *state, uint32_t nlan
 // so the lattice loads of a warp are the same coalesced 512-byte rows as in half_sweep_shared_vec.
 // ---------------------------------------------------------------------------------------------------
 template <int GEN>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 8)
 half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uint32_t gpr_inv, size_t batch_stride,
                         uint32_t nbatches, uint32_t ngroups, uint32_t rounds)
 {
