@@ -65,7 +65,7 @@ extern "C" {
  *   groups q, q + nlanes, q + 2 nlanes, ... in that order, for each group the coded batches b = 0..k-1, for each the four sites
  *   w = 0..3; the next number of the lane is the draw of (batch b, site 4g + w).  Every lane takes 4 k ceil((N/8) / nlanes)
  *   draws per half-sweep (a lane whose last group does not exist draws and discards).  Thresholds as for Philox (R5).
- *   nlanes defaults to min(N/8, 151552) (ising_get_lanes / ising_set_lanes); the state lives in the workspace. */
+ *   nlanes defaults to min(N/8, 151552 = one wave of threads) (ising_get_lanes / ising_set_lanes); the state lives in the workspace. */
 #define ISING_RNG_PR_SHARED 3      /* Parisi-Rapuano: ira[i] = ira[i-24] + ira[i-55]; R = ira[i] ^ ira[i-61];
                               seed words ira[0..61] of lane q = high words of SplitMix64 outputs q*62 + 1 .. q*62 + 62 of `seed` */
 #define ISING_RNG_MT19937_SHARED 4 /* MT19937, lane q seeded by init_genrand(high word of SplitMix64 output q + 1) */

@@ -32,14 +32,20 @@ struct Geometry {
     size_t s0_words;            // cached MINSTD seed states: 32 words per word of each colour array (fast layout only)
     bool fast;                  // half-rows are whole words: L is a multiple of 64
     int W;                      // words per thread of the word-parallel kernel (fast layout)
-    uint32_t lanes_default;     // lane modes (R19): min(N/8, 148 * 1024) generator lanes
 };
 
-constexpr uint32_t MAX_LANES = 148u * 1024u;  // one lane per thread, 1024 threads on each of the 148 SMs: one wave
+// Lane modes (R19): default number of generator lanes = min(N/8, one wave of threads on the 148 SMs: 8 CTAs of 128 threads
+// at 64 registers).
+constexpr uint32_t MAX_LANES = 148u * 1024u;
 
 inline bool lane_mode(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED || rng_mode == ISING_RNG_MT19937_SHARED; }
 inline bool shared_mode(int rng_mode) { return rng_mode == ISING_RNG_PHILOX_SHARED || lane_mode(rng_mode); }
 inline bool known_mode(int rng_mode) { return rng_mode >= ISING_RNG_PHILOX && rng_mode <= ISING_RNG_MT19937_SHARED; }
+inline uint32_t lanes_default(const Geometry &g, int rng_mode)
+{
+    (void)rng_mode;
+    return (uint32_t)(g.N / 8 < MAX_LANES ? g.N / 8 : MAX_LANES);
+}
 inline uint32_t lane_ring(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED ? 62u : rng_mode == ISING_RNG_MT19937_SHARED ? 624u : 0u; }
 
 bool make_geometry(int L, int nsamples, Geometry *g)
@@ -73,7 +79,6 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     // cached MINSTD seed states: 2 colours x one 4-byte word per site of every thread of the word-parallel grid (rows
     // whose lane count is not a power of two are padded, RowMap in sweep_kernels.cuh); N words when L = 64*2^k
     g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
-    g->lanes_default = (uint32_t)((g->N / 8 < MAX_LANES) ? g->N / 8 : MAX_LANES);
     return true;
 }
 
@@ -376,7 +381,7 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
     if (lane_mode(rng_mode) && L % 8 != 0) return ISING_EINVAL;            // groups of four sites must not leave their row
     *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
     if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
-    if (lane_mode(rng_mode)) *out += round_up((size_t)lane_ring(rng_mode) * g.lanes_default * sizeof(uint32_t), 256);
+    if (lane_mode(rng_mode)) *out += round_up((size_t)lane_ring(rng_mode) * lanes_default(g, rng_mode) * sizeof(uint32_t), 256);
     return ISING_OK;
 }
 
@@ -402,7 +407,7 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->s0_ready = false;
     h->slots_clean = false;
     h->lane_state = lane_mode(rng_mode) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
-    h->nlanes = lane_mode(rng_mode) ? h->g.lanes_default : 0;
+    h->nlanes = lane_mode(rng_mode) ? lanes_default(h->g, rng_mode) : 0;
     h->lanes_ready = false;
     *out = h;
     return ISING_OK;
@@ -598,7 +603,7 @@ int ising_get_lanes(const ising_t *h, uint32_t *nlanes)
 
 int ising_set_lanes(ising_t *h, uint32_t nlanes)
 {
-    if (!h || !lane_mode(h->rng_mode) || h->lanes_ready || nlanes < 1 || nlanes > h->g.lanes_default) return ISING_EINVAL;
+    if (!h || !lane_mode(h->rng_mode) || h->lanes_ready || nlanes < 1 || nlanes > lanes_default(h->g, h->rng_mode)) return ISING_EINVAL;
     h->nlanes = nlanes;
     return ISING_OK;
 }
@@ -641,10 +646,11 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
         count_odd_minstd<<<blocks, 128, 0, st>>>((uint32_t *)d_state, nlanes, ndraws, odd, sum);
     } else if (kind == ISING_RNG_PR_SHARED) {
         ln.pos0 = (uint32_t)(ndrawn_before % 62u);
-        count_odd_lanes<GEN_PR><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
+        if (ndraws >= 62) count_odd_lanes<GEN_PR, true><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
+        else count_odd_lanes<GEN_PR, false><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
     } else {
         ln.pos0 = (uint32_t)(ndrawn_before % 624u);
-        count_odd_lanes<GEN_MT><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
+        count_odd_lanes<GEN_MT, false><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
     }
     return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
 }

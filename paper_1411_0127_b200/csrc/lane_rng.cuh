@@ -44,43 +44,63 @@ __device__ __forceinline__ uint32_t mt_temper(uint32_t y)
     return y;
 }
 
-// Four consecutive draws of the lane whose words are st[r * stride]; pos is advanced by 4.
+// Four consecutive draws of the lane whose words are st[r * stride], in two steps so that a kernel can put other loads
+// between them: lane_load4 issues every state load of the four draws and advances pos by 4, lane_finish4 computes the
+// draws and stores the four new state words.
+template <int GEN> struct LaneOperands {
+    uint32_t v[GEN == GEN_PR ? 12 : 9];
+    uint32_t p[4];   // ring positions of the four draws (the words they overwrite)
+};
+
 template <int GEN>
-__device__ __forceinline__ void lane_next4(uint32_t *st, size_t stride, uint32_t &pos, uint32_t R[4])
+__device__ __forceinline__ void lane_load4(const uint32_t *st, size_t stride, uint32_t &pos, LaneOperands<GEN> &o)
 {
     constexpr uint32_t RING = LaneRing<GEN>::size;
     uint32_t p[5];
 #pragma unroll
     for (int d = 0; d < 5; ++d) p[d] = ring_add<RING>(pos, (uint32_t)d);
+#pragma unroll
+    for (int d = 0; d < 4; ++d) o.p[d] = p[d];
     if (GEN == GEN_PR) {
-        uint32_t a[4], b[4], c[4];
 #pragma unroll
         for (int d = 0; d < 4; ++d) {
-            a[d] = st[(size_t)ring_add<RING>(p[d], RING - 24) * stride];
-            b[d] = st[(size_t)ring_add<RING>(p[d], RING - 55) * stride];
-            c[d] = st[(size_t)p[d + 1] * stride];   // i - 61 = i + 1 (mod 62)
-        }
-#pragma unroll
-        for (int d = 0; d < 4; ++d) {
-            const uint32_t v = a[d] + b[d];
-            st[(size_t)p[d] * stride] = v;
-            R[d] = v ^ c[d];
+            o.v[d] = st[(size_t)ring_add<RING>(p[d], RING - 24) * stride];
+            o.v[4 + d] = st[(size_t)ring_add<RING>(p[d], RING - 55) * stride];
+            o.v[8 + d] = st[(size_t)p[d + 1] * stride];   // i - 61 = i + 1 (mod 62)
         }
     } else {
-        uint32_t m[5], x[4];
 #pragma unroll
-        for (int d = 0; d < 5; ++d) m[d] = st[(size_t)p[d] * stride];
+        for (int d = 0; d < 5; ++d) o.v[d] = st[(size_t)p[d] * stride];
 #pragma unroll
-        for (int d = 0; d < 4; ++d) x[d] = st[(size_t)ring_add<RING>(p[d], 397) * stride];
+        for (int d = 0; d < 4; ++d) o.v[5 + d] = st[(size_t)ring_add<RING>(p[d], 397) * stride];
+    }
+    pos = p[4];
+}
+
+template <int GEN>
+__device__ __forceinline__ void lane_finish4(uint32_t *st, size_t stride, const LaneOperands<GEN> &o, uint32_t R[4])
+{
 #pragma unroll
-        for (int d = 0; d < 4; ++d) {
-            const uint32_t y = (m[d] & 0x80000000u) | (m[d + 1] & 0x7fffffffu);
-            const uint32_t v = x[d] ^ (y >> 1) ^ ((y & 1u) ? 0x9908b0dfu : 0u);
-            st[(size_t)p[d] * stride] = v;
+    for (int d = 0; d < 4; ++d) {
+        if (GEN == GEN_PR) {
+            const uint32_t v = o.v[d] + o.v[4 + d];
+            st[(size_t)o.p[d] * stride] = v;
+            R[d] = v ^ o.v[8 + d];
+        } else {
+            const uint32_t y = (o.v[d] & 0x80000000u) | (o.v[d + 1] & 0x7fffffffu);
+            const uint32_t v = o.v[5 + d] ^ (y >> 1) ^ ((y & 1u) ? 0x9908b0dfu : 0u);
+            st[(size_t)o.p[d] * stride] = v;
             R[d] = mt_temper(v);
         }
     }
-    pos = p[4];
+}
+
+template <int GEN>
+__device__ __forceinline__ void lane_next4(uint32_t *st, size_t stride, uint32_t &pos, uint32_t R[4])
+{
+    LaneOperands<GEN> o;
+    lane_load4<GEN>(st, stride, pos, o);
+    lane_finish4<GEN>(st, stride, o, R);
 }
 
 __device__ __forceinline__ uint64_t splitmix64_output_dev(uint64_t seed, uint64_t n)
@@ -118,6 +138,9 @@ __global__ void __launch_bounds__(128) lanes_init(uint32_t *state, uint32_t nlan
 // unit of half_sweep_shared_vec), for each the coded batches b = 0 .. nbatches-1, and takes four draws per (group, batch)
 // in the order of R19; a lane whose last group does not exist still draws.  Consecutive lanes hold consecutive groups,
 // so the lattice loads of a warp are the same coalesced 512-byte rows as in half_sweep_shared_vec.
+//
+// (Holding the twelve state operands in registers across the lattice loads, so that both round trips overlap, spills at 64
+// registers and was slower: 0.249 against 0.239 ps/flip.)
 // ---------------------------------------------------------------------------------------------------
 template <int GEN>
 __global__ void __launch_bounds__(128, 8)
@@ -163,21 +186,33 @@ half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uin
 // PAPER.md:196-197, Table II: "its kernel version counting the fraction of odd numbers".  Every lane draws ndraws numbers
 // (a multiple of 4) continuing from ring position pos0; odd[q] = how many were odd, sum[q] = their sum mod 2^64.
 // ---------------------------------------------------------------------------------------------------
-template <int GEN>
+// STAGE (Parisi-Rapuano only): the 62-word rings of the CTA's 128 lanes are copied to shared memory (31 KB, word r of thread i
+// at ring[r * 128 + i]: conflict-free) for the duration of the launch and written back at the end: 852 -> 1313 G numbers/s.
+// (The same staging in the half-sweep kernel was slower than global-memory rings at every lane count -- 0.283 against 0.239
+// ps/flip at best: 7 x 31 KB of shared memory leave almost no L1 for the lattice loads -- and is not used there.)
+template <int GEN, bool STAGE>
 __global__ void __launch_bounds__(128)
 count_odd_lanes(const LaneArgs ln, uint64_t ndraws, unsigned long long *odd, unsigned long long *sum)
 {
+    static_assert(!STAGE || GEN == GEN_PR, "only the 62-word ring fits shared memory");
+    __shared__ uint32_t ring[STAGE ? 62 * 128 : 1];
     const uint32_t q = blockIdx.x * 128u + threadIdx.x;
     if (q >= ln.nlanes) return;
-    uint32_t *st = ln.state + q;
+    uint32_t *gst = ln.state + q;
+    uint32_t *st = STAGE ? ring + threadIdx.x : gst;
+    const size_t stride = STAGE ? 128u : ln.nlanes;
+    if (STAGE)
+        for (uint32_t r = 0; r < 62u; ++r) st[r * 128u] = gst[(size_t)r * ln.nlanes];
     uint32_t pos = ln.pos0;
     unsigned long long o = 0, s = 0;
     for (uint64_t n = 0; n < ndraws; n += 4) {
         uint32_t R[4];
-        lane_next4<GEN>(st, ln.nlanes, pos, R);
+        lane_next4<GEN>(st, stride, pos, R);
         o += (R[0] & 1u) + (R[1] & 1u) + (R[2] & 1u) + (R[3] & 1u);
         s += (unsigned long long)R[0] + R[1] + R[2] + R[3];
     }
+    if (STAGE)
+        for (uint32_t r = 0; r < 62u; ++r) gst[(size_t)r * ln.nlanes] = st[r * 128u];
     odd[q] = o;
     sum[q] = s;
 }

@@ -42,8 +42,9 @@ def assert_same_state(o, g, what=""):
 
 # nlanes None = the default min(N/8, 151552); the others give several rounds per lane and a ragged last round
 @pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
+# (16, 32, 7), (24, 64, 50): many rounds per lane, the ring wraps several times inside one launch
 @pytest.mark.parametrize("L,ns,nlanes", [(8, 32, None), (8, 64, 24), (16, 32, 100), (16, 96, 512), (24, 32, 333), (40, 32, None),
-                                         (40, 64, 1000), (64, 32, 4096)])
+                                         (40, 64, 1000), (64, 32, 4096), (16, 32, 7), (24, 64, 50)])
 def test_lane_mode_sweep_equals_the_oracle(mode, L, ns, nlanes):
     spins, J = synth.make_spins(L, ns, 71), synth.make_couplings(L, ns, 72)
     o, g = make_pair(L, ns, mode, nlanes, spins, J)
@@ -109,7 +110,7 @@ def test_lane_mode_argument_checks():
 # ------------------------------------------------------------------------------------------------ Table II: odd count
 
 @pytest.mark.parametrize("kind", [PHILOX, MINSTD, PR_SHARED, MT19937_SHARED])
-@pytest.mark.parametrize("nlanes,chunks", [(1, (4, 8)), (37, (64, 700, 1236)), (1000, (2000,))])
+@pytest.mark.parametrize("nlanes,chunks", [(1, (4, 8)), (37, (64, 700, 1236)), (1000, (2000,)), (300, (60, 64, 4))])
 def test_count_odd_equals_the_oracle(kind, nlanes, chunks):
     seed = 99
     nbytes = binding.ising_prng_state_bytes(kind, nlanes)
