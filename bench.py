@@ -39,8 +39,8 @@ ALG_BYTES_PER_FLIP = {0: 9 / 8, 1: 9 / 8 + 4}  # 9N/16 bytes per half-sweep = 1.
 # ira[i-24], ira[i-55], ira[i-61] and writes ira[i]; MT19937 in blocks of four draws reads mt[i..i+4], mt[i+397..i+400], writes 4
 LANE_STATE_BYTES_PER_DRAW = {3: 16.0, 4: 13.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch at L=1024 from the ncu --set full capture in
-# profiles/r1h_end_of_round.md (algorithmic: 9N/16 = 603,979,776 B)
-NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 57.63e6, 1: 2684.5e6 + 60.9e6}
+# profiles/r1m_end_of_round.md (algorithmic: 9N/16 = 603,979,776 B)
+NCU_TRAFFIC_BYTES_L1024 = {0: 537.05e6 + 59.04e6, 1: 2684.54e6 + 60.23e6}
 
 
 def measured_peaks():

@@ -55,6 +55,20 @@ def test_lane_mode_sweep_equals_the_oracle(mode, L, ns, nlanes):
 
 
 @pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
+def test_lane_mode_with_the_default_wave_of_lanes(mode):
+    """The launch configuration bench.py times: 151552 lanes (1184 CTAs of 128, one wave).  L = 128 has 262144 groups per colour:
+    two rounds per lane, the second one ragged; 64 samples = two coded batches."""
+    L, ns = 128, 64
+    spins, J = synth.make_spins(L, ns, 77), synth.make_couplings(L, ns, 78)
+    o, g = make_pair(L, ns, mode, None, spins, J)
+    assert g.ising_get_lanes() == 148 * 1024
+    for beta, n in ((1 / 1.1, 1), (0.5, 1)):
+        o.sweep(beta, n)
+        g.ising_sweep(beta, n)
+        assert_same_state(o, g, f"lane mode {mode}, default lanes, beta={beta}")
+
+
+@pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
 def test_lane_mode_many_half_sweeps_cross_the_mt_ring(mode):
     """L = 8, 2 batches, 3 lanes: 4 * 2 * ceil(64/3) = 176 draws per lane per half-sweep; 8 half-sweeps = 1408 draws cross the
     624-word MT block twice and the 62-word ring 22 times.  Sweeps split over several calls (the state persists)."""
@@ -127,6 +141,26 @@ def test_count_odd_equals_the_oracle(kind, nlanes, chunks):
         tot_all += tot.cpu().numpy().view(np.uint64)
         done += n
     want_odd, want_tot = ea3d.count_odd(kind, seed, nlanes, done)
+    assert np.array_equal(odd_all, want_odd)
+    assert np.array_equal(tot_all, want_tot)
+
+
+@pytest.mark.parametrize("kind", [PHILOX, MINSTD, PR_SHARED, MT19937_SHARED])
+def test_count_odd_in_the_bench_configuration(kind):
+    """bench.py's Table II run: 151552 lanes x 4096 draws per call (two calls here), every lane against the oracle."""
+    seed, nlanes, nd = synth.DYN_SEED, 148 * 1024, 4096
+    nbytes = binding.ising_prng_state_bytes(kind, nlanes)
+    state = torch.empty(nbytes, dtype=torch.uint8, device="cuda") if nbytes else None
+    binding.ising_prng_init(kind, seed, nlanes, state)
+    odd = torch.zeros(nlanes, dtype=torch.int64, device="cuda")
+    tot = torch.zeros(nlanes, dtype=torch.int64, device="cuda")
+    odd_all = np.zeros(nlanes, np.uint64)
+    tot_all = np.zeros(nlanes, np.uint64)
+    for r in range(2):
+        binding.ising_prng_count_odd(kind, seed, nlanes, r * nd, nd, state, odd, tot)
+        odd_all += odd.cpu().numpy().view(np.uint64)
+        tot_all += tot.cpu().numpy().view(np.uint64)
+    want_odd, want_tot = ea3d.count_odd(kind, seed, nlanes, 2 * nd)
     assert np.array_equal(odd_all, want_odd)
     assert np.array_equal(tot_all, want_tot)
 
