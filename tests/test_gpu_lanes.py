@@ -175,3 +175,36 @@ def test_count_odd_argument_checks():
     assert binding.ising_prng_state_bytes(MINSTD, 10) == 40
     assert binding.ising_prng_state_bytes(PR_SHARED, 10) == 62 * 40
     assert binding.ising_prng_state_bytes(MT19937_SHARED, 10) == 624 * 40
+
+
+# ------------------------------------------------------------------------------------------------ memory safety
+
+@pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
+@pytest.mark.parametrize("L,ns,nlanes", [(8, 32, None), (16, 64, 100), (24, 32, 7)])
+def test_lane_kernels_write_only_inside_their_buffers(mode, L, ns, nlanes):
+    """Memory safety without a sanitizer: the workspace (lattice + strided generator state) and the Table II state / result
+    buffers sit between guard regions filled with a pattern; after every entry point has run the guards must be untouched."""
+    nbytes = binding.ising_workspace_bytes(L, ns, mode)
+    G = 1 << 20
+    buf = torch.full((G + nbytes + G,), 0xA5, dtype=torch.uint8, device="cuda")
+    spins, J = synth.make_spins(L, ns, 95), synth.make_couplings(L, ns, 96)
+    g = Ising(L, ns, SEED, mode, workspace=buf[G:G + nbytes])
+    if nlanes is not None:
+        g.ising_set_lanes(nlanes)
+    g.ising_load_state(dev(spins), dev(J))
+    g.ising_sweep(1 / 1.1, 3)
+    g.ising_sweep_trace(1 / 1.1, 1, every_half_sweeps=1)
+    g.ising_get_spins()
+    torch.cuda.synchronize()
+    assert bool((buf[:G] == 0xA5).all()) and bool((buf[G + nbytes:] == 0xA5).all()), "workspace guard overwritten"
+    # Table II kernels: state and per-lane results between guards
+    n = 333
+    sb = binding.ising_prng_state_bytes(mode, n)
+    st = torch.full((G + sb + G,), 0xA5, dtype=torch.uint8, device="cuda")
+    res = torch.full((1024 + 2 * n + 1024,), 0x5A5A5A5A5A5A5A5A, dtype=torch.int64, device="cuda")
+    binding.ising_prng_init(mode, 5, n, st[G:G + sb])
+    for first, nd in ((0, 1000), (1000, 40), (1040, 64)):   # staged (>= 62 draws) and unstaged Parisi-Rapuano kernels
+        binding.ising_prng_count_odd(mode, 5, n, first, nd, st[G:G + sb], res[1024:1024 + n], res[1024 + n:1024 + 2 * n])
+    torch.cuda.synchronize()
+    assert bool((st[:G] == 0xA5).all()) and bool((st[G + sb:] == 0xA5).all()), "state guard overwritten"
+    assert bool((res[:1024] == 0x5A5A5A5A5A5A5A5A).all()) and bool((res[1024 + 2 * n:] == 0x5A5A5A5A5A5A5A5A).all()), "result guard"
