@@ -344,6 +344,32 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         else launch_pdl(energy_site_packed<1>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
         return check_launch(h);
     }
+    if (g.nsamples != 1 && g.Hc < (1ull << 31) && h->kernel_choice != 1) {  // bit-sliced column sums, one fused launch
+        if (!h->slots_clean) {
+            if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess ||
+                cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess)
+                return ISING_ECUDA;
+            h->slots_clean = true;
+        }
+        const LatticeArrays A = h->arrays(0);
+        MeasureArgs m;
+        for (int c = 0; c < 2; ++c) {
+            m.S[c] = A.S[c];
+            for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
+        }
+        m.L = g.L;
+        // chunk = nblocks x 256 sites per warp: long enough to amortise the 21 plane transposes at its end, short enough for
+        // several waves of CTAs (16 blocks = 4096 sites per warp from L = 256 x 32 samples on)
+        int nblocks = (int)(g.Hc / (256u * 2048u));
+        nblocks = nblocks < 1 ? 1 : nblocks > 16 ? 16 : nblocks;
+        static_assert(16 <= EN_MAX_BLOCKS, "counter planes");
+        const uint32_t cpc = (uint32_t)((g.Hc + 256u * nblocks - 1) / (256u * nblocks));
+        launch_pdl(energy_sample_packed_sliced, dim3((2 * cpc + 7) / 8, (unsigned)g.nbatches), dim3(256), st, m,
+                   (size_t)(8 * g.array_words), h->acc, (unsigned int *)(slots + 2 * ACC_SLOTS), (uint32_t)g.Hc, cpc, nblocks,
+                   g.nsamples, (long long)g.N, d_E, d_M);
+        return check_launch(h);
+    }
+    h->slots_clean = false;  // the generic kernels below leave their counts in acc
     if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess)
         return ISING_ECUDA;
     const int nb = g.nsamples == 1 ? 1 : g.nbatches;
@@ -460,6 +486,23 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
         const LatticeArrays A = h->arrays(b);
         const uint32_t *sp = d_spins + (size_t)b * 32 * W;
         const uint32_t *jp = d_J + (size_t)b * 32 * 3 * W;
+        if (g.L % 32 == 0 && h->kernel_choice != 1) {  // tile kernel: one launch per batch, all four arrays, both colours
+            GatherTileArgs t;
+            t.canon[0] = sp;
+            t.stride[0] = W;
+            t.out[0][0] = A.S[0];
+            t.out[0][1] = A.S[1];
+            for (int d = 0; d < 3; ++d) {
+                t.canon[1 + d] = jp + (size_t)d * W;
+                t.stride[1 + d] = 3 * W;
+                t.out[1 + d][0] = A.J[d][0];
+                t.out[1 + d][1] = A.J[d][1];
+            }
+            gather_sample_packed_tiles<<<dim3((unsigned)((W + 127) / 128), 4), 128, 0, st>>>(t, g.L, (uint32_t)W);
+            const int rc = check_launch(h);
+            if (rc != ISING_OK) return rc;
+            continue;
+        }
         for (int c = 0; c < 2; ++c) {
             gather_sample_packed<<<grid, 256, 0, st>>>(sp, W, A.S[c], c, g.L, g.Hc);
             for (int d = 0; d < 3; ++d)
@@ -490,6 +533,13 @@ int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
     }
     for (int b = 0; b < g.nbatches; ++b) {
         const LatticeArrays A = h->arrays(b);
+        if (g.L % 32 == 0 && h->kernel_choice != 1) {
+            scatter_sample_packed_tiles<<<(unsigned)((W + 127) / 128), 128, 0, st>>>(A.S[0], A.S[1], d_out + (size_t)b * 32 * W, W, g.L,
+                                                                                  (uint32_t)W);
+            const int rc = check_launch(h);
+            if (rc != ISING_OK) return rc;
+            continue;
+        }
         const dim3 grid((unsigned)((W + 255) / 256), 32);
         scatter_sample_packed<<<grid, 256, 0, st>>>(A.S[0], A.S[1], d_out + (size_t)b * 32 * W, W, g.L, W, g.N);
         const int rc = check_launch(h);

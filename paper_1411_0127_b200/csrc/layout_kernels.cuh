@@ -178,4 +178,92 @@ scatter_sample_packed(const uint32_t *__restrict__ S0, const uint32_t *__restric
     canon[sample * sample_stride + cw] = w;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Sample-packed, L a multiple of 32 (a canonical word = 32 consecutive x of one row): tile kernels.  One thread owns one
+// canonical word index cw of all 32 samples of a batch: 32 words (lane l reads word cw0 + l of sample s: 128 contiguous
+// bytes per warp load), transposed in registers as a 32 x 32 bit matrix (5 x 16 masked swaps), are the 32 site words of
+// the row segment; the 16 of each colour go out as four 128-bit stores.  The scatter kernel is the inverse.
+// ---------------------------------------------------------------------------------------------------
+template <int J>
+__device__ __forceinline__ void transpose32_stage(uint32_t (&A)[32])
+{
+    constexpr uint32_t m = J == 16 ? 0x0000FFFFu : J == 8 ? 0x00FF00FFu : J == 4 ? 0x0F0F0F0Fu : J == 2 ? 0x33333333u : 0x55555555u;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        if ((k & J) == 0) {
+            const uint32_t t = ((A[k] >> J) ^ A[k + J]) & m;
+            A[k] ^= t << J;
+            A[k + J] ^= t;
+        }
+    }
+}
+
+__device__ __forceinline__ void transpose32_in_registers(uint32_t (&A)[32])
+{  // bit b of A[s]  <->  bit s of A[b]
+    transpose32_stage<16>(A);
+    transpose32_stage<8>(A);
+    transpose32_stage<4>(A);
+    transpose32_stage<2>(A);
+    transpose32_stage<1>(A);
+}
+
+struct GatherTileArgs {
+    const uint32_t *canon[4];  // first sample of the batch: spins, Jx, Jy, Jz
+    uint64_t stride[4];        // words between consecutive samples
+    uint32_t *out[4][2];       // sample-packed arrays of the two colours
+};
+
+// grid = (ceil(ncw / 128), 4 arrays)
+__global__ void __launch_bounds__(128) gather_sample_packed_tiles(const __grid_constant__ GatherTileArgs a, int L, uint32_t ncw)
+{
+    const int arr = blockIdx.y;
+    const uint32_t cw = blockIdx.x * 128u + threadIdx.x;
+    if (cw >= ncw) return;
+    const uint32_t wpr = (uint32_t)L >> 5, r = cw / wpr, y = r % (uint32_t)L, z = r / (uint32_t)L;
+    const uint32_t base = ((uint32_t)L >> 1) * r + (cw - r * wpr) * 16u;   // colour rank of the first site of either colour
+    const uint32_t *__restrict__ src = a.canon[arr] + cw;
+    const uint64_t stride = a.stride[arr];
+    uint32_t A[32];
+#pragma unroll
+    for (int s = 0; s < 32; ++s) A[s] = __ldg(src + (uint64_t)s * stride);
+    transpose32_in_registers(A);   // A[b] = the 32 samples of site 32 cw + b
+    const bool odd0 = ((y + z) & 1u) != 0;   // colour 0 holds the odd x of this row
+    uint32_t *o0 = a.out[arr][0] + base, *o1 = a.out[arr][1] + base;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        uint4 v0, v1;
+        v0.x = odd0 ? A[8 * q + 1] : A[8 * q];     v1.x = odd0 ? A[8 * q] : A[8 * q + 1];
+        v0.y = odd0 ? A[8 * q + 3] : A[8 * q + 2]; v1.y = odd0 ? A[8 * q + 2] : A[8 * q + 3];
+        v0.z = odd0 ? A[8 * q + 5] : A[8 * q + 4]; v1.z = odd0 ? A[8 * q + 4] : A[8 * q + 5];
+        v0.w = odd0 ? A[8 * q + 7] : A[8 * q + 6]; v1.w = odd0 ? A[8 * q + 6] : A[8 * q + 7];
+        reinterpret_cast<uint4 *>(o0)[q] = v0;
+        reinterpret_cast<uint4 *>(o1)[q] = v1;
+    }
+}
+
+// grid = ceil(ncw / 128): canonical spins of the 32 samples of a batch from the two colour arrays
+__global__ void __launch_bounds__(128)
+scatter_sample_packed_tiles(const uint32_t *__restrict__ S0, const uint32_t *__restrict__ S1, uint32_t *__restrict__ canon,
+                            uint64_t sample_stride, int L, uint32_t ncw)
+{
+    const uint32_t cw = blockIdx.x * 128u + threadIdx.x;
+    if (cw >= ncw) return;
+    const uint32_t wpr = (uint32_t)L >> 5, r = cw / wpr, y = r % (uint32_t)L, z = r / (uint32_t)L;
+    const uint32_t base = ((uint32_t)L >> 1) * r + (cw - r * wpr) * 16u;
+    const bool odd0 = ((y + z) & 1u) != 0;
+    uint32_t A[32];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const uint4 v0 = __ldg(reinterpret_cast<const uint4 *>(S0 + base) + q);
+        const uint4 v1 = __ldg(reinterpret_cast<const uint4 *>(S1 + base) + q);
+        A[8 * q] = odd0 ? v1.x : v0.x;     A[8 * q + 1] = odd0 ? v0.x : v1.x;
+        A[8 * q + 2] = odd0 ? v1.y : v0.y; A[8 * q + 3] = odd0 ? v0.y : v1.y;
+        A[8 * q + 4] = odd0 ? v1.z : v0.z; A[8 * q + 5] = odd0 ? v0.z : v1.z;
+        A[8 * q + 6] = odd0 ? v1.w : v0.w; A[8 * q + 7] = odd0 ? v0.w : v1.w;
+    }
+    transpose32_in_registers(A);   // A[s] = canonical word cw of sample s
+#pragma unroll
+    for (int s = 0; s < 32; ++s) canon[(uint64_t)s * sample_stride + cw] = A[s];
+}
+
 }  // namespace isingk

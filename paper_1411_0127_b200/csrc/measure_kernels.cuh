@@ -191,6 +191,172 @@ energy_sample_packed(const MeasureArgs a, unsigned long long *acc /* [32][2] */,
     }
 }
 
+// Sample-packed, bit-sliced: the per-sample counts are the column sums of the bond words (and of the spin words).  A thread
+// adds the words of its sites into vertical counters, i.e. bit planes of weight 1, 2, 4, ...: eight words at a time go
+// through a carry-save adder tree (Harley-Seal: 7 full adders = 14 LOP3 per 8 words, the carry of weight 8 ripples into the
+// upper planes), about 4 logic operations per word instead of 32 ballots.  At the end of its chunk the warp transposes
+// every plane across its lanes (5 shuffle stages), after which lane b holds column b of all 32 lanes, i.e. sample b, and a
+// popcount per plane gives the counts.  A warp owns one chunk of nblocks x 8 x 32 consecutive sites of one colour
+// (coalesced loads: lane l takes the sites l, l + 32, ...); any even L.
+constexpr int EN_MAX_BLOCKS = 64;   // 8 sites x 64 blocks x 3 bonds = 1536 < 2^11 (bond planes), 512 spins < 2^10
+
+// (carry, sum) = a + b + c per bit: two LOP3
+__device__ __forceinline__ void full_add(uint32_t &carry, uint32_t &sum, uint32_t a, uint32_t b, uint32_t c)
+{
+    const uint32_t u = a ^ b;
+    carry = (a & b) | (u & c);
+    sum = u ^ c;
+}
+
+template <int KH>
+struct VerticalCounter {   // planes of weight 1, 2, 4 and KH planes of weight 8, 16, ...
+    uint32_t ones = 0, twos = 0, fours = 0, hi[KH] = {};
+    __device__ __forceinline__ void add8(const uint32_t *w)
+    {
+        uint32_t twosA, twosB, foursA, foursB, eights;
+        full_add(twosA, ones, ones, w[0], w[1]);
+        full_add(twosB, ones, ones, w[2], w[3]);
+        full_add(foursA, twos, twos, twosA, twosB);
+        full_add(twosA, ones, ones, w[4], w[5]);
+        full_add(twosB, ones, ones, w[6], w[7]);
+        full_add(foursB, twos, twos, twosA, twosB);
+        full_add(eights, fours, fours, foursA, foursB);
+#pragma unroll
+        for (int p = 0; p < KH; ++p) {
+            const uint32_t c = hi[p] & eights;
+            hi[p] ^= eights;
+            eights = c;
+        }
+    }
+};
+
+template <int J>
+__device__ __forceinline__ uint32_t warp_transpose32_stage(uint32_t x, int lane)
+{
+    constexpr uint32_t m = J == 16 ? 0x0000FFFFu : J == 8 ? 0x00FF00FFu : J == 4 ? 0x0F0F0F0Fu : J == 2 ? 0x33333333u : 0x55555555u;
+    const uint32_t other = __shfl_xor_sync(0xFFFFFFFFu, x, J);
+    return (lane & J) ? (((other >> J) & m) | (x & ~m)) : ((x & m) | ((other & m) << J));
+}
+// Lane i holds row i of a 32 x 32 bit matrix; returns column `lane` (bit i = bit `lane` of row i).
+__device__ __forceinline__ uint32_t warp_transpose32(uint32_t x, int lane)
+{
+    x = warp_transpose32_stage<16>(x, lane);
+    x = warp_transpose32_stage<8>(x, lane);
+    x = warp_transpose32_stage<4>(x, lane);
+    x = warp_transpose32_stage<2>(x, lane);
+    return warp_transpose32_stage<1>(x, lane);
+}
+
+template <int KH>
+__device__ __forceinline__ unsigned int column_count(const VerticalCounter<KH> &v, int lane)
+{   // the count of column `lane` summed over the 32 lanes of the warp
+    unsigned int n = __popc(warp_transpose32(v.ones, lane)) + 2u * __popc(warp_transpose32(v.twos, lane)) +
+                     4u * __popc(warp_transpose32(v.fours, lane));
+#pragma unroll
+    for (int p = 0; p < KH; ++p) n += (unsigned int)__popc(warp_transpose32(v.hi[p], lane)) << (3 + p);
+    return n;
+}
+
+// grid = (ceil(2 * chunks_per_colour / 8), batches) CTAs of 8 warps, one chunk per warp; blockIdx.y = coded batch, whose arrays
+// start batch_stride words after those of batch 0 (a holds batch 0) and whose counters are acc[64 b .. 64 b + 63].
+// One launch does everything, as in energy_site_packed: the counters are zero on entry, and the last CTA to finish (ticket)
+// turns them into E and M of all samples (R16) and clears counters and ticket for the next call.
+__global__ void __launch_bounds__(256, 3)
+energy_sample_packed_sliced(const __grid_constant__ MeasureArgs a, size_t batch_stride, unsigned long long *acc /* [batch][32][2] */,
+                            unsigned int *ticket, uint32_t Hc, uint32_t chunks_per_colour, int nblocks, int nsamples, long long N,
+                            long long *E, long long *M)
+{
+    __shared__ unsigned int sh_unsat[32], sh_up[32];
+    if (threadIdx.x < 32) { sh_unsat[threadIdx.x] = 0; sh_up[threadIdx.x] = 0; }
+    __syncthreads();
+    const uint32_t L = (uint32_t)a.L, H = L >> 1, HL = H * L;
+    const int lane = threadIdx.x & 31;
+    const uint32_t chunk = blockIdx.x * 8u + (threadIdx.x >> 5);
+    const size_t boff = (size_t)blockIdx.y * batch_stride;
+    acc += 64u * blockIdx.y;
+    wait_for_previous_kernel();
+    if (chunk < 2u * chunks_per_colour) {   // warp-uniform
+        const int c = chunk >= chunks_per_colour;
+        uint32_t j = (chunk - (c ? chunks_per_colour : 0u)) * (256u * (uint32_t)nblocks) + (uint32_t)lane;
+        uint32_t m = j % H, r = j / H, y = r % L, z = r / L;
+        const uint32_t *__restrict__ S = a.S[c] + boff, *__restrict__ So = a.S[1 - c] + boff;
+        const uint32_t *__restrict__ Jx = a.J[0][c] + boff, *__restrict__ Jy = a.J[1][c] + boff, *__restrict__ Jz = a.J[2][c] + boff;
+        VerticalCounter<8> bonds;   // 11 planes
+        VerticalCounter<7> spins;   // 10 planes
+        for (int blk = 0; blk < nblocks; ++blk) {
+            uint32_t e[24], s[8];
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                // indices of four sites first, then their 28 loads back to back, then the bond words: nothing between the
+                // loads depends on a loaded value, so all of them are in flight together
+                uint32_t js[4], jx[4], jy[4], jz[4], ok[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const bool valid = j < Hc;
+                    const uint32_t xodd = (y + z + (uint32_t)c) & 1u;
+                    ok[i] = valid ? 0xFFFFFFFFu : 0u;
+                    js[i] = valid ? j : 0u;
+                    jx[i] = valid ? j - m + (xodd ? (m + 1 == H ? 0u : m + 1) : m) : 0u;
+                    jy[i] = valid ? ((y + 1 == L) ? j - (HL - H) : j + H) : 0u;
+                    jz[i] = valid ? ((z + 1 == L) ? j - (Hc - HL) : j + HL) : 0u;
+                    j += 32u;
+                    m += 32u;
+                    while (m >= H) {
+                        m -= H;
+                        if (++y == L) { y = 0; ++z; }
+                    }
+                }
+                uint32_t rs[4], rjx[4], rjy[4], rjz[4], rox[4], roy[4], roz[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    rs[i] = __ldg(S + js[i]);
+                    rjx[i] = __ldg(Jx + js[i]);
+                    rjy[i] = __ldg(Jy + js[i]);
+                    rjz[i] = __ldg(Jz + js[i]);
+                    rox[i] = __ldg(So + jx[i]);
+                    roy[i] = __ldg(So + jy[i]);
+                    roz[i] = __ldg(So + jz[i]);
+                }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int k = 4 * half + i;
+                    s[k] = rs[i] & ok[i];
+                    e[3 * k] = (rjx[i] ^ rs[i] ^ rox[i]) & ok[i];
+                    e[3 * k + 1] = (rjy[i] ^ rs[i] ^ roy[i]) & ok[i];
+                    e[3 * k + 2] = (rjz[i] ^ rs[i] ^ roz[i]) & ok[i];
+                }
+            }
+            bonds.add8(e);
+            bonds.add8(e + 8);
+            bonds.add8(e + 16);
+            spins.add8(s);
+        }
+        atomicAdd(&sh_unsat[lane], column_count(bonds, lane));
+        atomicAdd(&sh_up[lane], column_count(spins, lane));
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        atomicAdd(&acc[2 * threadIdx.x], (unsigned long long)sh_unsat[threadIdx.x]);
+        atomicAdd(&acc[2 * threadIdx.x + 1], (unsigned long long)sh_up[threadIdx.x]);
+    }
+    __shared__ bool is_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        is_last = atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1;  // every other CTA's atomics are visible then
+    }
+    __syncthreads();
+    if (is_last) {
+        acc -= 64u * blockIdx.y;
+        for (int sidx = threadIdx.x; sidx < nsamples; sidx += 256) {   // read and clear
+            const unsigned long long tu = atomicExch(&acc[2 * sidx], 0ull), tp = atomicExch(&acc[2 * sidx + 1], 0ull);
+            if (E) E[sidx] = 2 * (long long)tu - 3 * N;
+            if (M) M[sidx] = 2 * (long long)tp - N;
+        }
+        if (threadIdx.x == 0) *ticket = 0u;
+    }
+}
+
 // E = 2*unsat - 3N, M = 2*up - N  (R16), one thread per sample (sample-packed and generic paths).
 __global__ void finalize_energy(const unsigned long long *acc, int nsamples, long long N, long long *E, long long *M)
 {

@@ -49,8 +49,10 @@ def assert_same_state(o, g, what=""):
 # ------------------------------------------------------------------------------------------------ load / get / energy
 
 @pytest.mark.parametrize("L,nsamples", [(4, 1), (6, 1), (16, 1), (24, 1), (64, 1), (128, 1), (256, 1), (4, 32), (6, 32),
-                                        (16, 64)])
+                                        (16, 64), (10, 32), (32, 32), (64, 96), (96, 32), (128, 64)])
 def test_layout_round_trip_and_energy(L, nsamples):
+    """Rows a9 / a10.  Sample-packed: the bit-sliced energy kernel (any L) and, for L a multiple of 32, the register-transpose
+    tile kernels of load / get; kernel choice 1 runs the one-bit-at-a-time kernels on the same data."""
     spins, J = synth.make_spins(L, nsamples, 7), synth.make_couplings(L, nsamples, 3)
     o, g = make_pair(L, nsamples, PHILOX, spins, J)
     assert_same_state(o, g, "after load")
@@ -58,6 +60,15 @@ def test_layout_round_trip_and_energy(L, nsamples):
     if nsamples == 1 and L >= 64:  # the generic measurement kernel on the same internal layout
         g.ising_set_kernel(1)
         assert_same_state(o, g, "generic measure")
+    if nsamples > 1:
+        g.ising_set_kernel(1)      # generic energy and scatter on the arrays the tile kernel wrote
+        assert_same_state(o, g, "generic measure / scatter after tile gather")
+        g.ising_load_state(dev(spins), dev(J))   # generic gather
+        g.ising_set_kernel(0)
+        assert_same_state(o, g, "tile scatter / sliced energy after generic gather")
+        o.sweep(0.7, 1)
+        g.ising_sweep(0.7, 1)
+        assert_same_state(o, g, "after a sweep")
 
 
 def test_energy_closed_forms_on_gpu():
