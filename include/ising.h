@@ -61,11 +61,12 @@ extern "C" {
 
 /* The same shared draw, taken from generators with STORED state, one per lane -- the paper's own scheme of one generator
  * per thread with a strided state array (R19).  nsamples = 32k and L % 8 == 0 only.
- *   The N/2 sites of a colour are numbered by their colour rank j and taken in groups of four, g = j >> 2.  Lane q serves the
- *   groups q, q + nlanes, q + 2 nlanes, ... in that order, for each group the coded batches b = 0..k-1, for each the four sites
- *   w = 0..3; the next number of the lane is the draw of (batch b, site 4g + w).  Every lane takes 4 k ceil((N/8) / nlanes)
- *   draws per half-sweep (a lane whose last group does not exist draws and discards).  Thresholds as for Philox (R5).
- *   nlanes defaults to min(N/8, 151552 = one wave of threads) (ising_get_lanes / ising_set_lanes); the state lives in the workspace. */
+ *   The N/2 sites of a colour are numbered by their colour rank j and taken in groups of four, g = j >> 2 (N/8 groups); with k
+ *   coded batches there are k N/8 units u = b * (N/8) + g.  Lane q serves the units q, q + nlanes, q + 2 nlanes, ... in that order,
+ *   for each the four sites w = 0..3 of its group; the next number of the lane is the draw of (batch b, site 4g + w).  Every lane
+ *   takes 4 ceil(k (N/8) / nlanes) draws per half-sweep (a lane whose last unit does not exist draws and discards).  Thresholds as
+ *   for Philox (R5).  nlanes defaults to min(k N/8, 151552 = one wave of threads) (ising_get_lanes / ising_set_lanes); the state
+ *   lives in the workspace. */
 #define ISING_RNG_PR_SHARED 3      /* Parisi-Rapuano: ira[i] = ira[i-24] + ira[i-55]; R = ira[i] ^ ira[i-61];
                               seed words ira[0..61] of lane q = high words of SplitMix64 outputs q*62 + 1 .. q*62 + 62 of `seed` */
 #define ISING_RNG_MT19937_SHARED 4 /* MT19937, lane q seeded by init_genrand(high word of SplitMix64 output q + 1) */

@@ -443,25 +443,27 @@ static inline uint32_t lane_next(int rng_mode, uint32_t *lane_state, uint64_t *n
 }
 
 /* The draws of one colour half-sweep (R19).  The N/2 sites of the colour are numbered by their colour rank j and
- * taken in groups of four, g = j >> 2 (ngroups = N/8 groups).  Lane q serves the groups g = q, q + nlanes, q + 2 nlanes, ...
- * in that order; for each group it serves the k coded batches b = 0..k-1 in turn, and for each the four sites w = 0..3 of
- * the group: the next number of the lane is the draw shared by the 32 samples of batch b at site j = 4g + w
- * (PAPER.md:228-232).  Every lane takes the same number of draws per half-sweep, 4 k ceil(ngroups / nlanes): a lane whose
- * last group does not exist draws and discards.  table[b * (N/2) + j] receives the draw. */
+ * taken in groups of four, g = j >> 2 (ngroups = N/8 groups); with k coded batches of 32 samples there are k * ngroups
+ * units u = b * ngroups + g, b = batch.  Lane q serves the units u = q, q + nlanes, q + 2 nlanes, ... in that order, and for
+ * each unit the four sites w = 0..3 of its group: the next number of the lane is the draw shared by the 32 samples of
+ * batch b at site j = 4g + w.  Every lane takes the same number of draws per half-sweep,
+ * 4 ceil(k ngroups / nlanes): a lane whose last unit does not exist draws and discards.  Small lattices fill the machine
+ * with many coded batches, which is why the units, not the groups, are dealt to the lanes.
+ * table[b * (N/2) + j] receives the draw. */
 int oracle_lanes_draw_table(int rng_mode, int64_t nlanes, uint32_t *state, uint64_t *ndrawn, int64_t ngroups, int k,
                             uint32_t *table)
 {
     const int W = oracle_lane_state_words(rng_mode);
     if (W == 0 || nlanes < 1 || ngroups < 1 || k < 1) return -1;
-    const int64_t rounds = (ngroups + nlanes - 1) / nlanes;
+    const int64_t units = (int64_t)k * ngroups;
+    const int64_t rounds = (units + nlanes - 1) / nlanes;
     for (int64_t q = 0; q < nlanes; ++q)
         for (int64_t m = 0; m < rounds; ++m) {
-            const int64_t g = q + m * nlanes;
-            for (int b = 0; b < k; ++b)
-                for (int w = 0; w < 4; ++w) {
-                    const uint32_t R = lane_next(rng_mode, state + q * W, &ndrawn[q]);
-                    if (g < ngroups) table[(int64_t)b * 4 * ngroups + 4 * g + w] = R;
-                }
+            const int64_t u = q + m * nlanes;
+            for (int w = 0; w < 4; ++w) {
+                const uint32_t R = lane_next(rng_mode, state + q * W, &ndrawn[q]);
+                if (u < units) table[4 * u + w] = R;   /* 4u + w = b * (N/2) + 4g + w */
+            }
         }
     return 0;
 }

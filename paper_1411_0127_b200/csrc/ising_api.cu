@@ -34,8 +34,8 @@ struct Geometry {
     int W;                      // words per thread of the word-parallel kernel (fast layout)
 };
 
-// Lane modes (R19): default number of generator lanes = min(N/8, one wave of threads on the 148 SMs: 8 CTAs of 128 threads
-// at 64 registers).
+// Lane modes (R19): default number of generator lanes = min(k N/8 units, one wave of threads on the 148 SMs: 8 CTAs of 128
+// threads at 64 registers).
 constexpr uint32_t MAX_LANES = 148u * 1024u;
 
 inline bool lane_mode(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED || rng_mode == ISING_RNG_MT19937_SHARED; }
@@ -44,7 +44,8 @@ inline bool known_mode(int rng_mode) { return rng_mode >= ISING_RNG_PHILOX && rn
 inline uint32_t lanes_default(const Geometry &g, int rng_mode)
 {
     (void)rng_mode;
-    return (uint32_t)(g.N / 8 < MAX_LANES ? g.N / 8 : MAX_LANES);
+    const uint64_t units = (g.N / 8) * (uint64_t)(g.nbatches > 0 ? g.nbatches : 1);
+    return (uint32_t)(units < MAX_LANES ? units : MAX_LANES);
 }
 inline uint32_t lane_ring(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED ? 62u : rng_mode == ISING_RNG_MT19937_SHARED ? 624u : 0u; }
 
@@ -209,9 +210,16 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 SharedRng sr;
                 sr.tlo = r.tlo; sr.thi = r.thi; sr.k0 = r.k0; sr.k1base = r.k1base;
                 const uint32_t gpr = (uint32_t)g.L / 8;
-                const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L, (unsigned)nb);
-                launch_pdl(half_sweep_shared_vec, grid, dim3(128), st, a, sr, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
-                           (size_t)(8 * g.array_words));
+                const uint32_t gpr_inv = (uint32_t)((0x100000000ull + gpr - 1) / gpr);
+                if (g.L < 32) {  // fewer than 128 groups per plane: the thread index runs over (batch, group)
+                    const uint64_t units = (uint64_t)nb * (g.N / 8);
+                    launch_pdl(half_sweep_shared_vec<true>, dim3((unsigned)((units + 127) / 128)), dim3(128), st, a, sr, gpr, gpr_inv,
+                               (size_t)(8 * g.array_words), (uint32_t)nb);
+                } else {
+                    const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L, (unsigned)nb);
+                    launch_pdl(half_sweep_shared_vec<false>, grid, dim3(128), st, a, sr, gpr, gpr_inv, (size_t)(8 * g.array_words),
+                               (uint32_t)nb);
+                }
                 const int rc = check_launch(h);
                 if (rc != ISING_OK) return rc;
                 break;
@@ -297,15 +305,17 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
     a.L = g.L;
     a.colour = c;
     a.T = T;
-    const uint32_t ngroups = (uint32_t)(g.N / 8), rounds = (ngroups + h->nlanes - 1) / h->nlanes;
-    const uint64_t per_half_sweep = 4ull * (uint64_t)g.nbatches * rounds;
+    const uint32_t ngroups = (uint32_t)(g.N / 8);
+    const uint64_t units = (uint64_t)g.nbatches * ngroups;   // (batch, group) pairs, batch-major (R19)
+    const uint32_t rounds = (uint32_t)((units + h->nlanes - 1) / h->nlanes);
+    const uint64_t per_half_sweep = 4ull * rounds;
     LaneArgs ln;
     ln.state = h->lane_state;
     ln.nlanes = h->nlanes;
     ln.pos0 = (uint32_t)((h->t % LaneRing<GEN>::size) * (per_half_sweep % LaneRing<GEN>::size) % LaneRing<GEN>::size);
     const uint32_t gpr = (uint32_t)g.L / 8;
     launch_pdl(half_sweep_shared_lanes<GEN>, dim3(blocks), dim3(128), st, a, ln, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
-               (size_t)(8 * g.array_words), (uint32_t)g.nbatches, ngroups, rounds);
+               (size_t)(8 * g.array_words), ngroups, units, rounds);
     const int rc = check_launch(h);
     if (rc != ISING_OK) return rc;
     h->t += 1;

@@ -134,18 +134,18 @@ __global__ void __launch_bounds__(128) lanes_init(uint32_t *state, uint32_t nlan
 
 // ---------------------------------------------------------------------------------------------------
 // Shared-draw half-sweep driven by lane generators (rng_mode 3, 4), sample-packed, L % 8 == 0.  Thread = lane q.  It
-// serves the groups g = q + m * nlanes, m = 0 .. rounds-1 (a group = four consecutive same-colour sites of a row, the
-// unit of half_sweep_shared_vec), for each the coded batches b = 0 .. nbatches-1, and takes four draws per (group, batch)
-// in the order of R19; a lane whose last group does not exist still draws.  Consecutive lanes hold consecutive groups,
-// so the lattice loads of a warp are the same coalesced 512-byte rows as in half_sweep_shared_vec.
-//
+// serves the units u = q + m * nlanes, m = 0 .. rounds-1, where unit u = b * ngroups + g is group g (four consecutive
+// same-colour sites of a row, the unit of half_sweep_shared_vec) of coded batch b, and takes four draws per unit (R19); a
+// lane whose last unit does not exist still draws.  Consecutive lanes hold consecutive groups of one batch, so the
+// lattice loads of a warp are the same coalesced 512-byte rows as in half_sweep_shared_vec; small lattices with many
+// batches fill the machine because the units, not the groups, are dealt to the lanes.
 // (Holding the twelve state operands in registers across the lattice loads, so that both round trips overlap, spills at 64
 // registers and was slower: 0.249 against 0.239 ps/flip.)
 // ---------------------------------------------------------------------------------------------------
 template <int GEN>
 __global__ void __launch_bounds__(128, 8)
 half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uint32_t gpr_inv, size_t batch_stride,
-                        uint32_t nbatches, uint32_t ngroups, uint32_t rounds)
+                        uint32_t ngroups, uint64_t units, uint32_t rounds)
 {
     const uint32_t q = blockIdx.x * 128u + threadIdx.x;
     if (q >= ln.nlanes) return;
@@ -155,30 +155,27 @@ half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uin
     const uint32_t per_plane = (uint32_t)a0.L * gpr;
     wait_for_previous_kernel();   // the state was written by the previous half-sweep
     for (uint32_t m = 0; m < rounds; ++m) {
-        const uint32_t g = q + m * ln.nlanes;
-        const bool valid = g < ngroups;
-        const uint32_t z = valid ? g / per_plane : 0u;
-        const uint32_t p = valid ? g - z * per_plane : 0u;
-        for (uint32_t b = 0; b < nbatches; ++b) {
-            uint32_t R[4];
-            lane_next4<GEN>(st, stride, pos, R);
-            if (!valid) continue;
-            SweepArgs a = a0;
-            const size_t off = (size_t)b * batch_stride;
-            a.S_act += off;
-            a.S_oth += off;
+        const uint64_t u = (uint64_t)q + (uint64_t)m * ln.nlanes;
+        uint32_t R[4];
+        lane_next4<GEN>(st, stride, pos, R);
+        if (u >= units) continue;
+        const uint32_t b = (uint32_t)(u / ngroups), g = (uint32_t)(u - (uint64_t)b * ngroups);
+        const uint32_t z = g / per_plane, p = g - z * per_plane;
+        SweepArgs a = a0;
+        const size_t off = (size_t)b * batch_stride;
+        a.S_act += off;
+        a.S_oth += off;
 #pragma unroll
-            for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
-            uint32_t j0, s[4], sum2[4], sum1[4], sum0[4], c4[4], c8[4], c12[4];
-            uint64_t site0;
-            vec_group_sums(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
-            shared_cond_words(R, a.T, c4, c8, c12);
-            uint32_t out[4];
+        for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
+        uint32_t j0, s[4], sum2[4], sum1[4], sum0[4], c4[4], c8[4], c12[4];
+        uint64_t site0;
+        vec_group_sums(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
+        shared_cond_words(R, a.T, c4, c8, c12);
+        uint32_t out[4];
 #pragma unroll
-            for (int w = 0; w < 4; ++w)
-                out[w] = s[w] ^ flip_mask(sum2[w], sum1[w], sum0[w], c4[w] | a.T.always4, c8[w] | a.T.always8, c12[w] | a.T.always12);
-            *reinterpret_cast<uint4 *>(a.S_act + j0) = *reinterpret_cast<const uint4 *>(out);
-        }
+        for (int w = 0; w < 4; ++w)
+            out[w] = s[w] ^ flip_mask(sum2[w], sum1[w], sum0[w], c4[w] | a.T.always4, c8[w] | a.T.always8, c12[w] | a.T.always12);
+        *reinterpret_cast<uint4 *>(a.S_act + j0) = *reinterpret_cast<const uint4 *>(out);
     }
 }
 

@@ -557,26 +557,39 @@ struct SharedRng {
     uint32_t tlo, thi, k0, k1base;
 };
 
+// FLAT (L < 32, where a plane has fewer than 128 groups): grid = ceil(batches * L * L * L/8 / 128), the thread index runs
+// over the units u = b * ngroups + g of all batches, so that small lattices with many coded batches (PAPER.md:151-153,
+// 308-310) keep every thread busy (L = 8 x 4096 batches: 0.58 -> 0.17 ps/flip).
+template <bool FLAT>
 __global__ void __launch_bounds__(128)
 half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups per row = L/8 */,
-                      uint32_t gpr_inv /* ceil(2^32 / gpr) */, size_t batch_stride)
+                      uint32_t gpr_inv /* ceil(2^32 / gpr) */, size_t batch_stride, uint32_t nbatches)
 {
+    const uint32_t L = (uint32_t)a.L;
+    uint32_t p = blockIdx.x * 128u + threadIdx.x, z = blockIdx.y, batch = blockIdx.z;
+    if (FLAT) {
+        const uint32_t per_plane = L * gpr, ngroups = per_plane * L;
+        if (p >= nbatches * ngroups) return;
+        batch = p / ngroups;
+        const uint32_t g = p - batch * ngroups;
+        z = g / per_plane;
+        p = g - z * per_plane;
+    } else if (p >= L * gpr) {
+        return;
+    }
     {
-        const size_t off = (size_t)blockIdx.z * batch_stride;
+        const size_t off = (size_t)batch * batch_stride;
         a.S_act += off;
         a.S_oth += off;
 #pragma unroll
         for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
     }
-    const uint32_t L = (uint32_t)a.L;
-    const uint32_t p = blockIdx.x * 128u + threadIdx.x;
-    if (p >= L * gpr) return;
     uint32_t j0, s[4], sum2[4], sum1[4], sum0[4];
     uint64_t site0;
-    vec_group_sums(a, gpr, gpr_inv, p, blockIdx.y, j0, site0, s, sum2, sum1, sum0);
+    vec_group_sums(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
 
     uint32_t R[4], c4[4], c8[4], c12[4];
-    philox4x32_10(rng.tlo, rng.thi, j0 >> 2, 0u, rng.k0, rng.k1base ^ blockIdx.z, R);
+    philox4x32_10(rng.tlo, rng.thi, j0 >> 2, 0u, rng.k0, rng.k1base ^ batch, R);
     shared_cond_words(R, a.T, c4, c8, c12);
 
     uint32_t out[4];

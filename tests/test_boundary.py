@@ -44,7 +44,7 @@ def test_thresholds_equal_the_oracle_table(rng_mode):
 
 def test_lane_modes_host_side():
     """rng modes 3, 4 (R19): thresholds are the Philox table; the workspace grows by the strided generator state
-    (62 / 624 words per lane; min(N/8, 148*1024) lanes: one wave of threads);
+    (62 / 624 words per lane; min(k N/8, 148*1024) lanes: one wave of threads);
     L % 8 and nsamples % 32 are required."""
     lib = binding.lib()
     out = C.c_size_t(0)
@@ -54,7 +54,7 @@ def test_lane_modes_host_side():
         assert lib.ising_workspace_bytes(16, 1, mode, C.byref(out)) == binding.EINVAL
         assert lib.ising_workspace_bytes(12, 32, mode, C.byref(out)) == binding.EINVAL
         for L, ns in ((8, 32), (64, 64), (256, 32)):
-            lanes = min(L**3 // 8, cap)
+            lanes = min((ns // 32) * L**3 // 8, cap)
             extra = binding.ising_workspace_bytes(L, ns, mode) - binding.ising_workspace_bytes(L, ns, binding.PHILOX_SHARED)
             assert 0 <= extra - 4 * ring * lanes < 256
         assert binding.ising_prng_state_bytes(mode, 1000) == 4 * ring * 1000

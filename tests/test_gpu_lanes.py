@@ -44,7 +44,8 @@ def assert_same_state(o, g, what=""):
 @pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
 # (16, 32, 7), (24, 64, 50): many rounds per lane, the ring wraps several times inside one launch
 @pytest.mark.parametrize("L,ns,nlanes", [(8, 32, None), (8, 64, 24), (16, 32, 100), (16, 96, 512), (24, 32, 333), (40, 32, None),
-                                         (40, 64, 1000), (64, 32, 4096), (16, 32, 7), (24, 64, 50)])
+                                         (40, 64, 1000), (64, 32, 4096), (16, 32, 7), (24, 64, 50), (8, 1024, None), (8, 160, 300),
+                                         (16, 96, None)])
 def test_lane_mode_sweep_equals_the_oracle(mode, L, ns, nlanes):
     spins, J = synth.make_spins(L, ns, 71), synth.make_couplings(L, ns, 72)
     o, g = make_pair(L, ns, mode, nlanes, spins, J)
@@ -70,7 +71,7 @@ def test_lane_mode_with_the_default_wave_of_lanes(mode):
 
 @pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
 def test_lane_mode_many_half_sweeps_cross_the_mt_ring(mode):
-    """L = 8, 2 batches, 3 lanes: 4 * 2 * ceil(64/3) = 176 draws per lane per half-sweep; 8 half-sweeps = 1408 draws cross the
+    """L = 8, 2 batches, 3 lanes: 4 * ceil(2 * 64 / 3) = 172 draws per lane per half-sweep; 8 half-sweeps = 1376 draws cross the
     624-word MT block twice and the 62-word ring 22 times.  Sweeps split over several calls (the state persists)."""
     L, ns = 8, 64
     spins, J = synth.make_spins(L, ns, 73), synth.make_couplings(L, ns, 74)
@@ -106,6 +107,7 @@ def test_lane_mode_argument_checks():
             Ising(12, 32, SEED, mode)         # L % 8 != 0
         g = Ising(16, 32, SEED, mode)
         assert g.ising_get_lanes() == 16**3 // 8
+        assert Ising(8, 96, SEED, mode).ising_get_lanes() == 3 * 8**3 // 8    # units = batches x groups
         with pytest.raises(binding.IsingError):
             g.ising_set_lanes(0)
         with pytest.raises(binding.IsingError):

@@ -305,7 +305,8 @@ def test_minstd_cached_seed_table_equals_recomputed_seeds(L):
 
 # ------------------------------------------------------------------------------------------------ shared-random-number mode
 
-@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (8, 32), (8, 64), (12, 32), (16, 64), (24, 32), (40, 32), (64, 32)])
+@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (8, 32), (8, 64), (12, 32), (16, 64), (24, 32), (40, 32), (64, 32),
+                                        (8, 320), (16, 160), (32, 96)])
 def test_shared_random_number_mode_equals_the_oracle(L, nsamples):
     """rng_mode 2 (R18): one Philox draw per 32-sample word.  The vectorised kernel (L % 8 == 0) and
     the generic sample-packed kernel (kernel choice 1, and every other L) against the oracle, trajectory and energies."""

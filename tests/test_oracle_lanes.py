@@ -92,7 +92,7 @@ def _lane_sequences(mode, seed, nlanes, n):
 
 
 @pytest.mark.parametrize("mode", [ea3d.PR_LANES, ea3d.MT_LANES])
-@pytest.mark.parametrize("ngroups,nlanes,k", [(8, 8, 1), (8, 3, 1), (27, 5, 2), (64, 24, 3), (8, 20, 2)])
+@pytest.mark.parametrize("ngroups,nlanes,k", [(8, 8, 1), (8, 3, 1), (27, 5, 2), (64, 24, 3), (8, 16, 2), (8, 13, 5)])
 def test_draw_table_follows_the_lane_order(mode, ngroups, nlanes, k):
     lib = ea3d.lib()
     w = lib.oracle_lane_state_words(mode)
@@ -100,8 +100,8 @@ def test_draw_table_follows_the_lane_order(mode, ngroups, nlanes, k):
     nd = np.zeros(nlanes, np.uint64)
     u32, u64 = C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
     lib.oracle_lanes_init(mode, 4242, nlanes, state.ctypes.data_as(u32), nd.ctypes.data_as(u64))
-    rounds = -(-ngroups // nlanes)
-    per_hs = 4 * k * rounds
+    rounds = -(-(k * ngroups) // nlanes)
+    per_hs = 4 * rounds
     seqs = _lane_sequences(mode, 4242, nlanes, 3 * per_hs)
     for hs in range(3):
         table = np.zeros(k * 4 * ngroups, np.uint32)
@@ -111,8 +111,9 @@ def test_draw_table_follows_the_lane_order(mode, ngroups, nlanes, k):
         for b in range(k):
             for j in range(4 * ngroups):
                 g, wd = j >> 2, j & 3
-                q, m = g % nlanes, g // nlanes
-                assert int(table[b * 4 * ngroups + j]) == seqs[q][hs * per_hs + (m * k + b) * 4 + wd], (hs, b, j)
+                u = b * ngroups + g                      # unit = (batch, group), batch-major
+                q, m = u % nlanes, u // nlanes
+                assert int(table[b * 4 * ngroups + j]) == seqs[q][hs * per_hs + m * 4 + wd], (hs, b, j)
 
 
 # ---------------------------------------------------------------- the sweep
@@ -133,7 +134,7 @@ def test_every_sample_follows_the_scalar_rule_with_the_lane_draws(mode):
         o.half_sweep(beta)
     got = o.spins_packed()
     N, ngroups, k = L**3, L**3 // 8, ns // 32
-    per_hs = 4 * k * -(-ngroups // nlanes)
+    per_hs = 4 * -(-(k * ngroups) // nlanes)
     seqs = _lane_sequences(mode, seed, nlanes, nhs * per_hs)
     T = ea3d.thresholds(beta, mode)
     W = (N + 31) // 32
@@ -157,7 +158,8 @@ def test_every_sample_follows_the_scalar_rule_with_the_lane_draws(mode):
                         dE = 2 * sg[i] * h
                         j = (x >> 1) + (L // 2) * (y + L * z)
                         g, wd = j >> 2, j & 3
-                        R = seqs[g % nlanes][t * per_hs + ((g // nlanes) * k + b) * 4 + wd]
+                        u = b * ngroups + g
+                        R = seqs[u % nlanes][t * per_hs + (u // nlanes) * 4 + wd]
                         if dE <= 0 or R < T[dE // 4 - 1]:
                             sg[i] = -sg[i]
         want = ea3d.spins_to_packed(np.array(sg, dtype=np.int8))
