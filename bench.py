@@ -155,6 +155,8 @@ def main():
     ap.add_argument("--no-shared", action="store_true", help="skip the shared-random-number (paper's AMSC) timing")
     ap.add_argument("--only-shared", action="store_true", help="time only the shared-random-number mode (for ncu captures)")
     ap.add_argument("--only-lanes", action="store_true", help="time only the stored-state lane generators (sweep and Table II)")
+    ap.add_argument("--scan-batches", action="store_true",
+                    help="the paper's Fig. 4 study: half-sweep time of small lattices against the number k of coded batches (shared draws)")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -337,6 +339,29 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.scan_batches:  # PAPER.md:308-310, Fig. 4: t_SW stays flat in k until the GPU is full, then grows linearly
+        rows = []
+        for Ls, ks in ((8, (1, 8, 64, 512, 4096)), (16, (1, 8, 64, 512)), (32, (1, 8, 64)), (64, (1, 8))):
+            for k in ks:
+                sp = torch.from_numpy(synth.make_spins(Ls, 32 * k).view(np.int32)).cuda()
+                Jc = torch.from_numpy(synth.make_couplings(Ls, 32 * k).view(np.int32)).cuda()
+                for mode in (2, 3, 4):
+                    g = Ising(Ls, 32 * k, synth.DYN_SEED, mode)
+                    g.ising_load_state(sp, Jc)
+                    g.ising_sweep(BETA, 2)
+                    torch.cuda.synchronize()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    g.ising_sweep(BETA, 50)
+                    b.record(stream)
+                    torch.cuda.synchronize()
+                    ms = a.elapsed_time(b)
+                    g.ising_destroy()
+                    rows.append({"L": Ls, "batches": k, "rng_mode": {2: "philox_shared", 3: "parisi_rapuano_lanes", 4: "mt19937_lanes"}[mode],
+                                 "half_sweep_us": 1e3 * ms / 100, "ps_per_flip": 1e9 * ms / (50 * 32 * k * Ls**3)})
+        print(json.dumps({"scan_batches": rows}))
         return
 
     if args.only_shared:
