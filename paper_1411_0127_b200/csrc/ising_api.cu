@@ -273,6 +273,9 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             else if (W == 3) launch_pdl(half_sweep_site_packed<RNG, 3>, grid, dim3(SWEEP_THREADS), st, a, sr);
             else if (W == 5) launch_pdl(half_sweep_site_packed<RNG, 5>, grid, dim3(SWEEP_THREADS), st, a, sr);
             else launch_pdl(half_sweep_site_packed<RNG, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
+        } else if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {  // any even L: the word update on operands gathered as bit windows
+            const uint64_t nw = (g.Hc + 31) / 32;
+            launch_pdl(half_sweep_site_packed_rows<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, r, (uint32_t)nw, (uint32_t)g.Hc);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             launch_pdl(half_sweep_site_packed_generic<RNG>, dim3((unsigned)((nw + 255) / 256)), dim3(256), st, a, r, (uint64_t)nw, (uint64_t)g.Hc);

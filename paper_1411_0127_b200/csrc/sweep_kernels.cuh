@@ -391,6 +391,95 @@ half_sweep_site_packed_generic(const SweepArgs a, const __grid_constant__ RngLau
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Site-packed, any even L (rows of L/2 bits that do not fill whole words: L = 16, 96, 250, ...): the word update of the
+// word-parallel kernel on operands gathered as bit windows.  The colour arrays are rank-linear (bit j of the array =
+// colour rank j), so a word covers 32 consecutive ranks, i.e. one or more row segments; within a segment every neighbour
+// set is a contiguous bit range of the other colour's array (the same columns of the row y+-1 / z+-1, or the row itself
+// shifted by one bit for +-x, with the periodic bit patched in), fetched as an unaligned 32-bit window (two loads and a
+// funnel shift).  The draws are those of cond_masks_site_packed_philox (word w = ranks 32w .. 32w+31, R9) or, for
+// MINSTD, one evaluation per segment with the canonical site index of its first bit (R11).  The paper's point that the
+// scheme must work for every L = 2n, not only powers of two, is what this kernel is for: about
+// 1 ps/flip instead of 12-55 for the one-site-at-a-time kernel it replaces (kernel choice 1 still selects that one).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t bit_window(const uint32_t *__restrict__ a, uint32_t pos)
+{   // bits pos .. pos+31 of the bit array (bits past the array's end are garbage that the caller masks out)
+    const uint32_t w = pos >> 5, sh = pos & 31u;
+    const uint32_t lo = __ldg(a + w);
+    const uint32_t hi = sh ? __ldg(a + w + 1) : 0u;
+    return __funnelshift_r(lo, hi, sh);
+}
+__device__ __forceinline__ uint32_t bit_at(const uint32_t *__restrict__ a, uint32_t pos) { return (__ldg(a + (pos >> 5)) >> (pos & 31u)) & 1u; }
+
+template <int RNG>
+__global__ void __launch_bounds__(128)
+half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_words, uint32_t Hc)
+{
+    const uint32_t w = blockIdx.x * 128u + threadIdx.x;
+    if (w >= n_words) return;
+    const uint32_t L = (uint32_t)a.L, H = L >> 1, LH = L * H;
+    const uint32_t j0 = 32u * w;
+    uint32_t remaining = Hc - j0 < 32u ? Hc - j0 : 32u, bitoff = 0;
+    uint32_t r = j0 / H, m = j0 - r * H, z = r / L, y = r - z * L;
+    wait_for_previous_kernel();
+    const uint32_t s = __ldg(a.S_act + w);
+    uint32_t J[6] = {__ldg(a.J_act[0] + w), 0u, __ldg(a.J_act[1] + w), 0u, __ldg(a.J_act[2] + w), 0u}, nb[6] = {0u, 0u, 0u, 0u, 0u, 0u};
+    uint32_t c4 = 0, c8 = 0, c12 = 0;
+    while (remaining > 0) {
+        const uint32_t len = remaining < H - m ? remaining : H - m;
+        const uint32_t segmask = (len == 32u ? 0xFFFFFFFFu : ((1u << len) - 1u)) << bitoff;
+        const uint32_t xodd = (y + z + (uint32_t)a.colour) & 1u;
+        const uint32_t P = r * H;                                   // rank of the first site of this row
+        const uint32_t Pyp = (y + 1 == L) ? P - (LH - H) : P + H, Pym = (y == 0) ? P + (LH - H) : P - H;
+        const uint32_t Pzp = (z + 1 == L) ? P - (Hc - LH) : P + LH, Pzm = (z == 0) ? P + (Hc - LH) : P - LH;
+        // +x: column m + xodd of the same row; the last column wraps to column 0 when xodd = 1
+        uint32_t wpx = bit_window(a.S_oth, P + m + xodd);
+        if (xodd && m + len == H) wpx = (wpx & ~(1u << (len - 1))) | (bit_at(a.S_oth, P) << (len - 1));
+        // -x: column m - 1 + xodd with its own coupling; column 0 wraps to column H-1 when xodd = 0
+        uint32_t wmx, jmx;
+        if (xodd) {
+            wmx = bit_window(a.S_oth, P + m);
+            jmx = bit_window(a.J_oth[0], P + m);
+        } else if (m == 0) {
+            wmx = (bit_window(a.S_oth, P) << 1) | bit_at(a.S_oth, P + H - 1);
+            jmx = (bit_window(a.J_oth[0], P) << 1) | bit_at(a.J_oth[0], P + H - 1);
+        } else {
+            wmx = bit_window(a.S_oth, P + m - 1);
+            jmx = bit_window(a.J_oth[0], P + m - 1);
+        }
+        nb[0] |= (wpx << bitoff) & segmask;
+        nb[1] |= (wmx << bitoff) & segmask;
+        J[1] |= (jmx << bitoff) & segmask;
+        nb[2] |= (bit_window(a.S_oth, Pyp + m) << bitoff) & segmask;
+        nb[3] |= (bit_window(a.S_oth, Pym + m) << bitoff) & segmask;
+        J[3] |= (bit_window(a.J_oth[1], Pym + m) << bitoff) & segmask;
+        nb[4] |= (bit_window(a.S_oth, Pzp + m) << bitoff) & segmask;
+        nb[5] |= (bit_window(a.S_oth, Pzm + m) << bitoff) & segmask;
+        J[5] |= (bit_window(a.J_oth[2], Pzm + m) << bitoff) & segmask;
+        if (RNG == 1) {   // MINSTD: stream id = canonical site index; bit b of the word is site0 + 2 (b - bitoff)
+            const uint64_t site0 = (uint64_t)L * r + 2u * m + xodd - 2ull * bitoff;
+            uint32_t d4, d8, d12;
+            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, 2u * rng.A, a.T, d4, d8, d12);
+            c4 |= d4 & segmask;
+            c8 |= d8 & segmask;
+            c12 |= d12 & segmask;
+        }
+        bitoff += len;
+        remaining -= len;
+        m += len;
+        if (m == H) {
+            m = 0;
+            ++r;
+            if (++y == L) { y = 0; ++z; }
+        }
+    }
+    if (RNG == 0) cond_masks_site_packed_philox(rng.pc, rng.ps[0], w, a.T, c4, c8, c12);
+    uint32_t sum2, sum1, sum0;
+    satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
+    const uint32_t valid = bitoff == 32u ? 0xFFFFFFFFu : (1u << bitoff) - 1u;   // the last word of the array may be partial
+    a.S_act[w] = s ^ (flip_mask(sum2, sum1, sum0, c4, c8, c12) & valid);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Sample-packed kernel (nsamples = 32 per batch), any even L >= 4.  A Philox group g = 4 consecutive same-colour sites
 // j = 4g..4g+3 needs one call per sample (bit), keyed by the sample (R9).  Neighbours are whole words, so no
 // x-alignment is needed.  A CTA has 4 warps.  PARTS = 1: one thread per group, all 32 samples (large lattices: index
