@@ -396,6 +396,10 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         m.L = g.L;
         if (g.nsamples != 1) {
             energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
+        } else if (h->kernel_choice != 1 && g.Hc < (1ull << 31)) {
+            const uint32_t nw = (uint32_t)((g.Hc + 31) / 32);
+            const unsigned need = (2 * nw + 255) / 256;
+            energy_site_packed_rows<<<need < 148u * 8u ? need : 148u * 8u, 256, 0, st>>>(m, h->acc, nw, (uint32_t)g.Hc);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc, nw, g.Hc);
