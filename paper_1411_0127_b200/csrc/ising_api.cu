@@ -490,6 +490,21 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
             return check_launch(h);
         }
         const uint64_t nw = (g.Hc + 31) / 32;
+        if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {  // word at a time, all four arrays and both colours in one launch
+            SplitArgs s;
+            s.narrays = 4;
+            s.L = g.L;
+            s.canon[0] = d_spins;
+            s.out[0][0] = A.S[0];
+            s.out[0][1] = A.S[1];
+            for (int d = 0; d < 3; ++d) {
+                s.canon[1 + d] = d_J + (size_t)d * W;
+                s.out[1 + d][0] = A.J[d][0];
+                s.out[1 + d][1] = A.J[d][1];
+            }
+            gather_site_packed_rows<<<dim3((unsigned)((nw + 127) / 128), 8), 128, 0, st>>>(s, (uint32_t)nw, (uint32_t)g.Hc, (uint64_t)W);
+            return check_launch(h);
+        }
         const unsigned grid = (unsigned)((nw + 255) / 256);
         for (int c = 0; c < 2; ++c) {
             gather_site_packed_generic<<<grid, 256, 0, st>>>(d_spins, A.S[c], c, g.L, nw, g.Hc);
@@ -543,6 +558,8 @@ int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
             const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
             if (g.W == 4) merge_colours_site_packed<4><<<(unsigned)((n / 4 + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
             else merge_colours_site_packed<1><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
+        } else if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {
+            scatter_site_packed_rows<<<(unsigned)((W + 127) / 128), 128, 0, st>>>(A.S[0], A.S[1], d_out, g.L, W, g.N);
         } else {
             scatter_site_packed_generic<<<(unsigned)((W + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L, W, g.N);
         }

@@ -138,6 +138,83 @@ scatter_site_packed_generic(const uint32_t *__restrict__ S0, const uint32_t *__r
     canon[cw] = w;
 }
 
+// Site-packed, any even L, word at a time (the bit windows of half_sweep_site_packed_rows).  gather: the row segments of an
+// output word are every second bit of a canonical bit range (a 64-bit window, even bits compressed); scatter: the row
+// segments of a canonical word interleave a bit range of each colour array (16-bit windows spread to alternate bits).
+__device__ __forceinline__ uint32_t canon_window(const uint32_t *__restrict__ a, uint64_t pos, uint64_t n_words)
+{   // bits pos .. pos+31 of a caller-owned array of n_words words; words past its end read as zero
+    const uint64_t w = pos >> 5;
+    const uint32_t sh = (uint32_t)pos & 31u;
+    const uint32_t lo = w < n_words ? __ldg(a + w) : 0u;
+    const uint32_t hi = (sh && w + 1 < n_words) ? __ldg(a + w + 1) : 0u;
+    return __funnelshift_r(lo, hi, sh);
+}
+
+// grid = (ceil(n_words / 128), 4 arrays x 2 colours)
+__global__ void __launch_bounds__(128)
+gather_site_packed_rows(const __grid_constant__ SplitArgs a, uint32_t n_words, uint32_t Hc, uint64_t n_canon_words)
+{
+    const uint32_t w = blockIdx.x * 128u + threadIdx.x;
+    if (w >= n_words) return;
+    const int arr = blockIdx.y >> 1, c = blockIdx.y & 1;
+    const uint32_t *__restrict__ canon = a.canon[arr];
+    const uint32_t L = (uint32_t)a.L, H = L >> 1;
+    const uint32_t j0 = 32u * w;
+    uint32_t remaining = Hc - j0 < 32u ? Hc - j0 : 32u, bitoff = 0;
+    uint32_t r = j0 / H, m = j0 - r * H, z = r / L, y = r - z * L;
+    uint32_t out = 0;
+    while (remaining > 0) {
+        const uint32_t len = remaining < H - m ? remaining : H - m;
+        const uint32_t segmask = (len == 32u ? 0xFFFFFFFFu : ((1u << len) - 1u)) << bitoff;
+        const uint32_t xodd = (y + z + (uint32_t)c) & 1u;
+        const uint64_t base = (uint64_t)L * r + 2u * m + xodd;   // canonical site index of the segment's first site
+        uint32_t v = compress_even_bits(canon_window(canon, base, n_canon_words));
+        if (len > 16u) v |= compress_even_bits(canon_window(canon, base + 32u, n_canon_words)) << 16;
+        out |= (v << bitoff) & segmask;
+        bitoff += len;
+        remaining -= len;
+        m += len;
+        if (m == H) {
+            m = 0;
+            ++r;
+            if (++y == L) { y = 0; ++z; }
+        }
+    }
+    a.out[arr][c][w] = out;
+}
+
+__global__ void __launch_bounds__(128)
+scatter_site_packed_rows(const uint32_t *__restrict__ S0, const uint32_t *__restrict__ S1, uint32_t *__restrict__ canon, int L_,
+                         uint64_t n_canon_words, uint64_t N)
+{
+    const uint64_t cw = (uint64_t)blockIdx.x * 128u + threadIdx.x;
+    if (cw >= n_canon_words) return;
+    const uint32_t L = (uint32_t)L_, H = L >> 1;
+    const uint64_t i0 = 32u * cw;
+    uint32_t remaining = N - i0 < 32u ? (uint32_t)(N - i0) : 32u, bitoff = 0;
+    uint32_t r = (uint32_t)(i0 / L), x = (uint32_t)(i0 - (uint64_t)r * L), z = r / L, y = r - z * L;
+    uint32_t out = 0;
+    while (remaining > 0) {
+        const uint32_t len = remaining < L - x ? remaining : L - x;
+        const uint32_t segmask = (len == 32u ? 0xFFFFFFFFu : ((1u << len) - 1u)) << bitoff;
+        const uint32_t xodd0 = (y + z) & 1u;                       // x parity of colour 0 in this row
+        const uint32_t xa0 = x + ((x ^ xodd0) & 1u), xa1 = x + ((x ^ xodd0 ^ 1u) & 1u);   // first x of either colour in the segment
+        const uint32_t P = r * H;
+        const uint32_t v = (spread_to_even_bits(bit_window(S0, P + (xa0 >> 1))) << (xa0 - x)) |
+                           (spread_to_even_bits(bit_window(S1, P + (xa1 >> 1))) << (xa1 - x));
+        out |= (v << bitoff) & segmask;
+        bitoff += len;
+        remaining -= len;
+        x += len;
+        if (x == L) {
+            x = 0;
+            ++r;
+            if (++y == L) { y = 0; ++z; }
+        }
+    }
+    canon[cw] = out;
+}
+
 // Sample-packed: word j of the colour-c array of a batch collects bit i(j,c) of the 32 samples' canonical arrays.
 // canon points at the first sample of the batch; consecutive samples are `sample_stride` words apart.
 __global__ void __launch_bounds__(256)
