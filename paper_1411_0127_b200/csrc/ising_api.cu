@@ -231,10 +231,20 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             if (g.L % 8 == 0 && h->kernel_choice != 1) {  // 128-bit loads
                 const uint32_t gpr = (uint32_t)g.L / 8, inv = (uint32_t)((0x100000000ull + gpr - 1) / gpr);
                 const uint64_t per_plane = (uint64_t)g.L * gpr;
+                const size_t bstride = (size_t)(8 * g.array_words);
+                if (nb > 1) {  // all coded batches in one launch (a is batch 0 here, b == 0)
+                    if (ngroups * (uint64_t)nb < 148u * 1024u)
+                        launch_pdl(half_sweep_sample_packed_vec<RNG, 4, true>, dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L, (unsigned)nb), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
+                    else
+                        launch_pdl(half_sweep_sample_packed_vec<RNG, 1, true>, dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L, (unsigned)nb), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
+                    const int rc = check_launch(h);
+                    if (rc != ISING_OK) return rc;
+                    break;
+                }
                 if (ngroups < 148u * 1024u)
-                    launch_pdl(half_sweep_sample_packed_vec<RNG, 4>, dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N);
+                    launch_pdl(half_sweep_sample_packed_vec<RNG, 4, false>, dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
                 else
-                    launch_pdl(half_sweep_sample_packed_vec<RNG, 1>, dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N);
+                    launch_pdl(half_sweep_sample_packed_vec<RNG, 1, false>, dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
             } else if (ngroups < 148u * 1024u)
                 launch_pdl(half_sweep_sample_packed<RNG, 4>, dim3((unsigned)((ngroups + 31) / 32)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
             else

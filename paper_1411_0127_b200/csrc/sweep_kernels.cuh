@@ -694,12 +694,24 @@ half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups p
 // spreads the 32 samples of a group over the four warps of the CTA, each updating one byte of the four words).
 // grid = (ceil(L * L/8 / (128 / PARTS)), L), one launch per batch of 32 samples.
 // ---------------------------------------------------------------------------------------------------
-template <int RNG, int PARTS>
+// MULTI: all coded batches in one launch (blockIdx.z = batch, arrays batch_stride words apart).  The launch constants
+// cannot be folded per (batch, sample) then, so the plain ten Philox rounds are run with the key (k0, k1base ^ sample);
+// a small lattice with many batches is one launch instead of one per batch.
+template <int RNG, int PARTS, bool MULTI>
 __global__ void __launch_bounds__(128)
-half_sweep_sample_packed_vec(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t gpr, uint32_t gpr_inv, uint64_t N)
+half_sweep_sample_packed_vec(SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t gpr, uint32_t gpr_inv, uint64_t N,
+                             size_t batch_stride)
 {
     constexpr int SPT = 32 / PARTS;
     const uint32_t L = (uint32_t)a.L;
+    const uint32_t sample0 = MULTI ? 32u * blockIdx.z : rng.sample_base;
+    if (MULTI) {
+        const size_t off = (size_t)blockIdx.z * batch_stride;
+        a.S_act += off;
+        a.S_oth += off;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
+    }
     const int part = PARTS == 1 ? 0 : (int)(threadIdx.x >> 5);  // warp-uniform
     const uint32_t p_raw = PARTS == 1 ? blockIdx.x * 128u + threadIdx.x : blockIdx.x * 32u + (threadIdx.x & 31u);
     const bool valid = p_raw < L * gpr;
@@ -715,13 +727,16 @@ half_sweep_sample_packed_vec(const SweepArgs a, const __grid_constant__ RngLaunc
     for (int i = 0; i < SPT; i += 2) {
         const int b = SPT * part + i;
         uint32_t R[8];
-        if (RNG == 0) {
+        if (RNG == 0 && MULTI) {
+            philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ (sample0 + (uint32_t)b), R);
+            philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ (sample0 + (uint32_t)b + 1u), R + 4);
+        } else if (RNG == 0) {
             philox_folded(rng.pc, rng.ps[b], g, R);
             philox_folded(rng.pc, rng.ps[b + 1], g, R + 4);
         } else {
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const uint64_t w0 = rng.seed + ((uint64_t)(rng.sample_base + b + e) * N + site0 + 1) * SPLITMIX_GAMMA;
+                const uint64_t w0 = rng.seed + ((uint64_t)(sample0 + b + e) * N + site0 + 1) * SPLITMIX_GAMMA;
 #pragma unroll
                 for (int w = 0; w < 4; ++w)  // consecutive sites of the colour are 2 apart in the canonical index
                     R[4 * e + w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(w0 + (uint64_t)w * (2 * SPLITMIX_GAMMA)));

@@ -164,7 +164,7 @@ def test_config2_L64_32_samples_philox():
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
-@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (10, 32), (16, 64)])
+@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (10, 32), (16, 64), (8, 160), (24, 96), (64, 64), (10, 64)])
 def test_sample_packed_small(L, nsamples, rng_mode):
     spins, J = synth.make_spins(L, nsamples, 21), synth.make_couplings(L, nsamples, 8)
     o, g = make_pair(L, nsamples, rng_mode, spins, J)
