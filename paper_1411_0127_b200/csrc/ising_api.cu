@@ -285,7 +285,13 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             else launch_pdl(half_sweep_site_packed<RNG, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
         } else if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {  // any even L: the word update on operands gathered as bit windows
             const uint64_t nw = (g.Hc + 31) / 32;
-            launch_pdl(half_sweep_site_packed_rows<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, r, (uint32_t)nw, (uint32_t)g.Hc);
+            SiteRng sr;   // the small per-launch constant block (the 1.4 KB RngLaunch doubles the enqueue cost of a tiny launch)
+            sr.pc = r.pc;
+            sr.ps = r.ps[0];
+            sr.seed = r.seed;
+            sr.A2 = 2u * r.A;
+            sr.s0tab = nullptr;
+            launch_pdl(half_sweep_site_packed_rows<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw, (uint32_t)g.Hc);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             launch_pdl(half_sweep_site_packed_generic<RNG>, dim3((unsigned)((nw + 255) / 256)), dim3(256), st, a, r, (uint64_t)nw, (uint64_t)g.Hc);

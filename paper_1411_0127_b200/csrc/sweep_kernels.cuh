@@ -412,7 +412,7 @@ __device__ __forceinline__ uint32_t bit_at(const uint32_t *__restrict__ a, uint3
 
 template <int RNG>
 __global__ void __launch_bounds__(128)
-half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_words, uint32_t Hc)
+half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t n_words, uint32_t Hc)
 {
     const uint32_t w = blockIdx.x * 128u + threadIdx.x;
     if (w >= n_words) return;
@@ -458,7 +458,7 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ RngLaunch
         if (RNG == 1) {   // MINSTD: stream id = canonical site index; bit b of the word is site0 + 2 (b - bitoff)
             const uint64_t site0 = (uint64_t)L * r + 2u * m + xodd - 2ull * bitoff;
             uint32_t d4, d8, d12;
-            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, 2u * rng.A, a.T, d4, d8, d12);
+            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, d4, d8, d12);
             c4 |= d4 & segmask;
             c8 |= d8 & segmask;
             c12 |= d12 & segmask;
@@ -472,7 +472,7 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ RngLaunch
             if (++y == L) { y = 0; ++z; }
         }
     }
-    if (RNG == 0) cond_masks_site_packed_philox(rng.pc, rng.ps[0], w, a.T, c4, c8, c12);
+    if (RNG == 0) cond_masks_site_packed_philox(rng.pc, rng.ps, w, a.T, c4, c8, c12);
     uint32_t sum2, sum1, sum0;
     satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
     const uint32_t valid = bitoff == 32u ? 0xFFFFFFFFu : (1u << bitoff) - 1u;   // the last word of the array may be partial
