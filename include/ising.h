@@ -60,7 +60,7 @@ extern "C" {
                               of the samples 32b..32b+31 is the ISING_RNG_PHILOX draw with the key's sample field = b (R18) */
 
 /* The same shared draw, taken from generators with STORED state, one per lane -- the paper's own scheme of one generator
- * per thread with a strided state array (R19).  nsamples = 32k and L % 8 == 0 only.
+ * per thread with a strided state array (R19).  nsamples = 32k only.
  *   The N/2 sites of a colour are numbered by their colour rank j and taken in groups of four, g = j >> 2 (N/8 groups); with k
  *   coded batches there are k N/8 units u = b * (N/8) + g.  Lane q serves the units q, q + nlanes, q + 2 nlanes, ... in that order,
  *   for each the four sites w = 0..3 of its group; the next number of the lane is the draw of (batch b, site 4g + w).  Every lane

@@ -332,9 +332,14 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
     ln.state = h->lane_state;
     ln.nlanes = h->nlanes;
     ln.pos0 = (uint32_t)((h->t % LaneRing<GEN>::size) * (per_half_sweep % LaneRing<GEN>::size) % LaneRing<GEN>::size);
-    const uint32_t gpr = (uint32_t)g.L / 8;
-    launch_pdl(half_sweep_shared_lanes<GEN>, dim3(blocks), dim3(128), st, a, ln, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
-               (size_t)(8 * g.array_words), ngroups, units, rounds);
+    if (g.L % 8 == 0) {
+        const uint32_t gpr = (uint32_t)g.L / 8;
+        launch_pdl(half_sweep_shared_lanes<GEN, true>, dim3(blocks), dim3(128), st, a, ln, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
+                   (size_t)(8 * g.array_words), ngroups, units, rounds);
+    } else {  // groups that straddle rows: per-word neighbour loads
+        launch_pdl(half_sweep_shared_lanes<GEN, false>, dim3(blocks), dim3(128), st, a, ln, 1u, 0u, (size_t)(8 * g.array_words), ngroups,
+                   units, rounds);
+    }
     const int rc = check_launch(h);
     if (rc != ISING_OK) return rc;
     h->t += 1;
@@ -437,7 +442,6 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
     if (!out || !make_geometry(L, nsamples, &g)) return ISING_EINVAL;
     if (!known_mode(rng_mode)) return ISING_EINVAL;
     if (shared_mode(rng_mode) && nsamples % 32 != 0) return ISING_EINVAL;  // one draw per 32-sample word
-    if (lane_mode(rng_mode) && L % 8 != 0) return ISING_EINVAL;            // groups of four sites must not leave their row
     *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
     if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
     if (lane_mode(rng_mode)) *out += round_up((size_t)lane_ring(rng_mode) * lanes_default(g, rng_mode) * sizeof(uint32_t), 256);

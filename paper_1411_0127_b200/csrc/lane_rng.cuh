@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(128) lanes_init(uint32_t *state, uint32_t nlan
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Shared-draw half-sweep driven by lane generators (rng_mode 3, 4), sample-packed, L % 8 == 0.  Thread = lane q.  It
+// Shared-draw half-sweep driven by lane generators (rng_mode 3, 4), sample-packed.  Thread = lane q.  It
 // serves the units u = q + m * nlanes, m = 0 .. rounds-1, where unit u = b * ngroups + g is group g (four consecutive
 // same-colour sites of a row, the unit of half_sweep_shared_vec) of coded batch b, and takes four draws per unit (R19); a
 // lane whose last unit does not exist still draws.  Consecutive lanes hold consecutive groups of one batch, so the
@@ -142,7 +142,8 @@ __global__ void __launch_bounds__(128) lanes_init(uint32_t *state, uint32_t nlan
 // (Holding the twelve state operands in registers across the lattice loads, so that both round trips overlap, spills at 64
 // registers and was slower: 0.249 against 0.239 ps/flip.)
 // ---------------------------------------------------------------------------------------------------
-template <int GEN>
+// VEC = false (L % 8 != 0): a group may straddle rows, its sums come from group_sums_any_L (one load per word).
+template <int GEN, bool VEC>
 __global__ void __launch_bounds__(128, 8)
 half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uint32_t gpr_inv, size_t batch_stride,
                         uint32_t ngroups, uint64_t units, uint32_t rounds)
@@ -160,7 +161,6 @@ half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uin
         lane_next4<GEN>(st, stride, pos, R);
         if (u >= units) continue;
         const uint32_t b = (uint32_t)(u / ngroups), g = (uint32_t)(u - (uint64_t)b * ngroups);
-        const uint32_t z = g / per_plane, p = g - z * per_plane;
         SweepArgs a = a0;
         const size_t off = (size_t)b * batch_stride;
         a.S_act += off;
@@ -168,8 +168,15 @@ half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uin
 #pragma unroll
         for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
         uint32_t j0, s[4], sum2[4], sum1[4], sum0[4], c4[4], c8[4], c12[4];
-        uint64_t site0;
-        vec_group_sums(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
+        if (VEC) {
+            const uint32_t z = g / per_plane, p = g - z * per_plane;
+            uint64_t site0;
+            vec_group_sums(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
+        } else {
+            uint64_t site[4];
+            j0 = 4u * g;
+            group_sums_any_L(a, g, s, sum2, sum1, sum0, site);
+        }
         shared_cond_words(R, a.T, c4, c8, c12);
         uint32_t out[4];
 #pragma unroll

@@ -487,23 +487,16 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
 // 8p..8p+7 (warp-uniform Philox constants), each warp updates byte p of its groups' words; the loads of the four warps
 // coincide (L1 hits).  This spreads a small lattice (config 2: 32768 groups) over every SM.
 // ---------------------------------------------------------------------------------------------------
-template <int RNG, int PARTS>
-__global__ void __launch_bounds__(128)
-half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_groups, uint64_t N)
+// Loads and field sums of the group g (colour ranks 4g .. 4g+3), sample-packed, any even L: the four sites may lie in
+// different rows, so every site computes its own six neighbour ranks.  site[w] = canonical index of site w (MINSTD ids).
+__device__ __forceinline__ void group_sums_any_L(const SweepArgs &a, uint32_t g, uint32_t s[4], uint32_t sum2[4], uint32_t sum1[4],
+                                                 uint32_t sum0[4], uint64_t site[4])
 {
-    constexpr int SPT = 32 / PARTS;  // samples per thread
-    const int part = PARTS == 1 ? 0 : (int)(threadIdx.x >> 5);  // warp-uniform
-    const uint32_t g_raw = PARTS == 1 ? blockIdx.x * 128u + threadIdx.x : blockIdx.x * 32u + (threadIdx.x & 31u);
-    const bool valid = g_raw < n_groups;
-    const uint32_t g = valid ? g_raw : n_groups - 1;  // keep the warp converged for the votes below
     const uint32_t L = (uint32_t)a.L, H = L >> 1, HL = H * L, Hc = HL * L;  // Hc = N/2 < 2^32 for L <= 2048
-    uint32_t s[4], sum2[4], sum1[4], sum0[4];
-    uint64_t site[4];
     const uint32_t j0 = 4u * g;
     uint32_t m = j0 % H;
     const uint32_t r0 = j0 / H;
     uint32_t y = r0 % L, z = r0 / L;
-    wait_for_previous_kernel();
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
         const uint32_t j = j0 + w;
@@ -529,6 +522,22 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
             if (++y == L) { y = 0; ++z; }
         }
     }
+}
+
+template <int RNG, int PARTS>
+__global__ void __launch_bounds__(128)
+half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_groups, uint64_t N)
+{
+    constexpr int SPT = 32 / PARTS;  // samples per thread
+    const int part = PARTS == 1 ? 0 : (int)(threadIdx.x >> 5);  // warp-uniform
+    const uint32_t g_raw = PARTS == 1 ? blockIdx.x * 128u + threadIdx.x : blockIdx.x * 32u + (threadIdx.x & 31u);
+    const bool valid = g_raw < n_groups;
+    const uint32_t g = valid ? g_raw : n_groups - 1;  // keep the warp converged for the votes below
+    uint32_t s[4], sum2[4], sum1[4], sum0[4];
+    uint64_t site[4];
+    const uint32_t j0 = 4u * g;
+    wait_for_previous_kernel();
+    group_sums_any_L(a, g, s, sum2, sum1, sum0, site);
     uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};
     if (RNG == 2) {  // shared draw: Eq. 15 verbatim, the cond words are all ones or zero
         uint32_t R[4];

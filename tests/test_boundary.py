@@ -45,14 +45,14 @@ def test_thresholds_equal_the_oracle_table(rng_mode):
 def test_lane_modes_host_side():
     """rng modes 3, 4 (R19): thresholds are the Philox table; the workspace grows by the strided generator state
     (62 / 624 words per lane; min(k N/8, 148*1024) lanes: one wave of threads);
-    L % 8 and nsamples % 32 are required."""
+    nsamples % 32 is required."""
     lib = binding.lib()
     out = C.c_size_t(0)
     for mode, ring, cap in ((binding.PR_SHARED, 62, 148 * 1024), (binding.MT19937_SHARED, 624, 148 * 1024)):
         for beta in (0.0, 0.4, 1 / 1.1, float("inf")):
             assert binding.ising_thresholds(beta, mode) == ea3d.thresholds(beta, mode) == ea3d.thresholds(beta, 0)
         assert lib.ising_workspace_bytes(16, 1, mode, C.byref(out)) == binding.EINVAL
-        assert lib.ising_workspace_bytes(12, 32, mode, C.byref(out)) == binding.EINVAL
+        assert lib.ising_workspace_bytes(12, 32, mode, C.byref(out)) == binding.OK      # any even L
         for L, ns in ((8, 32), (64, 64), (256, 32)):
             lanes = min((ns // 32) * L**3 // 8, cap)
             extra = binding.ising_workspace_bytes(L, ns, mode) - binding.ising_workspace_bytes(L, ns, binding.PHILOX_SHARED)

@@ -42,10 +42,12 @@ def assert_same_state(o, g, what=""):
 
 # nlanes None = the default min(N/8, 151552); the others give several rounds per lane and a ragged last round
 @pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
-# (16, 32, 7), (24, 64, 50): many rounds per lane, the ring wraps several times inside one launch
+# (16, 32, 7), (24, 64, 50): many rounds per lane, the ring wraps several times inside one launch; L = 4, 6, 10, 12, 20, 30: groups
+# of four sites that straddle rows (L % 8 != 0, per-word neighbour loads)
 @pytest.mark.parametrize("L,ns,nlanes", [(8, 32, None), (8, 64, 24), (16, 32, 100), (16, 96, 512), (24, 32, 333), (40, 32, None),
                                          (40, 64, 1000), (64, 32, 4096), (16, 32, 7), (24, 64, 50), (8, 1024, None), (8, 160, 300),
-                                         (16, 96, None)])
+                                         (16, 96, None), (4, 32, None), (6, 64, 5), (10, 32, None), (12, 96, 100), (20, 32, 333),
+                                         (30, 64, None)])
 def test_lane_mode_sweep_equals_the_oracle(mode, L, ns, nlanes):
     spins, J = synth.make_spins(L, ns, 71), synth.make_couplings(L, ns, 72)
     o, g = make_pair(L, ns, mode, nlanes, spins, J)
@@ -103,8 +105,6 @@ def test_lane_mode_argument_checks():
     for mode in (PR_SHARED, MT19937_SHARED):
         with pytest.raises(binding.IsingError):
             Ising(16, 1, SEED, mode)          # needs whole words of samples
-        with pytest.raises(binding.IsingError):
-            Ising(12, 32, SEED, mode)         # L % 8 != 0
         g = Ising(16, 32, SEED, mode)
         assert g.ising_get_lanes() == 16**3 // 8
         assert Ising(8, 96, SEED, mode).ising_get_lanes() == 3 * 8**3 // 8    # units = batches x groups
