@@ -157,6 +157,8 @@ def main():
     ap.add_argument("--only-lanes", action="store_true", help="time only the stored-state lane generators (sweep and Table II)")
     ap.add_argument("--scan-batches", action="store_true",
                     help="the paper's Fig. 4 study: half-sweep time of small lattices against the number k of coded batches (shared draws)")
+    ap.add_argument("--aux", action="store_true",
+                    help="rows a9 / a10 and the general-L kernels: load_state, energy, get_spins and a half-sweep per layout, with GB/s")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -339,6 +341,44 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.aux:  # measurement of the rows outside the headline step: every layout's load / energy / get and half-sweep
+        def avg_ms(fn, n=5):
+            fn()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(n):
+                fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / n
+
+        rows = []
+        for Ls, ns, mode, what in ((1024, 1, 0, "site-packed, L multiple of 64 (word-parallel kernels)"),
+                                   (1000, 1, 0, "site-packed, general even L (bit-window kernels)"),
+                                   (250, 1, 0, "site-packed, general even L (bit-window kernels)"),
+                                   (512, 32, 2, "sample-packed, L multiple of 32 (tile load/get, bit-sliced energy)"),
+                                   (128, 256, 2, "sample-packed, 8 coded batches"),
+                                   (100, 32, 2, "sample-packed, general even L (one bit at a time load/get)")):
+            sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
+            Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
+            out = torch.empty_like(sp)
+            g = Ising(Ls, ns, synth.DYN_SEED, mode)
+            state = ns * Ls**3 / 8 * 4  # packed spins + couplings, bytes
+            t_load = avg_ms(lambda: g.ising_load_state(sp, Jc))
+            t_sweep = avg_ms(lambda: g.ising_sweep(BETA, 2)) / 4
+            t_energy = avg_ms(lambda: g.ising_energy())
+            t_get = avg_ms(lambda: g.ising_get_spins(out))
+            g.ising_destroy()
+            rows.append({"L": Ls, "nsamples": ns, "layout": what, "rng_mode": mode,
+                         "load_state_ms": t_load, "load_GBps_read_plus_write": 2 * state / t_load / 1e6,
+                         "energy_ms": t_energy, "energy_GBps": state / t_energy / 1e6,
+                         "get_spins_ms": t_get, "get_GBps_read_plus_write": 2 * state / 4 / t_get / 1e6,
+                         "half_sweep_us": 1e3 * t_sweep, "ps_per_flip": 2e9 * t_sweep / (ns * Ls**3)})
+            del sp, Jc, out
+        print(json.dumps({"aux": rows}))
         return
 
     if args.scan_batches:  # PAPER.md:308-310, Fig. 4: t_SW stays flat in k until the GPU is full, then grows linearly
