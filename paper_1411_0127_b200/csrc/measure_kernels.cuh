@@ -4,6 +4,9 @@
 //   bond bit e = J ^ s_i ^ s_k (Eq. 11) is 1 exactly when -J sigma_i sigma_k = +1, so E = 2*popc(e over all bonds) - 3N,
 //   and M = 2*popc(s) - N.  The kernels accumulate the two popcounts per sample into uint64 counters (warp shuffle
 //   reduction, then a block reduction and one atomic pair per CTA); finalize_energy turns them into int64 E and M.
+//   Kernels: energy_site_packed<W> (L a multiple of 64, fused finalisation), energy_site_packed_rows (every other even L, bit
+//   windows), energy_sample_packed_sliced (sample-packed: bit-sliced column sums, all batches, fused finalisation), and the
+//   one-bit-at-a-time energy_site_packed_generic / energy_sample_packed (kernel choice 1).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

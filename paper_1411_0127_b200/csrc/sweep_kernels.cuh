@@ -10,9 +10,12 @@
 // have the same m in the other colour's arrays; its two x-neighbours are bits m and m-1 (xodd = 0) or m and m+1
 // (xodd = 1) of the other colour's half-row.
 //
-// Kernels: half_sweep_site_packed<RNG, W> (RNG 0 = Philox, 1 = MINSTD stateless, 2 = MINSTD with cached seed states),
-// minstd_fill_s0<W>, half_sweep_site_packed_generic<RNG>, half_sweep_sample_packed<RNG, PARTS> (RNG 2 = shared draw, R18),
-// half_sweep_shared_vec (shared draw, 128-bit loads, all coded batches in one launch).
+// Kernels: half_sweep_site_packed<RNG, W> (L a multiple of 64; RNG 0 = Philox, 1 = MINSTD stateless, 2 = MINSTD with cached
+// seed states), minstd_fill_s0<W>, half_sweep_site_packed_rows<RNG> (every other even L: operands gathered as bit windows),
+// half_sweep_site_packed_generic<RNG> (one site at a time; kernel choice 1), half_sweep_sample_packed<RNG, PARTS> (any L;
+// RNG 2 = shared draw, R18), half_sweep_sample_packed_vec<RNG, PARTS, MULTI> (L % 8 == 0, 128-bit loads, optionally all coded
+// batches in one launch), half_sweep_shared_vec<FLAT> (shared draw, 128-bit loads, all coded batches in one launch).
+// The lane-generator kernels (rng modes 3, 4) are in lane_rng.cuh.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
