@@ -152,7 +152,8 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
 /* Select the kernels: 0 = automatic (site-packed: the word-parallel kernel when L is a multiple of 64, with the cached seed
  * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
  * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),
- * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw).  All give the same bits;
+ * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = the bit-window kernel with its
+ * row-segment loop also for L >= 64 (where the automatic choice is the loop-free variant).  All give the same bits;
  * the tests use this to show that results do not depend on layout, thread mapping or caching. */
 int ising_set_kernel(ising_t *h, int which);
 

@@ -291,7 +291,10 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
             sr.seed = r.seed;
             sr.A2 = 2u * r.A;
             sr.s0tab = nullptr;
-            launch_pdl(half_sweep_site_packed_rows<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw, (uint32_t)g.Hc);
+            if (g.L >= 64 && h->kernel_choice != 3)   // rows of at least 32 bits: no segment loop (kernel choice 3 keeps the loop)
+                launch_pdl(half_sweep_site_packed_rows2<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw, (uint32_t)g.Hc);
+            else
+                launch_pdl(half_sweep_site_packed_rows<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw, (uint32_t)g.Hc);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
             launch_pdl(half_sweep_site_packed_generic<RNG>, dim3((unsigned)((nw + 255) / 256)), dim3(256), st, a, r, (uint64_t)nw, (uint64_t)g.Hc);
@@ -761,7 +764,7 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
 
 int ising_set_kernel(ising_t *h, int which)
 {
-    if (!h || which < 0 || which > 2) return ISING_EINVAL;
+    if (!h || which < 0 || which > 3) return ISING_EINVAL;
     h->kernel_choice = which;
     return ISING_OK;
 }

@@ -483,6 +483,94 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
 }
 
 // ---------------------------------------------------------------------------------------------------
+// The same for rows of at least 32 bits (L >= 64), without the segment loop: a word then lies in one row or straddles two
+// (bits 0..k-1 in row A, bits k..31 in row B), and in rank space its neighbour sets are ALMOST contiguous over both:
+//   +-y, +-z: rank j + off with the same offset for both rows unless one of them sits at a periodic boundary (3 of L
+//             straddling words): one unaligned window, a second one only in that rare case;
+//   +-x:      ranks j-1, j, j+1 of the other colour are the aligned word itself and its two one-bit shifts; which of them a
+//             bit takes depends on the x parity of its row (mask X); the periodic bit at a row end / row start inside the
+//             word is patched in.
+// The segment loop of half_sweep_site_packed_rows makes every warp pay for two segments as soon as one of its 32 words
+// straddles (always, for L < 2048); here the straddle costs a few mask operations: 933 -> 560 instructions per word.
+// ---------------------------------------------------------------------------------------------------
+template <int RNG>
+__global__ void __launch_bounds__(128)
+half_sweep_site_packed_rows2(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t n_words, uint32_t Hc)
+{
+    const uint32_t w = blockIdx.x * 128u + threadIdx.x;
+    if (w >= n_words) return;
+    const uint32_t L = (uint32_t)a.L, H = L >> 1, LH = L * H;
+    const uint32_t j0 = 32u * w;
+    const uint32_t rA = j0 / H, m0 = j0 - rA * H, zA = rA / L, yA = rA - zA * L;
+    const uint32_t nvalid = Hc - j0 < 32u ? Hc - j0 : 32u;
+    const uint32_t k = H - m0;                                   // bits 0..k-1 are in row A
+    const bool two = k < nvalid;                                 // bits k.. are in row B = the next row
+    uint32_t yB = yA + 1, zB = zA;
+    if (yB == L) { yB = 0; ++zB; }
+    const uint32_t xoddA = (yA + zA + (uint32_t)a.colour) & 1u, xoddB = (yB + zB + (uint32_t)a.colour) & 1u;
+    const uint32_t maskA = k >= 32u ? 0xFFFFFFFFu : (1u << k) - 1u, maskB = ~maskA;
+    const uint32_t X = (xoddA ? maskA : 0u) | (xoddB ? maskB : 0u);   // x parity of every bit's site
+    const uint32_t PA = rA * H;                                  // rank of the first site of row A; row B starts at PA + H
+    wait_for_previous_kernel();
+    const uint32_t s = __ldg(a.S_act + w);
+    uint32_t J[6], nb[6];
+    J[0] = __ldg(a.J_act[0] + w);
+    J[2] = __ldg(a.J_act[1] + w);
+    J[4] = __ldg(a.J_act[2] + w);
+    {   // +-x
+        const uint32_t lo = __ldg(a.S_oth + w), hi = __ldg(a.S_oth + w + 1), prev = w ? __ldg(a.S_oth + w - 1) : 0u;
+        const uint32_t jlo = __ldg(a.J_oth[0] + w), jprev = w ? __ldg(a.J_oth[0] + w - 1) : 0u;
+        nb[0] = (X & __funnelshift_r(lo, hi, 1)) | (~X & lo);
+        nb[1] = (X & lo) | (~X & __funnelshift_l(prev, lo, 1));
+        J[1] = (X & jlo) | (~X & __funnelshift_l(jprev, jlo, 1));
+        if (k <= 32u && xoddA) nb[0] = (nb[0] & ~(1u << (k - 1))) | (bit_at(a.S_oth, PA) << (k - 1));   // row A ends here: +x wraps
+        if (m0 == 0 && !xoddA) {                                                                        // row A starts here: -x wraps
+            nb[1] = (nb[1] & ~1u) | bit_at(a.S_oth, PA + H - 1);
+            J[1] = (J[1] & ~1u) | bit_at(a.J_oth[0], PA + H - 1);
+        }
+        if (two && !xoddB) {                                                                            // row B starts at bit k
+            nb[1] = (nb[1] & ~(1u << k)) | (bit_at(a.S_oth, PA + 2 * H - 1) << k);
+            J[1] = (J[1] & ~(1u << k)) | (bit_at(a.J_oth[0], PA + 2 * H - 1) << k);
+        }
+    }
+    {   // +-y, +-z: offsets in rank space (mod 2^32), per row
+        const uint32_t ypA = (yA + 1 == L) ? 0u - (LH - H) : H, ypB = (yB + 1 == L) ? 0u - (LH - H) : H;
+        const uint32_t ymA = (yA == 0) ? LH - H : 0u - H, ymB = (yB == 0) ? LH - H : 0u - H;
+        const uint32_t zpA = (zA + 1 == L) ? 0u - (Hc - LH) : LH, zpB = (zB + 1 == L) ? 0u - (Hc - LH) : LH;
+        const uint32_t zmA = (zA == 0) ? Hc - LH : 0u - LH, zmB = (zB == 0) ? Hc - LH : 0u - LH;
+        nb[2] = bit_window(a.S_oth, j0 + ypA);
+        nb[3] = bit_window(a.S_oth, j0 + ymA);
+        J[3] = bit_window(a.J_oth[1], j0 + ymA);
+        nb[4] = bit_window(a.S_oth, j0 + zpA);
+        nb[5] = bit_window(a.S_oth, j0 + zmA);
+        J[5] = bit_window(a.J_oth[2], j0 + zmA);
+        if (two && (ypA != ypB || ymA != ymB || zpA != zpB || zmA != zmB)) {   // a periodic boundary between the two rows: rare
+            // row B's windows start at its first bit k (j0 + offset alone may lie before the array)
+            const uint32_t jB = j0 + k;
+            nb[2] = (nb[2] & maskA) | (bit_window(a.S_oth, jB + ypB) << k);
+            nb[3] = (nb[3] & maskA) | (bit_window(a.S_oth, jB + ymB) << k);
+            J[3] = (J[3] & maskA) | (bit_window(a.J_oth[1], jB + ymB) << k);
+            nb[4] = (nb[4] & maskA) | (bit_window(a.S_oth, jB + zpB) << k);
+            nb[5] = (nb[5] & maskA) | (bit_window(a.S_oth, jB + zmB) << k);
+            J[5] = (J[5] & maskA) | (bit_window(a.J_oth[2], jB + zmB) << k);
+        }
+    }
+    uint32_t c4, c8, c12;
+    if (RNG == 0) {
+        cond_masks_site_packed_philox(rng.pc, rng.ps, w, a.T, c4, c8, c12);
+    } else {   // MINSTD: canonical site index of bit b = site0 + 2b within its row; both bases are referred to bit 0
+        const uint64_t siteA = (uint64_t)L * rA + 2u * m0 + xoddA;
+        const uint64_t siteB = (uint64_t)L * (rA + 1) + xoddB - 2ull * k;
+        cond_masks_site_packed_minstd_two(rng.seed + (siteA + 1) * SPLITMIX_GAMMA, rng.seed + (siteB + 1) * SPLITMIX_GAMMA, k,
+                                          2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
+    }
+    uint32_t sum2, sum1, sum0;
+    satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
+    const uint32_t valid = nvalid == 32u ? 0xFFFFFFFFu : (1u << nvalid) - 1u;
+    a.S_act[w] = s ^ (flip_mask(sum2, sum1, sum0, c4, c8, c12) & valid);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Sample-packed kernel (nsamples = 32 per batch), any even L >= 4.  A Philox group g = 4 consecutive same-colour sites
 // j = 4g..4g+3 needs one call per sample (bit), keyed by the sample (R9).  Neighbours are whole words, so no
 // x-alignment is needed.  A CTA has 4 warps.  PARTS = 1: one thread per group, all 32 samples (large lattices: index

@@ -123,4 +123,23 @@ ISING_HD void cond_masks_site_packed_minstd(uint64_t weyl0, uint64_t weyl_step, 
     finish_cond(T, c4, c8, c12);
 }
 
+// The same for a word whose bits 0..k-1 and k..31 lie in two different rows (general L): bit b uses the Weyl state
+// (b < k ? weylA : weylB) + b * weyl_step, where weylA / weylB are referred to bit 0 of the word.
+ISING_HD void cond_masks_site_packed_minstd_two(uint64_t weylA, uint64_t weylB, uint32_t k, uint64_t weyl_step, uint32_t A2,
+                                                const Thresholds &T, uint32_t &c4, uint32_t &c8, uint32_t &c12)
+{
+    c4 = 0; c8 = 0; c12 = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        uint32_t R[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const uint32_t b = (uint32_t)(4 * q + w);
+            R[w] = minstd_mulmod2(A2, minstd_seed_state_from_weyl((b < k ? weylA : weylB) + (uint64_t)b * weyl_step));
+        }
+        accumulate_cond<4>(R, 4 * q, T, c4, c8, c12);
+    }
+    finish_cond(T, c4, c8, c12);
+}
+
 }  // namespace isingk

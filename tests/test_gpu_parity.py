@@ -103,7 +103,7 @@ def test_config1_L16_philox_energy_every_half_sweep():
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
-@pytest.mark.parametrize("L", [4, 6, 10, 16, 18, 22, 24, 32, 34, 62, 64, 66, 96, 100, 126, 128, 130, 250, 256])
+@pytest.mark.parametrize("L", [4, 6, 10, 16, 18, 22, 24, 32, 34, 62, 64, 66, 70, 96, 100, 126, 128, 130, 190, 250, 256])
 def test_site_packed_trajectories(L, rng_mode):
     """Ragged and whole-word half-rows: the word-parallel kernel for L a multiple of 64, the bit-window kernel for every other
     even L (rows shorter than a word, rows of 33 / 62.5 / 125 bits straddling words, a partial last word), and the
@@ -116,11 +116,12 @@ def test_site_packed_trajectories(L, rng_mode):
         o.sweep(beta, 1)
     E, M = g.ising_sweep_trace(beta, nsw, every_half_sweeps=2 * nsw)
     assert_same_state(o, g, f"L={L}")
-    g1 = Ising(L, 1, SEED, rng_mode)
-    g1.ising_set_kernel(1)
-    g1.ising_load_state(dev(spins), dev(J))
-    g1.ising_sweep(beta, nsw)
-    assert torch.equal(g.ising_get_spins(), g1.ising_get_spins()), f"L={L}: kernel choice 1 differs"
+    for choice in (1, 3):     # one site at a time; the bit-window kernel with its segment loop (L >= 64 runs the loop-free one)
+        g1 = Ising(L, 1, SEED, rng_mode)
+        g1.ising_set_kernel(choice)
+        g1.ising_load_state(dev(spins), dev(J))
+        g1.ising_sweep(beta, nsw)
+        assert torch.equal(g.ising_get_spins(), g1.ising_get_spins()), f"L={L}: kernel choice {choice} differs"
     Eo, Mo = o.energy()
     assert int(E[0, 0]) == int(Eo[0]) and int(M[0, 0]) == int(Mo[0])
     assert int(Eo[0]) == int(o.dE_sum[0]) + int(ea3d.Oracle.energy(_loaded(L, 1, rng_mode, spins, J))[0][0])
