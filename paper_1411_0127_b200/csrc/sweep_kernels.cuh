@@ -491,7 +491,7 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
 //             bit takes depends on the x parity of its row (mask X); the periodic bit at a row end / row start inside the
 //             word is patched in.
 // The segment loop of half_sweep_site_packed_rows makes every warp pay for two segments as soon as one of its 32 words
-// straddles (always, for L < 2048); here the straddle costs a few mask operations: 933 -> 560 instructions per word.
+// straddles (always, for L < 2048); here the straddle costs a few mask operations: 933 -> 711 instructions per word (ncu).
 // ---------------------------------------------------------------------------------------------------
 template <int RNG>
 __global__ void __launch_bounds__(128)
