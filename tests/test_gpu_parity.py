@@ -606,3 +606,22 @@ def test_config5_L1024_full_size(rng_mode):
             assert int(finals[colour][i]) == int(before_bits[i]) ^ flips, (colour, x, y, z, dE, R)
             n_flipped += flips
         assert 0 < n_flipped < 2000
+
+
+@pytest.mark.parametrize("nsamples,rng_mode", [(1, PHILOX), (1, MINSTD), (32, PHILOX), (96, MINSTD), (96, PHILOX_SHARED)])
+def test_automatic_and_one_at_a_time_kernels_agree_over_sizes(nsamples, rng_mode):
+    """Every layout-specific kernel family (word-parallel, bit-window with and without the segment loop, vectorised / multi-batch
+    sample-packed, tile load / get, bit-sliced energy) against the one-site / one-bit-at-a-time kernels (choice 1) on the same
+    inputs: spins, energies and magnetisations after three sweeps, over lattice sizes of every alignment class."""
+    sizes = (4, 6, 10, 12, 20, 36, 48, 66, 72, 100, 136, 160, 200) if nsamples == 1 else (4, 6, 10, 12, 20, 36, 40, 48, 66, 72)
+    for L in sizes:
+        spins, J = synth.make_spins(L, nsamples, 3), synth.make_couplings(L, nsamples, 4)
+        res = []
+        for choice in (0, 1):
+            g = Ising(L, nsamples, 777, rng_mode)
+            g.ising_set_kernel(choice)
+            g.ising_load_state(dev(spins), dev(J))
+            E, M = g.ising_sweep_trace(0.8, 3, every_half_sweeps=3)
+            res.append((g.ising_get_spins().clone(), E.clone(), M.clone()))
+            g.ising_destroy()
+        assert all(torch.equal(a, b) for a, b in zip(res[0], res[1])), f"L={L} x {nsamples}, mode {rng_mode}"
