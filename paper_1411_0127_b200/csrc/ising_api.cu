@@ -493,8 +493,11 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
     const size_t W = g.canon_words;
     if (g.nsamples == 1) {
         const LatticeArrays A = h->arrays(0);
-        // the padding words of the arrays must not hold garbage (generic kernels read whole words)
-        if (cudaMemsetAsync(h->ws, 0, g.arrays_total_words * sizeof(uint32_t), st) != cudaSuccess) return ISING_ECUDA;
+        // the padding words of the arrays must not hold garbage (generic kernels read whole words); when L is a multiple of 64
+        // the arrays have no padding (L^3/64 words each) and the split kernel writes every word
+        if (g.array_words * 32 != g.Hc &&
+            cudaMemsetAsync(h->ws, 0, g.arrays_total_words * sizeof(uint32_t), st) != cudaSuccess)
+            return ISING_ECUDA;
         if (g.fast) {
             SplitArgs s;
             s.narrays = 4;
