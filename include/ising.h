@@ -134,6 +134,12 @@ int ising_set_t(ising_t *h, uint64_t t); /* ISING_EINVAL in the lane modes 3, 4:
 int ising_get_lanes(const ising_t *h, uint32_t *nlanes);
 int ising_set_lanes(ising_t *h, uint32_t nlanes);
 
+/* Lane modes only: resume from a checkpoint.  The whole run state is (the workspace bytes, t, nlanes): save a copy of the
+ * workspace with ising_get_t and ising_get_lanes; to resume, create a handle on a workspace holding those bytes and call
+ * ising_resume_lanes(h, t, nlanes), which sets the half-sweep counter and keeps the generator state found in the workspace
+ * instead of seeding it.  (In the other modes ising_get_spins + ising_load_state + ising_set_t do the same.) */
+int ising_resume_lanes(ising_t *h, uint64_t t, uint32_t nlanes);
+
 /* The paper's device-API generator benchmark (Table II): every lane draws numbers and counts the odd ones.
  * kind: ISING_RNG_PHILOX (no state; key (lo32 seed, hi32 seed), counter (lo32 c, hi32 c, lane, 0), c = draw number >> 2, output
  * word = draw number & 3), ISING_RNG_MINSTD (one word per lane, the seed state of stream `lane`, R11, advanced once per draw),

@@ -19,7 +19,7 @@ EXPORTS = (
     "ising_workspace_bytes", "ising_create", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
     "ising_get_spins", "ising_run_host", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
-    "ising_get_lanes", "ising_set_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
+    "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
 )
 
 _lib = None
@@ -56,6 +56,7 @@ def lib() -> C.CDLL:
                                               C.POINTER(C.c_uint32)]
     L.ising_get_lanes.argtypes = [vp, C.POINTER(C.c_uint32)]
     L.ising_set_lanes.argtypes = [vp, C.c_uint32]
+    L.ising_resume_lanes.argtypes = [vp, u64, C.c_uint32]
     L.ising_prng_state_bytes.argtypes = [i32, C.c_uint32, C.POINTER(sz)]
     L.ising_prng_init.argtypes = [i32, u64, C.c_uint32, vp, vp]
     L.ising_prng_count_odd.argtypes = [i32, u64, C.c_uint32, u64, u64, vp, vp, vp, vp]
@@ -223,6 +224,9 @@ class Ising:
 
     def ising_set_lanes(self, nlanes: int):
         _check(lib().ising_set_lanes(self._h, int(nlanes)), "ising_set_lanes")
+
+    def ising_resume_lanes(self, t: int, nlanes: int):
+        _check(lib().ising_resume_lanes(self._h, int(t), int(nlanes)), "ising_resume_lanes")
 
     def ising_set_kernel(self, which: int):
         _check(lib().ising_set_kernel(self._h, int(which)), "ising_set_kernel")

@@ -718,6 +718,15 @@ int ising_set_lanes(ising_t *h, uint32_t nlanes)
     return ISING_OK;
 }
 
+int ising_resume_lanes(ising_t *h, uint64_t t, uint32_t nlanes)
+{
+    if (!h || !lane_mode(h->rng_mode) || nlanes < 1 || nlanes > lanes_default(h->g, h->rng_mode)) return ISING_EINVAL;
+    h->t = t;
+    h->nlanes = nlanes;
+    h->lanes_ready = true;  // the generator state in the workspace is the checkpoint's
+    return ISING_OK;
+}
+
 int ising_prng_state_bytes(int kind, uint32_t nlanes, size_t *out)
 {
     if (!out || !known_mode(kind) || kind == ISING_RNG_PHILOX_SHARED || nlanes < 1) return ISING_EINVAL;

@@ -101,6 +101,28 @@ def test_lane_mode_special_temperatures(mode, beta):
     assert_same_state(o, g, f"lane mode beta={beta}")
 
 
+@pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
+def test_lane_mode_checkpoint_and_resume(mode):
+    """The run state is (workspace bytes, t, nlanes): a copy of the workspace taken after 3 sweeps, resumed in a new handle, continues
+    exactly like the uninterrupted run (and like the oracle)."""
+    L, ns, nlanes = 16, 64, 77
+    spins, J = synth.make_spins(L, ns, 81), synth.make_couplings(L, ns, 82)
+    o, g = make_pair(L, ns, mode, nlanes, spins, J)
+    g.ising_sweep(0.9, 3)
+    o.sweep(0.9, 3)
+    torch.cuda.synchronize()
+    saved, t = g.workspace.clone(), g.ising_get_t()
+    g.ising_sweep(0.9, 2)
+    o.sweep(0.9, 2)
+    r = Ising(L, ns, SEED, mode, workspace=saved)
+    r.ising_resume_lanes(t, nlanes)
+    r.ising_sweep(0.9, 2)
+    assert torch.equal(r.ising_get_spins(), g.ising_get_spins())
+    assert_same_state(o, r, "resumed run")
+    with pytest.raises(binding.IsingError):
+        Ising(16, 32, SEED, PHILOX).ising_resume_lanes(0, 1)
+
+
 def test_lane_mode_argument_checks():
     for mode in (PR_SHARED, MT19937_SHARED):
         with pytest.raises(binding.IsingError):
