@@ -106,6 +106,10 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
  * every sample (row a9).  d_E: nsamples int64; d_M: nsamples int64 or NULL. */
 int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream);
 
+/* Overlap of two samples of one handle, q = sum_i sigma_i^a sigma_i^b in [-N, N] (one int64 at d_q): the spin-glass order
+ * parameter when the two samples are replicas, i.e. were loaded with the same couplings.  nsamples = 32k only. */
+int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *stream);
+
 /* Write the spins in the canonical packed format: nsamples x W uint32 (row a10). */
 int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream);
 

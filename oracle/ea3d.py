@@ -40,6 +40,8 @@ def lib():
         L.oracle_thresholds.restype = C.c_int
         L.oracle_energy.argtypes = [C.c_int, C.c_int, i8p, i8p, i8p, i8p, i64p, i64p]
         L.oracle_energy.restype = None
+        L.oracle_overlap.argtypes = [C.c_int, i8p, i8p]
+        L.oracle_overlap.restype = C.c_int64
         L.oracle_minstd_init.argtypes = [C.c_int, C.c_int, C.c_uint64, u32p]
         L.oracle_minstd_init.restype = None
         L.oracle_half_sweep.argtypes = [C.c_int, C.c_int, i8p, i8p, i8p, i8p, C.c_uint64, C.c_int, C.c_uint64,
@@ -294,6 +296,10 @@ class Oracle:
         lib().oracle_energy(self.L, self.nsamples, _p(self.sigma, C.c_int8), _p(self.Jx, C.c_int8),
                             _p(self.Jy, C.c_int8), _p(self.Jz, C.c_int8), _p(E, C.c_int64), _p(M, C.c_int64))
         return E, M
+
+    def overlap(self, a: int, b: int) -> int:
+        """q_ab = sum_i sigma_i^a sigma_i^b (replicas)."""
+        return int(lib().oracle_overlap(self.L, _p(self.sigma[a], C.c_int8), _p(self.sigma[b], C.c_int8)))
 
     def site_flips(self, beta: float, sample: int, x: int, y: int, z: int, t: int | None = None):
         """(flips, dE, R) for one site of the active colour of half-sweep t, from the CURRENT state."""

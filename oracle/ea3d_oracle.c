@@ -210,6 +210,15 @@ void oracle_energy(int L, int nsamples, const int8_t *sigma, const int8_t *Jx, c
     }
 }
 
+/* Overlap of two replicas (samples with the same couplings, "we simulate four replicas at once"):
+ *   q_ab = sum_i sigma_i^a sigma_i^b,   an integer in [-N, N]; q_aa = N. */
+int64_t oracle_overlap(int L, const int8_t *sigma_a, const int8_t *sigma_b)
+{
+    int64_t N = (int64_t)L * L * L, q = 0;
+    for (int64_t i = 0; i < N; ++i) q += (int64_t)sigma_a[i] * (int64_t)sigma_b[i];
+    return q;
+}
+
 /* Fill the per-site MINSTD stream states with their seed states (R11). */
 void oracle_minstd_init(int L, int nsamples, uint64_t seed, uint32_t *state)
 {

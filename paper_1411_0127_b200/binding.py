@@ -19,7 +19,7 @@ EXPORTS = (
     "ising_workspace_bytes", "ising_create", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
     "ising_get_spins", "ising_run_host", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
-    "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
+    "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
 )
 
 _lib = None
@@ -43,6 +43,7 @@ def lib() -> C.CDLL:
     L.ising_sweep_trace.argtypes = [vp, dbl, i32, vp, vp, i32, vp]
     L.ising_energy.argtypes = [vp, vp, vp, vp]
     L.ising_get_spins.argtypes = [vp, vp, vp]
+    L.ising_overlap.argtypes = [vp, i32, i32, vp, vp]
     L.ising_run_host.argtypes = [vp, vp, vp, dbl, i32, vp, vp, vp, vp]
     L.ising_thresholds.argtypes = [dbl, i32, C.POINTER(u64)]
     L.ising_fnv1a64_host.argtypes = [vp, sz]
@@ -188,6 +189,14 @@ class Ising:
         M = torch.empty(self.nsamples, dtype=torch.int64, device=self.device)
         _check(lib().ising_energy(self._h, E.data_ptr(), M.data_ptr(), _stream_ptr(stream)), "ising_energy")
         return E, M
+
+    def ising_overlap(self, sample_a: int, sample_b: int, stream=None):
+        """Returns q_ab as a one-element int64 CUDA tensor."""
+        import torch
+
+        q = torch.empty(1, dtype=torch.int64, device=self.device)
+        _check(lib().ising_overlap(self._h, int(sample_a), int(sample_b), q.data_ptr(), _stream_ptr(stream)), "ising_overlap")
+        return q
 
     def ising_get_spins(self, out=None, stream=None):
         import torch

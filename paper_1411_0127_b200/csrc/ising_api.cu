@@ -64,7 +64,7 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
     // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs and the ticket of the word-parallel energy kernel
-    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1) * sizeof(unsigned long long), 256);
+    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1 + 2) * sizeof(unsigned long long), 256);  // + overlap counter
     g->fast = nsamples == 1 && L % 64 == 0;
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
     // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
@@ -101,6 +101,7 @@ struct ising {
     uint32_t nlanes;
     bool lanes_ready;
     bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
+    bool overlap_clean;  // the counter of ising_overlap is zero
 
     LatticeArrays arrays(int batch) const
     {
@@ -472,6 +473,7 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->s0tab = (rng_mode == ISING_RNG_MINSTD && h->g.s0_words) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->s0_ready = false;
     h->slots_clean = false;
+    h->overlap_clean = false;
     h->lane_state = lane_mode(rng_mode) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->nlanes = lane_mode(rng_mode) ? lanes_default(h->g, rng_mode) : 0;
     h->lanes_ready = false;
@@ -640,6 +642,27 @@ int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream)
 {
     if (!h || !d_E) return ISING_EINVAL;
     return measure(h, (long long *)d_E, (long long *)d_M, (cudaStream_t)stream);
+}
+
+int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *stream)
+{
+    if (!h || !d_q || h->g.nsamples == 1 || sample_a < 0 || sample_b < 0 || sample_a >= h->g.nsamples || sample_b >= h->g.nsamples)
+        return ISING_EINVAL;
+    if (h->g.Hc >= (1ull << 32)) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geometry &g = h->g;
+    // the counter pair lives behind the ticket of the energy kernels
+    unsigned long long *cnt = h->acc + 4 * (size_t)g.nsamples + 2 * ACC_SLOTS + 1;
+    if (!h->overlap_clean) {
+        if (cudaMemsetAsync(cnt, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
+        h->overlap_clean = true;   // finalize_overlap leaves it zero
+    }
+    const LatticeArrays A = h->arrays(sample_a >> 5), B = h->arrays(sample_b >> 5);
+    const unsigned need = (unsigned)((g.Hc + 255) / 256);
+    overlap_sample_packed<<<need < 148u * 8u ? need : 148u * 8u, 256, 0, st>>>(A.S[0], B.S[0], A.S[1], B.S[1], sample_a & 31, sample_b & 31,
+                                                                         (uint32_t)g.Hc, cnt);
+    finalize_overlap<<<1, 1, 0, st>>>(cnt, (long long)g.N, (long long *)d_q);
+    return check_launch(h, 2);
 }
 
 int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps, uint32_t *h_spins_out,

@@ -402,6 +402,26 @@ energy_sample_packed_sliced(const __grid_constant__ MeasureArgs a, size_t batch_
     }
 }
 
+// Overlap of two samples of a sample-packed handle (replicas): q = sum_i sigma^a_i sigma^b_i = N - 2 D with D the
+// number of sites where bit ia of sample a's word differs from bit ib of sample b's word.  Wa / Wb: the spin arrays (one
+// colour) of the batches holding a and b.  Persistent grid, one atomic per CTA; *cnt must be zero on entry.
+__global__ void __launch_bounds__(256)
+overlap_sample_packed(const uint32_t *__restrict__ Wa0, const uint32_t *__restrict__ Wb0, const uint32_t *__restrict__ Wa1,
+                      const uint32_t *__restrict__ Wb1, int ia, int ib, uint32_t Hc, unsigned long long *cnt)
+{
+    unsigned long long d = 0, unused = 0;
+    for (uint32_t j = blockIdx.x * 256u + threadIdx.x; j < Hc; j += gridDim.x * 256u)
+        d += (((__ldg(Wa0 + j) >> ia) ^ (__ldg(Wb0 + j) >> ib)) & 1u) + (((__ldg(Wa1 + j) >> ia) ^ (__ldg(Wb1 + j) >> ib)) & 1u);
+    block_accumulate2(d, unused, cnt);
+}
+
+__global__ void finalize_overlap(unsigned long long *cnt, long long N, long long *q)
+{
+    *q = N - 2 * (long long)cnt[0];
+    cnt[0] = 0;
+    cnt[1] = 0;
+}
+
 // E = 2*unsat - 3N, M = 2*up - N  (R16), one thread per sample (sample-packed and generic paths).
 __global__ void finalize_energy(const unsigned long long *acc, int nsamples, long long N, long long *E, long long *M)
 {

@@ -625,3 +625,24 @@ def test_automatic_and_one_at_a_time_kernels_agree_over_sizes(nsamples, rng_mode
             res.append((g.ising_get_spins().clone(), E.clone(), M.clone()))
             g.ising_destroy()
         assert all(torch.equal(a, b) for a, b in zip(res[0], res[1])), f"L={L} x {nsamples}, mode {rng_mode}"
+
+
+@pytest.mark.parametrize("L,nsamples", [(6, 32), (16, 64), (40, 96)])
+def test_overlap_of_replicas_equals_the_oracle(L, nsamples):
+    """ising_overlap: q_ab = sum_i sigma^a sigma^b for samples in the same and in different coded batches, on
+    replicas (same couplings, different initial spins) after a few sweeps."""
+    W = (L**3 + 31) // 32
+    J1 = synth.make_couplings(L, 1, 33)
+    J = np.tile(J1.reshape(1, 3, W), (nsamples, 1, 1))
+    spins = synth.make_spins(L, nsamples, 34)
+    o, g = make_pair(L, nsamples, PHILOX, spins, J)
+    o.sweep(0.9, 2)
+    g.ising_sweep(0.9, 2)
+    pairs = [(0, 0), (0, 1), (5, 31), (31, 5), (nsamples - 1, 0), (nsamples - 1, nsamples - 2), (7, nsamples - 9)]
+    for a, b in pairs:
+        assert int(g.ising_overlap(a, b)[0]) == o.overlap(a, b), (a, b)
+    assert int(g.ising_overlap(3, 3)[0]) == L**3
+    with pytest.raises(binding.IsingError):
+        g.ising_overlap(0, nsamples)
+    with pytest.raises(binding.IsingError):
+        Ising(64, 1, SEED, PHILOX).ising_overlap(0, 0)

@@ -384,3 +384,18 @@ def test_high_temperature_energy_of_the_ferromagnet_and_of_pm_J():
             o.sweep(beta, 1)
             acc.append(o.energy()[0][0] / N)
         assert abs(np.mean(acc) - expect) < 0.02, (np.mean(acc), expect)
+
+
+def test_overlap_against_closed_forms_and_a_library_dot_product():
+    """q_ab = sum_i sigma^a_i sigma^b_i: q_aa = N, q(a, -a) = -N, symmetry, and numpy's dot product."""
+    L, ns = 6, 4
+    o = ea3d.Oracle(L, ns, 1, ea3d.PHILOX)
+    rng = np.random.default_rng(9)
+    sg = (2 * rng.integers(0, 2, size=(ns, L**3)) - 1).astype(np.int8)
+    sg[3] = -sg[0]
+    o.load_arrays(sg, np.ones_like(sg), np.ones_like(sg), np.ones_like(sg))
+    N = L**3
+    assert o.overlap(0, 0) == N and o.overlap(0, 3) == -N
+    for a in range(ns):
+        for b in range(ns):
+            assert o.overlap(a, b) == o.overlap(b, a) == int(np.dot(sg[a].astype(np.int64), sg[b].astype(np.int64)))
