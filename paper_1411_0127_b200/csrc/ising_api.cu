@@ -225,7 +225,15 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 if (rc != ISING_OK) return rc;
                 break;
             }
-            launch_pdl(half_sweep_sample_packed<2, 1>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
+            if (nb > 1 && nb <= 65535 && h->kernel_choice != 1) {  // all coded batches in one launch (a is batch 0, b == 0)
+                launch_pdl(half_sweep_sample_packed<2, 1, true>, dim3((unsigned)((ngroups + 127) / 128), (unsigned)nb), dim3(128), st, a, r,
+                           (uint32_t)ngroups, (uint64_t)g.N, (size_t)(8 * g.array_words));
+                const int rc = check_launch(h);
+                if (rc != ISING_OK) return rc;
+                break;
+            }
+            launch_pdl(half_sweep_sample_packed<2, 1, false>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups,
+                       (uint64_t)g.N, (size_t)0);
         } else if (g.nsamples != 1) {
             const uint64_t ngroups = g.Hc / 4;
             // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs
@@ -233,7 +241,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                 const uint32_t gpr = (uint32_t)g.L / 8, inv = (uint32_t)((0x100000000ull + gpr - 1) / gpr);
                 const uint64_t per_plane = (uint64_t)g.L * gpr;
                 const size_t bstride = (size_t)(8 * g.array_words);
-                if (nb > 1) {  // all coded batches in one launch (a is batch 0 here, b == 0)
+                if (nb > 1 && nb <= 65535) {  // all coded batches in one launch (a is batch 0 here, b == 0)
                     if (ngroups * (uint64_t)nb < 148u * 1024u)
                         launch_pdl(half_sweep_sample_packed_vec<RNG, 4, true>, dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L, (unsigned)nb), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
                     else
@@ -246,10 +254,19 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                     launch_pdl(half_sweep_sample_packed_vec<RNG, 4, false>, dim3((unsigned)((per_plane + 31) / 32), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
                 else
                     launch_pdl(half_sweep_sample_packed_vec<RNG, 1, false>, dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L), dim3(128), st, a, r, gpr, inv, (uint64_t)g.N, bstride);
+            } else if (nb > 1 && nb <= 65535 && h->kernel_choice != 1) {  // any even L, all coded batches in one launch
+                const size_t bstride = (size_t)(8 * g.array_words);
+                if (ngroups * (uint64_t)nb < 148u * 1024u)
+                    launch_pdl(half_sweep_sample_packed<RNG, 4, true>, dim3((unsigned)((ngroups + 31) / 32), (unsigned)nb), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N, bstride);
+                else
+                    launch_pdl(half_sweep_sample_packed<RNG, 1, true>, dim3((unsigned)((ngroups + 127) / 128), (unsigned)nb), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N, bstride);
+                const int rc = check_launch(h);
+                if (rc != ISING_OK) return rc;
+                break;
             } else if (ngroups < 148u * 1024u)
-                launch_pdl(half_sweep_sample_packed<RNG, 4>, dim3((unsigned)((ngroups + 31) / 32)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
+                launch_pdl(half_sweep_sample_packed<RNG, 4, false>, dim3((unsigned)((ngroups + 31) / 32)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N, (size_t)0);
             else
-                launch_pdl(half_sweep_sample_packed<RNG, 1>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N);
+                launch_pdl(half_sweep_sample_packed<RNG, 1, false>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups, (uint64_t)g.N, (size_t)0);
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = g.W;

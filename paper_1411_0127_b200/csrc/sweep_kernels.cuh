@@ -615,11 +615,21 @@ __device__ __forceinline__ void group_sums_any_L(const SweepArgs &a, uint32_t g,
     }
 }
 
-template <int RNG, int PARTS>
+// MULTI: all coded batches in one launch (blockIdx.y = batch, arrays batch_stride words apart, plain Philox rounds keyed per
+// sample or, for the shared draw, per batch), as in half_sweep_sample_packed_vec.
+template <int RNG, int PARTS, bool MULTI>
 __global__ void __launch_bounds__(128)
-half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_groups, uint64_t N)
+half_sweep_sample_packed(SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t n_groups, uint64_t N, size_t batch_stride)
 {
     constexpr int SPT = 32 / PARTS;  // samples per thread
+    const uint32_t sample0 = MULTI ? 32u * blockIdx.y : rng.sample_base;
+    if (MULTI) {
+        const size_t off = (size_t)blockIdx.y * batch_stride;
+        a.S_act += off;
+        a.S_oth += off;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { a.J_act[d] += off; a.J_oth[d] += off; }
+    }
     const int part = PARTS == 1 ? 0 : (int)(threadIdx.x >> 5);  // warp-uniform
     const uint32_t g_raw = PARTS == 1 ? blockIdx.x * 128u + threadIdx.x : blockIdx.x * 32u + (threadIdx.x & 31u);
     const bool valid = g_raw < n_groups;
@@ -632,7 +642,8 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
     uint32_t c4[4] = {0, 0, 0, 0}, c8[4] = {0, 0, 0, 0}, c12[4] = {0, 0, 0, 0};
     if (RNG == 2) {  // shared draw: Eq. 15 verbatim, the cond words are all ones or zero
         uint32_t R[4];
-        philox_folded(rng.pc, rng.ps[0], g, R);
+        if (MULTI) philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ blockIdx.y, R);   // R18: key field = batch
+        else philox_folded(rng.pc, rng.ps[0], g, R);
         shared_cond_words(R, a.T, c4, c8, c12);
     }
     // PARTS = 1: a rolled loop over the 16 sample pairs (the unrolled body of 32 calls is 40 KB of code that every warp
@@ -642,13 +653,16 @@ half_sweep_sample_packed(const SweepArgs a, const __grid_constant__ RngLaunch rn
     for (int i = 0; i < SPT && RNG != 2; i += 2) {
         const int b = SPT * part + i;
         uint32_t R[8];
-        if (RNG == 0) {
+        if (RNG == 0 && MULTI) {
+            philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ (sample0 + (uint32_t)b), R);
+            philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ (sample0 + (uint32_t)b + 1u), R + 4);
+        } else if (RNG == 0) {
             philox_folded(rng.pc, rng.ps[b], g, R);
             philox_folded(rng.pc, rng.ps[b + 1], g, R + 4);
         } else {
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const uint64_t qs = (uint64_t)(rng.sample_base + b + e) * N;
+                const uint64_t qs = (uint64_t)(sample0 + b + e) * N;
 #pragma unroll
                 for (int w = 0; w < 4; ++w)
                     R[4 * e + w] = minstd_mulmod(rng.A, minstd_seed_state_from_weyl(rng.seed + (qs + site[w] + 1) * SPLITMIX_GAMMA));

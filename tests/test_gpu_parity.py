@@ -165,7 +165,7 @@ def test_config2_L64_32_samples_philox():
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
-@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (10, 32), (16, 64), (8, 160), (24, 96), (64, 64), (10, 64)])
+@pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (10, 32), (16, 64), (8, 160), (24, 96), (64, 64), (10, 64), (6, 96), (12, 160)])
 def test_sample_packed_small(L, nsamples, rng_mode):
     spins, J = synth.make_spins(L, nsamples, 21), synth.make_couplings(L, nsamples, 8)
     o, g = make_pair(L, nsamples, rng_mode, spins, J)
@@ -314,7 +314,7 @@ def test_minstd_cached_seed_table_equals_recomputed_seeds(L):
 # ------------------------------------------------------------------------------------------------ shared-random-number mode
 
 @pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (8, 32), (8, 64), (12, 32), (16, 64), (24, 32), (40, 32), (64, 32),
-                                        (8, 320), (16, 160), (32, 96)])
+                                        (8, 320), (16, 160), (32, 96), (6, 64), (10, 160), (12, 96)])
 def test_shared_random_number_mode_equals_the_oracle(L, nsamples):
     """rng_mode 2 (R18): one Philox draw per 32-sample word.  The vectorised kernel (L % 8 == 0) and
     the generic sample-packed kernel (kernel choice 1, and every other L) against the oracle, trajectory and energies."""
