@@ -559,33 +559,33 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
         return check_launch(h, 8);
     }
     const unsigned grid = (unsigned)((g.Hc + 255) / 256);
+    if (!(g.L % 32 == 0 && h->kernel_choice != 1)) {  // one bit at a time, all batches / arrays / colours per launch (<= 8191 batches each)
+        for (int b0 = 0; b0 < g.nbatches; b0 += 8191) {
+            const int nbh = g.nbatches - b0 < 8191 ? g.nbatches - b0 : 8191;
+            gather_sample_packed_all<<<dim3(grid, (unsigned)(8 * nbh)), 256, 0, st>>>(d_spins, d_J, h->ws, (uint64_t)g.array_words, (uint64_t)W,
+                                                                                 g.L, g.Hc, (uint32_t)b0);
+            const int rc = check_launch(h);
+            if (rc != ISING_OK) return rc;
+        }
+        return ISING_OK;
+    }
     for (int b = 0; b < g.nbatches; ++b) {
         const LatticeArrays A = h->arrays(b);
         const uint32_t *sp = d_spins + (size_t)b * 32 * W;
         const uint32_t *jp = d_J + (size_t)b * 32 * 3 * W;
-        if (g.L % 32 == 0 && h->kernel_choice != 1) {  // tile kernel: one launch per batch, all four arrays, both colours
-            GatherTileArgs t;
-            t.canon[0] = sp;
-            t.stride[0] = W;
-            t.out[0][0] = A.S[0];
-            t.out[0][1] = A.S[1];
-            for (int d = 0; d < 3; ++d) {
-                t.canon[1 + d] = jp + (size_t)d * W;
-                t.stride[1 + d] = 3 * W;
-                t.out[1 + d][0] = A.J[d][0];
-                t.out[1 + d][1] = A.J[d][1];
-            }
-            gather_sample_packed_tiles<<<dim3((unsigned)((W + 127) / 128), 4), 128, 0, st>>>(t, g.L, (uint32_t)W);
-            const int rc = check_launch(h);
-            if (rc != ISING_OK) return rc;
-            continue;
+        GatherTileArgs t;   // tile kernel: one launch per batch, all four arrays, both colours
+        t.canon[0] = sp;
+        t.stride[0] = W;
+        t.out[0][0] = A.S[0];
+        t.out[0][1] = A.S[1];
+        for (int d = 0; d < 3; ++d) {
+            t.canon[1 + d] = jp + (size_t)d * W;
+            t.stride[1 + d] = 3 * W;
+            t.out[1 + d][0] = A.J[d][0];
+            t.out[1 + d][1] = A.J[d][1];
         }
-        for (int c = 0; c < 2; ++c) {
-            gather_sample_packed<<<grid, 256, 0, st>>>(sp, W, A.S[c], c, g.L, g.Hc);
-            for (int d = 0; d < 3; ++d)
-                gather_sample_packed<<<grid, 256, 0, st>>>(jp + (size_t)d * W, 3 * W, A.J[d][c], c, g.L, g.Hc);
-        }
-        const int rc = check_launch(h, 8);
+        gather_sample_packed_tiles<<<dim3((unsigned)((W + 127) / 128), 4), 128, 0, st>>>(t, g.L, (uint32_t)W);
+        const int rc = check_launch(h);
         if (rc != ISING_OK) return rc;
     }
     return ISING_OK;
@@ -619,8 +619,10 @@ int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
             if (rc != ISING_OK) return rc;
             continue;
         }
-        const dim3 grid((unsigned)((W + 255) / 256), 32);
-        scatter_sample_packed<<<grid, 256, 0, st>>>(A.S[0], A.S[1], d_out + (size_t)b * 32 * W, W, g.L, W, g.N);
+        const int nbh = g.nbatches - b < 65535 ? g.nbatches - b : 65535;   // all remaining batches in one launch (blockIdx.z)
+        const dim3 grid((unsigned)((W + 255) / 256), 32, (unsigned)nbh);
+        scatter_sample_packed<<<grid, 256, 0, st>>>(A.S[0], A.S[1], d_out + (size_t)b * 32 * W, W, g.L, W, g.N, (uint64_t)(8 * g.array_words));
+        b += nbh - 1;
         const int rc = check_launch(h);
         if (rc != ISING_OK) return rc;
     }

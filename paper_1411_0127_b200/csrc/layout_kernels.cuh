@@ -215,33 +215,43 @@ scatter_site_packed_rows(const uint32_t *__restrict__ S0, const uint32_t *__rest
     canon[cw] = out;
 }
 
-// Sample-packed: word j of the colour-c array of a batch collects bit i(j,c) of the 32 samples' canonical arrays.
-// canon points at the first sample of the batch; consecutive samples are `sample_stride` words apart.
+// Sample-packed, one bit at a time (any even L): word j of the colour-c array of a batch collects bit i(j,c) of the 32 samples'
+// canonical arrays, for all coded batches, the four bit arrays and both colours in one launch: blockIdx.y = 8 * batch + 2 * array + colour
+// (array 0 = spins, 1..3 = Jx, Jy, Jz).  ws = the internal arrays (8 per batch, array_words each, S[0], S[1], Jx[0], Jx[1], ...).
 __global__ void __launch_bounds__(256)
-gather_sample_packed(const uint32_t *__restrict__ canon, uint64_t sample_stride, uint32_t *__restrict__ out, int colour, int L,
-                     uint64_t Hc)
+gather_sample_packed_all(const uint32_t *__restrict__ d_spins, const uint32_t *__restrict__ d_J, uint32_t *__restrict__ ws,
+                         uint64_t array_words, uint64_t W, int L, uint64_t Hc, uint32_t batch0)
 {
     const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= Hc) return;
+    const uint32_t b = batch0 + blockIdx.y / 8u, arr = (blockIdx.y & 7u) >> 1, colour = blockIdx.y & 1u;
+    const uint32_t *__restrict__ canon = arr == 0 ? d_spins + (uint64_t)b * 32 * W : d_J + (uint64_t)b * 32 * 3 * W + (uint64_t)(arr - 1) * W;
+    const uint64_t sample_stride = arr == 0 ? W : 3 * W;
+    uint32_t *__restrict__ out = ws + ((uint64_t)b * 8 + 2 * arr + colour) * array_words;
     const int H = L >> 1;
     const int m = (int)(j % H);
     const uint64_t r = j / H;
-    const int x = 2 * m + (((int)(r % L) + (int)(r / L) + colour) & 1);
+    const int x = 2 * m + (((int)(r % L) + (int)(r / L) + (int)colour) & 1);
     const uint64_t i = (uint64_t)x + (uint64_t)L * r;
     uint32_t w = 0;
 #pragma unroll 8
-    for (int b = 0; b < 32; ++b) w |= ((canon[b * sample_stride + (i >> 5)] >> (i & 31)) & 1u) << b;
+    for (int s = 0; s < 32; ++s) w |= ((canon[s * sample_stride + (i >> 5)] >> (i & 31)) & 1u) << s;
     out[j] = w;
 }
 
 // Sample-packed -> canonical spins: one thread per canonical word of one sample.
+// blockIdx.z = coded batch: its colour arrays start batch_stride words after S0 / S1, its canonical words 32 * sample_stride
+// words after canon.
 __global__ void __launch_bounds__(256)
 scatter_sample_packed(const uint32_t *__restrict__ S0, const uint32_t *__restrict__ S1, uint32_t *__restrict__ canon,
-                      uint64_t sample_stride, int L, uint64_t n_canon_words, uint64_t N)
+                      uint64_t sample_stride, int L, uint64_t n_canon_words, uint64_t N, uint64_t batch_stride)
 {
     const uint64_t cw = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int sample = blockIdx.y;  // within the batch
     if (cw >= n_canon_words) return;
+    S0 += (uint64_t)blockIdx.z * batch_stride;
+    S1 += (uint64_t)blockIdx.z * batch_stride;
+    canon += (uint64_t)blockIdx.z * 32 * sample_stride;
     uint32_t w = 0;
     for (int b = 0; b < 32; ++b) {
         const uint64_t i = 32 * cw + b;
