@@ -187,8 +187,29 @@ void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st
     cudaLaunchKernelEx(&cfg, kernel, args...);  // errors surface through cudaGetLastError in check_launch
 }
 
+// The word-parallel kernel for W words per thread, plain or with E and M of the resulting configuration (MEASURE).
+template <int RNG, int W>
+void launch_site_packed_w(bool measure, dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, unsigned long long *slots,
+                          long long N, long long *mE, long long *mM)
+{
+    if (measure) launch_pdl(half_sweep_site_packed<RNG, W, true>, grid, dim3(SWEEP_THREADS), st, a, sr, slots, N, mE, mM);
+    else launch_pdl(half_sweep_site_packed<RNG, W, false>, grid, dim3(SWEEP_THREADS), st, a, sr, (unsigned long long *)nullptr, 0ll,
+                    (long long *)nullptr, (long long *)nullptr);
+}
 template <int RNG>
-int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
+void launch_site_packed(int W, bool measure, dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, unsigned long long *slots,
+                        long long N, long long *mE, long long *mM)
+{
+    if (W == 4) launch_site_packed_w<RNG, 4>(measure, grid, st, a, sr, slots, N, mE, mM);
+    else if (W == 3) launch_site_packed_w<RNG, 3>(measure, grid, st, a, sr, slots, N, mE, mM);
+    else if (W == 5) launch_site_packed_w<RNG, 5>(measure, grid, st, a, sr, slots, N, mE, mM);
+    else launch_site_packed_w<RNG, 1>(measure, grid, st, a, sr, slots, N, mE, mM);
+}
+
+// mE / mM (device, may be null): where the half-sweep itself writes E and M of the configuration it leaves; honoured by the
+// word-parallel site-packed kernel only (see can_measure_in_sweep), ignored elsewhere.
+template <int RNG>
+int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long long *mE = nullptr, long long *mM = nullptr)
 {
     const Geometry &g = h->g;
     const int c = (int)(h->t & 1);
@@ -270,6 +291,11 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = g.W;
+            unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;   // ACC_SLOTS counter pairs + ticket (measure())
+            if ((mE || mM) && !h->slots_clean) {
+                if (cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
+                h->slots_clean = true;
+            }
             const int tpr_pad = row_map_tpr_pad(wpr / W);
             const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
             SiteRng sr;
@@ -293,14 +319,10 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
                     h->s0_ready = true;
                 }
                 sr.s0tab = tab[c];
-                if (W == 4) launch_pdl(half_sweep_site_packed<2, 4>, grid, dim3(SWEEP_THREADS), st, a, sr);
-                else if (W == 3) launch_pdl(half_sweep_site_packed<2, 3>, grid, dim3(SWEEP_THREADS), st, a, sr);
-                else if (W == 5) launch_pdl(half_sweep_site_packed<2, 5>, grid, dim3(SWEEP_THREADS), st, a, sr);
-                else launch_pdl(half_sweep_site_packed<2, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
-            } else if (W == 4) launch_pdl(half_sweep_site_packed<RNG, 4>, grid, dim3(SWEEP_THREADS), st, a, sr);
-            else if (W == 3) launch_pdl(half_sweep_site_packed<RNG, 3>, grid, dim3(SWEEP_THREADS), st, a, sr);
-            else if (W == 5) launch_pdl(half_sweep_site_packed<RNG, 5>, grid, dim3(SWEEP_THREADS), st, a, sr);
-            else launch_pdl(half_sweep_site_packed<RNG, 1>, grid, dim3(SWEEP_THREADS), st, a, sr);
+                launch_site_packed<2>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
+            } else {
+                launch_site_packed<RNG>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
+            }
         } else if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {  // any even L: the word update on operands gathered as bit windows
             const uint64_t nw = (g.Hc + 31) / 32;
             SiteRng sr;   // the small per-launch constant block (the 1.4 KB RngLaunch doubles the enqueue cost of a tiny launch)
@@ -367,12 +389,18 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
     return ISING_OK;
 }
 
-int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st)
+// Can the half-sweep kernel of this handle return E and M itself (half_sweep_site_packed<.., MEASURE = true>)?
+bool can_measure_in_sweep(const ising_t *h)
+{
+    return h->g.nsamples == 1 && h->g.fast && h->kernel_choice != 1 && (h->rng_mode == ISING_RNG_PHILOX || h->rng_mode == ISING_RNG_MINSTD);
+}
+
+int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long long *mE = nullptr, long long *mM = nullptr)
 {
     if (h->rng_mode == ISING_RNG_PR_SHARED) return launch_half_sweep_lanes<GEN_PR>(h, T, st);
     if (h->rng_mode == ISING_RNG_MT19937_SHARED) return launch_half_sweep_lanes<GEN_MT>(h, T, st);
     if (h->rng_mode == ISING_RNG_PHILOX_SHARED) return launch_half_sweep<2>(h, T, st);
-    return h->rng_mode == ISING_RNG_PHILOX ? launch_half_sweep<0>(h, T, st) : launch_half_sweep<1>(h, T, st);
+    return h->rng_mode == ISING_RNG_PHILOX ? launch_half_sweep<0>(h, T, st, mE, mM) : launch_half_sweep<1>(h, T, st, mE, mM);
 }
 
 int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
@@ -644,13 +672,18 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
     const Thresholds kt = kernel_thresholds(T);
     cudaStream_t st = (cudaStream_t)stream;
     size_t rec = 0;
+    const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps write E and M themselves: no extra launch
     for (int k = 1; k <= 2 * nsweeps; ++k) {
-        int rc = half_sweep(h, kt, st);
+        const bool record = trace && k % every_half_sweeps == 0;
+        long long *rE = record && d_E ? (long long *)d_E + rec * h->g.nsamples : nullptr;
+        long long *rM = record && d_M ? (long long *)d_M + rec * h->g.nsamples : nullptr;
+        int rc = fused && record ? half_sweep(h, kt, st, rE, rM) : half_sweep(h, kt, st);
         if (rc != ISING_OK) return rc;
-        if (trace && k % every_half_sweeps == 0) {
-            rc = measure(h, d_E ? (long long *)d_E + rec * h->g.nsamples : nullptr,
-                         d_M ? (long long *)d_M + rec * h->g.nsamples : nullptr, st);
-            if (rc != ISING_OK) return rc;
+        if (record) {
+            if (!fused) {
+                rc = measure(h, rE, rM, st);
+                if (rc != ISING_OK) return rc;
+            }
             ++rec;
         }
     }

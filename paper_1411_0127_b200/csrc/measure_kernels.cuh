@@ -15,44 +15,11 @@
 
 namespace isingk {
 
-// The word-parallel site-packed kernel spreads its per-CTA atomics over ACC_SLOTS counter pairs (one address would
-// serialise 16384 atomics in L2 at L = 1024); the last CTA adds them up.
-constexpr int ACC_SLOTS = 64;
-
 struct MeasureArgs {
     const uint32_t *S[2];
     const uint32_t *J[3][2];
     int L;
 };
-
-__device__ __forceinline__ void warp_reduce_add2(unsigned long long &a, unsigned long long &b)
-{
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        a += __shfl_down_sync(0xFFFFFFFFu, a, off);
-        b += __shfl_down_sync(0xFFFFFFFFu, b, off);
-    }
-}
-
-// Block-level sum of two counters, then one atomic pair per block.
-__device__ __forceinline__ void block_accumulate2(unsigned long long a, unsigned long long b, unsigned long long *acc)
-{
-    __shared__ unsigned long long sh[2][32];
-    warp_reduce_add2(a, b);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (lane == 0) { sh[0][warp] = a; sh[1][warp] = b; }
-    __syncthreads();
-    if (warp == 0) {
-        const int nw = (blockDim.x + 31) >> 5;
-        a = lane < nw ? sh[0][lane] : 0;
-        b = lane < nw ? sh[1][lane] : 0;
-        warp_reduce_add2(a, b);
-        if (lane == 0) {
-            atomicAdd(&acc[0], a);
-            atomicAdd(&acc[1], b);
-        }
-    }
-}
 
 // Site-packed, L a multiple of 64: the thread mapping of the half-sweep kernel (a thread owns W consecutive words of a half-row,
 // for both colours).  The +x neighbour of the colour-c site with bit m is bit m (xodd = 0) or bit m+1 (xodd = 1) of the
@@ -100,26 +67,7 @@ energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {
         }
     }
     block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
-    __shared__ bool is_last;
-    unsigned int *ticket = reinterpret_cast<unsigned int *>(acc + 2 * ACC_SLOTS);
-    if (threadIdx.x == 0) {
-        __threadfence();
-        is_last = atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1;  // every other CTA's atomics are visible then
-    }
-    __syncthreads();
-    if (is_last && threadIdx.x < 32) {  // warp 0 of the last CTA: read-and-clear the slots, two per lane
-        unsigned long long tu = 0, tp = 0;
-        for (int k = threadIdx.x; k < ACC_SLOTS; k += 32) {
-            tu += atomicExch(&acc[2 * k], 0ull);
-            tp += atomicExch(&acc[2 * k + 1], 0ull);
-        }
-        warp_reduce_add2(tu, tp);
-        if (threadIdx.x == 0) {
-            if (E) E[0] = 2 * (long long)tu - 3 * N;
-            if (M) M[0] = 2 * (long long)tp - N;
-            *ticket = 0u;
-        }
-    }
+    finalize_slots_last_cta(acc, N, E, M);
 }
 
 // Site-packed, any even L: one thread per word, one site at a time.

@@ -59,6 +59,66 @@ struct SweepArgs {
 // execute as few other instructions as possible: the 12 operand vectors are loaded first, the field sums of all W
 // words are reduced to three bit planes each (22 logic ops per 32 sites), and only then the random numbers are drawn.
 // ---------------------------------------------------------------------------------------------------
+// The word-parallel site-packed kernel spreads its per-CTA atomics over ACC_SLOTS counter pairs (one address would
+// serialise 16384 atomics in L2 at L = 1024); the last CTA adds them up.
+constexpr int ACC_SLOTS = 64;
+
+__device__ __forceinline__ void warp_reduce_add2(unsigned long long &a, unsigned long long &b)
+{
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        a += __shfl_down_sync(0xFFFFFFFFu, a, off);
+        b += __shfl_down_sync(0xFFFFFFFFu, b, off);
+    }
+}
+
+// Block-level sum of two counters, then one atomic pair per block.
+__device__ __forceinline__ void block_accumulate2(unsigned long long a, unsigned long long b, unsigned long long *acc)
+{
+    __shared__ unsigned long long sh[2][32];
+    warp_reduce_add2(a, b);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { sh[0][warp] = a; sh[1][warp] = b; }
+    __syncthreads();
+    if (warp == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        a = lane < nw ? sh[0][lane] : 0;
+        b = lane < nw ? sh[1][lane] : 0;
+        warp_reduce_add2(a, b);
+        if (lane == 0) {
+            atomicAdd(&acc[0], a);
+            atomicAdd(&acc[1], b);
+        }
+    }
+}
+
+// Last-CTA finalisation shared by energy_site_packed and the measuring half-sweep: the CTAs have added their counts to the
+// slots; the last one to finish (ticket counter behind the slots) sums them, writes E = 2 * unsatisfied - 3N and
+// M = 2 * up - N (R16) and clears slots and ticket for the next call.
+__device__ __forceinline__ void finalize_slots_last_cta(unsigned long long *acc, long long N, long long *E, long long *M)
+{
+    __shared__ bool is_last;
+    unsigned int *ticket = reinterpret_cast<unsigned int *>(acc + 2 * ACC_SLOTS);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        is_last = atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1;  // every other CTA's atomics are visible then
+    }
+    __syncthreads();
+    if (is_last && threadIdx.x < 32) {  // warp 0 of the last CTA: read-and-clear the slots, two per lane
+        unsigned long long tu = 0, tp = 0;
+        for (int k = threadIdx.x; k < ACC_SLOTS; k += 32) {
+            tu += atomicExch(&acc[2 * k], 0ull);
+            tp += atomicExch(&acc[2 * k + 1], 0ull);
+        }
+        warp_reduce_add2(tu, tp);
+        if (threadIdx.x == 0) {
+            if (E) E[0] = 2 * (long long)tu - 3 * N;
+            if (M) M[0] = 2 * (long long)tp - N;
+            *ticket = 0u;
+        }
+    }
+}
+
 template <int W> struct WordVec;
 template <> struct WordVec<1> { typedef uint32_t type; };
 template <> struct WordVec<2> { typedef uint2 type; };
@@ -181,9 +241,16 @@ __device__ __forceinline__ RowMap row_map(int L)
     return m;
 }
 
-template <int RNG, int W>
+// MEASURE: the half-sweep also returns E and M of the configuration it leaves (row a9 fused into rows a2-a8).  Every bond has
+// exactly one end in the active colour, so the number of satisfied bonds of the whole lattice is the sum over the active
+// sites of their count n (already in the three bit planes), with n -> 6 - n where the site flipped; the up spins are those of
+// the new active words plus the other colour's words of the same rows, which are loaded anyway.  About 15 popcounts per
+// word, then the slot accumulation and last-CTA finalisation of energy_site_packed: a trace of E and M per sweep costs no
+// extra launch and no extra pass over the 512 MiB (L = 1024: 78 us per record saved).
+template <int RNG, int W, bool MEASURE>
 __global__ void __launch_bounds__(SWEEP_THREADS)
-half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng)
+half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, unsigned long long *acc, long long N,
+                       long long *E, long long *M)
 {
     const int L = a.L;
     const int wpr = L >> 6;                 // words per half-row
@@ -199,6 +266,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     const uint32_t row_zm = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zm) + k0;
 
     uint32_t s[W], sum2[W], sum1[W], sum0[W];
+    unsigned int m_sat = 0, m_up = 0;   // MEASURE: satisfied bonds of this thread's sites, up spins of both colours
     const int xodd = (y + z + a.colour) & 1;
     wait_for_previous_kernel();
     {
@@ -236,8 +304,15 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
             const uint32_t nb[6] = {__funnelshift_r(o[k], o_next, sh_r), __funnelshift_l(B_prev, B[k], sh_l), oyp[k], oym[k], ozp[k],
                                     ozm[k]};
             satisfied_bond_count(s[k], J, nb, sum2[k], sum1[k], sum0[k]);
+            if (MEASURE) m_up += __popc(o[k]);
         }
     }
+    // after the flips f of a word: sum of n' = sum of n + 6 popc(f) - 2 (sum of n over the flipped bits)
+    auto measure_word = [&](int k, uint32_t f) {
+        m_sat += __popc(sum0[k]) + 2 * __popc(sum1[k]) + 4 * __popc(sum2[k]) + 6 * __popc(f);
+        m_sat -= 2 * (__popc(sum0[k] & f) + 2 * __popc(sum1[k] & f) + 4 * __popc(sum2[k] & f));
+        m_up += __popc(s[k]);
+    };
 
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
     if (RNG == 2) {
@@ -265,7 +340,9 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
             }
             if (half) {
                 finish_cond(a.T, c4, c8, c12);
-                s[k] ^= flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
+                const uint32_t f = flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
+                s[k] ^= f;
+                if (MEASURE) measure_word(k, f);
                 c4 = 0; c8 = 0; c12 = 0;
             }
 #pragma unroll
@@ -296,10 +373,18 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
             const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
             cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
         }
-        s[k] ^= flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
+        const uint32_t f = flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
+        s[k] ^= f;
+        if (MEASURE) measure_word(k, f);
     }
 
     if (rm.active) store_words<W>(a.S_act, row, s);
+    if (MEASURE) {
+        // unsatisfied bonds = 6 per active site - satisfied; idle lanes of a padded row shadow lane 0 and count nothing
+        const unsigned long long unsat = rm.active ? 192ull * W - m_sat : 0ull, up = rm.active ? m_up : 0ull;
+        block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
+        finalize_slots_last_cta(acc, N, E, M);
+    }
 }
 
 // Fills the seed table of colour `colour` with the thread mapping of half_sweep_site_packed<2, W> (same grid).

@@ -646,3 +646,34 @@ def test_overlap_of_replicas_equals_the_oracle(L, nsamples):
         g.ising_overlap(0, nsamples)
     with pytest.raises(binding.IsingError):
         Ising(64, 1, SEED, PHILOX).ising_overlap(0, 0)
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L", [64, 128, 192, 256, 320, 448])
+def test_energy_measured_inside_the_half_sweep_kernel(L, rng_mode):
+    """Trace records of the word-parallel layout come from the half-sweep kernel itself (MEASURE variant: satisfied bonds from
+    the field bit planes, n -> 6 - n where the site flipped).  E and M after every half-sweep (red and blue records) against the
+    one-site-at-a-time kernels with their separate energy kernel, for 1, 3, 4, 5 words per thread and a padded row (L = 448);
+    E-only and M-only traces; the oracle at the smaller sizes."""
+    spins, J = synth.make_spins(L, 1, 91), synth.make_couplings(L, 1, 92)
+    g = Ising(L, 1, SEED, rng_mode)
+    g.ising_load_state(dev(spins), dev(J))
+    r = Ising(L, 1, SEED, rng_mode)
+    r.ising_set_kernel(1)
+    r.ising_load_state(dev(spins), dev(J))
+    E, M = g.ising_sweep_trace(0.8, 3, every_half_sweeps=1)
+    Er, Mr = r.ising_sweep_trace(0.8, 3, every_half_sweeps=1)
+    assert torch.equal(E, Er) and torch.equal(M, Mr)
+    assert torch.equal(g.ising_get_spins(), r.ising_get_spins())
+    E2, none = g.ising_sweep_trace(0.8, 1, every_half_sweeps=2, want_M=False)      # E only, and the slots stay clean
+    Er2, Mr2 = r.ising_sweep_trace(0.8, 1, every_half_sweeps=2)
+    assert none is None and torch.equal(E2, Er2)
+    Eg, Mg = g.ising_energy()                                                        # the separate energy kernel agrees
+    assert int(Eg[0]) == int(Er2[-1, 0]) and int(Mg[0]) == int(Mr2[-1, 0])
+    if L <= 128:
+        o = ea3d.Oracle(L, 1, SEED, rng_mode)
+        o.load_packed(spins, J)
+        for k in range(6):
+            o.half_sweep(0.8)
+            Eo, Mo = o.energy()
+            assert (int(E[k, 0]), int(M[k, 0])) == (int(Eo[0]), int(Mo[0])), k
