@@ -76,9 +76,10 @@ typedef struct ising ising_t; /* opaque */
 /* Size in bytes of the device workspace ising_create needs for (L, nsamples, rng_mode): the internal spin and
  * coupling arrays (8 bit arrays per lattice), a canonical staging area used by
  * ising_run_host, the int64 accumulators of the measurement kernel and, in MINSTD mode with nsamples = 1 and
- * L a multiple of 64, a table of the per-site seed states s0 (4 bytes per site, R11).  No PRNG *state* is stored: both
- * generators are evaluated statelessly from (seed, sample, site, t) (R9, R12); the table only caches the
- * time-independent SplitMix64 seeding of the MINSTD streams and is filled by the first sweep call. */
+ * L a multiple of 64, a table of the per-site seed states s0 (4 bytes per site, R11).  In modes 0-2 no PRNG *state* is stored:
+ * both generators are evaluated statelessly from (seed, sample, site, t) (R9, R12); the table only caches the
+ * time-independent SplitMix64 seeding of the MINSTD streams and is filled by the first sweep call.  The lane modes 3, 4 add
+ * the strided generator state (62 or 624 words per lane, R19), seeded by the first sweep call. */
 int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out);
 
 /* Create a handle.  d_workspace: device memory, >= ising_workspace_bytes, 256-byte aligned.  The lattice
@@ -98,7 +99,9 @@ int ising_sweep(ising_t *h, double beta, int nsweeps, void *stream);
 
 /* As ising_sweep, and after every `every_half_sweeps`-th half-sweep of this call (counted from 1) writes the
  * energy (and magnetisation if d_M != NULL) of every sample to record r = 0,1,...:
- * d_E[r*nsamples + s].  d_E / d_M must hold (2*nsweeps / every_half_sweeps) * nsamples int64. */
+ * d_E[r*nsamples + s].  d_E / d_M must hold (2*nsweeps / every_half_sweeps) * nsamples int64.  (With nsamples = 1 and L a
+ * multiple of 64 the recording half-sweeps compute E and M themselves, from the field sums they already hold; otherwise a record
+ * is one launch of the energy kernel.) */
 int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_t *d_M, int every_half_sweeps,
                       void *stream);
 
