@@ -269,8 +269,10 @@ energy_sample_packed_sliced(const __grid_constant__ MeasureArgs a, size_t batch_
     acc += 64u * blockIdx.y;
     wait_for_previous_kernel();
     if (chunk < 2u * chunks_per_colour) {   // warp-uniform
-        const int c = chunk >= chunks_per_colour;
-        uint32_t j = (chunk - (c ? chunks_per_colour : 0u)) * (256u * (uint32_t)nblocks) + (uint32_t)lane;
+        // neighbouring warps take the two colours of the same stretch of ranks: the spin words one colour reads as neighbours
+        // are the other's own words and meet in the L2 (colour-major order read both spin arrays twice from HBM)
+        const int c = chunk & 1u;
+        uint32_t j = (chunk >> 1) * (256u * (uint32_t)nblocks) + (uint32_t)lane;
         uint32_t m = j % H, r = j / H, y = r % L, z = r / L;
         const uint32_t *__restrict__ S = a.S[c] + boff, *__restrict__ So = a.S[1 - c] + boff;
         const uint32_t *__restrict__ Jx = a.J[0][c] + boff, *__restrict__ Jy = a.J[1][c] + boff, *__restrict__ Jz = a.J[2][c] + boff;
