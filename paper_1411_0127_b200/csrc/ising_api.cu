@@ -376,11 +376,16 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
     ln.nlanes = h->nlanes;
     ln.pos0 = (uint32_t)((h->t % LaneRing<GEN>::size) * (per_half_sweep % LaneRing<GEN>::size) % LaneRing<GEN>::size);
     if (g.L % 8 == 0) {
-        const uint32_t gpr = (uint32_t)g.L / 8;
-        launch_pdl(half_sweep_shared_lanes<GEN, true>, dim3(blocks), dim3(128), st, a, ln, gpr, (uint32_t)((0x100000000ull + gpr - 1) / gpr),
-                   (size_t)(8 * g.array_words), ngroups, units, rounds);
+        const uint32_t gpr = (uint32_t)g.L / 8, gpr_inv = (uint32_t)((0x100000000ull + gpr - 1) / gpr);
+        // lattices beyond the L2 (126 MB): stream the read-once arrays past it (lane_rng.cuh)
+        if (g.arrays_total_words * sizeof(uint32_t) > (96u << 20))
+            launch_pdl(half_sweep_shared_lanes<GEN, true, true>, dim3(blocks), dim3(128), st, a, ln, gpr, gpr_inv, (size_t)(8 * g.array_words),
+                       ngroups, units, rounds);
+        else
+            launch_pdl(half_sweep_shared_lanes<GEN, true, false>, dim3(blocks), dim3(128), st, a, ln, gpr, gpr_inv, (size_t)(8 * g.array_words),
+                       ngroups, units, rounds);
     } else {  // groups that straddle rows: per-word neighbour loads
-        launch_pdl(half_sweep_shared_lanes<GEN, false>, dim3(blocks), dim3(128), st, a, ln, 1u, 0u, (size_t)(8 * g.array_words), ngroups,
+        launch_pdl(half_sweep_shared_lanes<GEN, false, false>, dim3(blocks), dim3(128), st, a, ln, 1u, 0u, (size_t)(8 * g.array_words), ngroups,
                    units, rounds);
     }
     const int rc = check_launch(h);

@@ -143,7 +143,11 @@ __global__ void __launch_bounds__(128) lanes_init(uint32_t *state, uint32_t nlan
 // registers and was slower: 0.249 against 0.239 ps/flip.)
 // ---------------------------------------------------------------------------------------------------
 // VEC = false (L % 8 != 0): a group may straddle rows, its sums come from group_sums_any_L (one load per word).
-template <int GEN, bool VEC>
+// STREAM (host: lattices larger than the L2): the couplings and the active spins, read once per half-sweep, are loaded
+// evict-first so that they do not push the generator state and the other colour's spins out of the L2 -- Parisi-Rapuano
+// at L = 512 x 32 samples: 0.231 -> 0.212 ps/flip; on lattices that fit the L2 the same hint costs 10-20 % (their couplings
+// would have stayed resident), hence the switch.
+template <int GEN, bool VEC, bool STREAM>
 __global__ void __launch_bounds__(128, 8)
 half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uint32_t gpr_inv, size_t batch_stride,
                         uint32_t ngroups, uint64_t units, uint32_t rounds)
@@ -171,7 +175,7 @@ half_sweep_shared_lanes(const SweepArgs a0, const LaneArgs ln, uint32_t gpr, uin
         if (VEC) {
             const uint32_t z = g / per_plane, p = g - z * per_plane;
             uint64_t site0;
-            vec_group_sums(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
+            vec_group_sums<STREAM>(a, gpr, gpr_inv, p, z, j0, site0, s, sum2, sum1, sum0);
         } else {
             uint64_t site[4];
             j0 = 4u * g;

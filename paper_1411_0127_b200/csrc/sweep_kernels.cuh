@@ -148,6 +148,14 @@ __device__ __forceinline__ void load_words(const uint32_t *__restrict__ p, size_
     }
 }
 
+// 128-bit load of words that are read exactly once per half-sweep (couplings, the active spins): ld.global.cs, evict-first,
+// so that they do not displace what is re-read (the other colour's spins, the lane generators' state) from the L2.
+__device__ __forceinline__ void load_words4_streaming(const uint32_t *__restrict__ p, size_t word_off, uint32_t out[4])
+{
+    const uint4 v = __ldcs(reinterpret_cast<const uint4 *>(p + word_off));
+    out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w;
+}
+
 template <int W>
 __device__ __forceinline__ void store_words(uint32_t *p, size_t word_off, const uint32_t in[W])
 {
@@ -784,6 +792,7 @@ half_sweep_sample_packed(SweepArgs a, const __grid_constant__ RngLaunch rng, uin
 // L/2 is a multiple of 4 and a group never leaves its row): own spins and couplings, the y+-1 / z+-1 neighbours and their
 // couplings are 128-bit loads; the two x-neighbours are the same four words of the other colour shifted by one word
 // (one extra 32-bit load each for spins and couplings).  p = index of the group within the plane z (y = p / gpr).
+template <bool STREAM = false>
 __device__ __forceinline__ void vec_group_sums(const SweepArgs &a, uint32_t gpr, uint32_t gpr_inv, uint32_t p, uint32_t z,
                                                uint32_t &j0, uint64_t &site0, uint32_t s[4], uint32_t sum2[4], uint32_t sum1[4],
                                                uint32_t sum0[4])
@@ -803,20 +812,34 @@ __device__ __forceinline__ void vec_group_sums(const SweepArgs &a, uint32_t gpr,
 
     uint32_t o[4], oyp[4], oym[4], ozp[4], ozm[4], jxa[4], jya[4], jza[4], jxo[4], jyo[4], jzo[4];
     wait_for_previous_kernel();
-    load_words<4>(a.S_act, j0, s);
-    load_words<4>(a.S_oth, j0, o);
-    load_words<4>(a.J_oth[0], j0, jxo);
+    if (STREAM) {
+        load_words4_streaming(a.S_act, j0, s);
+        load_words<4>(a.S_oth, j0, o);
+        load_words4_streaming(a.J_oth[0], j0, jxo);
+    } else {
+        load_words<4>(a.S_act, j0, s);
+        load_words<4>(a.S_oth, j0, o);
+        load_words<4>(a.J_oth[0], j0, jxo);
+    }
     const uint32_t o_extra = __ldg(a.S_oth + rowbase + m_extra);
     const uint32_t jxo_extra = __ldg(a.J_oth[0] + rowbase + m_extra);
-    load_words<4>(a.J_act[0], j0, jxa);
     load_words<4>(a.S_oth, jyp, oyp);
     load_words<4>(a.S_oth, jym, oym);
     load_words<4>(a.S_oth, jzp, ozp);
     load_words<4>(a.S_oth, jzm, ozm);
-    load_words<4>(a.J_act[1], j0, jya);
-    load_words<4>(a.J_act[2], j0, jza);
-    load_words<4>(a.J_oth[1], jym, jyo);
-    load_words<4>(a.J_oth[2], jzm, jzo);
+    if (STREAM) {
+        load_words4_streaming(a.J_act[0], j0, jxa);
+        load_words4_streaming(a.J_act[1], j0, jya);
+        load_words4_streaming(a.J_act[2], j0, jza);
+        load_words4_streaming(a.J_oth[1], jym, jyo);
+        load_words4_streaming(a.J_oth[2], jzm, jzo);
+    } else {
+        load_words<4>(a.J_act[0], j0, jxa);
+        load_words<4>(a.J_act[1], j0, jya);
+        load_words<4>(a.J_act[2], j0, jza);
+        load_words<4>(a.J_oth[1], jym, jyo);
+        load_words<4>(a.J_oth[2], jzm, jzo);
+    }
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
         // xodd = 0: +x is word m (own coupling), -x is word m-1 with that neighbour's coupling;
