@@ -232,3 +232,17 @@ def test_lane_kernels_write_only_inside_their_buffers(mode, L, ns, nlanes):
     torch.cuda.synchronize()
     assert bool((st[:G] == 0xA5).all()) and bool((st[G + sb:] == 0xA5).all()), "state guard overwritten"
     assert bool((res[:1024] == 0x5A5A5A5A5A5A5A5A).all()) and bool((res[1024 + 2 * n:] == 0x5A5A5A5A5A5A5A5A).all()), "result guard"
+
+
+@pytest.mark.parametrize("mode", [PR_SHARED, MT19937_SHARED])
+def test_lane_mode_long_run(mode):
+    """200 half-sweeps in uneven calls: the ring position handed to every launch ((t mod ring) * (draws per half-sweep mod ring)
+    mod ring) must track the generators exactly; 332 draws per lane and half-sweep, 66400 in total (106 MT19937 blocks)."""
+    L, ns, nlanes = 16, 64, 13
+    spins, J = synth.make_spins(L, ns, 87), synth.make_couplings(L, ns, 88)
+    o, g = make_pair(L, ns, mode, nlanes, spins, J)
+    for n in (1, 7, 30, 62):
+        o.sweep(1 / 1.1, n)
+        g.ising_sweep(1 / 1.1, n)
+        assert_same_state(o, g, f"after {n} more sweeps")
+    assert g.ising_get_t() == 200
