@@ -312,7 +312,9 @@ def main():
 
     def bench_lanes():
         return {"sweep": [bench_shared(512, 32, 4, 3), bench_shared(512, 32, 4, 4), bench_shared(128, 256, 20, 3)],
-                "table2_device_api": [bench_table2(k) for k in (0, 1, 3, 4)]}
+                "table2_device_api": [bench_table2(k) for k in (0, 1, 3, 4)],
+                # the launch configuration of the paper's Table II: 64 blocks x 256 threads, 2^15 draws each, 10 times
+                "table2_paper_launch_configuration": [bench_table2(k, nlanes=64 * 256, ndraws=1 << 15, reps=10) for k in (0, 1, 3, 4)]}
 
     if args.scan:
         from paper_1411_0127_b200 import PHILOX_SHARED
