@@ -157,6 +157,8 @@ def main():
     ap.add_argument("--only-lanes", action="store_true", help="time only the stored-state lane generators (sweep and Table II)")
     ap.add_argument("--scan-batches", action="store_true",
                     help="the paper's Fig. 4 study: half-sweep time of small lattices against the number k of coded batches (shared draws)")
+    ap.add_argument("--configs", action="store_true",
+                    help="the five configurations of BASELINE.json at their full sweep counts, with the outputs each one asks for")
     ap.add_argument("--aux", action="store_true",
                     help="rows a9 / a10 and the general-L kernels: load_state, energy, get_spins and a half-sweep per layout, with GB/s")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
@@ -343,6 +345,53 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.configs:  # BASELINE.json configs 1-5 as written: sweeps, and the observables each one records, inside the timed region
+        from paper_1411_0127_b200 import binding
+
+        rows = []
+        for idx in (1, 2, 3, 4, 5):
+            cfg, sp_np, J_np = synth.make_config(idx)
+            Ls, ns, nsweeps, beta = cfg["L"], cfg["nsamples"], cfg["sweeps"], cfg["beta"]
+            sp = torch.from_numpy(sp_np.view(np.int32)).cuda()
+            Jc = torch.from_numpy(J_np.view(np.int32)).cuda()
+            g = Ising(Ls, ns, synth.DYN_SEED, cfg["rng_mode"])
+            out = torch.empty_like(sp)
+
+            def run():
+                g.ising_set_t(0)
+                g.ising_load_state(sp, Jc)
+                if idx == 1:      # final spins and energy per half-sweep
+                    E, _ = g.ising_sweep_trace(beta, nsweeps, every_half_sweeps=1, want_M=False)
+                    g.ising_get_spins(out)
+                    return int(E[-1, 0])
+                if idx == 2:      # energy per site every 10 sweeps
+                    E, _ = g.ising_sweep_trace(beta, nsweeps, every_half_sweeps=20, want_M=False)
+                    return int(E[-1, 0])
+                if idx == 3:      # energy and magnetisation per sweep
+                    E, M = g.ising_sweep_trace(beta, nsweeps, every_half_sweeps=2)
+                    return int(E[-1, 0])
+                if idx == 4:      # 64-bit FNV-1a of the packed spin words every 10 sweeps (host side of the C ABI)
+                    h = 0
+                    for _ in range(nsweeps // 10):
+                        g.ising_sweep(beta, 10)
+                        h = binding.ising_fnv1a64_host(g.ising_get_spins(out).cpu().numpy())
+                    return h
+                g.ising_sweep(beta, nsweeps)
+                E, _ = g.ising_energy()
+                return int(E[0])
+
+            run()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            result = run()
+            torch.cuda.synchronize()
+            wall = time.perf_counter() - t0
+            g.ising_destroy()
+            rows.append({"config": idx, "L": Ls, "nsamples": ns, "sweeps": nsweeps, "rng_mode": cfg["rng_mode"], "wall_ms": 1e3 * wall,
+                         "ps_per_flip_including_outputs": 1e12 * wall / (nsweeps * ns * Ls**3), "last_output": result})
+        print(json.dumps({"configs": rows}))
         return
 
     if args.aux:  # measurement of the rows outside the headline step: every layout's load / energy / get and half-sweep
