@@ -16,6 +16,8 @@
 //   mix 26: IMAD.WIDE + 3 LOP3, all independent (17-26: which form of the 64-bit product overlaps with alu work?)
 //   mix 27..29: the Philox round with hi32 from DFMA.RM and the state kept in register pairs whose high word is the
 //           0x43300000 the DFMA result already carries (no moves), plus 0, 2, 4 extra LOP3
+//   mix 30: 2 Philox rounds via IMAD.WIDE on one state + 2 rounds via DFMA.RM + IMAD (lo) on another (do the fma-heavy and
+//           fp64 pipes take the two kinds of rounds side by side?)   mix 31: 3 IMAD.WIDE rounds per DFMA round (6 + 2)
 //   mix 11: the Philox round with hi32 of the products from the FP64 pipe (DFMA.RM of (2^52 + c) * M*2^-32 + 2^52 - M*2^20,
 //           exact) and lo32 from IMAD: the variant DESIGN.md section 6 lists as tried and rejected
 #include <cuda_runtime.h>
@@ -226,6 +228,26 @@ __global__ void __launch_bounds__(256) int_mix_kernel(uint32_t *out, int iters, 
 #pragma unroll
                     for (int x = 0; x < 2 * (MIX - 27); ++x) e[c] = lop3_xor3(e[c], k0, k1);
                 }
+            } else if (MIX == 30 || MIX == 31) {
+                const double Ms0 = 3528531795.0 * 0x1p-32, K0 = 0x1p52 - 3528531795.0 * 0x1p20;   // M0 = 0xD2511F53
+                const double Ms1 = 3449720151.0 * 0x1p-32, K1 = 0x1p52 - 3449720151.0 * 0x1p20;   // M1 = 0xCD9E8D57
+#pragma unroll
+                for (int rr = 0; rr < 2; ++rr) {
+                    double P = __fma_rd(d[c], Ms0, K0), Q = __fma_rd(g[c], Ms1, K1);
+                    const uint32_t l0 = (uint32_t)__double2loint(d[c]) * 0xD2511F53u, l1 = (uint32_t)__double2loint(g[c]) * 0xCD9E8D57u;
+                    xor_low_word(Q, l0, k0);
+                    xor_low_word(P, l1, k1);
+                    d[c] = Q;
+                    g[c] = P;
+#pragma unroll
+                    for (int ww = 0; ww < (MIX == 30 ? 1 : 3); ++ww) {
+                        uint32_t h0, l0w, h1, l1w;
+                        mul_wide(a[c], 0xD2511F53u, h0, l0w);
+                        mul_wide(b[c], 0xCD9E8D57u, h1, l1w);
+                        a[c] = lop3_xor3(h1, l0w, k0);
+                        b[c] = lop3_xor3(h0, l1w, k1);
+                    }
+                }
             } else {
                 const double Ms0 = 3528531795.0 * 0x1p-32, K0 = 0x1p52 - 3528531795.0 * 0x1p20;   // M0 = 0xD2511F53
                 const double Ms1 = 3449720151.0 * 0x1p-32, K1 = 0x1p52 - 3449720151.0 * 0x1p20;   // M1 = 0xCD9E8D57
@@ -255,13 +277,13 @@ int int_peak_run(int mix, int ctas, int iters, int reps, uint32_t *d_scratch, fl
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return -2;
     float best = 1e30f;
-    const double ops_per_iter[30] = {4.0 * CHAINS, 2.0 * CHAINS, 4.0 * CHAINS, 4.0 * CHAINS, 6.0 * CHAINS, 2.0 * CHAINS,
+    const double ops_per_iter[32] = {4.0 * CHAINS, 2.0 * CHAINS, 4.0 * CHAINS, 4.0 * CHAINS, 6.0 * CHAINS, 2.0 * CHAINS,
                                      2.0 * CHAINS, 5.0 * CHAINS, 6.0 * CHAINS, 7.0 * CHAINS, 8.0 * CHAINS, 6.0 * CHAINS,
                                      4.0 * CHAINS, 4.0 * CHAINS, 4.0 * CHAINS, 4.0 * CHAINS, 4.0 * CHAINS,
                                      4.0 * CHAINS, 8.0 * CHAINS, 2.0 * CHAINS, 2.0 * CHAINS, 4.0 * CHAINS, 6.0 * CHAINS,
                                      8.0 * CHAINS, 8.0 * CHAINS, 6.0 * CHAINS, 4.0 * CHAINS,
-                                     12.0 * CHAINS, 16.0 * CHAINS, 20.0 * CHAINS};
-    if (mix < 0 || mix > 29) return -1;
+                                     12.0 * CHAINS, 16.0 * CHAINS, 20.0 * CHAINS, 20.0 * CHAINS, 36.0 * CHAINS};
+    if (mix < 0 || mix > 31) return -1;
     for (int r = 0; r < reps + 1; ++r) {
         cudaEventRecord(e0);
         switch (mix) {
@@ -294,7 +316,9 @@ int int_peak_run(int mix, int ctas, int iters, int reps, uint32_t *d_scratch, fl
             case 26: int_mix_kernel<26><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
             case 27: int_mix_kernel<27><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
             case 28: int_mix_kernel<28><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
-            default: int_mix_kernel<29><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
+            case 29: int_mix_kernel<29><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
+            case 30: int_mix_kernel<30><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
+            default: int_mix_kernel<31><<<ctas, 256>>>(d_scratch, iters, 0x1234567u, 0x89abcdefu); break;
         }
         cudaEventRecord(e1);
         if (cudaEventSynchronize(e1) != cudaSuccess) return -2;

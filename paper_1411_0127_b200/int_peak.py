@@ -23,9 +23,10 @@ MIXES = {0: "LOP3 only", 1: "IMAD.WIDE.U32 only", 2: "IMAD.WIDE + LOP3 dependent
          20: "DFMA only", 21: "DFMA + LOP3 1:1 independent", 22: "IMAD.WIDE + IMAD (lo) 1:1",
          23: "Philox round from IMAD.HI + IMAD (lo), + 2 LOP3", 24: "Philox round (register multipliers) + 4 LOP3",
          25: "IMAD.WIDE + FFMA 1:1", 26: "IMAD.WIDE + 3 LOP3 independent",
-         27: "2 Philox rounds via DFMA.RM + IMAD (lo), state in register pairs", 28: "same + 2 x 2 LOP3", 29: "same + 2 x 4 LOP3"}
+         27: "2 Philox rounds via DFMA.RM + IMAD (lo), state in register pairs", 28: "same + 2 x 2 LOP3", 29: "same + 2 x 4 LOP3",
+         30: "2 rounds via IMAD.WIDE + 2 rounds via DFMA.RM, interleaved", 31: "6 rounds via IMAD.WIDE + 2 rounds via DFMA.RM, interleaved"}
 # source-level instructions per chain-iteration of each mix (csrc/int_peak.cu)
-OPS = {0: 4, 1: 2, 2: 4, 3: 4, 4: 6, 5: 2, 6: 2, 7: 5, 8: 6, 9: 7, 10: 8, 11: 6, 12: 4, 13: 4, 14: 4, 15: 4, 16: 4, 17: 4, 18: 8, 19: 2, 20: 2, 21: 4, 22: 6, 23: 8, 24: 8, 25: 6, 26: 4, 27: 12, 28: 16, 29: 20}
+OPS = {0: 4, 1: 2, 2: 4, 3: 4, 4: 6, 5: 2, 6: 2, 7: 5, 8: 6, 9: 7, 10: 8, 11: 6, 12: 4, 13: 4, 14: 4, 15: 4, 16: 4, 17: 4, 18: 8, 19: 2, 20: 2, 21: 4, 22: 6, 23: 8, 24: 8, 25: 6, 26: 4, 27: 12, 28: 16, 29: 20, 30: 20, 31: 36}
 
 
 def build(force: bool = False) -> str:
