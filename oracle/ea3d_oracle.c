@@ -23,7 +23,7 @@
  * The stored-state lane generators (rng_mode 3, 4; R19): MT19937 against C++ std::mt19937 (whose 10000th value
  * the C++ standard fixes) and numpy's legacy RandomState; Parisi-Rapuano against an unbounded-history restatement of the
  * paper's two lines in the test; the lane-driven sweep against a per-sample run fed with the same
- * draw table (tests/test_oracle_lanes.py).
+ * draw table (tests/test_oracle_lanes.py).  The replica overlap: closed forms and a library dot product (tests/test_oracle_chain.py).
  * No function is left "parity unpinned".
  */
 #include <math.h>
