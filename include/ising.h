@@ -99,9 +99,9 @@ int ising_sweep(ising_t *h, double beta, int nsweeps, void *stream);
 
 /* As ising_sweep, and after every `every_half_sweeps`-th half-sweep of this call (counted from 1) writes the
  * energy (and magnetisation if d_M != NULL) of every sample to record r = 0,1,...:
- * d_E[r*nsamples + s].  d_E / d_M must hold (2*nsweeps / every_half_sweeps) * nsamples int64.  (With nsamples = 1 and L a
- * multiple of 64 the recording half-sweeps compute E and M themselves, from the field sums they already hold; otherwise a record
- * is one launch of the energy kernel.) */
+ * d_E[r*nsamples + s].  d_E / d_M must hold (2*nsweeps / every_half_sweeps) * nsamples int64.  (With nsamples = 1 and L >= 64
+ * the recording half-sweeps compute E and M themselves, from the field sums they already hold; otherwise a record is one
+ * launch of the energy kernel.) */
 int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_t *d_M, int every_half_sweeps,
                       void *stream);
 

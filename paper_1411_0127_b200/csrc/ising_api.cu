@@ -331,9 +331,20 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             sr.seed = r.seed;
             sr.A2 = 2u * r.A;
             sr.s0tab = nullptr;
-            if (g.L >= 64 && h->kernel_choice != 3)   // rows of at least 32 bits: no segment loop (kernel choice 3 keeps the loop)
-                launch_pdl(half_sweep_site_packed_rows2<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw, (uint32_t)g.Hc);
-            else
+            if (g.L >= 64 && h->kernel_choice != 3) {  // rows of at least 32 bits: no segment loop (kernel choice 3 keeps the loop)
+                unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;
+                if (mE || mM) {
+                    if (!h->slots_clean) {
+                        if (cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
+                        h->slots_clean = true;
+                    }
+                    launch_pdl(half_sweep_site_packed_rows2<RNG, true>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw,
+                               (uint32_t)g.Hc, slots, (long long)g.N, mE, mM);
+                } else {
+                    launch_pdl(half_sweep_site_packed_rows2<RNG, false>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw,
+                               (uint32_t)g.Hc, (unsigned long long *)nullptr, 0ll, (long long *)nullptr, (long long *)nullptr);
+                }
+            } else
                 launch_pdl(half_sweep_site_packed_rows<RNG>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw, (uint32_t)g.Hc);
         } else {
             const uint64_t nw = (g.Hc + 31) / 32;
@@ -397,7 +408,9 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
 // Can the half-sweep kernel of this handle return E and M itself (half_sweep_site_packed<.., MEASURE = true>)?
 bool can_measure_in_sweep(const ising_t *h)
 {
-    return h->g.nsamples == 1 && h->g.fast && h->kernel_choice != 1 && (h->rng_mode == ISING_RNG_PHILOX || h->rng_mode == ISING_RNG_MINSTD);
+    if (h->g.nsamples != 1 || (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD)) return false;
+    if (h->g.fast) return h->kernel_choice != 1;                                                              // word-parallel kernel
+    return h->g.L >= 64 && h->kernel_choice != 1 && h->kernel_choice != 3 && h->g.Hc < (1ull << 32);          // loop-free bit-window kernel
 }
 
 int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long long *mE = nullptr, long long *mM = nullptr)

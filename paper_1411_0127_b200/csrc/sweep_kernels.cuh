@@ -586,12 +586,16 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
 // The segment loop of half_sweep_site_packed_rows makes every warp pay for two segments as soon as one of its 32 words
 // straddles (always, for L < 2048); here the straddle costs a few mask operations: 933 -> 711 instructions per word (ncu).
 // ---------------------------------------------------------------------------------------------------
-template <int RNG>
+// MEASURE: E and M of the resulting configuration, as in half_sweep_site_packed<.., MEASURE = true>.
+template <int RNG, bool MEASURE>
 __global__ void __launch_bounds__(128)
-half_sweep_site_packed_rows2(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t n_words, uint32_t Hc)
+half_sweep_site_packed_rows2(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t n_words, uint32_t Hc,
+                             unsigned long long *acc, long long N, long long *E, long long *M)
 {
-    const uint32_t w = blockIdx.x * 128u + threadIdx.x;
-    if (w >= n_words) return;
+    const uint32_t w_raw = blockIdx.x * 128u + threadIdx.x;
+    if (!MEASURE && w_raw >= n_words) return;
+    const bool live = w_raw < n_words;                 // MEASURE: every thread reaches the block reduction
+    const uint32_t w = live ? w_raw : n_words - 1;
     const uint32_t L = (uint32_t)a.L, H = L >> 1, LH = L * H;
     const uint32_t j0 = 32u * w;
     const uint32_t rA = j0 / H, m0 = j0 - rA * H, zA = rA / L, yA = rA - zA * L;
@@ -610,8 +614,10 @@ half_sweep_site_packed_rows2(const SweepArgs a, const __grid_constant__ SiteRng 
     J[0] = __ldg(a.J_act[0] + w);
     J[2] = __ldg(a.J_act[1] + w);
     J[4] = __ldg(a.J_act[2] + w);
+    uint32_t other_word;                               // the other colour's word of the same ranks (MEASURE: its up spins)
     {   // +-x
         const uint32_t lo = __ldg(a.S_oth + w), hi = __ldg(a.S_oth + w + 1), prev = w ? __ldg(a.S_oth + w - 1) : 0u;
+        other_word = lo;
         const uint32_t jlo = __ldg(a.J_oth[0] + w), jprev = w ? __ldg(a.J_oth[0] + w - 1) : 0u;
         nb[0] = (X & __funnelshift_r(lo, hi, 1)) | (~X & lo);
         nb[1] = (X & lo) | (~X & __funnelshift_l(prev, lo, 1));
@@ -660,7 +666,19 @@ half_sweep_site_packed_rows2(const SweepArgs a, const __grid_constant__ SiteRng 
     uint32_t sum2, sum1, sum0;
     satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
     const uint32_t valid = nvalid == 32u ? 0xFFFFFFFFu : (1u << nvalid) - 1u;
-    a.S_act[w] = s ^ (flip_mask(sum2, sum1, sum0, c4, c8, c12) & valid);
+    const uint32_t f = flip_mask(sum2, sum1, sum0, c4, c8, c12) & valid;
+    if (live) a.S_act[w] = s ^ f;
+    if (MEASURE) {
+        sum0 &= valid;
+        sum1 &= valid;
+        sum2 &= valid;
+        const unsigned sat = __popc(sum0) + 2 * __popc(sum1) + 4 * __popc(sum2) + 6 * __popc(f) -
+                             2 * (__popc(sum0 & f) + 2 * __popc(sum1 & f) + 4 * __popc(sum2 & f));
+        const unsigned long long unsat = live ? 6ull * nvalid - sat : 0ull;
+        const unsigned long long up = live ? (unsigned long long)(__popc((s ^ f) & valid) + __popc(other_word & valid)) : 0ull;
+        block_accumulate2(unsat, up, acc + 2 * (blockIdx.x & (ACC_SLOTS - 1)));
+        finalize_slots_last_cta(acc, N, E, M);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -649,12 +649,13 @@ def test_overlap_of_replicas_equals_the_oracle(L, nsamples):
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
-@pytest.mark.parametrize("L", [64, 128, 192, 256, 320, 448])
+@pytest.mark.parametrize("L", [64, 128, 192, 256, 320, 448, 66, 100, 126, 250])
 def test_energy_measured_inside_the_half_sweep_kernel(L, rng_mode):
     """Trace records of the word-parallel layout come from the half-sweep kernel itself (MEASURE variant: satisfied bonds from
     the field bit planes, n -> 6 - n where the site flipped).  E and M after every half-sweep (red and blue records) against the
-    one-site-at-a-time kernels with their separate energy kernel, for 1, 3, 4, 5 words per thread and a padded row (L = 448);
-    E-only and M-only traces; the oracle at the smaller sizes."""
+    one-site-at-a-time kernels with their separate energy kernel, for 1, 3, 4, 5 words per thread and a padded row (L = 448), and
+    for the loop-free bit-window kernel of general L (66, 100, 126, 250: rows straddling words, a partial last word); E-only
+    traces; the oracle at the smaller sizes."""
     spins, J = synth.make_spins(L, 1, 91), synth.make_couplings(L, 1, 92)
     g = Ising(L, 1, SEED, rng_mode)
     g.ising_load_state(dev(spins), dev(J))
