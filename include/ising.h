@@ -123,6 +123,15 @@ int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream);
 int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps,
                    uint32_t *h_spins_out, int64_t *h_E, int64_t *h_M, void *stream);
 
+/* The same job enqueued on `stream` without the final synchronisation: returns as soon as the copies and launches are queued.
+ * All host buffers must be pinned (cudaHostAlloc / torch pin_memory; with pageable memory the copies are staged by the driver
+ * and the call is no longer asynchronous) and must stay valid and untouched until the caller has synchronised the stream;
+ * h_spins_out / h_E / h_M hold the results only after that.  Meant for double buffering: two handles (two workspaces) on two
+ * streams, so that the PCIe copies of one job run under the sweeps of the other (bench.py's `e2e`).  One handle must not have two
+ * jobs in flight on different streams: its staging area and lattice arrays are reused by every call. */
+int ising_run_host_async(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps,
+                         uint32_t *h_spins_out, int64_t *h_E, int64_t *h_M, void *stream);
+
 /* Host only.  The acceptance thresholds for dE = 4, 8, 12 exactly as the kernels receive them (R5, R6):
  * out[k] in [0, 2^32] (Philox) or [0, 2^31-1] (MINSTD). */
 int ising_thresholds(double beta, int rng_mode, uint64_t out[3]);

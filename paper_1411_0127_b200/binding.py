@@ -17,7 +17,7 @@ OK, EINVAL, ECUDA = 0, -1, -2
 
 EXPORTS = (
     "ising_workspace_bytes", "ising_create", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
-    "ising_get_spins", "ising_run_host", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
+    "ising_get_spins", "ising_run_host", "ising_run_host_async", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
 )
@@ -45,6 +45,7 @@ def lib() -> C.CDLL:
     L.ising_get_spins.argtypes = [vp, vp, vp]
     L.ising_overlap.argtypes = [vp, i32, i32, vp, vp]
     L.ising_run_host.argtypes = [vp, vp, vp, dbl, i32, vp, vp, vp, vp]
+    L.ising_run_host_async.argtypes = [vp, vp, vp, dbl, i32, vp, vp, vp, vp]
     L.ising_thresholds.argtypes = [dbl, i32, C.POINTER(u64)]
     L.ising_fnv1a64_host.argtypes = [vp, sz]
     L.ising_fnv1a64_host.restype = u64
@@ -217,6 +218,16 @@ class Ising:
                                     _u32(h_spins_out) if h_spins_out is not None else None, E.data_ptr(), M.data_ptr(),
                                     _stream_ptr(stream)), "ising_run_host")
         return E, M
+
+    def ising_run_host_async(self, h_spins, h_J, beta: float, nsweeps: int, h_spins_out, h_E, h_M=None, stream=None):
+        """Enqueue the ising_run_host job on `stream` and return at once.  Every tensor must be a pinned CPU tensor the caller
+        keeps alive; results (h_spins_out, h_E, h_M) are valid after the stream has been synchronised."""
+        for x in (h_spins, h_J, h_spins_out, h_E, h_M):
+            assert x is None or (not x.is_cuda and x.is_pinned()), "ising_run_host_async needs pinned host tensors"
+        _check(lib().ising_run_host_async(self._h, _u32(h_spins), _u32(h_J), float(beta), int(nsweeps),
+                                          _u32(h_spins_out) if h_spins_out is not None else None, h_E.data_ptr(),
+                                          h_M.data_ptr() if h_M is not None else None, _stream_ptr(stream)),
+               "ising_run_host_async")
 
     def ising_get_t(self) -> int:
         t = C.c_uint64(0)

@@ -735,8 +735,8 @@ int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *st
     return check_launch(h, 2);
 }
 
-int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps, uint32_t *h_spins_out,
-                   int64_t *h_E, int64_t *h_M, void *stream)
+int ising_run_host_async(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps,
+                         uint32_t *h_spins_out, int64_t *h_E, int64_t *h_M, void *stream)
 {
     if (!h || !h_spins || !h_J || !h_E || nsweeps < 0 || !(beta >= 0.0)) return ISING_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -763,7 +763,15 @@ int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, dou
         return ISING_ECUDA;
     if (h_M && cudaMemcpyAsync(h_M, d_M, (size_t)g.nsamples * sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess)
         return ISING_ECUDA;
-    return cudaStreamSynchronize(st) == cudaSuccess ? ISING_OK : ISING_ECUDA;
+    return ISING_OK;
+}
+
+int ising_run_host(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps, uint32_t *h_spins_out,
+                   int64_t *h_E, int64_t *h_M, void *stream)
+{
+    const int rc = ising_run_host_async(h, h_spins, h_J, beta, nsweeps, h_spins_out, h_E, h_M, stream);
+    if (rc != ISING_OK) return rc;
+    return cudaStreamSynchronize((cudaStream_t)stream) == cudaSuccess ? ISING_OK : ISING_ECUDA;
 }
 
 int ising_thresholds(double beta, int rng_mode, uint64_t out[3])

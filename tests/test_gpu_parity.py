@@ -527,6 +527,35 @@ def test_run_host_every_layout(L, nsamples, rng_mode):
     assert np.array_equal(E2.numpy(), Eo)
 
 
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+def test_run_host_async_double_buffered(rng_mode):
+    """ising_run_host_async: two handles on two streams with six different jobs in flight alternately (the double buffering of
+    bench.py's e2e); every job's spins, E and M against the oracle."""
+    L, njobs = 128, 6
+    handles = [Ising(L, 1, SEED, rng_mode), Ising(L, 1, SEED, rng_mode)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    jobs = []
+    for k in range(njobs):
+        spins, J = synth.make_spins(L, 1, 200 + k), synth.make_couplings(L, 1, 300 + k)
+        jobs.append(dict(spins=spins, J=J, hs=torch.from_numpy(spins.view(np.int32)).pin_memory(),
+                         hJ=torch.from_numpy(J.view(np.int32)).pin_memory(),
+                         out=torch.empty(spins.size, dtype=torch.int32).pin_memory(),
+                         E=torch.zeros(1, dtype=torch.int64).pin_memory(), M=torch.zeros(1, dtype=torch.int64).pin_memory()))
+    torch.cuda.synchronize()
+    for k, jb in enumerate(jobs):
+        g, st = handles[k % 2], streams[k % 2]
+        g.ising_set_t(0)
+        g.ising_run_host_async(jb["hs"], jb["hJ"], 1 / 1.1, 2 + k % 3, jb["out"], jb["E"], jb["M"], stream=st)
+    for st in streams:
+        st.synchronize()
+    for k, jb in enumerate(jobs):
+        o = _loaded(L, 1, rng_mode, jb["spins"], jb["J"])
+        o.sweep(1 / 1.1, 2 + k % 3)
+        assert np.array_equal(jb["out"].numpy().view(np.uint32), o.spins_packed().reshape(-1)), f"job {k}"
+        Eo, Mo = o.energy()
+        assert int(jb["E"][0]) == int(Eo[0]) and int(jb["M"][0]) == int(Mo[0]), f"job {k}"
+
+
 # ------------------------------------------------------------------------------------------------ config 5, full size
 
 def _avail_gib():
