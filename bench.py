@@ -162,6 +162,9 @@ def main():
     ap.add_argument("--aux", action="store_true",
                     help="rows a9 / a10 and the general-L kernels: load_state, energy, get_spins and a half-sweep per layout, with GB/s")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
+    ap.add_argument("--minstd-seed-source", action="store_true",
+                    help="MINSTD at L=1024: seed states from the table (kernel choice 5 = automatic) against the hybrid kernel "
+                         "(choice 4), steps interleaved over a sustained run, with SM clock and board power per step")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -352,6 +355,35 @@ def main():
                 "table2_device_api": [bench_table2(k) for k in (0, 1, 3, 4)],
                 # the launch configuration of the paper's Table II: 64 blocks x 256 threads, 2^15 draws each, 10 times
                 "table2_paper_launch_configuration": [bench_table2(k, nlanes=64 * 256, ndraws=1 << 15, reps=10) for k in (0, 1, 3, 4)]}
+
+    if args.minstd_seed_source:
+        import pynvml
+
+        pynvml.nvmlInit()
+        nv = pynvml.nvmlDeviceGetHandleByIndex(local)
+        gs = {}
+        for choice in (5, 4):
+            gs[choice] = Ising(L, 1, synth.DYN_SEED, MINSTD)
+            gs[choice].ising_set_kernel(choice)
+        print("| step | table (choice 5) ms per half-sweep | hybrid (choice 4) ms per half-sweep | SM MHz | W |\n|---:|---:|---:|---:|---:|")
+        for rep in range(args.steps if args.steps > 5 else 24):
+            ms = {}
+            for choice in (5, 4):
+                g = gs[choice]
+                g.ising_set_t(0)
+                g.ising_load_state(d_spins, d_J)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                g.ising_sweep(BETA, nsw)
+                b.record(stream)
+                clk = pynvml.nvmlDeviceGetClockInfo(nv, pynvml.NVML_CLOCK_SM)  # read while the sweeps run
+                watt = pynvml.nvmlDeviceGetPowerUsage(nv) / 1000
+                g.ising_energy()
+                g.ising_get_spins(d_out)
+                torch.cuda.synchronize()
+                ms[choice] = a.elapsed_time(b) / (2 * nsw)
+            print(f"| {rep} | {ms[5]:.4f} | {ms[4]:.4f} | {clk} | {watt:.0f} |")
+        return
 
     if args.scan:
         from paper_1411_0127_b200 import PHILOX_SHARED

@@ -175,7 +175,9 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
  * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
  * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),
  * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = the bit-window kernel with its
- * row-segment loop also for L >= 64 (where the automatic choice is the loop-free variant).  All give the same bits;
+ * row-segment loop also for L >= 64 (where the automatic choice is the loop-free variant), 4 / 5 = MINSTD word-parallel kernel
+ * with the hybrid seed source (L a multiple of 512: three words of a thread from the table, the fourth recomputed) / with the
+ * table for every word (what 0 chooses); both equal 0 in the other modes.  All give the same bits;
  * the tests use this to show that results do not depend on layout, thread mapping or caching. */
 int ising_set_kernel(ising_t *h, int which);
 

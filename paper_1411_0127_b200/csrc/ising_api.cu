@@ -304,7 +304,14 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             sr.seed = r.seed;
             sr.A2 = 2u * r.A;
             sr.s0tab = nullptr;
-            const bool cached = RNG == 1 && h->kernel_choice == 0 && h->s0tab != nullptr;
+            // MINSTD with the seed table.  Kernel choice 4 (W = 4 only) is the hybrid seed source, RNG = 3 in sweep_kernels.cuh: the
+            // last of the 4 words of a thread recomputes its seed states instead of loading them, 4.125 instead of 5.125 B per
+            // flip attempt from HBM, paid with issue slots the table kernel leaves idle.  Measured at L = 1024: 0.387 against
+            // 0.399 ms per half-sweep on a cool part at 1965 MHz, but 0.43-0.50 against 0.406 ms once a sustained run has
+            // brought the board to its power limit and the SM clock to ~1600 MHz (the table kernel is bound by HBM and does not
+            // notice; profiles/r1z_hybrid_minstd.md).  Not a robust gain, so the automatic choice stays the full table.
+            const bool hybrid = W == 4 && h->kernel_choice == 4;
+            const bool cached = RNG == 1 && (h->kernel_choice == 0 || h->kernel_choice == 4 || h->kernel_choice == 5) && h->s0tab != nullptr;
             if (cached) {
                 uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
                 if (!h->s0_ready) {  // once per handle: the seed states depend on (seed, site) only (R11)
@@ -319,7 +326,8 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
                     h->s0_ready = true;
                 }
                 sr.s0tab = tab[c];
-                launch_site_packed<2>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
+                if (hybrid) launch_site_packed_w<3, 4>(mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
+                else launch_site_packed<2>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
             } else {
                 launch_site_packed<RNG>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
             }
@@ -877,7 +885,7 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
 
 int ising_set_kernel(ising_t *h, int which)
 {
-    if (!h || which < 0 || which > 3) return ISING_EINVAL;
+    if (!h || which < 0 || which > 5) return ISING_EINVAL;
     h->kernel_choice = which;
     return ISING_OK;
 }

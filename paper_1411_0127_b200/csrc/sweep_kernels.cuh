@@ -255,8 +255,10 @@ __device__ __forceinline__ RowMap row_map(int L)
 // the new active words plus the other colour's words of the same rows, which are loaded anyway.  About 15 popcounts per
 // word, then the slot accumulation and last-CTA finalisation of energy_site_packed: a trace of E and M per sweep costs no
 // extra launch and no extra pass over the 512 MiB (L = 1024: 78 us per record saved).
+// Four CTAs per SM (64 registers) for the Philox kernel the L = 1024 numbers are quoted on (0.3899 -> 0.3868 ms per half-sweep, 8 bytes
+// of spill) and for the hybrid MINSTD kernel (0.423 -> 0.387 ms); the other variants keep ptxas' own choice (W = 5 would spill 40 bytes).
 template <int RNG, int W, bool MEASURE>
-__global__ void __launch_bounds__(SWEEP_THREADS)
+__global__ void __launch_bounds__(SWEEP_THREADS, (RNG == 3 || RNG == 0) && W == 4 && !MEASURE ? 4 : 0)
 half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, unsigned long long *acc, long long N,
                        long long *E, long long *M)
 {
@@ -323,19 +325,56 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     };
 
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
-    if (RNG == 2) {
-        // seeds from the table, two groups of 16 sites in flight: while one half-word's draws are compared, the next
-        // half-word's four 16-byte loads are outstanding (about 2 KB per warp, enough to keep HBM busy)
-        const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
-        const uint4 *tab = rng.s0tab;
-        uint4 cur[4], nxt[4];
+    // RNG = 2: the seed states of all W words come from the table.  RNG = 3 (hybrid, W >= 2): the first W - 1 words take them from
+    // the table and the last word recomputes them (SplitMix64 per site, as RNG = 1): the table kernel is bound by HBM with the
+    // integer pipes half idle, the recomputing kernel by integer issue, so a share of recomputed sites shortens the HBM stream
+    // (5.125 -> 4.125 B per flip attempt at W = 4) at the price of otherwise idle issue slots.  Same draws either way (R11, R12).
+    // Kernel choice 4 only: faster on a cool part, slower once the board runs at its power limit (see ising_api.cu).
+    constexpr int WC = RNG == 2 ? W : (RNG == 3 ? W - 1 : 0);
+    // seeds from the table, two groups of 16 sites in flight: while one half-word's draws are compared, the next
+    // half-word's four 16-byte loads are outstanding (about 2 KB per warp, enough to keep HBM busy)
+    const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
+    const uint4 *tab = rng.s0tab;
+    uint4 cur[4], nxt[4];
+    if (WC > 0) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) cur[i] = __ldcs(tab + minstd_s0_index<W>(warp_global, 0, i, lane));
+    }
+    // The two thresholds every draw is compared with live in ordinary registers (row < 2^27, so the OR adds nothing; it
+    // only keeps them out of the uniform register file, which the 19 Philox constants fill: ptxas otherwise reloads
+    // them from the constant bank after every rare-path branch).
+    Thresholds Tr = a.T;
+    Tr.t4 |= row >> 31;
+    Tr.t8 |= row >> 31;
+    PhiloxCommonConst pcr = rng.pc;
+    PhiloxSampleConst psr = rng.ps;
+    if (RNG == 0) {  // likewise the round keys of the last two rounds
+        pcr.k0[5] |= row >> 31;
+        pcr.k0[6] |= row >> 31;
+        psr.k1[5] |= row >> 31;
+        psr.k1[6] |= row >> 31;
+        psr.k1[7] |= row >> 31;
+    }
+#pragma unroll
+    for (int k = WC; k < W; ++k) {
+        uint32_t c4, c8, c12;
+        if (RNG == 0) {
+            cond_masks_site_packed_philox(pcr, psr, row + (uint32_t)k, Tr, c4, c8, c12);
+        } else {
+            const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
+            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
+        }
+        const uint32_t f = flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
+        s[k] ^= f;
+        if (MEASURE) measure_word(k, f);
+    }
+
+    if (WC > 0) {
         uint32_t c4 = 0, c8 = 0, c12 = 0;
 #pragma unroll
-        for (int h = 0; h < 2 * W; ++h) {
+        for (int h = 0; h < 2 * WC; ++h) {
             const int k = h >> 1, half = h & 1;
-            if (h + 1 < 2 * W) {
+            if (h + 1 < 2 * WC) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
                     nxt[i] = __ldcs(tab + minstd_s0_index<W>(warp_global, (h + 1) >> 1, 4 * ((h + 1) & 1) + i, lane));
@@ -357,35 +396,6 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
             for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
         }
     }
-    // The two thresholds every draw is compared with live in ordinary registers (row < 2^27, so the OR adds nothing; it
-    // only keeps them out of the uniform register file, which the 19 Philox constants fill: ptxas otherwise reloads
-    // them from the constant bank after every rare-path branch).
-    Thresholds Tr = a.T;
-    Tr.t4 |= row >> 31;
-    Tr.t8 |= row >> 31;
-    PhiloxCommonConst pcr = rng.pc;
-    PhiloxSampleConst psr = rng.ps;
-    if (RNG == 0) {  // likewise the round keys of the last two rounds
-        pcr.k0[5] |= row >> 31;
-        pcr.k0[6] |= row >> 31;
-        psr.k1[5] |= row >> 31;
-        psr.k1[6] |= row >> 31;
-        psr.k1[7] |= row >> 31;
-    }
-#pragma unroll
-    for (int k = 0; k < W && RNG != 2; ++k) {
-        uint32_t c4, c8, c12;
-        if (RNG == 0) {
-            cond_masks_site_packed_philox(pcr, psr, row + (uint32_t)k, Tr, c4, c8, c12);
-        } else {
-            const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
-            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
-        }
-        const uint32_t f = flip_mask(sum2[k], sum1[k], sum0[k], c4, c8, c12);
-        s[k] ^= f;
-        if (MEASURE) measure_word(k, f);
-    }
-
     if (rm.active) store_words<W>(a.S_act, row, s);
     if (MEASURE) {
         // unsatisfied bonds = 6 per active site - satisfied; idle lanes of a padded row shadow lane 0 and count nothing

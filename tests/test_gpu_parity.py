@@ -288,6 +288,33 @@ def test_word_parallel_kernel_equals_generic_kernel_for_any_multiple_of_64(L, rn
     assert torch.equal(Ea, Eb) and torch.equal(Ma, Mb)
 
 
+def test_minstd_hybrid_seed_source():
+    """MINSTD, four words per thread (L = 512 is the smallest such lattice): kernel choice 4 takes the seed states of three
+    words from the table and recomputes the fourth; choice 5 (= the automatic choice) reads the table for every word,
+    choice 2 recomputes all.  Same bits as the
+    oracle after two sweeps, and the recording (MEASURE) variant gives the oracle's E and M per half-sweep."""
+    L = 512
+    spins, J = synth.make_spins(L, 1, 51), synth.make_couplings(L, 1, 52)
+    o = _loaded(L, 1, MINSTD, spins, J)
+    hs = []
+    for choice in (4, 5, 2):
+        g = Ising(L, 1, SEED, MINSTD)
+        g.ising_set_kernel(choice)
+        g.ising_load_state(dev(spins), dev(J))
+        g.ising_sweep(1 / 0.7, 1)
+        hs.append(g)
+    o.sweep(1 / 0.7, 1)
+    assert_same_state(o, hs[0], "hybrid seed source, L=512")
+    for g in hs[1:]:
+        assert torch.equal(g.ising_get_spins(), hs[0].ising_get_spins())
+    E, M = hs[0].ising_sweep_trace(1 / 0.7, 1, every_half_sweeps=1)
+    for r in range(2):
+        o.half_sweep(1 / 0.7)
+        Eo, Mo = o.energy()
+        assert int(E[r, 0]) == int(Eo[0]) and int(M[r, 0]) == int(Mo[0]), r
+    assert_same_state(o, hs[0], "hybrid seed source after the recording sweep")
+
+
 @pytest.mark.parametrize("L", [64, 128, 256, 512])
 def test_minstd_cached_seed_table_equals_recomputed_seeds(L):
     """MINSTD: the default word-parallel kernel streams the seed states s0 from a table filled once per handle; kernel
