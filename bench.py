@@ -425,6 +425,12 @@ def main():
             Jc = torch.from_numpy(J_np.view(np.int32)).cuda()
             g = Ising(Ls, ns, synth.DYN_SEED, cfg["rng_mode"])
             out = torch.empty_like(sp)
+            if idx == 4:
+                from concurrent.futures import ThreadPoolExecutor
+
+                snaps = [torch.empty(sp.shape, dtype=sp.dtype).pin_memory() for _ in range(nsweeps // 10)]
+                snap_ready = [torch.cuda.Event() for _ in snaps]
+                pool = ThreadPoolExecutor(max_workers=len(snaps))
 
             def run():
                 g.ising_set_t(0)
@@ -440,11 +446,21 @@ def main():
                     E, M = g.ising_sweep_trace(beta, nsweeps, every_half_sweeps=2)
                     return int(E[-1, 0])
                 if idx == 4:      # 64-bit FNV-1a of the packed spin words every 10 sweeps (host side of the C ABI)
-                    h = 0
-                    for _ in range(nsweeps // 10):
+                    # FNV-1a is sequential within one checksum (h = (h ^ byte) * prime, about 17 ms per 16 MiB on a host core),
+                    # but the ten checksums are independent: each snapshot goes to its own pinned buffer with an asynchronous
+                    # copy, and a host thread hashes it (the C call releases the GIL) while the GPU sweeps on
+                    def hash_when_ready(k):
+                        snap_ready[k].synchronize()
+                        return binding.ising_fnv1a64_host(snaps[k].numpy())
+
+                    futures = []
+                    for k in range(nsweeps // 10):
                         g.ising_sweep(beta, 10)
-                        h = binding.ising_fnv1a64_host(g.ising_get_spins(out).cpu().numpy())
-                    return h
+                        g.ising_get_spins(out)
+                        snaps[k].copy_(out, non_blocking=True)
+                        snap_ready[k].record(stream)
+                        futures.append(pool.submit(hash_when_ready, k))
+                    return [f.result() for f in futures][-1]
                 g.ising_sweep(beta, nsweeps)
                 E, _ = g.ising_energy()
                 return int(E[0])
