@@ -26,6 +26,11 @@
  *   PAPER.md:227); nsamples = 32*k uses a sample-packed layout (bits of a word = 32 disorder samples at
  *   one site, "AMSC" storage, with k coded batches).
  *
+ * Devices: a handle belongs to the CUDA device its workspace lives on.  ising_create refuses a workspace of another
+ *   device than the current one, and every call that launches work returns ISING_EINVAL when made with a different
+ *   device current (cudaSetDevice): the kernels would otherwise dereference another GPU's memory.  All d_* buffers of
+ *   a call must live on the handle's device.
+ *
  * Pointers: every pointer named d_* is DEVICE memory owned by the caller (e.g. a torch CUDA tensor), every
  *   h_* pointer is HOST memory owned by the caller.  The handle owns host metadata only; the workspace
  *   passed to ising_create must stay alive, and must not be written by the caller, until ising_destroy.
@@ -51,7 +56,10 @@ extern "C" {
                              misaligned, beta < 0 or NaN, nsweeps < 0 */
 #define ISING_ECUDA (-2)  /* a CUDA runtime call or kernel launch failed (sticky errors surface here too) */
 
-#define ISING_RNG_PHILOX 0 /* Philox4x32-10, key (lo32 seed, hi32 seed ^ sample), counter (t, colour-rank>>2)  (R9, R10) */
+#define ISING_RNG_PHILOX 0 /* Philox4x32-10, key (lo32 seed, hi32 seed ^ sample), counter (t, colour-rank>>2)  (R9, R10).
+                              Because the sample index is XORed into the high key word, (seed, sample) and
+                              (seed ^ (x << 32), sample ^ x) name the same stream: runs that must be independent need
+                              seeds that differ in their LOW 32 bits (the same holds for the batch index in mode 2). */
 #define ISING_RNG_MINSTD 1 /* MINSTD 16807 mod 2^31-1 (Eq. 7), one stream per site seeded by
                               SplitMix64 (R11), draw of sweep n = 16807^(n+1) * s0 mod (2^31-1) (R12) */
 
@@ -174,11 +182,9 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
 /* Select the kernels: 0 = automatic (site-packed: the word-parallel kernel when L is a multiple of 64, with the cached seed
  * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
  * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),
- * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = the bit-window kernel with its
- * row-segment loop also for L >= 64 (where the automatic choice is the loop-free variant), 4 / 5 = MINSTD word-parallel kernel
- * with the hybrid seed source (L a multiple of 512: three words of a thread from the table, the fourth recomputed) / with the
- * table for every word (what 0 chooses); both equal 0 in the other modes.  All give the same bits;
- * the tests use this to show that results do not depend on layout, thread mapping or caching. */
+ * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = as 0 but always one launch per
+ * colour half-sweep (never the persistent kernel that 0 uses for lattices resident in the L2).  All give the same bits; the
+ * tests use this to show that results do not depend on layout, thread mapping or caching. */
 int ising_set_kernel(ising_t *h, int which);
 
 /* Number of kernels this handle has launched so far. */

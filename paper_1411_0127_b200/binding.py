@@ -139,9 +139,12 @@ class Ising:
     spins (nsamples, W), couplings (nsamples, 3, W), W = ceil(L^3/32).
     """
 
-    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device="cuda:0", workspace=None):
-        """`workspace`: optional caller-owned uint8 CUDA tensor of at least ising_workspace_bytes bytes, 256-byte aligned
-        (default: allocated here)."""
+    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device=None, workspace=None):
+        """`device`: the CUDA device of the handle (default: torch's current device, so that a process that has called
+        torch.cuda.set_device(LOCAL_RANK) gets its own GPU).  `workspace`: optional caller-owned uint8 CUDA tensor of at least
+        ising_workspace_bytes bytes, 256-byte aligned (default: allocated here, on `device`).  Every call of the handle runs
+        with `device` current, takes its default stream from that device and rejects tensors that live elsewhere; the library
+        itself refuses a handle whose workspace is not on the current device (ISING_EINVAL)."""
         import torch
 
         self.L, self.nsamples, self.seed, self.rng_mode = L, nsamples, seed, rng_mode
@@ -149,27 +152,44 @@ class Ising:
         self.W = (self.N + 31) // 32
         nbytes = ising_workspace_bytes(L, nsamples, rng_mode)
         if workspace is None:
-            self.device = torch.device(device)
+            dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+            if dev.index is None:
+                dev = torch.device("cuda", torch.cuda.current_device())
+            self.device = dev
             # torch's caching allocator returns 512-byte aligned blocks
             workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         else:
             assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()
+            assert device is None or torch.device(device) == workspace.device, "workspace is not on `device`"
             self.device = workspace.device
             nbytes = workspace.numel()
         self.workspace = workspace
         h = C.c_void_p()
-        _check(lib().ising_create(L, nsamples, seed, rng_mode, self.workspace.data_ptr(), nbytes, C.byref(h)),
-               "ising_create")
+        with torch.cuda.device(self.device):
+            _check(lib().ising_create(L, nsamples, seed, rng_mode, self.workspace.data_ptr(), nbytes, C.byref(h)),
+                   "ising_create")
         self._h = h
+
+    def _on_device(self, *tensors):
+        """Guard for the device calls: makes the handle's device current (so that the launches, and the default stream, are
+        that device's) and checks that every CUDA tensor handed in lives on it."""
+        import torch
+
+        for x in tensors:
+            assert x is None or not x.is_cuda or x.device == self.device, \
+                f"tensor on {x.device}, handle on {self.device}: a kernel would dereference another GPU's memory"
+        return torch.cuda.device(self.device)
 
     # -- the C-ABI calls, same names
     def ising_load_state(self, spins, J, stream=None):
         assert spins.is_cuda and J.is_cuda and spins.is_contiguous() and J.is_contiguous()
         assert spins.numel() == self.nsamples * self.W and J.numel() == 3 * self.nsamples * self.W
-        _check(lib().ising_load_state(self._h, _u32(spins), _u32(J), _stream_ptr(stream)), "ising_load_state")
+        with self._on_device(spins, J):
+            _check(lib().ising_load_state(self._h, _u32(spins), _u32(J), _stream_ptr(stream)), "ising_load_state")
 
     def ising_sweep(self, beta: float, nsweeps: int, stream=None):
-        _check(lib().ising_sweep(self._h, float(beta), int(nsweeps), _stream_ptr(stream)), "ising_sweep")
+        with self._on_device():
+            _check(lib().ising_sweep(self._h, float(beta), int(nsweeps), _stream_ptr(stream)), "ising_sweep")
 
     def ising_sweep_trace(self, beta: float, nsweeps: int, every_half_sweeps: int = 1, want_M: bool = True, stream=None):
         """Returns (E, M) int64 CUDA tensors of shape (records, nsamples)."""
@@ -178,8 +198,9 @@ class Ising:
         nrec = (2 * nsweeps) // every_half_sweeps
         E = torch.empty((nrec, self.nsamples), dtype=torch.int64, device=self.device)
         M = torch.empty((nrec, self.nsamples), dtype=torch.int64, device=self.device) if want_M else None
-        _check(lib().ising_sweep_trace(self._h, float(beta), int(nsweeps), E.data_ptr(), M.data_ptr() if want_M else None,
-                                       int(every_half_sweeps), _stream_ptr(stream)), "ising_sweep_trace")
+        with self._on_device():
+            _check(lib().ising_sweep_trace(self._h, float(beta), int(nsweeps), E.data_ptr(), M.data_ptr() if want_M else None,
+                                           int(every_half_sweeps), _stream_ptr(stream)), "ising_sweep_trace")
         return E, M
 
     def ising_energy(self, stream=None):
@@ -188,7 +209,8 @@ class Ising:
 
         E = torch.empty(self.nsamples, dtype=torch.int64, device=self.device)
         M = torch.empty(self.nsamples, dtype=torch.int64, device=self.device)
-        _check(lib().ising_energy(self._h, E.data_ptr(), M.data_ptr(), _stream_ptr(stream)), "ising_energy")
+        with self._on_device():
+            _check(lib().ising_energy(self._h, E.data_ptr(), M.data_ptr(), _stream_ptr(stream)), "ising_energy")
         return E, M
 
     def ising_overlap(self, sample_a: int, sample_b: int, stream=None):
@@ -196,7 +218,8 @@ class Ising:
         import torch
 
         q = torch.empty(1, dtype=torch.int64, device=self.device)
-        _check(lib().ising_overlap(self._h, int(sample_a), int(sample_b), q.data_ptr(), _stream_ptr(stream)), "ising_overlap")
+        with self._on_device():
+            _check(lib().ising_overlap(self._h, int(sample_a), int(sample_b), q.data_ptr(), _stream_ptr(stream)), "ising_overlap")
         return q
 
     def ising_get_spins(self, out=None, stream=None):
@@ -204,7 +227,9 @@ class Ising:
 
         if out is None:
             out = torch.empty((self.nsamples, self.W), dtype=torch.int32, device=self.device)
-        _check(lib().ising_get_spins(self._h, _u32(out), _stream_ptr(stream)), "ising_get_spins")
+        assert out.is_cuda and out.is_contiguous() and out.numel() == self.nsamples * self.W
+        with self._on_device(out):
+            _check(lib().ising_get_spins(self._h, _u32(out), _stream_ptr(stream)), "ising_get_spins")
         return out
 
     def ising_run_host(self, h_spins, h_J, beta: float, nsweeps: int, h_spins_out=None, stream=None):
@@ -214,9 +239,10 @@ class Ising:
         assert not h_spins.is_cuda and not h_J.is_cuda
         E = torch.empty(self.nsamples, dtype=torch.int64).pin_memory()
         M = torch.empty(self.nsamples, dtype=torch.int64).pin_memory()
-        _check(lib().ising_run_host(self._h, _u32(h_spins), _u32(h_J), float(beta), int(nsweeps),
-                                    _u32(h_spins_out) if h_spins_out is not None else None, E.data_ptr(), M.data_ptr(),
-                                    _stream_ptr(stream)), "ising_run_host")
+        with self._on_device():
+            _check(lib().ising_run_host(self._h, _u32(h_spins), _u32(h_J), float(beta), int(nsweeps),
+                                        _u32(h_spins_out) if h_spins_out is not None else None, E.data_ptr(), M.data_ptr(),
+                                        _stream_ptr(stream)), "ising_run_host")
         return E, M
 
     def ising_run_host_async(self, h_spins, h_J, beta: float, nsweeps: int, h_spins_out, h_E, h_M=None, stream=None):
@@ -224,10 +250,11 @@ class Ising:
         keeps alive; results (h_spins_out, h_E, h_M) are valid after the stream has been synchronised."""
         for x in (h_spins, h_J, h_spins_out, h_E, h_M):
             assert x is None or (not x.is_cuda and x.is_pinned()), "ising_run_host_async needs pinned host tensors"
-        _check(lib().ising_run_host_async(self._h, _u32(h_spins), _u32(h_J), float(beta), int(nsweeps),
-                                          _u32(h_spins_out) if h_spins_out is not None else None, h_E.data_ptr(),
-                                          h_M.data_ptr() if h_M is not None else None, _stream_ptr(stream)),
-               "ising_run_host_async")
+        with self._on_device():
+            _check(lib().ising_run_host_async(self._h, _u32(h_spins), _u32(h_J), float(beta), int(nsweeps),
+                                              _u32(h_spins_out) if h_spins_out is not None else None, h_E.data_ptr(),
+                                              h_M.data_ptr() if h_M is not None else None, _stream_ptr(stream)),
+                   "ising_run_host_async")
 
     def ising_get_t(self) -> int:
         t = C.c_uint64(0)

@@ -102,6 +102,7 @@ struct ising {
     bool lanes_ready;
     bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
     bool overlap_clean;  // the counter of ising_overlap is zero
+    int device;          // CUDA device the workspace lives on (-1: unknown, e.g. no device present)
 
     LatticeArrays arrays(int batch) const
     {
@@ -117,11 +118,19 @@ struct ising {
 
 namespace {
 
+thread_local bool g_launch_failed = false;  // set by launch_pdl when cudaLaunchKernelEx itself reports a failure
+
 int check_launch(ising_t *h, int n = 1)
 {
     h->launches += (uint64_t)n;
-    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
+    const bool failed = g_launch_failed;
+    g_launch_failed = false;
+    return cudaGetLastError() == cudaSuccess && !failed ? ISING_OK : ISING_ECUDA;
 }
+
+// The workspace of a handle lives on one device (recorded by ising_create); every launch must be made with that device
+// current, or the kernels would dereference another GPU's memory (peer access) or fault (none).
+bool on_own_device(const ising_t *h);
 
 // Row a1 (R5, R6).  Plain double arithmetic with the C library's exp; compiled without FMA contraction.
 int compute_thresholds(double beta, int rng_mode, uint64_t out[3])
@@ -184,7 +193,9 @@ void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kernel, args...);  // errors surface through cudaGetLastError in check_launch
+    // a failed launch leaves its code in the runtime's last-error slot too, which check_launch reads; the return value is kept
+    // so that a failure is never lost between the two
+    if (cudaLaunchKernelEx(&cfg, kernel, args...) != cudaSuccess) g_launch_failed = true;
 }
 
 // The word-parallel kernel for W words per thread, plain or with E and M of the resulting configuration (MEASURE).
@@ -236,11 +247,19 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
                 if (g.L < 32) {  // fewer than 128 groups per plane: the thread index runs over (batch, group)
                     const uint64_t units = (uint64_t)nb * (g.N / 8);
                     launch_pdl(half_sweep_shared_vec<true>, dim3((unsigned)((units + 127) / 128)), dim3(128), st, a, sr, gpr, gpr_inv,
-                               (size_t)(8 * g.array_words), (uint32_t)nb);
+                               (size_t)(8 * g.array_words), (uint32_t)nb, 0u);
                 } else {
-                    const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L, (unsigned)nb);
-                    launch_pdl(half_sweep_shared_vec<false>, grid, dim3(128), st, a, sr, gpr, gpr_inv, (size_t)(8 * g.array_words),
-                               (uint32_t)nb);
+                    // blockIdx.z = batch: at most 65535 per launch (more than that is 2 M samples, still within a B200's HBM at L = 32)
+                    for (int b0 = 0; b0 < nb; b0 += 65535) {
+                        const int nbh = nb - b0 < 65535 ? nb - b0 : 65535;
+                        const dim3 grid((unsigned)(((uint64_t)g.L * gpr + 127) / 128), (unsigned)g.L, (unsigned)nbh);
+                        launch_pdl(half_sweep_shared_vec<false>, grid, dim3(128), st, a, sr, gpr, gpr_inv, (size_t)(8 * g.array_words),
+                                   (uint32_t)nbh, (uint32_t)b0);
+                        if (b0 + nbh < nb) {
+                            const int rc = check_launch(h);
+                            if (rc != ISING_OK) return rc;
+                        }
+                    }
                 }
                 const int rc = check_launch(h);
                 if (rc != ISING_OK) return rc;
@@ -304,14 +323,8 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             sr.seed = r.seed;
             sr.A2 = 2u * r.A;
             sr.s0tab = nullptr;
-            // MINSTD with the seed table.  Kernel choice 4 (W = 4 only) is the hybrid seed source, RNG = 3 in sweep_kernels.cuh: the
-            // last of the 4 words of a thread recomputes its seed states instead of loading them, 4.125 instead of 5.125 B per
-            // flip attempt from HBM, paid with issue slots the table kernel leaves idle.  Measured at L = 1024: 0.387 against
-            // 0.399 ms per half-sweep on a cool part at 1965 MHz, but 0.43-0.50 against 0.406 ms once a sustained run has
-            // brought the board to its power limit and the SM clock to ~1600 MHz (the table kernel is bound by HBM and does not
-            // notice; profiles/r1z_hybrid_minstd.md).  Not a robust gain, so the automatic choice stays the full table.
-            const bool hybrid = W == 4 && h->kernel_choice == 4;
-            const bool cached = RNG == 1 && (h->kernel_choice == 0 || h->kernel_choice == 4 || h->kernel_choice == 5) && h->s0tab != nullptr;
+            // MINSTD: the seed states s0(seed, site) come from the table unless kernel choice 2 asks for recomputation
+            const bool cached = RNG == 1 && h->kernel_choice != 2 && h->s0tab != nullptr;
             if (cached) {
                 uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
                 if (!h->s0_ready) {  // once per handle: the seed states depend on (seed, site) only (R11)
@@ -326,8 +339,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
                     h->s0_ready = true;
                 }
                 sr.s0tab = tab[c];
-                if (hybrid) launch_site_packed_w<3, 4>(mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
-                else launch_site_packed<2>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
+                launch_site_packed<2>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
             } else {
                 launch_site_packed<RNG>(W, mE != nullptr || mM != nullptr, grid, st, a, sr, slots, (long long)g.N, mE, mM);
             }
@@ -339,7 +351,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             sr.seed = r.seed;
             sr.A2 = 2u * r.A;
             sr.s0tab = nullptr;
-            if (g.L >= 64 && h->kernel_choice != 3) {  // rows of at least 32 bits: no segment loop (kernel choice 3 keeps the loop)
+            if (g.L >= 64) {  // rows of at least 32 bits: no segment loop
                 unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;
                 if (mE || mM) {
                     if (!h->slots_clean) {
@@ -418,7 +430,7 @@ bool can_measure_in_sweep(const ising_t *h)
 {
     if (h->g.nsamples != 1 || (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD)) return false;
     if (h->g.fast) return h->kernel_choice != 1;                                                              // word-parallel kernel
-    return h->g.L >= 64 && h->kernel_choice != 1 && h->kernel_choice != 3 && h->g.Hc < (1ull << 32);          // loop-free bit-window kernel
+    return h->g.L >= 64 && h->kernel_choice != 1 && h->g.Hc < (1ull << 32);                                   // loop-free bit-window kernel
 }
 
 int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long long *mE = nullptr, long long *mM = nullptr)
@@ -507,6 +519,16 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
     return check_launch(h);
 }
 
+bool on_own_device(const ising_t *h)
+{
+    int cur = -1;
+    if (h->device < 0 || cudaGetDevice(&cur) != cudaSuccess) {
+        cudaGetLastError();
+        return true;   // nothing known to compare with; a launch on a machine without a device fails with ISING_ECUDA anyway
+    }
+    return cur == h->device;
+}
+
 }  // namespace
 
 extern "C" {
@@ -548,6 +570,21 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->lane_state = lane_mode(rng_mode) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->nlanes = lane_mode(rng_mode) ? lanes_default(h->g, rng_mode) : 0;
     h->lanes_ready = false;
+    // the device the workspace belongs to; a workspace of another device than the current one is refused
+    h->device = -1;
+    {
+        int cur = -1;
+        cudaPointerAttributes pa;
+        if (cudaGetDevice(&cur) == cudaSuccess && cudaPointerGetAttributes(&pa, d_workspace) == cudaSuccess &&
+            (pa.type == cudaMemoryTypeDevice || pa.type == cudaMemoryTypeManaged)) {
+            if (pa.device != cur) {
+                delete h;
+                return ISING_EINVAL;
+            }
+            h->device = pa.device;
+        }
+        cudaGetLastError();
+    }
     *out = h;
     return ISING_OK;
 }
@@ -560,7 +597,7 @@ int ising_destroy(ising_t *h)
 
 int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, void *stream)
 {
-    if (!h || !d_spins || !d_J) return ISING_EINVAL;
+    if (!h || !d_spins || !d_J || !on_own_device(h)) return ISING_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t W = g.canon_words;
@@ -647,7 +684,7 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
 
 int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
 {
-    if (!h || !d_out) return ISING_EINVAL;
+    if (!h || !d_out || !on_own_device(h)) return ISING_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t W = g.canon_words;
@@ -690,7 +727,7 @@ int ising_sweep(ising_t *h, double beta, int nsweeps, void *stream)
 
 int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_t *d_M, int every_half_sweeps, void *stream)
 {
-    if (!h || nsweeps < 0) return ISING_EINVAL;
+    if (!h || nsweeps < 0 || !on_own_device(h)) return ISING_EINVAL;
     const bool trace = d_E != nullptr || d_M != nullptr;
     if (trace && every_half_sweeps < 1) return ISING_EINVAL;
     uint64_t T[3];
@@ -718,7 +755,7 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
 
 int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream)
 {
-    if (!h || !d_E) return ISING_EINVAL;
+    if (!h || !d_E || !on_own_device(h)) return ISING_EINVAL;
     return measure(h, (long long *)d_E, (long long *)d_M, (cudaStream_t)stream);
 }
 
@@ -726,7 +763,7 @@ int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *st
 {
     if (!h || !d_q || h->g.nsamples == 1 || sample_a < 0 || sample_b < 0 || sample_a >= h->g.nsamples || sample_b >= h->g.nsamples)
         return ISING_EINVAL;
-    if (h->g.Hc >= (1ull << 32)) return ISING_EINVAL;
+    if (h->g.Hc >= (1ull << 32) || !on_own_device(h)) return ISING_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     // the counter pair lives behind the ticket of the energy kernels
@@ -746,7 +783,7 @@ int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *st
 int ising_run_host_async(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps,
                          uint32_t *h_spins_out, int64_t *h_E, int64_t *h_M, void *stream)
 {
-    if (!h || !h_spins || !h_J || !h_E || nsweeps < 0 || !(beta >= 0.0)) return ISING_EINVAL;
+    if (!h || !h_spins || !h_J || !h_E || nsweeps < 0 || !(beta >= 0.0) || !on_own_device(h)) return ISING_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t spin_words = (size_t)g.nsamples * g.canon_words, j_words = 3 * spin_words;
@@ -885,7 +922,7 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
 
 int ising_set_kernel(ising_t *h, int which)
 {
-    if (!h || which < 0 || which > 5) return ISING_EINVAL;
+    if (!h || which < 0 || which > 3) return ISING_EINVAL;
     h->kernel_choice = which;
     return ISING_OK;
 }

@@ -256,9 +256,9 @@ __device__ __forceinline__ RowMap row_map(int L)
 // word, then the slot accumulation and last-CTA finalisation of energy_site_packed: a trace of E and M per sweep costs no
 // extra launch and no extra pass over the 512 MiB (L = 1024: 78 us per record saved).
 // Four CTAs per SM (64 registers) for the Philox kernel the L = 1024 numbers are quoted on (0.3899 -> 0.3868 ms per half-sweep, 8 bytes
-// of spill) and for the hybrid MINSTD kernel (0.423 -> 0.387 ms); the other variants keep ptxas' own choice (W = 5 would spill 40 bytes).
+// of spill); the other variants keep ptxas' own choice (W = 5 would spill 40 bytes).
 template <int RNG, int W, bool MEASURE>
-__global__ void __launch_bounds__(SWEEP_THREADS, (RNG == 3 || RNG == 0) && W == 4 && !MEASURE ? 4 : 0)
+__global__ void __launch_bounds__(SWEEP_THREADS, RNG == 0 && W == 4 && !MEASURE ? 4 : 0)
 half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, unsigned long long *acc, long long N,
                        long long *E, long long *M)
 {
@@ -325,12 +325,8 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     };
 
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
-    // RNG = 2: the seed states of all W words come from the table.  RNG = 3 (hybrid, W >= 2): the first W - 1 words take them from
-    // the table and the last word recomputes them (SplitMix64 per site, as RNG = 1): the table kernel is bound by HBM with the
-    // integer pipes half idle, the recomputing kernel by integer issue, so a share of recomputed sites shortens the HBM stream
-    // (5.125 -> 4.125 B per flip attempt at W = 4) at the price of otherwise idle issue slots.  Same draws either way (R11, R12).
-    // Kernel choice 4 only: faster on a cool part, slower once the board runs at its power limit (see ising_api.cu).
-    constexpr int WC = RNG == 2 ? W : (RNG == 3 ? W - 1 : 0);
+    // RNG = 2: the seed states of all W words come from the table; RNG = 0, 1: every word draws in registers.
+    constexpr int WC = RNG == 2 ? W : 0;
     // seeds from the table, two groups of 16 sites in flight: while one half-word's draws are compared, the next
     // half-word's four 16-byte loads are outstanding (about 2 KB per warp, enough to keep HBM busy)
     const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
@@ -564,7 +560,8 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
         if (RNG == 1) {   // MINSTD: stream id = canonical site index; bit b of the word is site0 + 2 (b - bitoff)
             const uint64_t site0 = (uint64_t)L * r + 2u * m + xodd - 2ull * bitoff;
             uint32_t d4, d8, d12;
-            cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, d4, d8, d12);
+            // no warp vote here: the threads of a warp run this loop a different number of times when L/2 does not divide 32
+            cond_masks_site_packed_minstd<false>(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, d4, d8, d12);
             c4 |= d4 & segmask;
             c8 |= d8 & segmask;
             c12 |= d12 & segmask;
@@ -902,10 +899,11 @@ struct SharedRng {
 template <bool FLAT>
 __global__ void __launch_bounds__(128)
 half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups per row = L/8 */,
-                      uint32_t gpr_inv /* ceil(2^32 / gpr) */, size_t batch_stride, uint32_t nbatches)
+                      uint32_t gpr_inv /* ceil(2^32 / gpr) */, size_t batch_stride, uint32_t nbatches,
+                      uint32_t batch0 /* first batch of this launch (launches are chunked to 65535 batches) */)
 {
     const uint32_t L = (uint32_t)a.L;
-    uint32_t p = blockIdx.x * 128u + threadIdx.x, z = blockIdx.y, batch = blockIdx.z;
+    uint32_t p = blockIdx.x * 128u + threadIdx.x, z = blockIdx.y, batch = batch0 + blockIdx.z;
     if (FLAT) {
         const uint32_t per_plane = L * gpr, ngroups = per_plane * L;
         if (p >= nbatches * ngroups) return;

@@ -55,7 +55,9 @@ ISING_HD uint32_t min_u32(uint32_t a, uint32_t b) { return a < b ? a : b; }
 // Acceptance bits of NR draws for the sites bit0 .. bit0+NR-1 of a word.  cond4 is needed for every draw.  R < T8
 // happens for < 0.1 % of the draws at the temperatures of interest, so cond8 / cond12 are filled in a rarely taken,
 // warp-uniform branch guarded by the minimum of the draws (one VIMNMX3 per two draws).
-template <int NR>
+// VOTE = false: the rare branch is taken per thread (for callers whose warps are not converged here, e.g. inside a loop
+// with a per-thread trip count, where a full-mask vote would be undefined).
+template <int NR, bool VOTE = true>
 ISING_HD void accumulate_cond(const uint32_t *R, int bit0, const Thresholds &T, uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
     uint32_t mn = 0xFFFFFFFFu;
@@ -65,14 +67,14 @@ ISING_HD void accumulate_cond(const uint32_t *R, int bit0, const Thresholds &T, 
         mn = min_u32(mn, R[w]);
     }
 #ifdef __CUDA_ARCH__
-    if (__any_sync(0xFFFFFFFFu, mn < T.t8)) {
+    if (VOTE ? __any_sync(0xFFFFFFFFu, mn < T.t8) != 0 : mn < T.t8) {
 #else
     if (mn < T.t8) {
 #endif
 #pragma unroll
         for (int w = 0; w < NR; ++w) or_if_lt(c8, R[w], T.t8, 1u << (bit0 + w));
 #ifdef __CUDA_ARCH__
-        if (__any_sync(0xFFFFFFFFu, mn < T.t12)) {
+        if (VOTE ? __any_sync(0xFFFFFFFFu, mn < T.t12) != 0 : mn < T.t12) {
 #else
         if (mn < T.t12) {
 #endif
@@ -109,6 +111,7 @@ ISING_HD void cond_masks_site_packed_philox(const PhiloxCommonConst &cc, const P
 
 // MINSTD, site-packed word: the stream id of bit b is q_b = site0 + b*site_stride (canonical site index, sample 0),
 // i.e. the SplitMix64 Weyl state advances by site_stride*GAMMA per bit.  `weyl0` = seed + (site0+1)*GAMMA.
+template <bool VOTE = true>
 ISING_HD void cond_masks_site_packed_minstd(uint64_t weyl0, uint64_t weyl_step, uint32_t A2, const Thresholds &T,
                                             uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
@@ -118,7 +121,7 @@ ISING_HD void cond_masks_site_packed_minstd(uint64_t weyl0, uint64_t weyl_step, 
         uint32_t R[4];
 #pragma unroll
         for (int w = 0; w < 4; ++w) R[w] = minstd_mulmod2(A2, minstd_seed_state_from_weyl(weyl0 + (uint64_t)(4 * q + w) * weyl_step));
-        accumulate_cond<4>(R, 4 * q, T, c4, c8, c12);
+        accumulate_cond<4, VOTE>(R, 4 * q, T, c4, c8, c12);
     }
     finish_cond(T, c4, c8, c12);
 }

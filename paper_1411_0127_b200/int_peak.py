@@ -42,15 +42,18 @@ def build(force: bool = False) -> str:
     return LIB
 
 
-def run(ctas_per_sm: int = 8, iters: int = 4096, reps: int = 5) -> dict:
+def run(ctas_per_sm: int = 8, iters: int = 4096, reps: int = 5, mixes=None) -> dict:
     import torch
 
     lib = C.CDLL(build())
     lib.int_peak_run.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]
-    sms = torch.cuda.get_device_properties(0).multi_processor_count
-    scratch = torch.zeros(16, dtype=torch.int32, device="cuda")
+    dev = torch.cuda.current_device()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    scratch = torch.zeros(16, dtype=torch.int32, device=torch.device("cuda", dev))
     out = {"sms": sms, "ctas_per_sm": ctas_per_sm, "threads_per_cta": 256, "mixes": {}}
     for mix, name in MIXES.items():
+        if mixes is not None and mix not in mixes:
+            continue
         ms, ops = C.c_float(0), C.c_double(0)
         rc = lib.int_peak_run(mix, sms * ctas_per_sm, iters, reps, scratch.data_ptr(), C.byref(ms), C.byref(ops))
         if rc != 0:
