@@ -207,6 +207,9 @@ def main():
     ap.add_argument("--aux", action="store_true",
                     help="rows a9 / a10 and the general-L kernels: load_state, energy, get_spins and a half-sweep per layout, with GB/s")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
+    ap.add_argument("--small", action="store_true",
+                    help="small lattices: time per half-sweep with the automatic kernels (0), one launch per half-sweep (3) and the "
+                         "persistent kernels everywhere (4), without records and with E and M after every half-sweep")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -425,6 +428,40 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.small:
+        rows = []
+        for Ls in (8, 16, 24, 32, 40, 64, 128, 192, 256, 320, 384, 448):
+            sp = torch.from_numpy(synth.make_spins(Ls, 1).view(np.int32)).cuda()
+            Jc = torch.from_numpy(synth.make_couplings(Ls, 1).view(np.int32)).cuda()
+            for mode in (PHILOX, MINSTD):
+                row = {"L": Ls, "rng_mode": ["philox", "minstd"][mode]}
+                for every in (0, 1):
+                    for choice in (0, 3, 4):
+                        g = Ising(Ls, 1, synth.DYN_SEED, mode)
+                        g.ising_set_kernel(choice)
+                        g.ising_load_state(sp, Jc)
+                        g.ising_sweep(BETA, 2)
+                        nsweeps = 500 if Ls <= 256 else 100
+                        best = None
+                        for _ in range(3):
+                            torch.cuda.synchronize()
+                            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                            a.record(stream)
+                            if every:
+                                g.ising_sweep_trace(BETA, nsweeps, every_half_sweeps=every)
+                            else:
+                                g.ising_sweep(BETA, nsweeps)
+                            b.record(stream)
+                            torch.cuda.synchronize()
+                            ms = a.elapsed_time(b)
+                            best = ms if best is None or ms < best else best
+                        g.ising_destroy()
+                        row[("recorded_" if every else "") + {0: "automatic", 3: "launch_per_half_sweep", 4: "persistent"}[choice] + "_us"] = \
+                            round(1e3 * best / (2 * nsweeps), 3)
+                rows.append(row)
+        print(json.dumps({"small": rows}))
         return
 
     if args.configs:  # BASELINE.json configs 1-5 as written: sweeps, and the observables each one records, inside the timed region

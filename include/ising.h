@@ -183,8 +183,11 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
  * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
  * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),
  * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = as 0 but always one launch per
- * colour half-sweep (never the persistent kernel that 0 uses for lattices resident in the L2).  All give the same bits; the
- * tests use this to show that results do not depend on layout, thread mapping or caching. */
+ * colour half-sweep, 4 = as 0 but the persistent kernels wherever they exist.  (0 runs all half-sweeps of a call in one launch
+ * where that is faster: one-sample lattices of at most 1024 words per colour, i.e. every even L <= 40, on one SM out of shared
+ * memory; recorded calls, ising_sweep_trace, at L = 64 and 128 as a dataflow of co-resident CTAs; 4 extends the latter to every
+ * call and every multiple of 64 below 512.)  All give the same bits; the tests use this to show that results do not depend on
+ * layout, thread mapping, caching or launch structure. */
 int ising_set_kernel(ising_t *h, int which);
 
 /* Number of kernels this handle has launched so far. */

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libising_b200.so")
 STAMP = LIB + ".srchash"  # git-ignored with the .so; travels with it to the GPU box
 SOURCES = ["ising_api.cu"]
-HEADERS = ["rng.cuh", "update.cuh", "sweep_kernels.cuh", "measure_kernels.cuh", "layout_kernels.cuh", "lane_rng.cuh",
+HEADERS = ["rng.cuh", "update.cuh", "sweep_kernels.cuh", "persistent.cuh", "measure_kernels.cuh", "layout_kernels.cuh", "lane_rng.cuh",
            os.path.join("..", "..", "include", "ising.h")]
 
 
@@ -21,7 +21,7 @@ def nvcc_path() -> str:
 def nvcc_command(out: str = LIB, extra: list[str] | None = None) -> list[str]:
     return [nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
             # the threshold table must be plain double arithmetic (R5): no FMA contraction on the host
-            "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", "-shared", "-o", out,
+            "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-shared", "-o", out,
             *[os.path.join(CSRC, s) for s in SOURCES], *(extra or [])]
 
 

@@ -10,6 +10,7 @@
 #include "lane_rng.cuh"
 #include "layout_kernels.cuh"
 #include "measure_kernels.cuh"
+#include "persistent.cuh"
 #include "sweep_kernels.cuh"
 
 using namespace isingk;
@@ -30,6 +31,9 @@ struct Geometry {
     size_t staging_words;       // canonical spins + couplings of all samples
     size_t acc_bytes;
     size_t s0_words;            // cached MINSTD seed states: 32 words per word of each colour array (fast layout only)
+    size_t epoch_words;         // tile epochs of the persistent kernels (0: this geometry has no persistent path)
+    uint32_t pgx, pgy;          // their tile grid
+    bool onchip;                // small enough for half_sweeps_on_chip (one CTA, the lattice in shared memory)
     bool fast;                  // half-rows are whole words: L is a multiple of 64
     int W;                      // words per thread of the word-parallel kernel (fast layout)
 };
@@ -64,7 +68,8 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
     // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs and the ticket of the word-parallel energy kernel
-    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1 + 2) * sizeof(unsigned long long), 256);  // + overlap counter
+    // ... + overlap counter (2)
+    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1 + 2) * sizeof(unsigned long long), 256);
     g->fast = nsamples == 1 && L % 64 == 0;
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
     // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
@@ -80,6 +85,17 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     // cached MINSTD seed states: 2 colours x one 4-byte word per site of every thread of the word-parallel grid (rows
     // whose lane count is not a power of two are padded, RowMap in sweep_kernels.cuh); N words when L = 64*2^k
     g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
+    // persistent paths (persistent.cuh): one-sample lattices with whole-word rows below L = 512 get a tile grid with epoch counters
+    // (used automatically up to L = 128, where it beats the launches); one-sample lattices of at most 1024 words per colour that
+    // are not of that kind (every other even L <= 40) run on one SM out of shared memory
+    g->epoch_words = 0;
+    g->pgx = g->pgy = 0;
+    if (g->fast && g->W != 4) {
+        g->pgx = (uint32_t)(L / (32 / row_map_tpr_pad((L >> 6) / g->W)));
+        g->pgy = (uint32_t)(L / (SWEEP_THREADS / 32));
+        g->epoch_words = (size_t)g->pgx * g->pgy;
+    }
+    g->onchip = nsamples == 1 && !g->fast && (g->Hc + 31) / 32 <= ONCHIP_MAX_WORDS;
     return true;
 }
 
@@ -103,6 +119,8 @@ struct ising {
     bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
     bool overlap_clean;  // the counter of ising_overlap is zero
     int device;          // CUDA device the workspace lives on (-1: unknown, e.g. no device present)
+    unsigned int *epochs;  // tile epochs of the persistent kernels (nullptr: no persistent path for this geometry / mode)
+    int persist_grid[2];   // co-resident CTAs of this handle's persistent kernel without / with records (0: not asked yet, -1: none)
 
     LatticeArrays arrays(int batch) const
     {
@@ -441,6 +459,154 @@ int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long long *mE =
     return h->rng_mode == ISING_RNG_PHILOX ? launch_half_sweep<0>(h, T, st, mE, mM) : launch_half_sweep<1>(h, T, st, mE, mM);
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Persistent path (persistent.cuh): all half-sweeps of a call in one cooperative launch, the CTAs synchronising tile by tile
+// through epoch counters.  Automatic (kernel choice 0 or 2) for the geometries make_geometry gives a tile grid.
+// ---------------------------------------------------------------------------------------------------------------------
+// `records`: the call records E / M (ising_sweep_trace).
+bool persistent_available(const ising_t *h, bool records)
+{
+    if (h->g.nsamples != 1 || (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD)) return false;
+    if (h->g.onchip) return h->kernel_choice == 0 || h->kernel_choice == 2 || h->kernel_choice == 4;
+    if (!h->epochs) return false;
+    if (h->kernel_choice == 4) return true;                                      // wherever there is a tile grid (L <= 448)
+    // automatic: where it beats the launches (profiles/r2b_persistent.md).  Without records the tile flags cost what the launch
+    // gap costs (2.3-2.6 us per half-sweep either way at L = 64, 128) and the launches win from L = 192 on; with records the
+    // persistent kernel's atomics into the record beat the last-CTA finalisation of a recording launch (3.2 against 4.5 us).
+    return (h->kernel_choice == 0 || h->kernel_choice == 2) && h->g.L <= 128 && records;
+}
+
+template <typename Kernel>
+int launch_cooperative(ising_t *h, Kernel kernel, int threads, int which, const PersistArgs &p, uint32_t ntiles, cudaStream_t st)
+{
+    if (h->persist_grid[which] == 0) {   // once per handle: how many CTAs of this kernel are resident at once
+        int per_sm = 0, sms = 0, dev = 0, coop = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess)
+            return ISING_ECUDA;
+        h->persist_grid[which] = coop && per_sm > 0 ? per_sm * sms : -1;
+    }
+    if (h->persist_grid[which] < 0) return ISING_EINVAL;
+    // every CTA walks over the same number of tiles (1024 tiles on 740 resident CTAs: 512 CTAs x 2 tiles, not 740 x 1.4)
+    const uint32_t cap = (uint32_t)h->persist_grid[which], rounds = (ntiles + cap - 1) / cap;
+    const unsigned grid = (ntiles + rounds - 1) / rounds;
+    uint32_t gx = h->g.pgx, gy = h->g.pgy;
+    void *args[] = {(void *)&p, (void *)&gx, (void *)&gy};
+    if (cudaLaunchCooperativeKernel((const void *)kernel, dim3(grid), dim3((unsigned)threads), args, 0, st) != cudaSuccess) {
+        cudaGetLastError();
+        return ISING_ECUDA;
+    }
+    return check_launch(h);
+}
+
+template <int RNG, int W>
+int launch_persistent_site(ising_t *h, const PersistArgs &p, bool records, cudaStream_t st)
+{
+    const uint32_t ntiles = h->g.pgx * h->g.pgy;
+    if (records) return launch_cooperative(h, persistent_site_packed<RNG, W, true>, SWEEP_THREADS, 1, p, ntiles, st);
+    return launch_cooperative(h, persistent_site_packed<RNG, W, false>, SWEEP_THREADS, 0, p, ntiles, st);
+}
+template <int RNG>
+int launch_persistent_site(ising_t *h, const PersistArgs &p, bool records, cudaStream_t st)
+{
+    switch (h->g.W) {
+        case 1: return launch_persistent_site<RNG, 1>(h, p, records, st);
+        case 3: return launch_persistent_site<RNG, 3>(h, p, records, st);
+        case 5: return launch_persistent_site<RNG, 5>(h, p, records, st);
+        default: return ISING_EINVAL;
+    }
+}
+
+// nhalf half-sweeps from the handle's counter on; site-packed handles record E / M after every `every`-th (0: none) into d_E / d_M.
+int sweep_persistent(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t every, long long *d_E, long long *d_M, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    if (g.onchip) {   // one CTA, the lattice in shared memory, every half-sweep and record of the call in one launch
+        PersistArgs p;
+        memset(&p, 0, sizeof(p));
+        p.A = h->arrays(0);
+        p.L = g.L;
+        p.T = T;
+        p.seed = h->seed;
+        p.t0 = h->t;
+        p.nhalf = nhalf;
+        p.every = (d_E || d_M) ? every : 0u;
+        p.A_first = h->rng_mode == ISING_RNG_MINSTD ? minstd_power((h->t >> 1) + 1) : 0u;
+        p.E = d_E;
+        p.M = d_M;
+        p.N = g.N;
+        const uint32_t nw = (uint32_t)((g.Hc + 31) / 32);
+        const size_t smem = 8 * (size_t)(nw + 1) * sizeof(uint32_t);
+        if (h->rng_mode == ISING_RNG_PHILOX) half_sweeps_on_chip<0><<<1, ONCHIP_THREADS, smem, st>>>(p, nw, (uint32_t)g.Hc);
+        else half_sweeps_on_chip<1><<<1, ONCHIP_THREADS, smem, st>>>(p, nw, (uint32_t)g.Hc);
+        const int rc = check_launch(h);
+        if (rc == ISING_OK) h->t += nhalf;
+        return rc;
+    }
+    const bool site = true;
+    const bool table = site && h->rng_mode == ISING_RNG_MINSTD && h->kernel_choice != 2 && h->s0tab != nullptr;
+    uint4 *tab[2] = {nullptr, nullptr};
+    if (table) {
+        tab[0] = (uint4 *)h->s0tab;
+        tab[1] = (uint4 *)(h->s0tab + g.s0_words / 2);
+        if (!h->s0_ready) {
+            const dim3 grid(g.pgx, g.pgy);
+            for (int cc = 0; cc < 2; ++cc) {
+                if (g.W == 3) minstd_fill_s0<3><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                else if (g.W == 5) minstd_fill_s0<5><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+                else minstd_fill_s0<1><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed);
+            }
+            const int rc = check_launch(h, 2);
+            if (rc != ISING_OK) return rc;
+            h->s0_ready = true;
+        }
+    }
+    const bool records = site && every != 0 && (d_E || d_M);
+    if (records) {   // the records receive their counts by atomics: preset them to -3N / -N
+        const uint32_t nrec = nhalf / every;
+        if (nrec) {
+            init_records<<<(nrec + 255) / 256, 256, 0, st>>>(d_E, d_M, nrec, (long long)g.N);
+            const int rc = check_launch(h);
+            if (rc != ISING_OK) return rc;
+        }
+    }
+    // epochs are 32-bit and restart with every launch: at most 2^30 half-sweeps per launch; a chunk ends on a record boundary so
+    // that `every` keeps its phase
+    uint32_t chunk_max = 1u << 30;
+    if (records) chunk_max -= chunk_max % every;
+    uint32_t done = 0, rec = 0;
+    while (done < nhalf) {
+        const uint32_t n = nhalf - done < chunk_max ? nhalf - done : chunk_max;
+        PersistArgs p;
+        memset(&p, 0, sizeof(p));
+        p.A = h->arrays(0);
+        p.L = g.L;
+        p.T = T;
+        p.seed = h->seed;
+        p.t0 = h->t;
+        p.nhalf = n;
+        p.every = records ? every : 0u;
+        p.A_first = h->rng_mode == ISING_RNG_MINSTD ? minstd_power((h->t >> 1) + 1) : 0u;
+        p.s0tab[0] = tab[0];
+        p.s0tab[1] = tab[1];
+        p.epoch = h->epochs;
+        p.E = records && d_E ? d_E + rec : nullptr;
+        p.M = records && d_M ? d_M + rec : nullptr;
+        p.N = g.N;
+        if (cudaMemsetAsync(h->epochs, 0, g.epoch_words * sizeof(uint32_t), st) != cudaSuccess) return ISING_ECUDA;
+        int rc;
+        if (h->rng_mode == ISING_RNG_PHILOX) rc = launch_persistent_site<0>(h, p, records, st);
+        else if (table) rc = launch_persistent_site<2>(h, p, records, st);
+        else rc = launch_persistent_site<1>(h, p, records, st);
+        if (rc != ISING_OK) return rc;
+        h->t += n;
+        done += n;
+        if (records) rec += n / every;
+    }
+    return ISING_OK;
+}
+
 int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
 {
     const Geometry &g = h->g;
@@ -541,6 +707,7 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
     if (shared_mode(rng_mode) && nsamples % 32 != 0) return ISING_EINVAL;  // one draw per 32-sample word
     *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
     if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
+    *out += round_up(g.epoch_words * sizeof(uint32_t), 256);   // tile epochs of the persistent kernels (unused by the lane modes)
     if (lane_mode(rng_mode)) *out += round_up((size_t)lane_ring(rng_mode) * lanes_default(g, rng_mode) * sizeof(uint32_t), 256);
     return ISING_OK;
 }
@@ -570,6 +737,11 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->lane_state = lane_mode(rng_mode) ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->nlanes = lane_mode(rng_mode) ? lanes_default(h->g, rng_mode) : 0;
     h->lanes_ready = false;
+    h->persist_grid[0] = h->persist_grid[1] = 0;
+    h->epochs = nullptr;
+    if (h->g.epoch_words && !lane_mode(rng_mode)) {   // the last area of the workspace
+        h->epochs = (unsigned int *)((char *)d_workspace + need - round_up(h->g.epoch_words * sizeof(uint32_t), 256));
+    }
     // the device the workspace belongs to; a workspace of another device than the current one is refused
     h->device = -1;
     {
@@ -734,6 +906,11 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
     if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
     const Thresholds kt = kernel_thresholds(T);
     cudaStream_t st = (cudaStream_t)stream;
+    if (nsweeps >= 1 && persistent_available(h, trace)) {   // all half-sweeps of the call in one launch (persistent.cuh)
+        const uint32_t nhalf = 2u * (uint32_t)nsweeps;
+        const int rc = sweep_persistent(h, kt, nhalf, trace ? (uint32_t)every_half_sweeps : 0u, (long long *)d_E, (long long *)d_M, st);
+        if (rc != ISING_EINVAL) return rc;   // EINVAL (before anything ran): no cooperative launch on this device; use the launches
+    }
     size_t rec = 0;
     const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps write E and M themselves: no extra launch
     for (int k = 1; k <= 2 * nsweeps; ++k) {
@@ -922,7 +1099,7 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
 
 int ising_set_kernel(ising_t *h, int which)
 {
-    if (!h || which < 0 || which > 3) return ISING_EINVAL;
+    if (!h || which < 0 || which > 4) return ISING_EINVAL;
     h->kernel_choice = which;
     return ISING_OK;
 }

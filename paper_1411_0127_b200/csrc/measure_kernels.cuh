@@ -35,7 +35,7 @@ energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {
                    long long N, long long *E, long long *M)
 {
     const int L = a.L, wpr = L >> 6;
-    const RowMap rm = row_map<W>(L);
+    const RowMap rm = row_map<W>(L, blockIdx.x, blockIdx.y);
     const int tpr = rm.tpr, y = rm.y, z = rm.z, k0 = rm.k0;
     const int yp = y + 1 == L ? 0 : y + 1, zp = z + 1 == L ? 0 : z + 1;
     const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;
@@ -100,43 +100,52 @@ energy_site_packed_generic(const MeasureArgs a, unsigned long long *acc, uint64_
 
 // Site-packed, any even L: one thread per word; the +x / +y / +z neighbours of its row segments are unaligned bit windows
 // of the other colour's array (bit_window, as in half_sweep_site_packed_rows); three popcounts per segment.
+// item = word w of colour 0 (item < n_words) or of colour 1; adds the word's unsatisfied +x / +y / +z bonds and up spins.
+template <bool PLAIN>
+__device__ __forceinline__ void rows_energy_item(const MeasureArgs &a, uint32_t item, uint32_t n_words, uint32_t Hc, unsigned long long &unsat,
+                                                 unsigned long long &up)
+{
+    const uint32_t L = (uint32_t)a.L, H = L >> 1, LH = L * H;
+    const int c = item >= n_words;
+    const uint32_t w = item - (c ? n_words : 0u), j0 = 32u * w;
+    uint32_t remaining = Hc - j0 < 32u ? Hc - j0 : 32u, bitoff = 0;
+    uint32_t r = j0 / H, m = j0 - r * H, z = r / L, y = r - z * L;
+    // (selects, not run-time indices into the argument struct: a local copy of it would otherwise live in local memory)
+    const uint32_t *So = c ? a.S[0] : a.S[1], *Sc = c ? a.S[1] : a.S[0];
+    const uint32_t *Jxc = c ? a.J[0][1] : a.J[0][0], *Jyc = c ? a.J[1][1] : a.J[1][0], *Jzc = c ? a.J[2][1] : a.J[2][0];
+    const uint32_t s = load_word<PLAIN>(Sc, w), jx = load_word<PLAIN>(Jxc, w), jy = load_word<PLAIN>(Jyc, w), jz = load_word<PLAIN>(Jzc, w);
+    uint32_t nx = 0, ny = 0, nz = 0;
+    while (remaining > 0) {
+        const uint32_t len = remaining < H - m ? remaining : H - m;
+        const uint32_t segmask = (len == 32u ? 0xFFFFFFFFu : ((1u << len) - 1u)) << bitoff;
+        const uint32_t xodd = (y + z + (uint32_t)c) & 1u;
+        const uint32_t P = r * H;
+        const uint32_t Pyp = (y + 1 == L) ? P - (LH - H) : P + H, Pzp = (z + 1 == L) ? P - (Hc - LH) : P + LH;
+        uint32_t wpx = bit_window<PLAIN>(So, P + m + xodd);
+        if (xodd && m + len == H) wpx = (wpx & ~(1u << (len - 1))) | (bit_at<PLAIN>(So, P) << (len - 1));
+        nx |= (wpx << bitoff) & segmask;
+        ny |= (bit_window<PLAIN>(So, Pyp + m) << bitoff) & segmask;
+        nz |= (bit_window<PLAIN>(So, Pzp + m) << bitoff) & segmask;
+        bitoff += len;
+        remaining -= len;
+        m += len;
+        if (m == H) {
+            m = 0;
+            ++r;
+            if (++y == L) { y = 0; ++z; }
+        }
+    }
+    const uint32_t valid = bitoff == 32u ? 0xFFFFFFFFu : (1u << bitoff) - 1u;
+    unsat += __popc((jx ^ s ^ nx) & valid) + __popc((jy ^ s ^ ny) & valid) + __popc((jz ^ s ^ nz) & valid);
+    up += __popc(s & valid);
+}
+
 __global__ void __launch_bounds__(256)
 energy_site_packed_rows(const __grid_constant__ MeasureArgs a, unsigned long long *acc, uint32_t n_words, uint32_t Hc)
 {
-    const uint32_t L = (uint32_t)a.L, H = L >> 1, LH = L * H;
     unsigned long long unsat = 0, up = 0;
-    for (uint32_t tid = blockIdx.x * 256u + threadIdx.x; tid < 2 * n_words; tid += gridDim.x * 256u) {   // persistent grid
-        const int c = tid >= n_words;
-        const uint32_t w = tid - (c ? n_words : 0u), j0 = 32u * w;
-        uint32_t remaining = Hc - j0 < 32u ? Hc - j0 : 32u, bitoff = 0;
-        uint32_t r = j0 / H, m = j0 - r * H, z = r / L, y = r - z * L;
-        const uint32_t *__restrict__ So = a.S[1 - c];
-        const uint32_t s = __ldg(a.S[c] + w), jx = __ldg(a.J[0][c] + w), jy = __ldg(a.J[1][c] + w), jz = __ldg(a.J[2][c] + w);
-        uint32_t nx = 0, ny = 0, nz = 0;
-        while (remaining > 0) {
-            const uint32_t len = remaining < H - m ? remaining : H - m;
-            const uint32_t segmask = (len == 32u ? 0xFFFFFFFFu : ((1u << len) - 1u)) << bitoff;
-            const uint32_t xodd = (y + z + (uint32_t)c) & 1u;
-            const uint32_t P = r * H;
-            const uint32_t Pyp = (y + 1 == L) ? P - (LH - H) : P + H, Pzp = (z + 1 == L) ? P - (Hc - LH) : P + LH;
-            uint32_t wpx = bit_window(So, P + m + xodd);
-            if (xodd && m + len == H) wpx = (wpx & ~(1u << (len - 1))) | (bit_at(So, P) << (len - 1));
-            nx |= (wpx << bitoff) & segmask;
-            ny |= (bit_window(So, Pyp + m) << bitoff) & segmask;
-            nz |= (bit_window(So, Pzp + m) << bitoff) & segmask;
-            bitoff += len;
-            remaining -= len;
-            m += len;
-            if (m == H) {
-                m = 0;
-                ++r;
-                if (++y == L) { y = 0; ++z; }
-            }
-        }
-        const uint32_t valid = bitoff == 32u ? 0xFFFFFFFFu : (1u << bitoff) - 1u;
-        unsat += __popc((jx ^ s ^ nx) & valid) + __popc((jy ^ s ^ ny) & valid) + __popc((jz ^ s ^ nz) & valid);
-        up += __popc(s & valid);
-    }
+    for (uint32_t tid = blockIdx.x * 256u + threadIdx.x; tid < 2 * n_words; tid += gridDim.x * 256u)   // persistent grid
+        rows_energy_item<false>(a, tid, n_words, Hc, unsat, up);
     block_accumulate2(unsat, up, acc);
 }
 

@@ -61,7 +61,7 @@ struct PhiloxCommonConst {
     uint32_t k0[7];  // K0_3 .. K0_9
 };
 
-inline void fold_philox(uint64_t seed, uint32_t sample, uint64_t t, PhiloxCommonConst *cc, PhiloxSampleConst *sc)
+ISING_HD void fold_philox(uint64_t seed, uint32_t sample, uint64_t t, PhiloxCommonConst *cc, PhiloxSampleConst *sc)
 {
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32) ^ sample;
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);

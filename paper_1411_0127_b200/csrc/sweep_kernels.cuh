@@ -148,6 +148,27 @@ __device__ __forceinline__ void load_words(const uint32_t *__restrict__ p, size_
     }
 }
 
+// Spin words.  COHERENT = false: the read-only path (ld.global.nc), for kernels that run one half-sweep per launch.
+// COHERENT = true: ld.global.cg (served by the L2, the point of coherence), for the persistent kernels in which other CTAs
+// rewrite the spin arrays between the half-sweeps of ONE launch: neither the non-coherent path nor a stale L1 line may
+// serve such a load.  (Couplings never change during a launch and always take the read-only path.)
+template <int W, bool COHERENT>
+__device__ __forceinline__ void load_spin_words(const uint32_t *p, size_t word_off, uint32_t out[W])
+{
+    if constexpr (!COHERENT) {
+        load_words<W>(p, word_off, out);
+    } else if constexpr (!IsVectorWidth<W>::value) {
+#pragma unroll
+        for (int k = 0; k < W; ++k) out[k] = __ldcg(p + word_off + k);
+    } else {
+        typedef typename WordVec<W>::type V;
+        const V v = __ldcg(reinterpret_cast<const V *>(p + word_off));
+        const uint32_t *pv = reinterpret_cast<const uint32_t *>(&v);
+#pragma unroll
+        for (int k = 0; k < W; ++k) out[k] = pv[k];
+    }
+}
+
 // 128-bit load of words that are read exactly once per half-sweep (couplings, the active spins): ld.global.cs, evict-first,
 // so that they do not displace what is re-read (the other colour's spins, the lane generators' state) from the L2.
 __device__ __forceinline__ void load_words4_streaming(const uint32_t *__restrict__ p, size_t word_off, uint32_t out[4])
@@ -229,7 +250,7 @@ inline int row_map_tpr_pad(int tpr)
 }
 
 template <int W>
-__device__ __forceinline__ RowMap row_map(int L)
+__device__ __forceinline__ RowMap row_map(int L, uint32_t bx, uint32_t by)
 {
     RowMap m;
     m.tpr = (L >> 6) / W;
@@ -240,8 +261,8 @@ __device__ __forceinline__ RowMap row_map(int L)
     const int lir = m.lane & (m.tpr_pad - 1);
     m.active = lir < m.tpr;
     m.lane_in_row = m.active ? lir : 0;
-    m.y = blockIdx.x * (32 >> lg) + (m.lane >> lg);
-    m.z = blockIdx.y * (SWEEP_THREADS / 32) + m.warp;
+    m.y = (int)bx * (32 >> lg) + (m.lane >> lg);
+    m.z = (int)by * (SWEEP_THREADS / 32) + m.warp;
     m.k0 = m.lane_in_row * W;
     const int base = m.lane & ~(m.tpr_pad - 1);
     m.next_lane = base | (m.lane_in_row + 1 == m.tpr ? 0 : m.lane_in_row + 1);
@@ -257,14 +278,17 @@ __device__ __forceinline__ RowMap row_map(int L)
 // extra launch and no extra pass over the 512 MiB (L = 1024: 78 us per record saved).
 // Four CTAs per SM (64 registers) for the Philox kernel the L = 1024 numbers are quoted on (0.3899 -> 0.3868 ms per half-sweep, 8 bytes
 // of spill); the other variants keep ptxas' own choice (W = 5 would spill 40 bytes).
-template <int RNG, int W, bool MEASURE>
-__global__ void __launch_bounds__(SWEEP_THREADS, RNG == 0 && W == 4 && !MEASURE ? 4 : 0)
-half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, unsigned long long *acc, long long N,
-                       long long *E, long long *M)
+// The update of one tile = the rows of one (virtual) CTA (bx, by) of the grid (L / (32 / tpr_pad), L / 8): the body of
+// half_sweep_site_packed (one tile per CTA) and of persistent_site_packed (a CTA walks over tiles, half-sweep after
+// half-sweep; COHERENT spin loads, see load_spin_words).  gx = x extent of that grid.  m_unsat / m_up (MEASURE): this
+// thread's unsatisfied bonds and up spins are ADDED to them.
+template <int RNG, int W, bool MEASURE, bool COHERENT>
+__device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteRng &rng, uint32_t bx, uint32_t by, uint32_t gx,
+                                                 unsigned long long &m_unsat, unsigned long long &m_up_out)
 {
     const int L = a.L;
     const int wpr = L >> 6;                 // words per half-row
-    const RowMap rm = row_map<W>(L);
+    const RowMap rm = row_map<W>(L, bx, by);
     const int tpr = rm.tpr, lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z, k0 = rm.k0;
 
     const int yp = y + 1 == L ? 0 : y + 1, ym = y == 0 ? L - 1 : y - 1;
@@ -278,18 +302,18 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     uint32_t s[W], sum2[W], sum1[W], sum0[W];
     unsigned int m_sat = 0, m_up = 0;   // MEASURE: satisfied bonds of this thread's sites, up spins of both colours
     const int xodd = (y + z + a.colour) & 1;
-    wait_for_previous_kernel();
+    if (!COHERENT) wait_for_previous_kernel();
     {
         uint32_t o[W], oyp[W], oym[W], ozp[W], ozm[W];
         uint32_t jxa[W], jya[W], jza[W], jxo[W], jyo[W], jzo[W];
-        load_words<W>(a.S_act, row, s);
-        load_words<W>(a.S_oth, row, o);
+        load_spin_words<W, COHERENT>(a.S_act, row, s);
+        load_spin_words<W, COHERENT>(a.S_oth, row, o);
         load_words<W>(a.J_oth[0], row, jxo);
         load_words<W>(a.J_act[0], row, jxa);
-        load_words<W>(a.S_oth, row_yp, oyp);
-        load_words<W>(a.S_oth, row_ym, oym);
-        load_words<W>(a.S_oth, row_zp, ozp);
-        load_words<W>(a.S_oth, row_zm, ozm);
+        load_spin_words<W, COHERENT>(a.S_oth, row_yp, oyp);
+        load_spin_words<W, COHERENT>(a.S_oth, row_ym, oym);
+        load_spin_words<W, COHERENT>(a.S_oth, row_zp, ozp);
+        load_spin_words<W, COHERENT>(a.S_oth, row_zm, ozm);
         load_words<W>(a.J_act[1], row, jya);
         load_words<W>(a.J_act[2], row, jza);
         load_words<W>(a.J_oth[1], row_ym, jyo);
@@ -329,7 +353,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
     constexpr int WC = RNG == 2 ? W : 0;
     // seeds from the table, two groups of 16 sites in flight: while one half-word's draws are compared, the next
     // half-word's four 16-byte loads are outstanding (about 2 KB per warp, enough to keep HBM busy)
-    const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
+    const uint32_t warp_global = (by * gx + bx) * (SWEEP_THREADS / 32) + warp;
     const uint4 *tab = rng.s0tab;
     uint4 cur[4], nxt[4];
     if (WC > 0) {
@@ -393,9 +417,21 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
         }
     }
     if (rm.active) store_words<W>(a.S_act, row, s);
-    if (MEASURE) {
+    if (MEASURE && rm.active) {
         // unsatisfied bonds = 6 per active site - satisfied; idle lanes of a padded row shadow lane 0 and count nothing
-        const unsigned long long unsat = rm.active ? 192ull * W - m_sat : 0ull, up = rm.active ? m_up : 0ull;
+        m_unsat += 192ull * W - m_sat;
+        m_up_out += m_up;
+    }
+}
+
+template <int RNG, int W, bool MEASURE>
+__global__ void __launch_bounds__(SWEEP_THREADS, RNG == 0 && W == 4 && !MEASURE ? 4 : 0)
+half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, unsigned long long *acc, long long N,
+                       long long *E, long long *M)
+{
+    unsigned long long unsat = 0, up = 0;
+    site_packed_tile<RNG, W, MEASURE, false>(a, rng, blockIdx.x, blockIdx.y, gridDim.x, unsat, up);
+    if (MEASURE) {
         block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
         finalize_slots_last_cta(acc, N, E, M);
     }
@@ -405,7 +441,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
 template <int W>
 __global__ void __launch_bounds__(SWEEP_THREADS) minstd_fill_s0(uint4 *tab, int L, int colour, uint64_t seed)
 {
-    const RowMap rm = row_map<W>(L);
+    const RowMap rm = row_map<W>(L, blockIdx.x, blockIdx.y);
     const int lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z, k0 = rm.k0;
     const int xodd = (y + z + colour) & 1;
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;
@@ -503,28 +539,37 @@ half_sweep_site_packed_generic(const SweepArgs a, const __grid_constant__ RngLau
 // scheme must work for every L = 2n, not only powers of two, is what this kernel is for: about
 // 1 ps/flip instead of 12-55 for the one-site-at-a-time kernel it replaces (kernel choice 1 still selects that one).
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t bit_window(const uint32_t *__restrict__ a, uint32_t pos)
+// PLAIN = false: loads through the read-only path (global arrays that no one writes during the launch); PLAIN = true: ordinary
+// loads through a generic pointer (arrays staged in shared memory by half_sweeps_on_chip, which are rewritten between half-sweeps).
+template <bool PLAIN>
+__device__ __forceinline__ uint32_t load_word(const uint32_t *a, uint32_t w)
+{
+    if constexpr (PLAIN) return a[w];
+    else return __ldg(a + w);
+}
+template <bool PLAIN = false>
+__device__ __forceinline__ uint32_t bit_window(const uint32_t *a, uint32_t pos)
 {   // bits pos .. pos+31 of the bit array (bits past the array's end are garbage that the caller masks out)
     const uint32_t w = pos >> 5, sh = pos & 31u;
-    const uint32_t lo = __ldg(a + w);
-    const uint32_t hi = sh ? __ldg(a + w + 1) : 0u;
+    const uint32_t lo = load_word<PLAIN>(a, w);
+    const uint32_t hi = sh ? load_word<PLAIN>(a, w + 1) : 0u;
     return __funnelshift_r(lo, hi, sh);
 }
-__device__ __forceinline__ uint32_t bit_at(const uint32_t *__restrict__ a, uint32_t pos) { return (__ldg(a + (pos >> 5)) >> (pos & 31u)) & 1u; }
+template <bool PLAIN = false>
+__device__ __forceinline__ uint32_t bit_at(const uint32_t *a, uint32_t pos) { return (load_word<PLAIN>(a, pos >> 5) >> (pos & 31u)) & 1u; }
 
-template <int RNG>
-__global__ void __launch_bounds__(128)
-half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t n_words, uint32_t Hc)
+// The update of word w (colour ranks 32 w .. 32 w + 31); returns the new word.  PLAIN: see load_word.  VOTE: the rare branch of
+// the acceptance is taken after a warp vote (all 32 lanes of the warp must be here) or per thread.
+template <int RNG, bool PLAIN, bool VOTE>
+__device__ __forceinline__ uint32_t rows_word_update(const SweepArgs &a, const SiteRng &rng, uint32_t w, uint32_t Hc)
 {
-    const uint32_t w = blockIdx.x * 128u + threadIdx.x;
-    if (w >= n_words) return;
     const uint32_t L = (uint32_t)a.L, H = L >> 1, LH = L * H;
     const uint32_t j0 = 32u * w;
     uint32_t remaining = Hc - j0 < 32u ? Hc - j0 : 32u, bitoff = 0;
     uint32_t r = j0 / H, m = j0 - r * H, z = r / L, y = r - z * L;
-    wait_for_previous_kernel();
-    const uint32_t s = __ldg(a.S_act + w);
-    uint32_t J[6] = {__ldg(a.J_act[0] + w), 0u, __ldg(a.J_act[1] + w), 0u, __ldg(a.J_act[2] + w), 0u}, nb[6] = {0u, 0u, 0u, 0u, 0u, 0u};
+    const uint32_t s = load_word<PLAIN>(a.S_act, w);
+    uint32_t J[6] = {load_word<PLAIN>(a.J_act[0], w), 0u, load_word<PLAIN>(a.J_act[1], w), 0u, load_word<PLAIN>(a.J_act[2], w), 0u};
+    uint32_t nb[6] = {0u, 0u, 0u, 0u, 0u, 0u};
     uint32_t c4 = 0, c8 = 0, c12 = 0;
     while (remaining > 0) {
         const uint32_t len = remaining < H - m ? remaining : H - m;
@@ -534,29 +579,29 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
         const uint32_t Pyp = (y + 1 == L) ? P - (LH - H) : P + H, Pym = (y == 0) ? P + (LH - H) : P - H;
         const uint32_t Pzp = (z + 1 == L) ? P - (Hc - LH) : P + LH, Pzm = (z == 0) ? P + (Hc - LH) : P - LH;
         // +x: column m + xodd of the same row; the last column wraps to column 0 when xodd = 1
-        uint32_t wpx = bit_window(a.S_oth, P + m + xodd);
-        if (xodd && m + len == H) wpx = (wpx & ~(1u << (len - 1))) | (bit_at(a.S_oth, P) << (len - 1));
+        uint32_t wpx = bit_window<PLAIN>(a.S_oth, P + m + xodd);
+        if (xodd && m + len == H) wpx = (wpx & ~(1u << (len - 1))) | (bit_at<PLAIN>(a.S_oth, P) << (len - 1));
         // -x: column m - 1 + xodd with its own coupling; column 0 wraps to column H-1 when xodd = 0
         uint32_t wmx, jmx;
         if (xodd) {
-            wmx = bit_window(a.S_oth, P + m);
-            jmx = bit_window(a.J_oth[0], P + m);
+            wmx = bit_window<PLAIN>(a.S_oth, P + m);
+            jmx = bit_window<PLAIN>(a.J_oth[0], P + m);
         } else if (m == 0) {
-            wmx = (bit_window(a.S_oth, P) << 1) | bit_at(a.S_oth, P + H - 1);
-            jmx = (bit_window(a.J_oth[0], P) << 1) | bit_at(a.J_oth[0], P + H - 1);
+            wmx = (bit_window<PLAIN>(a.S_oth, P) << 1) | bit_at<PLAIN>(a.S_oth, P + H - 1);
+            jmx = (bit_window<PLAIN>(a.J_oth[0], P) << 1) | bit_at<PLAIN>(a.J_oth[0], P + H - 1);
         } else {
-            wmx = bit_window(a.S_oth, P + m - 1);
-            jmx = bit_window(a.J_oth[0], P + m - 1);
+            wmx = bit_window<PLAIN>(a.S_oth, P + m - 1);
+            jmx = bit_window<PLAIN>(a.J_oth[0], P + m - 1);
         }
         nb[0] |= (wpx << bitoff) & segmask;
         nb[1] |= (wmx << bitoff) & segmask;
         J[1] |= (jmx << bitoff) & segmask;
-        nb[2] |= (bit_window(a.S_oth, Pyp + m) << bitoff) & segmask;
-        nb[3] |= (bit_window(a.S_oth, Pym + m) << bitoff) & segmask;
-        J[3] |= (bit_window(a.J_oth[1], Pym + m) << bitoff) & segmask;
-        nb[4] |= (bit_window(a.S_oth, Pzp + m) << bitoff) & segmask;
-        nb[5] |= (bit_window(a.S_oth, Pzm + m) << bitoff) & segmask;
-        J[5] |= (bit_window(a.J_oth[2], Pzm + m) << bitoff) & segmask;
+        nb[2] |= (bit_window<PLAIN>(a.S_oth, Pyp + m) << bitoff) & segmask;
+        nb[3] |= (bit_window<PLAIN>(a.S_oth, Pym + m) << bitoff) & segmask;
+        J[3] |= (bit_window<PLAIN>(a.J_oth[1], Pym + m) << bitoff) & segmask;
+        nb[4] |= (bit_window<PLAIN>(a.S_oth, Pzp + m) << bitoff) & segmask;
+        nb[5] |= (bit_window<PLAIN>(a.S_oth, Pzm + m) << bitoff) & segmask;
+        J[5] |= (bit_window<PLAIN>(a.J_oth[2], Pzm + m) << bitoff) & segmask;
         if (RNG == 1) {   // MINSTD: stream id = canonical site index; bit b of the word is site0 + 2 (b - bitoff)
             const uint64_t site0 = (uint64_t)L * r + 2u * m + xodd - 2ull * bitoff;
             uint32_t d4, d8, d12;
@@ -575,11 +620,21 @@ half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng r
             if (++y == L) { y = 0; ++z; }
         }
     }
-    if (RNG == 0) cond_masks_site_packed_philox(rng.pc, rng.ps, w, a.T, c4, c8, c12);
+    if (RNG == 0) cond_masks_site_packed_philox<VOTE>(rng.pc, rng.ps, w, a.T, c4, c8, c12);
     uint32_t sum2, sum1, sum0;
     satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
     const uint32_t valid = bitoff == 32u ? 0xFFFFFFFFu : (1u << bitoff) - 1u;   // the last word of the array may be partial
-    a.S_act[w] = s ^ (flip_mask(sum2, sum1, sum0, c4, c8, c12) & valid);
+    return s ^ (flip_mask(sum2, sum1, sum0, c4, c8, c12) & valid);
+}
+
+template <int RNG>
+__global__ void __launch_bounds__(128)
+half_sweep_site_packed_rows(const SweepArgs a, const __grid_constant__ SiteRng rng, uint32_t n_words, uint32_t Hc)
+{
+    const uint32_t w = blockIdx.x * 128u + threadIdx.x;
+    if (w >= n_words) return;
+    wait_for_previous_kernel();
+    a.S_act[w] = rows_word_update<RNG, false, true>(a, rng, w, Hc);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -817,7 +872,8 @@ half_sweep_sample_packed(SweepArgs a, const __grid_constant__ RngLaunch rng, uin
 // L/2 is a multiple of 4 and a group never leaves its row): own spins and couplings, the y+-1 / z+-1 neighbours and their
 // couplings are 128-bit loads; the two x-neighbours are the same four words of the other colour shifted by one word
 // (one extra 32-bit load each for spins and couplings).  p = index of the group within the plane z (y = p / gpr).
-template <bool STREAM = false>
+// COHERENT: spin words through the L2 (persistent kernels, see load_spin_words).
+template <bool STREAM = false, bool COHERENT = false>
 __device__ __forceinline__ void vec_group_sums(const SweepArgs &a, uint32_t gpr, uint32_t gpr_inv, uint32_t p, uint32_t z,
                                                uint32_t &j0, uint64_t &site0, uint32_t s[4], uint32_t sum2[4], uint32_t sum1[4],
                                                uint32_t sum0[4])
@@ -836,22 +892,22 @@ __device__ __forceinline__ void vec_group_sums(const SweepArgs &a, uint32_t gpr,
     const uint32_t m_extra = xodd ? (m0 + 4 == H ? 0u : m0 + 4) : (m0 == 0 ? H - 1 : m0 - 1);
 
     uint32_t o[4], oyp[4], oym[4], ozp[4], ozm[4], jxa[4], jya[4], jza[4], jxo[4], jyo[4], jzo[4];
-    wait_for_previous_kernel();
+    if (!COHERENT) wait_for_previous_kernel();
     if (STREAM) {
         load_words4_streaming(a.S_act, j0, s);
         load_words<4>(a.S_oth, j0, o);
         load_words4_streaming(a.J_oth[0], j0, jxo);
     } else {
-        load_words<4>(a.S_act, j0, s);
-        load_words<4>(a.S_oth, j0, o);
+        load_spin_words<4, COHERENT>(a.S_act, j0, s);
+        load_spin_words<4, COHERENT>(a.S_oth, j0, o);
         load_words<4>(a.J_oth[0], j0, jxo);
     }
-    const uint32_t o_extra = __ldg(a.S_oth + rowbase + m_extra);
+    const uint32_t o_extra = COHERENT ? __ldcg(a.S_oth + rowbase + m_extra) : __ldg(a.S_oth + rowbase + m_extra);
     const uint32_t jxo_extra = __ldg(a.J_oth[0] + rowbase + m_extra);
-    load_words<4>(a.S_oth, jyp, oyp);
-    load_words<4>(a.S_oth, jym, oym);
-    load_words<4>(a.S_oth, jzp, ozp);
-    load_words<4>(a.S_oth, jzm, ozm);
+    load_spin_words<4, COHERENT>(a.S_oth, jyp, oyp);
+    load_spin_words<4, COHERENT>(a.S_oth, jym, oym);
+    load_spin_words<4, COHERENT>(a.S_oth, jzp, ozp);
+    load_spin_words<4, COHERENT>(a.S_oth, jzm, ozm);
     if (STREAM) {
         load_words4_streaming(a.J_act[0], j0, jxa);
         load_words4_streaming(a.J_act[1], j0, jya);

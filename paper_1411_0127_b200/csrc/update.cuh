@@ -94,6 +94,7 @@ ISING_HD void finish_cond(const Thresholds &T, uint32_t &c4, uint32_t &c8, uint3
 // Site-packed word (bits = 32 consecutive sites of one colour of one lattice): colour rank of bit b is
 // j = 32*word_index + b, so Philox call q = 0..7 has counter g = 8*word_index + q and serves bits 4q..4q+3 (R9).
 // Two calls are generated together: four independent multiply chains hide the IMAD.WIDE latency at any occupancy.
+template <bool VOTE = true>
 ISING_HD void cond_masks_site_packed_philox(const PhiloxCommonConst &cc, const PhiloxSampleConst &sc, uint32_t word_index,
                                             const Thresholds &T, uint32_t &c4, uint32_t &c8, uint32_t &c12)
 {
@@ -104,7 +105,7 @@ ISING_HD void cond_masks_site_packed_philox(const PhiloxCommonConst &cc, const P
         uint32_t R[8];
         philox_folded(cc, sc, g0 + (uint32_t)q, R);
         philox_folded(cc, sc, g0 + (uint32_t)q + 1u, R + 4);
-        accumulate_cond<8>(R, 4 * q, T, c4, c8, c12);
+        accumulate_cond<8, VOTE>(R, 4 * q, T, c4, c8, c12);
     }
     finish_cond(T, c4, c8, c12);
 }

@@ -117,7 +117,7 @@ def test_argument_validation_without_a_gpu():
     t = C.c_uint64(99)
     assert lib.ising_get_t(h, C.byref(t)) == binding.OK and t.value == 0
     assert lib.ising_set_t(h, 6) == binding.OK and lib.ising_get_t(h, C.byref(t)) == binding.OK and t.value == 6
-    assert lib.ising_set_kernel(h, 4) == binding.EINVAL
+    assert lib.ising_set_kernel(h, 5) == binding.EINVAL
     assert lib.ising_kernel_launches(h) == 0
     assert lib.ising_destroy(h) == binding.OK
 

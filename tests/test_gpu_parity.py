@@ -752,3 +752,137 @@ def test_energy_measured_inside_the_half_sweep_kernel(L, rng_mode):
             o.half_sweep(0.8)
             Eo, Mo = o.energy()
             assert (int(E[k, 0]), int(M[k, 0])) == (int(Eo[0]), int(Mo[0])), k
+
+
+# ------------------------------------------------------------------------------------------------ persistent kernel
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L", [64, 128, 192, 256, 320, 448])
+def test_persistent_kernel_equals_one_launch_per_half_sweep(L, rng_mode):
+    """Lattices with whole-word rows below L = 512 can run all half-sweeps of a call in one cooperative launch, the CTAs
+    synchronising tile by tile through epoch counters (persistent.cuh; kernel choice 4, automatic for recorded calls at L = 64
+    and 128); kernel choice 3 keeps one launch per half-sweep.  Same spins, E and M records for every record spacing (1, 2, 3, 5
+    half-sweeps: records on red and on blue half-sweeps, a spacing that does not divide the call), from an odd starting counter
+    (the call begins with a blue half-sweep, and MINSTD changes its multiplier after the first half-sweep), over several
+    calls; the launch counts show which path ran; the oracle at the small sizes."""
+    spins, J = synth.make_spins(L, 1, 71), synth.make_couplings(L, 1, 72)
+    a = Ising(L, 1, SEED, rng_mode)
+    a.ising_set_kernel(4)   # the persistent kernel for every call
+    b = Ising(L, 1, SEED, rng_mode)
+    b.ising_set_kernel(3)
+    o = _loaded(L, 1, rng_mode, spins, J) if L <= 128 else None
+    for g in (a, b):
+        g.ising_load_state(dev(spins), dev(J))
+    la, lb = a.ising_kernel_launches(), b.ising_kernel_launches()
+    a.ising_sweep(0.8, 3)
+    b.ising_sweep(0.8, 3)
+    fills = 2 if rng_mode == MINSTD else 0          # the two seed-table launches
+    assert a.ising_kernel_launches() - la == 1 + fills and b.ising_kernel_launches() - lb == 6 + (2 if rng_mode == MINSTD else 0)
+    assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    if o is not None:
+        o.sweep(0.8, 3)
+        assert_same_state(o, a, f"persistent L={L}")
+    for every, nsw in ((1, 2), (2, 3), (3, 3), (5, 4)):
+        Ea, Ma = a.ising_sweep_trace(0.8, nsw, every_half_sweeps=every)
+        Eb, Mb = b.ising_sweep_trace(0.8, nsw, every_half_sweeps=every)
+        assert Ea.shape[0] == (2 * nsw) // every and torch.equal(Ea, Eb) and torch.equal(Ma, Mb), every
+        assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    if o is not None:
+        o.sweep(0.8, 12)
+        assert_same_state(o, a, f"persistent L={L} after the traces")
+    # odd starting counter
+    for g in (a, b):
+        g.ising_set_t(7)
+        g.ising_load_state(dev(spins), dev(J))
+    Ea, Ma = a.ising_sweep_trace(1 / 1.1, 2, every_half_sweeps=1, want_M=False)
+    Eb, Mb = b.ising_sweep_trace(1 / 1.1, 2, every_half_sweeps=1, want_M=False)
+    assert Ma is None and torch.equal(Ea, Eb) and torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert a.ising_get_t() == 11 == b.ising_get_t()
+    if o is not None and rng_mode == PHILOX:   # (the oracle's MINSTD streams are stored states: they cannot jump to t = 7)
+        o2 = _loaded(L, 1, rng_mode, spins, J)
+        o2.t = 7
+        for k in range(4):
+            o2.half_sweep(1 / 1.1)
+            assert int(Ea[k, 0]) == int(o2.energy()[0][0]), k
+        assert_same_state(o2, a, "odd starting counter")
+    Eg, Mg = a.ising_energy()           # the separate energy kernel still works on the state the persistent kernel left
+    assert int(Eg[0]) == int(Ea[-1, 0])
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+def test_persistent_kernel_long_call(rng_mode):
+    """66000 half-sweeps in one call = one cooperative launch, records every 1001 half-sweeps; against one launch per half-sweep."""
+    L, nsw, every = 64, 33000, 1001
+    spins, J = synth.make_spins(L, 1, 73), synth.make_couplings(L, 1, 74)
+    res = []
+    for choice in (0, 3):      # a recorded call at L = 64: the persistent kernel is the automatic choice
+        g = Ising(L, 1, SEED, rng_mode)
+        g.ising_set_kernel(choice)
+        g.ising_load_state(dev(spins), dev(J))
+        l0 = g.ising_kernel_launches()
+        E, M = g.ising_sweep_trace(1 / 1.1, nsw, every_half_sweeps=every)
+        res.append((E.clone(), M.clone(), g.ising_get_spins().clone(), g.ising_kernel_launches() - l0))
+        assert g.ising_get_t() == 2 * nsw
+    assert res[0][0].shape[0] == (2 * nsw) // every
+    assert all(torch.equal(x, y) for x, y in zip(res[0][:3], res[1][:3]))
+    assert res[0][3] <= 6 and res[1][3] >= 2 * nsw
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L", [4, 6, 10, 16, 18, 22, 24, 32, 34, 40])
+def test_on_chip_kernel_equals_the_oracle_and_one_launch_per_half_sweep(L, rng_mode):
+    """Lattices of at most 1024 words per colour (every even L <= 40) run all half-sweeps and records of a call in ONE launch of ONE
+    CTA out of shared memory (half_sweeps_on_chip; automatic).  Against the oracle half-sweep by half-sweep (E and M records of
+    every spacing, red and blue), against one launch per half-sweep (kernel choice 3), from an odd starting counter, across
+    several calls (the spins go back to global memory after every call), with the separate energy and get kernels afterwards."""
+    spins, J = synth.make_spins(L, 1, 77), synth.make_couplings(L, 1, 78)
+    o, a = make_pair(L, 1, rng_mode, spins, J)
+    b = Ising(L, 1, SEED, rng_mode)
+    b.ising_set_kernel(3)
+    b.ising_load_state(dev(spins), dev(J))
+    la = a.ising_kernel_launches()
+    E, M = a.ising_sweep_trace(1 / 1.1, 5, every_half_sweeps=1)
+    assert a.ising_kernel_launches() - la == 1
+    Eb, Mb = b.ising_sweep_trace(1 / 1.1, 5, every_half_sweeps=1)
+    assert torch.equal(E, Eb) and torch.equal(M, Mb)
+    for k in range(10):
+        o.half_sweep(1 / 1.1)
+        Eo, Mo = o.energy()
+        assert (int(E[k, 0]), int(M[k, 0])) == (int(Eo[0]), int(Mo[0])), k
+    assert_same_state(o, a, f"on-chip L={L}")
+    a.ising_sweep(0.5, 7)
+    o.sweep(0.5, 7)
+    assert_same_state(o, a, f"on-chip L={L}, second call")
+    E, none = a.ising_sweep_trace(0.9, 4, every_half_sweeps=3, want_M=False)     # records after half-sweeps 3 and 6 of 8
+    o.sweep(0.9, 1)
+    o.half_sweep(0.9)
+    e3 = int(o.energy()[0][0])
+    o.half_sweep(0.9)
+    o.sweep(0.9, 1)
+    e6 = int(o.energy()[0][0])
+    o.sweep(0.9, 1)
+    assert none is None and E.shape[0] == 2 and (int(E[0, 0]), int(E[1, 0])) == (e3, e6)
+    assert_same_state(o, a, f"on-chip L={L}, third call")
+    if rng_mode == PHILOX:   # odd starting counter (the oracle's stored MINSTD streams cannot jump)
+        o.t = 2**32 - 1
+        a.ising_set_t(2**32 - 1)
+        o.sweep(1 / 0.7, 2)
+        a.ising_sweep(1 / 0.7, 2)
+        assert a.ising_get_t() == 2**32 + 3
+        assert_same_state(o, a, "odd starting counter across 2^32")
+
+
+def test_config1_through_every_launch_structure():
+    """BASELINE.json config 1 (L = 16, E per half-sweep): the on-chip kernel (automatic), one launch per half-sweep (choice 3) and
+    the one-site-at-a-time kernels (choice 1) give the same 20 energies and the same final spins."""
+    cfg, spins, J = synth.make_config(1)
+    res = []
+    for choice in (0, 3, 1):
+        g = Ising(cfg["L"], 1, SEED, cfg["rng_mode"])
+        g.ising_set_kernel(choice)
+        g.ising_load_state(dev(spins), dev(J))
+        E, M = g.ising_sweep_trace(cfg["beta"], cfg["sweeps"], every_half_sweeps=1)
+        res.append((E.clone(), M.clone(), g.ising_get_spins().clone(), g.ising_kernel_launches()))
+    for r in res[1:]:
+        assert all(torch.equal(x, y) for x, y in zip(res[0][:3], r[:3]))
+    assert res[0][3] == 1 + 1 + 1 and res[1][3] >= 1 + 20 + 20      # load + one launch + get   against   load + 20 x (sweep + energy) + get
