@@ -207,6 +207,9 @@ def main():
     ap.add_argument("--aux", action="store_true",
                     help="rows a9 / a10 and the general-L kernels: load_state, energy, get_spins and a half-sweep per layout, with GB/s")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="z-slab decomposition (PAPER.md section V) of the L^3 lattice into this many slabs, all on this GPU: sweep time "
+                         "against the undivided lattice (the cost of the boundary / bulk split and of the plane exchange)")
     ap.add_argument("--small", action="store_true",
                     help="small lattices: time per half-sweep with the automatic kernels (0), one launch per half-sweep (3) and the "
                          "persistent kernels everywhere (4), without records and with E and M after every half-sweep")
@@ -428,6 +431,53 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.slabs:
+        from paper_1411_0127_b200 import IsingSlab, binding
+
+        rows = []
+        for mode in (PHILOX, MINSTD):
+            ref = Ising(L, 1, synth.DYN_SEED, mode)
+            ref.ising_load_state(d_spins, d_J)
+            ref.ising_sweep(BETA, 2)
+            times = {}
+            for G in sorted({1, args.slabs}):
+                hs = [IsingSlab(L, G, r, synth.DYN_SEED, mode) for r in range(G)]
+                for h in hs:
+                    h.ising_load_state(d_spins, d_J)
+                sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+                binding.ising_slab_sweep_local(hs, BETA, 2, sa, sb)
+                torch.cuda.synchronize()
+                best = None
+                for _ in range(3):
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(sa)
+                    binding.ising_slab_sweep_local(hs, BETA, nsw, sa, sb)
+                    b.record(sa)
+                    torch.cuda.synchronize()
+                    ms = a.elapsed_time(b)
+                    best = ms if best is None or ms < best else best
+                times[G] = best
+                out = torch.zeros_like(d_out)
+                for h in hs:
+                    h.ising_get_spins(out)
+                del hs
+            best = None
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                ref.ising_sweep(BETA, nsw)
+                b.record(stream)
+                torch.cuda.synchronize()
+                ms = a.elapsed_time(b)
+                best = ms if best is None or ms < best else best
+            ref.ising_destroy()
+            rows.append({"L": L, "rng_mode": ["philox", "minstd"][mode], "sweeps": nsw, "undivided_ms": best,
+                         "undivided_ps_per_flip": 1e9 * best / (nsw * N),
+                         **{f"slabs_{G}_ms": t for G, t in times.items()},
+                         **{f"slabs_{G}_over_undivided": t / best for G, t in times.items()}})
+        print(json.dumps({"slabs": rows}))
         return
 
     if args.small:

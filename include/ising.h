@@ -179,6 +179,40 @@ int ising_prng_init(int kind, uint64_t seed, uint32_t nlanes, void *d_state, voi
 int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndrawn_before, uint64_t ndraws, void *d_state,
                          uint64_t *d_odd, uint64_t *d_sum, void *stream);
 
+/* ---- z-slab domain decomposition (section V; Fig. 10) --------------------
+ * The lattice is cut along z into `nslabs` slabs of Lz = L / nslabs planes, one handle -- one GPU, in a multi-GPU run -- per slab;
+ * slab r owns the planes r Lz .. (r + 1) Lz - 1.  nsamples = 1, L a multiple of 64, Lz a multiple of 8, rng modes 0 and 1.
+ * A slab stores its own planes plus one halo plane below and above (copies of the neighbouring slabs' end planes, periodic), and
+ * a colour half-sweep of the lattice is, for every slab: the BOUNDARY kernel (the rows of CTAs that hold the first and last 8
+ * planes), then the exchange -- the updated colour's first owned plane goes to the upper halo of the slab below, its last owned
+ * plane to the lower halo of the slab above, L^2/16 bytes each (64 KiB at L = 1024), in both directions for each colour because
+ * in the standard checkerboard every plane holds both colours -- while the BULK kernel updates all other planes on
+ * a second stream (the paper's boundary / bulk overlap).  The library does the kernels; the exchange is the caller's (a peer
+ * cudaMemcpyAsync, NCCL send / recv, ...) between the buffers ising_slab_plane names, except for ising_slab_sweep_local, which
+ * drives all slabs of one process on one device itself.  Every draw is keyed by the site's position in the whole lattice (R9,
+ * R11), so the slabs together follow exactly the trajectory of the undivided lattice.
+ *
+ * On a slab handle: ising_load_state / ising_get_spins take the canonical arrays of the WHOLE lattice (the slab reads its planes
+ * and halos / writes its planes only); ising_energy gives the slab's share, E_r = 2 (unsatisfied +x,+y,+z bonds of its sites)
+ * - 3 L^2 Lz and M_r likewise, and sum_r E_r = E, sum_r M_r = M; ising_get_t / ising_set_t as usual; ising_sweep,
+ * ising_sweep_trace, ising_run_host* return ISING_EINVAL (a slab cannot sweep without its neighbours). */
+int ising_slab_workspace_bytes(int L, int nslabs, int rng_mode, size_t *out);
+int ising_create_slab(int L, int nslabs, int slab, uint64_t seed, int rng_mode, void *d_workspace, size_t workspace_bytes,
+                      ising_t **out);
+/* The two parts of the colour half-sweep t & 1 (thresholds as in ising_sweep).  The boundary part must see the halos of the
+ * previous half-sweep's exchange; the bulk part may run concurrently with the boundary part and the exchange on another stream,
+ * and advances t by one.  The next half-sweep needs both parts and the exchange complete, on this slab and its two neighbours. */
+int ising_slab_half_sweep_boundary(ising_t *h, double beta, void *stream);
+int ising_slab_half_sweep_bulk(ising_t *h, double beta, void *stream);
+/* Where the planes of the exchange live: *d_ptr = device address, *bytes = L^2/16.  which: 0 = first owned plane, 1 = last owned
+ * plane (to send down / up after a half-sweep of `colour`), 2 = lower halo, 3 = upper halo (to receive the plane 1 of the slab
+ * below / the plane 0 of the slab above). */
+int ising_slab_plane(ising_t *h, int colour, int which, void **d_ptr, size_t *bytes);
+/* nsweeps sweeps of a lattice whose `nslabs` slab handles (slabs[r] = slab r, all at the same counter t, same seed and mode) live
+ * in this process on the current device: boundary kernels and plane copies (cudaMemcpyAsync) on stream_a, bulk kernels on
+ * stream_b, an event pair between half-sweeps.  The two streams must differ; on return both have been made to wait for each other. */
+int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b);
+
 /* Select the kernels: 0 = automatic (site-packed: the word-parallel kernel when L is a multiple of 64, with the cached seed
  * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
  * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),

@@ -20,6 +20,8 @@ EXPORTS = (
     "ising_get_spins", "ising_run_host", "ising_run_host_async", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
+    "ising_slab_workspace_bytes", "ising_create_slab", "ising_slab_half_sweep_boundary", "ising_slab_half_sweep_bulk", "ising_slab_plane",
+    "ising_slab_sweep_local",
 )
 
 _lib = None
@@ -62,6 +64,12 @@ def lib() -> C.CDLL:
     L.ising_prng_state_bytes.argtypes = [i32, C.c_uint32, C.POINTER(sz)]
     L.ising_prng_init.argtypes = [i32, u64, C.c_uint32, vp, vp]
     L.ising_prng_count_odd.argtypes = [i32, u64, C.c_uint32, u64, u64, vp, vp, vp, vp]
+    L.ising_slab_workspace_bytes.argtypes = [i32, i32, i32, C.POINTER(sz)]
+    L.ising_create_slab.argtypes = [i32, i32, i32, u64, i32, vp, sz, C.POINTER(vp)]
+    L.ising_slab_half_sweep_boundary.argtypes = [vp, dbl, vp]
+    L.ising_slab_half_sweep_bulk.argtypes = [vp, dbl, vp]
+    L.ising_slab_plane.argtypes = [vp, i32, i32, C.POINTER(vp), C.POINTER(sz)]
+    L.ising_slab_sweep_local.argtypes = [C.POINTER(vp), i32, dbl, i32, vp, vp]
     L.ising_destroy.argtypes = [vp]
     L.ising_strerror.argtypes = [i32]
     L.ising_strerror.restype = C.c_char_p
@@ -291,3 +299,59 @@ class Ising:
             self.ising_destroy()
         except Exception:
             pass
+
+
+def ising_slab_workspace_bytes(L: int, nslabs: int, rng_mode: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().ising_slab_workspace_bytes(L, nslabs, rng_mode, C.byref(out)), "ising_slab_workspace_bytes")
+    return out.value
+
+
+class IsingSlab(Ising):
+    """Handle of one z-slab of an L^3 lattice cut into `nslabs` slabs (include/ising.h, "z-slab decomposition").
+    ising_load_state / ising_get_spins take the canonical arrays of the WHOLE lattice (the slab reads / writes its own planes);
+    ising_energy returns the slab's share of E and M (the shares of all slabs add up)."""
+
+    def __init__(self, L: int, nslabs: int, slab: int, seed: int = 0, rng_mode: int = PHILOX, device=None):
+        import torch
+
+        self.L, self.nsamples, self.seed, self.rng_mode = L, 1, seed, rng_mode
+        self.nslabs, self.slab = nslabs, slab
+        self.N = L ** 3
+        self.W = (self.N + 31) // 32
+        nbytes = ising_slab_workspace_bytes(L, nslabs, rng_mode)
+        dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        if dev.index is None:
+            dev = torch.device("cuda", torch.cuda.current_device())
+        self.device = dev
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            _check(lib().ising_create_slab(L, nslabs, slab, seed, rng_mode, self.workspace.data_ptr(), nbytes, C.byref(h)),
+                   "ising_create_slab")
+        self._h = h
+
+    def ising_slab_half_sweep_boundary(self, beta: float, stream=None):
+        with self._on_device():
+            _check(lib().ising_slab_half_sweep_boundary(self._h, float(beta), _stream_ptr(stream)), "ising_slab_half_sweep_boundary")
+
+    def ising_slab_half_sweep_bulk(self, beta: float, stream=None):
+        with self._on_device():
+            _check(lib().ising_slab_half_sweep_bulk(self._h, float(beta), _stream_ptr(stream)), "ising_slab_half_sweep_bulk")
+
+    def ising_slab_plane(self, colour: int, which: int):
+        """The plane as a uint8 view of the workspace: which = 0 first owned plane, 1 last owned plane (to send), 2 lower halo,
+        3 upper halo (to receive into)."""
+        ptr, nbytes = C.c_void_p(), C.c_size_t(0)
+        _check(lib().ising_slab_plane(self._h, int(colour), int(which), C.byref(ptr), C.byref(nbytes)), "ising_slab_plane")
+        off = ptr.value - self.workspace.data_ptr()
+        return self.workspace[off:off + nbytes.value]
+
+
+def ising_slab_sweep_local(slabs, beta: float, nsweeps: int, stream_a, stream_b):
+    """All slabs of a lattice in this process on one device: nsweeps sweeps, boundary kernels and plane copies on stream_a, bulk
+    kernels on stream_b (the paper's Fig. 10 with device-to-device copies as the exchange)."""
+    arr = (C.c_void_p * len(slabs))(*[s._h for s in slabs])
+    with slabs[0]._on_device():
+        _check(lib().ising_slab_sweep_local(arr, len(slabs), float(beta), int(nsweeps), stream_a.cuda_stream, stream_b.cuda_stream),
+               "ising_slab_sweep_local")

@@ -11,6 +11,7 @@
 #include "layout_kernels.cuh"
 #include "measure_kernels.cuh"
 #include "persistent.cuh"
+#include "slab_kernels.cuh"
 #include "sweep_kernels.cuh"
 
 using namespace isingk;
@@ -119,6 +120,7 @@ struct ising {
     bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
     bool overlap_clean;  // the counter of ising_overlap is zero
     int device;          // CUDA device the workspace lives on (-1: unknown, e.g. no device present)
+    int nslabs, slab, z0, Lz;  // z-slab handles (ising_create_slab): this handle owns the planes z0 .. z0 + Lz - 1; nslabs = 0 otherwise
     unsigned int *epochs;  // tile epochs of the persistent kernels (nullptr: no persistent path for this geometry / mode)
     int persist_grid[2];   // co-resident CTAs of this handle's persistent kernel without / with records (0: not asked yet, -1: none)
 
@@ -149,6 +151,9 @@ int check_launch(ising_t *h, int n = 1)
 // The workspace of a handle lives on one device (recorded by ising_create); every launch must be made with that device
 // current, or the kernels would dereference another GPU's memory (peer access) or fault (none).
 bool on_own_device(const ising_t *h);
+int slab_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, cudaStream_t st);
+int slab_get_spins(ising_t *h, uint32_t *d_out, cudaStream_t st);
+int slab_energy(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st);
 
 // Row a1 (R5, R6).  Plain double arithmetic with the C library's exp; compiled without FMA contraction.
 int compute_thresholds(double beta, int rng_mode, uint64_t out[3])
@@ -467,7 +472,14 @@ int half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long long *mE =
 bool persistent_available(const ising_t *h, bool records)
 {
     if (h->g.nsamples != 1 || (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD)) return false;
-    if (h->g.onchip) return h->kernel_choice == 0 || h->kernel_choice == 2 || h->kernel_choice == 4;
+    if (h->g.onchip) {
+        if (h->kernel_choice == 4) return true;
+        if (h->kernel_choice != 0 && h->kernel_choice != 2) return false;
+        // automatic: where one SM beats a launch per half-sweep on all of them (profiles/r2c_small.md): with records up to 512
+        // words per colour (L <= 32: 3.8-5.5 against 10.8-12.3 us per recorded half-sweep), without up to 216 (L <= 24)
+        const uint64_t nw = (h->g.Hc + 31) / 32;
+        return records ? nw <= 512 : nw <= 216;
+    }
     if (!h->epochs) return false;
     if (h->kernel_choice == 4) return true;                                      // wherever there is a tile grid (L <= 448)
     // automatic: where it beats the launches (profiles/r2b_persistent.md).  Without records the tile flags cost what the launch
@@ -685,6 +697,176 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
     return check_launch(h);
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// z-slab handles (slab_kernels.cuh)
+// ---------------------------------------------------------------------------------------------------------------------
+bool make_slab_geometry(int L, int nslabs, Geometry *g, int *Lz)
+{
+    if (!make_geometry(L, 1, g) || !g->fast) return false;                    // whole-word rows: L a multiple of 64
+    if (nslabs < 1 || L % nslabs != 0 || (L / nslabs) % (SWEEP_THREADS / 32) != 0) return false;   // a CTA row is 8 planes
+    *Lz = L / nslabs;
+    const size_t plane_words = (size_t)(L >> 6) * L;
+    g->array_words = round_up(plane_words * (size_t)(*Lz + 2), ALIGN_WORDS);
+    g->arrays_total_words = 8 * g->array_words;
+    g->staging_words = ALIGN_WORDS;                                            // no host-buffer path for slabs
+    g->s0_words = 2 * (size_t)L * (size_t)*Lz * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32;   // seed table of the slab's own planes
+    g->epoch_words = 0;
+    g->onchip = false;
+    return true;
+}
+
+SplitArgs slab_split_args(const ising_t *h, const uint32_t *d_spins, const uint32_t *d_J)
+{
+    const LatticeArrays A = h->arrays(0);
+    SplitArgs s;
+    s.narrays = 4;
+    s.L = h->g.L;
+    s.canon[0] = d_spins;
+    s.out[0][0] = A.S[0];
+    s.out[0][1] = A.S[1];
+    for (int d = 0; d < 3; ++d) {
+        s.canon[1 + d] = d_J + (size_t)d * h->g.canon_words;
+        s.out[1 + d][0] = A.J[d][0];
+        s.out[1 + d][1] = A.J[d][1];
+    }
+    return s;
+}
+
+dim3 slab_grid(const ising_t *h, unsigned rows);
+
+// MINSTD: the seed-state table of the slab's own planes (R11), once per handle.  It is filled by ising_load_state, not by the first
+// half-sweep, because the two parts of a half-sweep run on two streams and both read it: everything a handle does is ordered
+// after its load anyway.
+int slab_fill_seed_table(ising_t *h, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    if (h->rng_mode != ISING_RNG_MINSTD || !h->s0tab || h->s0_ready) return ISING_OK;
+    uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
+    const dim3 all = slab_grid(h, (unsigned)(h->Lz / (SWEEP_THREADS / 32)));
+    for (int cc = 0; cc < 2; ++cc) {
+        if (g.W == 4) minstd_fill_s0<4><<<all, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, h->z0);
+        else if (g.W == 3) minstd_fill_s0<3><<<all, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, h->z0);
+        else if (g.W == 5) minstd_fill_s0<5><<<all, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, h->z0);
+        else minstd_fill_s0<1><<<all, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, h->z0);
+    }
+    const int rc = check_launch(h, 2);
+    if (rc == ISING_OK) h->s0_ready = true;
+    return rc;
+}
+
+int slab_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, cudaStream_t st)
+{
+    const uint64_t n = (uint64_t)(h->g.L >> 6) * h->g.L * (h->Lz + 2);
+    split_colours_slab<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(slab_split_args(h, d_spins, d_J), h->z0, h->Lz + 2);
+    const int rc = check_launch(h);
+    return rc == ISING_OK ? slab_fill_seed_table(h, st) : rc;
+}
+
+int slab_get_spins(ising_t *h, uint32_t *d_out, cudaStream_t st)
+{
+    const LatticeArrays A = h->arrays(0);
+    const uint64_t n = (uint64_t)(h->g.L >> 6) * h->g.L * h->Lz;
+    merge_colours_slab<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, h->g.L, h->z0, h->Lz);
+    return check_launch(h);
+}
+
+dim3 slab_grid(const ising_t *h, unsigned rows)
+{
+    const int tpr_pad = row_map_tpr_pad((h->g.L >> 6) / h->g.W);
+    return dim3((unsigned)(h->g.L / (32 / tpr_pad)), rows);
+}
+
+int slab_energy(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    if (cudaMemsetAsync(h->acc, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
+    const LatticeArrays A = h->arrays(0);
+    MeasureArgs m;
+    for (int c = 0; c < 2; ++c) {
+        m.S[c] = A.S[c];
+        for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
+    }
+    m.L = g.L;
+    const dim3 grid = slab_grid(h, (unsigned)(h->Lz / (SWEEP_THREADS / 32)));
+    if (g.W == 4) energy_site_packed_slab<4><<<grid, SWEEP_THREADS, 0, st>>>(m, h->z0, h->acc);
+    else if (g.W == 3) energy_site_packed_slab<3><<<grid, SWEEP_THREADS, 0, st>>>(m, h->z0, h->acc);
+    else if (g.W == 5) energy_site_packed_slab<5><<<grid, SWEEP_THREADS, 0, st>>>(m, h->z0, h->acc);
+    else energy_site_packed_slab<1><<<grid, SWEEP_THREADS, 0, st>>>(m, h->z0, h->acc);
+    // the slab's share: E = 2 * unsatisfied - 3 N_slab, M = 2 * up - N_slab; the shares of all slabs add up to the lattice's (R16)
+    finalize_energy<<<1, 32, 0, st>>>(h->acc, 1, (long long)g.L * g.L * h->Lz, d_E, d_M);
+    return check_launch(h, 2);
+}
+
+template <int RNG, int W>
+void launch_slab_w(const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr)
+{
+    half_sweep_site_packed_slab<RNG, W><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+}
+template <int RNG>
+void launch_slab(int W, const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr)
+{
+    if (W == 4) launch_slab_w<RNG, 4>(grid, st, a, sr);
+    else if (W == 3) launch_slab_w<RNG, 3>(grid, st, a, sr);
+    else if (W == 5) launch_slab_w<RNG, 5>(grid, st, a, sr);
+    else launch_slab_w<RNG, 1>(grid, st, a, sr);
+}
+
+// part 0: the CTA rows holding the first and the last 8 planes of the slab (the paper's boundary kernel); part 1: the rows in
+// between (its bulk kernel).  Neither advances the counter.  A part without rows launches nothing.
+int slab_half_sweep_part(ising_t *h, const Thresholds &T, int part, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    const int nby = h->Lz / (SWEEP_THREADS / 32);
+    const int c = (int)(h->t & 1);
+    const LatticeArrays A = h->arrays(0);
+    SweepArgs a;
+    a.S_act = A.S[c];
+    a.S_oth = A.S[1 - c];
+    for (int d = 0; d < 3; ++d) { a.J_act[d] = A.J[d][c]; a.J_oth[d] = A.J[d][1 - c]; }
+    a.L = g.L;
+    a.colour = c;
+    a.T = T;
+    a.z0 = h->z0;
+    unsigned rows;
+    if (part == 0) {
+        a.by_first = 0;
+        a.by_stride = nby > 1 ? nby - 1 : 0;
+        rows = nby > 1 ? 2u : 1u;
+    } else {
+        if (nby <= 2) return ISING_OK;
+        a.by_first = 1;
+        a.by_stride = 1;
+        rows = (unsigned)(nby - 2);
+    }
+    RngLaunch r;
+    fill_rng_launch(h, 0, &r);
+    SiteRng sr;
+    sr.pc = r.pc;
+    sr.ps = r.ps[0];
+    sr.seed = r.seed;
+    sr.A2 = 2u * r.A;
+    sr.s0tab = nullptr;
+    const dim3 grid = slab_grid(h, rows);
+    if (h->rng_mode == ISING_RNG_PHILOX) {
+        launch_slab<0>(g.W, grid, st, a, sr);
+    } else if (h->kernel_choice != 2 && h->s0tab != nullptr && h->s0_ready) {   // MINSTD with the seed table (filled by the loader)
+        uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
+        sr.s0tab = tab[c];
+        launch_slab<2>(g.W, grid, st, a, sr);
+    } else {
+        launch_slab<1>(g.W, grid, st, a, sr);
+    }
+    return check_launch(h);
+}
+
+// which: 0 = first owned plane, 1 = last owned plane, 2 = lower halo, 3 = upper halo
+uint32_t *slab_plane_ptr(const ising_t *h, int colour, int which)
+{
+    const size_t plane_words = (size_t)(h->g.L >> 6) * h->g.L;
+    const int zl = which == 0 ? 1 : which == 1 ? h->Lz : which == 2 ? 0 : h->Lz + 1;
+    return h->arrays(0).S[colour] + plane_words * (size_t)zl;
+}
+
 bool on_own_device(const ising_t *h)
 {
     int cur = -1;
@@ -738,6 +920,7 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->nlanes = lane_mode(rng_mode) ? lanes_default(h->g, rng_mode) : 0;
     h->lanes_ready = false;
     h->persist_grid[0] = h->persist_grid[1] = 0;
+    h->nslabs = h->slab = h->z0 = h->Lz = 0;
     h->epochs = nullptr;
     if (h->g.epoch_words && !lane_mode(rng_mode)) {   // the last area of the workspace
         h->epochs = (unsigned int *)((char *)d_workspace + need - round_up(h->g.epoch_words * sizeof(uint32_t), 256));
@@ -770,6 +953,7 @@ int ising_destroy(ising_t *h)
 int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, void *stream)
 {
     if (!h || !d_spins || !d_J || !on_own_device(h)) return ISING_EINVAL;
+    if (h->nslabs) return slab_load_state(h, d_spins, d_J, (cudaStream_t)stream);
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t W = g.canon_words;
@@ -857,6 +1041,7 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
 int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
 {
     if (!h || !d_out || !on_own_device(h)) return ISING_EINVAL;
+    if (h->nslabs) return slab_get_spins(h, d_out, (cudaStream_t)stream);
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t W = g.canon_words;
@@ -900,6 +1085,7 @@ int ising_sweep(ising_t *h, double beta, int nsweeps, void *stream)
 int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_t *d_M, int every_half_sweeps, void *stream)
 {
     if (!h || nsweeps < 0 || !on_own_device(h)) return ISING_EINVAL;
+    if (h->nslabs) return ISING_EINVAL;   // a slab does not sweep on its own: ising_slab_half_sweep_* / ising_slab_sweep_local
     const bool trace = d_E != nullptr || d_M != nullptr;
     if (trace && every_half_sweeps < 1) return ISING_EINVAL;
     uint64_t T[3];
@@ -933,6 +1119,7 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
 int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream)
 {
     if (!h || !d_E || !on_own_device(h)) return ISING_EINVAL;
+    if (h->nslabs) return slab_energy(h, (long long *)d_E, (long long *)d_M, (cudaStream_t)stream);
     return measure(h, (long long *)d_E, (long long *)d_M, (cudaStream_t)stream);
 }
 
@@ -960,7 +1147,7 @@ int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *st
 int ising_run_host_async(ising_t *h, const uint32_t *h_spins, const uint32_t *h_J, double beta, int nsweeps,
                          uint32_t *h_spins_out, int64_t *h_E, int64_t *h_M, void *stream)
 {
-    if (!h || !h_spins || !h_J || !h_E || nsweeps < 0 || !(beta >= 0.0) || !on_own_device(h)) return ISING_EINVAL;
+    if (!h || !h_spins || !h_J || !h_E || nsweeps < 0 || !(beta >= 0.0) || !on_own_device(h) || h->nslabs) return ISING_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t spin_words = (size_t)g.nsamples * g.canon_words, j_words = 3 * spin_words;
@@ -1095,6 +1282,111 @@ int ising_prng_count_odd(int kind, uint64_t seed, uint32_t nlanes, uint64_t ndra
         count_odd_lanes<GEN_MT, false><<<blocks, 128, 0, st>>>(ln, ndraws, odd, sum);
     }
     return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
+}
+
+int ising_slab_workspace_bytes(int L, int nslabs, int rng_mode, size_t *out)
+{
+    Geometry g;
+    int Lz;
+    if (!out || !make_slab_geometry(L, nslabs, &g, &Lz)) return ISING_EINVAL;
+    if (rng_mode != ISING_RNG_PHILOX && rng_mode != ISING_RNG_MINSTD) return ISING_EINVAL;
+    *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
+    if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
+    return ISING_OK;
+}
+
+int ising_create_slab(int L, int nslabs, int slab, uint64_t seed, int rng_mode, void *d_workspace, size_t workspace_bytes, ising_t **out)
+{
+    size_t need = 0;
+    if (!out || !d_workspace || slab < 0 || slab >= nslabs) return ISING_EINVAL;
+    if (ising_slab_workspace_bytes(L, nslabs, rng_mode, &need) != ISING_OK) return ISING_EINVAL;
+    if (workspace_bytes < need || ((uintptr_t)d_workspace & 255u)) return ISING_EINVAL;
+    // a whole-lattice handle on a small dummy geometry gives every field its default; then the slab geometry replaces it
+    ising_t *h = nullptr;
+    {
+        size_t small = 0;
+        if (ising_workspace_bytes(4, 1, rng_mode, &small) != ISING_OK || small > workspace_bytes) return ISING_EINVAL;
+        const int rc = ising_create(4, 1, seed, rng_mode, d_workspace, workspace_bytes, &h);
+        if (rc != ISING_OK) return rc;
+    }
+    make_slab_geometry(L, nslabs, &h->g, &h->Lz);
+    h->nslabs = nslabs;
+    h->slab = slab;
+    h->z0 = slab * h->Lz;
+    h->staging = h->ws + h->g.arrays_total_words;
+    h->acc = (unsigned long long *)(h->staging + h->g.staging_words);
+    h->s0tab = rng_mode == ISING_RNG_MINSTD ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
+    h->epochs = nullptr;
+    *out = h;
+    return ISING_OK;
+}
+
+int ising_slab_half_sweep_boundary(ising_t *h, double beta, void *stream)
+{
+    if (!h || !h->nslabs || !on_own_device(h)) return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    return slab_half_sweep_part(h, kernel_thresholds(T), 0, (cudaStream_t)stream);
+}
+
+int ising_slab_half_sweep_bulk(ising_t *h, double beta, void *stream)
+{
+    if (!h || !h->nslabs || !on_own_device(h)) return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    const int rc = slab_half_sweep_part(h, kernel_thresholds(T), 1, (cudaStream_t)stream);
+    if (rc == ISING_OK) h->t += 1;
+    return rc;
+}
+
+int ising_slab_plane(ising_t *h, int colour, int which, void **d_ptr, size_t *bytes)
+{
+    if (!h || !h->nslabs || (colour != 0 && colour != 1) || which < 0 || which > 3 || !d_ptr || !bytes) return ISING_EINVAL;
+    *d_ptr = slab_plane_ptr(h, colour, which);
+    *bytes = (size_t)(h->g.L >> 6) * h->g.L * sizeof(uint32_t);
+    return ISING_OK;
+}
+
+int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b)
+{
+    if (!slabs || nslabs < 1 || nsweeps < 0 || !stream_a || !stream_b || stream_a == stream_b) return ISING_EINVAL;
+    for (int s = 0; s < nslabs; ++s)
+        if (!slabs[s] || slabs[s]->nslabs != nslabs || slabs[s]->slab != s || slabs[s]->g.L != slabs[0]->g.L ||
+            slabs[s]->t != slabs[0]->t || slabs[s]->rng_mode != slabs[0]->rng_mode || slabs[s]->seed != slabs[0]->seed ||
+            !on_own_device(slabs[s]))
+            return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, slabs[0]->rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    const Thresholds kt = kernel_thresholds(T);
+    cudaStream_t sa = (cudaStream_t)stream_a, sb = (cudaStream_t)stream_b;
+    cudaEvent_t ea, eb;
+    if (cudaEventCreateWithFlags(&ea, cudaEventDisableTiming) != cudaSuccess) return ISING_ECUDA;
+    if (cudaEventCreateWithFlags(&eb, cudaEventDisableTiming) != cudaSuccess) { cudaEventDestroy(ea); return ISING_ECUDA; }
+    const size_t plane_bytes = (size_t)(slabs[0]->g.L >> 6) * slabs[0]->g.L * sizeof(uint32_t);
+    int rc = ISING_OK;
+    // stream B first waits for whatever stream A holds on entry (the loader, a previous call)
+    if (cudaEventRecord(ea, sa) != cudaSuccess || cudaStreamWaitEvent(sb, ea, 0) != cudaSuccess) rc = ISING_ECUDA;
+    for (int k = 0; rc == ISING_OK && k < 2 * nsweeps; ++k) {
+        const int c = (int)(slabs[0]->t & 1);
+        // boundary kernels of all slabs, then the exchange of the updated colour's end planes: stream A
+        for (int s = 0; rc == ISING_OK && s < nslabs; ++s) rc = slab_half_sweep_part(slabs[s], kt, 0, sa);
+        for (int s = 0; rc == ISING_OK && s < nslabs; ++s) {
+            ising_t *below = slabs[(s + nslabs - 1) % nslabs], *above = slabs[(s + 1) % nslabs];
+            if (cudaMemcpyAsync(slab_plane_ptr(below, c, 3), slab_plane_ptr(slabs[s], c, 0), plane_bytes, cudaMemcpyDeviceToDevice, sa) != cudaSuccess ||
+                cudaMemcpyAsync(slab_plane_ptr(above, c, 2), slab_plane_ptr(slabs[s], c, 1), plane_bytes, cudaMemcpyDeviceToDevice, sa) != cudaSuccess)
+                rc = ISING_ECUDA;
+        }
+        // bulk kernels, concurrently: stream B (they touch neither the end planes nor the halos)
+        for (int s = 0; rc == ISING_OK && s < nslabs; ++s) rc = slab_half_sweep_part(slabs[s], kt, 1, sb);
+        // the next half-sweep starts when both streams are done with this one
+        if (rc == ISING_OK && (cudaEventRecord(ea, sa) != cudaSuccess || cudaEventRecord(eb, sb) != cudaSuccess ||
+                               cudaStreamWaitEvent(sb, ea, 0) != cudaSuccess || cudaStreamWaitEvent(sa, eb, 0) != cudaSuccess))
+            rc = ISING_ECUDA;
+        for (int s = 0; s < nslabs; ++s) slabs[s]->t += 1;
+    }
+    cudaEventDestroy(ea);
+    cudaEventDestroy(eb);
+    return rc;
 }
 
 int ising_set_kernel(ising_t *h, int which)

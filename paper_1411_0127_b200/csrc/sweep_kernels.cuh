@@ -47,6 +47,9 @@ struct SweepArgs {
     int L;
     int colour;
     Thresholds T;
+    // z-slab handles only (SLAB variants of the kernels; slab_kernels.cuh): the arrays hold the planes z0 - 1 .. z0 + Lz of the
+    // lattice (local plane 0 and Lz + 1 are halos), and a launch covers the rows of CTAs by_first + blockIdx.y * by_stride
+    int z0, by_first, by_stride;
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -282,26 +285,32 @@ __device__ __forceinline__ RowMap row_map(int L, uint32_t bx, uint32_t by)
 // half_sweep_site_packed (one tile per CTA) and of persistent_site_packed (a CTA walks over tiles, half-sweep after
 // half-sweep; COHERENT spin loads, see load_spin_words).  gx = x extent of that grid.  m_unsat / m_up (MEASURE): this
 // thread's unsatisfied bonds and up spins are ADDED to them.
-template <int RNG, int W, bool MEASURE, bool COHERENT>
+// SLAB: the arrays are those of a z-slab (see SweepArgs): the tile's planes are stored one plane up (the lower halo is plane 0),
+// their z-neighbours are simply the planes below and above (halos at the ends, no wrap), and everything keyed by the site -- the
+// colour of a row, the Philox counter, the MINSTD stream ids -- uses the plane's z in the whole lattice.
+template <int RNG, int W, bool MEASURE, bool COHERENT, bool SLAB = false>
 __device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteRng &rng, uint32_t bx, uint32_t by, uint32_t gx,
                                                  unsigned long long &m_unsat, unsigned long long &m_up_out)
 {
     const int L = a.L;
     const int wpr = L >> 6;                 // words per half-row
     const RowMap rm = row_map<W>(L, bx, by);
-    const int tpr = rm.tpr, lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z, k0 = rm.k0;
+    const int tpr = rm.tpr, lane = rm.lane, warp = rm.warp, y = rm.y, k0 = rm.k0;
+    const int z = SLAB ? rm.z + 1 : rm.z;          // plane in the arrays
+    const int zg = SLAB ? rm.z + a.z0 : rm.z;      // plane in the lattice
 
     const int yp = y + 1 == L ? 0 : y + 1, ym = y == 0 ? L - 1 : y - 1;
-    const int zp = z + 1 == L ? 0 : z + 1, zm = z == 0 ? L - 1 : z - 1;
+    const int zp = SLAB ? z + 1 : (z + 1 == L ? 0 : z + 1), zm = SLAB ? z - 1 : (z == 0 ? L - 1 : z - 1);
     const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;   // < 2^27 words for L <= 2048
     const uint32_t row_yp = (uint32_t)wpr * ((uint32_t)yp + (uint32_t)L * z) + k0;
     const uint32_t row_ym = (uint32_t)wpr * ((uint32_t)ym + (uint32_t)L * z) + k0;
     const uint32_t row_zp = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zp) + k0;
     const uint32_t row_zm = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zm) + k0;
+    const uint32_t row_g = SLAB ? (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zg) + k0 : row;   // the row's words in the lattice
 
     uint32_t s[W], sum2[W], sum1[W], sum0[W];
     unsigned int m_sat = 0, m_up = 0;   // MEASURE: satisfied bonds of this thread's sites, up spins of both colours
-    const int xodd = (y + z + a.colour) & 1;
+    const int xodd = (y + zg + a.colour) & 1;
     if (!COHERENT) wait_for_previous_kernel();
     {
         uint32_t o[W], oyp[W], oym[W], ozp[W], ozm[W];
@@ -348,7 +357,7 @@ __device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteR
         m_up += __popc(s[k]);
     };
 
-    const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;  // MINSTD stream ids
+    const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * zg) + (uint64_t)xodd;  // MINSTD stream ids
     // RNG = 2: the seed states of all W words come from the table; RNG = 0, 1: every word draws in registers.
     constexpr int WC = RNG == 2 ? W : 0;
     // seeds from the table, two groups of 16 sites in flight: while one half-word's draws are compared, the next
@@ -379,7 +388,7 @@ __device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteR
     for (int k = WC; k < W; ++k) {
         uint32_t c4, c8, c12;
         if (RNG == 0) {
-            cond_masks_site_packed_philox(pcr, psr, row + (uint32_t)k, Tr, c4, c8, c12);
+            cond_masks_site_packed_philox(pcr, psr, row_g + (uint32_t)k, Tr, c4, c8, c12);
         } else {
             const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
             cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
@@ -438,11 +447,12 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
 }
 
 // Fills the seed table of colour `colour` with the thread mapping of half_sweep_site_packed<2, W> (same grid).
+// z0: the lattice plane of the grid's first plane (0, or the first owned plane of a z-slab, whose table covers its own planes).
 template <int W>
-__global__ void __launch_bounds__(SWEEP_THREADS) minstd_fill_s0(uint4 *tab, int L, int colour, uint64_t seed)
+__global__ void __launch_bounds__(SWEEP_THREADS) minstd_fill_s0(uint4 *tab, int L, int colour, uint64_t seed, int z0 = 0)
 {
     const RowMap rm = row_map<W>(L, blockIdx.x, blockIdx.y);
-    const int lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z, k0 = rm.k0;
+    const int lane = rm.lane, warp = rm.warp, y = rm.y, z = rm.z + z0, k0 = rm.k0;
     const int xodd = (y + z + colour) & 1;
     const uint64_t row_site0 = (uint64_t)L * ((uint64_t)y + (uint64_t)L * z) + (uint64_t)xodd;
     const uint32_t warp_global = (blockIdx.y * gridDim.x + blockIdx.x) * (SWEEP_THREADS / 32) + warp;
