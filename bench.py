@@ -210,6 +210,10 @@ def main():
     ap.add_argument("--slabs", type=int, default=0,
                     help="z-slab decomposition (PAPER.md section V) of the L^3 lattice into this many slabs, all on this GPU: sweep time "
                          "against the undivided lattice (the cost of the boundary / bulk split and of the plane exchange)")
+    ap.add_argument("--sliced", action="store_true",
+                    help="the paper's sliced layout (Eq. 4-6) against the rank-linear arrays: half-sweep time, both rng modes (MINSTD "
+                         "without the seed table on both sides: same generator work, only the layout differs)")
+    ap.add_argument("--sizes", default="", help="--sliced: comma-separated lattice sizes instead of 256,512,1024")
     ap.add_argument("--small", action="store_true",
                     help="small lattices: time per half-sweep with the automatic kernels (0), one launch per half-sweep (3) and the "
                          "persistent kernels everywhere (4), without records and with E and M after every half-sweep")
@@ -445,6 +449,45 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.sliced:
+        rows = []
+        for Ls in ([int(v) for v in args.sizes.split(",")] if args.sizes else [256, 512, 1024]):
+            sp = torch.from_numpy(synth.make_spins(Ls, 1).view(np.int32)).cuda()
+            Jc = torch.from_numpy(synth.make_couplings(Ls, 1).view(np.int32)).cuda()
+            for mode, choice in ((PHILOX, 3), (MINSTD, 2)):   # one launch per half-sweep on both sides; MINSTD seeds recomputed on both
+                g = Ising(Ls, 1, synth.DYN_SEED, mode)
+                g.ising_set_kernel(choice)
+                g.ising_load_state(sp, Jc)
+                nsweeps = max(2, min(50, int(4e9 / Ls**3)))
+                res = {}
+                for name in ("rank_linear", "sliced"):
+                    if name == "sliced":
+                        g.ising_sliced_begin()
+                    sweep = (lambda n: g.ising_sliced_sweep(BETA, n)) if name == "sliced" else (lambda n: g.ising_sweep(BETA, n))
+                    sweep(1)
+                    best = None
+                    for _ in range(3):
+                        torch.cuda.synchronize()
+                        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        a.record(stream)
+                        sweep(nsweeps)
+                        b.record(stream)
+                        torch.cuda.synchronize()
+                        ms = a.elapsed_time(b)
+                        best = ms if best is None or ms < best else best
+                    if name == "sliced":
+                        g.ising_sliced_end()
+                    res[name] = best
+                g.ising_destroy()
+                rows.append({"L": Ls, "rng_mode": ["philox", "minstd (seeds recomputed)"][mode], "sweeps": nsweeps,
+                             "rank_linear_half_sweep_us": 1e3 * res["rank_linear"] / (2 * nsweeps),
+                             "sliced_half_sweep_us": 1e3 * res["sliced"] / (2 * nsweeps),
+                             "rank_linear_ps_per_flip": 1e9 * res["rank_linear"] / (nsweeps * Ls**3),
+                             "sliced_ps_per_flip": 1e9 * res["sliced"] / (nsweeps * Ls**3)})
+            del sp, Jc
+        print(json.dumps({"sliced": rows}))
         return
 
     if args.slabs:

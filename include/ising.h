@@ -213,6 +213,21 @@ int ising_slab_plane(ising_t *h, int colour, int which, void **d_ptr, size_t *by
  * stream_b, an event pair between half-sweeps.  The two streams must differ; on return both have been made to wait for each other. */
 int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b);
 
+/* ---- the paper's sliced layout (Eq. 4-6; Appendix A) ----
+ * An alternative internal layout of a one-sample lattice, kept beside the handle's own arrays in a caller-owned scratch buffer:
+ * x' = x, y' = y - x, z' = x - y + z; planes of constant z' are one-coloured; the colours are separate arrays of L/2 planes of L x L
+ * sites, rows of 32-site words along x.  L must be 64 * 2^e, rng modes 0 and 1.  It exists to MEASURE the layout against the
+ * rank-linear arrays: the trajectory is the same bit for bit, but the Philox draws of R9, four consecutive
+ * canonical sites per call, cost one call per site here.
+ *   ising_sliced_scratch_bytes  size of the scratch (the eight sliced arrays; 256-byte aligned device memory)
+ *   ising_sliced_begin          handle's spins and couplings -> sliced arrays
+ *   ising_sliced_sweep          nsweeps sweeps on the sliced arrays (one launch per colour half-sweep); advances t
+ *   ising_sliced_end            sliced spins -> the handle's arrays (after which ising_energy / ising_get_spins see them) */
+int ising_sliced_scratch_bytes(const ising_t *h, size_t *out);
+int ising_sliced_begin(ising_t *h, void *d_scratch, void *stream);
+int ising_sliced_sweep(ising_t *h, void *d_scratch, double beta, int nsweeps, void *stream);
+int ising_sliced_end(ising_t *h, void *d_scratch, void *stream);
+
 /* Select the kernels: 0 = automatic (site-packed: the word-parallel kernel when L is a multiple of 64, with the cached seed
  * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
  * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),

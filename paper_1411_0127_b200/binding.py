@@ -21,7 +21,7 @@ EXPORTS = (
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
     "ising_slab_workspace_bytes", "ising_create_slab", "ising_slab_half_sweep_boundary", "ising_slab_half_sweep_bulk", "ising_slab_plane",
-    "ising_slab_sweep_local",
+    "ising_slab_sweep_local", "ising_sliced_scratch_bytes", "ising_sliced_begin", "ising_sliced_sweep", "ising_sliced_end",
 )
 
 _lib = None
@@ -70,6 +70,10 @@ def lib() -> C.CDLL:
     L.ising_slab_half_sweep_bulk.argtypes = [vp, dbl, vp]
     L.ising_slab_plane.argtypes = [vp, i32, i32, C.POINTER(vp), C.POINTER(sz)]
     L.ising_slab_sweep_local.argtypes = [C.POINTER(vp), i32, dbl, i32, vp, vp]
+    L.ising_sliced_scratch_bytes.argtypes = [vp, C.POINTER(sz)]
+    L.ising_sliced_begin.argtypes = [vp, vp, vp]
+    L.ising_sliced_sweep.argtypes = [vp, vp, dbl, i32, vp]
+    L.ising_sliced_end.argtypes = [vp, vp, vp]
     L.ising_destroy.argtypes = [vp]
     L.ising_strerror.argtypes = [i32]
     L.ising_strerror.restype = C.c_char_p
@@ -263,6 +267,26 @@ class Ising:
                                               _u32(h_spins_out) if h_spins_out is not None else None, h_E.data_ptr(),
                                               h_M.data_ptr() if h_M is not None else None, _stream_ptr(stream)),
                    "ising_run_host_async")
+
+    # -- the paper's sliced layout beside the handle's own (include/ising.h)
+    def ising_sliced_begin(self, stream=None):
+        """Allocates the scratch on first use and copies the handle's state into the sliced layout."""
+        import torch
+
+        if getattr(self, "_sliced", None) is None:
+            n = C.c_size_t(0)
+            _check(lib().ising_sliced_scratch_bytes(self._h, C.byref(n)), "ising_sliced_scratch_bytes")
+            self._sliced = torch.empty(n.value, dtype=torch.uint8, device=self.device)
+        with self._on_device():
+            _check(lib().ising_sliced_begin(self._h, self._sliced.data_ptr(), _stream_ptr(stream)), "ising_sliced_begin")
+
+    def ising_sliced_sweep(self, beta: float, nsweeps: int, stream=None):
+        with self._on_device():
+            _check(lib().ising_sliced_sweep(self._h, self._sliced.data_ptr(), float(beta), int(nsweeps), _stream_ptr(stream)), "ising_sliced_sweep")
+
+    def ising_sliced_end(self, stream=None):
+        with self._on_device():
+            _check(lib().ising_sliced_end(self._h, self._sliced.data_ptr(), _stream_ptr(stream)), "ising_sliced_end")
 
     def ising_get_t(self) -> int:
         t = C.c_uint64(0)

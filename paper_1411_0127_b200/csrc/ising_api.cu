@@ -12,6 +12,7 @@
 #include "measure_kernels.cuh"
 #include "persistent.cuh"
 #include "slab_kernels.cuh"
+#include "sliced_kernels.cuh"
 #include "sweep_kernels.cuh"
 
 using namespace isingk;
@@ -1387,6 +1388,81 @@ int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps
     cudaEventDestroy(ea);
     cudaEventDestroy(eb);
     return rc;
+}
+
+// ---- the paper's sliced layout as an alternative internal layout (sliced_kernels.cuh) ----
+static bool sliced_ok(const ising_t *h)
+{
+    if (!h || h->nslabs || h->g.nsamples != 1 || !h->g.fast) return false;
+    if (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD) return false;
+    const int wpr = h->g.L >> 5;                     // words per sliced row; lanes per row must be a power of two
+    return (wpr & (wpr - 1)) == 0;
+}
+static SlicedArrays sliced_arrays(const ising_t *h, void *d_scratch)
+{
+    SlicedArrays B;
+    uint32_t *base = (uint32_t *)d_scratch;
+    B.S[0] = base;
+    B.S[1] = base + h->g.array_words;
+    for (int d = 0; d < 3; ++d)
+        for (int c = 0; c < 2; ++c) B.J[d][c] = base + (size_t)(2 + 2 * d + c) * h->g.array_words;
+    return B;
+}
+
+int ising_sliced_scratch_bytes(const ising_t *h, size_t *out)
+{
+    if (!out || !sliced_ok(h)) return ISING_EINVAL;
+    *out = h->g.arrays_total_words * sizeof(uint32_t);
+    return ISING_OK;
+}
+
+int ising_sliced_begin(ising_t *h, void *d_scratch, void *stream)
+{
+    if (!sliced_ok(h) || !d_scratch || ((uintptr_t)d_scratch & 255u) || !on_own_device(h)) return ISING_EINVAL;
+    const uint32_t words = (uint32_t)(h->g.N >> 6);
+    to_sliced_layout<<<(8u * words + 255u) / 256u, 256, 0, (cudaStream_t)stream>>>(h->arrays(0), sliced_arrays(h, d_scratch), h->g.L);
+    return check_launch(h);
+}
+
+int ising_sliced_sweep(ising_t *h, void *d_scratch, double beta, int nsweeps, void *stream)
+{
+    if (!sliced_ok(h) || !d_scratch || nsweeps < 0 || !on_own_device(h)) return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    const Thresholds kt = kernel_thresholds(T);
+    const SlicedArrays B = sliced_arrays(h, d_scratch);
+    const int L = h->g.L, wpr = L >> 5, W = wpr >= 8 ? 4 : 1;
+    const unsigned grid = (unsigned)(((uint64_t)(L >> 1) * L * (wpr / W)) / 256u);
+    for (int k = 0; k < 2 * nsweeps; ++k) {
+        RngLaunch r;
+        fill_rng_launch(h, 0, &r);
+        SiteRng sr;
+        sr.pc = r.pc;
+        sr.ps = r.ps[0];
+        sr.seed = r.seed;
+        sr.A2 = 2u * r.A;
+        sr.s0tab = nullptr;
+        const int c = (int)(h->t & 1);
+        if (h->rng_mode == ISING_RNG_PHILOX) {
+            if (W == 4) launch_pdl(half_sweep_sliced<0, 4>, dim3(grid), dim3(256), (cudaStream_t)stream, B, sr, L, c, kt);
+            else launch_pdl(half_sweep_sliced<0, 1>, dim3(grid), dim3(256), (cudaStream_t)stream, B, sr, L, c, kt);
+        } else {
+            if (W == 4) launch_pdl(half_sweep_sliced<1, 4>, dim3(grid), dim3(256), (cudaStream_t)stream, B, sr, L, c, kt);
+            else launch_pdl(half_sweep_sliced<1, 1>, dim3(grid), dim3(256), (cudaStream_t)stream, B, sr, L, c, kt);
+        }
+        const int rc = check_launch(h);
+        if (rc != ISING_OK) return rc;
+        h->t += 1;
+    }
+    return ISING_OK;
+}
+
+int ising_sliced_end(ising_t *h, void *d_scratch, void *stream)
+{
+    if (!sliced_ok(h) || !d_scratch || !on_own_device(h)) return ISING_EINVAL;
+    const uint32_t words = (uint32_t)(h->g.N >> 6);
+    from_sliced_layout<<<(2u * words + 255u) / 256u, 256, 0, (cudaStream_t)stream>>>(sliced_arrays(h, d_scratch), h->arrays(0), h->g.L);
+    return check_launch(h);
 }
 
 int ising_set_kernel(ising_t *h, int which)
