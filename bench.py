@@ -207,6 +207,10 @@ def main():
     ap.add_argument("--aux", action="store_true",
                     help="rows a9 / a10 and the general-L kernels: load_state, energy, get_spins and a half-sweep per layout, with GB/s")
     ap.add_argument("--scan", action="store_true", help="ps/flip of the sweep kernels over lattice sizes and modes (sweeps only)")
+    ap.add_argument("--slab-ranks", action="store_true",
+                    help="strong scaling instead of replicas: the ONE L^3 lattice of config 5 cut into WORLD_SIZE z-slabs, one per rank / GPU "
+                         "(PAPER.md section V), the two boundary planes of every colour half-sweep exchanged with NCCL send / recv "
+                         "(paper_1411_0127_b200/slabs.py); prints its own JSON line with \"scaling\": \"strong\"")
     ap.add_argument("--slabs", type=int, default=0,
                     help="z-slab decomposition (PAPER.md section V) of the L^3 lattice into this many slabs, all on this GPU: sweep time "
                          "against the undivided lattice (the cost of the boundary / bulk split and of the plane exchange)")
@@ -449,6 +453,48 @@ def main():
             rows.append({"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd", "philox_shared"][mode], "sweeps": nsweeps,
                          "half_sweep_us": 1e3 * ms / (2 * nsweeps), "ps_per_flip": 1e9 * ms / (nsweeps * ns * Ls**3)})
         print(json.dumps({"scan": rows}))
+        return
+
+    if args.slab_ranks:
+        # Strong scaling by z-slab decomposition.  Not the default N > 1 path (replicas), and NOT measured on more
+        # than one GPU in this build (one GPU per gpurun call): with WORLD_SIZE = 1 the slab is the whole lattice with halos and the
+        # exchange is a local copy.
+        from paper_1411_0127_b200 import IsingSlab, slabs
+
+        slab = IsingSlab(L, world, rank, synth.DYN_SEED, PHILOX)
+        full_spins = torch.from_numpy(synth.make_spins(L).view(np.int32)).cuda()     # every rank builds the same lattice (seeds 2 / 1)
+        full_J = torch.from_numpy(synth.make_couplings(L).view(np.int32)).cuda()
+        bulk_stream = torch.cuda.Stream()
+
+        def step():
+            slab.ising_set_t(0)
+            slab.ising_load_state(full_spins, full_J)
+            slabs.slab_sweep_distributed(slab, BETA, nsw, dist, rank, world, bulk_stream)
+            return slab.ising_energy()
+
+        for _ in range(args.warmup):
+            step()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            E, M = step()
+        e1.record(stream)
+        barrier()
+        ms = max_over_ranks(e0.elapsed_time(e1))
+        Et = torch.tensor([int(E[0]), int(M[0])], dtype=torch.int64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(Et)
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": 1e9 * ms / (args.steps * nsw * N), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                              "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "strong",
+                              "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+                              "config": {**headline_config(L, nsw, world), "parallelism": f"{world} z-slabs of {L // world} planes, one per GPU",
+                                         "step": "load_state of the slab + sweeps (boundary kernel, plane exchange, bulk kernel) + energy share"},
+                              "final_energy": int(Et[0]), "final_magnetisation": int(Et[1]),
+                              "exchange_bytes_per_half_sweep_per_rank": 2 * L * L // 16}))
+        if dist is not None:
+            dist.destroy_process_group()
         return
 
     if args.sliced:

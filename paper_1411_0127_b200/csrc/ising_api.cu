@@ -334,11 +334,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
         } else if (g.fast && h->kernel_choice != 1) {
             const int wpr = g.L >> 6;
             const int W = g.W;
-            unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;   // ACC_SLOTS counter pairs + ticket (measure())
-            if ((mE || mM) && !h->slots_clean) {
-                if (cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
-                h->slots_clean = true;
-            }
+            unsigned long long *slots = nullptr;   // (the measuring variant adds to the pre-set record itself: add_to_record)
             const int tpr_pad = row_map_tpr_pad(wpr / W);
             const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
             SiteRng sr;
@@ -376,12 +372,8 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             sr.A2 = 2u * r.A;
             sr.s0tab = nullptr;
             if (g.L >= 64) {  // rows of at least 32 bits: no segment loop
-                unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;
+                unsigned long long *slots = nullptr;
                 if (mE || mM) {
-                    if (!h->slots_clean) {
-                        if (cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
-                        h->slots_clean = true;
-                    }
                     launch_pdl(half_sweep_site_packed_rows2<RNG, true>, dim3((unsigned)((nw + 127) / 128)), dim3(128), st, a, sr, (uint32_t)nw,
                                (uint32_t)g.Hc, slots, (long long)g.N, mE, mM);
                 } else {
@@ -995,7 +987,7 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
                 s.out[1 + d][0] = A.J[d][0];
                 s.out[1 + d][1] = A.J[d][1];
             }
-            gather_site_packed_rows<<<dim3((unsigned)((nw + 127) / 128), 8), 128, 0, st>>>(s, (uint32_t)nw, (uint32_t)g.Hc, (uint64_t)W);
+            gather_site_packed_rows<<<dim3((unsigned)((nw + 127) / 128), 4), 128, 0, st>>>(s, (uint32_t)nw, (uint32_t)g.Hc, (uint64_t)W);
             return check_launch(h);
         }
         const unsigned grid = (unsigned)((nw + 255) / 256);
@@ -1099,7 +1091,15 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
         if (rc != ISING_EINVAL) return rc;   // EINVAL (before anything ran): no cooperative launch on this device; use the launches
     }
     size_t rec = 0;
-    const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps write E and M themselves: no extra launch
+    const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps add E and M to the records themselves
+    if (fused) {   // ... which are pre-set to -3N / -N here (add_to_record)
+        const uint32_t nrec = (uint32_t)((2 * (size_t)nsweeps) / (size_t)every_half_sweeps);
+        if (nrec) {
+            init_records<<<(nrec + 255) / 256, 256, 0, st>>>((long long *)d_E, (long long *)d_M, nrec, (long long)h->g.N);
+            const int rc = check_launch(h);
+            if (rc != ISING_OK) return rc;
+        }
+    }
     for (int k = 1; k <= 2 * nsweeps; ++k) {
         const bool record = trace && k % every_half_sweeps == 0;
         long long *rE = record && d_E ? (long long *)d_E + rec * h->g.nsamples : nullptr;

@@ -43,7 +43,7 @@ struct SplitArgs {
 };
 
 template <int V>  // V internal words (2V canonical words) per thread, V <= L/64
-__global__ void __launch_bounds__(256) split_colours_site_packed(const SplitArgs a)
+__global__ void __launch_bounds__(256) split_colours_site_packed(const __grid_constant__ SplitArgs a)
 {
     typedef typename WordVec<V>::type Vec;
     const int L = a.L, wpr = L >> 6;
@@ -66,8 +66,17 @@ __global__ void __launch_bounds__(256) split_colours_site_packed(const SplitArgs
             even[k] = compress_even_bits(c[2 * k]) | (compress_even_bits(c[2 * k + 1]) << 16);
             odd[k] = compress_even_bits(c[2 * k] >> 1) | (compress_even_bits(c[2 * k + 1] >> 1) << 16);
         }
-        *reinterpret_cast<Vec *>(a.out[q][p] + widx) = *reinterpret_cast<const Vec *>(even);
-        *reinterpret_cast<Vec *>(a.out[q][1 - p] + widx) = *reinterpret_cast<const Vec *>(odd);
+        // the VALUE is selected by the row's parity, not the array: every store instruction of a warp then writes one array, its
+        // lanes' rows back to back (512 contiguous bytes), instead of alternating between the two arrays row by row, which
+        // left half-written lines behind (739 MB of DRAM writes for 537 MB of output at L = 1024, profiles/r1p_aux_kernels.md)
+        uint32_t for0[V], for1[V];
+#pragma unroll
+        for (int k = 0; k < V; ++k) {
+            for0[k] = p ? odd[k] : even[k];
+            for1[k] = p ? even[k] : odd[k];
+        }
+        __stcs(reinterpret_cast<Vec *>(a.out[q][0] + widx), *reinterpret_cast<const Vec *>(for0));
+        __stcs(reinterpret_cast<Vec *>(a.out[q][1] + widx), *reinterpret_cast<const Vec *>(for1));
     }
 }
 
@@ -82,8 +91,8 @@ merge_colours_site_packed(const uint32_t *__restrict__ S0, const uint32_t *__res
     if (widx >= n) return;
     const uint64_t r = widx / (unsigned)wpr;
     const int p = (int)((r % (unsigned)L) + (r / (unsigned)L)) & 1;
-    const Vec ve = *reinterpret_cast<const Vec *>((p ? S1 : S0) + widx);
-    const Vec vo = *reinterpret_cast<const Vec *>((p ? S0 : S1) + widx);
+    const Vec v0 = *reinterpret_cast<const Vec *>(S0 + widx), v1 = *reinterpret_cast<const Vec *>(S1 + widx);   // contiguous per warp
+    const Vec ve = p ? v1 : v0, vo = p ? v0 : v1;
     uint32_t out[2 * V];
 #pragma unroll
     for (int k = 0; k < V; ++k) {
@@ -150,27 +159,36 @@ __device__ __forceinline__ uint32_t canon_window(const uint32_t *__restrict__ a,
     return __funnelshift_r(lo, hi, sh);
 }
 
-// grid = (ceil(n_words / 128), 4 arrays x 2 colours)
+// grid = (ceil(n_words / 128), 4 arrays).  Word w of BOTH colour arrays comes from the same canonical sites (colour ranks
+// 32 w .. 32 w + 31 of either colour are the 64 sites 64 w .. 64 w + 63 of the rows they lie in): the even sites of a row segment
+// belong to the colour with xodd = 0 there, the odd ones to the other, so one pass over the canonical windows fills both words
+// (one pass per colour read every canonical word twice from HBM: 996 MB for 500 MB at L = 1000).
 __global__ void __launch_bounds__(128)
 gather_site_packed_rows(const __grid_constant__ SplitArgs a, uint32_t n_words, uint32_t Hc, uint64_t n_canon_words)
 {
     const uint32_t w = blockIdx.x * 128u + threadIdx.x;
     if (w >= n_words) return;
-    const int arr = blockIdx.y >> 1, c = blockIdx.y & 1;
+    const int arr = blockIdx.y;
     const uint32_t *__restrict__ canon = a.canon[arr];
     const uint32_t L = (uint32_t)a.L, H = L >> 1;
     const uint32_t j0 = 32u * w;
     uint32_t remaining = Hc - j0 < 32u ? Hc - j0 : 32u, bitoff = 0;
     uint32_t r = j0 / H, m = j0 - r * H, z = r / L, y = r - z * L;
-    uint32_t out = 0;
+    uint32_t out0 = 0, out1 = 0;   // colour 0 / colour 1
     while (remaining > 0) {
         const uint32_t len = remaining < H - m ? remaining : H - m;
         const uint32_t segmask = (len == 32u ? 0xFFFFFFFFu : ((1u << len) - 1u)) << bitoff;
-        const uint32_t xodd = (y + z + (uint32_t)c) & 1u;
-        const uint64_t base = (uint64_t)L * r + 2u * m + xodd;   // canonical site index of the segment's first site
-        uint32_t v = compress_even_bits(canon_window(canon, base, n_canon_words));
-        if (len > 16u) v |= compress_even_bits(canon_window(canon, base + 32u, n_canon_words)) << 16;
-        out |= (v << bitoff) & segmask;
+        const uint32_t p = (y + z) & 1u;                          // colour of the even sites of this row
+        const uint64_t base = (uint64_t)L * r + 2u * m;          // canonical index of the segment's first pair of sites
+        const uint32_t w0 = canon_window(canon, base, n_canon_words);
+        uint32_t even = compress_even_bits(w0), odd = compress_even_bits(w0 >> 1);
+        if (len > 16u) {
+            const uint32_t w1 = canon_window(canon, base + 32u, n_canon_words);
+            even |= compress_even_bits(w1) << 16;
+            odd |= compress_even_bits(w1 >> 1) << 16;
+        }
+        out0 |= ((p ? odd : even) << bitoff) & segmask;
+        out1 |= ((p ? even : odd) << bitoff) & segmask;
         bitoff += len;
         remaining -= len;
         m += len;
@@ -180,7 +198,8 @@ gather_site_packed_rows(const __grid_constant__ SplitArgs a, uint32_t n_words, u
             if (++y == L) { y = 0; ++z; }
         }
     }
-    a.out[arr][c][w] = out;
+    a.out[arr][0][w] = out0;
+    a.out[arr][1][w] = out1;
 }
 
 __global__ void __launch_bounds__(128)

@@ -83,14 +83,6 @@ struct PersistArgs {
     uint64_t N;                 // sites
 };
 
-__global__ void init_records(long long *E, long long *M, uint32_t n, long long N)
-{
-    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= n) return;
-    if (E) E[r] = -3 * N;
-    if (M) M[r] = -N;
-}
-
 // Site-packed, L a multiple of 64 (the word-parallel tile update of sweep_kernels.cuh), RNG 0 = Philox, 1 = MINSTD stateless,
 // 2 = MINSTD with the seed table.  grid = co-resident CTAs <= tiles; gx x gy tiles per half-sweep.  RECORDS = false leaves the
 // measuring variant of the tile update out of the kernel (fewer registers, more resident CTAs).
@@ -127,14 +119,7 @@ persistent_site_packed(const __grid_constant__ PersistArgs p, uint32_t gx, uint3
             publish_tile(p.epoch + tile, k + 1);
         }
         if (RECORDS && record) {
-            __shared__ unsigned long long cta_sum[2];
-            if (threadIdx.x == 0) { cta_sum[0] = 0; cta_sum[1] = 0; }
-            __syncthreads();
-            block_accumulate2(unsat, up, cta_sum);
-            if (threadIdx.x == 0) {   // warp 0 did the adds to cta_sum: thread 0 sees its own
-                if (p.E) atomicAdd(reinterpret_cast<unsigned long long *>(p.E + rec), 2ull * cta_sum[0]);
-                if (p.M) atomicAdd(reinterpret_cast<unsigned long long *>(p.M + rec), 2ull * cta_sum[1]);
-            }
+            add_to_record(unsat, up, p.E ? p.E + rec : nullptr, p.M ? p.M + rec : nullptr);
             ++rec;
         }
         if (RNG != 0 && c == 1) A = minstd_mulmod(16807u, A);   // the next half-sweep belongs to the next sweep: 16807^(n+2)

@@ -77,7 +77,7 @@ energy_site_packed_slab(const MeasureArgs a, int z0, unsigned long long *acc)
 
 // Canonical arrays of the WHOLE lattice -> the slab's arrays (all Lz + 2 local planes, halos included), for `narrays` canonical bit
 // arrays at once; one thread per internal word.  Local plane zl holds lattice plane (z0 - 1 + zl) mod L.
-__global__ void __launch_bounds__(256) split_colours_slab(const SplitArgs a, int z0, int planes /* Lz + 2 */)
+__global__ void __launch_bounds__(256) split_colours_slab(const __grid_constant__ SplitArgs a, int z0, int planes /* Lz + 2 */)
 {
     const int L = a.L, wpr = L >> 6;
     const uint64_t n = (uint64_t)wpr * L * planes;

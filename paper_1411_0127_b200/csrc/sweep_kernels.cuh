@@ -122,6 +122,29 @@ __device__ __forceinline__ void finalize_slots_last_cta(unsigned long long *acc,
     }
 }
 
+// A recording half-sweep adds its counts straight into the record: E[0] and M[0] were pre-set to -3N and -N (init_records) and
+// receive 2 x (unsatisfied bonds) and 2 x (up spins) (R16) by one atomic pair per CTA.  Nothing waits for the sum: no ticket, no
+// last-CTA pass (that tail cost a recording launch 1.5 us at L = 256).
+__device__ __forceinline__ void add_to_record(unsigned long long unsat, unsigned long long up, long long *E, long long *M)
+{
+    __shared__ unsigned long long cta_sum[2];
+    if (threadIdx.x == 0) { cta_sum[0] = 0; cta_sum[1] = 0; }
+    __syncthreads();
+    block_accumulate2(unsat, up, cta_sum);   // warp 0 adds the CTA's totals to cta_sum; thread 0 then sees its own adds
+    if (threadIdx.x == 0) {
+        if (E) atomicAdd(reinterpret_cast<unsigned long long *>(E), 2ull * cta_sum[0]);
+        if (M) atomicAdd(reinterpret_cast<unsigned long long *>(M), 2ull * cta_sum[1]);
+    }
+}
+
+__global__ void init_records(long long *E, long long *M, uint32_t n, long long N)
+{
+    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    if (E) E[r] = -3 * N;
+    if (M) M[r] = -N;
+}
+
 template <int W> struct WordVec;
 template <> struct WordVec<1> { typedef uint32_t type; };
 template <> struct WordVec<2> { typedef uint2 type; };
@@ -440,10 +463,7 @@ half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constan
 {
     unsigned long long unsat = 0, up = 0;
     site_packed_tile<RNG, W, MEASURE, false>(a, rng, blockIdx.x, blockIdx.y, gridDim.x, unsat, up);
-    if (MEASURE) {
-        block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
-        finalize_slots_last_cta(acc, N, E, M);
-    }
+    if (MEASURE) add_to_record(unsat, up, E, M);
 }
 
 // Fills the seed table of colour `colour` with the thread mapping of half_sweep_site_packed<2, W> (same grid).
@@ -748,8 +768,7 @@ half_sweep_site_packed_rows2(const SweepArgs a, const __grid_constant__ SiteRng 
                              2 * (__popc(sum0 & f) + 2 * __popc(sum1 & f) + 4 * __popc(sum2 & f));
         const unsigned long long unsat = live ? 6ull * nvalid - sat : 0ull;
         const unsigned long long up = live ? (unsigned long long)(__popc((s ^ f) & valid) + __popc(other_word & valid)) : 0ull;
-        block_accumulate2(unsat, up, acc + 2 * (blockIdx.x & (ACC_SLOTS - 1)));
-        finalize_slots_last_cta(acc, N, E, M);
+        add_to_record(unsat, up, E, M);
     }
 }
 

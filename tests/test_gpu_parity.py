@@ -832,11 +832,12 @@ def test_persistent_kernel_long_call(rng_mode):
 @pytest.mark.parametrize("L", [4, 6, 10, 16, 18, 22, 24, 32, 34, 40])
 def test_on_chip_kernel_equals_the_oracle_and_one_launch_per_half_sweep(L, rng_mode):
     """Lattices of at most 1024 words per colour (every even L <= 40) run all half-sweeps and records of a call in ONE launch of ONE
-    CTA out of shared memory (half_sweeps_on_chip; automatic).  Against the oracle half-sweep by half-sweep (E and M records of
+    CTA out of shared memory (half_sweeps_on_chip).  Against the oracle half-sweep by half-sweep (E and M records of
     every spacing, red and blue), against one launch per half-sweep (kernel choice 3), from an odd starting counter, across
     several calls (the spins go back to global memory after every call), with the separate energy and get kernels afterwards."""
     spins, J = synth.make_spins(L, 1, 77), synth.make_couplings(L, 1, 78)
     o, a = make_pair(L, 1, rng_mode, spins, J)
+    a.ising_set_kernel(4)     # wherever it exists (automatic where it is the faster one: up to L = 32 with records, 24 without)
     b = Ising(L, 1, SEED, rng_mode)
     b.ising_set_kernel(3)
     b.ising_load_state(dev(spins), dev(J))
@@ -886,3 +887,31 @@ def test_config1_through_every_launch_structure():
     for r in res[1:]:
         assert all(torch.equal(x, y) for x, y in zip(res[0][:3], r[:3]))
     assert res[0][3] == 1 + 1 + 1 and res[1][3] >= 1 + 20 + 20      # load + one launch + get   against   load + 20 x (sweep + energy) + get
+
+
+def test_handle_belongs_to_the_current_device():
+    """A handle is created on torch's current device and every call runs there (the binding used to default to
+    cuda:0 whatever the process had selected).  With a second GPU visible, the same job on device 1 gives the same bits, and the
+    library refuses a call made with another device current."""
+    g = Ising(64, 1, SEED, PHILOX)
+    assert g.device.index == torch.cuda.current_device() and g.workspace.device == g.device
+    if torch.cuda.device_count() < 2:
+        return
+    spins, J = synth.make_spins(64, 1, 2), synth.make_couplings(64, 1, 1)
+    g.ising_load_state(dev(spins), dev(J))
+    g.ising_sweep(0.9, 3)
+    with torch.cuda.device(1):
+        h = Ising(64, 1, SEED, PHILOX)
+        assert h.device.index == 1 and h.workspace.device.index == 1
+        sp1 = torch.from_numpy(spins.view(np.int32)).to("cuda:1")
+        J1 = torch.from_numpy(J.view(np.int32)).to("cuda:1")
+        h.ising_load_state(sp1, J1)
+        h.ising_sweep(0.9, 3)
+        out1 = h.ising_get_spins()
+        assert out1.device.index == 1
+    assert torch.equal(out1.cpu(), g.ising_get_spins().cpu())
+    h.ising_sweep(0.9, 1)      # called with device 0 current: the binding switches to the handle's device for the call
+    with pytest.raises(AssertionError):
+        h.ising_load_state(dev(spins), dev(J))   # tensors of device 0 handed to a handle of device 1
+    # the C library itself refuses a launch for a handle of another device than the current one
+    assert binding.lib().ising_sweep(h._h, 0.9, 1, None) == binding.EINVAL
