@@ -4,9 +4,11 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 
 #include "../../include/ising.h"
+#include "graph_kernels.cuh"
 #include "lane_rng.cuh"
 #include "layout_kernels.cuh"
 #include "measure_kernels.cuh"
@@ -70,8 +72,8 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
     // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs and the ticket of the word-parallel energy kernel
-    // ... + overlap counter (2)
-    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1 + 2) * sizeof(unsigned long long), 256);
+    // ... + overlap counter (2), then (256-byte aligned) the device copy of the handle's slot of graph constants (graph_kernels.cuh)
+    g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1 + 2) * sizeof(unsigned long long), 256) + round_up(sizeof(DynConst), 256);
     g->fast = nsamples == 1 && L % 64 == 0;
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
     // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
@@ -121,6 +123,15 @@ struct ising {
     bool slots_clean;  // the slots and the ticket of the fused energy kernel are zero (it leaves them so)
     bool overlap_clean;  // the counter of ising_overlap is zero
     int device;          // CUDA device the workspace lives on (-1: unknown, e.g. no device present)
+    // CUDA-graph path (graph_kernels.cuh): the handle's constant slot (-1: none yet / none free), the device copy of its contents, a
+    // private stream to capture on (the caller's may be the legacy default stream), and the instantiated graphs
+    struct GraphEntry { cudaGraphExec_t exec; uint32_t K, every; bool records; uint64_t last_use; };
+    int dyn_slot;
+    DynConst *dyn;
+    cudaStream_t cap_stream;
+    GraphEntry graphs[8];
+    int ngraphs;
+    uint64_t graph_clock;
     int nslabs, slab, z0, Lz;  // z-slab handles (ising_create_slab): this handle owns the planes z0 .. z0 + Lz - 1; nslabs = 0 otherwise
     unsigned int *epochs;  // tile epochs of the persistent kernels (nullptr: no persistent path for this geometry / mode)
     int persist_grid[2];   // co-resident CTAs of this handle's persistent kernel without / with records (0: not asked yet, -1: none)
@@ -152,6 +163,7 @@ int check_launch(ising_t *h, int n = 1)
 // The workspace of a handle lives on one device (recorded by ising_create); every launch must be made with that device
 // current, or the kernels would dereference another GPU's memory (peer access) or fault (none).
 bool on_own_device(const ising_t *h);
+void release_graphs(ising_t *h);
 int slab_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, cudaStream_t st);
 int slab_get_spins(ising_t *h, uint32_t *d_out, cudaStream_t st);
 int slab_energy(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st);
@@ -474,11 +486,9 @@ bool persistent_available(const ising_t *h, bool records)
         return records ? nw <= 512 : nw <= 216;
     }
     if (!h->epochs) return false;
-    if (h->kernel_choice == 4) return true;                                      // wherever there is a tile grid (L <= 448)
-    // automatic: where it beats the launches (profiles/r2b_persistent.md).  Without records the tile flags cost what the launch
-    // gap costs (2.3-2.6 us per half-sweep either way at L = 64, 128) and the launches win from L = 192 on; with records the
-    // persistent kernel's atomics into the record beat the last-CTA finalisation of a recording launch (3.2 against 4.5 us).
-    return (h->kernel_choice == 0 || h->kernel_choice == 2) && h->g.L <= 128 && records;
+    // the dataflow kernel: on request only (kernel choice 4).  Its tile flags cost 1.4 us per half-sweep where a graph replay
+    // (graph_kernels.cuh, the automatic choice for these lattices) costs 0.5-0.9 us (profiles/r2j_launch_floor.md)
+    return h->kernel_choice == 4;
 }
 
 template <typename Kernel>
@@ -609,6 +619,168 @@ int sweep_persistent(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t e
         done += n;
         if (records) rec += n / every;
     }
+    return ISING_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// CUDA-graph path (graph_kernels.cuh): K half-sweeps per replay, for lattices whose half-sweep is shorter than a launch.
+// ---------------------------------------------------------------------------------------------------------------------
+std::mutex g_slot_mutex;
+bool g_slot_used[DYN_SLOTS] = {};
+
+void release_graphs(ising_t *h)
+{
+    for (int i = 0; i < h->ngraphs; ++i) cudaGraphExecDestroy(h->graphs[i].exec);
+    h->ngraphs = 0;
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    h->cap_stream = nullptr;
+    if (h->dyn_slot >= 0) {
+        std::lock_guard<std::mutex> lock(g_slot_mutex);
+        g_slot_used[h->dyn_slot] = false;
+        h->dyn_slot = -1;
+    }
+}
+
+// Which calls replay graphs: automatic kernels (choice 0 / 2), one-sample lattices with whole-word rows up to L = 128 (where a
+// half-sweep kernel is shorter than a launch: profiles/r2j_launch_floor.md), Philox or MINSTD.
+bool graph_geometry(const ising_t *h)
+{
+    const Geometry &g = h->g;
+    if (h->nslabs || (h->kernel_choice != 0 && h->kernel_choice != 2)) return false;
+    if (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD) return false;
+    return g.nsamples == 1 && g.fast && g.L <= 128;
+}
+
+bool acquire_slot(ising_t *h)
+{
+    if (h->dyn_slot >= 0) return true;
+    std::lock_guard<std::mutex> lock(g_slot_mutex);
+    for (int i = 0; i < DYN_SLOTS; ++i)
+        if (!g_slot_used[i]) {
+            g_slot_used[i] = true;
+            h->dyn_slot = i;
+            return true;
+        }
+    return false;
+}
+
+template <int RNG, int W>
+void capture_site_step(ising_t *h, bool rec, uint4 *tab0, uint4 *tab1, uint32_t k, uint32_t rec_off)
+{
+    const Geometry &g = h->g;
+    const dim3 grid(g.pgx, g.pgy);
+    const LatticeArrays A = h->arrays(0);
+    // captured with the programmatic-stream-serialization attribute: the edges between the half-sweeps of the graph become
+    // programmatic dependencies, i.e. the next kernel's CTAs start while the previous one drains, as in the stream launches
+    if (rec) launch_pdl(half_sweep_site_packed_graph<RNG, W, true>, grid, dim3(SWEEP_THREADS), h->cap_stream, A, g.L, h->seed, tab0, tab1, h->dyn_slot, k, rec_off);
+    else launch_pdl(half_sweep_site_packed_graph<RNG, W, false>, grid, dim3(SWEEP_THREADS), h->cap_stream, A, g.L, h->seed, tab0, tab1, h->dyn_slot, k, rec_off);
+}
+template <int RNG>
+void capture_site_step(ising_t *h, bool rec, uint4 *tab0, uint4 *tab1, uint32_t k, uint32_t rec_off)
+{
+    if (h->g.W == 3) capture_site_step<RNG, 3>(h, rec, tab0, tab1, k, rec_off);
+    else if (h->g.W == 5) capture_site_step<RNG, 5>(h, rec, tab0, tab1, k, rec_off);
+    else capture_site_step<RNG, 1>(h, rec, tab0, tab1, k, rec_off);
+}
+
+// The instantiated graph of K half-sweeps with a record after every `every`-th, built on first use.
+cudaGraphExec_t get_graph(ising_t *h, uint32_t K, uint32_t every, bool records)
+{
+    ++h->graph_clock;
+    for (int i = 0; i < h->ngraphs; ++i)
+        if (h->graphs[i].K == K && h->graphs[i].records == records && (!records || h->graphs[i].every == every)) {
+            h->graphs[i].last_use = h->graph_clock;
+            return h->graphs[i].exec;
+        }
+    if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+    DynConst *slot_addr = nullptr;
+    if (cudaGetSymbolAddress((void **)&slot_addr, c_dyn) != cudaSuccess) return nullptr;
+    slot_addr += h->dyn_slot;
+    const Geometry &g = h->g;
+    const bool table = g.nsamples == 1 && h->rng_mode == ISING_RNG_MINSTD && h->kernel_choice != 2 && h->s0tab != nullptr;
+    uint4 *tab0 = table ? (uint4 *)h->s0tab : nullptr, *tab1 = table ? (uint4 *)(h->s0tab + g.s0_words / 2) : nullptr;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) return nullptr;
+    dyn_prepare<<<1, DYN_MAX_SWEEPS, 0, h->cap_stream>>>(h->dyn);
+    cudaMemcpyAsync(slot_addr, h->dyn, sizeof(DynConst), cudaMemcpyDeviceToDevice, h->cap_stream);
+    uint32_t rec_off = 0;
+    for (uint32_t k = 0; k < K; ++k) {
+        const bool rec = records && (k + 1) % every == 0;
+        if (h->rng_mode == ISING_RNG_PHILOX) capture_site_step<0>(h, rec, tab0, tab1, k, rec_off);
+        else if (table) capture_site_step<2>(h, rec, tab0, tab1, k, rec_off);
+        else capture_site_step<1>(h, rec, tab0, tab1, k, rec_off);
+        if (rec) ++rec_off;
+    }
+    dyn_advance<<<1, 1, 0, h->cap_stream>>>(h->dyn, K, rec_off);
+    const bool launch_failed = g_launch_failed;
+    g_launch_failed = false;
+    const bool captured = cudaStreamEndCapture(h->cap_stream, &graph) == cudaSuccess && graph != nullptr && !launch_failed;
+    cudaGraphExec_t exec = nullptr;
+    if (captured && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+    if (graph) cudaGraphDestroy(graph);
+    if (!exec) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    int at = h->ngraphs;
+    if (at == 8) {   // evict the least recently used
+        at = 0;
+        for (int i = 1; i < 8; ++i)
+            if (h->graphs[i].last_use < h->graphs[at].last_use) at = i;
+        cudaGraphExecDestroy(h->graphs[at].exec);
+    } else {
+        ++h->ngraphs;
+    }
+    h->graphs[at] = {exec, K, every, records, h->graph_clock};
+    return exec;
+}
+
+// Replays graphs for as many whole chunks of K half-sweeps as fit into nhalf; returns the number of half-sweeps done (0: none, the
+// caller launches them), *nrec = records written.  Records (site-packed only): E / M pre-set by the caller.
+int sweep_graphs(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t every, long long *d_E, long long *d_M, cudaStream_t st,
+                 uint32_t *done, uint32_t *nrec)
+{
+    *done = 0;
+    *nrec = 0;
+    const bool records = every != 0 && (d_E || d_M);
+    if (!graph_geometry(h)) return ISING_OK;
+    uint32_t K;
+    if (records) {
+        if (every > 64) return ISING_OK;
+        const uint32_t cap = nhalf < 64 ? nhalf : 64;
+        K = every * (cap / every);
+    } else {
+        K = nhalf < 64 ? nhalf : 64;
+    }
+    if (K < 16 || !acquire_slot(h)) return ISING_OK;   // short calls are not worth a graph (building one costs a few hundred launches)
+    if (h->rng_mode == ISING_RNG_MINSTD && h->g.nsamples == 1 && h->kernel_choice != 2 && h->s0tab && !h->s0_ready) {
+        uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + h->g.s0_words / 2)};
+        const dim3 grid(h->g.pgx, h->g.pgy);
+        for (int cc = 0; cc < 2; ++cc) {
+            if (h->g.W == 3) minstd_fill_s0<3><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], h->g.L, cc, h->seed);
+            else if (h->g.W == 5) minstd_fill_s0<5><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], h->g.L, cc, h->seed);
+            else minstd_fill_s0<1><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], h->g.L, cc, h->seed);
+        }
+        const int rc = check_launch(h, 2);
+        if (rc != ISING_OK) return rc;
+        h->s0_ready = true;
+    }
+    cudaGraphExec_t exec = get_graph(h, K, every, records);
+    if (!exec) return ISING_OK;   // no graph: the caller's launches do the work
+    dyn_begin<<<1, 1, 0, st>>>(h->dyn, (unsigned long long)h->t, h->rng_mode == ISING_RNG_MINSTD ? 1u : 0u, records ? d_E : nullptr,
+                               records ? d_M : nullptr, T);
+    int rc = check_launch(h);
+    if (rc != ISING_OK) return rc;
+    const uint32_t nrep = nhalf / K;
+    for (uint32_t r = 0; r < nrep; ++r)
+        if (cudaGraphLaunch(exec, st) != cudaSuccess) {
+            cudaGetLastError();
+            return ISING_ECUDA;
+        }
+    h->launches += (uint64_t)nrep * (K + 2);
+    h->t += (uint64_t)nrep * K;
+    *done = nrep * K;
+    *nrec = records ? nrep * (K / every) : 0;
     return ISING_OK;
 }
 
@@ -914,6 +1086,11 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->lanes_ready = false;
     h->persist_grid[0] = h->persist_grid[1] = 0;
     h->nslabs = h->slab = h->z0 = h->Lz = 0;
+    h->dyn_slot = -1;
+    h->dyn = (DynConst *)((char *)h->acc + h->g.acc_bytes - round_up(sizeof(DynConst), 256));
+    h->cap_stream = nullptr;
+    h->ngraphs = 0;
+    h->graph_clock = 0;
     h->epochs = nullptr;
     if (h->g.epoch_words && !lane_mode(rng_mode)) {   // the last area of the workspace
         h->epochs = (unsigned int *)((char *)d_workspace + need - round_up(h->g.epoch_words * sizeof(uint32_t), 256));
@@ -939,6 +1116,7 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
 
 int ising_destroy(ising_t *h)
 {
+    if (h) release_graphs(h);
     delete h;
     return ISING_OK;
 }
@@ -1091,6 +1269,7 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
         if (rc != ISING_EINVAL) return rc;   // EINVAL (before anything ran): no cooperative launch on this device; use the launches
     }
     size_t rec = 0;
+    int k_first = 1;
     const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps add E and M to the records themselves
     if (fused) {   // ... which are pre-set to -3N / -N here (add_to_record)
         const uint32_t nrec = (uint32_t)((2 * (size_t)nsweeps) / (size_t)every_half_sweeps);
@@ -1100,7 +1279,17 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
             if (rc != ISING_OK) return rc;
         }
     }
-    for (int k = 1; k <= 2 * nsweeps; ++k) {
+    // whole chunks of half-sweeps replayed from a graph where a half-sweep is shorter than a launch (graph_kernels.cuh) ...
+    if (nsweeps >= 1 && (!trace || fused)) {
+        uint32_t done = 0, nrec = 0;
+        const int rc = sweep_graphs(h, kt, 2u * (uint32_t)nsweeps, trace ? (uint32_t)every_half_sweeps : 0u, (long long *)d_E, (long long *)d_M, st,
+                                    &done, &nrec);
+        if (rc != ISING_OK) return rc;
+        k_first += (int)done;
+        rec += nrec;
+    }
+    // ... the rest (or everything) one launch per half-sweep
+    for (int k = k_first; k <= 2 * nsweeps; ++k) {
         const bool record = trace && k % every_half_sweeps == 0;
         long long *rE = record && d_E ? (long long *)d_E + rec * h->g.nsamples : nullptr;
         long long *rM = record && d_M ? (long long *)d_M + rec * h->g.nsamples : nullptr;

@@ -148,8 +148,8 @@ ISING_HD uint32_t minstd_mulmod2(uint32_t A2, uint32_t s0)
     return (x1 & MINSTD_M) + (x1 >> 31);
 }
 
-inline uint32_t minstd_power(uint64_t n_plus_1)
-{  // 16807^(n+1) mod M by square-and-multiply (host, once per sweep)
+ISING_HD uint32_t minstd_power(uint64_t n_plus_1)
+{  // 16807^(n+1) mod M by square-and-multiply (host: once per sweep; device: graph_kernels.cuh, once per graph replay)
     uint64_t base = 16807u, acc = 1u, e = n_plus_1;
     while (e) {
         if (e & 1) acc = (acc * base) % MINSTD_M;

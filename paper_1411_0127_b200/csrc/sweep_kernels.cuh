@@ -1030,10 +1030,10 @@ half_sweep_shared_vec(SweepArgs a, const SharedRng rng, uint32_t gpr /* groups p
 // MULTI: all coded batches in one launch (blockIdx.z = batch, arrays batch_stride words apart).  The launch constants
 // cannot be folded per (batch, sample) then, so the plain ten Philox rounds are run with the key (k0, k1base ^ sample);
 // a small lattice with many batches is one launch instead of one per batch.
-template <int RNG, int PARTS, bool MULTI>
-__global__ void __launch_bounds__(128)
-half_sweep_sample_packed_vec(SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t gpr, uint32_t gpr_inv, uint64_t N,
-                             size_t batch_stride)
+// The body of half_sweep_sample_packed_vec (one launch per half-sweep) and of half_sweep_sample_packed_vec_graph (graph_kernels.cuh);
+// RL = RngLaunch, or any struct with the fields the chosen variant reads (MULTI: tlo, thi, k0, k1base, seed, A only).
+template <int RNG, int PARTS, bool MULTI, typename RL>
+__device__ __forceinline__ void sample_packed_vec_body(SweepArgs a, const RL &rng, uint32_t gpr, uint32_t gpr_inv, uint64_t N, size_t batch_stride)
 {
     constexpr int SPT = 32 / PARTS;
     const uint32_t L = (uint32_t)a.L;
@@ -1060,10 +1060,10 @@ half_sweep_sample_packed_vec(SweepArgs a, const __grid_constant__ RngLaunch rng,
     for (int i = 0; i < SPT; i += 2) {
         const int b = SPT * part + i;
         uint32_t R[8];
-        if (RNG == 0 && MULTI) {
+        if constexpr (RNG == 0 && MULTI) {
             philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ (sample0 + (uint32_t)b), R);
             philox4x32_10(rng.tlo, rng.thi, g, 0u, rng.k0, rng.k1base ^ (sample0 + (uint32_t)b + 1u), R + 4);
-        } else if (RNG == 0) {
+        } else if constexpr (RNG == 0) {
             philox_folded(rng.pc, rng.ps[b], g, R);
             philox_folded(rng.pc, rng.ps[b + 1], g, R + 4);
         } else {
@@ -1106,6 +1106,14 @@ half_sweep_sample_packed_vec(SweepArgs a, const __grid_constant__ RngLaunch rng,
 #pragma unroll
         for (int w = 0; w < 4; ++w) reinterpret_cast<unsigned char *>(a.S_act + j0 + w)[part] = (unsigned char)out[w];  // little-endian
     }
+}
+
+template <int RNG, int PARTS, bool MULTI>
+__global__ void __launch_bounds__(128)
+half_sweep_sample_packed_vec(SweepArgs a, const __grid_constant__ RngLaunch rng, uint32_t gpr, uint32_t gpr_inv, uint64_t N,
+                             size_t batch_stride)
+{
+    sample_packed_vec_body<RNG, PARTS, MULTI>(a, rng, gpr, gpr_inv, N, batch_stride);
 }
 
 }  // namespace isingk

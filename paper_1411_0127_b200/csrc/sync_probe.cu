@@ -8,6 +8,7 @@
 #include <cooperative_groups.h>
 #include <cstdio>
 #include <cstdint>
+
 namespace cg = cooperative_groups;
 
 __device__ __forceinline__ void grid_barrier(unsigned int *counter, unsigned int &target)
@@ -68,8 +69,58 @@ __global__ void __cluster_dims__(8, 1, 1) k_cluster(int n)
     cg::cluster_group c = cg::this_cluster();
     for (int i = 0; i < n; ++i) c.sync();
 }
+// launch floor: empty (and 1 us) kernels launched into a stream, plainly and with programmatic stream serialization, and replayed
+// from an instantiated graph of 200 nodes
+__global__ void k_empty(int *p) { asm volatile("griddepcontrol.wait;" ::: "memory"); if (p && threadIdx.x == 1000) *p = 1; }
+__global__ void k_work(int *p, int n)
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    int v = threadIdx.x;
+    for (int i = 0; i < n; ++i) v = v * 1664525 + 1013904223;
+    if (v == 12345) *p = v;
+}
+template <typename... A> void launch_pdl(void (*k)(A...), dim3 g, dim3 b, cudaStream_t st, A... a)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = g; cfg.blockDim = b; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k, a...);
+}
+static void launch_floor()
+{
+    int *d; cudaMalloc(&d, 4);
+    cudaStream_t st; cudaStreamCreate(&st);
+    cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+    const int N = 20000;
+    const char *names[4] = {"stream launch, empty kernel", "stream launch + programmatic dependent launch, empty kernel",
+                            "stream launch + programmatic dependent launch, 1 us kernel", "graph of 200 empty kernels, replayed"};
+    for (int mode = 0; mode < 4; ++mode) for (int grid : {16, 148, 1024}) {
+        for (int i = 0; i < 100; ++i) k_empty<<<grid, 128, 0, st>>>(d);
+        cudaStreamSynchronize(st);
+        cudaEventRecord(a, st);
+        if (mode == 0) for (int i = 0; i < N; ++i) k_empty<<<grid, 128, 0, st>>>(d);
+        if (mode == 1) for (int i = 0; i < N; ++i) launch_pdl(k_empty, dim3(grid), dim3(128), st, d);
+        if (mode == 2) for (int i = 0; i < N; ++i) launch_pdl(k_work, dim3(grid), dim3(128), st, d, 2000);
+        if (mode == 3) {
+            cudaGraph_t g; cudaGraphExec_t ge;
+            cudaStreamBeginCapture(st, cudaStreamCaptureModeGlobal);
+            for (int i = 0; i < 200; ++i) k_empty<<<grid, 128, 0, st>>>(d);
+            cudaStreamEndCapture(st, &g); cudaGraphInstantiate(&ge, g, 0);
+            cudaEventRecord(a, st);
+            for (int i = 0; i < N / 200; ++i) cudaGraphLaunch(ge, st);
+        }
+        cudaEventRecord(b, st); cudaEventSynchronize(b);
+        float ms; cudaEventElapsedTime(&ms, a, b);
+        printf("%-64s grid %4d x 128 threads: %.3f us per kernel\n", names[mode], grid, 1e3 * ms / N);
+    }
+}
+
 int main()
 {
+    launch_floor();
     unsigned int *ctr; uint32_t *data; unsigned int *flag;
     cudaMalloc(&ctr, 4); cudaMalloc(&data, 4 * 2048 * 1024); cudaMalloc(&flag, 4 * 32 * 4096);
     cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);

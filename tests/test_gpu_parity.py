@@ -810,22 +810,93 @@ def test_persistent_kernel_equals_one_launch_per_half_sweep(L, rng_mode):
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
-def test_persistent_kernel_long_call(rng_mode):
-    """66000 half-sweeps in one call = one cooperative launch, records every 1001 half-sweeps; against one launch per half-sweep."""
+def test_long_recorded_call_through_every_launch_structure(rng_mode):
+    """66000 half-sweeps in one call with a record every 1001 (too far apart for a graph with records: one launch per half-sweep),
+    the persistent kernel (choice 4: one cooperative launch) and one launch per half-sweep (choice 3): same records and spins."""
     L, nsw, every = 64, 33000, 1001
     spins, J = synth.make_spins(L, 1, 73), synth.make_couplings(L, 1, 74)
     res = []
-    for choice in (0, 3):      # a recorded call at L = 64: the persistent kernel is the automatic choice
+    for choice in (0, 4, 3):
         g = Ising(L, 1, SEED, rng_mode)
         g.ising_set_kernel(choice)
         g.ising_load_state(dev(spins), dev(J))
-        l0 = g.ising_kernel_launches()
         E, M = g.ising_sweep_trace(1 / 1.1, nsw, every_half_sweeps=every)
-        res.append((E.clone(), M.clone(), g.ising_get_spins().clone(), g.ising_kernel_launches() - l0))
+        res.append((E.clone(), M.clone(), g.ising_get_spins().clone()))
         assert g.ising_get_t() == 2 * nsw
     assert res[0][0].shape[0] == (2 * nsw) // every
-    assert all(torch.equal(x, y) for x, y in zip(res[0][:3], res[1][:3]))
-    assert res[0][3] <= 6 and res[1][3] >= 2 * nsw
+    for r in res[1:]:
+        assert all(torch.equal(x, y) for x, y in zip(res[0], r))
+
+
+@pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
+@pytest.mark.parametrize("L,nsamples", [(64, 1), (128, 1), (192, 1), (64, 32)])
+def test_graph_replays_equal_one_launch_per_half_sweep(L, nsamples, rng_mode):
+    """Calls of 16 half-sweeps and more on the one-sample lattices L = 64 and 128 replay CUDA graphs of up to 64 half-sweeps whose
+    kernels take the half-sweep counter, the thresholds and the record position from a slot of constant memory (graph_kernels.cuh;
+    automatic); kernel choice 3 keeps one launch per half-sweep (as does every other geometry: L = 192 and the sample-packed
+    lattice are here to show that the same calls go through there too).  Same spins and records: calls of different lengths (graph
+    cache, remainders launched), record spacings 1, 2, 3, 7 and 20, another beta, an odd starting counter across 2^32, and the
+    oracle at the small sizes."""
+    spins, J = synth.make_spins(L, nsamples, 87), synth.make_couplings(L, nsamples, 88)
+    a = Ising(L, nsamples, SEED, rng_mode)
+    b = Ising(L, nsamples, SEED, rng_mode)
+    b.ising_set_kernel(3)
+    small = nsamples * L**3 <= 64**3 * 2
+    o = _loaded(L, nsamples, rng_mode, spins, J) if small else None
+    for g in (a, b):
+        g.ising_load_state(dev(spins), dev(J))
+    la = a.ising_kernel_launches()
+    for beta, n in ((1 / 1.1, 40), (0.6, 9), (1 / 1.1, 37), (0.6, 40)):     # 80 = 64 + 16 launched; 18; 74 = 64 + 10; again 80
+        a.ising_sweep(beta, n)
+        b.ising_sweep(beta, n)
+        assert torch.equal(a.ising_get_spins(), b.ising_get_spins()), (beta, n)
+        if o is not None:
+            o.sweep(beta, n)
+    if nsamples == 1 and L <= 128:
+        assert a.ising_kernel_launches() - la > 4 * 66      # the replays count their kernels (64 half-sweeps + 2 per replay)
+    if o is not None:
+        assert_same_state(o, a, f"graphs L={L} x {nsamples}")
+    for every, n in ((1, 20), (2, 33), (3, 30), (7, 35), (20, 40)):
+        Ea, Ma = a.ising_sweep_trace(0.8, n, every_half_sweeps=every)
+        Eb, Mb = b.ising_sweep_trace(0.8, n, every_half_sweeps=every)
+        assert Ea.shape[0] == (2 * n) // every and torch.equal(Ea, Eb) and torch.equal(Ma, Mb), every
+        assert torch.equal(a.ising_get_spins(), b.ising_get_spins()), every
+    Ea, none = a.ising_sweep_trace(0.8, 16, every_half_sweeps=2, want_M=False)
+    Eb, _ = b.ising_sweep_trace(0.8, 16, every_half_sweeps=2, want_M=False)
+    assert none is None and torch.equal(Ea, Eb)
+    for g in (a, b):
+        g.ising_set_t(2**32 - 21)
+        g.ising_sweep(1 / 1.1, 20)
+    assert a.ising_get_t() == 2**32 + 19 and torch.equal(a.ising_get_spins(), b.ising_get_spins())
+    assert torch.equal(a.ising_energy()[0], b.ising_energy()[0])
+
+
+def test_graph_replays_of_two_handles_on_two_streams():
+    """Every graph-using handle has its own slot of constant memory: two handles replaying graphs concurrently on two streams (and a
+    third one created and destroyed in between) do not disturb each other."""
+    L = 64
+    jobs = []
+    for i, (seed_s, mode) in enumerate(((91, PHILOX), (92, MINSTD))):
+        spins, J = synth.make_spins(L, 1, seed_s), synth.make_couplings(L, 1, seed_s + 10)
+        g = Ising(L, 1, SEED + i, mode)
+        r = Ising(L, 1, SEED + i, mode)
+        r.ising_set_kernel(3)
+        for h in (g, r):
+            h.ising_load_state(dev(spins), dev(J))
+        jobs.append((g, r, torch.cuda.Stream()))
+    torch.cuda.synchronize()
+    tmp = Ising(L, 1, 5, PHILOX)
+    tmp.ising_load_state(dev(synth.make_spins(L, 1, 1)), dev(synth.make_couplings(L, 1, 2)))
+    tmp.ising_sweep(0.5, 20)
+    tmp.ising_destroy()
+    for rep in range(3):
+        for g, r, st in jobs:
+            g.ising_sweep(1 / 1.1 if rep != 1 else 0.4, 64, stream=st)
+    torch.cuda.synchronize()
+    for g, r, st in jobs:
+        for rep in range(3):
+            r.ising_sweep(1 / 1.1 if rep != 1 else 0.4, 64)
+        assert torch.equal(g.ising_get_spins(), r.ising_get_spins())
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
