@@ -1,19 +1,18 @@
 // persistent.cuh -- many half-sweeps in ONE launch, for small lattices ("a CUDA graph or a persistent
 // cooperative kernel is used for small L"; the paper's small-L saturation study).
 //
-// The paper launches two kernels per sweep.  On a B200 a half-sweep of a small lattice is 0.3-6 us of work, and the
-// gap between two dependent launches, even with programmatic dependent launch, is 2.6 us: configs 1-3 of BASELINE.json were
-// launch-bound.  Measured here (profiles/r2b_persistent.md): that gap is not host overhead but the latency of the memory system.
-// A grid-wide release / acquire barrier over 148-296 co-resident CTAs costs 1.3-1.5 us, a flag handed from one CTA to its
-// neighbour 1.45 us, a cluster barrier 0.25 us, a CTA barrier 0.02 us.  Two kernels follow from that:
+// The paper launches two kernels per sweep.  On a B200 a half-sweep of a small lattice is 0.3-6 us of work, while a
+// launch into a stream costs the host 2.35 us and any synchronisation that crosses the L2 about 1.4 us
+// (profiles/r2j_launch_floor.md: a grid-wide release / acquire barrier over 148-296 co-resident CTAs 1.3-1.4 us, a flag handed from
+// one CTA to its neighbours 1.45 us, a graph edge 0.5-0.9 us, a cluster barrier 0.23 us, a CTA barrier 0.02 us).  Two kernels:
 //
 // half_sweeps_on_chip<RNG> -- lattices of at most 1024 words per colour (every even L <= 40; config 1, L = 16).  ONE CTA stages
 //   the eight bit arrays in shared memory, runs ALL half-sweeps of the call there with a CTA barrier between them (the bit-window
 //   word update of half_sweep_site_packed_rows on shared-memory operands), computes the records (E, M per recorded half-sweep)
 //   itself, and writes the spins back at the end: no launch, no L2 round trip between half-sweeps.
 //
-// persistent_site_packed<RNG, W, RECORDS> -- one-sample lattices with whole-word rows below L = 512: automatic for recorded
-//   calls (ising_sweep_trace) at L = 64 and 128, everywhere else on request (kernel choice 4).  A grid of co-resident CTAs (cudaLaunchCooperativeKernel) runs as a dataflow over TILES (the rows of one CTA of the
+// persistent_site_packed<RNG, W, RECORDS> -- one-sample lattices with whole-word rows below L = 512, ON REQUEST only (kernel
+//   choice 4).  A grid of co-resident CTAs (cudaLaunchCooperativeKernel) runs as a dataflow over TILES (the rows of one CTA of the
 //   per-launch kernel): the update of a tile at half-sweep k + 1 reads only the tile itself and its four neighbours in the (y, z)
 //   tile grid as half-sweep k left them, so
 //   * every tile has an epoch counter in global memory = the number of half-sweeps it has completed in this launch;
@@ -27,10 +26,11 @@
 //   * recording half-sweeps use the MEASURE variant of the tile update and add their counts straight into the record: E[r] and M[r]
 //     are pre-set to -3N and -N by init_records and receive 2 x (unsatisfied bonds) and 2 x (up spins) (R16) by one atomic pair
 //     per CTA; nothing waits for a record.
-//   Measured: without records it ties with one launch per half-sweep at L = 64 and 128 (2.3-2.6 us either way: the flag latency is
-//   paid per tile and is as long as the launch gap) and loses from L = 192 on (L = 256: 10.3 against 8.1 us); with a record per
-//   half-sweep it wins at L = 64 and 128 (3.2 against 4.5 us).  Hence the automatic choice.  The sample-packed variant of the
-//   same scheme was slower than the launches at every size (config 2: 9.1 against 5.8 us per half-sweep) and is not in the product.
+//   Measured (profiles/r2k_small.md): never the fastest.  The flag latency is paid per tile and is as long as a launch: 2.3-2.6 us
+//   per half-sweep at L = 64 and 128 where graph replays (graph_kernels.cuh, the automatic choice there) take 2.1-2.3, 10.3 against
+//   8.1 us at L = 256.  A first version with a grid-wide barrier per half-sweep was slower still, and the sample-packed variant of
+//   the dataflow ran config 2 at 9.1 against 5.8 us per half-sweep and is not in the library.  The kernel is kept, tested, as the
+//   reproducible record of that result.
 // The results are bit-identical to one launch per half-sweep: the draws are keyed by (site, t), not by the thread mapping.
 #pragma once
 #include <cuda_runtime.h>
