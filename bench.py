@@ -439,8 +439,8 @@ def main():
             Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
             g = Ising(Ls, ns, synth.DYN_SEED, mode)
             g.ising_load_state(sp, Jc)
-            g.ising_sweep(BETA, 2)
             nsweeps = max(2, min(200, int(2e10 / (ns * Ls**3))))
+            g.ising_sweep(BETA, nsweeps if ns * Ls**3 <= 256**3 else 2)   # warm-up (small lattices: the same call, so that its CUDA graph exists)
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
