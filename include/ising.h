@@ -24,7 +24,8 @@
  *     bits above N in the last word are ignored on input and zero on output.
  *   nsamples = 1 uses a site-packed internal layout (bits of a word = 32 sites of one lattice, "SMSC",
  *   PAPER.md:227); nsamples = 32*k uses a sample-packed layout (bits of a word = 32 disorder samples at
- *   one site, "AMSC" storage, with k coded batches).
+ *   one site, "AMSC" storage, with k coded batches) or, where every sample draws
+ *   its own random numbers and L is a multiple of 64, a batch of nsamples site-packed lattices (ising_create_layout).
  *
  * Devices: a handle belongs to the CUDA device its workspace lives on.  ising_create refuses a workspace of another
  *   device than the current one, and every call that launches work returns ISING_EINVAL when made with a different
@@ -94,6 +95,23 @@ int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out);
  * content is undefined until ising_load_state.  seed keys the dynamics' random numbers (R9, R11). */
 int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_workspace, size_t workspace_bytes,
                  ising_t **out);
+
+/* The same with the internal layout of a many-sample handle chosen by the caller (ising_create = ISING_LAYOUT_AUTO).
+ *   ISING_LAYOUT_SAMPLE_PACKED  bits of a word = 32 samples at one site, the paper's AMSC storage; nsamples = 32k.
+ *   ISING_LAYOUT_BATCH          nsamples site-packed lattices one after the other (bits of a word = 32 sites of one sample, the
+ *                               paper's SMSC coding, for every sample), all samples in every launch.  Only where the
+ *                               samples draw their own numbers (rng modes 0, 1) and L is a multiple of 64: there sample s IS the
+ *                               one-sample lattice with the Philox key word k1 ^ s (R9) / the MINSTD streams s N .. s N + N - 1
+ *                               (R11), the sample-packed storage has no shared draw to amortise, and this layout is the faster one
+ *                               (DESIGN.md section 6).  ISING_EINVAL elsewhere.
+ *   ISING_LAYOUT_AUTO           ISING_LAYOUT_BATCH where it is allowed, else sample-packed (nsamples = 1: site-packed).
+ * The layout changes no result and nothing at this boundary: the canonical format is per sample in either case, and
+ * ising_workspace_bytes is enough for both. */
+#define ISING_LAYOUT_AUTO 0
+#define ISING_LAYOUT_SAMPLE_PACKED 1
+#define ISING_LAYOUT_BATCH 2
+int ising_create_layout(int L, int nsamples, uint64_t seed, int rng_mode, int layout, void *d_workspace, size_t workspace_bytes,
+                        ising_t **out);
 
 /* Load spins and couplings given in the canonical packed format (device pointers) into the internal
  * layout.  Does not change the half-sweep counter. */
@@ -228,15 +246,17 @@ int ising_sliced_begin(ising_t *h, void *d_scratch, void *stream);
 int ising_sliced_sweep(ising_t *h, void *d_scratch, double beta, int nsweeps, void *stream);
 int ising_sliced_end(ising_t *h, void *d_scratch, void *stream);
 
-/* Select the kernels: 0 = automatic (site-packed: the word-parallel kernel when L is a multiple of 64, with the cached seed
- * table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised / tile / bit-sliced
- * kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep, energy, load, get),
- * 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = as 0 but always one launch per
- * colour half-sweep, 4 = as 0 but the persistent kernels wherever they exist.  (0 runs all half-sweeps of a call in one launch
- * where that is faster: one-sample lattices of at most 1024 words per colour, i.e. every even L <= 40, on one SM out of shared
- * memory; recorded calls, ising_sweep_trace, at L = 64 and 128 as a dataflow of co-resident CTAs; 4 extends the latter to every
- * call and every multiple of 64 below 512.)  All give the same bits; the tests use this to show that results do not depend on
- * layout, thread mapping, caching or launch structure. */
+/* Select the kernels: 0 = automatic (site-packed lattices, one sample or a batch: the word-parallel kernel when L is a multiple of
+ * 64, with the cached seed table in MINSTD mode, the bit-window kernel for every other even L; sample-packed: the vectorised /
+ * tile / bit-sliced kernels where L allows them), 1 = force the generic one-site- or one-bit-at-a-time kernels (half-sweep,
+ * energy, load, get), 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = as 0 but always
+ * one launch per colour half-sweep, 4 = as 0 but the persistent kernels wherever they exist, 5 = as 0 without the cluster-resident
+ * kernel.  0 runs all half-sweeps of a call in ONE launch where that is faster: one-sample lattices of at most 1024 words per
+ * colour (every even L <= 40) on one SM out of shared memory; L = 64 (one sample, or up to 128 samples with Philox) with one
+ * thread-block cluster per sample and the lattice in distributed shared memory; and replays CUDA graphs of up to 64 half-sweeps at
+ * L = 128, one sample (and at L = 64 under choice 5).  4 extends the cluster-resident kernel to L = 128 and to any number of samples
+ * and adds the dataflow kernel of co-resident CTAs for one-sample multiples of 64 below 512.  All give the same bits; the tests use
+ * this to show that results do not depend on layout, thread mapping, caching or launch structure. */
 int ising_set_kernel(ising_t *h, int which);
 
 /* Number of kernels this handle has launched so far. */

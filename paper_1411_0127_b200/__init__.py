@@ -4,4 +4,4 @@
 inputs; `build` compiles the library in-tree for sm_100a.  The compute path is CUDA only.
 """
 from . import synth  # noqa: F401
-from .binding import MINSTD, MT19937_SHARED, PHILOX, PHILOX_SHARED, PR_SHARED, Ising, IsingError, IsingSlab  # noqa: F401
+from .binding import LAYOUT_AUTO, LAYOUT_BATCH, LAYOUT_SAMPLE_PACKED, MINSTD, MT19937_SHARED, PHILOX, PHILOX_SHARED, PR_SHARED, Ising, IsingError, IsingSlab  # noqa: F401

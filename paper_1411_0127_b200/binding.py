@@ -13,10 +13,11 @@ from . import build as _build
 
 PHILOX, MINSTD, PHILOX_SHARED = 0, 1, 2
 PR_SHARED, MT19937_SHARED = 3, 4  # shared draw from stored-state lane generators (include/ising.h, R19)
+LAYOUT_AUTO, LAYOUT_SAMPLE_PACKED, LAYOUT_BATCH = 0, 1, 2  # ising_create_layout
 OK, EINVAL, ECUDA = 0, -1, -2
 
 EXPORTS = (
-    "ising_workspace_bytes", "ising_create", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
+    "ising_workspace_bytes", "ising_create", "ising_create_layout", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
     "ising_get_spins", "ising_run_host", "ising_run_host_async", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
@@ -40,6 +41,7 @@ def lib() -> C.CDLL:
     vp, u64, i32, sz, dbl = C.c_void_p, C.c_uint64, C.c_int, C.c_size_t, C.c_double
     L.ising_workspace_bytes.argtypes = [i32, i32, i32, C.POINTER(sz)]
     L.ising_create.argtypes = [i32, i32, u64, i32, vp, sz, C.POINTER(vp)]
+    L.ising_create_layout.argtypes = [i32, i32, u64, i32, i32, vp, sz, C.POINTER(vp)]
     L.ising_load_state.argtypes = [vp, vp, vp, vp]
     L.ising_sweep.argtypes = [vp, dbl, i32, vp]
     L.ising_sweep_trace.argtypes = [vp, dbl, i32, vp, vp, i32, vp]
@@ -151,7 +153,8 @@ class Ising:
     spins (nsamples, W), couplings (nsamples, 3, W), W = ceil(L^3/32).
     """
 
-    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device=None, workspace=None):
+    def __init__(self, L: int, nsamples: int = 1, seed: int = 0, rng_mode: int = PHILOX, device=None, workspace=None,
+                 layout: int = LAYOUT_AUTO):
         """`device`: the CUDA device of the handle (default: torch's current device, so that a process that has called
         torch.cuda.set_device(LOCAL_RANK) gets its own GPU).  `workspace`: optional caller-owned uint8 CUDA tensor of at least
         ising_workspace_bytes bytes, 256-byte aligned (default: allocated here, on `device`).  Every call of the handle runs
@@ -159,7 +162,7 @@ class Ising:
         itself refuses a handle whose workspace is not on the current device (ISING_EINVAL)."""
         import torch
 
-        self.L, self.nsamples, self.seed, self.rng_mode = L, nsamples, seed, rng_mode
+        self.L, self.nsamples, self.seed, self.rng_mode, self.layout = L, nsamples, seed, rng_mode, layout
         self.N = L ** 3
         self.W = (self.N + 31) // 32
         nbytes = ising_workspace_bytes(L, nsamples, rng_mode)
@@ -178,8 +181,8 @@ class Ising:
         self.workspace = workspace
         h = C.c_void_p()
         with torch.cuda.device(self.device):
-            _check(lib().ising_create(L, nsamples, seed, rng_mode, self.workspace.data_ptr(), nbytes, C.byref(h)),
-                   "ising_create")
+            _check(lib().ising_create_layout(L, nsamples, seed, rng_mode, layout, self.workspace.data_ptr(), nbytes, C.byref(h)),
+                   "ising_create_layout")
         self._h = h
 
     def _on_device(self, *tensors):

@@ -1,0 +1,246 @@
+// cluster_kernels.cuh -- whole trajectories of small lattices out of distributed shared memory: one thread-block cluster per
+// sample, all half-sweeps of a call in one launch (many small systems to fill the GPU; SURVEY.md section 3:
+// "a persistent kernel is used for small L").
+//
+// A lattice with whole-word rows whose eight bit arrays fit the shared memory of a cluster (L = 64: 128 KiB, L = 128: 1 MiB) never
+// has to leave the SMs between half-sweeps.  The cluster of C CTAs cuts it along z: CTA r holds the planes r L/C .. (r + 1) L/C - 1
+// of all eight arrays and updates them; the planes below and above its own live in the neighbouring CTAs' shared memory and are read
+// there directly (distributed shared memory, ld through mapa-translated addresses) -- the paper's slab decomposition of section V
+// with the SMs of one cluster in the place of the GPUs, and without the exchange step, since a remote plane can be
+// read in place.  Between two half-sweeps there is ONE cluster barrier (all stores of the active colour before any load of the next
+// half-sweep, which also orders the remote reads of the colour that is overwritten next), and it is split: a thread arrives when its
+// store is done, then draws the random numbers of its first word of the NEXT half-sweep -- the acceptance masks depend on
+// (site, t) only, not on the spins, and are three quarters of the work -- and only then waits.  The barrier's latency (0.23 us,
+// profiles/r2j_launch_floor.md) and the skew between the CTAs disappear behind the generator; nothing crosses the L2 and no launch
+// happens until the call's last half-sweep.  Samples are independent (batch_kernels.cuh), so a grid is one cluster per sample and
+// clusters never talk to each other; C is chosen so that samples x C fills the 148 SMs (32 samples: C = 4; one sample: C = 16,
+// the non-portable maximum).
+//   Records (ising_sweep_trace): after a recording half-sweep every CTA counts the unsatisfied bonds and up spins of its slab in a
+// pass of its own (out of line, so that the update loop pays nothing for it) and adds them to the pre-set record (add_to_record);
+// a second barrier keeps the next half-sweep from overwriting what the pass reads.
+//   The bits are those of one launch per half-sweep: the draws are keyed by (sample, site, t), not by the thread mapping (R9, R11).
+#pragma once
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sweep_kernels.cuh"
+
+namespace isingk {
+
+namespace cg = cooperative_groups;
+
+constexpr int CLUSTER_MAX_THREADS = 1024;
+
+struct ClusterArgs {
+    LatticeArrays A;         // the arrays of sample 0
+    size_t lattice_stride;   // words between the arrays of consecutive samples
+    int L;
+    Thresholds T;
+    uint64_t seed, t0, N;
+    uint32_t nhalf, every;   // half-sweeps of this launch; record after every `every`-th (0: never)
+    uint32_t A_first;        // MINSTD: 16807^(n+1) mod M of the sweep n = t0 >> 1
+    uint32_t nsamples, sample0;
+    long long *E, *M;        // record r of sample s at E[r * nsamples + s] (pre-set by init_records); either may be null
+};
+
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+// Addresses in the shared::cluster window (32 bits): a CTA's own shared memory and its neighbours' are read the same way.
+__device__ __forceinline__ uint32_t cluster_address(const void *smem_ptr, uint32_t rank)
+{
+    uint32_t a;
+    asm("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(a) : "r"((uint32_t)__cvta_generic_to_shared(smem_ptr)), "r"(rank));
+    return a;
+}
+__device__ __forceinline__ uint32_t cluster_load(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+
+// What the update of one word needs to know about its place and does not change from one half-sweep to the next.
+struct WordPlace {
+    uint32_t wl;                 // index of the word in the CTA's slab of each array
+    uint32_t w_yp, w_ym;         // the same bit one row up / down (periodic within the plane)
+    uint32_t zp_addr, zm_addr;   // shared::cluster address of the word one plane up / down IN ARRAY 0 (this slab's or a neighbour's)
+    uint32_t w_next, w_prev;     // next / previous word of the row (periodic); WPR > 1 only
+    uint32_t xodd0;              // (y + z) & 1: a site of colour c with bit m has x = 2m + (xodd0 ^ c)
+    uint32_t wg;                 // index of the word in the lattice's colour array (Philox counter, R9)
+    uint64_t site_even;          // canonical site of bit 0 if xodd were 0 (MINSTD stream ids, R11)
+};
+
+template <int WPR>
+__device__ __forceinline__ WordPlace place_word(uint32_t wl, uint32_t L, uint32_t Lz, uint32_t z0, uint32_t a_self, uint32_t a_up, uint32_t a_dn)
+{
+    const uint32_t plane = L * WPR;
+    const uint32_t k = WPR == 1 ? 0u : wl % WPR, row = wl / WPR, y = row % L, zl = row / L;
+    WordPlace w;
+    w.wl = wl;
+    w.w_yp = y + 1 == L ? wl - (plane - WPR) : wl + WPR;
+    w.w_ym = y == 0 ? wl + plane - WPR : wl - WPR;
+    // z neighbours: in this slab, or the first / last plane of the slab above / below
+    const bool top = zl + 1 == Lz, bot = zl == 0;
+    w.zp_addr = (top ? a_up : a_self) + 4u * (top ? wl - (Lz - 1) * plane : wl + plane);
+    w.zm_addr = (bot ? a_dn : a_self) + 4u * (bot ? wl + (Lz - 1) * plane : wl - plane);
+    w.w_next = k + 1 == WPR ? wl - (WPR - 1) : wl + 1;
+    w.w_prev = k == 0 ? wl + (WPR - 1) : wl - 1;
+    w.xodd0 = (y + z0 + zl) & 1u;
+    w.wg = z0 * plane + wl;
+    w.site_even = (uint64_t)L * ((uint64_t)y + (uint64_t)L * (z0 + zl)) + 64ull * k;
+    return w;
+}
+
+// E and M of the configuration in shared memory, this CTA's share: unsatisfied +x, +y, +z bonds and up spins of the sites of its slab
+// (each bond once, R16), as energy_tile counts them.  Kept out of line: it runs for the recording half-sweeps only and must not
+// cost the update loop any registers.
+template <int WPR>
+__device__ __noinline__ void cluster_energy_pass(const uint32_t *sm, uint32_t nw, uint32_t L, uint32_t Lz, uint32_t z0, uint32_t a_self,
+                                                 uint32_t a_up, uint32_t a_dn, unsigned int *unsat_out, unsigned int *up_out)
+{
+    unsigned int unsat = 0, up = 0;
+    for (uint32_t wl = threadIdx.x; wl < nw; wl += blockDim.x) {
+        const WordPlace w = place_word<WPR>(wl, L, Lz, z0, a_self, a_up, a_dn);
+#pragma unroll
+        for (uint32_t c = 0; c < 2; ++c) {
+            const uint32_t act = c * nw, oth = nw - act;
+            const uint32_t s = sm[act + wl], o = sm[oth + wl];
+            const uint32_t o_next = WPR > 1 ? sm[oth + w.w_next] : o;
+            const uint32_t nx = __funnelshift_r(o, o_next, w.xodd0 ^ c);
+            const uint32_t oyp = sm[oth + w.w_yp], ozp = cluster_load(w.zp_addr + 4u * oth);
+            unsat += __popc(sm[2 * nw + act + wl] ^ s ^ nx) + __popc(sm[4 * nw + act + wl] ^ s ^ oyp) + __popc(sm[6 * nw + act + wl] ^ s ^ ozp);
+            up += __popc(s);
+        }
+    }
+    *unsat_out = unsat;
+    *up_out = up;
+}
+
+// RNG 0 = Philox, 1 = MINSTD (stateless, R11 / R12).  WPR = words per half-row = L / 64.  Cluster of C = gridDim.x / samples CTAs
+// (cluster dimension attribute of the launch); blockDim.x = min(1024, words per colour and CTA), a thread owns the words
+// tid, tid + blockDim.x, ... of its CTA's slab.  SINGLE: exactly one word per thread (blockDim.x = words per colour and CTA), whose
+// place is then computed once, before the first half-sweep.  Dynamic shared memory: 8 arrays of L^2 WPR (L / C) words in the order
+// S[0], S[1], Jx[0], Jx[1], Jy[0], Jy[1], Jz[0], Jz[1].
+template <int RNG, int WPR, bool RECORDS, bool SINGLE>
+__global__ void __launch_bounds__(CLUSTER_MAX_THREADS, 1)
+half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
+{
+    extern __shared__ uint32_t sm[];
+    cg::cluster_group cluster = cg::this_cluster();
+    const uint32_t C = cluster.num_blocks(), r = cluster.block_rank();
+    const uint32_t sample = p.sample0 + blockIdx.x / C;
+    const uint32_t L = (uint32_t)p.L, Lz = L / C;
+    const uint32_t plane = L * WPR;              // words of one plane of one array
+    const uint32_t nw = plane * Lz;              // words of one array in this CTA
+    const uint32_t z0 = r * Lz;
+
+    // ---- load the slab -------------------------------------------------------------------------------------------------
+    {
+        const size_t goff = (size_t)sample * p.lattice_stride + (size_t)z0 * plane;
+        for (uint32_t i = threadIdx.x; i < nw; i += blockDim.x) {
+            sm[i] = p.A.S[0][goff + i];
+            sm[nw + i] = p.A.S[1][goff + i];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                sm[(2 + 2 * d) * nw + i] = p.A.J[d][0][goff + i];
+                sm[(3 + 2 * d) * nw + i] = p.A.J[d][1][goff + i];
+            }
+        }
+    }
+    // this slab and the slabs above and below (periodic) in the shared::cluster window: the same offsets in every CTA
+    const uint32_t a_self = cluster_address(sm, r);
+    const uint32_t a_up = cluster_address(sm, r + 1 == C ? 0 : r + 1), a_dn = cluster_address(sm, r == 0 ? C - 1 : r - 1);
+
+    const uint64_t seed = RNG == 0 ? p.seed : p.seed + (uint64_t)sample * p.N * SPLITMIX_GAMMA;   // R11: streams s N .. s N + N - 1
+    uint32_t A = p.A_first, rec = 0;
+    PhiloxCommonConst pc;
+    PhiloxSampleConst ps;
+    // the masks of word `w` for colour c with the constants of the current half-sweep
+    auto masks = [&](const WordPlace &w, int c, uint32_t &c4, uint32_t &c8, uint32_t &c12) {
+        if (RNG == 0) cond_masks_site_packed_philox(pc, ps, w.wg, p.T, c4, c8, c12);
+        else cond_masks_site_packed_minstd(seed + (w.site_even + (w.xodd0 ^ (uint32_t)c) + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, 2u * A, p.T, c4, c8, c12);
+    };
+
+    // first word of the thread, half-sweep 0: masks before the barrier that ends the load
+    const WordPlace first = place_word<WPR>(threadIdx.x, L, Lz, z0, a_self, a_up, a_dn);
+    uint32_t c4 = 0, c8 = 0, c12 = 0;
+    if (RNG == 0) fold_philox_keys(p.seed, sample, &pc, &ps);
+    if (p.nhalf) {
+        if (RNG == 0) fold_philox_time(p.seed, sample, p.t0, &pc, &ps);
+        masks(first, (int)(p.t0 & 1), c4, c8, c12);
+    }
+    cluster_arrive();
+    cluster_wait();
+
+    // Half-sweeps in runs that end at a record (RECORDS) or at the end of the call: the loop over a run is the same code with and
+    // without records.
+    const uint32_t run = RECORDS && p.every != 0 ? p.every : p.nhalf;
+    for (uint32_t k0 = 0; k0 < p.nhalf; k0 += run) {
+    const uint32_t k1 = k0 + run < p.nhalf ? k0 + run : p.nhalf;
+    for (uint32_t kk = k0; kk < k1; ++kk) {
+        const uint64_t t = p.t0 + kk;
+        const int c = (int)(t & 1);
+        const uint32_t act = (uint32_t)c * nw, oth = nw - act;   // offsets of the active / other colour within a pair of arrays
+        for (uint32_t wl = threadIdx.x; wl < nw; wl += blockDim.x) {
+            WordPlace w = first;
+            if (!SINGLE && wl != threadIdx.x) {   // later words of the thread: place and masks now
+                w = place_word<WPR>(wl, L, Lz, z0, a_self, a_up, a_dn);
+                masks(w, c, c4, c8, c12);
+            }
+            const uint32_t xodd = w.xodd0 ^ (uint32_t)c;
+            uint32_t s = sm[act + w.wl];
+            const uint32_t o = sm[oth + w.wl];
+            const uint32_t jxo = sm[2 * nw + oth + w.wl], jxa = sm[2 * nw + act + w.wl];
+            const uint32_t oyp = sm[oth + w.w_yp], oym = sm[oth + w.w_ym];
+            const uint32_t ozp = cluster_load(w.zp_addr + 4u * oth), ozm = cluster_load(w.zm_addr + 4u * oth);
+            const uint32_t jya = sm[4 * nw + act + w.wl], jza = sm[6 * nw + act + w.wl];
+            const uint32_t jyo = sm[4 * nw + oth + w.w_ym], jzo = cluster_load(w.zm_addr + 4u * (6 * nw + oth));
+            // x neighbours (row a3; see site_packed_tile): the bit that crosses the word boundary comes from the row's next /
+            // previous word (periodic), which for WPR = 1 is the word itself
+            const uint32_t B = jxo ^ o;
+            uint32_t o_next = o, B_prev = B;
+            if (WPR > 1) {
+                o_next = sm[oth + w.w_next];
+                B_prev = sm[2 * nw + oth + w.w_prev] ^ sm[oth + w.w_prev];
+            }
+            const uint32_t J[6] = {jxa, 0u, jya, jyo, jza, jzo};
+            const uint32_t nb[6] = {__funnelshift_r(o, o_next, xodd), __funnelshift_l(B_prev, B, 1u - xodd), oyp, oym, ozp, ozm};
+            uint32_t sum2, sum1, sum0;
+            satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
+            const uint32_t f = flip_mask(sum2, sum1, sum0, c4, c8, c12);
+            s ^= f;
+            sm[act + w.wl] = s;
+            if (SINGLE) break;
+        }
+        cluster_arrive();
+        if (RNG != 0 && c == 1) A = minstd_mulmod(16807u, A);   // the next half-sweep belongs to the next sweep
+        if (kk + 1 < p.nhalf) {   // the draws of the thread's first word for the next half-sweep, under the barrier
+            if (RNG == 0) fold_philox_time(p.seed, sample, t + 1, &pc, &ps);
+            masks(first, 1 - c, c4, c8, c12);
+        }
+        cluster_wait();
+    }
+    if (RECORDS && k1 == k0 + run) {   // a pass of its own over the slab, and a barrier before the next half-sweep overwrites what it reads
+        unsigned int unsat, up;
+        cluster_energy_pass<WPR>(sm, nw, L, Lz, z0, a_self, a_up, a_dn, &unsat, &up);
+        add_to_record(unsat, up, p.E ? p.E + (size_t)rec * p.nsamples + sample : nullptr,
+                      p.M ? p.M + (size_t)rec * p.nsamples + sample : nullptr);
+        ++rec;
+        cluster_arrive();
+        cluster_wait();
+    }
+    }
+
+    // ---- store the spins (every remote read of this slab is complete: its reader has passed the last barrier) -----------
+    {
+        const size_t goff = (size_t)sample * p.lattice_stride + (size_t)z0 * plane;
+        for (uint32_t i = threadIdx.x; i < nw; i += blockDim.x) {
+            p.A.S[0][goff + i] = sm[i];
+            p.A.S[1][goff + i] = sm[nw + i];
+        }
+    }
+}
+
+}  // namespace isingk

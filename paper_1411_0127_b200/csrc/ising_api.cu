@@ -8,6 +8,8 @@
 #include <new>
 
 #include "../../include/ising.h"
+#include "batch_kernels.cuh"
+#include "cluster_kernels.cuh"
 #include "graph_kernels.cuh"
 #include "lane_rng.cuh"
 #include "layout_kernels.cuh"
@@ -28,6 +30,8 @@ inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Geometry {
     int L, nsamples, nbatches;  // nbatches = 0: site-packed
+    bool batched;               // nsamples > 1 site-packed lattices one after the other (batch_kernels.cuh); then nbatches = 0
+    int nlat;                   // site-packed lattices in the workspace: 1, or nsamples when batched (0: sample-packed)
     uint64_t N, Hc;             // sites, sites per colour
     size_t canon_words;         // W = ceil(N/32)
     size_t array_words;         // words of one internal bit array (padded)
@@ -57,24 +61,34 @@ inline uint32_t lanes_default(const Geometry &g, int rng_mode)
 }
 inline uint32_t lane_ring(int rng_mode) { return rng_mode == ISING_RNG_PR_SHARED ? 62u : rng_mode == ISING_RNG_MT19937_SHARED ? 624u : 0u; }
 
-bool make_geometry(int L, int nsamples, Geometry *g)
+// Which (L, nsamples, rng_mode) can be stored as a batch of site-packed lattices: independent draws (modes 0, 1), whole-word rows.
+inline bool batch_layout_possible(int L, int nsamples, int rng_mode)
+{
+    return nsamples > 1 && L % 64 == 0 && (rng_mode == ISING_RNG_PHILOX || rng_mode == ISING_RNG_MINSTD);
+}
+
+// batched: nsamples > 1 as a batch of site-packed lattices (the caller has checked batch_layout_possible)
+bool make_geometry(int L, int nsamples, Geometry *g, bool batched = false)
 {
     if (L < 4 || (L & 1) || L > MAX_L) return false;
     if (!(nsamples == 1 || (nsamples > 0 && nsamples % 32 == 0))) return false;
+    const bool site = nsamples == 1 || batched;
     g->L = L;
     g->nsamples = nsamples;
-    g->nbatches = nsamples == 1 ? 0 : nsamples / 32;
+    g->batched = batched && nsamples > 1;
+    g->nlat = site ? nsamples : 0;
+    g->nbatches = site ? 0 : nsamples / 32;
     g->N = (uint64_t)L * L * L;
     g->Hc = g->N / 2;
     g->canon_words = (size_t)((g->N + 31) / 32);
-    const size_t raw = nsamples == 1 ? (size_t)((g->Hc + 31) / 32) : (size_t)g->Hc;
+    const size_t raw = site ? (size_t)((g->Hc + 31) / 32) : (size_t)g->Hc;
     g->array_words = round_up(raw, ALIGN_WORDS);
-    g->arrays_total_words = 8 * g->array_words * (nsamples == 1 ? 1 : (size_t)g->nbatches);
+    g->arrays_total_words = 8 * g->array_words * (site ? (size_t)nsamples : (size_t)g->nbatches);
     g->staging_words = round_up((size_t)nsamples * 4 * g->canon_words, ALIGN_WORDS);
     // popcounts + E, M of ising_run_host, then the ACC_SLOTS counter pairs and the ticket of the word-parallel energy kernel
     // ... + overlap counter (2), then (256-byte aligned) the device copy of the handle's slot of graph constants (graph_kernels.cuh)
     g->acc_bytes = round_up(((size_t)nsamples * 4 + 2 * ACC_SLOTS + 1 + 2) * sizeof(unsigned long long), 256) + round_up(sizeof(DynConst), 256);
-    g->fast = nsamples == 1 && L % 64 == 0;
+    g->fast = site && L % 64 == 0;
     // Words per thread of the word-parallel kernel: 4 (one 128-bit load per operand array) from L = 512 on; below that
     // the lattice is a fraction of one wave of CTAs and one word per thread gives the most parallelism (measured).
     g->W = 1;
@@ -85,10 +99,14 @@ bool make_geometry(int L, int nsamples, Geometry *g)
         if (odd == 3 || odd == 5) g->W = odd;  // rows of 3 * 2^e or 5 * 2^e words: 3 or 5 words per thread, no idle lanes
         else if (odd == 1 && wpr >= 8) g->W = 4;
         // other odd parts (7, 9, 11, ...): one word per thread, the row padded to a power of two of lanes
+        // a batch of lattices has the samples for parallelism: as many words per thread as the row allows (L = 128: 2, L = 256: 4)
+        if (g->batched && odd == 1 && wpr >= 2) g->W = wpr >= 4 ? 4 : 2;
     }
     // cached MINSTD seed states: 2 colours x one 4-byte word per site of every thread of the word-parallel grid (rows
     // whose lane count is not a power of two are padded, RowMap in sweep_kernels.cuh); N words when L = 64*2^k
+    // (a batch: one table per sample, as long as all of them stay below 4 GiB; beyond that the seeds are recomputed)
     g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
+    if (g->batched) g->s0_words = g->s0_words * (size_t)nsamples <= (1ull << 30) ? g->s0_words * (size_t)nsamples : 0;
     // persistent paths (persistent.cuh): one-sample lattices with whole-word rows below L = 512 get a tile grid with epoch counters
     // (used automatically up to L = 128, where it beats the launches); one-sample lattices of at most 1024 words per colour that
     // are not of that kind (every other even L <= 40) run on one SM out of shared memory
@@ -97,7 +115,7 @@ bool make_geometry(int L, int nsamples, Geometry *g)
     if (g->fast && g->W != 4) {
         g->pgx = (uint32_t)(L / (32 / row_map_tpr_pad((L >> 6) / g->W)));
         g->pgy = (uint32_t)(L / (SWEEP_THREADS / 32));
-        g->epoch_words = (size_t)g->pgx * g->pgy;
+        g->epoch_words = g->batched ? 0 : (size_t)g->pgx * g->pgy;
     }
     g->onchip = nsamples == 1 && !g->fast && (g->Hc + 31) / 32 <= ONCHIP_MAX_WORDS;
     return true;
@@ -134,6 +152,8 @@ struct ising {
     uint64_t graph_clock;
     int nslabs, slab, z0, Lz;  // z-slab handles (ising_create_slab): this handle owns the planes z0 .. z0 + Lz - 1; nslabs = 0 otherwise
     unsigned int *epochs;  // tile epochs of the persistent kernels (nullptr: no persistent path for this geometry / mode)
+    bool no_cluster;       // kernel choice 5: the automatic choice without the cluster-resident kernels
+    int cluster_size;      // CTAs per cluster of the cluster-resident kernel (0: not asked yet, -1: none for this handle / device)
     int persist_grid[2];   // co-resident CTAs of this handle's persistent kernel without / with records (0: not asked yet, -1: none)
 
     LatticeArrays arrays(int batch) const
@@ -198,15 +218,16 @@ Thresholds kernel_thresholds(const uint64_t T[3])
 void fill_rng_launch(const ising_t *h, int batch, RngLaunch *r)
 {
     memset(r, 0, sizeof(*r));
-    const uint32_t sample_base = (uint32_t)(batch * 32);
-    r->seed = h->seed;
+    // (a batch of site-packed lattices: `batch` is the sample, a one-sample lattice whose key / seed is that of the sample)
+    const uint32_t sample_base = h->g.batched ? (uint32_t)batch : (uint32_t)(batch * 32);
+    r->seed = h->g.batched ? h->seed + (uint64_t)batch * h->g.N * SPLITMIX_GAMMA : h->seed;
     r->tlo = (uint32_t)h->t;
     r->thi = (uint32_t)(h->t >> 32);
     r->k0 = (uint32_t)h->seed;
-    r->k1base = (uint32_t)(h->seed >> 32);
+    r->k1base = (uint32_t)(h->seed >> 32) ^ (h->g.batched ? sample_base : 0u);
     r->sample_base = sample_base;
     if (h->rng_mode == ISING_RNG_PHILOX) {
-        const int ns = h->g.nsamples == 1 ? 1 : 32;
+        const int ns = h->g.nbatches == 0 ? 1 : 32;
         for (int s = 0; s < ns; ++s) fold_philox(h->seed, sample_base + (uint32_t)s, h->t, &r->pc, &r->ps[s]);
     } else if (h->rng_mode == ISING_RNG_PHILOX_SHARED) {
         fold_philox(h->seed, (uint32_t)batch, h->t, &r->pc, &r->ps[0]);  // R18: the sample field of the key is the batch
@@ -253,6 +274,62 @@ void launch_site_packed(int W, bool measure, dim3 grid, cudaStream_t st, const S
     else launch_site_packed_w<RNG, 1>(measure, grid, st, a, sr, slots, N, mE, mM);
 }
 
+// The same for a batch of lattices (batch_kernels.cuh): grid.z = samples of this launch.
+template <int RNG, int W>
+void launch_batch_w(bool measure, dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, const BatchInfo &bi, long long *mE,
+                    long long *mM)
+{
+    if (measure) launch_pdl(half_sweep_site_packed_batch<RNG, W, true>, grid, dim3(SWEEP_THREADS), st, a, sr, bi, mE, mM);
+    else launch_pdl(half_sweep_site_packed_batch<RNG, W, false>, grid, dim3(SWEEP_THREADS), st, a, sr, bi, (long long *)nullptr,
+                    (long long *)nullptr);
+}
+template <int RNG>
+void launch_batch(int W, bool measure, dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, const BatchInfo &bi, long long *mE,
+                  long long *mM)
+{
+    if (W == 4) launch_batch_w<RNG, 4>(measure, grid, st, a, sr, bi, mE, mM);
+    else if (W == 2) launch_batch_w<RNG, 2>(measure, grid, st, a, sr, bi, mE, mM);
+    else if (W == 3) launch_batch_w<RNG, 3>(measure, grid, st, a, sr, bi, mE, mM);
+    else if (W == 5) launch_batch_w<RNG, 5>(measure, grid, st, a, sr, bi, mE, mM);
+    else launch_batch_w<RNG, 1>(measure, grid, st, a, sr, bi, mE, mM);
+}
+
+BatchInfo batch_info(const ising_t *h, uint32_t sample0)
+{
+    BatchInfo bi;
+    bi.lattice_stride = 8 * h->g.array_words;
+    bi.tab_stride = h->g.s0_words / 2 / (size_t)h->g.nsamples / 4;   // uint4 elements of one sample's table of one colour
+    bi.N = h->g.N;
+    bi.t = h->t;
+    bi.nsamples = (uint32_t)h->g.nsamples;
+    bi.sample0 = sample0;
+    return bi;
+}
+
+// MINSTD, batch of lattices: the seed tables of all samples (colour c of sample s at tab[c] + s * tab_stride), once per handle.
+int batch_fill_seed_tables(ising_t *h, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    if (h->s0_ready) return ISING_OK;
+    uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
+    for (int s0 = 0; s0 < g.nsamples; s0 += 65535) {
+        const int ns = g.nsamples - s0 < 65535 ? g.nsamples - s0 : 65535;
+        const dim3 grid(g.pgx ? g.pgx : (unsigned)(g.L / (32 / row_map_tpr_pad((g.L >> 6) / g.W))), (unsigned)(g.L / (SWEEP_THREADS / 32)), (unsigned)ns);
+        const BatchInfo bi = batch_info(h, (uint32_t)s0);
+        for (int cc = 0; cc < 2; ++cc) {
+            if (g.W == 4) minstd_fill_s0_batch<4><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, bi);
+            else if (g.W == 2) minstd_fill_s0_batch<2><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, bi);
+            else if (g.W == 3) minstd_fill_s0_batch<3><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, bi);
+            else if (g.W == 5) minstd_fill_s0_batch<5><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, bi);
+            else minstd_fill_s0_batch<1><<<grid, SWEEP_THREADS, 0, st>>>(tab[cc], g.L, cc, h->seed, bi);
+        }
+        const int rc = check_launch(h, 2);
+        if (rc != ISING_OK) return rc;
+    }
+    h->s0_ready = true;
+    return ISING_OK;
+}
+
 // mE / mM (device, may be null): where the half-sweep itself writes E and M of the configuration it leaves; honoured by the
 // word-parallel site-packed kernel only (see can_measure_in_sweep), ignored elsewhere.
 template <int RNG>
@@ -260,7 +337,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
 {
     const Geometry &g = h->g;
     const int c = (int)(h->t & 1);
-    const int nb = g.nsamples == 1 ? 1 : g.nbatches;
+    const int nb = g.nbatches == 0 ? g.nlat : g.nbatches;
     for (int b = 0; b < nb; ++b) {
         const LatticeArrays A = h->arrays(b);
         SweepArgs a;
@@ -310,7 +387,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             }
             launch_pdl(half_sweep_sample_packed<2, 1, false>, dim3((unsigned)((ngroups + 127) / 128)), dim3(128), st, a, r, (uint32_t)ngroups,
                        (uint64_t)g.N, (size_t)0);
-        } else if (g.nsamples != 1) {
+        } else if (g.nbatches != 0) {
             const uint64_t ngroups = g.Hc / 4;
             // small lattices: 4 threads per group (8 samples each) so that the grid covers the 148 SMs
             if (g.L % 8 == 0 && h->kernel_choice != 1) {  // 128-bit loads
@@ -357,6 +434,28 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             sr.s0tab = nullptr;
             // MINSTD: the seed states s0(seed, site) come from the table unless kernel choice 2 asks for recomputation
             const bool cached = RNG == 1 && h->kernel_choice != 2 && h->s0tab != nullptr;
+            if (g.batched) {   // all samples in one launch (blockIdx.z = sample; a, sr are sample 0 here, b == 0)
+                sr.seed = h->seed;
+                if (cached) {
+                    const int rc = batch_fill_seed_tables(h, st);
+                    if (rc != ISING_OK) return rc;
+                    sr.s0tab = (uint4 *)(h->s0tab + (c ? g.s0_words / 2 : 0));
+                }
+                for (int s0 = 0; s0 < g.nsamples; s0 += 65535) {
+                    const int ns = g.nsamples - s0 < 65535 ? g.nsamples - s0 : 65535;
+                    const BatchInfo bi = batch_info(h, (uint32_t)s0);
+                    const dim3 gridb(grid.x, grid.y, (unsigned)ns);
+                    if (cached) launch_batch<2>(W, mE != nullptr || mM != nullptr, gridb, st, a, sr, bi, mE, mM);
+                    else launch_batch<RNG>(W, mE != nullptr || mM != nullptr, gridb, st, a, sr, bi, mE, mM);
+                    if (s0 + ns < g.nsamples) {
+                        const int rc = check_launch(h);
+                        if (rc != ISING_OK) return rc;
+                    }
+                }
+                const int rc = check_launch(h);
+                if (rc != ISING_OK) return rc;
+                break;
+            }
             if (cached) {
                 uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
                 if (!h->s0_ready) {  // once per handle: the seed states depend on (seed, site) only (R11)
@@ -456,7 +555,7 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
 // Can the half-sweep kernel of this handle return E and M itself (half_sweep_site_packed<.., MEASURE = true>)?
 bool can_measure_in_sweep(const ising_t *h)
 {
-    if (h->g.nsamples != 1 || (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD)) return false;
+    if (h->g.nbatches != 0 || (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD)) return false;
     if (h->g.fast) return h->kernel_choice != 1;                                                              // word-parallel kernel
     return h->g.L >= 64 && h->kernel_choice != 1 && h->g.Hc < (1ull << 32);                                   // loop-free bit-window kernel
 }
@@ -620,6 +719,144 @@ int sweep_persistent(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t e
         if (records) rec += n / every;
     }
     return ISING_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Cluster-resident path (cluster_kernels.cuh): one thread-block cluster per sample, the lattice in distributed shared memory, all
+// half-sweeps of the call in one launch.  L = 64 and 128, one sample or a batch of lattices, Philox or MINSTD.
+// ---------------------------------------------------------------------------------------------------------------------
+template <int RNG, int WPR>
+auto cluster_kernel(bool records, bool single)
+{
+    if (single) return records ? half_sweeps_cluster<RNG, WPR, true, true> : half_sweeps_cluster<RNG, WPR, false, true>;
+    return records ? half_sweeps_cluster<RNG, WPR, true, false> : half_sweeps_cluster<RNG, WPR, false, false>;
+}
+
+// single: one word per thread (the slab of a CTA has at most 1024 words per array)
+void (*cluster_kernel_of(const ising_t *h, bool records, bool single))(const ClusterArgs)
+{
+    const bool philox = h->rng_mode == ISING_RNG_PHILOX;
+    if (h->g.L == 64) return philox ? cluster_kernel<0, 1>(records, single) : cluster_kernel<1, 1>(records, single);
+    return philox ? cluster_kernel<0, 2>(records, single) : cluster_kernel<1, 2>(records, single);
+}
+
+struct ClusterShape { int C, threads; size_t smem; bool single; };
+
+ClusterShape cluster_shape(const ising_t *h, int C)
+{
+    const Geometry &g = h->g;
+    const size_t nw = (size_t)g.L * (size_t)(g.L >> 6) * (size_t)(g.L / C);   // words of one array in one CTA
+    ClusterShape s;
+    s.C = C;
+    s.threads = nw < (size_t)CLUSTER_MAX_THREADS ? (int)nw : CLUSTER_MAX_THREADS;
+    s.smem = 8 * nw * sizeof(uint32_t);
+    s.single = nw <= (size_t)CLUSTER_MAX_THREADS;
+    return s;
+}
+
+// CTAs per cluster for this handle (0: no cluster path): the largest power of two up to 16 with samples x C <= the SMs of the
+// device, at least what the shared memory asks for; checked once per handle against what the device can co-schedule.
+int cluster_size_of(ising_t *h)
+{
+    if (h->cluster_size != 0) return h->cluster_size > 0 ? h->cluster_size : 0;
+    h->cluster_size = -1;
+    const Geometry &g = h->g;
+    if (h->nslabs || !g.fast || g.nbatches != 0 || (g.L != 64 && g.L != 128)) return 0;
+    if (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD) return 0;
+    int dev = 0, sms = 0, smem_max = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    int C = 16;
+    while (C > 1 && (long long)g.nsamples * C > sms) C >>= 1;
+    while (C <= 16 && cluster_shape(h, C).smem > (size_t)smem_max) C <<= 1;
+    for (; C <= 16; C <<= 1) {   // the first size the device accepts
+        const ClusterShape cs = cluster_shape(h, C);
+        if (cs.smem > (size_t)smem_max) continue;
+        bool ok = true;
+        for (int records = 0; records < 2 && ok; ++records) {
+            auto kernel = cluster_kernel_of(h, records != 0, cs.single);
+            ok = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs.smem) == cudaSuccess &&
+                 (C <= 8 || cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess);
+            if (!ok) break;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)C);
+            cfg.blockDim = dim3((unsigned)cs.threads);
+            cfg.dynamicSmemBytes = cs.smem;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)C;
+            attr[0].val.clusterDim.y = 1;
+            attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            int nclusters = 0;
+            ok = cudaOccupancyMaxActiveClusters(&nclusters, kernel, &cfg) == cudaSuccess && nclusters >= 1;
+        }
+        if (ok) {
+            h->cluster_size = C;
+            return C;
+        }
+        cudaGetLastError();
+    }
+    return 0;
+}
+
+// Which calls run there.  Automatic (kernel choice 0 / 2): where it was measured faster than the launches (profiles/r2m_cluster.md):
+// L = 64 with Philox up to 128 samples (one sample: 1.2 against 2.2 us per half-sweep; 32 samples: 3.7 against 5.2; 256 samples: the
+// launches fill the GPU as well), with MINSTD one sample only (the batch launches read cached seed states, this kernel recomputes
+// them).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay with the launches (the slab is
+// loaded and stored once per call).
+bool cluster_available(ising_t *h, uint32_t nhalf)
+{
+    if (h->kernel_choice == 1 || h->kernel_choice == 3 || h->no_cluster || nhalf < 8) return false;
+    if (h->kernel_choice != 4) {
+        if (h->g.L != 64) return false;
+        if (h->rng_mode == ISING_RNG_PHILOX ? h->g.nsamples > 128 : h->g.nsamples != 1) return false;
+    }
+    return cluster_size_of(h) > 0;
+}
+
+// records: E / M pre-set by the caller (init_records), record r of sample s at [r * nsamples + s].
+int sweep_cluster(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t every, long long *d_E, long long *d_M, cudaStream_t st)
+{
+    const Geometry &g = h->g;
+    const bool records = every != 0 && (d_E || d_M);
+    const ClusterShape cs = cluster_shape(h, h->cluster_size);
+    ClusterArgs p;
+    memset(&p, 0, sizeof(p));
+    p.A = h->arrays(0);
+    p.lattice_stride = 8 * g.array_words;
+    p.L = g.L;
+    p.T = T;
+    p.seed = h->seed;
+    p.t0 = h->t;
+    p.N = g.N;
+    p.nhalf = nhalf;
+    p.every = records ? every : 0u;
+    p.A_first = h->rng_mode == ISING_RNG_MINSTD ? minstd_power((h->t >> 1) + 1) : 0u;
+    p.nsamples = (uint32_t)g.nsamples;
+    p.sample0 = 0;
+    p.E = records ? d_E : nullptr;
+    p.M = records ? d_M : nullptr;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((size_t)g.nsamples * cs.C));
+    cfg.blockDim = dim3((unsigned)cs.threads);
+    cfg.dynamicSmemBytes = cs.smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cs.C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, cluster_kernel_of(h, records, cs.single), p) != cudaSuccess) g_launch_failed = true;
+    const int rc = check_launch(h);
+    if (rc == ISING_OK) h->t += nhalf;
+    return rc;
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -788,6 +1025,32 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
 {
     const Geometry &g = h->g;
     unsigned long long *slots = h->acc + 4 * (size_t)g.nsamples;
+    if (g.batched && h->kernel_choice != 1) {   // every sample in one launch, the counts added to the pre-set E[s], M[s]
+        init_records<<<(unsigned)((g.nsamples + 255) / 256), 256, 0, st>>>(d_E, d_M, (uint32_t)g.nsamples, (long long)g.N);
+        int rc = check_launch(h);
+        if (rc != ISING_OK) return rc;
+        const LatticeArrays A = h->arrays(0);
+        MeasureArgs m;
+        for (int c = 0; c < 2; ++c) {
+            m.S[c] = A.S[c];
+            for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
+        }
+        m.L = g.L;
+        const int tpr_pad = row_map_tpr_pad((g.L >> 6) / g.W);
+        for (int s0 = 0; s0 < g.nsamples; s0 += 65535) {
+            const int ns = g.nsamples - s0 < 65535 ? g.nsamples - s0 : 65535;
+            const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)), (unsigned)ns);
+            const BatchInfo bi = batch_info(h, (uint32_t)s0);
+            if (g.W == 4) launch_pdl(energy_site_packed_batch<4>, grid, dim3(SWEEP_THREADS), st, m, bi, d_E, d_M);
+            else if (g.W == 2) launch_pdl(energy_site_packed_batch<2>, grid, dim3(SWEEP_THREADS), st, m, bi, d_E, d_M);
+            else if (g.W == 3) launch_pdl(energy_site_packed_batch<3>, grid, dim3(SWEEP_THREADS), st, m, bi, d_E, d_M);
+            else if (g.W == 5) launch_pdl(energy_site_packed_batch<5>, grid, dim3(SWEEP_THREADS), st, m, bi, d_E, d_M);
+            else launch_pdl(energy_site_packed_batch<1>, grid, dim3(SWEEP_THREADS), st, m, bi, d_E, d_M);
+            rc = check_launch(h);
+            if (rc != ISING_OK) return rc;
+        }
+        return ISING_OK;
+    }
     if (g.nsamples == 1 && g.fast && h->kernel_choice != 1) {  // one fused launch (measure_kernels.cuh)
         if (!h->slots_clean) {
             if (cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
@@ -808,7 +1071,7 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
         else launch_pdl(energy_site_packed<1>, grid, dim3(SWEEP_THREADS), st, m, slots, (long long)g.N, d_E, d_M);
         return check_launch(h);
     }
-    if (g.nsamples != 1 && g.Hc < (1ull << 31) && h->kernel_choice != 1) {  // bit-sliced column sums, one fused launch
+    if (g.nbatches != 0 && g.Hc < (1ull << 31) && h->kernel_choice != 1) {  // bit-sliced column sums, one fused launch
         if (!h->slots_clean) {
             if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess ||
                 cudaMemsetAsync(slots, 0, (2 * ACC_SLOTS + 1) * sizeof(unsigned long long), st) != cudaSuccess)
@@ -836,7 +1099,7 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
     h->slots_clean = false;  // the generic kernels below leave their counts in acc
     if (cudaMemsetAsync(h->acc, 0, (size_t)g.nsamples * 2 * sizeof(unsigned long long), st) != cudaSuccess)
         return ISING_ECUDA;
-    const int nb = g.nsamples == 1 ? 1 : g.nbatches;
+    const int nb = g.nbatches == 0 ? g.nlat : g.nbatches;
     for (int b = 0; b < nb; ++b) {
         const LatticeArrays A = h->arrays(b);
         MeasureArgs m;
@@ -845,15 +1108,15 @@ int measure(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
             for (int d = 0; d < 3; ++d) m.J[d][c] = A.J[d][c];
         }
         m.L = g.L;
-        if (g.nsamples != 1) {
+        if (g.nbatches != 0) {
             energy_sample_packed<<<(unsigned)((2 * g.Hc + 255) / 256), 256, 0, st>>>(m, h->acc + (size_t)b * 64, g.Hc);
         } else if (h->kernel_choice != 1 && g.Hc < (1ull << 31)) {
             const uint32_t nw = (uint32_t)((g.Hc + 31) / 32);
             const unsigned need = (2 * nw + 255) / 256;
             energy_site_packed_rows<<<need < 148u * 8u ? need : 148u * 8u, 256, 0, st>>>(m, h->acc, nw, (uint32_t)g.Hc);
-        } else {
+        } else {   // (a batch of lattices under kernel choice 1: lattice b counts into the pair of sample b)
             const uint64_t nw = (g.Hc + 31) / 32;
-            energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc, nw, g.Hc);
+            energy_site_packed_generic<<<(unsigned)((2 * nw + 255) / 256), 256, 0, st>>>(m, h->acc + 2 * (size_t)b, nw, g.Hc);
         }
         const int rc = check_launch(h);
         if (rc != ISING_OK) return rc;
@@ -883,7 +1146,7 @@ bool make_slab_geometry(int L, int nslabs, Geometry *g, int *Lz)
 SplitArgs slab_split_args(const ising_t *h, const uint32_t *d_spins, const uint32_t *d_J)
 {
     const LatticeArrays A = h->arrays(0);
-    SplitArgs s;
+    SplitArgs s = {};
     s.narrays = 4;
     s.L = h->g.L;
     s.canon[0] = d_spins;
@@ -1046,29 +1309,52 @@ bool on_own_device(const ising_t *h)
 
 extern "C" {
 
+// Workspace of one geometry: arrays, staging, accumulators, seed table / lane state, tile epochs.
+static size_t geometry_bytes(const Geometry &g, int rng_mode)
+{
+    size_t n = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
+    if (rng_mode == ISING_RNG_MINSTD) n += g.s0_words * sizeof(uint32_t);
+    n += round_up(g.epoch_words * sizeof(uint32_t), 256);   // tile epochs of the persistent kernels (unused by the lane modes)
+    if (lane_mode(rng_mode)) n += round_up((size_t)lane_ring(rng_mode) * lanes_default(g, rng_mode) * sizeof(uint32_t), 256);
+    return n;
+}
+
 int ising_workspace_bytes(int L, int nsamples, int rng_mode, size_t *out)
 {
     Geometry g;
     if (!out || !make_geometry(L, nsamples, &g)) return ISING_EINVAL;
     if (!known_mode(rng_mode)) return ISING_EINVAL;
     if (shared_mode(rng_mode) && nsamples % 32 != 0) return ISING_EINVAL;  // one draw per 32-sample word
-    *out = (g.arrays_total_words + g.staging_words) * sizeof(uint32_t) + g.acc_bytes;
-    if (rng_mode == ISING_RNG_MINSTD) *out += g.s0_words * sizeof(uint32_t);
-    *out += round_up(g.epoch_words * sizeof(uint32_t), 256);   // tile epochs of the persistent kernels (unused by the lane modes)
-    if (lane_mode(rng_mode)) *out += round_up((size_t)lane_ring(rng_mode) * lanes_default(g, rng_mode) * sizeof(uint32_t), 256);
+    *out = geometry_bytes(g, rng_mode);
+    if (batch_layout_possible(L, nsamples, rng_mode)) {   // enough for either layout (ising_create_layout)
+        make_geometry(L, nsamples, &g, true);
+        const size_t nb = geometry_bytes(g, rng_mode);
+        if (nb > *out) *out = nb;
+    }
     return ISING_OK;
 }
 
 int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_workspace, size_t workspace_bytes,
                  ising_t **out)
 {
+    return ising_create_layout(L, nsamples, seed, rng_mode, ISING_LAYOUT_AUTO, d_workspace, workspace_bytes, out);
+}
+
+int ising_create_layout(int L, int nsamples, uint64_t seed, int rng_mode, int layout, void *d_workspace, size_t workspace_bytes,
+                        ising_t **out)
+{
     size_t need = 0;
     if (!out || !d_workspace) return ISING_EINVAL;
+    if (layout != ISING_LAYOUT_AUTO && layout != ISING_LAYOUT_SAMPLE_PACKED && layout != ISING_LAYOUT_BATCH) return ISING_EINVAL;
     if (ising_workspace_bytes(L, nsamples, rng_mode, &need) != ISING_OK) return ISING_EINVAL;
     if (workspace_bytes < need || ((uintptr_t)d_workspace & 255u)) return ISING_EINVAL;
+    const bool can_batch = batch_layout_possible(L, nsamples, rng_mode);
+    if (layout == ISING_LAYOUT_BATCH && !can_batch) return ISING_EINVAL;
+    if (layout == ISING_LAYOUT_SAMPLE_PACKED && nsamples == 1) return ISING_EINVAL;
+    const bool batched = can_batch && layout != ISING_LAYOUT_SAMPLE_PACKED;
     ising_t *h = new (std::nothrow) ising_t;
     if (!h) return ISING_EINVAL;
-    make_geometry(L, nsamples, &h->g);
+    make_geometry(L, nsamples, &h->g, batched);
     h->seed = seed;
     h->rng_mode = rng_mode;
     h->t = 0;
@@ -1085,6 +1371,8 @@ int ising_create(int L, int nsamples, uint64_t seed, int rng_mode, void *d_works
     h->nlanes = lane_mode(rng_mode) ? lanes_default(h->g, rng_mode) : 0;
     h->lanes_ready = false;
     h->persist_grid[0] = h->persist_grid[1] = 0;
+    h->cluster_size = 0;
+    h->no_cluster = false;
     h->nslabs = h->slab = h->z0 = h->Lz = 0;
     h->dyn_slot = -1;
     h->dyn = (DynConst *)((char *)h->acc + h->g.acc_bytes - round_up(sizeof(DynConst), 256));
@@ -1128,33 +1416,42 @@ int ising_load_state(ising_t *h, const uint32_t *d_spins, const uint32_t *d_J, v
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t W = g.canon_words;
-    if (g.nsamples == 1) {
+    if (g.nbatches == 0) {
         const LatticeArrays A = h->arrays(0);
         // the padding words of the arrays must not hold garbage (generic kernels read whole words); when L is a multiple of 64
         // the arrays have no padding (L^3/64 words each) and the split kernel writes every word
         if (g.array_words * 32 != g.Hc &&
             cudaMemsetAsync(h->ws, 0, g.arrays_total_words * sizeof(uint32_t), st) != cudaSuccess)
             return ISING_ECUDA;
-        if (g.fast) {
-            SplitArgs s;
-            s.narrays = 4;
-            s.L = g.L;
-            s.canon[0] = d_spins;
-            s.out[0][0] = A.S[0];
-            s.out[0][1] = A.S[1];
-            for (int d = 0; d < 3; ++d) {
-                s.canon[1 + d] = d_J + (size_t)d * W;
-                s.out[1 + d][0] = A.J[d][0];
-                s.out[1 + d][1] = A.J[d][1];
+        if (g.fast) {   // (a batch of lattices: blockIdx.y = sample, at most 65535 per launch)
+            for (int s0 = 0; s0 < g.nlat; s0 += 65535) {
+                const int ns = g.nlat - s0 < 65535 ? g.nlat - s0 : 65535;
+                const LatticeArrays As = h->arrays(s0);
+                SplitArgs s = {};
+                s.narrays = 4;
+                s.L = g.L;
+                s.canon[0] = d_spins + (size_t)s0 * W;
+                s.canon_stride[0] = W;
+                s.out[0][0] = As.S[0];
+                s.out[0][1] = As.S[1];
+                for (int d = 0; d < 3; ++d) {
+                    s.canon[1 + d] = d_J + ((size_t)s0 * 3 + (size_t)d) * W;
+                    s.canon_stride[1 + d] = 3 * W;
+                    s.out[1 + d][0] = As.J[d][0];
+                    s.out[1 + d][1] = As.J[d][1];
+                }
+                s.out_stride = 8 * g.array_words;
+                const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
+                if (g.W == 4) split_colours_site_packed<4><<<dim3((unsigned)((n / 4 + 255) / 256), (unsigned)ns), 256, 0, st>>>(s);
+                else split_colours_site_packed<1><<<dim3((unsigned)((n + 255) / 256), (unsigned)ns), 256, 0, st>>>(s);
+                const int rc = check_launch(h);
+                if (rc != ISING_OK) return rc;
             }
-            const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
-            if (g.W == 4) split_colours_site_packed<4><<<(unsigned)((n / 4 + 255) / 256), 256, 0, st>>>(s);
-            else split_colours_site_packed<1><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s);
-            return check_launch(h);
+            return ISING_OK;
         }
         const uint64_t nw = (g.Hc + 31) / 32;
         if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {  // word at a time, all four arrays and both colours in one launch
-            SplitArgs s;
+            SplitArgs s = {};
             s.narrays = 4;
             s.L = g.L;
             s.canon[0] = d_spins;
@@ -1216,12 +1513,22 @@ int ising_get_spins(ising_t *h, uint32_t *d_out, void *stream)
     cudaStream_t st = (cudaStream_t)stream;
     const Geometry &g = h->g;
     const size_t W = g.canon_words;
-    if (g.nsamples == 1) {
+    if (g.nbatches == 0) {
         const LatticeArrays A = h->arrays(0);
-        if (g.fast) {
+        if (g.fast) {   // (a batch of lattices: blockIdx.y = sample)
             const uint64_t n = (uint64_t)(g.L >> 6) * g.L * g.L;
-            if (g.W == 4) merge_colours_site_packed<4><<<(unsigned)((n / 4 + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
-            else merge_colours_site_packed<1><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(A.S[0], A.S[1], d_out, g.L);
+            const size_t in_stride = 8 * g.array_words;
+            for (int s0 = 0; s0 < g.nlat; s0 += 65535) {
+                const int ns = g.nlat - s0 < 65535 ? g.nlat - s0 : 65535;
+                const LatticeArrays As = h->arrays(s0);
+                uint32_t *out = d_out + (size_t)s0 * W;
+                if (g.W == 4) merge_colours_site_packed<4><<<dim3((unsigned)((n / 4 + 255) / 256), (unsigned)ns), 256, 0, st>>>(As.S[0], As.S[1], out, g.L, in_stride, W);
+                else merge_colours_site_packed<1><<<dim3((unsigned)((n + 255) / 256), (unsigned)ns), 256, 0, st>>>(As.S[0], As.S[1], out, g.L, in_stride, W);
+                if (s0 + ns < g.nlat) {
+                    const int rc = check_launch(h);
+                    if (rc != ISING_OK) return rc;
+                }
+            }
         } else if (h->kernel_choice != 1 && g.Hc < (1ull << 32)) {
             scatter_site_packed_rows<<<(unsigned)((W + 127) / 128), 128, 0, st>>>(A.S[0], A.S[1], d_out, g.L, W, g.N);
         } else {
@@ -1263,22 +1570,27 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
     if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
     const Thresholds kt = kernel_thresholds(T);
     cudaStream_t st = (cudaStream_t)stream;
-    if (nsweeps >= 1 && persistent_available(h, trace)) {   // all half-sweeps of the call in one launch (persistent.cuh)
+    const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps add E and M to the records themselves
+    // small lattices whose arrays fit a cluster's shared memory: the whole call in one launch (cluster_kernels.cuh), below
+    const bool in_cluster = nsweeps >= 1 && (!trace || fused) && cluster_available(h, 2u * (uint32_t)nsweeps);
+    if (!in_cluster && nsweeps >= 1 && persistent_available(h, trace)) {   // all half-sweeps of the call in one launch (persistent.cuh)
         const uint32_t nhalf = 2u * (uint32_t)nsweeps;
         const int rc = sweep_persistent(h, kt, nhalf, trace ? (uint32_t)every_half_sweeps : 0u, (long long *)d_E, (long long *)d_M, st);
         if (rc != ISING_EINVAL) return rc;   // EINVAL (before anything ran): no cooperative launch on this device; use the launches
     }
     size_t rec = 0;
     int k_first = 1;
-    const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps add E and M to the records themselves
-    if (fused) {   // ... which are pre-set to -3N / -N here (add_to_record)
+    if (fused) {   // the records are pre-set to -3N / -N here (add_to_record)
         const uint32_t nrec = (uint32_t)((2 * (size_t)nsweeps) / (size_t)every_half_sweeps);
         if (nrec) {
-            init_records<<<(nrec + 255) / 256, 256, 0, st>>>((long long *)d_E, (long long *)d_M, nrec, (long long)h->g.N);
+            const uint32_t n = nrec * (uint32_t)h->g.nsamples;   // (a batch of lattices: one entry per record and sample)
+            init_records<<<(n + 255) / 256, 256, 0, st>>>((long long *)d_E, (long long *)d_M, n, (long long)h->g.N);
             const int rc = check_launch(h);
             if (rc != ISING_OK) return rc;
         }
     }
+    if (in_cluster)
+        return sweep_cluster(h, kt, 2u * (uint32_t)nsweeps, trace ? (uint32_t)every_half_sweeps : 0u, (long long *)d_E, (long long *)d_M, st);
     // whole chunks of half-sweeps replayed from a graph where a half-sweep is shorter than a launch (graph_kernels.cuh) ...
     if (nsweeps >= 1 && (!trace || fused)) {
         uint32_t done = 0, nrec = 0;
@@ -1325,6 +1637,14 @@ int ising_overlap(ising_t *h, int sample_a, int sample_b, int64_t *d_q, void *st
     if (!h->overlap_clean) {
         if (cudaMemsetAsync(cnt, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return ISING_ECUDA;
         h->overlap_clean = true;   // finalize_overlap leaves it zero
+    }
+    if (g.batched) {   // two site-packed lattices: popcount of the XOR of their spin arrays
+        const LatticeArrays A = h->arrays(sample_a), B = h->arrays(sample_b);
+        const uint32_t nw = (uint32_t)(g.Hc / 32);
+        const unsigned need = (nw + 255) / 256;
+        overlap_site_packed<<<need < 148u * 8u ? need : 148u * 8u, 256, 0, st>>>(A.S[0], B.S[0], g.array_words, nw, cnt);
+        finalize_overlap<<<1, 1, 0, st>>>(cnt, (long long)g.N, (long long *)d_q);
+        return check_launch(h, 2);
     }
     const LatticeArrays A = h->arrays(sample_a >> 5), B = h->arrays(sample_b >> 5);
     const unsigned need = (unsigned)((g.Hc + 255) / 256);
@@ -1656,8 +1976,9 @@ int ising_sliced_end(ising_t *h, void *d_scratch, void *stream)
 
 int ising_set_kernel(ising_t *h, int which)
 {
-    if (!h || which < 0 || which > 4) return ISING_EINVAL;
-    h->kernel_choice = which;
+    if (!h || which < 0 || which > 5) return ISING_EINVAL;
+    h->no_cluster = which == 5;               // 5 = 0 without the cluster-resident kernels
+    h->kernel_choice = which == 5 ? 0 : which;
     return ISING_OK;
 }
 

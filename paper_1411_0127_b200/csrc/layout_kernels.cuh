@@ -40,6 +40,8 @@ struct SplitArgs {
     uint32_t *out[4][2];  // [array][colour]
     int narrays;
     int L;
+    // a batch of lattices (batch_kernels.cuh), blockIdx.y = sample: words between consecutive samples in canon[q] / in out[q][c]
+    size_t canon_stride[4], out_stride;
 };
 
 template <int V>  // V internal words (2V canonical words) per thread, V <= L/64
@@ -54,8 +56,9 @@ __global__ void __launch_bounds__(256) split_colours_site_packed(const __grid_co
     const int p = (int)((r % (unsigned)L) + (r / (unsigned)L)) & 1;
     for (int q = 0; q < a.narrays; ++q) {
         uint32_t c[2 * V], even[V], odd[V];
-        const Vec lo = __ldcs(reinterpret_cast<const Vec *>(a.canon[q] + 2 * widx));
-        const Vec hi = __ldcs(reinterpret_cast<const Vec *>(a.canon[q] + 2 * widx + V));
+        const uint32_t *canon = a.canon[q] + (size_t)blockIdx.y * a.canon_stride[q];
+        const Vec lo = __ldcs(reinterpret_cast<const Vec *>(canon + 2 * widx));
+        const Vec hi = __ldcs(reinterpret_cast<const Vec *>(canon + 2 * widx + V));
 #pragma unroll
         for (int k = 0; k < V; ++k) {
             c[k] = reinterpret_cast<const uint32_t *>(&lo)[k];
@@ -75,17 +78,22 @@ __global__ void __launch_bounds__(256) split_colours_site_packed(const __grid_co
             for0[k] = p ? odd[k] : even[k];
             for1[k] = p ? even[k] : odd[k];
         }
-        __stcs(reinterpret_cast<Vec *>(a.out[q][0] + widx), *reinterpret_cast<const Vec *>(for0));
-        __stcs(reinterpret_cast<Vec *>(a.out[q][1] + widx), *reinterpret_cast<const Vec *>(for1));
+        const size_t so = (size_t)blockIdx.y * a.out_stride;
+        __stcs(reinterpret_cast<Vec *>(a.out[q][0] + so + widx), *reinterpret_cast<const Vec *>(for0));
+        __stcs(reinterpret_cast<Vec *>(a.out[q][1] + so + widx), *reinterpret_cast<const Vec *>(for1));
     }
 }
 
 template <int V>
 __global__ void __launch_bounds__(256)
-merge_colours_site_packed(const uint32_t *__restrict__ S0, const uint32_t *__restrict__ S1, uint32_t *__restrict__ canon, int L)
+merge_colours_site_packed(const uint32_t *__restrict__ S0, const uint32_t *__restrict__ S1, uint32_t *__restrict__ canon, int L,
+                          size_t in_stride = 0, size_t canon_stride = 0)   // a batch of lattices: blockIdx.y = sample
 {
     typedef typename WordVec<V>::type Vec;
     const int wpr = L >> 6;
+    S0 += (size_t)blockIdx.y * in_stride;
+    S1 += (size_t)blockIdx.y * in_stride;
+    canon += (size_t)blockIdx.y * canon_stride;
     const uint64_t n = (uint64_t)wpr * L * L;
     const uint64_t widx = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * V;
     if (widx >= n) return;

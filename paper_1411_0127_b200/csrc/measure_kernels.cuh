@@ -29,20 +29,21 @@ struct MeasureArgs {
 // One launch does everything: the CTAs add their counts to the slots, and the last CTA to finish (a ticket counter
 // behind the slots) sums the slots, writes E and M (R16), and clears slots and counter for the next call, so a trace of
 // E per half-sweep costs one small launch per record instead of memset + kernel + finalize.
+// The counts of one tile = the rows of CTA (bx, by) of the grid (L / (32 / tpr_pad), L / 8): this thread's unsatisfied bonds and up
+// spins are returned in unsat / up.
 template <int W>
-__global__ void __launch_bounds__(SWEEP_THREADS)
-energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {unsatisfied bonds, up spins}, then the ticket */,
-                   long long N, long long *E, long long *M)
+__device__ __forceinline__ void energy_tile(const MeasureArgs &a, uint32_t bx, uint32_t by, unsigned int &unsat, unsigned int &up)
 {
     const int L = a.L, wpr = L >> 6;
-    const RowMap rm = row_map<W>(L, blockIdx.x, blockIdx.y);
+    const RowMap rm = row_map<W>(L, bx, by);
     const int tpr = rm.tpr, y = rm.y, z = rm.z, k0 = rm.k0;
     const int yp = y + 1 == L ? 0 : y + 1, zp = z + 1 == L ? 0 : z + 1;
     const uint32_t row = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * z) + k0;
     const uint32_t row_yp = (uint32_t)wpr * ((uint32_t)yp + (uint32_t)L * z) + k0;
     const uint32_t row_zp = (uint32_t)wpr * ((uint32_t)y + (uint32_t)L * zp) + k0;
     const int next_lane = rm.next_lane;
-    unsigned int unsat = 0, up = 0;
+    unsat = 0;
+    up = 0;
     wait_for_previous_kernel();
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
@@ -66,6 +67,15 @@ energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {
             }
         }
     }
+}
+
+template <int W>
+__global__ void __launch_bounds__(SWEEP_THREADS)
+energy_site_packed(const MeasureArgs a, unsigned long long *acc /* ACC_SLOTS x {unsatisfied bonds, up spins}, then the ticket */,
+                   long long N, long long *E, long long *M)
+{
+    unsigned int unsat, up;
+    energy_tile<W>(a, blockIdx.x, blockIdx.y, unsat, up);
     block_accumulate2(unsat, up, acc + 2 * ((blockIdx.x + blockIdx.y * gridDim.x) & (ACC_SLOTS - 1)));
     finalize_slots_last_cta(acc, N, E, M);
 }

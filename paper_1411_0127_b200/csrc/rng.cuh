@@ -77,6 +77,27 @@ ISING_HD void fold_philox(uint64_t seed, uint32_t sample, uint64_t t, PhiloxComm
     for (int r = 2; r < 10; ++r) sc->k1[r - 2] = k1 + (uint32_t)r * PHILOX_W1;
 }
 
+// The same in two steps, for kernels that run many half-sweeps: the round keys depend on (seed, sample) only, the four words
+// a, b, d, e on t as well.
+ISING_HD void fold_philox_keys(uint64_t seed, uint32_t sample, PhiloxCommonConst *cc, PhiloxSampleConst *sc)
+{
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32) ^ sample;
+    for (int r = 3; r < 10; ++r) cc->k0[r - 3] = k0 + (uint32_t)r * PHILOX_W0;
+    for (int r = 2; r < 10; ++r) sc->k1[r - 2] = k1 + (uint32_t)r * PHILOX_W1;
+}
+ISING_HD void fold_philox_time(uint64_t seed, uint32_t sample, uint64_t t, PhiloxCommonConst *cc, PhiloxSampleConst *sc)
+{
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32) ^ sample;
+    const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
+    const uint64_t P0 = (uint64_t)PHILOX_M0 * tlo;
+    const uint32_t A2 = (uint32_t)(P0 >> 32) ^ k1;
+    const uint64_t B = (uint64_t)PHILOX_M1 * A2;
+    cc->a = thi ^ k0;
+    sc->b = (uint32_t)(B >> 32) ^ (k0 + PHILOX_W0);
+    sc->d = (uint32_t)P0 ^ (k1 + PHILOX_W1);
+    sc->e = (uint32_t)B ^ (k0 + 2u * PHILOX_W0);
+}
+
 ISING_HD void philox_folded(const PhiloxCommonConst &cc, const PhiloxSampleConst &sc, uint32_t g, uint32_t out[4])
 {
     // round 0.  (Forming M1 * g for the calls of a thread as M1 * g_base + a compile-time constant turns 31 of 32 of these

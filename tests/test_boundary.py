@@ -88,17 +88,20 @@ def test_argument_validation_without_a_gpu():
         assert nbytes >= ns * (N // 8) * 8 and nbytes % 256 == 0
         # MINSTD adds the seed-state table (4 bytes per site) where the word-parallel layout applies
         # (word-parallel layout: L a multiple of 64; rows whose lane count is not a power of two are padded)
+        # (many samples with L a multiple of 64 are stored as a batch of such lattices: one table per sample)
         table = 0
-        if ns == 1 and L % 64 == 0:
+        if L % 64 == 0:
             wpr = odd = L // 64
             while odd % 2 == 0:
                 odd //= 2
             W = odd if odd in (3, 5) else (4 if odd == 1 and wpr >= 8 else 1)  # words per thread
+            if ns > 1 and odd == 1 and wpr >= 2:
+                W = 4 if wpr >= 4 else 2
             pad = 1
             while pad < wpr // W:
                 pad *= 2
-            table = 4 * 2 * L * L * pad * W * 32
-            assert table >= 4 * N and (table == 4 * N) == (odd in (1, 3, 5))
+            table = 4 * 2 * L * L * pad * W * 32 * ns
+            assert table >= 4 * N * ns and (table == 4 * N * ns) == (odd in (1, 3, 5))
         assert binding.ising_workspace_bytes(L, ns, 1) == nbytes + table
     assert binding.ising_workspace_bytes(1024, 1, 0) < 1100 * 2**20
     h = C.c_void_p()
@@ -117,7 +120,17 @@ def test_argument_validation_without_a_gpu():
     t = C.c_uint64(99)
     assert lib.ising_get_t(h, C.byref(t)) == binding.OK and t.value == 0
     assert lib.ising_set_t(h, 6) == binding.OK and lib.ising_get_t(h, C.byref(t)) == binding.OK and t.value == 6
-    assert lib.ising_set_kernel(h, 5) == binding.EINVAL
+    assert lib.ising_set_kernel(h, 5) == binding.OK and lib.ising_set_kernel(h, 6) == binding.EINVAL
+    # layouts (ising_create_layout): a batch of site-packed lattices only for many samples with their own draws and whole-word rows
+    h2 = C.c_void_p()
+    big = C.c_void_p(1 << 20)
+    assert lib.ising_create_layout(64, 32, 1, 0, binding.LAYOUT_BATCH, big, 1 << 30, C.byref(h2)) == binding.OK
+    assert lib.ising_destroy(h2) == binding.OK
+    assert lib.ising_create_layout(64, 32, 1, 1, binding.LAYOUT_SAMPLE_PACKED, big, 1 << 30, C.byref(h2)) == binding.OK
+    assert lib.ising_destroy(h2) == binding.OK
+    for L, ns, mode, layout in ((64, 32, 2, binding.LAYOUT_BATCH), (32, 32, 0, binding.LAYOUT_BATCH), (64, 1, 0, binding.LAYOUT_BATCH),
+                                (64, 1, 0, binding.LAYOUT_SAMPLE_PACKED), (64, 32, 0, 3), (64, 32, 0, -1)):
+        assert lib.ising_create_layout(L, ns, 1, mode, layout, big, 1 << 30, C.byref(h2)) == binding.EINVAL, (L, ns, mode, layout)
     assert lib.ising_kernel_launches(h) == 0
     assert lib.ising_destroy(h) == binding.OK
 

@@ -16,7 +16,7 @@ import pytest
 torch = pytest.importorskip("torch")
 
 from oracle import ea3d  # noqa: E402
-from paper_1411_0127_b200 import MINSTD, PHILOX, PHILOX_SHARED, Ising, binding, synth  # noqa: E402
+from paper_1411_0127_b200 import LAYOUT_AUTO, LAYOUT_SAMPLE_PACKED, MINSTD, PHILOX, PHILOX_SHARED, Ising, binding, synth  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 SEED = synth.DYN_SEED
@@ -30,10 +30,10 @@ def host_u32(t) -> np.ndarray:
     return t.cpu().numpy().view(np.uint32)
 
 
-def make_pair(L, nsamples, rng_mode, spins, J, seed=SEED):
+def make_pair(L, nsamples, rng_mode, spins, J, seed=SEED, layout=LAYOUT_AUTO):
     o = ea3d.Oracle(L, nsamples, seed, rng_mode)
     o.load_packed(spins, J)
-    g = Ising(L, nsamples, seed, rng_mode)
+    g = Ising(L, nsamples, seed, rng_mode, layout=layout)
     g.ising_load_state(dev(spins), dev(J))
     return o, g
 
@@ -55,7 +55,8 @@ def test_layout_round_trip_and_energy(L, nsamples):
     """Rows a9 / a10.  Sample-packed: the bit-sliced energy kernel (any L) and, for L a multiple of 32, the register-transpose
     tile kernels of load / get; kernel choice 1 runs the one-bit-at-a-time kernels on the same data."""
     spins, J = synth.make_spins(L, nsamples, 7), synth.make_couplings(L, nsamples, 3)
-    o, g = make_pair(L, nsamples, PHILOX, spins, J)
+    # (many samples: the sample-packed arrays, which is what this test is about; L = 64 and 128 would be a batch otherwise)
+    o, g = make_pair(L, nsamples, PHILOX, spins, J, layout=LAYOUT_SAMPLE_PACKED if nsamples > 1 else LAYOUT_AUTO)
     assert_same_state(o, g, "after load")
     assert np.array_equal(host_u32(g.ising_get_spins()), spins)
     if nsamples == 1 and L >= 64:  # the generic measurement kernel on the same internal layout
@@ -166,11 +167,29 @@ def test_config2_L64_32_samples_philox():
     assert len(set(E[-1].tolist())) > 16  # the 32 samples really are different systems
 
 
+def test_config2_in_the_sample_packed_layout_and_by_launches():
+    """Config 2 runs, by default, as a batch of 32 site-packed lattices in the cluster-resident kernel (the test above).  The same
+    1000 sweeps in the paper's sample-packed storage, and in the batch layout with one launch per half-sweep: same records, same
+    spins."""
+    cfg, spins, J = synth.make_config(2)
+    res = []
+    for layout, choice in ((LAYOUT_AUTO, 0), (LAYOUT_SAMPLE_PACKED, 0), (LAYOUT_AUTO, 3)):
+        g = Ising(cfg["L"], 32, SEED, cfg["rng_mode"], layout=layout)
+        g.ising_set_kernel(choice)
+        g.ising_load_state(dev(spins), dev(J))
+        E, _ = g.ising_sweep_trace(cfg["beta"], cfg["sweeps"], every_half_sweeps=20, want_M=False)
+        res.append((E.clone(), g.ising_get_spins().clone(), g.ising_kernel_launches()))
+        g.ising_destroy()
+    for r in res[1:]:
+        assert torch.equal(res[0][0], r[0]) and torch.equal(res[0][1], r[1])
+    assert res[0][2] <= 4 and res[2][2] >= 2000      # one launch against one per half-sweep
+
+
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
 @pytest.mark.parametrize("L,nsamples", [(4, 32), (6, 32), (10, 32), (16, 64), (8, 160), (24, 96), (64, 64), (10, 64), (6, 96), (12, 160)])
 def test_sample_packed_small(L, nsamples, rng_mode):
     spins, J = synth.make_spins(L, nsamples, 21), synth.make_couplings(L, nsamples, 8)
-    o, g = make_pair(L, nsamples, rng_mode, spins, J)
+    o, g = make_pair(L, nsamples, rng_mode, spins, J, layout=LAYOUT_SAMPLE_PACKED)
     o.sweep(0.7, 6)
     g.ising_sweep(0.7, 6)
     assert_same_state(o, g, f"L={L} x {nsamples}")
@@ -479,8 +498,8 @@ def test_sample_packed_vector_kernel_equals_scalar_kernel(L, nsamples, rng_mode)
     """L % 8 == 0: the sample-packed kernel with 128-bit loads (default) against the scalar-load kernel (kernel choice 1),
     both thread-per-group variants (L = 128 x 32 has more than 148 x 1024 groups)."""
     spins, J = synth.make_spins(L, nsamples, 81), synth.make_couplings(L, nsamples, 82)
-    a = Ising(L, nsamples, SEED, rng_mode)
-    b = Ising(L, nsamples, SEED, rng_mode)
+    a = Ising(L, nsamples, SEED, rng_mode, layout=LAYOUT_SAMPLE_PACKED)
+    b = Ising(L, nsamples, SEED, rng_mode, layout=LAYOUT_SAMPLE_PACKED)
     b.ising_set_kernel(1)
     for g in (a, b):
         g.ising_load_state(dev(spins), dev(J))
@@ -499,8 +518,8 @@ def test_sample_packed_L256_vector_kernels_equal_scalar_kernel(rng_mode, nsample
     W = L**3 // 32
     d_spins = torch.randint(-2**31, 2**31 - 1, (nsamples * W,), dtype=torch.int32, device="cuda", generator=gen)
     d_J = torch.randint(-2**31, 2**31 - 1, (nsamples * 3 * W,), dtype=torch.int32, device="cuda", generator=gen)
-    a = Ising(L, nsamples, SEED, rng_mode)
-    b = Ising(L, nsamples, SEED, rng_mode)
+    a = Ising(L, nsamples, SEED, rng_mode, layout=LAYOUT_SAMPLE_PACKED)
+    b = Ising(L, nsamples, SEED, rng_mode, layout=LAYOUT_SAMPLE_PACKED)
     b.ising_set_kernel(1)
     for g in (a, b):
         g.ising_load_state(d_spins, d_J)
@@ -515,7 +534,7 @@ def test_sample_packed_large_lattice_one_thread_per_group(rng_mode):
     sample-packed kernel runs (smaller lattices use four threads per group); two batches exercise the batch loop."""
     L, ns = 128, 64
     spins, J = synth.make_spins(L, ns, 71), synth.make_couplings(L, ns, 72)
-    o, g = make_pair(L, ns, rng_mode, spins, J)
+    o, g = make_pair(L, ns, rng_mode, spins, J, layout=LAYOUT_SAMPLE_PACKED)
     o.sweep(1 / 1.1, 1)
     g.ising_sweep(1 / 1.1, 1)
     assert_same_state(o, g, f"sample-packed L={L} x {ns}")
@@ -839,6 +858,7 @@ def test_graph_replays_equal_one_launch_per_half_sweep(L, nsamples, rng_mode):
     oracle at the small sizes."""
     spins, J = synth.make_spins(L, nsamples, 87), synth.make_couplings(L, nsamples, 88)
     a = Ising(L, nsamples, SEED, rng_mode)
+    a.ising_set_kernel(5)     # the automatic choice without the cluster-resident kernel, which otherwise takes L = 64
     b = Ising(L, nsamples, SEED, rng_mode)
     b.ising_set_kernel(3)
     small = nsamples * L**3 <= 64**3 * 2
@@ -879,6 +899,7 @@ def test_graph_replays_of_two_handles_on_two_streams():
     for i, (seed_s, mode) in enumerate(((91, PHILOX), (92, MINSTD))):
         spins, J = synth.make_spins(L, 1, seed_s), synth.make_couplings(L, 1, seed_s + 10)
         g = Ising(L, 1, SEED + i, mode)
+        g.ising_set_kernel(5)
         r = Ising(L, 1, SEED + i, mode)
         r.ising_set_kernel(3)
         for h in (g, r):
