@@ -591,7 +591,7 @@ def main():
             for mode in (PHILOX, MINSTD):
                 row = {"L": Ls, "rng_mode": ["philox", "minstd"][mode]}
                 for every in (0, 1):
-                    for choice in (0, 3, 4):
+                    for choice in (0, 3, 5, 4):
                         g = Ising(Ls, 1, synth.DYN_SEED, mode)
                         g.ising_set_kernel(choice)
                         g.ising_load_state(sp, Jc)
@@ -611,10 +611,45 @@ def main():
                             ms = a.elapsed_time(b)
                             best = ms if best is None or ms < best else best
                         g.ising_destroy()
-                        row[("recorded_" if every else "") + {0: "automatic", 3: "launch_per_half_sweep", 4: "persistent"}[choice] + "_us"] = \
-                            round(1e3 * best / (2 * nsweeps), 3)
+                        name = {0: "automatic", 3: "launch_per_half_sweep", 5: "automatic_without_cluster_kernel", 4: "persistent"}[choice]
+                        row[("recorded_" if every else "") + name + "_us"] = round(1e3 * best / (2 * nsweeps), 3)
                 rows.append(row)
-        print(json.dumps({"small": rows}))
+        # many samples with their own draws: the paper's sample-packed storage, the batch of site-packed lattices by launches, and the
+        # automatic choice (batch; at L = 64 the cluster-resident kernel where it is faster)
+        from paper_1411_0127_b200 import LAYOUT_BATCH, LAYOUT_SAMPLE_PACKED
+        many = []
+        for Ls, ns in ((64, 32), (64, 64), (64, 128), (64, 256), (128, 32), (256, 32)):
+            sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
+            Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
+            for mode in (PHILOX, MINSTD):
+                row = {"L": Ls, "nsamples": ns, "rng_mode": ["philox", "minstd"][mode]}
+                for name, layout, choice in (("sample_packed", LAYOUT_SAMPLE_PACKED, 0), ("batch_launches", LAYOUT_BATCH, 3),
+                                             ("automatic", 0, 0)):
+                    g = Ising(Ls, ns, synth.DYN_SEED, mode, layout=layout)
+                    g.ising_set_kernel(choice)
+                    g.ising_load_state(sp, Jc)
+                    nsweeps = max(4, min(500, int(4e10 / (Ls**3 * ns)) // 2))
+                    g.ising_sweep(BETA, nsweeps)
+                    for every in (0, 20):
+                        best = None
+                        for _ in range(3):
+                            torch.cuda.synchronize()
+                            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                            a.record(stream)
+                            if every:
+                                g.ising_sweep_trace(BETA, nsweeps, every_half_sweeps=every)
+                            else:
+                                g.ising_sweep(BETA, nsweeps)
+                            b.record(stream)
+                            torch.cuda.synchronize()
+                            ms = a.elapsed_time(b)
+                            best = ms if best is None or ms < best else best
+                        row[("recorded_every_20_" if every else "") + name + "_us"] = round(1e3 * best / (2 * nsweeps), 3)
+                        row[("recorded_every_20_" if every else "") + name + "_ps_per_flip"] = round(1e9 * best / (nsweeps * ns * Ls**3), 4)
+                    g.ising_destroy()
+                many.append(row)
+            del sp, Jc
+        print(json.dumps({"small": rows, "many_samples": many}))
         return
 
     if args.configs:  # BASELINE.json configs 1-5 as written: sweeps, and the observables each one records, inside the timed region

@@ -16,8 +16,8 @@
 // clusters never talk to each other; C is chosen so that samples x C fills the 148 SMs (32 samples: C = 4; one sample: C = 16,
 // the non-portable maximum).
 //   Records (ising_sweep_trace): after a recording half-sweep every CTA counts the unsatisfied bonds and up spins of its slab in a
-// pass of its own (out of line, so that the update loop pays nothing for it) and adds them to the pre-set record (add_to_record);
-// a second barrier keeps the next half-sweep from overwriting what the pass reads.
+// pass of its own (out of line, so that the update loop pays nothing for it) and adds them to the pre-set record (R16, as
+// add_to_record does) one arrive later; a second barrier keeps the next half-sweep from overwriting what the pass reads.
 //   The bits are those of one launch per half-sweep: the draws are keyed by (sample, site, t), not by the thread mapping (R9, R11).
 #pragma once
 #include <cooperative_groups.h>
@@ -174,6 +174,21 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
     cluster_arrive();
     cluster_wait();
 
+    // The record of a run is added to global memory one arrive later: the release of an arrive waits for the thread's outstanding
+    // global operations, so an atomic issued just before it would put an L2 round trip (1-2 us) on every record's critical path;
+    // issued just after an arrive it completes under the next half-sweep's draws.
+    __shared__ unsigned long long rec_sum[2];
+    bool rec_pending = false;
+    auto flush_record = [&]() {
+        if (RECORDS && rec_pending) {
+            if (threadIdx.x == 0) {
+                if (p.E) atomicAdd(reinterpret_cast<unsigned long long *>(p.E + (size_t)rec * p.nsamples + sample), 2ull * rec_sum[0]);   // R16
+                if (p.M) atomicAdd(reinterpret_cast<unsigned long long *>(p.M + (size_t)rec * p.nsamples + sample), 2ull * rec_sum[1]);
+            }
+            ++rec;
+            rec_pending = false;
+        }
+    };
     // Half-sweeps in runs that end at a record (RECORDS) or at the end of the call: the loop over a run is the same code with and
     // without records.
     const uint32_t run = RECORDS && p.every != 0 ? p.every : p.nhalf;
@@ -215,6 +230,7 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
             if (SINGLE) break;
         }
         cluster_arrive();
+        if (RECORDS) flush_record();
         if (RNG != 0 && c == 1) A = minstd_mulmod(16807u, A);   // the next half-sweep belongs to the next sweep
         if (kk + 1 < p.nhalf) {   // the draws of the thread's first word for the next half-sweep, under the barrier
             if (RNG == 0) fold_philox_time(p.seed, sample, t + 1, &pc, &ps);
@@ -225,13 +241,15 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
     if (RECORDS && k1 == k0 + run) {   // a pass of its own over the slab, and a barrier before the next half-sweep overwrites what it reads
         unsigned int unsat, up;
         cluster_energy_pass<WPR>(sm, nw, L, Lz, z0, a_self, a_up, a_dn, &unsat, &up);
-        add_to_record(unsat, up, p.E ? p.E + (size_t)rec * p.nsamples + sample : nullptr,
-                      p.M ? p.M + (size_t)rec * p.nsamples + sample : nullptr);
-        ++rec;
+        if (threadIdx.x == 0) { rec_sum[0] = 0; rec_sum[1] = 0; }
+        __syncthreads();
+        block_accumulate2(unsat, up, rec_sum);   // the CTA's totals; they go to the record after the next arrive (below)
+        rec_pending = true;
         cluster_arrive();
         cluster_wait();
     }
     }
+    flush_record();
 
     // ---- store the spins (every remote read of this slab is complete: its reader has passed the last barrier) -----------
     {

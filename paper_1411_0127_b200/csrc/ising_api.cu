@@ -809,12 +809,17 @@ int cluster_size_of(ising_t *h)
 // launches fill the GPU as well), with MINSTD one sample only (the batch launches read cached seed states, this kernel recomputes
 // them).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay with the launches (the slab is
 // loaded and stored once per call).
-bool cluster_available(ising_t *h, uint32_t nhalf)
+// `every`: record spacing of the call in half-sweeps (0: no records).  A record costs this kernel 1.9 us (a pass over the slab and
+// a second, unhidden barrier) where a measuring launch costs 0.6 us more than a plain one: densely recorded calls stay with the
+// launches / graph replays when there is one sample (with 32 samples the launches are slower at any spacing: 6.1 against 5.8 us
+// per half-sweep with a record after each).
+bool cluster_available(ising_t *h, uint32_t nhalf, uint32_t every)
 {
     if (h->kernel_choice == 1 || h->kernel_choice == 3 || h->no_cluster || nhalf < 8) return false;
     if (h->kernel_choice != 4) {
         if (h->g.L != 64) return false;
         if (h->rng_mode == ISING_RNG_PHILOX ? h->g.nsamples > 128 : h->g.nsamples != 1) return false;
+        if (every != 0 && h->g.nsamples == 1 && every < (h->rng_mode == ISING_RNG_PHILOX ? 4u : 16u)) return false;
     }
     return cluster_size_of(h) > 0;
 }
@@ -1572,7 +1577,7 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
     cudaStream_t st = (cudaStream_t)stream;
     const bool fused = trace && can_measure_in_sweep(h);   // the recording half-sweeps add E and M to the records themselves
     // small lattices whose arrays fit a cluster's shared memory: the whole call in one launch (cluster_kernels.cuh), below
-    const bool in_cluster = nsweeps >= 1 && (!trace || fused) && cluster_available(h, 2u * (uint32_t)nsweeps);
+    const bool in_cluster = nsweeps >= 1 && (!trace || fused) && cluster_available(h, 2u * (uint32_t)nsweeps, trace ? (uint32_t)every_half_sweeps : 0u);
     if (!in_cluster && nsweeps >= 1 && persistent_available(h, trace)) {   // all half-sweeps of the call in one launch (persistent.cuh)
         const uint32_t nhalf = 2u * (uint32_t)nsweeps;
         const int rc = sweep_persistent(h, kt, nhalf, trace ? (uint32_t)every_half_sweeps : 0u, (long long *)d_E, (long long *)d_M, st);

@@ -149,18 +149,18 @@ def test_batch_run_host_and_guards(rng_mode):
 
 # ------------------------------------------------------------------------------------------------ cluster-resident kernel
 
-# (L, samples, kernel choice): 0 = where the library takes this kernel by itself (L = 64: one sample -> clusters of 16 CTAs,
-# 32 samples -> 4, 64 -> 2, 96 -> 1 with four words per thread); 4 = on request (L = 128, two words per row: 16 and 8 CTAs)
-CLUSTER_CASES = [(64, 1, 0), (64, 32, 0), (64, 64, 0), (64, 96, 0), (128, 1, 4), (128, 32, 4)]
+# (L, samples): L = 64: one sample -> clusters of 16 CTAs, 32 samples -> 4, 64 -> 2, 96 -> 1 with four words per thread;
+# L = 128 (two words per row): 16 and 8 CTAs.  Kernel choice 4 = this kernel for every call it exists for (by itself the library
+# takes it at L = 64 for calls without records or with sparse ones: the next test).
+CLUSTER_CASES = [(64, 1), (64, 32), (64, 64), (64, 96), (128, 1), (128, 32)]
 
 
 @pytest.mark.parametrize("rng_mode", [PHILOX, MINSTD])
-@pytest.mark.parametrize("L,ns,choice", CLUSTER_CASES)
-def test_cluster_resident_kernel_equals_the_oracle(L, ns, choice, rng_mode):
+@pytest.mark.parametrize("L,ns", CLUSTER_CASES)
+def test_cluster_resident_kernel_equals_the_oracle(L, ns, rng_mode):
     """Calls of 8 half-sweeps and more run in ONE launch; E and M after every half-sweep, after every third, and none, final spins
     and energies against the oracle; a start at an odd counter (blue first)."""
-    if rng_mode == MINSTD and ns > 1:
-        choice = 4     # with MINSTD the library keeps many samples on the launches (cached seed states); on request here
+    choice = 4
     spins, J = synth.make_spins(L, ns, 7), synth.make_couplings(L, ns, 3)
     nsw = 5
     o, rec = oracle_trace(L, ns, rng_mode, spins, J, 0.6, 2 * nsw)
@@ -218,7 +218,10 @@ def test_cluster_resident_kernel_equals_one_launch_per_half_sweep(L, ns, choice,
         g.ising_load_state(dev(spins), dev(J))
     nsw = 200 if L == 64 and ns <= 32 else 30
     for every in (20, 7):
+        n0 = a.ising_kernel_launches()
         Ea, Ma = a.ising_sweep_trace(1 / 1.1, nsw, every_half_sweeps=every)
+        if choice == 4 or rng_mode == PHILOX:
+            assert a.ising_kernel_launches() - n0 == 2, "the pre-set of the records and ONE launch"
         Eb, Mb = b.ising_sweep_trace(1 / 1.1, nsw, every_half_sweeps=every)
         assert Ea.shape[0] == 2 * nsw // every and torch.equal(Ea, Eb) and torch.equal(Ma, Mb), every
         assert torch.equal(a.ising_get_spins(), b.ising_get_spins())
