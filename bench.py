@@ -697,12 +697,16 @@ def main():
             return out
 
         rows = []
-        for idx in (1, 2, 3, 4, 5):
+        from paper_1411_0127_b200 import LAYOUT_AUTO, LAYOUT_SAMPLE_PACKED
+
+        # config 2 twice: in the library's own layout for 32 samples with their own draws (a batch of site-packed lattices, run by the
+        # cluster-resident kernel) and in the paper's sample-packed storage, "one sample per bit of each uint32"
+        for idx, layout in ((1, LAYOUT_AUTO), (2, LAYOUT_AUTO), (2, LAYOUT_SAMPLE_PACKED), (3, LAYOUT_AUTO), (4, LAYOUT_AUTO), (5, LAYOUT_AUTO)):
             cfg, sp_np, J_np = synth.make_config(idx)
             Ls, ns, nsweeps, beta = cfg["L"], cfg["nsamples"], cfg["sweeps"], cfg["beta"]
             sp = torch.from_numpy(sp_np.view(np.int32)).cuda()
             Jc = torch.from_numpy(J_np.view(np.int32)).cuda()
-            g = Ising(Ls, ns, synth.DYN_SEED, cfg["rng_mode"])
+            g = Ising(Ls, ns, synth.DYN_SEED, cfg["rng_mode"], layout=layout)
             out = torch.empty_like(sp)
             if idx == 4:
                 from concurrent.futures import ThreadPoolExecutor
@@ -765,7 +769,9 @@ def main():
             if "fnv" in res:
                 got["fnv"] = res["fnv"]
             g.ising_destroy()
-            row = {"config": idx, "L": Ls, "nsamples": ns, "sweeps": nsweeps, "rng_mode": cfg["rng_mode"], "wall_ms": 1e3 * wall,
+            row = {"config": idx, "layout": "sample-packed (on request)" if layout == LAYOUT_SAMPLE_PACKED else
+                   ("batch of site-packed lattices" if ns > 1 else "site-packed"),
+                   "L": Ls, "nsamples": ns, "sweeps": nsweeps, "rng_mode": cfg["rng_mode"], "wall_ms": 1e3 * wall,
                    "ps_per_flip_including_outputs": 1e12 * wall / (nsweeps * ns * Ls**3), "kernel_launches": launches,
                    "us_per_half_sweep_including_outputs": 1e6 * wall / (2 * nsweeps),
                    "last_output": got["fnv"][-1] if "fnv" in got else (got["E"][-1] if idx != 2 else got["E"][-1][0])}
