@@ -56,6 +56,7 @@ extern "C" {
                              rng_mode, a mode that does not support (L, nsamples), null pointer, workspace too small /
                              misaligned, beta < 0 or NaN, nsweeps < 0 */
 #define ISING_ECUDA (-2)  /* a CUDA runtime call or kernel launch failed (sticky errors surface here too) */
+#define ISING_ELIMIT (-3) /* ising_energy_static only: L beyond ISING_STATIC_MAX_L, the size its fixed scratch is built for */
 
 #define ISING_RNG_PHILOX 0 /* Philox4x32-10, key (lo32 seed, hi32 seed ^ sample), counter (t, colour-rank>>2)  (R9, R10).
                               Because the sample index is XORed into the high key word, (seed, sample) and
@@ -134,6 +135,19 @@ int ising_sweep_trace(ising_t *h, double beta, int nsweeps, int64_t *d_E, int64_
 /* E[s] = - sum over the 3N bonds of J sigma sigma (Eq. 1, each bond once; R16) and M[s] = sum_i sigma_i for
  * every sample (row a9).  d_E: nsamples int64; d_M: nsamples int64 or NULL. */
 int ising_energy(ising_t *h, int64_t *d_E, int64_t *d_M, void *stream);
+
+/* The same E and M (row a9; Eq. 1, R16) for ONE sample given in the canonical packed format, for callers that cannot allocate: no
+ * handle, no workspace, and the library calls no cudaMalloc / cudaFree / allocating routine on this path (code under CUDA graph
+ * capture, serving loops, harnesses that forbid allocation).  d_spins: L^3/32 uint32, d_J: 3 x L^3/32 uint32 (device, read only);
+ * d_E: one int64; d_M: one int64 or NULL (device, written); asynchronous on `stream`, on the CURRENT device.
+ *   The scratch the kernels need -- the eight colour-separated bit arrays (row a10) and the counter slots of the energy kernel --
+ * is a fixed array in the library's device image: 8 x ISING_STATIC_MAX_L^3 / 16 bytes + 1040 = 1 MiB + 1 KiB, held by every GPU
+ * that loads the library until the process exits.  Hence the limits: L a multiple of 64 (else ISING_EINVAL) and
+ * L <= ISING_STATIC_MAX_L (else ISING_ELIMIT: use a handle).  ALL calls on a device share that array: calls that overlap on the
+ * GPU (two streams, two host threads) race and give wrong results; calls on one stream are safe, each one clears the counters it
+ * needs zeroed and overwrites the arrays whole, so nothing of an earlier call is seen. */
+#define ISING_STATIC_MAX_L 128
+int ising_energy_static(int L, const uint32_t *d_spins, const uint32_t *d_J, int64_t *d_E, int64_t *d_M, void *stream);
 
 /* Overlap of two samples of one handle, q = sum_i sigma_i^a sigma_i^b in [-N, N] (one int64 at d_q): the spin-glass order
  * parameter when the two samples are replicas, i.e. were loaded with the same couplings.  nsamples = 32k only. */

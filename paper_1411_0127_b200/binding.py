@@ -14,7 +14,8 @@ from . import build as _build
 PHILOX, MINSTD, PHILOX_SHARED = 0, 1, 2
 PR_SHARED, MT19937_SHARED = 3, 4  # shared draw from stored-state lane generators (include/ising.h, R19)
 LAYOUT_AUTO, LAYOUT_SAMPLE_PACKED, LAYOUT_BATCH = 0, 1, 2  # ising_create_layout
-OK, EINVAL, ECUDA = 0, -1, -2
+OK, EINVAL, ECUDA, ELIMIT = 0, -1, -2, -3
+STATIC_MAX_L = 128  # ising_energy_static
 
 EXPORTS = (
     "ising_workspace_bytes", "ising_create", "ising_create_layout", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
@@ -22,7 +23,7 @@ EXPORTS = (
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
     "ising_slab_workspace_bytes", "ising_create_slab", "ising_slab_half_sweep_boundary", "ising_slab_half_sweep_bulk", "ising_slab_plane",
-    "ising_slab_sweep_local", "ising_sliced_scratch_bytes", "ising_sliced_begin", "ising_sliced_sweep", "ising_sliced_end",
+    "ising_energy_static", "ising_slab_sweep_local", "ising_sliced_scratch_bytes", "ising_sliced_begin", "ising_sliced_sweep", "ising_sliced_end",
 )
 
 _lib = None
@@ -48,6 +49,7 @@ def lib() -> C.CDLL:
     L.ising_energy.argtypes = [vp, vp, vp, vp]
     L.ising_get_spins.argtypes = [vp, vp, vp]
     L.ising_overlap.argtypes = [vp, i32, i32, vp, vp]
+    L.ising_energy_static.argtypes = [i32, vp, vp, vp, vp, vp]
     L.ising_run_host.argtypes = [vp, vp, vp, dbl, i32, vp, vp, vp, vp]
     L.ising_run_host_async.argtypes = [vp, vp, vp, dbl, i32, vp, vp, vp, vp]
     L.ising_thresholds.argtypes = [dbl, i32, C.POINTER(u64)]
@@ -139,6 +141,20 @@ def _stream_ptr(stream=None) -> int:
     import torch
 
     return (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+
+
+def ising_energy_static(L: int, spins, J, E, M=None, stream=None) -> None:
+    """E (and M) of ONE canonical packed sample without a handle, a workspace or any allocation: the scratch is a fixed array in
+    the library (include/ising.h: L a multiple of 64, L <= STATIC_MAX_L; calls that overlap on the GPU race).  spins: (L^3/32,)
+    and J: (3 L^3/32,) 4-byte-element CUDA tensors; E, M: caller-owned one-element int64 CUDA tensors, written asynchronously on
+    `stream` (default: torch's current stream) of the tensors' device.  Nothing is allocated here either."""
+    import torch
+
+    assert spins.is_cuda and J.is_cuda and E.is_cuda and E.dtype == torch.int64 and (M is None or (M.is_cuda and M.dtype == torch.int64))
+    assert spins.is_contiguous() and J.is_contiguous() and spins.numel() * 32 == L**3 and J.numel() * 32 == 3 * L**3 or L % 64 != 0 or L > STATIC_MAX_L
+    with torch.cuda.device(spins.device):
+        _check(lib().ising_energy_static(int(L), spins.data_ptr(), J.data_ptr(), E.data_ptr(), M.data_ptr() if M is not None else None,
+                                         _stream_ptr(stream)), "ising_energy_static")
 
 
 def _u32(t):

@@ -2011,12 +2011,89 @@ int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double 
     return ISING_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// ising_energy_static: E and M of a canonical packed configuration with NO caller workspace and no allocation of any kind
+// (include/ising.h).  The scratch -- the eight colour-separated bit arrays the energy kernel reads, and its counter slots -- lives
+// in a file-scope device array of fixed size, which every GPU that loads the library holds until the process exits.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int STATIC_MAX_L = ISING_STATIC_MAX_L;
+constexpr size_t STATIC_ARRAY_WORDS = (size_t)STATIC_MAX_L * STATIC_MAX_L * STATIC_MAX_L / 64;   // one colour array at the largest L
+constexpr size_t STATIC_SLOT_WORDS = 2 * (2 * ACC_SLOTS + 2);                                      // counter pairs + ticket, as uint32 words
+constexpr size_t STATIC_SCRATCH_WORDS = 8 * STATIC_ARRAY_WORDS + STATIC_SLOT_WORDS;                // 1 MiB + 1040 B at L = 128
+
+// In host code this name is a host-side stand-in, not a device address: the kernels get the address cudaGetSymbolAddress returns.
+static __device__ __align__(256) uint32_t g_static_scratch[STATIC_SCRATCH_WORDS];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+uint32_t *g_static_ptr[STATIC_MAX_DEVICES] = {};   // device address of g_static_scratch on each device, looked up once per device
+
+// The scratch of the CURRENT device (nullptr: no device / lookup failed).  Every device has its own copy of a __device__ variable,
+// so the address is taken once per device, with that device current.
+uint32_t *static_scratch_of_current_device()
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= STATIC_MAX_DEVICES) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void *p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess || !p) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        g_static_ptr[dev] = (uint32_t *)p;
+    }
+    return g_static_ptr[dev];
+}
+
+}  // namespace
+
+int ising_energy_static(int L, const uint32_t *d_spins, const uint32_t *d_J, int64_t *d_E, int64_t *d_M, void *stream)
+{
+    if (!d_spins || !d_J || !d_E || L < 64 || L % 64 != 0) return ISING_EINVAL;
+    if (L > STATIC_MAX_L) return ISING_ELIMIT;
+    uint32_t *scratch = static_scratch_of_current_device();
+    if (!scratch) return ISING_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t aw = (size_t)L * L * L / 64;   // words of one colour array (no padding when L is a multiple of 64)
+    const size_t W = (size_t)L * L * L / 32;    // canonical words per bit array
+    unsigned long long *slots = (unsigned long long *)(scratch + 8 * STATIC_ARRAY_WORDS);
+    // the array keeps the last call's contents: the counters and the ticket must start at zero (the arrays are overwritten whole)
+    if (cudaMemsetAsync(slots, 0, STATIC_SLOT_WORDS * sizeof(uint32_t), st) != cudaSuccess) return ISING_ECUDA;
+    SplitArgs s = {};
+    MeasureArgs m;
+    s.narrays = 4;
+    s.L = L;
+    m.L = L;
+    for (int q = 0; q < 4; ++q) {       // q = 0: spins, 1 + d: couplings of direction d
+        s.canon[q] = q == 0 ? d_spins : d_J + (size_t)(q - 1) * W;
+        for (int c = 0; c < 2; ++c) {
+            s.out[q][c] = scratch + (size_t)(2 * q + c) * aw;
+            if (q == 0) m.S[c] = s.out[q][c];
+            else m.J[q - 1][c] = s.out[q][c];
+        }
+    }
+    // words per thread as make_geometry chooses them for L <= 128: one
+    const uint64_t n = (uint64_t)(L >> 6) * L * L;
+    split_colours_site_packed<1><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s);
+    const int tpr_pad = row_map_tpr_pad(L >> 6);
+    const dim3 grid((unsigned)(L / (32 / tpr_pad)), (unsigned)(L / (SWEEP_THREADS / 32)));
+    energy_site_packed<1><<<grid, SWEEP_THREADS, 0, st>>>(m, slots, (long long)L * L * L, (long long *)d_E, (long long *)d_M);
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
+}
+
 const char *ising_strerror(int code)
 {
     switch (code) {
         case ISING_OK: return "ok";
         case ISING_EINVAL: return "invalid argument";
         case ISING_ECUDA: return "CUDA error";
+        case ISING_ELIMIT: return "size beyond the fixed scratch of ising_energy_static (L <= ISING_STATIC_MAX_L)";
         default: return "unknown error";
     }
 }
