@@ -44,9 +44,9 @@ LANE_STATE_BYTES_PER_DRAW = {3: 16.0, 4: 13.0}
 # belongs to the kernel sources it was captured on: `kernel_sources_sha256` is kernel_sources_hash() at capture time, and
 # the bench line prints `traffic` only while the sources still hash to it (null otherwise, with a note).
 NCU_TRAFFIC_L1024 = {
-    "kernel_sources_sha256": "e315f2df378099b82362b3107d7bf75dcbcc35d71ee4c86f7362b5e650dc227a",
-    "capture": "profiles/r2z_end_of_round.md",
-    0: 537.05e6 + 58.61e6, 1: 2684.53e6 + 61.61e6,
+    "kernel_sources_sha256": "200688f003616987ca7ca7b8dd9fe1dc69f411033281600f6c08fe7dd27d663b",
+    "capture": "profiles/r2n_end_of_round.md",
+    0: 537.05e6 + 58.26e6, 1: 2684.52e6 + 60.48e6,
 }
 
 
