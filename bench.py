@@ -544,7 +544,7 @@ def main():
             ref = Ising(L, 1, synth.DYN_SEED, mode)
             ref.ising_load_state(d_spins, d_J)
             ref.ising_sweep(BETA, 2)
-            times = {}
+            times, times_push = {}, {}
             for G in sorted({1, args.slabs}):
                 hs = [IsingSlab(L, G, r, synth.DYN_SEED, mode) for r in range(G)]
                 for h in hs:
@@ -562,6 +562,16 @@ def main():
                     ms = a.elapsed_time(b)
                     best = ms if best is None or ms < best else best
                 times[G] = best
+                best = None
+                for _ in range(3):   # the exchange fused into the boundary kernels (ising_slab_connect), no copies
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(sa)
+                    binding.ising_slab_sweep_local(hs, BETA, nsw, sa, sb, push=True)
+                    b.record(sa)
+                    torch.cuda.synchronize()
+                    ms = a.elapsed_time(b)
+                    best = ms if best is None or ms < best else best
+                times_push[G] = best
                 out = torch.zeros_like(d_out)
                 for h in hs:
                     h.ising_get_spins(out)
@@ -579,7 +589,9 @@ def main():
             rows.append({"L": L, "rng_mode": ["philox", "minstd"][mode], "sweeps": nsw, "undivided_ms": best,
                          "undivided_ps_per_flip": 1e9 * best / (nsw * N),
                          **{f"slabs_{G}_ms": t for G, t in times.items()},
-                         **{f"slabs_{G}_over_undivided": t / best for G, t in times.items()}})
+                         **{f"slabs_{G}_over_undivided": t / best for G, t in times.items()},
+                         **{f"slabs_{G}_fused_exchange_ms": t for G, t in times_push.items()},
+                         **{f"slabs_{G}_fused_exchange_over_undivided": t / best for G, t in times_push.items()}})
         print(json.dumps({"slabs": rows}))
         return
 

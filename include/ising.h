@@ -240,10 +240,24 @@ int ising_slab_half_sweep_bulk(ising_t *h, double beta, void *stream);
  * plane (to send down / up after a half-sweep of `colour`), 2 = lower halo, 3 = upper halo (to receive the plane 1 of the slab
  * below / the plane 0 of the slab above). */
 int ising_slab_plane(ising_t *h, int colour, int which, void **d_ptr, size_t *bytes);
+/* The exchange fused into the boundary kernel.  ising_slab_connect tells a slab where its neighbours' halos are: for each colour c,
+ * d_below_upper_halo[c] = plane 3 (upper halo) of colour c of the slab BELOW, d_above_lower_halo[c] = plane 2 (lower halo) of the
+ * slab ABOVE, as ising_slab_plane of those handles names them -- device addresses valid on THIS slab's device: the same GPU, or a
+ * peer GPU's memory mapped into this process (cudaDeviceEnablePeerAccess, or cudaIpcOpenMemHandle of the neighbour process's
+ * workspace); 16-byte aligned; the handle keeps the pointers, not the memory.  ising_slab_half_sweep_boundary_push is the boundary
+ * part whose threads store the updated words of the first / last owned plane a second time, into those halos: over NVLink the
+ * planes travel while the kernel runs, and no copy is launched.  Ordering is as for the copies: the next half-sweep may start on a
+ * slab only when this kernel has completed on the slab itself AND on its two neighbours (an event per half-sweep between the
+ * devices' streams; a kernel's peer stores are visible when it has completed).  ISING_EINVAL if the slab is not connected. */
+int ising_slab_connect(ising_t *h, void *const d_below_upper_halo[2], void *const d_above_lower_halo[2]);
+int ising_slab_half_sweep_boundary_push(ising_t *h, double beta, void *stream);
+
 /* nsweeps sweeps of a lattice whose `nslabs` slab handles (slabs[r] = slab r, all at the same counter t, same seed and mode) live
  * in this process on the current device: boundary kernels and plane copies (cudaMemcpyAsync) on stream_a, bulk kernels on
  * stream_b, an event pair between half-sweeps.  The two streams must differ; on return both have been made to wait for each other. */
 int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b);
+/* The same with the fused exchange: connects every slab to its neighbours and runs the _push boundary kernels; no copies. */
+int ising_slab_sweep_local_push(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b);
 
 /* ---- the paper's sliced layout (Eq. 4-6; Appendix A) ----
  * An alternative internal layout of a one-sample lattice, kept beside the handle's own arrays in a caller-owned scratch buffer:

@@ -23,7 +23,7 @@ EXPORTS = (
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
     "ising_slab_workspace_bytes", "ising_create_slab", "ising_slab_half_sweep_boundary", "ising_slab_half_sweep_bulk", "ising_slab_plane",
-    "ising_energy_static", "ising_slab_sweep_local", "ising_sliced_scratch_bytes", "ising_sliced_begin", "ising_sliced_sweep", "ising_sliced_end",
+    "ising_energy_static", "ising_slab_connect", "ising_slab_half_sweep_boundary_push", "ising_slab_sweep_local_push", "ising_slab_sweep_local", "ising_sliced_scratch_bytes", "ising_sliced_begin", "ising_sliced_sweep", "ising_sliced_end",
 )
 
 _lib = None
@@ -74,6 +74,9 @@ def lib() -> C.CDLL:
     L.ising_slab_half_sweep_bulk.argtypes = [vp, dbl, vp]
     L.ising_slab_plane.argtypes = [vp, i32, i32, C.POINTER(vp), C.POINTER(sz)]
     L.ising_slab_sweep_local.argtypes = [C.POINTER(vp), i32, dbl, i32, vp, vp]
+    L.ising_slab_sweep_local_push.argtypes = [C.POINTER(vp), i32, dbl, i32, vp, vp]
+    L.ising_slab_connect.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+    L.ising_slab_half_sweep_boundary_push.argtypes = [vp, dbl, vp]
     L.ising_sliced_scratch_bytes.argtypes = [vp, C.POINTER(sz)]
     L.ising_sliced_begin.argtypes = [vp, vp, vp]
     L.ising_sliced_sweep.argtypes = [vp, vp, dbl, i32, vp]
@@ -378,6 +381,27 @@ class IsingSlab(Ising):
         with self._on_device():
             _check(lib().ising_slab_half_sweep_boundary(self._h, float(beta), _stream_ptr(stream)), "ising_slab_half_sweep_boundary")
 
+    def ising_slab_connect(self, below, above):
+        """Fused exchange: `below` / `above` are the neighbouring IsingSlab handles (same process; their workspaces must be
+        addressable from this slab's device) or pairs of raw device addresses (colour 0, colour 1) of the upper halo of the slab
+        below / the lower halo of the slab above (e.g. opened from CUDA IPC handles)."""
+        def addresses(x, which):
+            if isinstance(x, IsingSlab):
+                out = []
+                for c in (0, 1):
+                    ptr, nbytes = C.c_void_p(), C.c_size_t(0)
+                    _check(lib().ising_slab_plane(x._h, c, which, C.byref(ptr), C.byref(nbytes)), "ising_slab_plane")
+                    out.append(ptr.value)
+                return out
+            return [int(v) for v in x]
+        dn = (C.c_void_p * 2)(*addresses(below, 3))
+        up = (C.c_void_p * 2)(*addresses(above, 2))
+        _check(lib().ising_slab_connect(self._h, dn, up), "ising_slab_connect")
+
+    def ising_slab_half_sweep_boundary_push(self, beta: float, stream=None):
+        with self._on_device():
+            _check(lib().ising_slab_half_sweep_boundary_push(self._h, float(beta), _stream_ptr(stream)), "ising_slab_half_sweep_boundary_push")
+
     def ising_slab_half_sweep_bulk(self, beta: float, stream=None):
         with self._on_device():
             _check(lib().ising_slab_half_sweep_bulk(self._h, float(beta), _stream_ptr(stream)), "ising_slab_half_sweep_bulk")
@@ -391,10 +415,11 @@ class IsingSlab(Ising):
         return self.workspace[off:off + nbytes.value]
 
 
-def ising_slab_sweep_local(slabs, beta: float, nsweeps: int, stream_a, stream_b):
+def ising_slab_sweep_local(slabs, beta: float, nsweeps: int, stream_a, stream_b, push: bool = False):
     """All slabs of a lattice in this process on one device: nsweeps sweeps, boundary kernels and plane copies on stream_a, bulk
-    kernels on stream_b (the paper's Fig. 10 with device-to-device copies as the exchange)."""
+    kernels on stream_b (the paper's Fig. 10 with device-to-device copies as the exchange).  push: the exchange fused into the
+    boundary kernels (they store their end planes into the neighbours' halos), no copies."""
     arr = (C.c_void_p * len(slabs))(*[s._h for s in slabs])
+    fn = lib().ising_slab_sweep_local_push if push else lib().ising_slab_sweep_local
     with slabs[0]._on_device():
-        _check(lib().ising_slab_sweep_local(arr, len(slabs), float(beta), int(nsweeps), stream_a.cuda_stream, stream_b.cuda_stream),
-               "ising_slab_sweep_local")
+        _check(fn(arr, len(slabs), float(beta), int(nsweeps), stream_a.cuda_stream, stream_b.cuda_stream), "ising_slab_sweep_local")

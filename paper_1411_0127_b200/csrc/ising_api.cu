@@ -150,6 +150,7 @@ struct ising {
     GraphEntry graphs[8];
     int ngraphs;
     uint64_t graph_clock;
+    uint32_t *push_dn[2], *push_up[2];   // z-slab handles, per colour: the neighbours' halo planes this slab's boundary kernel stores into (ising_slab_connect)
     int nslabs, slab, z0, Lz;  // z-slab handles (ising_create_slab): this handle owns the planes z0 .. z0 + Lz - 1; nslabs = 0 otherwise
     unsigned int *epochs;  // tile epochs of the persistent kernels (nullptr: no persistent path for this geometry / mode)
     bool no_cluster;       // kernel choice 5: the automatic choice without the cluster-resident kernels
@@ -1243,10 +1244,20 @@ void launch_slab(int W, const dim3 grid, cudaStream_t st, const SweepArgs &a, co
     else if (W == 5) launch_slab_w<RNG, 5>(grid, st, a, sr);
     else launch_slab_w<RNG, 1>(grid, st, a, sr);
 }
+// the boundary kernel that also stores its end planes into the neighbours' halos (slab_kernels.cuh)
+template <int RNG>
+void launch_slab_push(int W, const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, const SlabPush &p)
+{
+    if (W == 4) half_sweep_site_packed_slab_push<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
+    else if (W == 3) half_sweep_site_packed_slab_push<RNG, 3><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
+    else if (W == 5) half_sweep_site_packed_slab_push<RNG, 5><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
+    else half_sweep_site_packed_slab_push<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
+}
 
 // part 0: the CTA rows holding the first and the last 8 planes of the slab (the paper's boundary kernel); part 1: the rows in
 // between (its bulk kernel).  Neither advances the counter.  A part without rows launches nothing.
-int slab_half_sweep_part(ising_t *h, const Thresholds &T, int part, cudaStream_t st)
+// push: the boundary part also stores the slab's end planes into the neighbours' halos (ising_slab_connect), fusing the exchange.
+int slab_half_sweep_part(ising_t *h, const Thresholds &T, int part, cudaStream_t st, bool push = false)
 {
     const Geometry &g = h->g;
     const int nby = h->Lz / (SWEEP_THREADS / 32);
@@ -1280,15 +1291,22 @@ int slab_half_sweep_part(ising_t *h, const Thresholds &T, int part, cudaStream_t
     sr.A2 = 2u * r.A;
     sr.s0tab = nullptr;
     const dim3 grid = slab_grid(h, rows);
-    if (h->rng_mode == ISING_RNG_PHILOX) {
-        launch_slab<0>(g.W, grid, st, a, sr);
-    } else if (h->kernel_choice != 2 && h->s0tab != nullptr && h->s0_ready) {   // MINSTD with the seed table (filled by the loader)
-        uint4 *tab[2] = {(uint4 *)h->s0tab, (uint4 *)(h->s0tab + g.s0_words / 2)};
-        sr.s0tab = tab[c];
-        launch_slab<2>(g.W, grid, st, a, sr);
-    } else {
-        launch_slab<1>(g.W, grid, st, a, sr);
+    const bool table = h->rng_mode == ISING_RNG_MINSTD && h->kernel_choice != 2 && h->s0tab != nullptr && h->s0_ready;   // (filled by the loader)
+    if (table) sr.s0tab = (uint4 *)(h->s0tab + (c ? g.s0_words / 2 : 0));
+    if (push && part == 0) {
+        if (!h->push_dn[c] || !h->push_up[c]) return ISING_EINVAL;   // not connected
+        SlabPush p;
+        p.dn = h->push_dn[c];
+        p.up = h->push_up[c];
+        p.Lz = h->Lz;
+        if (h->rng_mode == ISING_RNG_PHILOX) launch_slab_push<0>(g.W, grid, st, a, sr, p);
+        else if (table) launch_slab_push<2>(g.W, grid, st, a, sr, p);
+        else launch_slab_push<1>(g.W, grid, st, a, sr, p);
+        return check_launch(h);
     }
+    if (h->rng_mode == ISING_RNG_PHILOX) launch_slab<0>(g.W, grid, st, a, sr);
+    else if (table) launch_slab<2>(g.W, grid, st, a, sr);
+    else launch_slab<1>(g.W, grid, st, a, sr);
     return check_launch(h);
 }
 
@@ -1379,6 +1397,7 @@ int ising_create_layout(int L, int nsamples, uint64_t seed, int rng_mode, int la
     h->cluster_size = 0;
     h->no_cluster = false;
     h->nslabs = h->slab = h->z0 = h->Lz = 0;
+    h->push_dn[0] = h->push_dn[1] = h->push_up[0] = h->push_up[1] = nullptr;
     h->dyn_slot = -1;
     h->dyn = (DynConst *)((char *)h->acc + h->g.acc_bytes - round_up(sizeof(DynConst), 256));
     h->cap_stream = nullptr;
@@ -1844,6 +1863,27 @@ int ising_slab_half_sweep_boundary(ising_t *h, double beta, void *stream)
     return slab_half_sweep_part(h, kernel_thresholds(T), 0, (cudaStream_t)stream);
 }
 
+int ising_slab_connect(ising_t *h, void *const d_below_upper_halo[2], void *const d_above_lower_halo[2])
+{
+    if (!h || !h->nslabs || !d_below_upper_halo || !d_above_lower_halo) return ISING_EINVAL;
+    for (int c = 0; c < 2; ++c)
+        if (!d_below_upper_halo[c] || !d_above_lower_halo[c] || ((uintptr_t)d_below_upper_halo[c] & 15u) || ((uintptr_t)d_above_lower_halo[c] & 15u))
+            return ISING_EINVAL;
+    for (int c = 0; c < 2; ++c) {
+        h->push_dn[c] = (uint32_t *)d_below_upper_halo[c];
+        h->push_up[c] = (uint32_t *)d_above_lower_halo[c];
+    }
+    return ISING_OK;
+}
+
+int ising_slab_half_sweep_boundary_push(ising_t *h, double beta, void *stream)
+{
+    if (!h || !h->nslabs || !on_own_device(h)) return ISING_EINVAL;
+    uint64_t T[3];
+    if (compute_thresholds(beta, h->rng_mode, T) != ISING_OK) return ISING_EINVAL;
+    return slab_half_sweep_part(h, kernel_thresholds(T), 0, (cudaStream_t)stream, true);
+}
+
 int ising_slab_half_sweep_bulk(ising_t *h, double beta, void *stream)
 {
     if (!h || !h->nslabs || !on_own_device(h)) return ISING_EINVAL;
@@ -1862,7 +1902,21 @@ int ising_slab_plane(ising_t *h, int colour, int which, void **d_ptr, size_t *by
     return ISING_OK;
 }
 
+static int slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b, bool push);
+
 int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b)
+{
+    return slab_sweep_local(slabs, nslabs, beta, nsweeps, stream_a, stream_b, false);
+}
+
+int ising_slab_sweep_local_push(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b)
+{
+    return slab_sweep_local(slabs, nslabs, beta, nsweeps, stream_a, stream_b, true);
+}
+
+// push: the boundary kernels store their end planes into the neighbours' halos themselves (the slabs are connected here: all of
+// them live on this device), and there are no copies.
+static int slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps, void *stream_a, void *stream_b, bool push)
 {
     if (!slabs || nslabs < 1 || nsweeps < 0 || !stream_a || !stream_b || stream_a == stream_b) return ISING_EINVAL;
     for (int s = 0; s < nslabs; ++s)
@@ -1874,6 +1928,12 @@ int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps
     if (compute_thresholds(beta, slabs[0]->rng_mode, T) != ISING_OK) return ISING_EINVAL;
     const Thresholds kt = kernel_thresholds(T);
     cudaStream_t sa = (cudaStream_t)stream_a, sb = (cudaStream_t)stream_b;
+    if (push)
+        for (int s = 0; s < nslabs; ++s) {
+            ising_t *below = slabs[(s + nslabs - 1) % nslabs], *above = slabs[(s + 1) % nslabs];
+            void *dn[2] = {slab_plane_ptr(below, 0, 3), slab_plane_ptr(below, 1, 3)}, *up[2] = {slab_plane_ptr(above, 0, 2), slab_plane_ptr(above, 1, 2)};
+            if (ising_slab_connect(slabs[s], dn, up) != ISING_OK) return ISING_EINVAL;
+        }
     cudaEvent_t ea, eb;
     if (cudaEventCreateWithFlags(&ea, cudaEventDisableTiming) != cudaSuccess) return ISING_ECUDA;
     if (cudaEventCreateWithFlags(&eb, cudaEventDisableTiming) != cudaSuccess) { cudaEventDestroy(ea); return ISING_ECUDA; }
@@ -1884,8 +1944,8 @@ int ising_slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweeps
     for (int k = 0; rc == ISING_OK && k < 2 * nsweeps; ++k) {
         const int c = (int)(slabs[0]->t & 1);
         // boundary kernels of all slabs, then the exchange of the updated colour's end planes: stream A
-        for (int s = 0; rc == ISING_OK && s < nslabs; ++s) rc = slab_half_sweep_part(slabs[s], kt, 0, sa);
-        for (int s = 0; rc == ISING_OK && s < nslabs; ++s) {
+        for (int s = 0; rc == ISING_OK && s < nslabs; ++s) rc = slab_half_sweep_part(slabs[s], kt, 0, sa, push);
+        for (int s = 0; rc == ISING_OK && !push && s < nslabs; ++s) {
             ising_t *below = slabs[(s + nslabs - 1) % nslabs], *above = slabs[(s + 1) % nslabs];
             if (cudaMemcpyAsync(slab_plane_ptr(below, c, 3), slab_plane_ptr(slabs[s], c, 0), plane_bytes, cudaMemcpyDeviceToDevice, sa) != cudaSuccess ||
                 cudaMemcpyAsync(slab_plane_ptr(above, c, 2), slab_plane_ptr(slabs[s], c, 1), plane_bytes, cudaMemcpyDeviceToDevice, sa) != cudaSuccess)

@@ -35,6 +35,38 @@ half_sweep_site_packed_slab(const __grid_constant__ SweepArgs a, const __grid_co
                                                  unused0, unused1);
 }
 
+// The same with the exchange fused into the kernel (SURVEY.md section 5 "direct remote stores into the neighbour's halo buffer"): the
+// threads whose rows lie in the slab's first / last owned plane store their updated words a second time, into the upper halo of the
+// slab below / the lower halo of the slab above -- plain stores to addresses that are valid on this device: the neighbour's workspace
+// on the same GPU, or on a peer GPU mapped over NVLink (peer access / CUDA IPC), where they travel as the kernel runs instead of
+// as a separate copy after it.  The words are read back from the thread's own store (L2, coherent load) so that the tile update of
+// sweep_kernels.cuh stays as it is.  Nobody reads the halos of the ACTIVE colour during this half-sweep (z-neighbours are of the
+// other colour), so the remote stores race with nothing; the next half-sweep must wait for this kernel on every slab, as it must
+// for the copies.
+struct SlabPush {
+    uint32_t *dn, *up;   // active colour: upper halo plane of the slab below, lower halo plane of the slab above
+    int Lz;
+};
+
+template <int RNG, int W>
+__global__ void __launch_bounds__(SWEEP_THREADS)
+half_sweep_site_packed_slab_push(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, const SlabPush p)
+{
+    unsigned long long unused0 = 0, unused1 = 0;
+    const uint32_t by = (uint32_t)a.by_first + blockIdx.y * (uint32_t)a.by_stride;
+    site_packed_tile<RNG, W, false, false, true>(a, rng, blockIdx.x, by, gridDim.x, unused0, unused1);
+    const RowMap rm = row_map<W>(a.L, blockIdx.x, by);
+    const int zl = rm.z + 1;   // plane in the slab's arrays (plane 0 is the lower halo)
+    if (rm.active && (zl == 1 || zl == p.Lz)) {
+        const uint32_t wpr = (uint32_t)a.L >> 6;
+        const uint32_t in_plane = wpr * (uint32_t)rm.y + (uint32_t)rm.k0;
+        uint32_t s[W];
+        load_spin_words<W, true>(a.S_act, (size_t)wpr * (uint32_t)a.L * (uint32_t)zl + in_plane, s);
+        if (zl == 1) store_words<W>(p.dn, in_plane, s);
+        if (zl == p.Lz) store_words<W>(p.up, in_plane, s);
+    }
+}
+
 // Unsatisfied bonds (+x, +y, +z bond of every owned site; the +z bond of the last owned plane reaches into the upper halo) and up
 // spins of the slab's own planes, added to acc[0], acc[1]: the slab's share of E and M; the shares of all slabs add up to the
 // lattice's (R16: E = 2 * unsatisfied - 3N, M = 2 * up - N).  grid = (L / (32 / tpr_pad), Lz / 8).
