@@ -430,13 +430,18 @@ def main():
         from paper_1411_0127_b200 import PHILOX_SHARED
 
         rows = []
-        cases = [(Ls, 1, m) for Ls in (64, 128, 256, 512, 1024, 2048) for m in (PHILOX, MINSTD)]
+        cases = [(Ls, 1, m) for Ls in (64, 128, 256, 512, 1024, 2048, 3072, 4096) for m in (PHILOX, MINSTD)]
         cases += [(Ls, 32, m) for Ls in (32, 64, 128, 256) for m in (PHILOX, MINSTD)]
         cases += [(64, 32, PHILOX_SHARED), (128, 32, PHILOX_SHARED), (128, 256, PHILOX_SHARED), (256, 32, PHILOX_SHARED),
                   (512, 32, PHILOX_SHARED)]
         for Ls, ns, mode in cases:
-            sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
-            Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
+            if Ls > 2048:   # 3.4-8.6 GiB of spin bits: random bits drawn on the device (the recipe's SplitMix64 stream on the host takes minutes)
+                gen = torch.Generator(device="cuda").manual_seed(Ls)
+                sp = torch.randint(-2**31, 2**31 - 1, (1, Ls**3 // 32), dtype=torch.int32, device="cuda", generator=gen)
+                Jc = torch.randint(-2**31, 2**31 - 1, (1, 3, Ls**3 // 32), dtype=torch.int32, device="cuda", generator=gen)
+            else:
+                sp = torch.from_numpy(synth.make_spins(Ls, ns).view(np.int32)).cuda()
+                Jc = torch.from_numpy(synth.make_couplings(Ls, ns).view(np.int32)).cuda()
             g = Ising(Ls, ns, synth.DYN_SEED, mode)
             g.ising_load_state(sp, Jc)
             nsweeps = max(2, min(200, int(2e10 / (ns * Ls**3))))

@@ -15,6 +15,9 @@
  *
  * Conventions
  *   N = L^3, site i = x + L*(y + L*z), colour (x+y+z)&1, red = 0 is updated at even half-sweep index t (R8).
+ *   Sizes: every even L from 4 to 2048 (all layouts and modes); one-sample lattices also L = 2560, 3072 and 4096, where the
+ *   Philox group index passes 2^32 (at L = 4096) and its high word enters the counter (R9), the MINSTD seed states are recomputed instead of
+ *   cached, and the workspace is 15.6, 27 and 64 GiB (L = 4096: 32 GiB of bit arrays + 32 GiB of canonical staging).
  *   The half-sweep counter t starts at 0 in ising_create and keeps counting over all sweep calls, so a
  *   trajectory does not depend on how sweeps are batched into calls.
  *   Canonical packed format (the only format that crosses this boundary):
@@ -52,7 +55,7 @@ extern "C" {
 #endif
 
 #define ISING_OK 0
-#define ISING_EINVAL (-1) /* bad argument: L odd or < 4 or > 2048, nsamples not 1 or a multiple of 32, unknown
+#define ISING_EINVAL (-1) /* bad argument: L odd or < 4 or > 4096 (beyond 2048: one sample and L = 2560, 3072 or 4096 only), nsamples not 1 or a multiple of 32, unknown
                              rng_mode, a mode that does not support (L, nsamples), null pointer, workspace too small /
                              misaligned, beta < 0 or NaN, nsweeps < 0 */
 #define ISING_ECUDA (-2)  /* a CUDA runtime call or kernel launch failed (sticky errors surface here too) */

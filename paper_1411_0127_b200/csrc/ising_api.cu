@@ -24,7 +24,8 @@ using namespace isingk;
 namespace {
 
 constexpr size_t ALIGN_WORDS = 64;  // 256-byte alignment of every internal array
-constexpr int MAX_L = 2048;         // keeps the Philox group index g = j>>2 below 2^32 (rng.cuh)
+constexpr int MAX_L = 4096;         // Philox group index g = j>>2 below 2^33: counter word c3 = hi32(g) is 0 or 1 (rng.cuh, R9)
+constexpr int MAX_L_32BIT_GROUPS = 2048;   // up to here every layout is available (and g < 2^32; g passes 2^32 from L = 3252 on)
 
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -72,6 +73,12 @@ bool make_geometry(int L, int nsamples, Geometry *g, bool batched = false)
 {
     if (L < 4 || (L & 1) || L > MAX_L) return false;
     if (!(nsamples == 1 || (nsamples > 0 && nsamples % 32 == 0))) return false;
+    if (L > MAX_L_32BIT_GROUPS) {   // beyond 2^32 groups: one sample, the word-parallel layout with a row in at most 32 lanes
+        const int wpr = L >> 6;     // (L = 2560, 3072, 4096: rows of 5, 3, 1 x 2^e words)
+        int odd = wpr;
+        while (odd % 2 == 0) odd /= 2;
+        if (nsamples != 1 || L % 64 != 0 || !(odd == 1 || odd == 3 || odd == 5)) return false;
+    }
     const bool site = nsamples == 1 || batched;
     g->L = L;
     g->nsamples = nsamples;
@@ -107,12 +114,13 @@ bool make_geometry(int L, int nsamples, Geometry *g, bool batched = false)
     // (a batch: one table per sample, as long as all of them stay below 4 GiB; beyond that the seeds are recomputed)
     g->s0_words = g->fast ? 2 * (size_t)L * L * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32 : 0;
     if (g->batched) g->s0_words = g->s0_words * (size_t)nsamples <= (1ull << 30) ? g->s0_words * (size_t)nsamples : 0;
+    if (L > MAX_L_32BIT_GROUPS) g->s0_words = 0;   // 67-275 GB of table: the seeds are recomputed
     // persistent paths (persistent.cuh): one-sample lattices with whole-word rows below L = 512 get a tile grid with epoch counters
     // (used automatically up to L = 128, where it beats the launches); one-sample lattices of at most 1024 words per colour that
     // are not of that kind (every other even L <= 40) run on one SM out of shared memory
     g->epoch_words = 0;
     g->pgx = g->pgy = 0;
-    if (g->fast && g->W != 4) {
+    if (g->fast && g->W != 4 && L <= MAX_L_32BIT_GROUPS) {
         g->pgx = (uint32_t)(L / (32 / row_map_tpr_pad((L >> 6) / g->W)));
         g->pgy = (uint32_t)(L / (SWEEP_THREADS / 32));
         g->epoch_words = g->batched ? 0 : (size_t)g->pgx * g->pgy;
@@ -256,11 +264,39 @@ void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st
     if (cudaLaunchKernelEx(&cfg, kernel, args...) != cudaSuccess) g_launch_failed = true;
 }
 
+// The constants of the word-parallel kernels from the launch block; beyond L = 2048 also Philox's b, e for the counter word c3 = 1.
+SiteRng site_rng_of(const ising_t *h, const RngLaunch &r)
+{
+    SiteRng sr;
+    sr.pc = r.pc;
+    sr.ps = r.ps[0];
+    sr.seed = r.seed;
+    sr.A2 = 2u * r.A;
+    sr.s0tab = nullptr;
+    sr.b_hi = sr.e_hi = 0u;
+    if (h->rng_mode == ISING_RNG_PHILOX && h->g.L > MAX_L_32BIT_GROUPS) {
+        PhiloxCommonConst pc1;
+        PhiloxSampleConst ps1;
+        fold_philox(h->seed, 0u, h->t, &pc1, &ps1, 1u);
+        sr.b_hi = ps1.b;
+        sr.e_hi = ps1.e;
+    }
+    return sr;
+}
+
 // The word-parallel kernel for W words per thread, plain or with E and M of the resulting configuration (MEASURE).
 template <int RNG, int W>
 void launch_site_packed_w(bool measure, dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, unsigned long long *slots,
                           long long N, long long *mE, long long *mM)
 {
+    // lattices beyond L = 2048 with Philox: the instance that knows about the counter word c3 (sweep_kernels.cuh, BIG)
+    if (RNG == 0 && W >= 3 && a.L > MAX_L_32BIT_GROUPS) {
+        constexpr int WB = W >= 3 ? W : 4;
+        if (measure) launch_pdl(half_sweep_site_packed<0, WB, true, true>, grid, dim3(SWEEP_THREADS), st, a, sr, slots, N, mE, mM);
+        else launch_pdl(half_sweep_site_packed<0, WB, false, true>, grid, dim3(SWEEP_THREADS), st, a, sr, (unsigned long long *)nullptr, 0ll,
+                        (long long *)nullptr, (long long *)nullptr);
+        return;
+    }
     if (measure) launch_pdl(half_sweep_site_packed<RNG, W, true>, grid, dim3(SWEEP_THREADS), st, a, sr, slots, N, mE, mM);
     else launch_pdl(half_sweep_site_packed<RNG, W, false>, grid, dim3(SWEEP_THREADS), st, a, sr, (unsigned long long *)nullptr, 0ll,
                     (long long *)nullptr, (long long *)nullptr);
@@ -427,12 +463,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
             unsigned long long *slots = nullptr;   // (the measuring variant adds to the pre-set record itself: add_to_record)
             const int tpr_pad = row_map_tpr_pad(wpr / W);
             const dim3 grid((unsigned)(g.L / (32 / tpr_pad)), (unsigned)(g.L / (SWEEP_THREADS / 32)));
-            SiteRng sr;
-            sr.pc = r.pc;
-            sr.ps = r.ps[0];
-            sr.seed = r.seed;
-            sr.A2 = 2u * r.A;
-            sr.s0tab = nullptr;
+            SiteRng sr = site_rng_of(h, r);
             // MINSTD: the seed states s0(seed, site) come from the table unless kernel choice 2 asks for recomputation
             const bool cached = RNG == 1 && h->kernel_choice != 2 && h->s0tab != nullptr;
             if (g.batched) {   // all samples in one launch (blockIdx.z = sample; a, sr are sample 0 here, b == 0)
@@ -1144,6 +1175,7 @@ bool make_slab_geometry(int L, int nslabs, Geometry *g, int *Lz)
     g->arrays_total_words = 8 * g->array_words;
     g->staging_words = ALIGN_WORDS;                                            // no host-buffer path for slabs
     g->s0_words = 2 * (size_t)L * (size_t)*Lz * row_map_tpr_pad((L >> 6) / g->W) * g->W * 32;   // seed table of the slab's own planes
+    if (L > MAX_L_32BIT_GROUPS) g->s0_words = 0;                                                 // (recomputed beyond L = 2048, as for the whole lattice)
     g->epoch_words = 0;
     g->onchip = false;
     return true;
@@ -1234,7 +1266,22 @@ int slab_energy(ising_t *h, long long *d_E, long long *d_M, cudaStream_t st)
 template <int RNG, int W>
 void launch_slab_w(const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr)
 {
+    if (RNG == 0 && W >= 3 && a.L > MAX_L_32BIT_GROUPS) {
+        constexpr int WB = W >= 3 ? W : 4;
+        half_sweep_site_packed_slab<0, WB, true><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+        return;
+    }
     half_sweep_site_packed_slab<RNG, W><<<grid, SWEEP_THREADS, 0, st>>>(a, sr);
+}
+template <int RNG, int W>
+void launch_slab_push_w(const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, const SlabPush &p)
+{
+    if (RNG == 0 && W >= 3 && a.L > MAX_L_32BIT_GROUPS) {
+        constexpr int WB = W >= 3 ? W : 4;
+        half_sweep_site_packed_slab_push<0, WB, true><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
+        return;
+    }
+    half_sweep_site_packed_slab_push<RNG, W><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
 }
 template <int RNG>
 void launch_slab(int W, const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr)
@@ -1248,10 +1295,10 @@ void launch_slab(int W, const dim3 grid, cudaStream_t st, const SweepArgs &a, co
 template <int RNG>
 void launch_slab_push(int W, const dim3 grid, cudaStream_t st, const SweepArgs &a, const SiteRng &sr, const SlabPush &p)
 {
-    if (W == 4) half_sweep_site_packed_slab_push<RNG, 4><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
-    else if (W == 3) half_sweep_site_packed_slab_push<RNG, 3><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
-    else if (W == 5) half_sweep_site_packed_slab_push<RNG, 5><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
-    else half_sweep_site_packed_slab_push<RNG, 1><<<grid, SWEEP_THREADS, 0, st>>>(a, sr, p);
+    if (W == 4) launch_slab_push_w<RNG, 4>(grid, st, a, sr, p);
+    else if (W == 3) launch_slab_push_w<RNG, 3>(grid, st, a, sr, p);
+    else if (W == 5) launch_slab_push_w<RNG, 5>(grid, st, a, sr, p);
+    else launch_slab_push_w<RNG, 1>(grid, st, a, sr, p);
 }
 
 // part 0: the CTA rows holding the first and the last 8 planes of the slab (the paper's boundary kernel); part 1: the rows in
@@ -1284,12 +1331,7 @@ int slab_half_sweep_part(ising_t *h, const Thresholds &T, int part, cudaStream_t
     }
     RngLaunch r;
     fill_rng_launch(h, 0, &r);
-    SiteRng sr;
-    sr.pc = r.pc;
-    sr.ps = r.ps[0];
-    sr.seed = r.seed;
-    sr.A2 = 2u * r.A;
-    sr.s0tab = nullptr;
+    SiteRng sr = site_rng_of(h, r);
     const dim3 grid = slab_grid(h, rows);
     const bool table = h->rng_mode == ISING_RNG_MINSTD && h->kernel_choice != 2 && h->s0tab != nullptr && h->s0_ready;   // (filled by the loader)
     if (table) sr.s0tab = (uint4 *)(h->s0tab + (c ? g.s0_words / 2 : 0));
@@ -1849,7 +1891,7 @@ int ising_create_slab(int L, int nslabs, int slab, uint64_t seed, int rng_mode, 
     h->z0 = slab * h->Lz;
     h->staging = h->ws + h->g.arrays_total_words;
     h->acc = (unsigned long long *)(h->staging + h->g.staging_words);
-    h->s0tab = rng_mode == ISING_RNG_MINSTD ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
+    h->s0tab = rng_mode == ISING_RNG_MINSTD && h->g.s0_words ? (uint32_t *)((char *)h->acc + h->g.acc_bytes) : nullptr;
     h->epochs = nullptr;
     *out = h;
     return ISING_OK;
@@ -1967,7 +2009,7 @@ static int slab_sweep_local(ising_t **slabs, int nslabs, double beta, int nsweep
 // ---- the paper's sliced layout as an alternative internal layout (sliced_kernels.cuh) ----
 static bool sliced_ok(const ising_t *h)
 {
-    if (!h || h->nslabs || h->g.nsamples != 1 || !h->g.fast) return false;
+    if (!h || h->nslabs || h->g.nsamples != 1 || !h->g.fast || h->g.L > MAX_L_32BIT_GROUPS) return false;
     if (h->rng_mode != ISING_RNG_PHILOX && h->rng_mode != ISING_RNG_MINSTD) return false;
     const int wpr = h->g.L >> 5;                     // words per sliced row; lanes per row must be a power of two
     return (wpr & (wpr - 1)) == 0;
@@ -2061,7 +2103,7 @@ int ising_hostcheck_update_word(int rng_mode, uint64_t seed, uint64_t t, double 
     if (rng_mode == ISING_RNG_PHILOX) {
         PhiloxCommonConst pc;
         PhiloxSampleConst ps;
-        fold_philox(seed, 0, t, &pc, &ps);
+        fold_philox(seed, 0, t, &pc, &ps, (uint32_t)((8 * word_index) >> 32));   // counter word c3 = hi32(g), g = 8 x word index + q (R9)
         cond_masks_site_packed_philox(pc, ps, (uint32_t)word_index, kt, c4, c8, c12);
     } else {
         cond_masks_site_packed_minstd(seed + (site0 + 1) * SPLITMIX_GAMMA, site_stride * SPLITMIX_GAMMA,

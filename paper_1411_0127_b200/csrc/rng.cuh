@@ -18,8 +18,8 @@ namespace isingk {
 // Philox4x32-10 (Salmon et al., SC'11; R10).  Round r = 0..9 with round key
 // (K0_r, K1_r) = (k0 + r*W0, k1 + r*W1):
 //     (hi0:lo0) = M0*c0,  (hi1:lo1) = M1*c2,   (c0,c1,c2,c3) <- (hi1^c1^K0_r, lo1, hi0^c3^K1_r, lo0)
-// Keying (R9): key = (lo32 seed, hi32 seed ^ sample); counter = (lo32 t, hi32 t, g, 0) with g = j>>2 the
-// colour rank of the site divided by 4 (g < 2^32 for every supported L); output word j&3 is site j's draw.
+// Keying (R9): key = (lo32 seed, hi32 seed ^ sample); counter = (lo32 t, hi32 t, lo32 g, hi32 g) with g = j>>2 the
+// colour rank of the site divided by 4 (g = N/8 at most: below 2^32 up to L = 3250, below 2^33 up to L = 4096); output word j&3 is site j's draw.
 // ---------------------------------------------------------------------------------------------------
 constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
 constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
@@ -61,12 +61,14 @@ struct PhiloxCommonConst {
     uint32_t k0[7];  // K0_3 .. K0_9
 };
 
-ISING_HD void fold_philox(uint64_t seed, uint32_t sample, uint64_t t, PhiloxCommonConst *cc, PhiloxSampleConst *sc)
+// c3 = hi32(g): 0 for every group index below 2^32 (every lattice up to L = 3250); L = 4096 has g < 2^33 and folds a
+// second set for c3 = 1, which differs in b and e only (c3 enters round 0 through A2, and A2 only through B).
+ISING_HD void fold_philox(uint64_t seed, uint32_t sample, uint64_t t, PhiloxCommonConst *cc, PhiloxSampleConst *sc, uint32_t c3 = 0u)
 {
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32) ^ sample;
     const uint32_t tlo = (uint32_t)t, thi = (uint32_t)(t >> 32);
     const uint64_t P0 = (uint64_t)PHILOX_M0 * tlo;
-    const uint32_t A2 = (uint32_t)(P0 >> 32) ^ k1;  // c3 = hi32(g) = 0
+    const uint32_t A2 = (uint32_t)(P0 >> 32) ^ c3 ^ k1;
     const uint32_t A3 = (uint32_t)P0;
     const uint64_t B = (uint64_t)PHILOX_M1 * A2;
     cc->a = thi ^ k0;

@@ -26,12 +26,12 @@
 namespace isingk {
 
 // grid = (L / (32 / tpr_pad), number of CTA rows of this launch); the CTA row is a.by_first + blockIdx.y * a.by_stride.
-template <int RNG, int W>
+template <int RNG, int W, bool BIG = false>
 __global__ void __launch_bounds__(SWEEP_THREADS)
 half_sweep_site_packed_slab(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng)
 {
     unsigned long long unused0 = 0, unused1 = 0;
-    site_packed_tile<RNG, W, false, false, true>(a, rng, blockIdx.x, (uint32_t)a.by_first + blockIdx.y * (uint32_t)a.by_stride, gridDim.x,
+    site_packed_tile<RNG, W, false, false, true, BIG>(a, rng, blockIdx.x, (uint32_t)a.by_first + blockIdx.y * (uint32_t)a.by_stride, gridDim.x,
                                                  unused0, unused1);
 }
 
@@ -48,13 +48,13 @@ struct SlabPush {
     int Lz;
 };
 
-template <int RNG, int W>
+template <int RNG, int W, bool BIG = false>
 __global__ void __launch_bounds__(SWEEP_THREADS)
 half_sweep_site_packed_slab_push(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, const SlabPush p)
 {
     unsigned long long unused0 = 0, unused1 = 0;
     const uint32_t by = (uint32_t)a.by_first + blockIdx.y * (uint32_t)a.by_stride;
-    site_packed_tile<RNG, W, false, false, true>(a, rng, blockIdx.x, by, gridDim.x, unused0, unused1);
+    site_packed_tile<RNG, W, false, false, true, BIG>(a, rng, blockIdx.x, by, gridDim.x, unused0, unused1);
     const RowMap rm = row_map<W>(a.L, blockIdx.x, by);
     const int zl = rm.z + 1;   // plane in the slab's arrays (plane 0 is the lower halo)
     if (rm.active && (zl == 1 || zl == p.Lz)) {

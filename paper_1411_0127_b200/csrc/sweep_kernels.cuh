@@ -225,6 +225,7 @@ struct SiteRng {  // per-launch PRNG constants of the site-packed kernel (one sa
     uint64_t seed;  // MINSTD
     uint32_t A2;    // MINSTD: 2 * (16807^(n+1) mod M) for the sweep n = t>>1 of this launch
     uint4 *s0tab;   // MINSTD with cached seeds (RNG = 2): seed states s0 of the active colour, see minstd_s0_index
+    uint32_t b_hi, e_hi;   // Philox, lattices beyond L = 2048 (BIG): ps.b, ps.e for the groups g >= 2^32 (counter word c3 = 1, R9)
 };
 
 // Cached MINSTD seed states (RNG = 2).  s0 = (SplitMix64(seed, site) >> 34) + 1 (R11) does not depend on time, so it
@@ -311,7 +312,10 @@ __device__ __forceinline__ RowMap row_map(int L, uint32_t bx, uint32_t by)
 // SLAB: the arrays are those of a z-slab (see SweepArgs): the tile's planes are stored one plane up (the lower halo is plane 0),
 // their z-neighbours are simply the planes below and above (halos at the ends, no wrap), and everything keyed by the site -- the
 // colour of a row, the Philox counter, the MINSTD stream ids -- uses the plane's z in the whole lattice.
-template <int RNG, int W, bool MEASURE, bool COHERENT, bool SLAB = false>
+// BIG: lattices beyond L = 2048, whose Philox group index g = 8 x (word index) + q reaches 2^32: the words from index 2^29 on
+// take the constants folded for the counter word c3 = hi32(g) = 1 (R9; fold_philox).  Nothing else changes: the word index itself
+// stays below 2^30 up to L = 4096, and the MINSTD stream ids are 64-bit anyway.
+template <int RNG, int W, bool MEASURE, bool COHERENT, bool SLAB = false, bool BIG = false>
 __device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteRng &rng, uint32_t bx, uint32_t by, uint32_t gx,
                                                  unsigned long long &m_unsat, unsigned long long &m_up_out)
 {
@@ -411,7 +415,15 @@ __device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteR
     for (int k = WC; k < W; ++k) {
         uint32_t c4, c8, c12;
         if (RNG == 0) {
-            cond_masks_site_packed_philox(pcr, psr, row_g + (uint32_t)k, Tr, c4, c8, c12);
+            if (BIG) {
+                PhiloxSampleConst psw = psr;
+                const bool hi = ((row_g + (uint32_t)k) >> 29) != 0u;
+                psw.b = hi ? rng.b_hi : psr.b;
+                psw.e = hi ? rng.e_hi : psr.e;
+                cond_masks_site_packed_philox(pcr, psw, row_g + (uint32_t)k, Tr, c4, c8, c12);
+            } else {
+                cond_masks_site_packed_philox(pcr, psr, row_g + (uint32_t)k, Tr, c4, c8, c12);
+            }
         } else {
             const uint64_t site0 = row_site0 + 64ull * (uint64_t)(k0 + k);
             cond_masks_site_packed_minstd(rng.seed + (site0 + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, rng.A2, a.T, c4, c8, c12);
@@ -456,13 +468,13 @@ __device__ __forceinline__ void site_packed_tile(const SweepArgs &a, const SiteR
     }
 }
 
-template <int RNG, int W, bool MEASURE>
+template <int RNG, int W, bool MEASURE, bool BIG = false>
 __global__ void __launch_bounds__(SWEEP_THREADS, RNG == 0 && W == 4 && !MEASURE ? 4 : 0)
 half_sweep_site_packed(const __grid_constant__ SweepArgs a, const __grid_constant__ SiteRng rng, unsigned long long *acc, long long N,
                        long long *E, long long *M)
 {
     unsigned long long unsat = 0, up = 0;
-    site_packed_tile<RNG, W, MEASURE, false>(a, rng, blockIdx.x, blockIdx.y, gridDim.x, unsat, up);
+    site_packed_tile<RNG, W, MEASURE, false, false, BIG>(a, rng, blockIdx.x, blockIdx.y, gridDim.x, unsat, up);
     if (MEASURE) add_to_record(unsat, up, E, M);
 }
 

@@ -75,7 +75,7 @@ def test_fnv1a64_host():
 def test_argument_validation_without_a_gpu():
     lib = binding.lib()
     out = C.c_size_t(0)
-    for L, ns in ((3, 1), (2, 1), (0, 1), (-4, 1), (4096, 1), (16, 2), (16, 0), (16, 48)):
+    for L, ns in ((3, 1), (2, 1), (0, 1), (-4, 1), (8192, 1), (4098, 1), (2050, 1), (2112, 1), (4096, 32), (16, 2), (16, 0), (16, 48)):
         assert lib.ising_workspace_bytes(L, ns, 0, C.byref(out)) == binding.EINVAL, (L, ns)
     assert lib.ising_workspace_bytes(16, 1, 7, C.byref(out)) == binding.EINVAL
     assert lib.ising_workspace_bytes(16, 1, 2, C.byref(out)) == binding.EINVAL   # shared draws need 32-sample words
@@ -104,6 +104,10 @@ def test_argument_validation_without_a_gpu():
             assert table >= 4 * N * ns and (table == 4 * N * ns) == (odd in (1, 3, 5))
         assert binding.ising_workspace_bytes(L, ns, 1) == nbytes + table
     assert binding.ising_workspace_bytes(1024, 1, 0) < 1100 * 2**20
+    # beyond 2^32 Philox groups (L > 2048): one sample, rows of 1, 3, 5 x 2^e words; no MINSTD seed table there
+    for L in (2560, 3072, 4096):
+        nbytes = binding.ising_workspace_bytes(L, 1, 0)
+        assert 8 * L**3 // 8 <= nbytes < 8 * L**3 // 8 + 2**20 and binding.ising_workspace_bytes(L, 1, 1) == nbytes
     h = C.c_void_p()
     assert lib.ising_create(16, 1, 1, 0, None, 1 << 20, C.byref(h)) == binding.EINVAL
     assert lib.ising_create(16, 1, 1, 0, C.c_void_p(256), 16, C.byref(h)) == binding.EINVAL      # too small
@@ -224,3 +228,38 @@ def test_host_word_update_all_bond_patterns_and_draw_levels():
             R = ea3d.philox4x32_10((t, 0, j >> 2, 0), (seed, 0))[j & 3]
             flip = dE <= 0 or R < T[dE // 4 - 1]
             assert ((got >> b) & 1) == (((ops[0] >> b) & 1) ^ int(flip)), (word_index, b, dE, R)
+
+
+def test_host_word_update_with_a_group_index_beyond_2_to_32():
+    """L = 4096 has Philox group indices g = j >> 2 of 2^32 and more, whose high word is the counter word c3 (R9); the other sizes
+    beyond 2048 (2560, 3072) stay below.  The kernels' word update (folded constants for c3 = 0 and c3 = 1) against 'flip iff
+    dE <= 0 or R < T[dE]' with R from the oracle's draw of the site at its coordinates, for words on both sides of g = 2^32, the
+    two words next to it, and the last word of the array."""
+    seed, beta = 0xABCDEF0123456789, 0.05
+    T = ea3d.thresholds(beta, 0)
+    rng = np.random.default_rng(5)
+    for L in (4096, 3072, 2560):
+        wpr = L // 64
+        n_words = wpr * L * L                      # words of one colour array
+        assert (n_words > 2**29) == (L == 4096) and n_words <= 2**30
+        picks = [n_words - 1, 0] + [int(v) for v in rng.integers(0, n_words, 5)]
+        if L == 4096:
+            picks += [2**29 - 1, 2**29, 2**29 + 1]
+        for word_index in picks:
+            t = int(rng.integers(0, 2**34))
+            colour = t & 1
+            k, row = word_index % wpr, word_index // wpr
+            y, z = row % L, row // L
+            xodd = (y + z + colour) & 1
+            ops = [int(v) for v in rng.integers(0, 2**32, 13, dtype=np.uint64)]
+            got = binding.ising_hostcheck_update_word(0, seed, t, beta, ops, word_index)
+            for b in range(32):
+                s = 2 * ((ops[0] >> b) & 1) - 1
+                h = sum((1 - 2 * ((ops[7 + d] >> b) & 1)) * (2 * ((ops[1 + d] >> b) & 1) - 1) for d in range(6))
+                dE = 2 * s * h
+                x = 2 * (32 * k + b) + xodd       # bit b of word k of the half-row
+                j = (x >> 1) + (L // 2) * (y + L * z)
+                assert j == 32 * word_index + b and (j >> 2 >= 2**32) == (word_index >= 2**29)
+                R = ea3d.philox_draw(L, seed, 0, x, y, z, t)
+                flip = dE <= 0 or R < T[dE // 4 - 1]
+                assert ((got >> b) & 1) == (((ops[0] >> b) & 1) ^ int(flip)), (L, word_index, b, dE, R)

@@ -463,7 +463,7 @@ def test_no_kernel_writes_outside_the_workspace(L, nsamples, rng_mode, kernel):
 
 @pytest.mark.parametrize("rng_mode,kernel", [(PHILOX, 0), (MINSTD, 2)])
 def test_maximum_size_L2048_word_parallel_equals_generic(rng_mode, kernel):
-    """L = 2048 is the largest lattice the library accepts (Philox group index < 2^32): 2^33 spins, 1 GiB of spin bits.
+    """L = 2048 is the largest lattice every layout and mode accepts (tests/test_gpu_large.py goes beyond): 2^33 spins, 1 GiB of spin bits.
     The oracle cannot hold it (34 GB of int8 per array); the word-parallel kernel is compared with the generic
     one-site-at-a-time kernel over one sweep, and the energy bookkeeping with the spin count."""
     L = 2048
