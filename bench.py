@@ -44,9 +44,9 @@ LANE_STATE_BYTES_PER_DRAW = {3: 16.0, 4: 13.0}
 # belongs to the kernel sources it was captured on: `kernel_sources_sha256` is kernel_sources_hash() at capture time, and
 # the bench line prints `traffic` only while the sources still hash to it (null otherwise, with a note).
 NCU_TRAFFIC_L1024 = {
-    "kernel_sources_sha256": "200688f003616987ca7ca7b8dd9fe1dc69f411033281600f6c08fe7dd27d663b",
+    "kernel_sources_sha256": "d4d8c25eb7ad193dfa890c5abb33e3977afe6a37b478e91ca40ae419a7ead5eb",
     "capture": "profiles/r2n_end_of_round.md",
-    0: 537.05e6 + 58.26e6, 1: 2684.52e6 + 60.48e6,
+    0: 537.05e6 + 59.28e6, 1: 2684.53e6 + 61.07e6,
 }
 
 

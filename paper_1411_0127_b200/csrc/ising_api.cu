@@ -611,7 +611,7 @@ bool persistent_available(const ising_t *h, bool records)
     if (h->g.onchip) {
         if (h->kernel_choice == 4) return true;
         if (h->kernel_choice != 0 && h->kernel_choice != 2) return false;
-        // automatic: where one SM beats a launch per half-sweep on all of them (profiles/r2c_small.md): with records up to 512
+        // automatic: where one SM beats a launch per half-sweep on all of them (profiles/r2n_small.md): with records up to 512
         // words per colour (L <= 32: 3.8-5.5 against 10.8-12.3 us per recorded half-sweep), without up to 216 (L <= 24)
         const uint64_t nw = (h->g.Hc + 31) / 32;
         return records ? nw <= 512 : nw <= 216;
@@ -801,10 +801,16 @@ int cluster_size_of(ising_t *h)
         cudaGetLastError();
         return 0;
     }
-    int C = 16;
-    while (C > 1 && (long long)g.nsamples * C > sms) C >>= 1;
-    while (C <= 16 && cluster_shape(h, C).smem > (size_t)smem_max) C <<= 1;
-    for (; C <= 16; C <<= 1) {   // the first size the device accepts
+    int pref = 16;
+    while (pref > 1 && (long long)g.nsamples * pref > sms) pref >>= 1;
+    while (pref <= 16 && cluster_shape(h, pref).smem > (size_t)smem_max) pref <<= 1;
+    // the preferred size, then smaller ones (a device that cannot co-schedule 16 CTAs), then larger ones: the first the device accepts
+    int order[10], n = 0;
+    for (int c = pref; c >= 1; c >>= 1) order[n++] = c;
+    for (int c = 2 * pref; c <= 16; c <<= 1) order[n++] = c;
+    for (int k = 0; k < n; ++k) {
+        const int C = order[k];
+        if (C > 16) continue;
         const ClusterShape cs = cluster_shape(h, C);
         if (cs.smem > (size_t)smem_max) continue;
         bool ok = true;
@@ -836,7 +842,7 @@ int cluster_size_of(ising_t *h)
     return 0;
 }
 
-// Which calls run there.  Automatic (kernel choice 0 / 2): where it was measured faster than the launches (profiles/r2m_cluster.md):
+// Which calls run there.  Automatic (kernel choice 0 / 2): where it was measured faster than the launches (profiles/r2n_small.md):
 // L = 64 with Philox up to 128 samples (one sample: 1.2 against 2.2 us per half-sweep; 32 samples: 3.7 against 5.2; 256 samples: the
 // launches fill the GPU as well), with MINSTD one sample only (the batch launches read cached seed states, this kernel recomputes
 // them).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay with the launches (the slab is

@@ -1,6 +1,6 @@
 """Synchronisation-latency probe (csrc/sync_probe.cu): grid-wide barriers, neighbour flags and a cluster barrier on the GPU it runs on.
 `python -m paper_1411_0127_b200.sync_probe` builds the standalone program next to the library and prints its table
-(profiles/r2b_persistent.md)."""
+(profiles/r2j_launch_floor.md)."""
 from __future__ import annotations
 
 import os
