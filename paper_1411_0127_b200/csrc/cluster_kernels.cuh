@@ -60,6 +60,13 @@ __device__ __forceinline__ uint32_t cluster_load(uint32_t addr)
     asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
     return v;
 }
+template <int BYTE_OFFSET>   // the same with a compile-time offset in the instruction
+__device__ __forceinline__ uint32_t cluster_load_at(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared::cluster.u32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(BYTE_OFFSET) : "memory");
+    return v;
+}
 
 // What the update of one word needs to know about its place and does not change from one half-sweep to the next.
 struct WordPlace {
@@ -120,20 +127,23 @@ __device__ __noinline__ void cluster_energy_pass(const uint32_t *sm, uint32_t nw
 
 // RNG 0 = Philox, 1 = MINSTD (stateless, R11 / R12).  WPR = words per half-row = L / 64.  Cluster of C = gridDim.x / samples CTAs
 // (cluster dimension attribute of the launch); blockDim.x = min(1024, words per colour and CTA), a thread owns the words
-// tid, tid + blockDim.x, ... of its CTA's slab.  SINGLE: exactly one word per thread (blockDim.x = words per colour and CTA), whose
-// place is then computed once, before the first half-sweep.  Dynamic shared memory: 8 arrays of L^2 WPR (L / C) words in the order
-// S[0], S[1], Jx[0], Jx[1], Jy[0], Jy[1], Jz[0], Jz[1].
-template <int RNG, int WPR, bool RECORDS, bool SINGLE>
-__global__ void __launch_bounds__(CLUSTER_MAX_THREADS, 1)
+// tid, tid + blockDim.x, ... of its CTA's slab.  NW > 0: exactly one word per thread and NW = blockDim.x = words per colour and CTA
+// known at compile time (L = 64 in clusters of 16, 8, 4 CTAs: 256, 512, 1024): the thread's place is computed once, before the
+// first half-sweep, and the twelve operand loads of a half-sweep are four base addresses plus offsets in the instructions (a
+// twelfth of the update's instructions were address arithmetic otherwise).  NW = 0: any slab size, several words per thread.
+// Dynamic shared memory: 8 arrays of L^2 WPR (L / C) words in the order S[0], S[1], Jx[0], Jx[1], Jy[0], Jy[1], Jz[0], Jz[1].
+template <int RNG, int WPR, bool RECORDS, int NW>
+__global__ void __launch_bounds__(NW > 0 ? NW : CLUSTER_MAX_THREADS, 1)
 half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
 {
     extern __shared__ uint32_t sm[];
+    constexpr bool SINGLE = NW > 0;
     cg::cluster_group cluster = cg::this_cluster();
     const uint32_t C = cluster.num_blocks(), r = cluster.block_rank();
     const uint32_t sample = p.sample0 + blockIdx.x / C;
     const uint32_t L = (uint32_t)p.L, Lz = L / C;
     const uint32_t plane = L * WPR;              // words of one plane of one array
-    const uint32_t nw = plane * Lz;              // words of one array in this CTA
+    const uint32_t nw = SINGLE ? (uint32_t)NW : plane * Lz;   // words of one array in this CTA
     const uint32_t z0 = r * Lz;
 
     // ---- load the slab -------------------------------------------------------------------------------------------------
@@ -205,20 +215,25 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
                 masks(w, c, c4, c8, c12);
             }
             const uint32_t xodd = w.xodd0 ^ (uint32_t)c;
-            uint32_t s = sm[act + w.wl];
-            const uint32_t o = sm[oth + w.wl];
-            const uint32_t jxo = sm[2 * nw + oth + w.wl], jxa = sm[2 * nw + act + w.wl];
-            const uint32_t oyp = sm[oth + w.w_yp], oym = sm[oth + w.w_ym];
-            const uint32_t ozp = cluster_load(w.zp_addr + 4u * oth), ozm = cluster_load(w.zm_addr + 4u * oth);
-            const uint32_t jya = sm[4 * nw + act + w.wl], jza = sm[6 * nw + act + w.wl];
-            const uint32_t jyo = sm[4 * nw + oth + w.w_ym], jzo = cluster_load(w.zm_addr + 4u * (6 * nw + oth));
+            // four bases in this CTA's arrays, two in the window of the cluster; everything else is a fixed distance away
+            uint32_t *const pa = sm + act + w.wl;
+            const uint32_t *const po = sm + oth + w.wl, *const pyp = sm + oth + w.w_yp, *const pym = sm + oth + w.w_ym;
+            const uint32_t zp = w.zp_addr + 4u * oth, zm = w.zm_addr + 4u * oth;
+            uint32_t s = pa[0];
+            const uint32_t o = po[0];
+            const uint32_t jxo = po[2 * nw], jxa = pa[2 * nw];
+            const uint32_t oyp = pyp[0], oym = pym[0];
+            const uint32_t ozp = cluster_load(zp), ozm = cluster_load(zm);
+            const uint32_t jya = pa[4 * nw], jza = pa[6 * nw];
+            const uint32_t jyo = pym[4 * nw], jzo = SINGLE ? cluster_load_at<24 * NW>(zm) : cluster_load(zm + 24u * nw);
             // x neighbours (row a3; see site_packed_tile): the bit that crosses the word boundary comes from the row's next /
             // previous word (periodic), which for WPR = 1 is the word itself
             const uint32_t B = jxo ^ o;
             uint32_t o_next = o, B_prev = B;
             if (WPR > 1) {
+                const uint32_t *const pp = sm + oth + w.w_prev;
                 o_next = sm[oth + w.w_next];
-                B_prev = sm[2 * nw + oth + w.w_prev] ^ sm[oth + w.w_prev];
+                B_prev = pp[2 * nw] ^ pp[0];
             }
             const uint32_t J[6] = {jxa, 0u, jya, jyo, jza, jzo};
             const uint32_t nb[6] = {__funnelshift_r(o, o_next, xodd), __funnelshift_l(B_prev, B, 1u - xodd), oyp, oym, ozp, ozm};
@@ -226,7 +241,7 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
             satisfied_bond_count(s, J, nb, sum2, sum1, sum0);
             const uint32_t f = flip_mask(sum2, sum1, sum0, c4, c8, c12);
             s ^= f;
-            sm[act + w.wl] = s;
+            pa[0] = s;
             if (SINGLE) break;
         }
         cluster_arrive();

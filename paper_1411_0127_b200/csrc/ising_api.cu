@@ -758,21 +758,24 @@ int sweep_persistent(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t e
 // half-sweeps of the call in one launch.  L = 64 and 128, one sample or a batch of lattices, Philox or MINSTD.
 // ---------------------------------------------------------------------------------------------------------------------
 template <int RNG, int WPR>
-auto cluster_kernel(bool records, bool single)
+auto cluster_kernel(bool records, int nw_fixed)
 {
-    if (single) return records ? half_sweeps_cluster<RNG, WPR, true, true> : half_sweeps_cluster<RNG, WPR, false, true>;
-    return records ? half_sweeps_cluster<RNG, WPR, true, false> : half_sweeps_cluster<RNG, WPR, false, false>;
+    // one word per thread with the slab size known at compile time (L = 64 in clusters of 16, 8, 4 CTAs), or the general kernel
+    if (WPR == 1 && nw_fixed == 256) return records ? half_sweeps_cluster<RNG, 1, true, 256> : half_sweeps_cluster<RNG, 1, false, 256>;
+    if (WPR == 1 && nw_fixed == 512) return records ? half_sweeps_cluster<RNG, 1, true, 512> : half_sweeps_cluster<RNG, 1, false, 512>;
+    if (WPR == 1 && nw_fixed == 1024) return records ? half_sweeps_cluster<RNG, 1, true, 1024> : half_sweeps_cluster<RNG, 1, false, 1024>;
+    return records ? half_sweeps_cluster<RNG, WPR, true, 0> : half_sweeps_cluster<RNG, WPR, false, 0>;
 }
 
-// single: one word per thread (the slab of a CTA has at most 1024 words per array)
-void (*cluster_kernel_of(const ising_t *h, bool records, bool single))(const ClusterArgs)
+// nw_fixed: words per colour and CTA when every thread has exactly one of them (0: several words per thread)
+void (*cluster_kernel_of(const ising_t *h, bool records, int nw_fixed))(const ClusterArgs)
 {
     const bool philox = h->rng_mode == ISING_RNG_PHILOX;
-    if (h->g.L == 64) return philox ? cluster_kernel<0, 1>(records, single) : cluster_kernel<1, 1>(records, single);
-    return philox ? cluster_kernel<0, 2>(records, single) : cluster_kernel<1, 2>(records, single);
+    if (h->g.L == 64) return philox ? cluster_kernel<0, 1>(records, nw_fixed) : cluster_kernel<1, 1>(records, nw_fixed);
+    return philox ? cluster_kernel<0, 2>(records, 0) : cluster_kernel<1, 2>(records, 0);
 }
 
-struct ClusterShape { int C, threads; size_t smem; bool single; };
+struct ClusterShape { int C, threads; size_t smem; int nw_fixed; };
 
 ClusterShape cluster_shape(const ising_t *h, int C)
 {
@@ -782,7 +785,7 @@ ClusterShape cluster_shape(const ising_t *h, int C)
     s.C = C;
     s.threads = nw < (size_t)CLUSTER_MAX_THREADS ? (int)nw : CLUSTER_MAX_THREADS;
     s.smem = 8 * nw * sizeof(uint32_t);
-    s.single = nw <= (size_t)CLUSTER_MAX_THREADS;
+    s.nw_fixed = nw <= (size_t)CLUSTER_MAX_THREADS ? (int)nw : 0;
     return s;
 }
 
@@ -815,7 +818,7 @@ int cluster_size_of(ising_t *h)
         if (cs.smem > (size_t)smem_max) continue;
         bool ok = true;
         for (int records = 0; records < 2 && ok; ++records) {
-            auto kernel = cluster_kernel_of(h, records != 0, cs.single);
+            auto kernel = cluster_kernel_of(h, records != 0, cs.nw_fixed);
             ok = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs.smem) == cudaSuccess &&
                  (C <= 8 || cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess);
             if (!ok) break;
@@ -847,17 +850,17 @@ int cluster_size_of(ising_t *h)
 // launches fill the GPU as well), with MINSTD one sample only (the batch launches read cached seed states, this kernel recomputes
 // them).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay with the launches (the slab is
 // loaded and stored once per call).
-// `every`: record spacing of the call in half-sweeps (0: no records).  A record costs this kernel 1.9 us (a pass over the slab and
-// a second, unhidden barrier) where a measuring launch costs 0.6 us more than a plain one: densely recorded calls stay with the
-// launches / graph replays when there is one sample (with 32 samples the launches are slower at any spacing: 6.1 against 5.8 us
-// per half-sweep with a record after each).
+// `every`: record spacing of the call in half-sweeps (0: no records).  A record costs this kernel 1.2-1.9 us (a pass over the slab and
+// a second, unhidden barrier) where a measuring launch costs 0.6 us more than a plain one.  With Philox it still wins at every
+// spacing (one sample, a record after every half-sweep: 2.3 against 2.8 us by graph replays; 32 samples: 5.8 against 6.1 by
+// launches); with MINSTD, whose seeds it recomputes, densely recorded one-sample calls stay with the graph replays (3.1 against 2.8).
 bool cluster_available(ising_t *h, uint32_t nhalf, uint32_t every)
 {
     if (h->kernel_choice == 1 || h->kernel_choice == 3 || h->no_cluster || nhalf < 8) return false;
     if (h->kernel_choice != 4) {
         if (h->g.L != 64) return false;
         if (h->rng_mode == ISING_RNG_PHILOX ? h->g.nsamples > 128 : h->g.nsamples != 1) return false;
-        if (every != 0 && h->g.nsamples == 1 && every < (h->rng_mode == ISING_RNG_PHILOX ? 4u : 16u)) return false;
+        if (every != 0 && h->g.nsamples == 1 && h->rng_mode == ISING_RNG_MINSTD && every < 16u) return false;
     }
     return cluster_size_of(h) > 0;
 }
@@ -896,7 +899,7 @@ int sweep_cluster(ising_t *h, const Thresholds &T, uint32_t nhalf, uint32_t ever
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (cudaLaunchKernelEx(&cfg, cluster_kernel_of(h, records, cs.single), p) != cudaSuccess) g_launch_failed = true;
+    if (cudaLaunchKernelEx(&cfg, cluster_kernel_of(h, records, cs.nw_fixed), p) != cudaSuccess) g_launch_failed = true;
     const int rc = check_launch(h);
     if (rc == ISING_OK) h->t += nhalf;
     return rc;
