@@ -15,9 +15,9 @@
 // happens until the call's last half-sweep.  Samples are independent (batch_kernels.cuh), so a grid is one cluster per sample and
 // clusters never talk to each other; C is chosen so that samples x C fills the 148 SMs (32 samples: C = 4; one sample: C = 16,
 // the non-portable maximum).
-//   Records (ising_sweep_trace): after a recording half-sweep every CTA counts the unsatisfied bonds and up spins of its slab in a
-// pass of its own (out of line, so that the update loop pays nothing for it) and adds them to the pre-set record (R16, as
-// add_to_record does) one arrive later; a second barrier keeps the next half-sweep from overwriting what the pass reads.
+//   Records (ising_sweep_trace): a recording half-sweep runs a second copy of the update that counts, as the measuring tile update
+// does, the satisfied bonds from the field sums it holds and the up spins of both colours, and adds the CTA's totals to the
+// pre-set record (R16, as add_to_record does) behind the arrive; the other half-sweeps run the plain copy.
 //   The bits are those of one launch per half-sweep: the draws are keyed by (sample, site, t), not by the thread mapping (R9, R11).
 #pragma once
 #include <cooperative_groups.h>
@@ -68,6 +68,9 @@ __device__ __forceinline__ uint32_t cluster_load_at(uint32_t addr)
     return v;
 }
 
+struct false_type_tag { static constexpr bool value = false; };
+struct true_type_tag { static constexpr bool value = true; };
+
 // What the update of one word needs to know about its place and does not change from one half-sweep to the next.
 struct WordPlace {
     uint32_t wl;                 // index of the word in the CTA's slab of each array
@@ -98,31 +101,6 @@ __device__ __forceinline__ WordPlace place_word(uint32_t wl, uint32_t L, uint32_
     w.wg = z0 * plane + wl;
     w.site_even = (uint64_t)L * ((uint64_t)y + (uint64_t)L * (z0 + zl)) + 64ull * k;
     return w;
-}
-
-// E and M of the configuration in shared memory, this CTA's share: unsatisfied +x, +y, +z bonds and up spins of the sites of its slab
-// (each bond once, R16), as energy_tile counts them.  Kept out of line: it runs for the recording half-sweeps only and must not
-// cost the update loop any registers.
-template <int WPR>
-__device__ __noinline__ void cluster_energy_pass(const uint32_t *sm, uint32_t nw, uint32_t L, uint32_t Lz, uint32_t z0, uint32_t a_self,
-                                                 uint32_t a_up, uint32_t a_dn, unsigned int *unsat_out, unsigned int *up_out)
-{
-    unsigned int unsat = 0, up = 0;
-    for (uint32_t wl = threadIdx.x; wl < nw; wl += blockDim.x) {
-        const WordPlace w = place_word<WPR>(wl, L, Lz, z0, a_self, a_up, a_dn);
-#pragma unroll
-        for (uint32_t c = 0; c < 2; ++c) {
-            const uint32_t act = c * nw, oth = nw - act;
-            const uint32_t s = sm[act + wl], o = sm[oth + wl];
-            const uint32_t o_next = WPR > 1 ? sm[oth + w.w_next] : o;
-            const uint32_t nx = __funnelshift_r(o, o_next, w.xodd0 ^ c);
-            const uint32_t oyp = sm[oth + w.w_yp], ozp = cluster_load(w.zp_addr + 4u * oth);
-            unsat += __popc(sm[2 * nw + act + wl] ^ s ^ nx) + __popc(sm[4 * nw + act + wl] ^ s ^ oyp) + __popc(sm[6 * nw + act + wl] ^ s ^ ozp);
-            up += __popc(s);
-        }
-    }
-    *unsat_out = unsat;
-    *up_out = up;
 }
 
 // RNG 0 = Philox, 1 = MINSTD (stateless, R11 / R12).  WPR = words per half-row = L / 64.  Cluster of C = gridDim.x / samples CTAs
@@ -184,30 +162,19 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
     cluster_arrive();
     cluster_wait();
 
-    // The record of a run is added to global memory one arrive later: the release of an arrive waits for the thread's outstanding
-    // global operations, so an atomic issued just before it would put an L2 round trip (1-2 us) on every record's critical path;
-    // issued just after an arrive it completes under the next half-sweep's draws.
+    // One half-sweep kk of the launch.  MEAS (the last half-sweep of a run that ends at a record): the thread also counts, as the
+    // measuring tile update of sweep_kernels.cuh does, the satisfied bonds of the configuration it leaves -- every bond has exactly
+    // one end in the active colour, so they are the sum over the active sites of the count n in the three bit planes, with
+    // n -> 6 - n where the site flipped -- and the up spins of its word of either colour; after the arrive the CTA's totals go to
+    // the record (R16, pre-set by init_records) by one atomic pair, which completes under the draws of the next half-sweep.  The
+    // plain copy of the body is the same code as in the kernel without records.
     __shared__ unsigned long long rec_sum[2];
-    bool rec_pending = false;
-    auto flush_record = [&]() {
-        if (RECORDS && rec_pending) {
-            if (threadIdx.x == 0) {
-                if (p.E) atomicAdd(reinterpret_cast<unsigned long long *>(p.E + (size_t)rec * p.nsamples + sample), 2ull * rec_sum[0]);   // R16
-                if (p.M) atomicAdd(reinterpret_cast<unsigned long long *>(p.M + (size_t)rec * p.nsamples + sample), 2ull * rec_sum[1]);
-            }
-            ++rec;
-            rec_pending = false;
-        }
-    };
-    // Half-sweeps in runs that end at a record (RECORDS) or at the end of the call: the loop over a run is the same code with and
-    // without records.
-    const uint32_t run = RECORDS && p.every != 0 ? p.every : p.nhalf;
-    for (uint32_t k0 = 0; k0 < p.nhalf; k0 += run) {
-    const uint32_t k1 = k0 + run < p.nhalf ? k0 + run : p.nhalf;
-    for (uint32_t kk = k0; kk < k1; ++kk) {
+    auto half_sweep = [&](uint32_t kk, auto meas) {
+        constexpr bool MEAS = decltype(meas)::value;
         const uint64_t t = p.t0 + kk;
         const int c = (int)(t & 1);
         const uint32_t act = (uint32_t)c * nw, oth = nw - act;   // offsets of the active / other colour within a pair of arrays
+        unsigned int m_sat = 0, m_up = 0, m_words = 0;
         for (uint32_t wl = threadIdx.x; wl < nw; wl += blockDim.x) {
             WordPlace w = first;
             if (!SINGLE && wl != threadIdx.x) {   // later words of the thread: place and masks now
@@ -242,29 +209,41 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
             const uint32_t f = flip_mask(sum2, sum1, sum0, c4, c8, c12);
             s ^= f;
             pa[0] = s;
+            if (MEAS) {
+                m_sat += __popc(sum0) + 2 * __popc(sum1) + 4 * __popc(sum2) + 6 * __popc(f);
+                m_sat -= 2 * (__popc(sum0 & f) + 2 * __popc(sum1 & f) + 4 * __popc(sum2 & f));
+                m_up += __popc(s) + __popc(o);
+                ++m_words;
+            }
             if (SINGLE) break;
         }
         cluster_arrive();
-        if (RECORDS) flush_record();
+        if (MEAS) {
+            if (threadIdx.x == 0) { rec_sum[0] = 0; rec_sum[1] = 0; }
+            __syncthreads();
+            block_accumulate2(192ull * m_words - m_sat, m_up, rec_sum);   // (a CTA barrier inside; warp 0 adds the totals)
+            if (threadIdx.x == 0) {
+                if (p.E) atomicAdd(reinterpret_cast<unsigned long long *>(p.E + (size_t)rec * p.nsamples + sample), 2ull * rec_sum[0]);
+                if (p.M) atomicAdd(reinterpret_cast<unsigned long long *>(p.M + (size_t)rec * p.nsamples + sample), 2ull * rec_sum[1]);
+            }
+            ++rec;
+        }
         if (RNG != 0 && c == 1) A = minstd_mulmod(16807u, A);   // the next half-sweep belongs to the next sweep
         if (kk + 1 < p.nhalf) {   // the draws of the thread's first word for the next half-sweep, under the barrier
             if (RNG == 0) fold_philox_time(p.seed, sample, t + 1, &pc, &ps);
             masks(first, 1 - c, c4, c8, c12);
         }
         cluster_wait();
+    };
+    // Half-sweeps in runs that end at a record (RECORDS) or at the end of the call
+    const uint32_t run = RECORDS && p.every != 0 ? p.every : p.nhalf;
+    for (uint32_t k0 = 0; k0 < p.nhalf; k0 += run) {
+        const uint32_t k1 = k0 + run < p.nhalf ? k0 + run : p.nhalf;
+        const bool record = RECORDS && k1 == k0 + run;
+        const uint32_t k_plain = record ? k1 - 1 : k1;
+        for (uint32_t kk = k0; kk < k_plain; ++kk) half_sweep(kk, false_type_tag());
+        if (record) half_sweep(k1 - 1, true_type_tag());
     }
-    if (RECORDS && k1 == k0 + run) {   // a pass of its own over the slab, and a barrier before the next half-sweep overwrites what it reads
-        unsigned int unsat, up;
-        cluster_energy_pass<WPR>(sm, nw, L, Lz, z0, a_self, a_up, a_dn, &unsat, &up);
-        if (threadIdx.x == 0) { rec_sum[0] = 0; rec_sum[1] = 0; }
-        __syncthreads();
-        block_accumulate2(unsat, up, rec_sum);   // the CTA's totals; they go to the record after the next arrive (below)
-        rec_pending = true;
-        cluster_arrive();
-        cluster_wait();
-    }
-    }
-    flush_record();
 
     // ---- store the spins (every remote read of this slab is complete: its reader has passed the last barrier) -----------
     {

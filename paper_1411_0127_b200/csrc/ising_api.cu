@@ -850,17 +850,16 @@ int cluster_size_of(ising_t *h)
 // launches fill the GPU as well), with MINSTD one sample only (the batch launches read cached seed states, this kernel recomputes
 // them).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay with the launches (the slab is
 // loaded and stored once per call).
-// `every`: record spacing of the call in half-sweeps (0: no records).  A record costs this kernel 1.2-1.9 us (a pass over the slab and
-// a second, unhidden barrier) where a measuring launch costs 0.6 us more than a plain one.  With Philox it still wins at every
-// spacing (one sample, a record after every half-sweep: 2.3 against 2.8 us by graph replays; 32 samples: 5.8 against 6.1 by
-// launches); with MINSTD, whose seeds it recomputes, densely recorded one-sample calls stay with the graph replays (3.1 against 2.8).
+// `every`: record spacing of the call in half-sweeps (0: no records).  A recording half-sweep runs the measuring copy of the update
+// and costs 0.6 us more than a plain one, so the kernel wins at every spacing (one sample, a record after EVERY half-sweep: 1.75
+// against 2.8 us by graph replays with Philox, 2.5 against 2.8 with MINSTD; 32 samples: 3.7 against 5.3 us by launches).
 bool cluster_available(ising_t *h, uint32_t nhalf, uint32_t every)
 {
+    (void)every;
     if (h->kernel_choice == 1 || h->kernel_choice == 3 || h->no_cluster || nhalf < 8) return false;
     if (h->kernel_choice != 4) {
         if (h->g.L != 64) return false;
         if (h->rng_mode == ISING_RNG_PHILOX ? h->g.nsamples > 128 : h->g.nsamples != 1) return false;
-        if (every != 0 && h->g.nsamples == 1 && h->rng_mode == ISING_RNG_MINSTD && every < 16u) return false;
     }
     return cluster_size_of(h) > 0;
 }
