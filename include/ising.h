@@ -183,6 +183,15 @@ int ising_thresholds(double beta, int rng_mode, uint64_t out[3]);
  * checksum of BASELINE.json config 4 over the canonical packed spin words (little-endian bytes). */
 uint64_t ising_fnv1a64_host(const void *h_data, size_t nbytes);
 
+/* The same checksum of `nbytes` bytes of DEVICE memory (4-byte aligned), computed on the device in parallel and written to *d_out
+ * (device, one uint64), asynchronously on `stream`: the value is the one the byte-by-byte definition gives, bit for bit.  (The XOR of
+ * FNV-1a touches the low byte only, h ^ b = h + d with d from the low byte, and the low byte follows an 8-bit recurrence of its own;
+ * so the hash of a chunk is h_start P^n + sum_i d_i P^(n-i), and chunks are processed in parallel once the low byte at each
+ * chunk's start is known: csrc/fnv_kernels.cuh.  16 MiB take 0.2 ms instead of 17 ms on a host core.)  d_scratch: device memory of
+ * ising_fnv1a64_scratch_bytes(nbytes) bytes (7.6 MB at most), 8-byte aligned, owned by the caller, overwritten. */
+int ising_fnv1a64_scratch_bytes(size_t nbytes, size_t *out);
+int ising_fnv1a64(const void *d_data, size_t nbytes, void *d_scratch, size_t scratch_bytes, uint64_t *d_out, void *stream);
+
 /* Half-sweep counter t of the handle (get / set): with ising_get_spins + ising_load_state this makes a run
  * resumable bit-exactly, because no PRNG state exists outside (seed, t). */
 int ising_get_t(const ising_t *h, uint64_t *t);

@@ -19,7 +19,7 @@ STATIC_MAX_L = 128  # ising_energy_static
 
 EXPORTS = (
     "ising_workspace_bytes", "ising_create", "ising_create_layout", "ising_load_state", "ising_sweep", "ising_sweep_trace", "ising_energy",
-    "ising_get_spins", "ising_run_host", "ising_run_host_async", "ising_thresholds", "ising_fnv1a64_host", "ising_get_t", "ising_set_t",
+    "ising_get_spins", "ising_run_host", "ising_run_host_async", "ising_thresholds", "ising_fnv1a64_host", "ising_fnv1a64_scratch_bytes", "ising_fnv1a64", "ising_get_t", "ising_set_t",
     "ising_set_kernel", "ising_kernel_launches", "ising_hostcheck_update_word", "ising_destroy", "ising_strerror",
     "ising_overlap", "ising_get_lanes", "ising_set_lanes", "ising_resume_lanes", "ising_prng_state_bytes", "ising_prng_init", "ising_prng_count_odd",
     "ising_slab_workspace_bytes", "ising_create_slab", "ising_slab_half_sweep_boundary", "ising_slab_half_sweep_bulk", "ising_slab_plane",
@@ -55,6 +55,8 @@ def lib() -> C.CDLL:
     L.ising_thresholds.argtypes = [dbl, i32, C.POINTER(u64)]
     L.ising_fnv1a64_host.argtypes = [vp, sz]
     L.ising_fnv1a64_host.restype = u64
+    L.ising_fnv1a64_scratch_bytes.argtypes = [sz, C.POINTER(sz)]
+    L.ising_fnv1a64.argtypes = [vp, sz, vp, sz, vp, vp]
     L.ising_get_t.argtypes = [vp, C.POINTER(u64)]
     L.ising_set_t.argtypes = [vp, u64]
     L.ising_set_kernel.argtypes = [vp, i32]
@@ -97,6 +99,30 @@ def ising_workspace_bytes(L: int, nsamples: int, rng_mode: int) -> int:
     out = C.c_size_t(0)
     _check(lib().ising_workspace_bytes(L, nsamples, rng_mode, C.byref(out)), "ising_workspace_bytes")
     return out.value
+
+
+def ising_fnv1a64_scratch_bytes(nbytes: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().ising_fnv1a64_scratch_bytes(nbytes, C.byref(out)), "ising_fnv1a64_scratch_bytes")
+    return out.value
+
+
+def ising_fnv1a64(data, out=None, scratch=None, stream=None):
+    """64-bit FNV-1a of the bytes of a contiguous CUDA tensor, computed on the device (include/ising.h).  Returns a one-element
+    int64 CUDA tensor holding the 64 bits (asynchronous on `stream`); `out` / `scratch` may be passed to avoid allocations."""
+    import torch
+
+    assert data.is_cuda and data.is_contiguous()
+    nbytes = data.numel() * data.element_size()
+    need = ising_fnv1a64_scratch_bytes(nbytes)
+    if scratch is None:
+        scratch = torch.empty(need, dtype=torch.uint8, device=data.device)
+    if out is None:
+        out = torch.empty(1, dtype=torch.int64, device=data.device)
+    with torch.cuda.device(data.device):
+        _check(lib().ising_fnv1a64(data.data_ptr(), nbytes, scratch.data_ptr(), scratch.numel(), out.data_ptr(), _stream_ptr(stream)),
+               "ising_fnv1a64")
+    return out
 
 
 def ising_thresholds(beta: float, rng_mode: int) -> tuple[int, int, int]:

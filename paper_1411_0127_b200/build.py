@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libising_b200.so")
 STAMP = LIB + ".srchash"  # git-ignored with the .so; travels with it to the GPU box
 SOURCES = ["ising_api.cu"]
-HEADERS = ["rng.cuh", "update.cuh", "sweep_kernels.cuh", "batch_kernels.cuh", "cluster_kernels.cuh", "graph_kernels.cuh", "persistent.cuh", "slab_kernels.cuh", "sliced_kernels.cuh", "measure_kernels.cuh", "layout_kernels.cuh", "lane_rng.cuh",
+HEADERS = ["rng.cuh", "update.cuh", "sweep_kernels.cuh", "batch_kernels.cuh", "cluster_kernels.cuh", "fnv_kernels.cuh", "graph_kernels.cuh", "persistent.cuh", "slab_kernels.cuh", "sliced_kernels.cuh", "measure_kernels.cuh", "layout_kernels.cuh", "lane_rng.cuh",
            os.path.join("..", "..", "include", "ising.h")]
 
 

@@ -10,6 +10,7 @@
 #include "../../include/ising.h"
 #include "batch_kernels.cuh"
 #include "cluster_kernels.cuh"
+#include "fnv_kernels.cuh"
 #include "graph_kernels.cuh"
 #include "lane_rng.cuh"
 #include "layout_kernels.cuh"
@@ -1782,6 +1783,41 @@ uint64_t ising_fnv1a64_host(const void *h_data, size_t nbytes)
         hsh *= 0x100000001b3ull;
     }
     return hsh;
+}
+
+int ising_fnv1a64_scratch_bytes(size_t nbytes, size_t *out)
+{
+    if (!out) return ISING_EINVAL;
+    *out = fnv_scratch_bytes(fnv_plan(nbytes));
+    return ISING_OK;
+}
+
+int ising_fnv1a64(const void *d_data, size_t nbytes, void *d_scratch, size_t scratch_bytes, uint64_t *d_out, void *stream)
+{
+    if (!d_out || (nbytes && !d_data) || ((uintptr_t)d_data & 3u)) return ISING_EINVAL;
+    const FnvPlan p = fnv_plan(nbytes);
+    if (nbytes && (!d_scratch || scratch_bytes < fnv_scratch_bytes(p) || ((uintptr_t)d_scratch & 7u))) return ISING_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint8_t *maps = (uint8_t *)d_scratch, *sub_maps = maps + (size_t)p.nchunks * 256, *start = sub_maps + (size_t)p.nchunks * FNV_SUB * 256;
+    unsigned long long *sums = (unsigned long long *)(start + ((size_t)p.nchunks + 7) / 8 * 8);
+    if (p.nchunks) {
+        static std::mutex once;
+        static bool smem_set[64] = {};
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return ISING_ECUDA;
+        {
+            std::lock_guard<std::mutex> lock(once);
+            if (!smem_set[dev]) {   // once per device: the maps of all chunks in the shared memory of one CTA
+                if (cudaFuncSetAttribute(fnv_chunk_starts, cudaFuncAttributeMaxDynamicSharedMemorySize, FNV_MAX_CHUNKS * 256) != cudaSuccess) return ISING_ECUDA;
+                smem_set[dev] = true;
+            }
+        }
+        fnv_low_byte_maps<<<p.nchunks, FNV_SUB * 32, 0, st>>>((const uint8_t *)d_data, p, maps, sub_maps);
+        fnv_chunk_starts<<<1, 256, (size_t)p.nchunks * 256, st>>>(maps, p.nchunks, start);
+        fnv_chunk_sums<<<p.nchunks, FNV_SUB, 0, st>>>((const uint8_t *)d_data, p, start, sub_maps, sums);
+    }
+    fnv_combine<<<1, 1024, 0, st>>>(p, sums, (unsigned long long *)d_out);
+    return cudaGetLastError() == cudaSuccess ? ISING_OK : ISING_ECUDA;
 }
 
 int ising_get_t(const ising_t *h, uint64_t *t)

@@ -217,8 +217,10 @@ def test_config4_L512_philox_fnv_checksums():
     for r in range(nsw // 10):
         o.sweep(cfg["beta"], 10)
         g.ising_sweep(cfg["beta"], 10)
-        got = binding.ising_fnv1a64_host(host_u32(g.ising_get_spins()))
+        d_spins = g.ising_get_spins()
+        got = binding.ising_fnv1a64_host(host_u32(d_spins))
         assert got == ea3d.fnv1a64(o.spins_packed()), f"checksum after {10 * (r + 1)} sweeps"
+        assert int(binding.ising_fnv1a64(d_spins)[0]) & (2**64 - 1) == got, "the checksum computed on the device"
     assert_same_state(o, g, "config 4 final")
     # and the remaining sweeps of the config against the generic kernel (second GPU implementation)
     g2 = Ising(cfg["L"], 1, SEED, cfg["rng_mode"])
@@ -1007,3 +1009,38 @@ def test_handle_belongs_to_the_current_device():
         h.ising_load_state(dev(spins), dev(J))   # tensors of device 0 handed to a handle of device 1
     # the C library itself refuses a launch for a handle of another device than the current one
     assert binding.lib().ising_sweep(h._h, 0.9, 1, None) == binding.EINVAL
+
+
+# ------------------------------------------------------------------------------------------------ FNV-1a on the device
+
+@pytest.mark.parametrize("nbytes", [0, 1, 2, 3, 4, 5, 255, 256, 257, 1000, 4099, 229376, 229380, 1 << 20, (1 << 24) + 4])
+def test_fnv1a64_on_the_device_equals_the_definition(nbytes):
+    """ising_fnv1a64 (parallel: low-byte maps per chunk, composed, then per-chunk sums) against the byte-by-byte definition as the
+    oracle and the host routine compute it: empty input, lengths that are not multiples of 4, one chunk, the chunk boundary, 896
+    chunks, random bytes and the all-0xff / all-zero strings."""
+    rng = np.random.default_rng(nbytes)
+    for kind in ("random", "ff", "zero"):
+        if kind == "random":
+            host = rng.integers(0, 256, nbytes, dtype=np.uint8)
+        else:
+            host = np.full(nbytes, 0xFF if kind == "ff" else 0, dtype=np.uint8)
+        pad = (-nbytes) % 4
+        d = torch.from_numpy(np.concatenate([host, np.zeros(pad, dtype=np.uint8)])).cuda()[:nbytes]
+        got = int(binding.ising_fnv1a64(d)[0]) & (2**64 - 1)
+        assert got == ea3d.fnv1a64(host) == binding.ising_fnv1a64_host(host), (nbytes, kind)
+        if nbytes > 1 << 20 and kind == "random":
+            break
+
+
+def test_fnv1a64_on_the_device_of_the_spins_of_a_run():
+    """The use config 4 makes of it: the checksum of the canonical spins after some sweeps, device routine = host routine."""
+    L = 128
+    g = Ising(L, 1, SEED, PHILOX)
+    g.ising_load_state(dev(synth.make_spins(L, 1, 3)), dev(synth.make_couplings(L, 1, 4)))
+    scratch = torch.empty(binding.ising_fnv1a64_scratch_bytes(L**3 // 8), dtype=torch.uint8, device="cuda")
+    out = torch.empty(1, dtype=torch.int64, device="cuda")
+    for _ in range(3):
+        g.ising_sweep(1 / 1.1, 2)
+        spins = g.ising_get_spins()
+        binding.ising_fnv1a64(spins, out=out, scratch=scratch)
+        assert int(out[0]) & (2**64 - 1) == binding.ising_fnv1a64_host(host_u32(spins))
