@@ -109,3 +109,36 @@ def test_lattices_beyond_L2048(L, rng_mode):
     assert np.array_equal(_bits(out.flatten(), i), _bits(d_spins, i) ^ flips), "blue sites against the oracle's rule"
     assert g.ising_get_t() == 3
     g.ising_destroy()
+
+
+def test_z_slabs_of_the_L4096_lattice():
+    """L = 4096 cut into two z-slabs (the upper one holds the Philox groups beyond 2^32): one sweep with the exchange by copies and
+    one with the exchange fused into the boundary kernels, against the undivided lattice."""
+    from paper_1411_0127_b200 import IsingSlab, binding
+
+    L, G, beta = 4096, 2, 1 / 1.1
+    W = L**3 // 32
+    gen = torch.Generator(device="cuda").manual_seed(99)
+    d_spins = torch.randint(-2**31, 2**31 - 1, (W,), dtype=torch.int32, device="cuda", generator=gen)
+    d_J = torch.randint(-2**31, 2**31 - 1, (3 * W,), dtype=torch.int32, device="cuda", generator=gen)
+    ref = Ising(L, 1, SEED, PHILOX)
+    ref.ising_load_state(d_spins, d_J)
+    ref.ising_sweep(beta, 2)
+    want = ref.ising_get_spins().flatten()
+    Er, Mr = (int(v[0]) for v in ref.ising_energy())
+    ref.ising_destroy()
+    del ref
+    torch.cuda.empty_cache()
+    hs = [IsingSlab(L, G, r, SEED, PHILOX) for r in range(G)]
+    for h in hs:
+        h.ising_load_state(d_spins, d_J)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    binding.ising_slab_sweep_local(hs, beta, 1, sa, sb)
+    binding.ising_slab_sweep_local(hs, beta, 1, sa, sb, push=True)
+    torch.cuda.synchronize()
+    out = torch.zeros(W, dtype=torch.int32, device="cuda")
+    for h in hs:
+        h.ising_get_spins(out)
+    assert torch.equal(out, want)
+    assert sum(int(h.ising_energy()[0][0]) for h in hs) == Er and sum(int(h.ising_energy()[1][0]) for h in hs) == Mr
