@@ -31,6 +31,7 @@ namespace isingk {
 namespace cg = cooperative_groups;
 
 constexpr int CLUSTER_MAX_THREADS = 1024;
+constexpr int CLUSTER_SEED_CACHE_MAX_NW = 512;   // MINSTD: cached seed states need 256 bytes of shared memory per thread
 
 struct ClusterArgs {
     LatticeArrays A;         // the arrays of sample 0
@@ -145,14 +146,42 @@ half_sweeps_cluster(const __grid_constant__ ClusterArgs p)
     uint32_t A = p.A_first, rec = 0;
     PhiloxCommonConst pc;
     PhiloxSampleConst ps;
+    // MINSTD with one word per thread and at most 512 threads: the thread's 2 x 32 seed states s0 (R11: they depend on the site only)
+    // are computed once per launch and kept in shared memory behind the arrays, [colour][bit][thread]; a draw is then one
+    // multiplication mod 2^31 - 1 (R12) instead of a SplitMix64 evaluation and that multiplication.
+    constexpr bool SEED_CACHE = RNG == 1 && NW > 0 && NW <= CLUSTER_SEED_CACHE_MAX_NW;
+    uint32_t *const seeds = sm + 8 * nw;
     // the masks of word `w` for colour c with the constants of the current half-sweep
     auto masks = [&](const WordPlace &w, int c, uint32_t &c4, uint32_t &c8, uint32_t &c12) {
-        if (RNG == 0) cond_masks_site_packed_philox(pc, ps, w.wg, p.T, c4, c8, c12);
-        else cond_masks_site_packed_minstd(seed + (w.site_even + (w.xodd0 ^ (uint32_t)c) + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, 2u * A, p.T, c4, c8, c12);
+        if (RNG == 0) {
+            cond_masks_site_packed_philox(pc, ps, w.wg, p.T, c4, c8, c12);
+        } else if (SEED_CACHE) {
+            c4 = 0; c8 = 0; c12 = 0;
+            const uint32_t *sc = seeds + (uint32_t)c * 32u * (uint32_t)NW + threadIdx.x;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                uint32_t R[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) R[i] = minstd_mulmod2(2u * A, sc[(4 * q + i) * NW]);
+                accumulate_cond<4>(R, 4 * q, p.T, c4, c8, c12);
+            }
+            finish_cond(p.T, c4, c8, c12);
+        } else {
+            cond_masks_site_packed_minstd(seed + (w.site_even + (w.xodd0 ^ (uint32_t)c) + 1) * SPLITMIX_GAMMA, 2 * SPLITMIX_GAMMA, 2u * A, p.T, c4, c8, c12);
+        }
     };
 
     // first word of the thread, half-sweep 0: masks before the barrier that ends the load
     const WordPlace first = place_word<WPR>(threadIdx.x, L, Lz, z0, a_self, a_up, a_dn);
+    if (SEED_CACHE) {
+#pragma unroll 1
+        for (uint32_t c = 0; c < 2; ++c) {
+            const uint64_t weyl0 = seed + (first.site_even + (first.xodd0 ^ c) + 1) * SPLITMIX_GAMMA;
+#pragma unroll 4
+            for (uint32_t b = 0; b < 32; ++b)
+                seeds[(c * 32u + b) * (uint32_t)NW + threadIdx.x] = minstd_seed_state_from_weyl(weyl0 + (uint64_t)b * (2 * SPLITMIX_GAMMA));
+        }
+    }
     uint32_t c4 = 0, c8 = 0, c12 = 0;
     if (RNG == 0) fold_philox_keys(p.seed, sample, &pc, &ps);
     if (p.nhalf) {

@@ -787,6 +787,8 @@ ClusterShape cluster_shape(const ising_t *h, int C)
     s.threads = nw < (size_t)CLUSTER_MAX_THREADS ? (int)nw : CLUSTER_MAX_THREADS;
     s.smem = 8 * nw * sizeof(uint32_t);
     s.nw_fixed = nw <= (size_t)CLUSTER_MAX_THREADS ? (int)nw : 0;
+    // MINSTD, one word per thread, at most 512 threads (and L = 64, where those kernels exist): the cached seed states of the thread
+    if (h->rng_mode == ISING_RNG_MINSTD && g.L == 64 && s.nw_fixed && s.nw_fixed <= CLUSTER_SEED_CACHE_MAX_NW) s.smem += 256 * nw;
     return s;
 }
 
