@@ -809,6 +809,11 @@ int cluster_size_of(ising_t *h)
     }
     int pref = 16;
     while (pref > 1 && (long long)g.nsamples * pref > sms) pref >>= 1;
+    // MINSTD: clusters of 8 CTAs of 512 threads keep the seed states in shared memory; the clusters of many samples then run in waves
+    // MINSTD at L = 64: clusters of at least 8 CTAs (at most 512 threads each) keep the seed states of their words in shared memory,
+    // which is worth more than having all clusters resident at once: the clusters of many samples then run in waves, each through
+    // all half-sweeps of the call (samples are independent)
+    if (h->rng_mode == ISING_RNG_MINSTD && pref < 8 && g.L == 64) pref = 8;
     while (pref <= 16 && cluster_shape(h, pref).smem > (size_t)smem_max) pref <<= 1;
     // the preferred size, then smaller ones (a device that cannot co-schedule 16 CTAs), then larger ones: the first the device accepts
     int order[10], n = 0;
@@ -849,10 +854,11 @@ int cluster_size_of(ising_t *h)
 }
 
 // Which calls run there.  Automatic (kernel choice 0 / 2): where it was measured faster than the launches (profiles/r2n_small.md):
-// L = 64 with Philox up to 128 samples (one sample: 1.2 against 2.2 us per half-sweep; 32 samples: 3.7 against 5.2; 256 samples: the
-// launches fill the GPU as well), with MINSTD one sample only (the batch launches read cached seed states, this kernel recomputes
-// them).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay with the launches (the slab is
-// loaded and stored once per call).
+// L = 64 with Philox up to 128 samples (one sample: 1.15 against 2.2 us per half-sweep; 32 samples: 3.6 against 5.2; from 256 samples
+// on the launches fill the GPU as well), with MINSTD any number of samples (seed states cached in shared memory, clusters of 8 CTAs
+// running in waves: 32 samples 3.8 against 4.0 us, 128 samples 11.3 against 13.7, 512 samples 0.655 against 0.725 ps per flip
+// attempt -- no seed table goes through HBM).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay
+// with the launches (the slab is loaded and stored once per call).
 // `every`: record spacing of the call in half-sweeps (0: no records).  A recording half-sweep runs the measuring copy of the update
 // and costs 0.6 us more than a plain one, so the kernel wins at every spacing (one sample, a record after EVERY half-sweep: 1.75
 // against 2.8 us by graph replays with Philox, 2.5 against 2.8 with MINSTD; 32 samples: 3.7 against 5.3 us by launches).
@@ -862,7 +868,7 @@ bool cluster_available(ising_t *h, uint32_t nhalf, uint32_t every)
     if (h->kernel_choice == 1 || h->kernel_choice == 3 || h->no_cluster || nhalf < 8) return false;
     if (h->kernel_choice != 4) {
         if (h->g.L != 64) return false;
-        if (h->rng_mode == ISING_RNG_PHILOX ? h->g.nsamples > 128 : h->g.nsamples != 1) return false;
+        if (h->rng_mode == ISING_RNG_PHILOX && h->g.nsamples > 128) return false;
     }
     return cluster_size_of(h) > 0;
 }

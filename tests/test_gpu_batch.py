@@ -206,9 +206,8 @@ def test_cluster_resident_kernel_equals_the_oracle(L, ns, rng_mode):
 @pytest.mark.parametrize("L,ns,choice", [(64, 1, 0), (64, 32, 0), (64, 128, 0), (128, 32, 4)])
 def test_cluster_resident_kernel_equals_one_launch_per_half_sweep(L, ns, choice, rng_mode):
     """Longer calls against kernel choice 3 (one launch per half-sweep): 200 sweeps with records every 20 half-sweeps and every 7,
-    calls of different lengths (short ones stay with the launches), another beta, special temperatures."""
-    if rng_mode == MINSTD and ns > 1:
-        choice = 4
+    calls of different lengths (short ones stay with the launches), another beta, special temperatures.  (MINSTD with many samples:
+    clusters of 8 CTAs with the seed states cached in shared memory, more clusters than fit the GPU at once, running in waves.)"""
     spins, J = synth.make_spins(L, ns, 87), synth.make_couplings(L, ns, 88)
     a = Ising(L, ns, SEED, rng_mode)
     a.ising_set_kernel(choice)
