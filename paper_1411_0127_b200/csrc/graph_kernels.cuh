@@ -3,7 +3,8 @@
 //
 // Measured on this part (profiles/r2j_launch_floor.md): a kernel launched into a stream costs at least 2.35 us, with or without
 // programmatic dependent launch, whatever it does -- that is the rate at which the host can submit launches -- while empty kernels
-// replayed from an instantiated graph follow each other every 0.5-0.9 us.  For the one-sample lattices L = 64 and 128, whose
+// replayed from an instantiated graph follow each other every 0.5-0.9 us.  For the one-sample lattices L = 64 and 128 (L = 64 is since served by the cluster-resident kernel of cluster_kernels.cuh, and comes
+// here only under kernel choice 5), whose
 // half-sweep kernel runs for about 2 us, graph replays are 10-25 % faster than launches (2.1-2.3 against 2.6-2.7 us per half-sweep);
 // from L = 192 on the kernels are longer than a launch and the stream launches, which overlap consecutive kernels by programmatic
 // dependent launch, are as fast or faster, and the sample-packed variant lost at every size (its per-sample Philox constants do not

@@ -27,7 +27,7 @@
 //     are pre-set to -3N and -N by init_records and receive 2 x (unsatisfied bonds) and 2 x (up spins) (R16) by one atomic pair
 //     per CTA; nothing waits for a record.
 //   Measured (profiles/r2n_small.md): never the fastest.  The flag latency is paid per tile and is as long as a launch: 2.3-2.6 us
-//   per half-sweep at L = 64 and 128 where graph replays (graph_kernels.cuh, the automatic choice there) take 2.1-2.3, 10.3 against
+//   per half-sweep at L = 64 and 128 where graph replays (graph_kernels.cuh) take 2.1-2.3 and the cluster-resident kernel (cluster_kernels.cuh) 0.9-1.2 at L = 64, 10.3 against
 //   8.1 us at L = 256.  A first version with a grid-wide barrier per half-sweep was slower still, and the sample-packed variant of
 //   the dataflow ran config 2 at 9.1 against 5.8 us per half-sweep and is not in the library.  The kernel is kept, tested, as the
 //   reproducible record of that result.
