@@ -188,8 +188,8 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default: 20; the reference arm, whose step is 3.4 s of CPU work: 3)")
+    ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default: 5; reference arm: 1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=1024)
     ap.add_argument("--sweeps", type=int, default=20)
@@ -222,6 +222,10 @@ def main():
                     help="small lattices: time per half-sweep with the automatic kernels (0), one launch per half-sweep (3) and the "
                          "persistent kernels everywhere (4), without records and with E and M after every half-sweep")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 3 if args.impl == "reference" else 20
+    if args.warmup is None:
+        args.warmup = 1 if args.impl == "reference" else 5
     if args.impl == "reference":
         return run_reference(args)
 
