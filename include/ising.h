@@ -292,7 +292,7 @@ int ising_sliced_end(ising_t *h, void *d_scratch, void *stream);
  * energy, load, get), 2 = the word-parallel kernel without the seed table (MINSTD seeds recomputed per draw), 3 = as 0 but always
  * one launch per colour half-sweep, 4 = as 0 but the persistent kernels wherever they exist, 5 = as 0 without the cluster-resident
  * kernel.  0 runs all half-sweeps of a call in ONE launch where that is faster: one-sample lattices of at most 1024 words per
- * colour (every even L <= 40) on one SM out of shared memory; L = 64 (one sample, or many: up to 128 with Philox, any number with MINSTD) with one
+ * colour (every even L <= 40) on one SM out of shared memory; L = 64 (one sample, or many: up to 256 with Philox, any number with MINSTD) with one
  * thread-block cluster per sample and the lattice in distributed shared memory; and replays CUDA graphs of up to 64 half-sweeps at
  * L = 128, one sample (and at L = 64 under choice 5).  4 extends the cluster-resident kernel to L = 128 and to any number of samples
  * and adds the dataflow kernel of co-resident CTAs for one-sample multiples of 64 below 512.  All give the same bits; the tests use

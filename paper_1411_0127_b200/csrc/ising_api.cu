@@ -814,6 +814,8 @@ int cluster_size_of(ising_t *h)
     // which is worth more than having all clusters resident at once: the clusters of many samples then run in waves, each through
     // all half-sweeps of the call (samples are independent)
     if (h->rng_mode == ISING_RNG_MINSTD && pref < 8 && g.L == 64) pref = 8;
+    // Philox at L = 64: not below 4 CTAs (one word per thread, slab size a compile-time constant); more samples run in waves
+    if (h->rng_mode == ISING_RNG_PHILOX && pref < 4 && g.L == 64) pref = 4;
     while (pref <= 16 && cluster_shape(h, pref).smem > (size_t)smem_max) pref <<= 1;
     // the preferred size, then smaller ones (a device that cannot co-schedule 16 CTAs), then larger ones: the first the device accepts
     int order[10], n = 0;
@@ -854,8 +856,9 @@ int cluster_size_of(ising_t *h)
 }
 
 // Which calls run there.  Automatic (kernel choice 0 / 2): where it was measured faster than the launches (profiles/r2n_small.md):
-// L = 64 with Philox up to 128 samples (one sample: 1.15 against 2.2 us per half-sweep; 32 samples: 3.6 against 5.2; from 256 samples
-// on the launches fill the GPU as well), with MINSTD any number of samples (seed states cached in shared memory, clusters of 8 CTAs
+// L = 64 with Philox up to 256 samples (one sample: 1.15 against 2.2 us per half-sweep; 32 samples: 3.6 against 5.2; 64 / 128 / 256
+// samples in clusters of 4 CTAs running in waves: 7.3 / 14.5 / 28.9 against 8.4 / 15.6 / 29.9; from 512 samples on the launches fill
+// the GPU as well), with MINSTD any number of samples (seed states cached in shared memory, clusters of 8 CTAs
 // running in waves: 32 samples 3.8 against 4.0 us, 128 samples 11.3 against 13.7, 512 samples 0.655 against 0.725 ps per flip
 // attempt -- no seed table goes through HBM).  On request (choice 4): every case it exists for, L = 128 included.  Short calls stay
 // with the launches (the slab is loaded and stored once per call).
@@ -868,7 +871,7 @@ bool cluster_available(ising_t *h, uint32_t nhalf, uint32_t every)
     if (h->kernel_choice == 1 || h->kernel_choice == 3 || h->no_cluster || nhalf < 8) return false;
     if (h->kernel_choice != 4) {
         if (h->g.L != 64) return false;
-        if (h->rng_mode == ISING_RNG_PHILOX && h->g.nsamples > 128) return false;
+        if (h->rng_mode == ISING_RNG_PHILOX && h->g.nsamples > 256) return false;
     }
     return cluster_size_of(h) > 0;
 }
