@@ -8,8 +8,8 @@
 // Hence for a chunk of n bytes  h_end = h_start * P^n + sum_i d_i * P^(n - i),  where the d_i depend on the data and on the low
 // byte at the start of the chunk only.  Three small steps:
 //   1. fnv_low_byte_maps: for every sub-chunk (a chunk = 32 sub-chunks), the map (low byte at its start) -> (low byte at its end),
-//      by running the 8-bit recurrence from all 256 starting values (two integer instructions per value and byte: the high bits of
-//      the register do not matter); the 32 maps of a chunk are composed into the chunk's map;
+//      by running the 8-bit recurrence from all 256 starting values (one integer instruction per value and byte: two values share
+//      a register in 16-bit lanes); the 32 maps of a chunk are composed into the chunk's map;
 //   2. fnv_chunk_starts: one CTA composes the chunk maps in order (they sit in shared memory): the low byte at every chunk's start;
 //   3. fnv_chunk_sums: every sub-chunk runs once more from its actual start (a walk through the chunk's 32 maps) and accumulates
 //      acc <- (acc + d) * P;  the chunk folds its 32 parts, and fnv_combine folds the chunks,  h <- h * P^n_c + acc_c,  as a tree
@@ -23,7 +23,8 @@
 namespace isingk {
 
 constexpr uint64_t FNV_OFFSET = 0xcbf29ce484222325ull, FNV_PRIME = 0x100000001b3ull;
-constexpr int FNV_MAX_CHUNKS = 896;     // 896 x 256 bytes of maps = 224 KiB: the shared memory of one CTA (step 2)
+constexpr int FNV_MAX_CHUNKS = 888;     // 888 x 256 bytes of maps = 222 KiB fit the shared memory of one CTA (step 2); 888 = 3 x 2 x 148:
+                                        // three full waves of step 1 at two CTAs of 1024 threads per SM (896 would leave a fourth wave of 8)
 constexpr int FNV_SUB = 32;             // sub-chunks per chunk: the unit of steps 1 and 3
 constexpr int FNV_STARTS_PER_THREAD = 8;
 
@@ -68,27 +69,33 @@ __global__ void __launch_bounds__(FNV_SUB * 32) fnv_low_byte_maps(const uint8_t 
     const uint32_t c = blockIdx.x, j = threadIdx.x >> 5, g = threadIdx.x & 31u;
     uint64_t begin, n;
     fnv_sub_range(p, c, j, begin, n);
-    uint32_t x[FNV_STARTS_PER_THREAD];
+    // two starting values per register, in 16-bit lanes: a lane holds a byte, byte * 0xb3 < 2^16 stays in its lane, and the mask
+    // that cuts it back to a byte is folded into the XOR of the next step: one LOP3 and one IMAD per byte and TWO values
+    constexpr int NREG = FNV_STARTS_PER_THREAD / 2;
+    uint32_t x[NREG];
 #pragma unroll
-    for (int k = 0; k < FNV_STARTS_PER_THREAD; ++k) x[k] = g * FNV_STARTS_PER_THREAD + k;
+    for (int k = 0; k < NREG; ++k) x[k] = (g * FNV_STARTS_PER_THREAD + 2 * k) | ((g * FNV_STARTS_PER_THREAD + 2 * k + 1) << 16);
     const uint32_t *words = reinterpret_cast<const uint32_t *>(data + begin);   // begin is a multiple of 4, data 4-byte aligned
     const uint32_t nwords = (uint32_t)(n / 4);
     for (uint32_t w = 0; w < nwords; ++w) {
         const uint32_t v = __ldg(words + w);
 #pragma unroll
         for (int b4 = 0; b4 < 4; ++b4) {
-            const uint32_t b = v >> (8 * b4);   // only the low byte of (x ^ b) * 0xb3 matters, so neither b nor x is masked
+            const uint32_t bb = __byte_perm(v, 0u, 0x4040u | (uint32_t)b4 | ((uint32_t)b4 << 8));   // byte b4 of v in both lanes
 #pragma unroll
-            for (int k = 0; k < FNV_STARTS_PER_THREAD; ++k) x[k] = (x[k] ^ b) * 0xb3u;
+            for (int k = 0; k < NREG; ++k) x[k] = ((x[k] & 0x00ff00ffu) ^ bb) * 0xb3u;
         }
     }
     for (uint64_t i = 4ull * nwords; i < n; ++i) {   // the last bytes of data whose length is not a multiple of 4
-        const uint32_t b = data[begin + i];
+        const uint32_t bb = (uint32_t)data[begin + i] * 0x00010001u;
 #pragma unroll
-        for (int k = 0; k < FNV_STARTS_PER_THREAD; ++k) x[k] = (x[k] ^ b) * 0xb3u;
+        for (int k = 0; k < NREG; ++k) x[k] = ((x[k] & 0x00ff00ffu) ^ bb) * 0xb3u;
     }
 #pragma unroll
-    for (int k = 0; k < FNV_STARTS_PER_THREAD; ++k) sm[j][g * FNV_STARTS_PER_THREAD + k] = (uint8_t)x[k];
+    for (int k = 0; k < NREG; ++k) {
+        sm[j][g * FNV_STARTS_PER_THREAD + 2 * k] = (uint8_t)x[k];
+        sm[j][g * FNV_STARTS_PER_THREAD + 2 * k + 1] = (uint8_t)(x[k] >> 16);
+    }
     __syncthreads();
     uint32_t *out = reinterpret_cast<uint32_t *>(sub_maps + (size_t)c * FNV_SUB * 256);
     for (uint32_t i = threadIdx.x; i < FNV_SUB * 64; i += FNV_SUB * 32) out[i] = reinterpret_cast<const uint32_t *>(&sm[0][0])[i];
