@@ -1032,6 +1032,24 @@ def test_fnv1a64_on_the_device_equals_the_definition(nbytes):
             break
 
 
+@pytest.mark.parametrize("nbytes", [1000, 227332, (1 << 22) + 3])
+def test_fnv1a64_scratch_between_guards(nbytes):
+    """Memory safety without a sanitizer: the scratch of ising_fnv1a64 sits between two guard regions, and so does the input."""
+    G = 1 << 20
+    sb = binding.ising_fnv1a64_scratch_bytes(nbytes)
+    buf = torch.full((G + sb + G,), 0xA5, dtype=torch.uint8, device="cuda")
+    host = np.random.default_rng(nbytes).integers(0, 256, nbytes, dtype=np.uint8)
+    data = torch.full((G + nbytes + G,), 0x5A, dtype=torch.uint8, device="cuda")
+    data[G:G + nbytes] = torch.from_numpy(host).cuda()
+    out = torch.full((3,), 0x1234, dtype=torch.int64, device="cuda")
+    binding.ising_fnv1a64(data[G:G + nbytes], out=out[1:2], scratch=buf[G:G + sb])
+    torch.cuda.synchronize()
+    assert int(out[1]) & (2**64 - 1) == ea3d.fnv1a64(host)
+    assert int(out[0]) == 0x1234 and int(out[2]) == 0x1234
+    assert bool((buf[:G] == 0xA5).all()) and bool((buf[G + sb:] == 0xA5).all()), "scratch guard overwritten"
+    assert bool((data[:G] == 0x5A).all()) and bool((data[G + nbytes:] == 0x5A).all()), "input guard overwritten"
+
+
 def test_fnv1a64_on_the_device_of_the_spins_of_a_run():
     """The use config 4 makes of it: the checksum of the canonical spins after some sweeps, device routine = host routine."""
     L = 128
