@@ -378,7 +378,7 @@ int launch_half_sweep(ising_t *h, const Thresholds &T, cudaStream_t st, long lon
     const int nb = g.nbatches == 0 ? g.nlat : g.nbatches;
     for (int b = 0; b < nb; ++b) {
         const LatticeArrays A = h->arrays(b);
-        SweepArgs a;
+        SweepArgs a{};
         a.S_act = A.S[c];
         a.S_oth = A.S[1 - c];
         for (int d = 0; d < 3; ++d) { a.J_act[d] = A.J[d][c]; a.J_oth[d] = A.J[d][1 - c]; }
@@ -551,7 +551,7 @@ int launch_half_sweep_lanes(ising_t *h, const Thresholds &T, cudaStream_t st)
     }
     const int c = (int)(h->t & 1);
     const LatticeArrays A = h->arrays(0);
-    SweepArgs a;
+    SweepArgs a{};
     a.S_act = A.S[c];
     a.S_oth = A.S[1 - c];
     for (int d = 0; d < 3; ++d) { a.J_act[d] = A.J[d][c]; a.J_oth[d] = A.J[d][1 - c]; }
@@ -1330,7 +1330,7 @@ int slab_half_sweep_part(ising_t *h, const Thresholds &T, int part, cudaStream_t
     const int nby = h->Lz / (SWEEP_THREADS / 32);
     const int c = (int)(h->t & 1);
     const LatticeArrays A = h->arrays(0);
-    SweepArgs a;
+    SweepArgs a{};
     a.S_act = A.S[c];
     a.S_oth = A.S[1 - c];
     for (int d = 0; d < 3; ++d) { a.J_act[d] = A.J[d][c]; a.J_oth[d] = A.J[d][1 - c]; }
